@@ -1,0 +1,217 @@
+/*
+ * eagle_verify.h - C ABI of the B200 (sm_100a) FP8 EAGLE tree-verification library.
+ *
+ * The one hot path this library implements (BASELINE.json:north_star): the target model's
+ * forward pass over all nodes of a draft-token tree against a paged bf16 KV cache, with FP8
+ * (E4M3) W8A8 linear layers, followed by greedy acceptance and the KV append:
+ *     verify(tree, cache) -> accepted tokens + bonus token + compacted KV.
+ * Paper passages that define the operations (PAPER.md = the paper text, section / line):
+ *   - PAPER.md:98  (sec. 3.2) FP8 (E4M3) weight-and-activation quantization (W8A8), min-max
+ *     post-training quantization, static scales from calibration data.
+ *   - PAPER.md:361 (App. E)   draft trees "verified in a single forward pass of the target model
+ *     via tree attention"; greedy drafts = a single candidate chain.
+ *   - PAPER.md:92  (sec. 3.1) verification preserves the target model's output (lossless).
+ * Readings of everything the paper leaves open are listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Plain C, no C++/torch types.  Every function returns 0 (EV_OK) or a negative ev_status;
+ *     none throws, aborts or prints.  ev_last_error() gives a thread-local message.
+ *   - "dev_" pointers are CUDA device pointers (e.g. tensor.data_ptr()); "host_" pointers are
+ *     host memory.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - Ownership: the caller owns every buffer it passes and must keep it alive until the stream
+ *     has passed the call.  The library owns handles, quantized weights, the page pool and its
+ *     workspaces; they are released by the matching *_destroy.
+ *   - Asynchrony: calls taking a stream only enqueue work; outputs are valid after the caller
+ *     synchronises that stream.  ev_verify performs no host synchronisation and no allocation.
+ *     Data-dependent failures (bad parent index, token id out of range, sequence over capacity)
+ *     are reported per sequence in ev_verify_out.dev_status, not by return code.
+ *   - Layouts: all matrices row-major.  Weights [out_channels][in_channels] (K contiguous).
+ *     Hidden states / logits [token][channel].  Batched tree arrays [B][T] with T = n_nodes_max.
+ *   - A tree: node 0 is the root = the last emitted token, whose KV is not yet cached
+ *     (DESIGN.md R-root); parents[0] = -1 and 0 <= parents[i] < i.  T <= 64.
+ *     Node i sits at position ctx_len + depth(i) (north_star (3)) and its K/V are written to
+ *     slot ctx_len + i of the sequence during the forward pass.
+ */
+#ifndef EAGLE_VERIFY_H
+#define EAGLE_VERIFY_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EV_MAX_TREE_NODES 64
+
+typedef enum {
+    EV_OK = 0,
+    EV_EINVAL = -1,    /* bad argument (null pointer, shape mismatch, unsupported config) */
+    EV_ENOMEM = -2,    /* device or host allocation failed */
+    EV_ECAPACITY = -3, /* page pool / sequence slots / workspace exhausted */
+    EV_ECUDA = -4,     /* a CUDA runtime or driver call failed; see ev_last_error() */
+    EV_ESTATE = -5     /* call not valid in the handle's current state (e.g. weights missing) */
+} ev_status;
+
+/* per-sequence status bits written to ev_verify_out.dev_status */
+#define EV_SEQ_OK 0
+#define EV_SEQ_BAD_TREE 1     /* parents[] malformed or n_nodes out of range */
+#define EV_SEQ_BAD_TOKEN 2    /* a token id outside [0, vocab) */
+#define EV_SEQ_OVER_CAPACITY 4 /* ctx_len + n_nodes exceeds the sequence's reserved pages */
+
+typedef struct ev_model ev_model;
+typedef struct ev_cache ev_cache;
+
+typedef struct {
+    int n_layers, hidden, n_q_heads, n_kv_heads;
+    int head_dim;         /* 64 or 128 */
+    int ffn, vocab;
+    float rms_eps, rope_theta;
+    int page_size;        /* tokens per KV page; 16 */
+    int act_scale_mode;   /* 0 = dynamic per-token activation scales; 1 = static calibrated */
+    int max_batch;        /* B upper bound per ev_verify call */
+    int max_tree_nodes;   /* T upper bound, <= EV_MAX_TREE_NODES */
+    int max_ctx;          /* upper bound on ctx_len + tree nodes of any sequence (RoPE table) */
+} ev_config;
+
+typedef enum {
+    EV_W_EMBED = 0, /* [vocab][hidden] bf16, kept bf16 */
+    EV_W_Q = 1, EV_W_K = 2, EV_W_V = 3, EV_W_O = 4, EV_W_GATE = 5, EV_W_UP = 6, EV_W_DOWN = 7,
+    EV_W_LM_HEAD = 8,                    /* 1..8: quantized to E4M3 on arrival */
+    EV_W_NORM1 = 9, EV_W_NORM2 = 10, EV_W_NORMF = 11 /* RMSNorm gains [hidden] bf16; default 1.0 */
+} ev_weight_kind;
+
+/* ---- model: quantize / calibrate weights -------------------------------------------------- */
+
+/* Creates an empty model (allocates quantized-weight storage, workspaces sized from max_batch *
+ * max_tree_nodes, the fp64-built RoPE table).  Errors: EV_EINVAL, EV_ENOMEM, EV_ECUDA. */
+int ev_model_create(const ev_config* cfg, ev_model** out);
+
+/* Uploads one weight.  dev_bf16: [rows][cols] bf16 on the device, read during the call's stream
+ * work and not retained.  Matrices EV_W_Q..EV_W_LM_HEAD are quantized per output channel (row):
+ * s_w[n] = max_k|W[n,k]| / 448 (1 for a zero row), code = E4M3_RNE_sat(W[n,k] / s_w[n])
+ * (PAPER.md:98 min-max PTQ; BASELINE.json per-output-channel).  rows/cols must match cfg. */
+int ev_model_set_weight(ev_model*, int kind, int layer, const void* dev_bf16, long rows, long cols,
+                        void* stream);
+
+/* Returns device pointers (owned by the library, valid until destroy) to the E4M3 codes [rows][cols]
+ * and fp32 scales [rows] of a quantized matrix (kinds 1..8).  Q/K/V (and GATE/UP) are views into
+ * fused storage: rows are contiguous per kind. */
+int ev_model_get_quantized(ev_model*, int kind, int layer, const uint8_t** dev_codes,
+                           const float** dev_scales, long* rows, long* cols);
+
+/* Static activation scales (act_scale_mode 1; "Static quantization sets scales offline
+ * from activation statistics collected on calibration data"; DESIGN.md R-static): runs
+ * dev_hidden [n_tok][hidden] fp32 as the layer-0 residual stream of n_tok causal tokens at positions
+ * 0..n_tok-1 with dynamic scales, records per quantization site (4 per layer + LM head input) the
+ * absmax over all tokens and channels, and sets scale = absmax / 448 for every later call.
+ * Any n_tok <= max_ctx (processed in chunks of max_tree_nodes tokens against a temporary cache).
+ * Setup call: synchronises the stream internally.  dev_layer_inputs (optional, may be NULL) receives the residual
+ * stream entering every layer and after the last: [n_layers+1][n_tok][hidden] fp32. */
+int ev_model_calibrate(ev_model*, const float* dev_hidden, int n_tok, float* dev_layer_inputs,
+                       void* stream);
+
+/* Copies the 4*n_layers+1 static scales to host_out in site order
+ * (layer-major: qkv_in, o_in, gateup_in, down_in; then lm_in).  Synchronous. */
+int ev_model_get_static_scales(ev_model*, float* host_out);
+/* Overrides them (same order); used to replay externally calibrated scales. */
+int ev_model_set_static_scales(ev_model*, const float* host_in);
+
+int ev_model_destroy(ev_model*);
+
+/* ---- paged bf16 KV cache ------------------------------------------------------------------- */
+
+/* Pool of n_pages pages; each page holds page_size tokens for all layers.
+ * Device layout: [layer][page][K|V][kv_head][page_size][head_dim] bf16. */
+int ev_cache_create(ev_model*, long n_pages, int max_seqs, ev_cache** out);
+
+/* Reserves ceil(capacity_tokens / page_size) pages for a new sequence (ctx_len = 0) and returns
+ * its slot.  host_pages (optional): explicit physical page ids to use (tests of page-order
+ * invariance); NULL = take from the free list.  EV_ECAPACITY when pages or slots run out. */
+int ev_cache_add_seq(ev_cache*, int capacity_tokens, const int* host_pages, int* seq_slot_out);
+int ev_cache_free_seq(ev_cache*, int seq_slot);
+
+/* Context KV by definition: the K/V the quantized model yields for the token ids under causal
+ * attention, appended after each sequence's current ctx_len.  host_token_ids: the sequences' ids
+ * concatenated (host memory); host_lens[i] ids for sequence host_seq_slots[i].  Runs chain trees of
+ * up to max_tree_nodes tokens per sequence per pass with every node accepted (no LM head).
+ * Setup call: synchronises the stream after every pass. */
+int ev_cache_prefill(ev_model*, ev_cache*, int n_seqs, const int* host_seq_slots,
+                     const int32_t* host_token_ids, const int* host_lens, void* stream);
+
+/* Dense export/import of one sequence's first n_tokens slots for layers [layer_begin, layer_end):
+ * dev_dense: [layer][K|V][kv_head][n_tokens][head_dim] bf16.  import also sets ctx_len = n_tokens
+ * when set_len != 0. */
+int ev_cache_export_seq(ev_cache*, int seq_slot, int layer_begin, int layer_end, int n_tokens,
+                        void* dev_dense, void* stream);
+int ev_cache_import_seq(ev_cache*, int seq_slot, int layer_begin, int layer_end, int n_tokens,
+                        const void* dev_dense, int set_len, void* stream);
+
+/* ctx_len lives on the device (ev_verify with commit advances it without host involvement).
+ * set: enqueued on the stream.  get: synchronises the stream. */
+int ev_cache_set_len(ev_cache*, int seq_slot, int ctx_len, void* stream);
+int ev_cache_get_len(ev_cache*, int seq_slot, int* ctx_len, void* stream);
+int ev_cache_destroy(ev_cache*);
+
+/* ---- verify --------------------------------------------------------------------------------- */
+
+typedef struct {
+    int n_seqs;                 /* B <= max_batch */
+    int n_nodes_max;            /* T <= max_tree_nodes; row stride of the [B][T] arrays */
+    const int32_t* dev_seq_slots; /* [B] cache slots */
+    const int32_t* dev_tokens;  /* [B][T] node tokens; [b][0] = root */
+    const int32_t* dev_parents; /* [B][T] parent indices; [b][0] = -1 */
+    const int32_t* dev_n_nodes; /* [B] nodes in use per sequence, or NULL = all T */
+    int commit;                 /* 1 = compact accepted KV to slots L..L+a and set ctx_len = L+a+1 */
+    int force_accept_all;       /* 1 = (prefill) treat every node as accepted; chain trees only */
+    const float* dev_hidden_override; /* lock-step debug: [n_layers+1][B*T][hidden]; layer l reads
+                                     its input from slice l instead of the previous layer's output
+                                     (slice n_layers feeds the LM head); or NULL */
+    int override_first_only;    /* 1 = only slice 0 (replaces the embedding) is read */
+} ev_verify_in;
+
+typedef struct {
+    int32_t* dev_accept_len;    /* [B] a = accepted draft tokens, 0..depth */
+    int32_t* dev_accept_nodes;  /* [B][T] accepted path incl. root at [0] (a+1 valid) = KV-compaction
+                                   source indices; rest -1 */
+    int32_t* dev_out_tokens;    /* [B][T] accepted tokens then the bonus token (a+1 valid); rest -1 */
+    int32_t* dev_new_ctx_len;   /* [B] L + a + 1 (whether or not commit is set) */
+    int32_t* dev_status;        /* [B] EV_SEQ_* bits */
+    int32_t* dev_argmax;        /* optional [B][T] target argmax per node (lowest id on ties) */
+    float* dev_logits;          /* optional [B*T][vocab] */
+    float* dev_hidden;          /* optional [n_layers+1][B*T][hidden] residual stream taps */
+    /* optional per-kernel taps of one layer (all may be NULL) */
+    int tap_layer;
+    uint8_t* dev_tap_xq;  float* dev_tap_sx;     /* RMSNorm1+quant: [M][hidden] codes, [M] scales */
+    float* dev_tap_qkv;                          /* after RoPE: [M][(Hq+2Hkv)*d] (K,V pre-bf16) */
+    float* dev_tap_attn;                         /* attention output [M][Hq*d] fp32 */
+    uint8_t* dev_tap_aq;  float* dev_tap_sa;     /* its quantization */
+    float* dev_tap_hmid;                         /* residual after O-proj [M][hidden] */
+    float* dev_tap_gu;                           /* gate|up GEMM output [M][2*ffn] */
+    uint8_t* dev_tap_tq;  float* dev_tap_st;     /* SwiGLU + quant: [M][ffn] codes, [M] scales */
+} ev_verify_out;
+
+/* One verify step for B sequences.  M = B*T rows are processed together by
+ * every decoder layer.  Required outputs: accept_len, accept_nodes, out_tokens, new_ctx_len, status.
+ * Errors (host-detectable only): EV_EINVAL, EV_ECAPACITY (B or T over the model's maxima), EV_ESTATE
+ * (weights missing / not calibrated in static mode), EV_ECUDA (launch failure). */
+int ev_verify(ev_model*, ev_cache*, const ev_verify_in*, ev_verify_out*, void* stream);
+
+/* ---- single operators (per-kernel parity tests; same kernels the step uses) ------------------ */
+
+/* y[M][N] = (codes_x . W_kind^T) * s_x[m] * s_w[n] with the product GEMM kernel. */
+int ev_op_linear(ev_model*, int kind, int layer, const uint8_t* dev_codes_x, const float* dev_sx,
+                 int M, float* dev_out, void* stream);
+/* per-token dynamic (or static, scale > 0) E4M3 quantization of fp32 rows */
+int ev_op_quantize_rows(ev_model*, const float* dev_x, int M, int K, float static_scale,
+                        uint8_t* dev_codes, float* dev_sx, void* stream);
+
+/* ---- introspection ---------------------------------------------------------------------------- */
+const char* ev_last_error(void);
+/* kernels launched by the calling thread's library calls since the last reset */
+long ev_launch_count(int reset);
+int ev_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EAGLE_VERIFY_H */

@@ -1,0 +1,329 @@
+"""Thin ctypes binding of include/eagle_verify.h: same names, argument marshalling only.
+
+Every step of the hot path runs inside libeagle_verify.so; torch is used here for device memory
+and streams.  There is no CPU fallback: if the library is missing or a call fails, an exception
+is raised.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libeagle_verify.so")
+
+EV_OK, EV_EINVAL, EV_ENOMEM, EV_ECAPACITY, EV_ECUDA, EV_ESTATE = 0, -1, -2, -3, -4, -5
+EV_W = dict(embed=0, wq=1, wk=2, wv=3, wo=4, wgate=5, wup=6, wdown=7, lm_head=8, norm1=9, norm2=10, normf=11)
+EV_SEQ_BAD_TREE, EV_SEQ_BAD_TOKEN, EV_SEQ_OVER_CAPACITY = 1, 2, 4
+
+
+class EvError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"eagle_verify error {code}: {msg}")
+        self.code = code
+
+
+class ev_config(C.Structure):
+    _fields_ = [("n_layers", C.c_int), ("hidden", C.c_int), ("n_q_heads", C.c_int), ("n_kv_heads", C.c_int),
+                ("head_dim", C.c_int), ("ffn", C.c_int), ("vocab", C.c_int), ("rms_eps", C.c_float),
+                ("rope_theta", C.c_float), ("page_size", C.c_int), ("act_scale_mode", C.c_int),
+                ("max_batch", C.c_int), ("max_tree_nodes", C.c_int), ("max_ctx", C.c_int)]
+
+
+class ev_verify_in(C.Structure):
+    _fields_ = [("n_seqs", C.c_int), ("n_nodes_max", C.c_int), ("dev_seq_slots", C.c_void_p),
+                ("dev_tokens", C.c_void_p), ("dev_parents", C.c_void_p), ("dev_n_nodes", C.c_void_p),
+                ("commit", C.c_int), ("force_accept_all", C.c_int), ("dev_hidden_override", C.c_void_p),
+                ("override_first_only", C.c_int)]
+
+
+class ev_verify_out(C.Structure):
+    _fields_ = [("dev_accept_len", C.c_void_p), ("dev_accept_nodes", C.c_void_p), ("dev_out_tokens", C.c_void_p),
+                ("dev_new_ctx_len", C.c_void_p), ("dev_status", C.c_void_p), ("dev_argmax", C.c_void_p),
+                ("dev_logits", C.c_void_p), ("dev_hidden", C.c_void_p), ("tap_layer", C.c_int),
+                ("dev_tap_xq", C.c_void_p), ("dev_tap_sx", C.c_void_p), ("dev_tap_qkv", C.c_void_p),
+                ("dev_tap_attn", C.c_void_p), ("dev_tap_aq", C.c_void_p), ("dev_tap_sa", C.c_void_p),
+                ("dev_tap_hmid", C.c_void_p), ("dev_tap_gu", C.c_void_p), ("dev_tap_tq", C.c_void_p),
+                ("dev_tap_st", C.c_void_p)]
+
+
+# every symbol include/eagle_verify.h declares: name -> (restype, argtypes)
+_P = C.c_void_p
+SIGNATURES = {
+    "ev_model_create": (C.c_int, [C.POINTER(ev_config), C.POINTER(_P)]),
+    "ev_model_set_weight": (C.c_int, [_P, C.c_int, C.c_int, _P, C.c_long, C.c_long, _P]),
+    "ev_model_get_quantized": (C.c_int, [_P, C.c_int, C.c_int, C.POINTER(_P), C.POINTER(_P), C.POINTER(C.c_long), C.POINTER(C.c_long)]),
+    "ev_model_calibrate": (C.c_int, [_P, _P, C.c_int, _P, _P]),
+    "ev_model_get_static_scales": (C.c_int, [_P, _P]),
+    "ev_model_set_static_scales": (C.c_int, [_P, _P]),
+    "ev_model_destroy": (C.c_int, [_P]),
+    "ev_cache_create": (C.c_int, [_P, C.c_long, C.c_int, C.POINTER(_P)]),
+    "ev_cache_add_seq": (C.c_int, [_P, C.c_int, _P, C.POINTER(C.c_int)]),
+    "ev_cache_free_seq": (C.c_int, [_P, C.c_int]),
+    "ev_cache_prefill": (C.c_int, [_P, _P, C.c_int, _P, _P, _P, _P]),
+    "ev_cache_export_seq": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
+    "ev_cache_import_seq": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, C.c_int, _P, C.c_int, _P]),
+    "ev_cache_set_len": (C.c_int, [_P, C.c_int, C.c_int, _P]),
+    "ev_cache_get_len": (C.c_int, [_P, C.c_int, C.POINTER(C.c_int), _P]),
+    "ev_cache_destroy": (C.c_int, [_P]),
+    "ev_verify": (C.c_int, [_P, _P, C.POINTER(ev_verify_in), C.POINTER(ev_verify_out), _P]),
+    "ev_op_linear": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
+    "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
+    "ev_last_error": (C.c_char_p, []),
+    "ev_launch_count": (C.c_long, [C.c_int]),
+    "ev_version": (C.c_int, []),
+}
+
+_lib = None
+
+
+def load_library():
+    """Loads libeagle_verify.so (built by paper_2606_18502_b200.build).  Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise EvError(EV_ESTATE, f"{LIB_PATH} not built; run `python -m paper_2606_18502_b200.build` "
+                                     "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = lib
+    return _lib
+
+
+def _check(rc):
+    if rc != EV_OK:
+        raise EvError(rc, load_library().ev_last_error().decode())
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def ev_last_error():
+    return load_library().ev_last_error().decode()
+
+
+def ev_launch_count(reset=False):
+    return load_library().ev_launch_count(1 if reset else 0)
+
+
+class _DevView:
+    """Zero-copy view of library-owned device memory (CUDA array interface)."""
+
+    def __init__(self, ptr, shape, typestr):
+        self.__cuda_array_interface__ = dict(shape=tuple(shape), typestr=typestr, data=(int(ptr), False), version=2)
+
+
+class Model:
+    """ev_model handle."""
+
+    def __init__(self, shape, max_batch, max_tree_nodes, max_ctx, page_size=16, act_scale_mode=0):
+        self.lib = load_library()
+        self.cfg = ev_config(shape.n_layers, shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim,
+                             shape.ffn, shape.vocab, shape.rms_eps, shape.rope_theta, page_size, act_scale_mode,
+                             max_batch, max_tree_nodes, max_ctx)
+        self.shape = shape
+        h = C.c_void_p()
+        _check(self.lib.ev_model_create(C.byref(self.cfg), C.byref(h)))
+        self.h = h
+
+    def ev_model_set_weight(self, kind, layer, w_bf16):
+        """w_bf16: torch.bfloat16 CUDA tensor [rows, cols] (gains: [hidden])."""
+        import torch
+        assert w_bf16.is_cuda and w_bf16.dtype == torch.bfloat16 and w_bf16.is_contiguous()
+        rows, cols = (1, w_bf16.shape[0]) if w_bf16.dim() == 1 else w_bf16.shape
+        _check(self.lib.ev_model_set_weight(self.h, EV_W[kind] if isinstance(kind, str) else kind, layer, _ptr(w_bf16),
+                                            rows, cols, _stream()))
+
+    def ev_model_get_quantized(self, kind, layer):
+        """-> (codes uint8 [rows, cols], scales float32 [rows]) as torch CUDA tensors (copies)."""
+        import torch
+        codes, scales, rows, cols = C.c_void_p(), C.c_void_p(), C.c_long(), C.c_long()
+        _check(self.lib.ev_model_get_quantized(self.h, EV_W[kind], layer, C.byref(codes), C.byref(scales),
+                                               C.byref(rows), C.byref(cols)))
+        torch.cuda.current_stream().synchronize()
+        out_c = torch.as_tensor(_DevView(codes.value, (rows.value, cols.value), "|u1"), device="cuda").clone()
+        out_s = torch.as_tensor(_DevView(scales.value, (rows.value,), "<f4"), device="cuda").clone()
+        return out_c, out_s
+
+    def ev_model_calibrate(self, hidden_f32, want_layer_inputs=False):
+        import torch
+        assert hidden_f32.is_cuda and hidden_f32.dtype == torch.float32 and hidden_f32.is_contiguous()
+        n = hidden_f32.shape[0]
+        taps = torch.empty((self.cfg.n_layers + 1, n, self.cfg.hidden), dtype=torch.float32, device="cuda") \
+            if want_layer_inputs else None
+        _check(self.lib.ev_model_calibrate(self.h, _ptr(hidden_f32), n, _ptr(taps), _stream()))
+        return taps
+
+    def ev_model_get_static_scales(self):
+        import numpy as np
+        out = np.empty(4 * self.cfg.n_layers + 1, dtype=np.float32)
+        _check(self.lib.ev_model_get_static_scales(self.h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def ev_model_set_static_scales(self, scales):
+        import numpy as np
+        s = np.ascontiguousarray(scales, dtype=np.float32)
+        assert s.shape == (4 * self.cfg.n_layers + 1,)
+        _check(self.lib.ev_model_set_static_scales(self.h, s.ctypes.data_as(C.c_void_p)))
+
+    def ev_op_linear(self, kind, layer, codes_x, sx):
+        import torch
+        M = codes_x.shape[0]
+        n_out = {"wq": self.shape.q_dim + 2 * self.shape.kv_dim, "wo": self.shape.hidden, "wgate": 2 * self.shape.ffn,
+                 "wdown": self.shape.hidden, "lm_head": self.shape.vocab}[kind]
+        out = torch.empty((M, n_out), dtype=torch.float32, device="cuda")
+        _check(self.lib.ev_op_linear(self.h, EV_W[kind], layer, _ptr(codes_x.contiguous()), _ptr(sx.contiguous()), M,
+                                     _ptr(out), _stream()))
+        return out
+
+    def ev_op_quantize_rows(self, x, static_scale=0.0):
+        import torch
+        M, K = x.shape
+        codes = torch.empty((M, K), dtype=torch.uint8, device="cuda")
+        sx = torch.empty((M,), dtype=torch.float32, device="cuda")
+        _check(self.lib.ev_op_quantize_rows(self.h, _ptr(x.contiguous()), M, K, float(static_scale), _ptr(codes), _ptr(sx),
+                                            _stream()))
+        return codes, sx
+
+    def ev_model_destroy(self):
+        if self.h:
+            self.lib.ev_model_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.ev_model_destroy()
+        except Exception:
+            pass
+
+
+class Cache:
+    """ev_cache handle."""
+
+    def __init__(self, model, n_pages, max_seqs):
+        self.lib, self.model = model.lib, model
+        h = C.c_void_p()
+        _check(self.lib.ev_cache_create(model.h, n_pages, max_seqs, C.byref(h)))
+        self.h = h
+
+    def ev_cache_add_seq(self, capacity_tokens, pages=None):
+        slot = C.c_int(-1)
+        arr = None
+        if pages is not None:
+            arr = (C.c_int * len(pages))(*pages)
+        _check(self.lib.ev_cache_add_seq(self.h, capacity_tokens, arr, C.byref(slot)))
+        return slot.value
+
+    def ev_cache_free_seq(self, slot):
+        _check(self.lib.ev_cache_free_seq(self.h, slot))
+
+    def ev_cache_prefill(self, slots, ids_list):
+        """ids_list: one host int32 array per sequence."""
+        import numpy as np
+        n = len(slots)
+        sl = (C.c_int * n)(*slots)
+        lens = (C.c_int * n)(*[len(x) for x in ids_list])
+        cat = np.ascontiguousarray(np.concatenate([np.asarray(x, dtype=np.int32) for x in ids_list]), dtype=np.int32)
+        _check(self.lib.ev_cache_prefill(self.model.h, self.h, n, sl, cat.ctypes.data_as(C.c_void_p), lens, _stream()))
+
+    def _dense_shape(self, lb, le, n_tokens):
+        c = self.model.cfg
+        return (le - lb, 2, c.n_kv_heads, n_tokens, c.head_dim)
+
+    def ev_cache_export_seq(self, slot, layer_begin, layer_end, n_tokens):
+        import torch
+        out = torch.empty(self._dense_shape(layer_begin, layer_end, n_tokens), dtype=torch.bfloat16, device="cuda")
+        _check(self.lib.ev_cache_export_seq(self.h, slot, layer_begin, layer_end, n_tokens, _ptr(out), _stream()))
+        return out
+
+    def ev_cache_import_seq(self, slot, layer_begin, layer_end, dense_bf16, set_len=True):
+        n_tokens = dense_bf16.shape[3]
+        assert tuple(dense_bf16.shape) == self._dense_shape(layer_begin, layer_end, n_tokens) and dense_bf16.is_contiguous()
+        _check(self.lib.ev_cache_import_seq(self.h, slot, layer_begin, layer_end, n_tokens, _ptr(dense_bf16),
+                                            1 if set_len else 0, _stream()))
+
+    def ev_cache_set_len(self, slot, n):
+        _check(self.lib.ev_cache_set_len(self.h, slot, n, _stream()))
+
+    def ev_cache_get_len(self, slot):
+        v = C.c_int(0)
+        _check(self.lib.ev_cache_get_len(self.h, slot, C.byref(v), _stream()))
+        return v.value
+
+    def ev_cache_destroy(self):
+        if self.h:
+            self.lib.ev_cache_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.ev_cache_destroy()
+        except Exception:
+            pass
+
+
+class VerifyBuffers:
+    """Device buffers of one ev_verify call, allocated once and reused (no allocation per step)."""
+
+    def __init__(self, model, B, T, want_logits=False, want_hidden=False, want_argmax=True, tap_layer=-1):
+        import torch
+        c = model.cfg
+        i32 = dict(dtype=torch.int32, device="cuda")
+        self.B, self.T, self.model = B, T, model
+        self.seq_slots = torch.zeros(B, **i32)
+        self.tokens = torch.zeros((B, T), **i32)
+        self.parents = torch.zeros((B, T), **i32)
+        self.n_nodes = torch.full((B,), T, **i32)
+        self.accept_len = torch.zeros(B, **i32)
+        self.accept_nodes = torch.zeros((B, T), **i32)
+        self.out_tokens = torch.zeros((B, T), **i32)
+        self.new_ctx_len = torch.zeros(B, **i32)
+        self.status = torch.zeros(B, **i32)
+        self.argmax = torch.zeros((B, T), **i32) if want_argmax else None
+        self.logits = torch.empty((B * T, c.vocab), dtype=torch.float32, device="cuda") if want_logits else None
+        self.hidden = torch.empty((c.n_layers + 1, B * T, c.hidden), dtype=torch.float32, device="cuda") if want_hidden else None
+        self.hidden_override = None
+        self.tap_layer = tap_layer
+        self.taps = {}
+        if tap_layer >= 0:
+            M, H, F = B * T, c.hidden, c.ffn
+            qd = c.n_q_heads * c.head_dim
+            qkvd = qd + 2 * c.n_kv_heads * c.head_dim
+            f32 = dict(dtype=torch.float32, device="cuda")
+            u8 = dict(dtype=torch.uint8, device="cuda")
+            self.taps = dict(xq=torch.empty((M, H), **u8), sx=torch.empty(M, **f32), qkv=torch.empty((M, qkvd), **f32),
+                             attn=torch.empty((M, qd), **f32), aq=torch.empty((M, qd), **u8), sa=torch.empty(M, **f32),
+                             hmid=torch.empty((M, H), **f32), gu=torch.empty((M, 2 * F), **f32),
+                             tq=torch.empty((M, F), **u8), st=torch.empty(M, **f32))
+
+    def set_inputs(self, seq_slots, tokens, parents, n_nodes=None):
+        import numpy as np
+        import torch
+        self.seq_slots.copy_(torch.as_tensor(np.asarray(seq_slots, dtype=np.int32)))
+        self.tokens.copy_(torch.as_tensor(np.asarray(tokens, dtype=np.int32).reshape(self.B, self.T)))
+        self.parents.copy_(torch.as_tensor(np.asarray(parents, dtype=np.int32).reshape(self.B, self.T)))
+        if n_nodes is not None:
+            self.n_nodes.copy_(torch.as_tensor(np.asarray(n_nodes, dtype=np.int32)))
+
+
+def ev_verify(model, cache, buf, commit=True, use_n_nodes=True, override_first_only=False):
+    """One verify step on the current torch CUDA stream; asynchronous (outputs valid after a sync)."""
+    vin = ev_verify_in(buf.B, buf.T, buf.seq_slots.data_ptr(), buf.tokens.data_ptr(), buf.parents.data_ptr(),
+                       buf.n_nodes.data_ptr() if use_n_nodes else None, 1 if commit else 0, 0,
+                       buf.hidden_override.data_ptr() if buf.hidden_override is not None else None,
+                       1 if override_first_only else 0)
+    t = buf.taps
+    g = lambda k: t[k].data_ptr() if k in t else None  # noqa: E731
+    vout = ev_verify_out(buf.accept_len.data_ptr(), buf.accept_nodes.data_ptr(), buf.out_tokens.data_ptr(),
+                         buf.new_ctx_len.data_ptr(), buf.status.data_ptr(),
+                         buf.argmax.data_ptr() if buf.argmax is not None else None,
+                         buf.logits.data_ptr() if buf.logits is not None else None,
+                         buf.hidden.data_ptr() if buf.hidden is not None else None, buf.tap_layer,
+                         g("xq"), g("sx"), g("qkv"), g("attn"), g("aq"), g("sa"), g("hmid"), g("gu"), g("tq"), g("st"))
+    _check(model.lib.ev_verify(model.h, cache.h, C.byref(vin), C.byref(vout), _stream()))

@@ -1,0 +1,912 @@
+// C-ABI implementation (include/eagle_verify.h): handles, quantized-weight storage, page pool,
+// and the verify-step schedule.  Every step of the path runs in the kernels of ev_*.cuh; the host
+// code here only validates arguments, owns memory and enqueues launches on the caller's stream.
+#include "../../include/eagle_verify.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ev_attention.cuh"
+#include "ev_common.cuh"
+#include "ev_elementwise.cuh"
+#include "ev_gemm.cuh"
+
+using namespace ev;
+
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+thread_local std::string g_err;
+thread_local long g_launches = 0;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+#define CUDA_TRY(expr)                                                                                    \
+    do {                                                                                                  \
+        cudaError_t _e = (expr);                                                                          \
+        if (_e != cudaSuccess)                                                                            \
+            return fail(EV_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(_e) + " @" + std::to_string(__LINE__)); \
+    } while (0)
+#define LAUNCH_CHECK()                                                                                    \
+    do {                                                                                                  \
+        ++g_launches;                                                                                     \
+        cudaError_t _e = cudaGetLastError();                                                              \
+        if (_e != cudaSuccess)                                                                            \
+            return fail(EV_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(_e) + " @" + std::to_string(__LINE__)); \
+    } while (0)
+#define EV_TRY(expr)                \
+    do {                            \
+        int _r = (expr);            \
+        if (_r != EV_OK) return _r; \
+    } while (0)
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+PFN_encodeTiled g_encode = nullptr;
+
+int get_encode() {
+    if (g_encode) return EV_OK;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !fn)
+        return fail(EV_ECUDA, "cuTensorMapEncodeTiled entry point not available (no CUDA driver?)");
+    g_encode = (PFN_encodeTiled)fn;
+    return EV_OK;
+}
+
+// 2-D uint8 tensor [rows][cols] (cols contiguous), box = [box_rows][128 bytes], 128-byte swizzle
+int make_tmap(CUtensorMap* tm, const void* base, long rows, long cols, int box_rows) {
+    EV_TRY(get_encode());
+    cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)cols};
+    cuuint32_t box[2] = {128u, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1u, 1u};
+    CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(EV_ECUDA, "cuTensorMapEncodeTiled failed, code " + std::to_string((int)r));
+    return EV_OK;
+}
+
+constexpr int N_TOK_VARIANTS = 5;
+const int kTokVariants[N_TOK_VARIANTS] = {16, 32, 64, 128, 256};
+
+struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, with one TMA map per token-tile size
+    uint8_t* codes = nullptr;
+    float* scale = nullptr;
+    long K = 0;
+    CUtensorMap tm[N_TOK_VARIANTS];
+};
+
+struct QMat {  // a quantized weight matrix [N][K]
+    uint8_t* codes = nullptr;
+    float* scale = nullptr;
+    long N = 0, K = 0;
+    CUtensorMap tm;
+};
+
+struct LayerW {
+    QMat qkv, o, gu, down;
+    __nv_bfloat16* g1 = nullptr;
+    __nv_bfloat16* g2 = nullptr;
+    unsigned have = 0;  // bit per ev_weight_kind
+};
+
+long round_up(long x, long m) { return (x + m - 1) / m * m; }
+
+}  // namespace
+
+struct ev_model {
+    ev_config cfg;
+    int M_cap = 0, M_pad = 0, qkv_dim = 0, q_dim = 0, kv_dim = 0, max_pos = 0;
+    std::vector<LayerW> layers;
+    QMat lm;
+    __nv_bfloat16* embed = nullptr;
+    __nv_bfloat16* gf = nullptr;
+    bool have_embed = false, have_lm = false;
+    float2* rope_cs = nullptr;
+    // workspaces
+    float* h = nullptr;
+    ActBuf xq, aq, tq;
+    float* qkv = nullptr;
+    float* attn = nullptr;
+    float* gu = nullptr;
+    float* o_part = nullptr;
+    float* ml_part = nullptr;
+    long split_rows_budget = 0;
+    float* splitk_partial = nullptr;
+    long splitk_floats = 0;
+    // tree state
+    int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
+    unsigned long long *anc = nullptr, *argmax_keys = nullptr;
+    // static activation scales
+    int n_sites = 0;
+    float* static_scales = nullptr;  // device [n_sites]
+    float* site_amax = nullptr;      // device [n_sites]
+    bool calibrated = false, recording = false;
+    int num_sms = 148;
+    bool use_splitk = false, naive_gemm = false;
+    std::vector<void*> allocs;
+};
+
+struct ev_cache {
+    ev_model* model = nullptr;
+    long n_pages = 0;
+    int max_seqs = 0, max_pages = 0;
+    long layer_stride = 0;  // elements
+    __nv_bfloat16* pool = nullptr;
+    int32_t* page_table = nullptr;  // device [max_seqs][max_pages]
+    int32_t* ctx_len = nullptr;     // device [max_seqs]
+    int32_t* capacity = nullptr;    // device [max_seqs]
+    std::vector<int> free_pages;
+    std::vector<std::vector<int>> seq_pages;
+    std::vector<char> seq_used;
+    std::vector<int> len_bound;  // host-side upper bound of each sequence's ctx_len (sizes the key-split grid)
+    // prefill staging
+    int32_t *pf_tokens = nullptr, *pf_parents = nullptr, *pf_nn = nullptr, *pf_slots = nullptr;
+    int32_t *pf_out = nullptr;
+};
+
+namespace {
+
+template <class T>
+int dev_alloc(ev_model* m, T** p, size_t count) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, count * sizeof(T) > 0 ? count * sizeof(T) : 16);
+    if (e != cudaSuccess) return fail(EV_ENOMEM, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    if (m) m->allocs.push_back(q);
+    *p = (T*)q;
+    return EV_OK;
+}
+
+int alloc_actbuf(ev_model* m, ActBuf* b, long K) {
+    b->K = K;
+    EV_TRY(dev_alloc(m, &b->codes, (size_t)m->M_pad * K));
+    EV_TRY(dev_alloc(m, &b->scale, (size_t)m->M_pad));
+    cudaMemset(b->codes, 0, (size_t)m->M_pad * K);
+    for (int i = 0; i < N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&b->tm[i], b->codes, m->M_pad, K, kTokVariants[i]));
+    return EV_OK;
+}
+
+int alloc_qmat(ev_model* m, QMat* q, long N, long K) {
+    q->N = N;
+    q->K = K;
+    EV_TRY(dev_alloc(m, &q->codes, (size_t)N * K));
+    EV_TRY(dev_alloc(m, &q->scale, (size_t)N));
+    EV_TRY(make_tmap(&q->tm, q->codes, N, K, GEMM_WROWS));
+    return EV_OK;
+}
+
+template <int TOK, int EPI>
+int launch_gemm_inst(cudaStream_t st, const CUtensorMap& tmW, const CUtensorMap& tmX, const GemmArgs& a, int splits) {
+    using S = GemmSmem<TOK>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<TOK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL));
+        attr_set = true;
+    }
+    dim3 grid((a.N + GEMM_WROWS - 1) / GEMM_WROWS, (a.M + TOK - 1) / TOK, splits);
+    gemm_e4m3_kernel<TOK, EPI><<<grid, GEMM_THREADS, S::TOTAL, st>>>(tmW, tmX, a);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+
+template <int EPI>
+int launch_gemm_epi(cudaStream_t st, const CUtensorMap& tmW, const ActBuf& x, const GemmArgs& a, int splits) {
+    int v = N_TOK_VARIANTS - 1;
+    for (int i = 0; i < N_TOK_VARIANTS; ++i)
+        if (a.M <= kTokVariants[i]) { v = i; break; }
+    switch (v) {
+        case 0: return launch_gemm_inst<16, EPI>(st, tmW, x.tm[0], a, splits);
+        case 1: return launch_gemm_inst<32, EPI>(st, tmW, x.tm[1], a, splits);
+        case 2: return launch_gemm_inst<64, EPI>(st, tmW, x.tm[2], a, splits);
+        case 3: return launch_gemm_inst<128, EPI>(st, tmW, x.tm[3], a, splits);
+        default: return launch_gemm_inst<256, EPI>(st, tmW, x.tm[4], a, splits);
+    }
+}
+
+// y = x . W^T with scales; epi: EPI_STORE / EPI_RESID (in place on out) / EPI_ARGMAX
+int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, float* out, int ldo,
+               unsigned long long* keys) {
+    GemmArgs a;
+    a.M = M; a.N = (int)w.N; a.K = (int)w.K;
+    a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
+    a.partial = nullptr; a.argmax_keys = keys;
+    const int total_kb = (int)((w.K + GEMM_BK - 1) / GEMM_BK);
+    a.kb_per_split = total_kb;
+    if (m->naive_gemm && epi != EPI_ARGMAX) {
+        dim3 grid((a.N + 127) / 128, M);
+        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, a.N, a.K, a.sx, a.sw, out, ldo, epi == EPI_RESID);
+        LAUNCH_CHECK();
+        return EV_OK;
+    }
+    int splits = 1;
+    const int tiles = (a.N + GEMM_WROWS - 1) / GEMM_WROWS;
+    if (m->use_splitk && epi != EPI_ARGMAX && M <= 256 && tiles * 2 <= m->num_sms && total_kb >= 8) {
+        splits = std::min(std::min(m->num_sms / tiles, total_kb / 4), 8);
+        a.kb_per_split = (total_kb + splits - 1) / splits;
+        splits = (total_kb + a.kb_per_split - 1) / a.kb_per_split;
+        if ((long)splits * M * a.N > m->splitk_floats) splits = 1, a.kb_per_split = total_kb;
+    }
+    if (splits > 1) {
+        a.partial = m->splitk_partial;
+        EV_TRY(launch_gemm_epi<EPI_PARTIAL>(st, w.tm, x, a, splits));
+        const long total = (long)M * a.N;
+        const int blocks = (int)std::min<long>((total + 255) / 256, 148 * 8);
+        splitk_finish_kernel<<<blocks, 256, 0, st>>>(m->splitk_partial, splits, M, a.N, a.sx, a.sw, out, ldo, epi == EPI_RESID);
+        LAUNCH_CHECK();
+        return EV_OK;
+    }
+    switch (epi) {
+        case EPI_STORE: return launch_gemm_epi<EPI_STORE>(st, w.tm, x, a, 1);
+        case EPI_RESID: return launch_gemm_epi<EPI_RESID>(st, w.tm, x, a, 1);
+        case EPI_ARGMAX: return launch_gemm_epi<EPI_ARGMAX>(st, w.tm, x, a, 1);
+    }
+    return fail(EV_EINVAL, "bad epilogue");
+}
+
+QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
+    QuantOut q;
+    q.codes = b.codes;
+    q.sx = b.scale;
+    q.static_scale = (m->cfg.act_scale_mode == 1 && !m->recording) ? m->static_scales + site : nullptr;
+    q.site_amax = m->recording ? m->site_amax + site : nullptr;
+    return q;
+}
+
+int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
+    CUDA_TRY(cudaMemcpyAsync(dst, src, (size_t)n * sizeof(float), cudaMemcpyDeviceToDevice, st));
+    return EV_OK;
+}
+
+template <int D>
+int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
+    constexpr int smem = 2 * 2 * ATT_CH * D * 2;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(tree_attn_partial_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        attr_set = true;
+    }
+    tree_attn_partial_kernel<D><<<grid, ATT_THREADS, smem, st>>>(a);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+
+// the verify-step schedule; max_keys_hint: upper bound of ctx_len + T over the
+// batch known to the host (sizes the key-split grid; the kernels read the true lengths on the device)
+int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* out, cudaStream_t st, bool need_lm) {
+    const ev_config& cfg = m->cfg;
+    const int B = in->n_seqs, T = in->n_nodes_max, M = B * T;
+    const int H = cfg.hidden, D = cfg.head_dim, F = cfg.ffn;
+
+    TreePrepArgs tp;
+    tp.B = B; tp.T = T; tp.vocab = cfg.vocab; tp.page_size = cfg.page_size;
+    tp.seq_slots = in->dev_seq_slots; tp.tokens = in->dev_tokens; tp.parents = in->dev_parents; tp.n_nodes = in->dev_n_nodes;
+    tp.ctx_len = c->ctx_len; tp.capacity = c->capacity; tp.max_seqs = c->max_seqs; tp.max_pos = m->max_pos;
+    tp.Lsnap = m->Lsnap; tp.nn_eff = m->nn_eff; tp.status = out->dev_status; tp.depth = m->depth; tp.pos = m->pos;
+    tp.anc = m->anc; tp.argmax_keys = m->argmax_keys;
+    tree_prep_kernel<<<(B + 63) / 64, 64, 0, st>>>(tp);
+    LAUNCH_CHECK();
+
+    const float* ovr = in->dev_hidden_override;
+    if (ovr) {
+        EV_TRY(copy_f32(st, ovr, m->h, (long)M * H));
+    } else {
+        embed_gather_kernel<<<M, EW_THREADS, 0, st>>>(in->dev_tokens, cfg.vocab, m->embed, H, m->h);
+        LAUNCH_CHECK();
+    }
+    if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden, (long)M * H));
+
+    // key-split plan for attention: enough CTAs for ~2 waves, bounded by the partial-output workspace
+    const int R = T * (cfg.n_q_heads / cfg.n_kv_heads);
+    const int row_groups = (R + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
+    int max_keys = 0;
+    for (int i = 0; i < c->max_seqs; ++i)
+        if (c->seq_used[i]) max_keys = std::max(max_keys, c->len_bound[i]);
+    max_keys = std::min(max_keys + T, cfg.max_ctx);
+    if (in->commit)
+        for (int i = 0; i < c->max_seqs; ++i)
+            if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * cfg.page_size);
+    int n_splits;
+    {
+        const long base = (long)B * cfg.n_kv_heads * row_groups;
+        long want = (2L * m->num_sms + base - 1) / base;
+        const long chunks = (max_keys + ATT_CH - 1) / ATT_CH;
+        want = std::max(1L, std::min(want, chunks));
+        want = std::min(want, std::max(1L, m->split_rows_budget / M));
+        n_splits = (int)want;
+    }
+    int split_len = (int)round_up((max_keys + n_splits - 1) / n_splits, ATT_CH);
+    n_splits = (max_keys + split_len - 1) / split_len;
+
+    for (int l = 0; l < cfg.n_layers; ++l) {
+        LayerW& w = m->layers[l];
+        const bool tap = (out->tap_layer == l);
+        if (ovr && !in->override_first_only && l > 0) EV_TRY(copy_f32(st, ovr + (size_t)l * M * H, m->h, (long)M * H));
+        // --- attention block ---
+        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
+        LAUNCH_CHECK();
+        if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
+        if (tap && out->dev_tap_sx) EV_TRY(copy_f32(st, m->xq.scale, out->dev_tap_sx, M));
+        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_STORE, m->qkv, m->qkv_dim, nullptr));
+        RopeArgs ra;
+        ra.qkv = m->qkv; ra.ld = m->qkv_dim; ra.Hq = cfg.n_q_heads; ra.Hkv = cfg.n_kv_heads; ra.D = D; ra.T = T;
+        ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
+        ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
+        ra.pool = c->pool + (size_t)l * c->layer_stride;
+        rope_kvwrite_kernel<<<M, EW_THREADS, 0, st>>>(ra);
+        LAUNCH_CHECK();
+        if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
+        AttnArgs aa;
+        aa.q = m->qkv; aa.q_ld = m->qkv_dim; aa.T = T; aa.G = cfg.n_q_heads / cfg.n_kv_heads; aa.Hq = cfg.n_q_heads;
+        aa.Hkv = cfg.n_kv_heads; aa.pool = ra.pool; aa.page_table = c->page_table; aa.max_pages = c->max_pages;
+        aa.page_size = cfg.page_size; aa.seq_slots = in->dev_seq_slots; aa.Lsnap = m->Lsnap; aa.nn_eff = m->nn_eff;
+        aa.anc = m->anc; aa.split_len = split_len; aa.n_splits = n_splits; aa.scale = 1.0f / sqrtf((float)D);
+        aa.o_part = m->o_part; aa.ml_part = m->ml_part;
+        dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
+        if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
+        MergeArgs ma;
+        ma.T = T; ma.Hq = cfg.n_q_heads; ma.D = D; ma.n_splits = n_splits; ma.split_len = split_len;
+        ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part; ma.attn = m->attn;
+        ma.q = quant_out(m, m->aq, 4 * l + 1);
+        attn_merge_quant_kernel<<<M, EW_THREADS, 0, st>>>(ma);
+        LAUNCH_CHECK();
+        if (tap && out->dev_tap_attn) EV_TRY(copy_f32(st, m->attn, out->dev_tap_attn, (long)M * m->q_dim));
+        if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
+        if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
+        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RESID, m->h, H, nullptr));
+        if (tap && out->dev_tap_hmid) EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H));
+        // --- MLP block ---
+        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
+        LAUNCH_CHECK();
+        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_STORE, m->gu, 2 * F, nullptr));
+        if (tap && out->dev_tap_gu) EV_TRY(copy_f32(st, m->gu, out->dev_tap_gu, (long)M * 2 * F));
+        swiglu_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->gu, F, quant_out(m, m->tq, 4 * l + 3));
+        LAUNCH_CHECK();
+        if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
+        if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
+        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RESID, m->h, H, nullptr));
+        if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H));
+    }
+    if (need_lm) {
+        if (ovr && !in->override_first_only) EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H));
+        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers));
+        LAUNCH_CHECK();
+        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, out->dev_logits, cfg.vocab, m->argmax_keys));
+    }
+    AcceptArgs ac;
+    ac.B = B; ac.T = T; ac.commit = in->commit; ac.force_all = in->force_accept_all;
+    ac.tokens = in->dev_tokens; ac.parents = in->dev_parents; ac.nn_eff = m->nn_eff; ac.status = out->dev_status;
+    ac.Lsnap = m->Lsnap; ac.seq_slots = in->dev_seq_slots; ac.argmax_keys = m->argmax_keys; ac.argmax_out = out->dev_argmax;
+    ac.accept_len = out->dev_accept_len; ac.accept_nodes = out->dev_accept_nodes; ac.out_tokens = out->dev_out_tokens;
+    ac.new_ctx_len = out->dev_new_ctx_len; ac.ctx_len = c->ctx_len;
+    accept_walk_kernel<<<(B + 63) / 64, 64, 0, st>>>(ac);
+    LAUNCH_CHECK();
+    if (in->commit && !in->force_accept_all) {
+        CompactArgs ca;
+        ca.T = T; ca.Hkv = cfg.n_kv_heads; ca.D = D; ca.page_size = cfg.page_size; ca.max_pages = c->max_pages;
+        ca.layer_stride = c->layer_stride; ca.pool = c->pool; ca.page_table = c->page_table; ca.seq_slots = in->dev_seq_slots;
+        ca.Lsnap = m->Lsnap; ca.accept_len = out->dev_accept_len; ca.accept_nodes = out->dev_accept_nodes;
+        kv_compact_kernel<<<dim3(B, cfg.n_layers), EW_THREADS, 0, st>>>(ca);
+        LAUNCH_CHECK();
+    }
+    return EV_OK;
+}
+
+int check_ready(ev_model* m, bool need_lm) {
+    if (!m->have_embed) return fail(EV_ESTATE, "embedding not set");
+    const unsigned need = (1u << EV_W_Q) | (1u << EV_W_K) | (1u << EV_W_V) | (1u << EV_W_O) | (1u << EV_W_GATE) |
+                          (1u << EV_W_UP) | (1u << EV_W_DOWN);
+    for (size_t l = 0; l < m->layers.size(); ++l)
+        if ((m->layers[l].have & need) != need) return fail(EV_ESTATE, "layer " + std::to_string(l) + ": weights missing");
+    if (need_lm && !m->have_lm) return fail(EV_ESTATE, "lm_head not set");
+    if (m->cfg.act_scale_mode == 1 && !m->calibrated && !m->recording)
+        return fail(EV_ESTATE, "static activation scales: model not calibrated");
+    return EV_OK;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+const char* ev_last_error(void) { return g_err.c_str(); }
+long ev_launch_count(int reset) {
+    long v = g_launches;
+    if (reset) g_launches = 0;
+    return v;
+}
+int ev_version(void) { return 1; }
+
+int ev_model_create(const ev_config* cfg, ev_model** out) {
+    if (!cfg || !out) return fail(EV_EINVAL, "null argument");
+    *out = nullptr;
+    if (cfg->n_layers < 1 || cfg->hidden < 16 || cfg->n_q_heads < 1 || cfg->n_kv_heads < 1 || cfg->ffn < 16 || cfg->vocab < 1)
+        return fail(EV_EINVAL, "bad model dimensions");
+    if (cfg->head_dim != 64 && cfg->head_dim != 128) return fail(EV_EINVAL, "head_dim must be 64 or 128");
+    if (cfg->n_q_heads % cfg->n_kv_heads) return fail(EV_EINVAL, "n_q_heads must be a multiple of n_kv_heads");
+    if (cfg->hidden % 16 || cfg->ffn % 16) return fail(EV_EINVAL, "hidden and ffn must be multiples of 16 (TMA row pitch)");
+    if (cfg->page_size < 1 || cfg->page_size > 256) return fail(EV_EINVAL, "page_size out of range");
+    if (cfg->max_tree_nodes < 1 || cfg->max_tree_nodes > EV_MAX_TREE_NODES) return fail(EV_EINVAL, "max_tree_nodes must be 1..64");
+    if (cfg->max_batch < 1 || cfg->max_ctx < 1) return fail(EV_EINVAL, "max_batch / max_ctx must be positive");
+    if (cfg->act_scale_mode != 0 && cfg->act_scale_mode != 1) return fail(EV_EINVAL, "act_scale_mode must be 0 or 1");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(EV_ECUDA, "no CUDA device");
+    ev_model* m = new ev_model();
+    m->cfg = *cfg;
+    m->M_cap = cfg->max_batch * cfg->max_tree_nodes;
+    m->M_pad = (int)round_up(m->M_cap, 256);
+    m->q_dim = cfg->n_q_heads * cfg->head_dim;
+    m->kv_dim = cfg->n_kv_heads * cfg->head_dim;
+    m->qkv_dim = m->q_dim + 2 * m->kv_dim;
+    m->max_pos = cfg->max_ctx;
+    m->n_sites = 4 * cfg->n_layers + 1;
+    m->layers.resize(cfg->n_layers);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    m->use_splitk = getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) != 0;
+    m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
+    const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
+    int rc = EV_OK;
+    auto A = [&](int r) { if (rc == EV_OK) rc = r; };
+    for (auto& L : m->layers) {
+        A(alloc_qmat(m, &L.qkv, m->qkv_dim, H));
+        A(alloc_qmat(m, &L.o, H, m->q_dim));
+        A(alloc_qmat(m, &L.gu, 2 * F, H));
+        A(alloc_qmat(m, &L.down, H, F));
+    }
+    A(alloc_qmat(m, &m->lm, V, H));
+    A(dev_alloc(m, &m->embed, (size_t)V * H));
+    A(dev_alloc(m, &m->h, (size_t)m->M_pad * H));
+    A(alloc_actbuf(m, &m->xq, H));
+    A(alloc_actbuf(m, &m->aq, m->q_dim));
+    A(alloc_actbuf(m, &m->tq, F));
+    A(dev_alloc(m, &m->qkv, (size_t)m->M_pad * m->qkv_dim));
+    A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
+    A(dev_alloc(m, &m->gu, (size_t)m->M_pad * 2 * F));
+    m->split_rows_budget = std::max<long>(2L * m->M_cap, 4096);
+    A(dev_alloc(m, &m->o_part, (size_t)m->split_rows_budget * m->q_dim));
+    A(dev_alloc(m, &m->ml_part, (size_t)m->split_rows_budget * cfg->n_q_heads * 2));
+    m->splitk_floats = 8L * std::min(m->M_cap, 256) * std::max<long>(m->qkv_dim, H);
+    A(dev_alloc(m, &m->splitk_partial, (size_t)m->splitk_floats));
+    A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
+    A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
+    A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->pos, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->anc, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->argmax_keys, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->static_scales, (size_t)m->n_sites));
+    A(dev_alloc(m, &m->site_amax, (size_t)m->n_sites));
+    A(dev_alloc(m, &m->rope_cs, (size_t)m->max_pos * (cfg->head_dim / 2)));
+    if (rc == EV_OK) {
+        // RoPE table: angle = p * theta^(-2j/d) in fp64, cos/sin rounded to fp32 (DESIGN.md R-rope)
+        const int D2 = cfg->head_dim / 2;
+        std::vector<float2> tab((size_t)m->max_pos * D2);
+        std::vector<double> inv(D2);
+        for (int j = 0; j < D2; ++j) inv[j] = std::pow((double)cfg->rope_theta, -(2.0 * j) / (double)cfg->head_dim);
+        for (long p = 0; p < m->max_pos; ++p)
+            for (int j = 0; j < D2; ++j) {
+                const double ang = (double)p * inv[j];
+                tab[(size_t)p * D2 + j] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+            }
+        if (cudaMemcpy(m->rope_cs, tab.data(), tab.size() * sizeof(float2), cudaMemcpyHostToDevice) != cudaSuccess)
+            rc = fail(EV_ECUDA, "rope table upload failed");
+    }
+    if (rc != EV_OK) {
+        std::string keep = g_err;
+        ev_model_destroy(m);
+        g_err = keep;
+        return rc;
+    }
+    *out = m;
+    return EV_OK;
+}
+
+int ev_model_destroy(ev_model* m) {
+    if (!m) return EV_OK;
+    cudaDeviceSynchronize();
+    for (void* p : m->allocs) cudaFree(p);
+    delete m;
+    return EV_OK;
+}
+
+int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, long rows, long cols, void* stream) {
+    if (!m || !dev_bf16) return fail(EV_EINVAL, "null argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const ev_config& c = m->cfg;
+    const long H = c.hidden, F = c.ffn, V = c.vocab;
+    const bool per_layer = (kind >= EV_W_Q && kind <= EV_W_DOWN) || kind == EV_W_NORM1 || kind == EV_W_NORM2;
+    if (per_layer && (layer < 0 || layer >= c.n_layers)) return fail(EV_EINVAL, "layer out of range");
+    auto shape_is = [&](long r, long k) { return rows == r && cols == k; };
+    auto bad_shape = [&]() { return fail(EV_EINVAL, "weight shape does not match the model config"); };
+    auto quant = [&](QMat& q, long row_off) -> int {
+        quantize_weight_rows_kernel<<<(unsigned)rows, EW_THREADS, 0, st>>>((const __nv_bfloat16*)dev_bf16, cols,
+                                                                          q.codes + row_off * q.K, q.scale + row_off);
+        LAUNCH_CHECK();
+        return EV_OK;
+    };
+    switch (kind) {
+        case EV_W_EMBED:
+            if (!shape_is(V, H)) return bad_shape();
+            CUDA_TRY(cudaMemcpyAsync(m->embed, dev_bf16, (size_t)V * H * 2, cudaMemcpyDeviceToDevice, st));
+            m->have_embed = true;
+            return EV_OK;
+        case EV_W_Q: if (!shape_is(m->q_dim, H)) return bad_shape(); EV_TRY(quant(m->layers[layer].qkv, 0)); break;
+        case EV_W_K: if (!shape_is(m->kv_dim, H)) return bad_shape(); EV_TRY(quant(m->layers[layer].qkv, m->q_dim)); break;
+        case EV_W_V: if (!shape_is(m->kv_dim, H)) return bad_shape(); EV_TRY(quant(m->layers[layer].qkv, m->q_dim + m->kv_dim)); break;
+        case EV_W_O: if (!shape_is(H, m->q_dim)) return bad_shape(); EV_TRY(quant(m->layers[layer].o, 0)); break;
+        case EV_W_GATE: if (!shape_is(F, H)) return bad_shape(); EV_TRY(quant(m->layers[layer].gu, 0)); break;
+        case EV_W_UP: if (!shape_is(F, H)) return bad_shape(); EV_TRY(quant(m->layers[layer].gu, F)); break;
+        case EV_W_DOWN: if (!shape_is(H, F)) return bad_shape(); EV_TRY(quant(m->layers[layer].down, 0)); break;
+        case EV_W_LM_HEAD:
+            if (!shape_is(V, H)) return bad_shape();
+            EV_TRY(quant(m->lm, 0));
+            m->have_lm = true;
+            return EV_OK;
+        case EV_W_NORM1: case EV_W_NORM2: case EV_W_NORMF: {
+            if (!(shape_is(1, H) || shape_is(H, 1))) return bad_shape();
+            __nv_bfloat16** dst = kind == EV_W_NORM1 ? &m->layers[layer].g1 : kind == EV_W_NORM2 ? &m->layers[layer].g2 : &m->gf;
+            if (!*dst) EV_TRY(dev_alloc(m, dst, (size_t)H));
+            CUDA_TRY(cudaMemcpyAsync(*dst, dev_bf16, (size_t)H * 2, cudaMemcpyDeviceToDevice, st));
+            return EV_OK;
+        }
+        default: return fail(EV_EINVAL, "unknown weight kind");
+    }
+    m->layers[layer].have |= 1u << kind;
+    return EV_OK;
+}
+
+int ev_model_get_quantized(ev_model* m, int kind, int layer, const uint8_t** codes, const float** scales, long* rows, long* cols) {
+    if (!m || !codes || !scales) return fail(EV_EINVAL, "null argument");
+    if (kind >= EV_W_Q && kind <= EV_W_DOWN && (layer < 0 || layer >= m->cfg.n_layers)) return fail(EV_EINVAL, "layer out of range");
+    const long F = m->cfg.ffn;
+    QMat* q = nullptr;
+    long off = 0, n = 0;
+    switch (kind) {
+        case EV_W_Q: q = &m->layers[layer].qkv; off = 0; n = m->q_dim; break;
+        case EV_W_K: q = &m->layers[layer].qkv; off = m->q_dim; n = m->kv_dim; break;
+        case EV_W_V: q = &m->layers[layer].qkv; off = m->q_dim + m->kv_dim; n = m->kv_dim; break;
+        case EV_W_O: q = &m->layers[layer].o; n = q->N; break;
+        case EV_W_GATE: q = &m->layers[layer].gu; off = 0; n = F; break;
+        case EV_W_UP: q = &m->layers[layer].gu; off = F; n = F; break;
+        case EV_W_DOWN: q = &m->layers[layer].down; n = q->N; break;
+        case EV_W_LM_HEAD: q = &m->lm; n = q->N; break;
+        default: return fail(EV_EINVAL, "kind is not a quantized matrix");
+    }
+    *codes = q->codes + off * q->K;
+    *scales = q->scale + off;
+    if (rows) *rows = n;
+    if (cols) *cols = q->K;
+    return EV_OK;
+}
+
+int ev_model_get_static_scales(ev_model* m, float* host_out) {
+    if (!m || !host_out) return fail(EV_EINVAL, "null argument");
+    if (!m->calibrated) return fail(EV_ESTATE, "not calibrated");
+    CUDA_TRY(cudaMemcpy(host_out, m->static_scales, m->n_sites * sizeof(float), cudaMemcpyDeviceToHost));
+    return EV_OK;
+}
+int ev_model_set_static_scales(ev_model* m, const float* host_in) {
+    if (!m || !host_in) return fail(EV_EINVAL, "null argument");
+    CUDA_TRY(cudaMemcpy(m->static_scales, host_in, m->n_sites * sizeof(float), cudaMemcpyHostToDevice));
+    m->calibrated = true;
+    return EV_OK;
+}
+
+// ---- cache ---------------------------------------------------------------------------------------
+int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
+    if (!m || !out || n_pages < 1 || max_seqs < 1) return fail(EV_EINVAL, "bad argument");
+    *out = nullptr;
+    ev_cache* c = new ev_cache();
+    c->model = m;
+    c->n_pages = n_pages;
+    c->max_seqs = max_seqs;
+    const ev_config& cfg = m->cfg;
+    c->max_pages = (cfg.max_ctx + cfg.page_size - 1) / cfg.page_size;
+    c->layer_stride = n_pages * 2L * cfg.n_kv_heads * cfg.page_size * cfg.head_dim;
+    const size_t pool_elems = (size_t)cfg.n_layers * c->layer_stride;
+    bool ok = cudaMalloc((void**)&c->pool, pool_elems * 2) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->page_table, (size_t)max_seqs * c->max_pages * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->ctx_len, (size_t)max_seqs * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->capacity, (size_t)max_seqs * 4) == cudaSuccess;
+    const size_t pf = (size_t)m->M_cap;
+    ok = ok && cudaMalloc((void**)&c->pf_tokens, pf * 4) == cudaSuccess && cudaMalloc((void**)&c->pf_parents, pf * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->pf_nn, (size_t)cfg.max_batch * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->pf_slots, (size_t)cfg.max_batch * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->pf_out, (pf * 2 + (size_t)cfg.max_batch * 3) * 4) == cudaSuccess;
+    if (!ok) {
+        ev_cache_destroy(c);
+        return fail(EV_ENOMEM, "KV pool allocation failed");
+    }
+    cudaMemset(c->pool, 0, pool_elems * 2);
+    cudaMemset(c->page_table, 0, (size_t)max_seqs * c->max_pages * 4);
+    cudaMemset(c->ctx_len, 0, (size_t)max_seqs * 4);
+    cudaMemset(c->capacity, 0, (size_t)max_seqs * 4);
+    c->free_pages.resize(n_pages);
+    for (long i = 0; i < n_pages; ++i) c->free_pages[i] = (int)(n_pages - 1 - i);  // pop_back yields 0,1,2,...
+    c->seq_pages.resize(max_seqs);
+    c->seq_used.assign(max_seqs, 0);
+    c->len_bound.assign(max_seqs, 0);
+    *out = c;
+    return EV_OK;
+}
+
+int ev_cache_destroy(ev_cache* c) {
+    if (!c) return EV_OK;
+    cudaDeviceSynchronize();
+    cudaFree(c->pool); cudaFree(c->page_table); cudaFree(c->ctx_len); cudaFree(c->capacity);
+    cudaFree(c->pf_tokens); cudaFree(c->pf_parents); cudaFree(c->pf_nn); cudaFree(c->pf_slots); cudaFree(c->pf_out);
+    delete c;
+    return EV_OK;
+}
+
+int ev_cache_add_seq(ev_cache* c, int capacity_tokens, const int* host_pages, int* seq_slot_out) {
+    if (!c || !seq_slot_out || capacity_tokens < 1) return fail(EV_EINVAL, "bad argument");
+    const int P = c->model->cfg.page_size;
+    const int need = (capacity_tokens + P - 1) / P;
+    if (need > c->max_pages) return fail(EV_ECAPACITY, "capacity exceeds max_ctx");
+    int slot = -1;
+    for (int i = 0; i < c->max_seqs; ++i)
+        if (!c->seq_used[i]) { slot = i; break; }
+    if (slot < 0) return fail(EV_ECAPACITY, "no free sequence slot");
+    std::vector<int> pages;
+    if (host_pages) {
+        for (int i = 0; i < need; ++i) {
+            const int pg = host_pages[i];
+            auto it = std::find(c->free_pages.begin(), c->free_pages.end(), pg);
+            if (pg < 0 || pg >= c->n_pages || it == c->free_pages.end()) {
+                for (int q : pages) c->free_pages.push_back(q);
+                return fail(EV_EINVAL, "requested page is not free");
+            }
+            c->free_pages.erase(it);
+            pages.push_back(pg);
+        }
+    } else {
+        if ((long)c->free_pages.size() < need) return fail(EV_ECAPACITY, "out of KV pages");
+        for (int i = 0; i < need; ++i) { pages.push_back(c->free_pages.back()); c->free_pages.pop_back(); }
+    }
+    std::vector<int32_t> row(c->max_pages, 0);
+    for (int i = 0; i < need; ++i) row[i] = pages[i];
+    const int32_t cap = need * P, zero = 0;
+    CUDA_TRY(cudaMemcpy(c->page_table + (size_t)slot * c->max_pages, row.data(), row.size() * 4, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(c->capacity + slot, &cap, 4, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(c->ctx_len + slot, &zero, 4, cudaMemcpyHostToDevice));
+    c->seq_pages[slot] = pages;
+    c->seq_used[slot] = 1;
+    c->len_bound[slot] = 0;
+    *seq_slot_out = slot;
+    return EV_OK;
+}
+
+int ev_cache_free_seq(ev_cache* c, int slot) {
+    if (!c || slot < 0 || slot >= c->max_seqs || !c->seq_used[slot]) return fail(EV_EINVAL, "bad sequence slot");
+    for (int pg : c->seq_pages[slot]) c->free_pages.push_back(pg);
+    c->seq_pages[slot].clear();
+    c->seq_used[slot] = 0;
+    const int32_t zero = 0;
+    CUDA_TRY(cudaMemcpy(c->capacity + slot, &zero, 4, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(c->ctx_len + slot, &zero, 4, cudaMemcpyHostToDevice));
+    return EV_OK;
+}
+
+int ev_cache_set_len(ev_cache* c, int slot, int ctx_len, void* stream) {
+    if (!c || slot < 0 || slot >= c->max_seqs || !c->seq_used[slot] || ctx_len < 0) return fail(EV_EINVAL, "bad argument");
+    if (ctx_len > (int)c->seq_pages[slot].size() * c->model->cfg.page_size) return fail(EV_ECAPACITY, "ctx_len exceeds capacity");
+    set_i32_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(c->ctx_len + slot, ctx_len);
+    LAUNCH_CHECK();
+    c->len_bound[slot] = ctx_len;
+    return EV_OK;
+}
+int ev_cache_get_len(ev_cache* c, int slot, int* ctx_len, void* stream) {
+    if (!c || !ctx_len || slot < 0 || slot >= c->max_seqs || !c->seq_used[slot]) return fail(EV_EINVAL, "bad argument");
+    int32_t v = 0;
+    CUDA_TRY(cudaMemcpyAsync(&v, c->ctx_len + slot, 4, cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CUDA_TRY(cudaStreamSynchronize((cudaStream_t)stream));
+    *ctx_len = v;
+    c->len_bound[slot] = v;
+    return EV_OK;
+}
+
+static int dense_copy(ev_cache* c, int slot, int lb, int le, int n_tokens, void* dense, int to_dense, cudaStream_t st) {
+    if (!c || !dense || slot < 0 || slot >= c->max_seqs || !c->seq_used[slot]) return fail(EV_EINVAL, "bad argument");
+    const ev_config& cfg = c->model->cfg;
+    if (lb < 0 || le > cfg.n_layers || lb >= le || n_tokens < 1) return fail(EV_EINVAL, "bad layer / token range");
+    if (n_tokens > (int)c->seq_pages[slot].size() * cfg.page_size) return fail(EV_ECAPACITY, "n_tokens exceeds capacity");
+    DenseCopyArgs a;
+    a.Hkv = cfg.n_kv_heads; a.D = cfg.head_dim; a.page_size = cfg.page_size; a.n_tokens = n_tokens; a.layer_begin = lb;
+    a.layer_stride = c->layer_stride; a.pool = c->pool; a.page_row = c->page_table + (size_t)slot * c->max_pages;
+    a.dense = (__nv_bfloat16*)dense; a.to_dense = to_dense;
+    dense_copy_kernel<<<dim3(n_tokens, le - lb), 128, 0, st>>>(a);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+int ev_cache_export_seq(ev_cache* c, int slot, int lb, int le, int n_tokens, void* dense, void* stream) {
+    return dense_copy(c, slot, lb, le, n_tokens, dense, 1, (cudaStream_t)stream);
+}
+int ev_cache_import_seq(ev_cache* c, int slot, int lb, int le, int n_tokens, const void* dense, int set_len, void* stream) {
+    EV_TRY(dense_copy(c, slot, lb, le, n_tokens, const_cast<void*>(dense), 0, (cudaStream_t)stream));
+    if (set_len) return ev_cache_set_len(c, slot, n_tokens, stream);
+    return EV_OK;
+}
+
+// ---- verify ----------------------------------------------------------------------------------------
+int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* out, void* stream) {
+    if (!m || !c || !in || !out) return fail(EV_EINVAL, "null argument");
+    if (c->model != m) return fail(EV_EINVAL, "cache belongs to another model");
+    if (in->n_seqs < 1 || in->n_nodes_max < 1) return fail(EV_EINVAL, "n_seqs and n_nodes_max must be positive");
+    if (in->n_seqs > m->cfg.max_batch || in->n_nodes_max > m->cfg.max_tree_nodes)
+        return fail(EV_ECAPACITY, "batch or tree size exceeds the model's max_batch / max_tree_nodes");
+    if (!in->dev_seq_slots || !in->dev_tokens || !in->dev_parents) return fail(EV_EINVAL, "null input array");
+    if (!out->dev_accept_len || !out->dev_accept_nodes || !out->dev_out_tokens || !out->dev_new_ctx_len || !out->dev_status)
+        return fail(EV_EINVAL, "null required output array");
+    const bool need_lm = !in->force_accept_all || m->recording;
+    EV_TRY(check_ready(m, need_lm));
+    return run_forward(m, c, in, out, (cudaStream_t)stream, need_lm);
+}
+
+int ev_cache_prefill(ev_model* m, ev_cache* c, int n_seqs, const int* host_seq_slots, const int32_t* host_token_ids,
+                     const int* host_lens, void* stream) {
+    if (!m || !c || !host_seq_slots || !host_token_ids || !host_lens || n_seqs < 1) return fail(EV_EINVAL, "bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int T = m->cfg.max_tree_nodes, Bmax = m->cfg.max_batch;
+    std::vector<long> off(n_seqs + 1, 0);
+    for (int i = 0; i < n_seqs; ++i) {
+        if (host_lens[i] < 0) return fail(EV_EINVAL, "negative length");
+        off[i + 1] = off[i] + host_lens[i];
+    }
+    std::vector<int> done(n_seqs, 0);
+    std::vector<int32_t> tok((size_t)Bmax * T), par((size_t)Bmax * T), nn(Bmax), slots(Bmax);
+    ev_verify_out o;
+    memset(&o, 0, sizeof(o));
+    o.tap_layer = -1;
+    o.dev_accept_len = c->pf_out;
+    o.dev_new_ctx_len = c->pf_out + Bmax;
+    o.dev_status = c->pf_out + 2 * Bmax;
+    o.dev_accept_nodes = c->pf_out + 3 * Bmax;
+    o.dev_out_tokens = o.dev_accept_nodes + (size_t)m->M_cap;
+    while (true) {
+        int B = 0;
+        for (int i = 0; i < n_seqs && B < Bmax; ++i) {
+            const int rem = host_lens[i] - done[i];
+            if (rem <= 0) continue;
+            const int n = std::min(rem, T);
+            for (int j = 0; j < T; ++j) {
+                tok[(size_t)B * T + j] = j < n ? host_token_ids[off[i] + done[i] + j] : 0;
+                par[(size_t)B * T + j] = j - 1;
+            }
+            nn[B] = n;
+            slots[B] = host_seq_slots[i];
+            done[i] += n;
+            ++B;
+        }
+        if (B == 0) break;
+        CUDA_TRY(cudaMemcpyAsync(c->pf_tokens, tok.data(), (size_t)B * T * 4, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(c->pf_parents, par.data(), (size_t)B * T * 4, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(c->pf_nn, nn.data(), (size_t)B * 4, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(c->pf_slots, slots.data(), (size_t)B * 4, cudaMemcpyHostToDevice, st));
+        ev_verify_in in;
+        memset(&in, 0, sizeof(in));
+        in.n_seqs = B; in.n_nodes_max = T; in.dev_seq_slots = c->pf_slots; in.dev_tokens = c->pf_tokens;
+        in.dev_parents = c->pf_parents; in.dev_n_nodes = c->pf_nn; in.commit = 1; in.force_accept_all = 1;
+        EV_TRY(ev_verify(m, c, &in, &o, stream));
+        CUDA_TRY(cudaStreamSynchronize(st));  // host staging buffers are reused by the next pass
+        std::vector<int32_t> status(B);
+        CUDA_TRY(cudaMemcpy(status.data(), o.dev_status, (size_t)B * 4, cudaMemcpyDeviceToHost));
+        for (int i = 0; i < B; ++i)
+            if (status[i]) return fail(status[i] & EV_SEQ_OVER_CAPACITY ? EV_ECAPACITY : EV_EINVAL,
+                                       "prefill: sequence rejected, status " + std::to_string(status[i]));
+    }
+    return EV_OK;
+}
+
+int ev_model_calibrate(ev_model* m, const float* dev_hidden, int n_tok, float* dev_layer_inputs, void* stream) {
+    if (!m || !dev_hidden || n_tok < 1) return fail(EV_EINVAL, "bad argument");
+    if (n_tok > m->cfg.max_ctx) return fail(EV_ECAPACITY, "n_tok exceeds max_ctx");
+    cudaStream_t st = (cudaStream_t)stream;
+    const ev_config& cfg = m->cfg;
+    const int T = cfg.max_tree_nodes, H = cfg.hidden;
+    ev_cache* c = nullptr;
+    EV_TRY(ev_cache_create(m, (n_tok + cfg.page_size - 1) / cfg.page_size + 1, 1, &c));
+    int slot = -1, rc = ev_cache_add_seq(c, n_tok, nullptr, &slot);
+    float* taps = nullptr;
+    if (rc == EV_OK && dev_layer_inputs && cudaMalloc((void**)&taps, (size_t)(cfg.n_layers + 1) * T * H * 4) != cudaSuccess)
+        rc = fail(EV_ENOMEM, "calibration tap buffer");
+    if (rc == EV_OK && cudaMemsetAsync(m->site_amax, 0, m->n_sites * 4, st) != cudaSuccess) rc = fail(EV_ECUDA, "memset");
+    m->recording = true;
+    std::vector<int32_t> tok(T, 0), par(T);
+    for (int j = 0; j < T; ++j) par[j] = j - 1;
+    ev_verify_out o;
+    memset(&o, 0, sizeof(o));
+    o.tap_layer = -1;
+    o.dev_accept_len = c->pf_out; o.dev_new_ctx_len = c->pf_out + 1; o.dev_status = c->pf_out + 2;
+    o.dev_accept_nodes = c->pf_out + 3; o.dev_out_tokens = c->pf_out + 3 + T;
+    o.dev_hidden = taps;
+    for (int p0 = 0; rc == EV_OK && p0 < n_tok; p0 += T) {
+        const int n = std::min(T, n_tok - p0);
+        const int32_t nn = n, sl = slot;
+        auto cp = [&](void* d, const void* s, size_t b) { if (rc == EV_OK && cudaMemcpyAsync(d, s, b, cudaMemcpyHostToDevice, st) != cudaSuccess) rc = fail(EV_ECUDA, "H2D copy"); };
+        cp(c->pf_tokens, tok.data(), (size_t)T * 4);
+        cp(c->pf_parents, par.data(), (size_t)T * 4);
+        cp(c->pf_nn, &nn, 4);
+        cp(c->pf_slots, &sl, 4);
+        ev_verify_in in;
+        memset(&in, 0, sizeof(in));
+        in.n_seqs = 1; in.n_nodes_max = n; in.dev_seq_slots = c->pf_slots; in.dev_tokens = c->pf_tokens;
+        in.dev_parents = c->pf_parents; in.dev_n_nodes = c->pf_nn; in.commit = 1; in.force_accept_all = 1;
+        in.dev_hidden_override = dev_hidden + (size_t)p0 * H; in.override_first_only = 1;
+        if (rc == EV_OK) rc = ev_verify(m, c, &in, &o, stream);
+        if (rc == EV_OK && taps)
+            for (int l = 0; l <= cfg.n_layers && rc == EV_OK; ++l)
+                if (cudaMemcpyAsync(dev_layer_inputs + ((size_t)l * n_tok + p0) * H, taps + (size_t)l * n * H, (size_t)n * H * 4,
+                                    cudaMemcpyDeviceToDevice, st) != cudaSuccess) rc = fail(EV_ECUDA, "tap copy");
+        if (rc == EV_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = fail(EV_ECUDA, "calibration pass failed");
+    }
+    m->recording = false;
+    if (rc == EV_OK) {
+        std::vector<float> amax(m->n_sites), sc(m->n_sites);
+        if (cudaMemcpy(amax.data(), m->site_amax, m->n_sites * 4, cudaMemcpyDeviceToHost) != cudaSuccess) rc = fail(EV_ECUDA, "D2H copy");
+        for (int i = 0; i < m->n_sites; ++i) sc[i] = amax[i] > 0.f ? amax[i] / 448.0f : 1.0f;
+        if (rc == EV_OK && cudaMemcpy(m->static_scales, sc.data(), m->n_sites * 4, cudaMemcpyHostToDevice) != cudaSuccess) rc = fail(EV_ECUDA, "H2D copy");
+        if (rc == EV_OK) m->calibrated = true;
+    }
+    std::string keep = g_err;
+    if (taps) cudaFree(taps);
+    ev_cache_destroy(c);
+    g_err = keep;
+    return rc;
+}
+
+// ---- single operators --------------------------------------------------------------------------------
+int ev_op_quantize_rows(ev_model* m, const float* dev_x, int M, int K, float static_scale, uint8_t* dev_codes, float* dev_sx,
+                        void* stream) {
+    if (!m || !dev_x || !dev_codes || !dev_sx || M < 1 || K < 4 || K % 4) return fail(EV_EINVAL, "bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    QuantOut q;
+    q.codes = dev_codes; q.sx = dev_sx; q.static_scale = nullptr; q.site_amax = nullptr;
+    if (static_scale > 0.f) {
+        CUDA_TRY(cudaMemcpyAsync(m->site_amax, &static_scale, 4, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        q.static_scale = m->site_amax;
+    }
+    quantize_rows_kernel<<<M, EW_THREADS, 0, st>>>(dev_x, K, q);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+
+int ev_op_linear(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, const float* dev_sx, int M, float* dev_out,
+                 void* stream) {
+    if (!m || !dev_codes_x || !dev_sx || !dev_out || M < 1) return fail(EV_EINVAL, "bad argument");
+    if (M > m->M_cap) return fail(EV_ECAPACITY, "M exceeds max_batch * max_tree_nodes");
+    cudaStream_t st = (cudaStream_t)stream;
+    QMat* w = nullptr;
+    ActBuf* x = nullptr;
+    if (kind != EV_W_LM_HEAD && (layer < 0 || layer >= m->cfg.n_layers)) return fail(EV_EINVAL, "layer out of range");
+    // fused storage: Q/K/V and GATE/UP are computed together (the kernel the step uses)
+    switch (kind) {
+        case EV_W_Q: w = &m->layers[layer].qkv; x = &m->xq; break;
+        case EV_W_O: w = &m->layers[layer].o; x = &m->aq; break;
+        case EV_W_GATE: w = &m->layers[layer].gu; x = &m->xq; break;
+        case EV_W_DOWN: w = &m->layers[layer].down; x = &m->tq; break;
+        case EV_W_LM_HEAD: w = &m->lm; x = &m->xq; break;
+        default: return fail(EV_EINVAL, "ev_op_linear: kind must be Q (=fused QKV), O, GATE (=fused gate|up), DOWN or LM_HEAD");
+    }
+    CUDA_TRY(cudaMemcpyAsync(x->codes, dev_codes_x, (size_t)M * w->K, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(x->scale, dev_sx, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+    if (kind == EV_W_LM_HEAD) {
+        CUDA_TRY(cudaMemsetAsync(m->argmax_keys, 0, (size_t)M * 8, st));
+        return run_linear(m, st, *w, *x, M, EPI_ARGMAX, dev_out, (int)w->N, m->argmax_keys);
+    }
+    return run_linear(m, st, *w, *x, M, EPI_STORE, dev_out, (int)w->N, nullptr);
+}
+
+}  // extern "C"

@@ -1,0 +1,296 @@
+// K5: tree-masked GQA attention over the paged bf16 KV cache ("tree attention";
+// BASELINE.json:north_star (2)), split over the key axis, + K7: merge of the splits fused with the
+// per-token absmax / E4M3 quantization that feeds the O projection.
+//
+// One CTA = (sequence b, kv head, group of 8 row tiles, key split).  The query rows of one kv head
+// are the T nodes x G query heads that share it (row = node*G + g), 16 rows per warp.  Keys are the
+// L committed context slots followed by the T tree slots L..L+T-1 (written by the RoPE/KV-write
+// kernel just before); a tree key j is visible to node i iff j is an ancestor-or-self of i (bit j
+// of anc[i]).  Pages are gathered with 16-byte cp.async into XOR-swizzled shared memory (each
+// (page, K|V, head) block is page_size*D*2 contiguous bytes), double buffered; Q.K^T and P.V run on
+// the tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with Q and P each split into
+// hi + lo bf16 parts so that ~16 mantissa bits survive (DESIGN.md section 6 "attention precision");
+// the online softmax is done in fp32 registers with warp shuffles across the 4 lanes of a row.
+#pragma once
+#include "ev_common.cuh"
+#include "ev_elementwise.cuh"
+
+namespace ev {
+
+constexpr int ATT_THREADS = 256;
+constexpr int ATT_WARPS = 8;
+constexpr int ATT_CH = 64;  // keys per pipeline chunk
+
+struct AttnArgs {
+    const float* q;       // qkv buffer after RoPE; q head h of row m at q[m*q_ld + h*D]
+    int q_ld, T, G, Hq, Hkv;
+    const __nv_bfloat16* pool;  // this layer: [page][2][Hkv][page_size][D]
+    const int32_t* page_table;  // [max_seqs][max_pages]
+    int max_pages, page_size;
+    const int32_t* seq_slots;   // [B]
+    const int32_t* Lsnap;       // [B]
+    const int32_t* nn_eff;      // [B]
+    const unsigned long long* anc;  // [B][T]
+    int split_len;              // keys per split, multiple of ATT_CH
+    int n_splits;               // grid.x
+    float scale;                // 1/sqrt(D)
+    float* o_part;              // [M][Hq][n_splits][D]
+    float* ml_part;             // [M][Hq][n_splits][2]  (running max, running sum)
+};
+
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+    asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+// D(16x8, fp32) += A(16x16 bf16, row) * B(16x8 bf16, col)
+__device__ __forceinline__ void mma_bf16(float* d, const uint32_t* a, uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+        : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+        : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+// x = hi + lo with hi = bf16(x), lo = bf16(x - hi); packs two values (first in the low half)
+__device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+    const __nv_bfloat16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
+    const __nv_bfloat16 l0 = __float2bfloat16_rn(x0 - __bfloat162float(h0));
+    const __nv_bfloat16 l1 = __float2bfloat16_rn(x1 - __bfloat162float(h1));
+    hi = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+    lo = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+}
+__device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool valid) {
+    const int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(sz) : "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnArgs a) {
+    constexpr int ROWB = D * 2;           // bytes per key row
+    constexpr int CPR = ROWB / 16;        // 16-byte chunks per row
+    constexpr int TILE = ATT_CH * ROWB;   // bytes per K (or V) tile
+    constexpr int KT = D / 16;            // k-tiles of the Q.K^T contraction
+    extern __shared__ __align__(128) uint8_t att_smem[];  // [2 stages][K tile | V tile]
+
+    const int split = blockIdx.x;
+    const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
+    const int b = blockIdx.z;
+    const int nn = a.nn_eff[b];
+    if (nn == 0) return;
+    const int L = a.Lsnap[b];
+    const int n_keys = L + nn;
+    const int k_begin = split * a.split_len;
+    if (k_begin >= n_keys) return;
+    const int k_end = min(k_begin + a.split_len, n_keys);
+    const int n_chunks = (k_end - k_begin + ATT_CH - 1) / ATT_CH;
+    const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int R = a.T * a.G;
+    const int rt = rg * ATT_WARPS + warp;
+    const bool active = rt * 16 < R;
+    const int row0 = rt * 16 + (lane >> 2), row1 = row0 + 8;
+    const int node0 = row0 / a.G, g0 = row0 % a.G, node1 = row1 / a.G, g1 = row1 % a.G;
+    const bool v0 = active && row0 < R && node0 < nn, v1 = active && row1 < R && node1 < nn;
+    const unsigned long long anc0 = v0 ? a.anc[b * a.T + node0] : 0ull, anc1 = v1 ? a.anc[b * a.T + node1] : 0ull;
+
+    // ---- Q fragments (A operand), split hi/lo ----
+    uint32_t qhi[KT][4], qlo[KT][4];
+    {
+        const float* q0 = a.q + (size_t)(b * a.T + (v0 ? node0 : 0)) * a.q_ld + (size_t)(kvh * a.G + (v0 ? g0 : 0)) * D;
+        const float* q1 = a.q + (size_t)(b * a.T + (v1 ? node1 : 0)) * a.q_ld + (size_t)(kvh * a.G + (v1 ? g1 : 0)) * D;
+#pragma unroll
+        for (int kt = 0; kt < KT; ++kt) {
+            const int c = kt * 16 + (lane & 3) * 2;
+            float2 x00 = v0 ? *reinterpret_cast<const float2*>(q0 + c) : make_float2(0.f, 0.f);
+            float2 x10 = v1 ? *reinterpret_cast<const float2*>(q1 + c) : make_float2(0.f, 0.f);
+            float2 x01 = v0 ? *reinterpret_cast<const float2*>(q0 + c + 8) : make_float2(0.f, 0.f);
+            float2 x11 = v1 ? *reinterpret_cast<const float2*>(q1 + c + 8) : make_float2(0.f, 0.f);
+            split2(x00.x, x00.y, qhi[kt][0], qlo[kt][0]);
+            split2(x10.x, x10.y, qhi[kt][1], qlo[kt][1]);
+            split2(x01.x, x01.y, qhi[kt][2], qlo[kt][2]);
+            split2(x11.x, x11.y, qhi[kt][3], qlo[kt][3]);
+        }
+    }
+
+    // ---- page gather: chunk ch -> stage ----
+    auto load_chunk = [&](int stage, int ch) {
+        uint8_t* kt_s = att_smem + stage * 2 * TILE;
+        uint8_t* vt_s = kt_s + TILE;
+        const int kbase = k_begin + ch * ATT_CH;
+        for (int i = threadIdx.x; i < ATT_CH * CPR; i += ATT_THREADS) {
+            const int r = i / CPR, c = i % CPR;
+            const int kidx = kbase + r;
+            const bool ok = kidx < k_end;
+            const int kk = ok ? kidx : k_begin;
+            const size_t base = (size_t)pt[kk / a.page_size] * 2 * a.Hkv * a.page_size * D +
+                                (size_t)kvh * a.page_size * D + (size_t)(kk % a.page_size) * D + (size_t)c * 8;
+            const int so = r * ROWB + ((c ^ (r & 7)) * 16);
+            cp_async16_zfill(kt_s + so, a.pool + base, ok);
+            cp_async16_zfill(vt_s + so, a.pool + base + (size_t)a.Hkv * a.page_size * D, ok);
+        }
+    };
+
+    float o[D / 8][4];
+#pragma unroll
+    for (int i = 0; i < D / 8; ++i) { o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f; }
+    float m0 = -INFINITY, m1 = -INFINITY, l0 = 0.f, l1 = 0.f;
+
+    load_chunk(0, 0);
+    cp_async_commit();
+    for (int ch = 0; ch < n_chunks; ++ch) {
+        if (ch + 1 < n_chunks) {
+            load_chunk((ch + 1) & 1, ch + 1);
+            cp_async_commit();
+            cp_async_wait<1>();
+        } else {
+            cp_async_wait<0>();
+        }
+        __syncthreads();
+        if (active) {
+            const uint32_t ks = smem_u32(att_smem + (ch & 1) * 2 * TILE);
+            const uint32_t vs = ks + TILE;
+            const int kbase = k_begin + ch * ATT_CH;
+            // ---- S = Q K^T (16 rows x 64 keys per warp) ----
+            float s[ATT_CH / 8][4];
+#pragma unroll
+            for (int nt = 0; nt < ATT_CH / 8; ++nt) {
+                s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
+                const int r = nt * 8 + (lane & 7);
+#pragma unroll
+                for (int kp = 0; kp < KT / 2; ++kp) {
+                    const int c = kp * 4 + (lane >> 3);
+                    uint32_t b0, b1, b2, b3;
+                    ldsm_x4(ks + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
+                    mma_bf16(s[nt], qhi[2 * kp], b0, b1);
+                    mma_bf16(s[nt], qlo[2 * kp], b0, b1);
+                    mma_bf16(s[nt], qhi[2 * kp + 1], b2, b3);
+                    mma_bf16(s[nt], qlo[2 * kp + 1], b2, b3);
+                }
+            }
+            // ---- scale, mask, row max ----
+            const bool need_mask = kbase + ATT_CH > L;  // chunk touches tree keys or the split end
+            float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+            for (int nt = 0; nt < ATT_CH / 8; ++nt) {
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    float v = mul_rn(s[nt][e], a.scale);
+                    if (need_mask) {
+                        const int kidx = kbase + nt * 8 + (lane & 3) * 2 + (e & 1);
+                        const unsigned long long am = (e < 2) ? anc0 : anc1;
+                        const bool ok = kidx < k_end && (kidx < L || ((am >> (kidx - L)) & 1ull));
+                        if (!ok) v = -INFINITY;
+                    }
+                    s[nt][e] = v;
+                    if (e < 2) mx0 = fmaxf(mx0, v); else mx1 = fmaxf(mx1, v);
+                }
+            }
+            mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 1));
+            mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, 2));
+            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 1));
+            mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
+            const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
+            const float mu0 = (mn0 == -INFINITY) ? 0.f : mn0, mu1 = (mn1 == -INFINITY) ? 0.f : mn1;
+            const float c0 = __expf(m0 - mu0), c1 = __expf(m1 - mu1);  // exp(-inf) = 0 on the first chunk
+            m0 = mn0; m1 = mn1;
+            l0 *= c0; l1 *= c1;
+#pragma unroll
+            for (int i = 0; i < D / 8; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
+#pragma unroll
+            for (int nt = 0; nt < ATT_CH / 8; ++nt) {
+                s[nt][0] = __expf(s[nt][0] - mu0); s[nt][1] = __expf(s[nt][1] - mu0);
+                s[nt][2] = __expf(s[nt][2] - mu1); s[nt][3] = __expf(s[nt][3] - mu1);
+                l0 += s[nt][0] + s[nt][1];
+                l1 += s[nt][2] + s[nt][3];
+            }
+            // ---- O += P V ----
+#pragma unroll
+            for (int kt2 = 0; kt2 < ATT_CH / 16; ++kt2) {
+                uint32_t phi[4], plo[4];
+                split2(s[2 * kt2][0], s[2 * kt2][1], phi[0], plo[0]);
+                split2(s[2 * kt2][2], s[2 * kt2][3], phi[1], plo[1]);
+                split2(s[2 * kt2 + 1][0], s[2 * kt2 + 1][1], phi[2], plo[2]);
+                split2(s[2 * kt2 + 1][2], s[2 * kt2 + 1][3], phi[3], plo[3]);
+                const int r = kt2 * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
+#pragma unroll
+                for (int np = 0; np < D / 16; ++np) {
+                    const int c = np * 2 + (lane >> 4);
+                    uint32_t b0, b1, b2, b3;
+                    ldsm_x4_trans(vs + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
+                    mma_bf16(o[2 * np], phi, b0, b1);
+                    mma_bf16(o[2 * np], plo, b0, b1);
+                    mma_bf16(o[2 * np + 1], phi, b2, b3);
+                    mma_bf16(o[2 * np + 1], plo, b2, b3);
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (!active) return;
+    l0 += __shfl_xor_sync(0xffffffffu, l0, 1);
+    l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+    l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
+    l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+    if (row0 < R) {
+        const size_t pi = ((size_t)(b * a.T + node0) * a.Hq + kvh * a.G + g0) * a.n_splits + split;
+        float* op = a.o_part + pi * D + (lane & 3) * 2;
+#pragma unroll
+        for (int i = 0; i < D / 8; ++i) *reinterpret_cast<float2*>(op + i * 8) = make_float2(o[i][0], o[i][1]);
+        if ((lane & 3) == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m0, l0);
+    }
+    if (row1 < R) {
+        const size_t pi = ((size_t)(b * a.T + node1) * a.Hq + kvh * a.G + g1) * a.n_splits + split;
+        float* op = a.o_part + pi * D + (lane & 3) * 2;
+#pragma unroll
+        for (int i = 0; i < D / 8; ++i) *reinterpret_cast<float2*>(op + i * 8) = make_float2(o[i][2], o[i][3]);
+        if ((lane & 3) == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m1, l1);
+    }
+}
+
+// ---- merge of the key splits (fixed order 0..ns-1) + per-token absmax + E4M3 quantize -----------
+struct MergeArgs {
+    int T, Hq, D, n_splits, split_len;
+    const int32_t* Lsnap;
+    const int32_t* nn_eff;
+    const float* o_part;
+    const float* ml_part;
+    float* attn;   // [M][Hq*D] fp32 merged output (workspace; also the debug tap)
+    QuantOut q;
+};
+__global__ void __launch_bounds__(EW_THREADS) attn_merge_quant_kernel(MergeArgs a) {
+    __shared__ float red[EW_THREADS / 32];
+    const int m = blockIdx.x;
+    const int b = m / a.T, node = m % a.T;
+    const int nn = a.nn_eff[b];
+    const int K = a.Hq * a.D;
+    float* out = a.attn + (size_t)m * K;
+    const bool valid = node < nn;
+    const int ns = valid ? (a.Lsnap[b] + nn + a.split_len - 1) / a.split_len : 0;
+    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4) {
+        float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (valid) {
+            const int h = i / a.D, d = i % a.D;
+            const size_t pi = ((size_t)m * a.Hq + h) * a.n_splits;
+            float mx = -INFINITY;
+            for (int s = 0; s < ns; ++s) mx = fmaxf(mx, a.ml_part[(pi + s) * 2]);
+            float den = 0.f;
+            float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s = 0; s < ns; ++s) {
+                const float2 ml = *reinterpret_cast<const float2*>(a.ml_part + (pi + s) * 2);
+                const float w = (ml.x == -INFINITY) ? 0.f : __expf(ml.x - mx);
+                const float4 ov = *reinterpret_cast<const float4*>(a.o_part + (pi + s) * a.D + d);
+                den += w * ml.y;
+                num.x += w * ov.x; num.y += w * ov.y; num.z += w * ov.z; num.w += w * ov.w;
+            }
+            r = make_float4(div_rn(num.x, den), div_rn(num.y, den), div_rn(num.z, den), div_rn(num.w, den));
+        }
+        *reinterpret_cast<float4*>(out + i) = r;
+    }
+    __syncthreads();
+    quantize_row(m, K, [&](int i) -> float { return out[i]; }, a.q, red);
+}
+
+}  // namespace ev

@@ -1,0 +1,393 @@
+// HBM-/latency-bound kernels of the verify step: weight quantizer (K1), embedding gather (K11),
+// RMSNorm + per-token absmax + E4M3 quantize (K3), RoPE + paged KV write (K4), SwiGLU + quantize
+// (K6), tree bookkeeping, argmax finalize (K8), greedy acceptance walk (K9), KV compaction (K10).
+// All element-wise arithmetic uses explicitly rounded fp32 operations (ev::mul_rn ...) so each
+// value is bit-identical to the method's definition given the same inputs.
+#pragma once
+#include "ev_common.cuh"
+
+namespace ev {
+
+constexpr int EW_THREADS = 256;
+
+__device__ __forceinline__ float block_max(float v, float* red) {
+    v = warp_max(v);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    __syncthreads();
+    if (l == 0) red[w] = v;
+    __syncthreads();
+    float r = red[0];
+#pragma unroll
+    for (int i = 1; i < EW_THREADS / 32; ++i) r = fmaxf(r, red[i]);
+    return r;
+}
+
+// ---- K1: per-output-channel absmax -> scale, E4M3 codes --------------------------------------
+// one CTA per output channel (row); cols % 8 == 0
+__global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const __nv_bfloat16* __restrict__ w, long cols,
+                                                                          uint8_t* __restrict__ codes,
+                                                                          float* __restrict__ scales) {
+    __shared__ float red[EW_THREADS / 32];
+    const long row = blockIdx.x;
+    const uint4* src = reinterpret_cast<const uint4*>(w + row * cols);
+    const int nvec = (int)(cols / 8);
+    float amax = 0.f;
+    for (int i = threadIdx.x; i < nvec; i += EW_THREADS) {
+        uint4 v = __ldg(src + i);
+        const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            amax = fmaxf(amax, fabsf(__uint_as_float(u[j] << 16)));
+            amax = fmaxf(amax, fabsf(__uint_as_float(u[j] & 0xFFFF0000u)));
+        }
+    }
+    amax = block_max(amax, red);
+    const float s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
+    if (threadIdx.x == 0) scales[row] = s;
+    uint2* dst = reinterpret_cast<uint2*>(codes + row * cols);
+    for (int i = threadIdx.x; i < nvec; i += EW_THREADS) {
+        uint4 v = __ldg(src + i);
+        const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+        float f[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            f[2 * j] = div_rn(__uint_as_float(u[j] << 16), s);
+            f[2 * j + 1] = div_rn(__uint_as_float(u[j] & 0xFFFF0000u), s);
+        }
+        uint2 o;
+        o.x = e4m3x4(f[0], f[1], f[2], f[3]);
+        o.y = e4m3x4(f[4], f[5], f[6], f[7]);
+        dst[i] = o;
+    }
+}
+
+// ---- tree bookkeeping: one thread per sequence -----------------------------------------------
+struct TreePrepArgs {
+    int B, T, vocab, page_size;
+    const int32_t* seq_slots;  // [B]
+    const int32_t* tokens;     // [B][T]
+    const int32_t* parents;    // [B][T]
+    const int32_t* n_nodes;    // [B] or null
+    const int32_t* ctx_len;    // [max_seqs] (device state)
+    const int32_t* capacity;   // [max_seqs] tokens
+    int max_seqs, max_pos;
+    int32_t* Lsnap;            // [B] context length at entry
+    int32_t* nn_eff;           // [B] nodes in use (0 when the sequence is rejected)
+    int32_t* status;           // [B]
+    int32_t* depth;            // [B][T]
+    int32_t* pos;              // [B][T] RoPE position = L + depth
+    unsigned long long* anc;   // [B][T] ancestor-or-self bit masks
+    unsigned long long* argmax_keys;  // [B*T] reset to 0 here
+};
+
+__global__ void tree_prep_kernel(TreePrepArgs a) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= a.B) return;
+    const int T = a.T;
+    int st = 0;
+    const int slot = a.seq_slots[b];
+    int nn = a.n_nodes ? a.n_nodes[b] : T;
+    int L = 0;
+    if (slot < 0 || slot >= a.max_seqs) {
+        st |= 4;
+    } else {
+        L = a.ctx_len[slot];
+        if (nn < 1 || nn > T) st |= 1;
+        else if (L + nn > a.capacity[slot] || L + nn > a.max_pos) st |= 4;
+    }
+    if (!(st & 1)) {
+        for (int i = 0; i < nn; ++i) {
+            const int p = a.parents[b * T + i];
+            const int tk = a.tokens[b * T + i];
+            if (tk < 0 || tk >= a.vocab) st |= 2;
+            if (i == 0 ? (p != -1) : (p < 0 || p >= i)) { st |= 1; break; }
+        }
+    }
+    a.status[b] = st;
+    a.Lsnap[b] = L;
+    a.nn_eff[b] = st ? 0 : nn;
+    for (int i = 0; i < T; ++i) {
+        int d = 0;
+        unsigned long long m = 1ull;  // padding / rejected rows see the root only
+        if (!st && i < nn) {
+            const int p = a.parents[b * T + i];
+            if (i > 0) { d = a.depth[b * T + p] + 1; m = a.anc[b * T + p] | (1ull << i); }
+        }
+        a.depth[b * T + i] = d;
+        a.pos[b * T + i] = L + d;
+        a.anc[b * T + i] = m;
+        a.argmax_keys[b * T + i] = 0ull;
+    }
+}
+
+// ---- K11: embedding gather: residual stream (fp32) <- bf16 rows --------------------------------
+__global__ void __launch_bounds__(EW_THREADS) embed_gather_kernel(const int32_t* __restrict__ tokens, int vocab,
+                                                                  const __nv_bfloat16* __restrict__ table, int H,
+                                                                  float* __restrict__ h) {
+    const int m = blockIdx.x;
+    const int tk = tokens[m];
+    const bool ok = tk >= 0 && tk < vocab;
+    const uint32_t* src = reinterpret_cast<const uint32_t*>(table + (size_t)(ok ? tk : 0) * H);
+    float2* dst = reinterpret_cast<float2*>(h + (size_t)m * H);
+    for (int i = threadIdx.x; i < H / 2; i += EW_THREADS) {
+        const uint32_t u = ok ? __ldg(src + i) : 0u;
+        dst[i] = make_float2(__uint_as_float(u << 16), __uint_as_float(u & 0xFFFF0000u));
+    }
+}
+
+// ---- per-token quantization of a row already held as fp32 values produced by `val(i)` ----------
+// shared tail of K3 / K6 / ev_op_quantize_rows: absmax -> scale -> codes
+struct QuantOut {
+    uint8_t* codes;            // [M][K]
+    float* sx;                 // [M]
+    const float* static_scale; // null = dynamic per-token
+    float* site_amax;          // null, or calibration accumulator (atomicMax on the float's bits)
+};
+
+template <class F>
+__device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut& q, float* red) {
+    float amax = 0.f;
+    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) amax = fmaxf(amax, fabsf(val(i + j)));
+    }
+    amax = block_max(amax, red);
+    float s;
+    if (q.static_scale) s = *q.static_scale;
+    else s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
+    if (threadIdx.x == 0) {
+        q.sx[m] = s;
+        if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
+    }
+    uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
+    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4)
+        dst[i >> 2] = e4m3x4(div_rn(val(i), s), div_rn(val(i + 1), s), div_rn(val(i + 2), s), div_rn(val(i + 3), s));
+}
+
+// ---- K3: RMSNorm + quantize; one CTA per token; H % 4 == 0 --------------------------------------
+__global__ void __launch_bounds__(EW_THREADS) rmsnorm_quant_kernel(const float* __restrict__ h, int H,
+                                                                   const __nv_bfloat16* __restrict__ gain, float eps,
+                                                                   QuantOut q) {
+    __shared__ float red[EW_THREADS / 32];
+    __shared__ double dred[EW_THREADS / 32];
+    const int m = blockIdx.x;
+    const float* x = h + (size_t)m * H;
+    double acc = 0.0;  // mean of squares accumulated in fp64, rounded once (DESIGN.md R-accum)
+    for (int i = threadIdx.x * 4; i < H; i += EW_THREADS * 4) {
+        const float4 v = *reinterpret_cast<const float4*>(x + i);
+        acc += (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z + (double)v.w * v.w;
+    }
+    acc = warp_sum(acc);
+    if ((threadIdx.x & 31) == 0) dred[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int i = 0; i < EW_THREADS / 32; ++i) tot += dred[i];
+    const float ms = (float)(tot / (double)H);
+    const float r = div_rn(1.0f, sqrtf(add_rn(ms, eps)));
+    auto val = [&](int i) -> float {
+        const float g = gain ? __bfloat162float(gain[i]) : 1.0f;
+        return mul_rn(mul_rn(x[i], r), g);
+    };
+    quantize_row(m, H, val, q, red);
+}
+
+// plain per-token quantization of fp32 rows (attention output uses the fused merge kernel instead)
+__global__ void __launch_bounds__(EW_THREADS) quantize_rows_kernel(const float* __restrict__ x, int K, QuantOut q) {
+    __shared__ float red[EW_THREADS / 32];
+    const int m = blockIdx.x;
+    const float* row = x + (size_t)m * K;
+    quantize_row(m, K, [&](int i) -> float { return row[i]; }, q, red);
+}
+
+// ---- K6: SwiGLU + quantize; gu = [M][2F] (gate | up); one CTA per token; F % 4 == 0 -------------
+__device__ __forceinline__ float swiglu_f(float g, float u) {
+    // t = (g / (1 + exp(-g))) * u, fp32 ops in this order; expf is the full-range libdevice one
+    return mul_rn(div_rn(g, add_rn(1.0f, expf(-g))), u);
+}
+__global__ void __launch_bounds__(EW_THREADS) swiglu_quant_kernel(const float* __restrict__ gu, int F, QuantOut q) {
+    __shared__ float red[EW_THREADS / 32];
+    const int m = blockIdx.x;
+    const float* g = gu + (size_t)m * 2 * F;
+    const float* u = g + F;
+    quantize_row(m, F, [&](int i) -> float { return swiglu_f(g[i], u[i]); }, q, red);
+}
+
+// ---- K4: RoPE (positions = L + depth) on q, k in place (fp32) + K,V -> bf16 pages ----------------
+struct RopeArgs {
+    float* qkv;           // [M][ld]; q heads, then k heads, then v heads
+    int ld, Hq, Hkv, D, T;
+    const int32_t* pos;   // [M]
+    const float2* cs;     // [max_pos][D/2] (cos, sin) built on the host in fp64
+    const int32_t* seq_slots;  // [B]
+    const int32_t* Lsnap;      // [B]
+    const int32_t* nn_eff;     // [B]
+    const int32_t* page_table; // [max_seqs][max_pages]
+    int max_pages, page_size;
+    __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D]
+};
+__global__ void __launch_bounds__(EW_THREADS) rope_kvwrite_kernel(RopeArgs a) {
+    const int m = blockIdx.x;
+    const int b = m / a.T, node = m % a.T;
+    const int D = a.D, D2 = D / 2;
+    float* row = a.qkv + (size_t)m * a.ld;
+    const float2* cs = a.cs + (size_t)a.pos[m] * D2;
+    const bool write = node < a.nn_eff[b];
+    __nv_bfloat16* kdst = nullptr;
+    __nv_bfloat16* vdst = nullptr;
+    if (write) {
+        const int slot_tok = a.Lsnap[b] + node;
+        const int page = a.page_table[(size_t)a.seq_slots[b] * a.max_pages + slot_tok / a.page_size];
+        const size_t base = (size_t)page * 2 * a.Hkv * a.page_size * D + (size_t)(slot_tok % a.page_size) * D;
+        kdst = a.pool + base;
+        vdst = a.pool + base + (size_t)a.Hkv * a.page_size * D;
+    }
+    const int n_rot = (a.Hq + a.Hkv) * D2;
+    for (int i = threadIdx.x; i < n_rot; i += EW_THREADS) {
+        const int head = i / D2, j = i % D2;
+        float* x = row + head * D;
+        const float2 c = cs[j];
+        const float lo = x[j], hi = x[j + D2];
+        const float rlo = sub_rn(mul_rn(lo, c.x), mul_rn(hi, c.y));
+        const float rhi = add_rn(mul_rn(hi, c.x), mul_rn(lo, c.y));
+        x[j] = rlo;
+        x[j + D2] = rhi;
+        if (head >= a.Hq && write) {
+            __nv_bfloat16* kd = kdst + (size_t)(head - a.Hq) * a.page_size * D;
+            kd[j] = __float2bfloat16_rn(rlo);
+            kd[j + D2] = __float2bfloat16_rn(rhi);
+        }
+    }
+    if (write) {
+        const float* v = row + (a.Hq + a.Hkv) * D;
+        for (int i = threadIdx.x; i < a.Hkv * D; i += EW_THREADS) {
+            const int head = i / D, j = i % D;
+            vdst[(size_t)head * a.page_size * D + j] = __float2bfloat16_rn(v[i]);
+        }
+    }
+}
+
+// ---- K8 finalize + K9 greedy acceptance walk + ctx_len update: one thread per sequence ---------
+struct AcceptArgs {
+    int B, T, commit, force_all;
+    const int32_t* tokens;
+    const int32_t* parents;
+    const int32_t* nn_eff;
+    const int32_t* status;
+    const int32_t* Lsnap;
+    const int32_t* seq_slots;
+    const unsigned long long* argmax_keys;  // [B*T] packed (ordered logit bits << 32 | ~index)
+    int32_t* argmax_out;                    // optional [B][T]
+    int32_t* accept_len;
+    int32_t* accept_nodes;
+    int32_t* out_tokens;
+    int32_t* new_ctx_len;
+    int32_t* ctx_len;                       // device state, advanced when commit
+};
+__global__ void accept_walk_kernel(AcceptArgs a) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= a.B) return;
+    const int T = a.T, nn = a.nn_eff[b], L = a.Lsnap[b];
+    const int32_t* tok = a.tokens + b * T;
+    const int32_t* par = a.parents + b * T;
+    int32_t* path = a.accept_nodes + b * T;
+    int32_t* out = a.out_tokens + b * T;
+    for (int i = 0; i < T; ++i) {
+        path[i] = -1;
+        out[i] = -1;
+        if (a.argmax_out) a.argmax_out[b * T + i] = (i < nn) ? (int32_t)(0xFFFFFFFFu - (uint32_t)a.argmax_keys[b * T + i]) : -1;
+    }
+    if (nn == 0) {  // rejected sequence
+        a.accept_len[b] = 0;
+        a.new_ctx_len[b] = L;
+        return;
+    }
+    int n_path = 1;
+    path[0] = 0;
+    if (a.force_all) {
+        for (int i = 1; i < nn; ++i) path[i] = i;
+        n_path = nn;
+    } else {
+        int cur = 0;
+        while (true) {
+            const int32_t want = (int32_t)(0xFFFFFFFFu - (uint32_t)a.argmax_keys[b * T + cur]);
+            int nxt = -1;
+            for (int c = cur + 1; c < nn; ++c)
+                if (par[c] == cur && tok[c] == want) { nxt = c; break; }
+            if (nxt < 0) break;
+            path[n_path++] = nxt;
+            cur = nxt;
+        }
+        for (int j = 1; j < n_path; ++j) out[j - 1] = tok[path[j]];
+        out[n_path - 1] = (int32_t)(0xFFFFFFFFu - (uint32_t)a.argmax_keys[b * T + cur]);
+    }
+    a.accept_len[b] = n_path - 1;
+    a.new_ctx_len[b] = L + n_path;
+    if (a.commit) a.ctx_len[a.seq_slots[b]] = L + n_path;
+}
+
+// ---- K10: KV compaction: slot L+path[j] -> slot L+j (j = 1..a), all layers, K and V -----------
+// sources are never overwritten before they are read (path[j] >= j, strictly increasing), so all
+// moves of a sequence run in parallel.  grid (B, n_layers).
+struct CompactArgs {
+    int T, Hkv, D, page_size, max_pages;
+    long layer_stride;  // elements per layer in the pool
+    __nv_bfloat16* pool;
+    const int32_t* page_table;
+    const int32_t* seq_slots;
+    const int32_t* Lsnap;
+    const int32_t* accept_len;
+    const int32_t* accept_nodes;
+};
+__global__ void __launch_bounds__(EW_THREADS) kv_compact_kernel(CompactArgs a) {
+    const int b = blockIdx.x, layer = blockIdx.y;
+    const int n = a.accept_len[b];
+    const int L = a.Lsnap[b];
+    const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+    __nv_bfloat16* pool = a.pool + (size_t)layer * a.layer_stride;
+    const int vec_per_head = a.D / 8;              // uint4 = 8 bf16
+    const int per_tok = 2 * a.Hkv * vec_per_head;  // K|V x heads
+    for (int j = 1; j <= n; ++j) {
+        const int src_node = a.accept_nodes[b * a.T + j];
+        if (src_node == j) continue;
+        const int ss = L + src_node, ds = L + j;
+        const size_t sbase = (size_t)pt[ss / a.page_size] * 2 * a.Hkv * a.page_size * a.D + (size_t)(ss % a.page_size) * a.D;
+        const size_t dbase = (size_t)pt[ds / a.page_size] * 2 * a.Hkv * a.page_size * a.D + (size_t)(ds % a.page_size) * a.D;
+        for (int i = threadIdx.x; i < per_tok; i += EW_THREADS) {
+            const int kvh = i / vec_per_head, c = i % vec_per_head;  // kvh in [0, 2*Hkv)
+            const size_t off = (size_t)kvh * a.page_size * a.D + (size_t)c * 8;
+            *reinterpret_cast<uint4*>(pool + dbase + off) = *reinterpret_cast<const uint4*>(pool + sbase + off);
+        }
+    }
+}
+
+// ---- dense <-> paged copies for export/import (one CTA per (token, layer)) ---------------------
+struct DenseCopyArgs {
+    int Hkv, D, page_size, n_tokens, layer_begin;
+    long layer_stride;
+    __nv_bfloat16* pool;
+    const int32_t* page_row;   // this sequence's page-table row
+    __nv_bfloat16* dense;      // [layer][2][Hkv][n_tokens][D]
+    int to_dense;
+};
+__global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
+    const int t = blockIdx.x, li = blockIdx.y;
+    __nv_bfloat16* pool = a.pool + (size_t)(a.layer_begin + li) * a.layer_stride;
+    const size_t pbase = (size_t)a.page_row[t / a.page_size] * 2 * a.Hkv * a.page_size * a.D + (size_t)(t % a.page_size) * a.D;
+    const int vec_per_head = a.D / 8;
+    for (int i = threadIdx.x; i < 2 * a.Hkv * vec_per_head; i += 128) {
+        const int kvh = i / vec_per_head, c = i % vec_per_head;
+        uint4* p = reinterpret_cast<uint4*>(pool + pbase + (size_t)kvh * a.page_size * a.D + (size_t)c * 8);
+        uint4* d = reinterpret_cast<uint4*>(a.dense + (((size_t)li * 2 * a.Hkv + kvh) * a.n_tokens + t) * a.D + (size_t)c * 8);
+        if (a.to_dense) *d = *p; else *p = *d;
+    }
+}
+
+__global__ void set_i32_kernel(int32_t* p, int32_t v) { *p = v; }
+
+// out[M][H] f32 copy (hidden taps)
+__global__ void __launch_bounds__(EW_THREADS) copy_f32_kernel(const float4* __restrict__ src, float4* __restrict__ dst, long n4) {
+    for (long i = blockIdx.x * (long)EW_THREADS + threadIdx.x; i < n4; i += (long)gridDim.x * EW_THREADS) dst[i] = src[i];
+}
+
+}  // namespace ev

@@ -1,0 +1,282 @@
+"""config[0]-scale parity of the whole verify step, CUDA path vs oracle (BASELINE.json:north_star
+tolerances): per-layer hidden rel-L2 <= 1e-2, logits max|d| <= 2e-2 * sigma(oracle logits), accepted
+tokens and KV-compaction indices bit-exact except where the oracle's top-2 gap < 1e-3."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import verify_oracle as vo
+from helpers import oracle_model, fresh_cache, rel_l2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+TOL_HIDDEN, TOL_LOGIT_SIGMA, GAP = 1e-2, 2e-2, 1e-3
+
+
+@pytest.fixture(scope="module")
+def setup():
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import gpu_model
+    spec = wl.CONFIGS[0]
+    gm = gpu_model(spec.model, spec.seed, max_batch=4, max_tree_nodes=64, max_ctx=512)
+    om = oracle_model(spec.model, spec.seed)
+    return spec, gm, om, ev
+
+
+def _oracle_ctx(om, ids, cap=256):
+    oc = fresh_cache(om, cap)
+    vo.prefill(om, oc, 0, ids)
+    return oc
+
+
+def _check_against_oracle(buf, res, T, sigma=None):
+    hid = buf.hidden.cpu().numpy()
+    for l, h_ref in enumerate(res["hidden"]):
+        assert rel_l2(hid[l, :T], h_ref) <= TOL_HIDDEN, (l, rel_l2(hid[l, :T], h_ref))
+    lg = buf.logits.cpu().numpy()[:T]
+    sigma = sigma or float(res["logits"].std())
+    assert np.max(np.abs(lg - res["logits"])) <= TOL_LOGIT_SIGMA * sigma
+    srt = np.sort(res["logits"], axis=1)
+    gap_ok = (srt[:, -1] - srt[:, -2]) >= GAP
+    am = buf.argmax.cpu().numpy().reshape(-1)[:T]
+    assert np.array_equal(am[gap_ok], res["argmax"][gap_ok])
+    return gap_ok
+
+
+def test_config0_verify_on_imported_oracle_kv(setup):
+    """form (a) of SURVEY 8(c)-6: context KV from the oracle's own prefill, imported."""
+    from gpu_helpers import import_oracle_kv, run_verify, export_kv_bits
+    spec, gm, om, ev = setup
+    ids = wl.context_ids(spec, 0, spec.ctx_len)
+    oc = _oracle_ctx(om, ids)
+    parents = wl.chain_parents(spec.n_nodes)
+    toks = wl.draft_tokens_uniform(spec, parents, 0)
+    cache = ev.Cache(gm, 64, 4)
+    slot = cache.ev_cache_add_seq(256)
+    import_oracle_kv(cache, slot, oc, 0, spec.ctx_len, spec.model.n_layers)
+    res = vo.verify(om, oc, 0, toks, parents, commit=True, want_hidden=True)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None], commit=True)
+    assert buf.status.cpu().tolist() == [0]
+    gap_ok = _check_against_oracle(buf, res, spec.n_nodes)
+    if gap_ok[res["path"]].all():
+        a = res["accept_len"]
+        assert buf.accept_len.cpu().tolist() == [a]
+        assert buf.accept_nodes.cpu().numpy()[0, :a + 1].tolist() == res["path"]
+        assert buf.out_tokens.cpu().numpy()[0, :a + 1].tolist() == res["out_tokens"]
+        assert buf.new_ctx_len.cpu().tolist() == [spec.ctx_len + a + 1]
+        assert cache.ev_cache_get_len(slot) == spec.ctx_len + a + 1
+        # appended + compacted KV equals the oracle's (bf16, allow 1 ulp on a few elements)
+        n = spec.ctx_len + a + 1
+        g = export_kv_bits(cache, slot, 0, spec.model.n_layers, n)
+        o = np.stack([oc.export_dense(l, 0, n) for l in range(spec.model.n_layers)])
+        diff = g.astype(np.int32) - o.astype(np.int32)
+        assert np.max(np.abs(diff)) <= 1 and np.count_nonzero(diff) <= 1e-3 * diff.size
+
+
+def test_config0_full_pipeline_gpu_prefill(setup):
+    """form (b): the GPU prefills the 128 context tokens itself."""
+    from gpu_helpers import run_verify, export_kv_bits
+    spec, gm, om, ev = setup
+    ids = wl.context_ids(spec, 0, spec.ctx_len)
+    oc = _oracle_ctx(om, ids)
+    cache = ev.Cache(gm, 64, 4)
+    slot = cache.ev_cache_add_seq(256)
+    cache.ev_cache_prefill([slot], [ids])
+    assert cache.ev_cache_get_len(slot) == spec.ctx_len
+    g = wl.bf16_bits_to_f32(export_kv_bits(cache, slot, 0, 2, spec.ctx_len))
+    o = wl.bf16_bits_to_f32(np.stack([oc.export_dense(l, 0, spec.ctx_len) for l in range(2)]))
+    assert rel_l2(g, o) <= 1e-2
+    parents = wl.chain_parents(spec.n_nodes)
+    toks = wl.draft_tokens_uniform(spec, parents, 0)
+    res = vo.verify(om, oc, 0, toks, parents, commit=False, want_hidden=True)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None])
+    _check_against_oracle(buf, res, spec.n_nodes)
+
+
+def test_per_kernel_taps_lock_step(setup):
+    """Each kernel of layer 1 checked on the GPU's own layer input: RMSNorm+quant codes, RoPE'd q/k/v,
+    attention output, O-proj residual, gate/up, SwiGLU+quant codes, layer output."""
+    from gpu_helpers import import_oracle_kv, run_verify
+    spec, gm, om, ev = setup
+    ids = wl.context_ids(spec, 0, 100)
+    oc = _oracle_ctx(om, ids)
+    parents = wl.tree_parents(26, (4, 3, 2, 2, 1))
+    toks = wl.draft_tokens_uniform(wl.CONFIGS[2], parents, 1) % spec.model.vocab
+    cache = ev.Cache(gm, 64, 4)
+    slot = cache.ev_cache_add_seq(256)
+    import_oracle_kv(cache, slot, oc, 0, 100, 2)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None], tap_layer=1)
+    h_in = buf.hidden.cpu().numpy()[1]
+    taps = {}
+    h_out = vo.layer_forward(om, 1, h_in, oc, 0, 100, parents, taps=taps)
+    t = {k: v.cpu().numpy() for k, v in buf.taps.items()}
+    assert np.array_equal(t["sx"], taps["sx"])
+    assert np.mean(t["xq"] != taps["xq"]) <= 1e-4
+    Hq, Hkv, d = 4, 2, 64
+    qkv = t["qkv"]
+    assert rel_l2(qkv[:, :Hq * d], taps["q"].reshape(26, -1)) <= 1e-5
+    assert rel_l2(qkv[:, Hq * d:(Hq + Hkv) * d], taps["k"].reshape(26, -1)) <= 1e-5
+    assert rel_l2(qkv[:, (Hq + Hkv) * d:], taps["v"].reshape(26, -1)) <= 1e-5
+    assert rel_l2(t["attn"], taps["attn"]) <= 2e-5, rel_l2(t["attn"], taps["attn"])
+    assert np.mean(t["aq"] != taps["aq"]) <= 2e-3
+    assert rel_l2(t["hmid"], taps["h_mid"]) <= 1e-3
+    gu_ref = np.concatenate([taps["g"], taps["u"]], axis=1)
+    assert rel_l2(t["gu"], gu_ref) <= 1e-2
+    assert rel_l2(buf.hidden.cpu().numpy()[2], h_out) <= 1e-2
+
+
+def test_trees_padding_batch_and_page_permutation(setup):
+    from gpu_helpers import import_oracle_kv, run_verify
+    spec, gm, om, ev = setup
+    V = spec.model.vocab
+    rng = np.random.default_rng(5)
+    ctxs = [37, 100, 16, 65]
+    trees = [wl.tree_parents(60, (4, 3, 2, 2, 1, 1)), wl.tree_parents(26, (4, 3, 2, 2, 1)), wl.chain_parents(4), wl.chain_parents(1)]
+    T = 60
+    cache = ev.Cache(gm, 80, 4)
+    perm = rng.permutation(80).tolist()
+    slots, ocs, toks_all, par_all, nn = [], [], np.zeros((4, T), np.int32), np.zeros((4, T), np.int32), []
+    for b, (L, p) in enumerate(zip(ctxs, trees)):
+        ids = rng.integers(0, V, L).astype(np.int32)
+        oc = _oracle_ctx(om, ids)
+        slot = cache.ev_cache_add_seq(L + T, pages=perm[b * 20:b * 20 + (L + T + 15) // 16])
+        import_oracle_kv(cache, slot, oc, 0, L, 2)
+        slots.append(slot)
+        ocs.append(oc)
+        n = len(p)
+        toks_all[b, :n] = rng.integers(0, V, n)
+        par_all[b, :n] = p
+        par_all[b, n:] = 0
+        nn.append(n)
+    buf = run_verify(gm, cache, slots, toks_all, par_all, n_nodes=nn, commit=True)
+    assert buf.status.cpu().tolist() == [0, 0, 0, 0]
+    hid = buf.hidden.cpu().numpy().reshape(3, 4, T, -1)
+    lg = buf.logits.cpu().numpy().reshape(4, T, -1)
+    for b in range(4):
+        n = nn[b]
+        res = vo.verify(om, ocs[b], 0, toks_all[b, :n], par_all[b, :n], commit=True, want_hidden=True)
+        for l in range(3):
+            assert rel_l2(hid[l, b, :n], res["hidden"][l]) <= TOL_HIDDEN
+        assert np.max(np.abs(lg[b, :n] - res["logits"])) <= TOL_LOGIT_SIGMA * res["logits"].std()
+        srt = np.sort(res["logits"], axis=1)
+        if ((srt[:, -1] - srt[:, -2]) >= GAP).all():
+            a = res["accept_len"]
+            assert buf.accept_len.cpu().numpy()[b] == a
+            assert buf.accept_nodes.cpu().numpy()[b, :a + 1].tolist() == res["path"]
+            assert buf.out_tokens.cpu().numpy()[b, :a + 1].tolist() == res["out_tokens"]
+            assert (buf.accept_nodes.cpu().numpy()[b, a + 1:] == -1).all()
+
+
+def test_acceptance_and_compaction_exactness_decoupled(setup):
+    """(ii) of the protocol: the oracle's walk on the GPU's own argmax reproduces the GPU's path, tokens and
+    lengths bit-exactly; (iii) the compacted cache equals the gather of the pre-compaction slots."""
+    from gpu_helpers import import_oracle_kv, run_verify, export_kv_bits
+    spec, gm, om, ev = setup
+    V = spec.model.vocab
+    rng = np.random.default_rng(9)
+    L = 50
+    ids = rng.integers(0, V, L).astype(np.int32)
+    oc = _oracle_ctx(om, ids)
+    parents = wl.tree_parents(26, (4, 3, 2, 2, 1))
+    # plant the oracle's greedy continuation on a non-first branch so that compaction moves slots
+    greedy = vo.decode_greedy(om, _oracle_ctx(om, ids), 0, 7, 5)
+    toks = rng.integers(0, V, 26).astype(np.int32)
+    toks[0] = 7
+    kids = lambda n: [c for c in range(26) if parents[c] == n]  # noqa: E731
+    cur = 0
+    for d in range(4):
+        ch = kids(cur)
+        if not ch:
+            break
+        pick = ch[-1]
+        toks[pick] = greedy[d]
+        cur = pick
+    cache = ev.Cache(gm, 64, 4)
+    slot = cache.ev_cache_add_seq(128)
+    import_oracle_kv(cache, slot, oc, 0, L, 2)
+    pre = run_verify(gm, cache, [slot], toks[None], parents[None], commit=False)
+    kv_pre = export_kv_bits(cache, slot, 0, 2, L + 26)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None], commit=True)
+    am = buf.argmax.cpu().numpy()[0]
+    path, out = vo.accept_walk(toks, parents, am)
+    a = len(path) - 1
+    assert a >= 2, "planted branch should be accepted"
+    assert buf.accept_len.cpu().tolist() == [a]
+    assert buf.accept_nodes.cpu().numpy()[0, :a + 1].tolist() == path
+    assert buf.out_tokens.cpu().numpy()[0, :a + 1].tolist() == out
+    assert path != list(range(a + 1)), "compaction must actually move slots in this test"
+    kv_post = export_kv_bits(cache, slot, 0, 2, L + a + 1)
+    assert np.array_equal(kv_post[:, :, :, :L], kv_pre[:, :, :, :L])
+    assert np.array_equal(kv_post[:, :, :, L:], kv_pre[:, :, :, [L + p for p in path]])
+    assert np.array_equal(pre.argmax.cpu().numpy(), buf.argmax.cpu().numpy())
+
+
+def test_status_codes_and_rejected_sequences(setup):
+    from gpu_helpers import run_verify
+    spec, gm, om, ev = setup
+    cache = ev.Cache(gm, 16, 4)
+    s0 = cache.ev_cache_add_seq(32)
+    s1 = cache.ev_cache_add_seq(32)
+    s2 = cache.ev_cache_add_seq(16)
+    cache.ev_cache_set_len(s2, 14)           # 14 + 4 > 16 -> over capacity
+    toks = np.array([[1, 2, 3, 4], [1, 2, 5000, 4], [1, 2, 3, 4], [1, 2, 3, 4]], dtype=np.int32)
+    par = np.array([[-1, 0, 1, 2], [-1, 0, 1, 2], [-1, 0, 1, 2], [-1, 0, 3, 1]], dtype=np.int32)
+    buf = run_verify(gm, cache, [s0, s1, s2, s0], toks, par, commit=False)
+    st = buf.status.cpu().tolist()
+    assert st[0] == 0 and st[1] & 2 and st[2] & 4 and st[3] & 1
+    assert buf.accept_len.cpu().tolist()[1:] == [0, 0, 0]
+    assert np.isfinite(buf.logits.cpu().numpy()[:4]).all()
+    # host-detectable errors
+    import paper_2606_18502_b200 as evm
+    big = evm.VerifyBuffers(gm, 5, 4)
+    with pytest.raises(evm.EvError) as e:
+        evm.ev_verify(gm, cache, big)
+    assert e.value.code == -3
+    with pytest.raises(evm.EvError):
+        cache.ev_cache_add_seq(100000)
+
+
+def test_gpu_speculative_loop_is_lossless_vs_oracle_greedy(setup):
+    """PAPER.md:92 on the GPU: the multi-step speculative loop (planted + random drafts) emits the oracle's
+    greedy sequence; positions after a sub-1e-3 top-2 gap are void."""
+    from gpu_helpers import import_oracle_kv, run_verify
+    spec, gm, om, ev = setup
+    V = spec.model.vocab
+    rng = np.random.default_rng(21)
+    L, n_tok = 40, 24
+    ids = rng.integers(0, V, L).astype(np.int32)
+    oc = _oracle_ctx(om, ids, cap=128)
+    # oracle greedy + its top-2 gaps
+    greedy, gaps, tok = [], [], 11
+    for _ in range(n_tok):
+        lg, _ = vo.forward_tree(om, oc, 0, np.array([tok]), np.array([-1]))
+        oc.ctx_len[0] += 1
+        s = np.sort(lg[0])
+        gaps.append(s[-1] - s[-2])
+        tok = int(np.argmax(lg[0]))
+        greedy.append(tok)
+    first_void = next((i for i, g in enumerate(gaps) if g < GAP), n_tok)
+    cache = ev.Cache(gm, 64, 4)
+    slot = cache.ev_cache_add_seq(128)
+    import_oracle_kv(cache, slot, _oracle_ctx(om, ids), 0, L, 2)
+    parents = wl.tree_parents(12, (3, 2, 2))
+    emitted, root, steps = [], 11, 0
+    buf = ev.VerifyBuffers(gm, 1, 12, want_logits=False, want_hidden=False)
+    while len(emitted) < n_tok:
+        toks = rng.integers(0, V, 12).astype(np.int32)
+        toks[0] = root
+        cur, pos = 0, len(emitted)
+        for c in range(1, 12):          # plant the true continuation down the first-child chain
+            if parents[c] == cur and pos < n_tok and rng.random() < 0.8:
+                toks[c] = greedy[pos]
+                cur, pos = c, pos + 1
+        run_verify(gm, cache, [slot], toks[None], parents[None], commit=True, buf=buf)
+        a = int(buf.accept_len.cpu()[0])
+        out = buf.out_tokens.cpu().numpy()[0, :a + 1].tolist()
+        emitted += out
+        root = out[-1]
+        steps += 1
+    n = min(first_void, n_tok)
+    assert emitted[:n] == greedy[:n]
+    assert steps < n_tok, "speculation should accept drafts"
