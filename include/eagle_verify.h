@@ -150,6 +150,8 @@ int ev_cache_import_seq(ev_cache*, int seq_slot, int layer_begin, int layer_end,
  * set: enqueued on the stream.  get: synchronises the stream. */
 int ev_cache_set_len(ev_cache*, int seq_slot, int ctx_len, void* stream);
 int ev_cache_get_len(ev_cache*, int seq_slot, int* ctx_len, void* stream);
+/* Sets the ctx_len of up to 64 sequences with one launch (rewinds a batch between timed steps). */
+int ev_cache_set_lens(ev_cache*, int n, const int* host_slots, const int* host_lens, void* stream);
 int ev_cache_destroy(ev_cache*);
 
 /* ---- verify --------------------------------------------------------------------------------- */
@@ -196,6 +198,15 @@ typedef struct {
  * (weights missing / not calibrated in static mode), EV_ECUDA (launch failure). */
 int ev_verify(ev_model*, ev_cache*, const ev_verify_in*, ev_verify_out*, void* stream);
 
+/* The same step with HOST buffers: copies tokens/parents/slots (and n_nodes, may be NULL) to the device,
+ * runs ev_verify, copies the five result arrays back ([B] or [B][n_nodes] int32) and synchronises the
+ * stream.  Host buffers should be pinned for the copies to be asynchronous.  This is the end-to-end
+ * call bench.py times. */
+int ev_verify_host(ev_model*, ev_cache*, int n_seqs, int n_nodes, const int32_t* host_seq_slots,
+                   const int32_t* host_tokens, const int32_t* host_parents, const int32_t* host_n_nodes,
+                   int commit, int32_t* host_accept_len, int32_t* host_accept_nodes,
+                   int32_t* host_out_tokens, int32_t* host_new_ctx_len, int32_t* host_status, void* stream);
+
 /* ---- single operators (per-kernel parity tests; same kernels the step uses) ------------------ */
 
 /* y[M][N] = (codes_x . W_kind^T) * s_x[m] * s_w[n] with the product GEMM kernel. */
@@ -206,6 +217,12 @@ int ev_op_quantize_rows(ev_model*, const float* dev_x, int M, int K, float stati
                         uint8_t* dev_codes, float* dev_sx, void* stream);
 
 /* ---- introspection ---------------------------------------------------------------------------- */
+/* Device timing per kernel class with CUDA events recorded on the launching stream around each
+ * launch (classes: 0 FP8 GEMM, 1 tree attention, 2 attention merge+quant, 3 RMSNorm+quant,
+ * 4 RoPE+KV write, 5 SwiGLU+quant, 6 other).  enable(1) starts recording; read() synchronises the
+ * device, sums elapsed ms and launch counts per class into the host arrays and clears the record. */
+int ev_profile_enable(ev_model*, int on);
+int ev_profile_read(ev_model*, double* host_ms_by_class, long* host_count_by_class, int n_classes);
 const char* ev_last_error(void);
 /* kernels launched by the calling thread's library calls since the last reset */
 long ev_launch_count(int reset);

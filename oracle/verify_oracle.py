@@ -28,6 +28,9 @@ Pins: tests/test_oracle_*.py.  End-to-end logits of th
 random model have no external truth: "parity unpinned" for that single item, everything it is
 composed of is pinned on small shapes.
 """
+import os
+from concurrent.futures import ThreadPoolExecutor
+
 import numpy as np
 
 from . import e4m3
@@ -38,6 +41,7 @@ except Exception:  # pragma: no cover
     _torch = None
 
 F32 = np.float32
+_N_THREADS = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
 _LUT64 = e4m3.decode_table()
 
 
@@ -74,12 +78,22 @@ def quantize_weight(w_bf16_bits):
     BASELINE.json:configs[0] "E4M3 per-output-channel absmax scales"; PAPER.md:98 "min-max".
     s_w[n] = max_k |W[n,k]| / 448 (fp32 IEEE division; 1 for an all-zero row);
     Wq[n,k] = encode(W[n,k] / s_w[n]) (fp32 IEEE division).  DESIGN.md R-quant."""
-    w = bf16_bits_to_f32(w_bf16_bits)
-    amax = np.max(np.abs(w), axis=1).astype(F32)
-    s = (amax / F32(448.0)).astype(F32)
-    s = np.where(amax == 0, F32(1.0), s).astype(F32)
-    codes = e4m3.encode((w / s[:, None]).astype(F32))
-    return codes, s
+    def rows(block):
+        w = bf16_bits_to_f32(block)
+        amax = np.max(np.abs(w), axis=1).astype(F32)
+        s = (amax / F32(448.0)).astype(F32)
+        s = np.where(amax == 0, F32(1.0), s).astype(F32)
+        return e4m3.encode((w / s[:, None]).astype(F32)), s
+
+    w_bf16_bits = np.asarray(w_bf16_bits)
+    n = w_bf16_bits.shape[0]
+    if w_bf16_bits.size < (1 << 22):
+        return rows(w_bf16_bits)
+    # rows are independent: big matrices go through a thread pool in row blocks (same arithmetic)
+    step = max(1, (1 << 21) // w_bf16_bits.shape[1])
+    with ThreadPoolExecutor(max_workers=_N_THREADS) as ex:
+        parts = list(ex.map(lambda r0: rows(w_bf16_bits[r0:r0 + step]), range(0, n, step)))
+    return np.concatenate([p[0] for p in parts]), np.concatenate([p[1] for p in parts])
 
 
 def quantize_rows(x, static_scale=None):

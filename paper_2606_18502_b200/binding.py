@@ -62,9 +62,13 @@ SIGNATURES = {
     "ev_cache_export_seq": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, C.c_int, _P, _P]),
     "ev_cache_import_seq": (C.c_int, [_P, C.c_int, C.c_int, C.c_int, C.c_int, _P, C.c_int, _P]),
     "ev_cache_set_len": (C.c_int, [_P, C.c_int, C.c_int, _P]),
+    "ev_cache_set_lens": (C.c_int, [_P, C.c_int, _P, _P, _P]),
     "ev_cache_get_len": (C.c_int, [_P, C.c_int, C.POINTER(C.c_int), _P]),
     "ev_cache_destroy": (C.c_int, [_P]),
     "ev_verify": (C.c_int, [_P, _P, C.POINTER(ev_verify_in), C.POINTER(ev_verify_out), _P]),
+    "ev_verify_host": (C.c_int, [_P, _P, C.c_int, C.c_int, _P, _P, _P, _P, C.c_int, _P, _P, _P, _P, _P, _P]),
+    "ev_profile_enable": (C.c_int, [_P, C.c_int]),
+    "ev_profile_read": (C.c_int, [_P, _P, _P, C.c_int]),
     "ev_op_linear": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
     "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
     "ev_last_error": (C.c_char_p, []),
@@ -191,6 +195,19 @@ class Model:
                                             _stream()))
         return codes, sx
 
+    PROFILE_CLASSES = ("gemm_fp8", "tree_attention", "attn_merge_quant", "rmsnorm_quant", "rope_kvwrite", "swiglu_quant", "other")
+
+    def ev_profile_enable(self, on=True):
+        _check(self.lib.ev_profile_enable(self.h, 1 if on else 0))
+
+    def ev_profile_read(self):
+        """-> {class: (total_ms, launches)} since enable / the last read."""
+        n = len(self.PROFILE_CLASSES)
+        ms = (C.c_double * n)()
+        cnt = (C.c_long * n)()
+        _check(self.lib.ev_profile_read(self.h, ms, cnt, n))
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(self.PROFILE_CLASSES)}
+
     def ev_model_destroy(self):
         if self.h:
             self.lib.ev_model_destroy(self.h)
@@ -250,6 +267,10 @@ class Cache:
 
     def ev_cache_set_len(self, slot, n):
         _check(self.lib.ev_cache_set_len(self.h, slot, n, _stream()))
+
+    def ev_cache_set_lens(self, slots, lens):
+        n = len(slots)
+        _check(self.lib.ev_cache_set_lens(self.h, n, (C.c_int * n)(*slots), (C.c_int * n)(*lens), _stream()))
 
     def ev_cache_get_len(self, slot):
         v = C.c_int(0)
@@ -327,3 +348,14 @@ def ev_verify(model, cache, buf, commit=True, use_n_nodes=True, override_first_o
                          buf.hidden.data_ptr() if buf.hidden is not None else None, buf.tap_layer,
                          g("xq"), g("sx"), g("qkv"), g("attn"), g("aq"), g("sa"), g("hmid"), g("gu"), g("tq"), g("st"))
     _check(model.lib.ev_verify(model.h, cache.h, C.byref(vin), C.byref(vout), _stream()))
+
+
+def ev_verify_host(model, cache, host, commit=True):
+    """End-to-end step with HOST (pinned) int32 tensors: host = dict(seq_slots[B], tokens[B,T], parents[B,T],
+    n_nodes[B] or None, accept_len[B], accept_nodes[B,T], out_tokens[B,T], new_ctx_len[B], status[B]).
+    Copies in, verifies, copies out, synchronises."""
+    B, T = host["tokens"].shape
+    p = lambda k: C.c_void_p(host[k].data_ptr()) if host.get(k) is not None else None  # noqa: E731
+    _check(model.lib.ev_verify_host(model.h, cache.h, B, T, p("seq_slots"), p("tokens"), p("parents"), p("n_nodes"),
+                                    1 if commit else 0, p("accept_len"), p("accept_nodes"), p("out_tokens"),
+                                    p("new_ctx_len"), p("status"), _stream()))

@@ -103,6 +103,9 @@ struct LayerW {
 
 long round_up(long x, long m) { return (x + m - 1) / m * m; }
 
+enum ProfClass { PC_GEMM = 0, PC_ATTN, PC_ATTN_MERGE, PC_NORM_QUANT, PC_ROPE_KV, PC_SWIGLU, PC_OTHER, PC_COUNT };
+struct ProfRec { cudaEvent_t a, b; int cls; };
+
 }  // namespace
 
 struct ev_model {
@@ -135,6 +138,9 @@ struct ev_model {
     bool calibrated = false, recording = false;
     int num_sms = 148;
     bool use_splitk = false, naive_gemm = false;
+    bool profile = false;
+    std::vector<ProfRec> prof;
+    size_t prof_used = 0;
     std::vector<void*> allocs;
 };
 
@@ -157,6 +163,23 @@ struct ev_cache {
 };
 
 namespace {
+
+// records a CUDA-event pair around the launches issued in its scope when profiling is on
+struct ProfScope {
+    ev_model* m; cudaStream_t st; ProfRec* r = nullptr;
+    ProfScope(ev_model* m_, cudaStream_t st_, int cls) : m(m_), st(st_) {
+        if (!m->profile) return;
+        if (m->prof_used == m->prof.size()) {
+            ProfRec n;
+            cudaEventCreate(&n.a); cudaEventCreate(&n.b);
+            m->prof.push_back(n);
+        }
+        r = &m->prof[m->prof_used++];
+        r->cls = cls;
+        cudaEventRecord(r->a, st);
+    }
+    ~ProfScope() { if (r) cudaEventRecord(r->b, st); }
+};
 
 template <class T>
 int dev_alloc(ev_model* m, T** p, size_t count) {
@@ -217,6 +240,7 @@ int launch_gemm_epi(cudaStream_t st, const CUtensorMap& tmW, const ActBuf& x, co
 // y = x . W^T with scales; epi: EPI_STORE / EPI_RESID (in place on out) / EPI_ARGMAX
 int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, float* out, int ldo,
                unsigned long long* keys) {
+    ProfScope prof_scope(m, st, PC_GEMM);
     GemmArgs a;
     a.M = M; a.N = (int)w.N; a.K = (int)w.K;
     a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
@@ -270,7 +294,7 @@ int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
 
 template <int D>
 int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
-    constexpr int smem = 2 * 2 * ATT_CH * D * 2;
+    constexpr int smem = 2 * 2 * ATT_CH * D * 2 + ATT_WARPS * 3 * 16 * D * 2;
     static bool attr_set = false;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(tree_attn_partial_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -333,8 +357,11 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         const bool tap = (out->tap_layer == l);
         if (ovr && !in->override_first_only && l > 0) EV_TRY(copy_f32(st, ovr + (size_t)l * M * H, m->h, (long)M * H));
         // --- attention block ---
-        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
-        LAUNCH_CHECK();
+        {
+            ProfScope ps(m, st, PC_NORM_QUANT);
+            rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
+            LAUNCH_CHECK();
+        }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sx) EV_TRY(copy_f32(st, m->xq.scale, out->dev_tap_sx, M));
         EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_STORE, m->qkv, m->qkv_dim, nullptr));
@@ -343,8 +370,11 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
         ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
         ra.pool = c->pool + (size_t)l * c->layer_stride;
-        rope_kvwrite_kernel<<<M, EW_THREADS, 0, st>>>(ra);
-        LAUNCH_CHECK();
+        {
+            ProfScope ps(m, st, PC_ROPE_KV);
+            rope_kvwrite_kernel<<<M, EW_THREADS, 0, st>>>(ra);
+            LAUNCH_CHECK();
+        }
         if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
         AttnArgs aa;
         aa.q = m->qkv; aa.q_ld = m->qkv_dim; aa.T = T; aa.G = cfg.n_q_heads / cfg.n_kv_heads; aa.Hq = cfg.n_q_heads;
@@ -353,25 +383,37 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         aa.anc = m->anc; aa.split_len = split_len; aa.n_splits = n_splits; aa.scale = 1.0f / sqrtf((float)D);
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
         dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
-        if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
+        {
+            ProfScope ps(m, st, PC_ATTN);
+            if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
+        }
         MergeArgs ma;
         ma.T = T; ma.Hq = cfg.n_q_heads; ma.D = D; ma.n_splits = n_splits; ma.split_len = split_len;
         ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part; ma.attn = m->attn;
         ma.q = quant_out(m, m->aq, 4 * l + 1);
-        attn_merge_quant_kernel<<<M, EW_THREADS, 0, st>>>(ma);
-        LAUNCH_CHECK();
+        {
+            ProfScope ps(m, st, PC_ATTN_MERGE);
+            attn_merge_quant_kernel<<<M, EW_THREADS, 0, st>>>(ma);
+            LAUNCH_CHECK();
+        }
         if (tap && out->dev_tap_attn) EV_TRY(copy_f32(st, m->attn, out->dev_tap_attn, (long)M * m->q_dim));
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
         EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RESID, m->h, H, nullptr));
         if (tap && out->dev_tap_hmid) EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H));
         // --- MLP block ---
-        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
-        LAUNCH_CHECK();
+        {
+            ProfScope ps(m, st, PC_NORM_QUANT);
+            rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
+            LAUNCH_CHECK();
+        }
         EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_STORE, m->gu, 2 * F, nullptr));
         if (tap && out->dev_tap_gu) EV_TRY(copy_f32(st, m->gu, out->dev_tap_gu, (long)M * 2 * F));
-        swiglu_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->gu, F, quant_out(m, m->tq, 4 * l + 3));
-        LAUNCH_CHECK();
+        {
+            ProfScope ps(m, st, PC_SWIGLU);
+            swiglu_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->gu, F, quant_out(m, m->tq, 4 * l + 3));
+            LAUNCH_CHECK();
+        }
         if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
         EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RESID, m->h, H, nullptr));
@@ -516,6 +558,7 @@ int ev_model_destroy(ev_model* m) {
     if (!m) return EV_OK;
     cudaDeviceSynchronize();
     for (void* p : m->allocs) cudaFree(p);
+    for (auto& r : m->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     delete m;
     return EV_OK;
 }
@@ -705,6 +748,21 @@ int ev_cache_set_len(ev_cache* c, int slot, int ctx_len, void* stream) {
     set_i32_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(c->ctx_len + slot, ctx_len);
     LAUNCH_CHECK();
     c->len_bound[slot] = ctx_len;
+    return EV_OK;
+}
+int ev_cache_set_lens(ev_cache* c, int n, const int* host_slots, const int* host_lens, void* stream) {
+    if (!c || !host_slots || !host_lens || n < 1 || n > c->model->cfg.max_batch) return fail(EV_EINVAL, "bad argument");
+    for (int i = 0; i < n; ++i) {
+        const int s = host_slots[i];
+        if (s < 0 || s >= c->max_seqs || !c->seq_used[s] || host_lens[i] < 0) return fail(EV_EINVAL, "bad slot or length");
+        if (host_lens[i] > (int)c->seq_pages[s].size() * c->model->cfg.page_size) return fail(EV_ECAPACITY, "ctx_len exceeds capacity");
+    }
+    SetLensArgs a;
+    if (n > SetLensArgs::MAX) return fail(EV_EINVAL, "at most 64 sequences per call");
+    a.n = n;
+    for (int i = 0; i < n; ++i) { a.slot[i] = host_slots[i]; a.len[i] = host_lens[i]; c->len_bound[host_slots[i]] = host_lens[i]; }
+    set_lens_kernel<<<1, 64, 0, (cudaStream_t)stream>>>(c->ctx_len, a);
+    LAUNCH_CHECK();
     return EV_OK;
 }
 int ev_cache_get_len(ev_cache* c, int slot, int* ctx_len, void* stream) {
@@ -907,6 +965,65 @@ int ev_op_linear(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, c
         return run_linear(m, st, *w, *x, M, EPI_ARGMAX, dev_out, (int)w->N, m->argmax_keys);
     }
     return run_linear(m, st, *w, *x, M, EPI_STORE, dev_out, (int)w->N, nullptr);
+}
+
+
+// ---- host-buffer entry point: copies in, one verify step, copies out, synchronises ---------------------
+int ev_verify_host(ev_model* m, ev_cache* c, int n_seqs, int n_nodes, const int32_t* host_seq_slots,
+                   const int32_t* host_tokens, const int32_t* host_parents, const int32_t* host_n_nodes, int commit,
+                   int32_t* host_accept_len, int32_t* host_accept_nodes, int32_t* host_out_tokens,
+                   int32_t* host_new_ctx_len, int32_t* host_status, void* stream) {
+    if (!m || !c || !host_seq_slots || !host_tokens || !host_parents || !host_accept_len || !host_accept_nodes ||
+        !host_out_tokens || !host_new_ctx_len || !host_status)
+        return fail(EV_EINVAL, "null argument");
+    if (n_seqs < 1 || n_nodes < 1) return fail(EV_EINVAL, "n_seqs and n_nodes must be positive");
+    if (n_seqs > m->cfg.max_batch || n_nodes > m->cfg.max_tree_nodes) return fail(EV_ECAPACITY, "batch or tree too large");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t BT = (size_t)n_seqs * n_nodes;
+    CUDA_TRY(cudaMemcpyAsync(c->pf_tokens, host_tokens, BT * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(c->pf_parents, host_parents, BT * 4, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(c->pf_slots, host_seq_slots, (size_t)n_seqs * 4, cudaMemcpyHostToDevice, st));
+    if (host_n_nodes) CUDA_TRY(cudaMemcpyAsync(c->pf_nn, host_n_nodes, (size_t)n_seqs * 4, cudaMemcpyHostToDevice, st));
+    const int Bmax = m->cfg.max_batch;
+    ev_verify_in in;
+    memset(&in, 0, sizeof(in));
+    in.n_seqs = n_seqs; in.n_nodes_max = n_nodes; in.dev_seq_slots = c->pf_slots; in.dev_tokens = c->pf_tokens;
+    in.dev_parents = c->pf_parents; in.dev_n_nodes = host_n_nodes ? c->pf_nn : nullptr; in.commit = commit;
+    ev_verify_out o;
+    memset(&o, 0, sizeof(o));
+    o.tap_layer = -1;
+    o.dev_accept_len = c->pf_out; o.dev_new_ctx_len = c->pf_out + Bmax; o.dev_status = c->pf_out + 2 * Bmax;
+    o.dev_accept_nodes = c->pf_out + 3 * Bmax; o.dev_out_tokens = o.dev_accept_nodes + (size_t)m->M_cap;
+    EV_TRY(ev_verify(m, c, &in, &o, stream));
+    CUDA_TRY(cudaMemcpyAsync(host_accept_len, o.dev_accept_len, (size_t)n_seqs * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(host_new_ctx_len, o.dev_new_ctx_len, (size_t)n_seqs * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(host_status, o.dev_status, (size_t)n_seqs * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(host_accept_nodes, o.dev_accept_nodes, BT * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(host_out_tokens, o.dev_out_tokens, BT * 4, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return EV_OK;
+}
+
+// ---- per-kernel-class device timing (CUDA events on the launching stream) ----------------------------------
+int ev_profile_enable(ev_model* m, int on) {
+    if (!m) return fail(EV_EINVAL, "null argument");
+    m->profile = on != 0;
+    m->prof_used = 0;
+    return EV_OK;
+}
+int ev_profile_read(ev_model* m, double* host_ms_by_class, long* host_count_by_class, int n_classes) {
+    if (!m || !host_ms_by_class || !host_count_by_class || n_classes < 1) return fail(EV_EINVAL, "bad argument");
+    for (int i = 0; i < n_classes; ++i) { host_ms_by_class[i] = 0.0; host_count_by_class[i] = 0; }
+    CUDA_TRY(cudaDeviceSynchronize());
+    for (size_t i = 0; i < m->prof_used; ++i) {
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, m->prof[i].a, m->prof[i].b));
+        const int c = m->prof[i].cls < n_classes ? m->prof[i].cls : n_classes - 1;
+        host_ms_by_class[c] += ms;
+        host_count_by_class[c] += 1;
+    }
+    m->prof_used = 0;
+    return EV_OK;
 }
 
 }  // extern "C"

@@ -9,7 +9,9 @@
 // of anc[i]).  Pages are gathered with 16-byte cp.async into XOR-swizzled shared memory (each
 // (page, K|V, head) block is page_size*D*2 contiguous bytes), double buffered; Q.K^T and P.V run on
 // the tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with Q and P each split into
-// hi + lo bf16 parts so that ~16 mantissa bits survive (DESIGN.md section 6 "attention precision");
+// hi + mid + lo bf16 parts: 3 x 8 significand bits represent an fp32 value exactly, K and V are bf16
+// already, so every product is exact and only the fp32 accumulation rounds (DESIGN.md section 6
+// "attention precision": a 2-way split left 2^-17 errors that flip E4M3 codes downstream);
 // the online softmax is done in fp32 registers with warp shuffles across the 4 lanes of a row.
 #pragma once
 #include "ev_common.cuh"
@@ -61,6 +63,17 @@ __device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_
     hi = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
     lo = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
 }
+// x = hi + mid + lo exactly (8 + 8 + 8 significand bits)
+__device__ __forceinline__ void split3(float x0, float x1, uint32_t& hi, uint32_t& mid, uint32_t& lo) {
+    const __nv_bfloat16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
+    const float r0 = x0 - __bfloat162float(h0), r1 = x1 - __bfloat162float(h1);
+    const __nv_bfloat16 m0 = __float2bfloat16_rn(r0), m1 = __float2bfloat16_rn(r1);
+    const __nv_bfloat16 l0 = __float2bfloat16_rn(r0 - __bfloat162float(m0));
+    const __nv_bfloat16 l1 = __float2bfloat16_rn(r1 - __bfloat162float(m1));
+    hi = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
+    mid = (uint32_t)__bfloat16_as_ushort(m0) | ((uint32_t)__bfloat16_as_ushort(m1) << 16);
+    lo = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
+}
 __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsrc, bool valid) {
     const int sz = valid ? 16 : 0;
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(sz) : "memory");
@@ -72,7 +85,8 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     constexpr int CPR = ROWB / 16;        // 16-byte chunks per row
     constexpr int TILE = ATT_CH * ROWB;   // bytes per K (or V) tile
     constexpr int KT = D / 16;            // k-tiles of the Q.K^T contraction
-    extern __shared__ __align__(128) uint8_t att_smem[];  // [2 stages][K tile | V tile]
+    constexpr int QTILE = 16 * ROWB;      // one warp's 16 query rows, one bf16 part
+    extern __shared__ __align__(128) uint8_t att_smem[];  // [2 stages][K tile | V tile] [warp][hi|mid|lo][16 rows]
 
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
@@ -96,23 +110,31 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     const bool v0 = active && row0 < R && node0 < nn, v1 = active && row1 < R && node1 < nn;
     const unsigned long long anc0 = v0 ? a.anc[b * a.T + node0] : 0ull, anc1 = v1 ? a.anc[b * a.T + node1] : 0ull;
 
-    // ---- Q fragments (A operand), split hi/lo ----
-    uint32_t qhi[KT][4], qlo[KT][4];
+    // ---- Q rows -> this warp's shared-memory tiles, split hi/mid/lo (A operand, read by ldmatrix) ----
+    const uint32_t qs = smem_u32(att_smem + 4 * TILE + warp * 3 * QTILE);
     {
+        uint8_t* qsp = att_smem + 4 * TILE + warp * 3 * QTILE;
         const float* q0 = a.q + (size_t)(b * a.T + (v0 ? node0 : 0)) * a.q_ld + (size_t)(kvh * a.G + (v0 ? g0 : 0)) * D;
         const float* q1 = a.q + (size_t)(b * a.T + (v1 ? node1 : 0)) * a.q_ld + (size_t)(kvh * a.G + (v1 ? g1 : 0)) * D;
+        const int r0 = lane >> 2, r1 = r0 + 8;
 #pragma unroll
-        for (int kt = 0; kt < KT; ++kt) {
-            const int c = kt * 16 + (lane & 3) * 2;
-            float2 x00 = v0 ? *reinterpret_cast<const float2*>(q0 + c) : make_float2(0.f, 0.f);
-            float2 x10 = v1 ? *reinterpret_cast<const float2*>(q1 + c) : make_float2(0.f, 0.f);
-            float2 x01 = v0 ? *reinterpret_cast<const float2*>(q0 + c + 8) : make_float2(0.f, 0.f);
-            float2 x11 = v1 ? *reinterpret_cast<const float2*>(q1 + c + 8) : make_float2(0.f, 0.f);
-            split2(x00.x, x00.y, qhi[kt][0], qlo[kt][0]);
-            split2(x10.x, x10.y, qhi[kt][1], qlo[kt][1]);
-            split2(x01.x, x01.y, qhi[kt][2], qlo[kt][2]);
-            split2(x11.x, x11.y, qhi[kt][3], qlo[kt][3]);
+        for (int c8 = 0; c8 < D / 8; ++c8) {
+            const int c = c8 * 8 + (lane & 3) * 2;
+            const float2 x0 = v0 ? *reinterpret_cast<const float2*>(q0 + c) : make_float2(0.f, 0.f);
+            const float2 x1 = v1 ? *reinterpret_cast<const float2*>(q1 + c) : make_float2(0.f, 0.f);
+            uint32_t h, md, l;
+            split3(x0.x, x0.y, h, md, l);
+            const int o0 = r0 * ROWB + ((c8 ^ (r0 & 7)) * 16) + (lane & 3) * 4;
+            *reinterpret_cast<uint32_t*>(qsp + o0) = h;
+            *reinterpret_cast<uint32_t*>(qsp + QTILE + o0) = md;
+            *reinterpret_cast<uint32_t*>(qsp + 2 * QTILE + o0) = l;
+            split3(x1.x, x1.y, h, md, l);
+            const int o1 = r1 * ROWB + ((c8 ^ (r1 & 7)) * 16) + (lane & 3) * 4;
+            *reinterpret_cast<uint32_t*>(qsp + o1) = h;
+            *reinterpret_cast<uint32_t*>(qsp + QTILE + o1) = md;
+            *reinterpret_cast<uint32_t*>(qsp + 2 * QTILE + o1) = l;
         }
+        __syncwarp();
     }
 
     // ---- page gather: chunk ch -> stage ----
@@ -156,18 +178,32 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
             // ---- S = Q K^T (16 rows x 64 keys per warp) ----
             float s[ATT_CH / 8][4];
 #pragma unroll
-            for (int nt = 0; nt < ATT_CH / 8; ++nt) {
-                s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
-                const int r = nt * 8 + (lane & 7);
+            for (int nt = 0; nt < ATT_CH / 8; ++nt) s[nt][0] = s[nt][1] = s[nt][2] = s[nt][3] = 0.f;
 #pragma unroll
-                for (int kp = 0; kp < KT / 2; ++kp) {
+            for (int kp = 0; kp < KT / 2; ++kp) {
+                uint32_t qa[2][3][4];  // [k-tile of the pair][hi|mid|lo][A fragment]
+                {
+                    const int r = ((lane >> 3) & 1) * 8 + (lane & 7);
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        const int c = (2 * kp + t) * 2 + (lane >> 4);
+                        const uint32_t ad = qs + r * ROWB + ((c ^ (r & 7)) * 16);
+#pragma unroll
+                        for (int part = 0; part < 3; ++part)
+                            ldsm_x4(ad + part * QTILE, qa[t][part][0], qa[t][part][1], qa[t][part][2], qa[t][part][3]);
+                    }
+                }
+#pragma unroll
+                for (int nt = 0; nt < ATT_CH / 8; ++nt) {
+                    const int r = nt * 8 + (lane & 7);
                     const int c = kp * 4 + (lane >> 3);
                     uint32_t b0, b1, b2, b3;
                     ldsm_x4(ks + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
-                    mma_bf16(s[nt], qhi[2 * kp], b0, b1);
-                    mma_bf16(s[nt], qlo[2 * kp], b0, b1);
-                    mma_bf16(s[nt], qhi[2 * kp + 1], b2, b3);
-                    mma_bf16(s[nt], qlo[2 * kp + 1], b2, b3);
+#pragma unroll
+                    for (int part = 2; part >= 0; --part) {  // smallest parts first
+                        mma_bf16(s[nt], qa[0][part], b0, b1);
+                        mma_bf16(s[nt], qa[1][part], b2, b3);
+                    }
                 }
             }
             // ---- scale, mask, row max ----
@@ -194,36 +230,37 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
             mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, 2));
             const float mn0 = fmaxf(m0, mx0), mn1 = fmaxf(m1, mx1);
             const float mu0 = (mn0 == -INFINITY) ? 0.f : mn0, mu1 = (mn1 == -INFINITY) ? 0.f : mn1;
-            const float c0 = __expf(m0 - mu0), c1 = __expf(m1 - mu1);  // exp(-inf) = 0 on the first chunk
+            const float c0 = expf(m0 - mu0), c1 = expf(m1 - mu1);  // exp(-inf) = 0 on the first chunk
             m0 = mn0; m1 = mn1;
             l0 *= c0; l1 *= c1;
 #pragma unroll
             for (int i = 0; i < D / 8; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
 #pragma unroll
             for (int nt = 0; nt < ATT_CH / 8; ++nt) {
-                s[nt][0] = __expf(s[nt][0] - mu0); s[nt][1] = __expf(s[nt][1] - mu0);
-                s[nt][2] = __expf(s[nt][2] - mu1); s[nt][3] = __expf(s[nt][3] - mu1);
+                s[nt][0] = expf(s[nt][0] - mu0); s[nt][1] = expf(s[nt][1] - mu0);
+                s[nt][2] = expf(s[nt][2] - mu1); s[nt][3] = expf(s[nt][3] - mu1);
                 l0 += s[nt][0] + s[nt][1];
                 l1 += s[nt][2] + s[nt][3];
             }
             // ---- O += P V ----
 #pragma unroll
             for (int kt2 = 0; kt2 < ATT_CH / 16; ++kt2) {
-                uint32_t phi[4], plo[4];
-                split2(s[2 * kt2][0], s[2 * kt2][1], phi[0], plo[0]);
-                split2(s[2 * kt2][2], s[2 * kt2][3], phi[1], plo[1]);
-                split2(s[2 * kt2 + 1][0], s[2 * kt2 + 1][1], phi[2], plo[2]);
-                split2(s[2 * kt2 + 1][2], s[2 * kt2 + 1][3], phi[3], plo[3]);
+                uint32_t pp[3][4];  // hi | mid | lo
+                split3(s[2 * kt2][0], s[2 * kt2][1], pp[0][0], pp[1][0], pp[2][0]);
+                split3(s[2 * kt2][2], s[2 * kt2][3], pp[0][1], pp[1][1], pp[2][1]);
+                split3(s[2 * kt2 + 1][0], s[2 * kt2 + 1][1], pp[0][2], pp[1][2], pp[2][2]);
+                split3(s[2 * kt2 + 1][2], s[2 * kt2 + 1][3], pp[0][3], pp[1][3], pp[2][3]);
                 const int r = kt2 * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
 #pragma unroll
                 for (int np = 0; np < D / 16; ++np) {
                     const int c = np * 2 + (lane >> 4);
                     uint32_t b0, b1, b2, b3;
                     ldsm_x4_trans(vs + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
-                    mma_bf16(o[2 * np], phi, b0, b1);
-                    mma_bf16(o[2 * np], plo, b0, b1);
-                    mma_bf16(o[2 * np + 1], phi, b2, b3);
-                    mma_bf16(o[2 * np + 1], plo, b2, b3);
+#pragma unroll
+                    for (int part = 2; part >= 0; --part) {
+                        mma_bf16(o[2 * np], pp[part], b0, b1);
+                        mma_bf16(o[2 * np + 1], pp[part], b2, b3);
+                    }
                 }
             }
         }
@@ -280,7 +317,7 @@ __global__ void __launch_bounds__(EW_THREADS) attn_merge_quant_kernel(MergeArgs 
             float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
             for (int s = 0; s < ns; ++s) {
                 const float2 ml = *reinterpret_cast<const float2*>(a.ml_part + (pi + s) * 2);
-                const float w = (ml.x == -INFINITY) ? 0.f : __expf(ml.x - mx);
+                const float w = (ml.x == -INFINITY) ? 0.f : expf(ml.x - mx);
                 const float4 ov = *reinterpret_cast<const float4*>(a.o_part + (pi + s) * a.D + d);
                 den += w * ml.y;
                 num.x += w * ov.x; num.y += w * ov.y; num.z += w * ov.z; num.w += w * ov.w;

@@ -384,6 +384,10 @@ __global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
 }
 
 __global__ void set_i32_kernel(int32_t* p, int32_t v) { *p = v; }
+struct SetLensArgs { static constexpr int MAX = 64; int n; int slot[MAX]; int len[MAX]; };
+__global__ void set_lens_kernel(int32_t* ctx_len, SetLensArgs a) {
+    if ((int)threadIdx.x < a.n) ctx_len[a.slot[threadIdx.x]] = a.len[threadIdx.x];
+}
 
 // out[M][H] f32 copy (hidden taps)
 __global__ void __launch_bounds__(EW_THREADS) copy_f32_kernel(const float4* __restrict__ src, float4* __restrict__ dst, long n4) {

@@ -1,0 +1,151 @@
+"""8B-shape parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled
+outputs the oracle computes one by one: the GPU runs the whole step (all 32 layers,
+whole batch); for sampled (sequence, layer) pairs the oracle recomputes that layer from the GPU's own layer
+input and the GPU's exported KV of that layer (verify = f(weights, KV, tree), DESIGN.md R-kv-input) and the
+outputs are compared at the north_star tolerances: hidden rel-L2 <= 1e-2 per layer, logits <= 2e-2 sigma,
+argmax equal where the oracle's top-2 gap >= 1e-3, acceptance walk / compaction indices bit-exact."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import verify_oracle as vo
+from helpers import rel_l2, LAYER_KINDS
+
+pytestmark = [pytest.mark.gpu, pytest.mark.slow8b]
+torch = pytest.importorskip("torch")
+
+TOL_HIDDEN, TOL_LOGIT_SIGMA, GAP = 1e-2, 2e-2, 1e-3
+
+
+def _setup(spec, sample_layers, batch=None, ctx_override=None):
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import bf16_cuda_to_bits
+    shape = spec.model
+    B = batch or spec.batch
+    ctx = wl.context_lengths(spec)[:B] if ctx_override is None else np.asarray(ctx_override, dtype=np.int32)
+    model = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=int(ctx.max()) + 72, page_size=spec.page_size,
+                     act_scale_mode=spec.act_scale_mode)
+    host = {}
+    for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
+        w = wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda")
+        model.ev_model_set_weight(kind, layer, w)
+        if kind == "lm_head" or (kind != "embed" and layer in sample_layers):
+            host[(kind, layer)] = bf16_cuda_to_bits(w)
+        del w
+    torch.cuda.synchronize()
+    om = vo.OracleModel(shape, act_scale_mode=spec.act_scale_mode)
+    for (kind, layer), bits in host.items():
+        om.set_weight(kind, layer, bits)
+    return ev, model, om, ctx
+
+
+def _check_quantized_weights(model, om, layer):
+    for kind in ("wq", "wdown"):
+        cg, sg = model.ev_model_get_quantized(kind, layer)
+        co, so = om.w[(kind, layer)]
+        assert np.array_equal(sg.cpu().numpy(), so) and np.array_equal(cg.cpu().numpy(), co), (kind, layer)
+
+
+def _run_config(spec, sample_layers, sample_seqs, batch=None, ctx_override=None):
+    from gpu_helpers import export_kv_bits, run_verify
+    ev, model, om, ctx = _setup(spec, sample_layers, batch, ctx_override)
+    shape = spec.model
+    B, T = len(ctx), spec.n_nodes
+    parents = wl.chain_parents(T) if spec.tree_caps is None else wl.tree_parents(T, spec.tree_caps)
+    for l in sample_layers[:1]:
+        _check_quantized_weights(model, om, l)
+    if spec.act_scale_mode == 1:
+        calib = wl.calibration_hidden(spec)
+        taps = model.ev_model_calibrate(torch.from_numpy(calib).cuda(), want_layer_inputs=True)
+        scales = model.ev_model_get_static_scales()
+        # the oracle calibrates each sampled layer from the GPU's own input of that layer (needs causal KV of the
+        # calibration run itself: recomputed by the oracle layer on an empty cache, chain of 512 tokens)
+        par = np.arange(-1, calib.shape[0] - 1)
+        for l in sample_layers:
+            rec = {}
+            oc = vo.OracleKV(om, calib.shape[0] // spec.page_size + 2, spec.page_size)
+            oc.add_seq(0, calib.shape[0])
+            vo.layer_forward(om, l, taps[l].cpu().numpy(), oc, 0, 0, par, record=rec)
+            for j, site in enumerate(vo.SITES):
+                ref = np.float32(rec[(site, l)]) / np.float32(448.0)
+                assert abs(float(scales[4 * l + j]) - float(ref)) <= 2e-3 * float(ref), (l, site, scales[4 * l + j], ref)
+        rec = {}
+        vo.lm_head(om, taps[shape.n_layers].cpu().numpy(), record=rec)
+        ref = np.float32(rec[("lm_in", 0)]) / np.float32(448.0)
+        assert abs(float(scales[-1]) - float(ref)) <= 2e-3 * float(ref)
+        # both sides now use the GPU's calibrated constants (one model, DESIGN.md R-static)
+        for l in range(shape.n_layers):
+            for j, site in enumerate(vo.SITES):
+                om.static[(site, l)] = np.float32(scales[4 * l + j])
+        om.static[("lm_in", 0)] = np.float32(scales[-1])
+    pages = sum((int(L) + 64) // spec.page_size + 2 for L in ctx)
+    cache = ev.Cache(model, pages, B)
+    slots = [cache.ev_cache_add_seq(int(L) + 64) for L in ctx]
+    cache.ev_cache_prefill(slots, [wl.context_ids(spec, b, int(ctx[b])) for b in range(B)])
+    tokens = np.stack([wl.draft_tokens_uniform(spec, parents, b) for b in range(B)])
+    tap_layer = sample_layers[0]
+    buf = run_verify(model, cache, slots, tokens, np.tile(parents, (B, 1)), commit=False, want_logits=True,
+                     want_hidden=True, tap_layer=tap_layer)
+    assert (buf.status.cpu().numpy() == 0).all()
+    hid = buf.hidden.cpu().numpy().reshape(shape.n_layers + 1, B, T, shape.hidden)
+    logits = buf.logits.cpu().numpy().reshape(B, T, shape.vocab)
+    am = buf.argmax.cpu().numpy()
+    report = []
+    for b in sample_seqs:
+        L = int(ctx[b])
+        for l in sample_layers:
+            oc = vo.OracleKV(om, (L + T) // spec.page_size + 2, spec.page_size)
+            oc.add_seq(0, L + T)
+            oc.import_dense(l, 0, export_kv_bits(cache, slots[b], l, l + 1, L)[0])
+            oc.ctx_len[0] = L
+            taps = {}
+            h_ref = vo.layer_forward(om, l, hid[l, b], oc, 0, L, parents, taps=taps)
+            err = rel_l2(hid[l + 1, b], h_ref)
+            report.append((b, l, err))
+            assert err <= TOL_HIDDEN, (b, l, err)
+            # appended tree K/V (bf16) equal the oracle's up to 1 ulp on a few elements
+            g = export_kv_bits(cache, slots[b], l, l + 1, L + T)[0][:, :, L:]
+            o = oc.export_dense(l, 0, L + T)[:, :, L:]
+            d = g.astype(np.int32) - o.astype(np.int32)
+            assert np.max(np.abs(d)) <= 1 and np.count_nonzero(d) <= 1e-3 * d.size
+            if l == tap_layer:
+                t = {k: v.cpu().numpy().reshape(B, T, -1)[b] for k, v in buf.taps.items() if v.dim() == 2}
+                assert np.mean(t["xq"] != taps["xq"]) <= 1e-4
+                assert rel_l2(t["attn"], taps["attn"]) <= 1e-5, rel_l2(t["attn"], taps["attn"])
+                assert np.mean(t["aq"] != taps["aq"]) <= 1e-3
+        lg_ref = vo.lm_head(om, hid[shape.n_layers, b])
+        sigma = float(lg_ref.std())
+        dl = float(np.max(np.abs(logits[b] - lg_ref)))
+        report.append((b, "lm", dl / sigma))
+        assert dl <= TOL_LOGIT_SIGMA * sigma, (b, dl, sigma)
+        srt = np.sort(lg_ref, axis=1)
+        ok = (srt[:, -1] - srt[:, -2]) >= GAP
+        assert np.array_equal(am[b][ok], np.argmax(lg_ref, axis=1)[ok])
+    # acceptance walk + compaction indices, bit-exact on the GPU's own argmax, every sequence
+    acc = buf.accept_len.cpu().numpy()
+    nodes = buf.accept_nodes.cpu().numpy()
+    outs = buf.out_tokens.cpu().numpy()
+    newl = buf.new_ctx_len.cpu().numpy()
+    for b in range(B):
+        path, out = vo.accept_walk(tokens[b], parents, am[b])
+        a = len(path) - 1
+        assert acc[b] == a and nodes[b, :a + 1].tolist() == path and outs[b, :a + 1].tolist() == out
+        assert newl[b] == int(ctx[b]) + a + 1
+    print("8B parity report (seq, layer|lm, rel-L2 | max|d|/sigma):", report)
+    return report
+
+
+def test_config1_b1_L2048_tree60_full_size():
+    _run_config(wl.CONFIGS[1], sample_layers=[0, 17, 31], sample_seqs=[0])
+
+
+def test_config2_b32_L4096_tree26_full_size():
+    _run_config(wl.CONFIGS[2], sample_layers=[1, 30], sample_seqs=[0, 31])
+
+
+def test_config3_b64_mixed_context_chain3_full_size():
+    _run_config(wl.CONFIGS[3], sample_layers=[2], sample_seqs=[0, 63])
+
+
+def test_config4_b8_L16384_tree60_static_scales_full_size():
+    _run_config(wl.CONFIGS[4], sample_layers=[0, 16], sample_seqs=[7])

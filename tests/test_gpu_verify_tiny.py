@@ -75,7 +75,11 @@ def test_config0_verify_on_imported_oracle_kv(setup):
 
 
 def test_config0_full_pipeline_gpu_prefill(setup):
-    """form (b): the GPU prefills the 128 context tokens itself."""
+    """form (b): the GPU prefills the 128 context tokens itself.  The prefill is pinned by comparing its KV
+    with the oracle's prefill; the verify step then takes the GPU's exported KV as its input on both sides
+    (DESIGN.md R-kv-input: verify = f(weights, KV, tree)), which keeps the two checks independent: a single
+    E4M3 code flip among the ~390k quantized elements of the prefill would otherwise be amplified by the
+    next quantizers beyond any fixed tolerance ("chaos at the E4M3 step")."""
     from gpu_helpers import run_verify, export_kv_bits
     spec, gm, om, ev = setup
     ids = wl.context_ids(spec, 0, spec.ctx_len)
@@ -84,12 +88,18 @@ def test_config0_full_pipeline_gpu_prefill(setup):
     slot = cache.ev_cache_add_seq(256)
     cache.ev_cache_prefill([slot], [ids])
     assert cache.ev_cache_get_len(slot) == spec.ctx_len
-    g = wl.bf16_bits_to_f32(export_kv_bits(cache, slot, 0, 2, spec.ctx_len))
+    gbits = export_kv_bits(cache, slot, 0, 2, spec.ctx_len)
+    g = wl.bf16_bits_to_f32(gbits)
     o = wl.bf16_bits_to_f32(np.stack([oc.export_dense(l, 0, spec.ctx_len) for l in range(2)]))
     assert rel_l2(g, o) <= 1e-2
+    assert rel_l2(g[0], o[0]) <= 1e-3          # layer 0 sees no upstream quantizer but its own
+    oc2 = fresh_cache(om, 256)
+    for l in range(2):
+        oc2.import_dense(l, 0, gbits[l])
+    oc2.ctx_len[0] = spec.ctx_len
     parents = wl.chain_parents(spec.n_nodes)
     toks = wl.draft_tokens_uniform(spec, parents, 0)
-    res = vo.verify(om, oc, 0, toks, parents, commit=False, want_hidden=True)
+    res = vo.verify(om, oc2, 0, toks, parents, commit=False, want_hidden=True)
     buf = run_verify(gm, cache, [slot], toks[None], parents[None])
     _check_against_oracle(buf, res, spec.n_nodes)
 
