@@ -252,10 +252,13 @@ def main():
     sampler.start()
     ev.ev_launch_count(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.profiler.start()          # no-op unless run under ncu --profile-from-start off
     e0.record()
     for _ in range(args.steps):
         step()
     e1.record()
+    torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
     barrier()
     launches = ev.ev_launch_count()
     ms = e0.elapsed_time(e1)
@@ -276,7 +279,9 @@ def main():
     model.ev_profile_enable(False)
     work = algorithmic_work(spec, ctx, parents)
     pk = peaks()
-    gemm_ms, gemm_n = prof["gemm_fp8"]
+    gemm_ms = sum(v[0] for k, v in prof.items() if k.startswith("gemm_"))
+    gemm_n = sum(v[1] for k, v in prof.items() if k.startswith("gemm_"))
+    per_launch_us = {k: round(1e3 * v[0] / max(v[1], 1), 2) for k, v in prof.items()}
     attn_ms, attn_n = prof["tree_attention"]
     share = {k: round(v[0] / max(sum(x[0] for x in prof.values()), 1e-9), 4) for k, v in prof.items()}
     gemm_gbs = work["weight_bytes"] * args.steps / (gemm_ms * 1e-3) / 1e9
@@ -288,7 +293,8 @@ def main():
                 "peak": pk["hbm_gbs"], "peak_source": pk["source"] + " (MEASURED_PEAKS.json hbm_gbs)" if pk["source"] == "measured" else "fallback (B200_PROFILING.md)",
                 "unit": "GB/s", "frac": round(gemm_gbs / pk["hbm_gbs"], 4),
                 "bytes_per_launch": work["weight_bytes"] / (gemm_n / args.steps), "launches_per_step": gemm_n // args.steps,
-                "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic, "time_share_by_class": share}
+                "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic, "time_share_by_class": share,
+                "avg_launch_us_by_class": per_launch_us}
     fp8_peak = 2 * pk["bf16_tflops"] * 1e12
     t_roof = max((work["weight_bytes"] + work["kv_bytes"]) / (pk["hbm_gbs"] * 1e9), work["flops"] / fp8_peak)
 

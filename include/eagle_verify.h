@@ -218,8 +218,8 @@ int ev_op_quantize_rows(ev_model*, const float* dev_x, int M, int K, float stati
 
 /* ---- introspection ---------------------------------------------------------------------------- */
 /* Device timing per kernel class with CUDA events recorded on the launching stream around each
- * launch (classes: 0 FP8 GEMM, 1 tree attention, 2 attention merge+quant, 3 RMSNorm+quant,
- * 4 RoPE+KV write, 5 SwiGLU+quant, 6 other).  enable(1) starts recording; read() synchronises the
+ * launch (classes: 0..4 FP8 GEMM of QKV / O / gate-up / down / LM head, 5 tree attention, 6 attention
+ * merge+quant, 7 RMSNorm+quant, 8 RoPE+KV write, 9 SwiGLU+quant, 10 other).  enable(1) starts recording; read() synchronises the
  * device, sums elapsed ms and launch counts per class into the host arrays and clears the record. */
 int ev_profile_enable(ev_model*, int on);
 int ev_profile_read(ev_model*, double* host_ms_by_class, long* host_count_by_class, int n_classes);

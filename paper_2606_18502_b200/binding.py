@@ -195,7 +195,8 @@ class Model:
                                             _stream()))
         return codes, sx
 
-    PROFILE_CLASSES = ("gemm_fp8", "tree_attention", "attn_merge_quant", "rmsnorm_quant", "rope_kvwrite", "swiglu_quant", "other")
+    PROFILE_CLASSES = ("gemm_qkv", "gemm_o", "gemm_gateup", "gemm_down", "gemm_lm_head", "tree_attention", "attn_merge_quant",
+                       "rmsnorm_quant", "rope_kvwrite", "swiglu_quant", "other")
 
     def ev_profile_enable(self, on=True):
         _check(self.lib.ev_profile_enable(self.h, 1 if on else 0))

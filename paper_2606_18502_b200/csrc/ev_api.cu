@@ -103,7 +103,8 @@ struct LayerW {
 
 long round_up(long x, long m) { return (x + m - 1) / m * m; }
 
-enum ProfClass { PC_GEMM = 0, PC_ATTN, PC_ATTN_MERGE, PC_NORM_QUANT, PC_ROPE_KV, PC_SWIGLU, PC_OTHER, PC_COUNT };
+enum ProfClass { PC_GEMM_QKV = 0, PC_GEMM_O, PC_GEMM_GATEUP, PC_GEMM_DOWN, PC_GEMM_LM, PC_ATTN, PC_ATTN_MERGE, PC_NORM_QUANT,
+                 PC_ROPE_KV, PC_SWIGLU, PC_OTHER, PC_COUNT };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
 }  // namespace
@@ -239,8 +240,8 @@ int launch_gemm_epi(cudaStream_t st, const CUtensorMap& tmW, const ActBuf& x, co
 
 // y = x . W^T with scales; epi: EPI_STORE / EPI_RESID (in place on out) / EPI_ARGMAX
 int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, float* out, int ldo,
-               unsigned long long* keys) {
-    ProfScope prof_scope(m, st, PC_GEMM);
+               unsigned long long* keys, int prof_cls) {
+    ProfScope prof_scope(m, st, prof_cls);
     GemmArgs a;
     a.M = M; a.N = (int)w.N; a.K = (int)w.K;
     a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
@@ -364,7 +365,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sx) EV_TRY(copy_f32(st, m->xq.scale, out->dev_tap_sx, M));
-        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_STORE, m->qkv, m->qkv_dim, nullptr));
+        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_STORE, m->qkv, m->qkv_dim, nullptr, PC_GEMM_QKV));
         RopeArgs ra;
         ra.qkv = m->qkv; ra.ld = m->qkv_dim; ra.Hq = cfg.n_q_heads; ra.Hkv = cfg.n_kv_heads; ra.D = D; ra.T = T;
         ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
@@ -399,7 +400,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         if (tap && out->dev_tap_attn) EV_TRY(copy_f32(st, m->attn, out->dev_tap_attn, (long)M * m->q_dim));
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
-        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RESID, m->h, H, nullptr));
+        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RESID, m->h, H, nullptr, PC_GEMM_O));
         if (tap && out->dev_tap_hmid) EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H));
         // --- MLP block ---
         {
@@ -407,7 +408,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
             rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
             LAUNCH_CHECK();
         }
-        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_STORE, m->gu, 2 * F, nullptr));
+        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_STORE, m->gu, 2 * F, nullptr, PC_GEMM_GATEUP));
         if (tap && out->dev_tap_gu) EV_TRY(copy_f32(st, m->gu, out->dev_tap_gu, (long)M * 2 * F));
         {
             ProfScope ps(m, st, PC_SWIGLU);
@@ -416,14 +417,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         }
         if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
-        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RESID, m->h, H, nullptr));
+        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RESID, m->h, H, nullptr, PC_GEMM_DOWN));
         if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H));
     }
     if (need_lm) {
         if (ovr && !in->override_first_only) EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H));
         rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers));
         LAUNCH_CHECK();
-        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, out->dev_logits, cfg.vocab, m->argmax_keys));
+        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, out->dev_logits, cfg.vocab, m->argmax_keys, PC_GEMM_LM));
     }
     AcceptArgs ac;
     ac.B = B; ac.T = T; ac.commit = in->commit; ac.force_all = in->force_accept_all;
@@ -962,9 +963,9 @@ int ev_op_linear(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, c
     CUDA_TRY(cudaMemcpyAsync(x->scale, dev_sx, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
     if (kind == EV_W_LM_HEAD) {
         CUDA_TRY(cudaMemsetAsync(m->argmax_keys, 0, (size_t)M * 8, st));
-        return run_linear(m, st, *w, *x, M, EPI_ARGMAX, dev_out, (int)w->N, m->argmax_keys);
+        return run_linear(m, st, *w, *x, M, EPI_ARGMAX, dev_out, (int)w->N, m->argmax_keys, PC_OTHER);
     }
-    return run_linear(m, st, *w, *x, M, EPI_STORE, dev_out, (int)w->N, nullptr);
+    return run_linear(m, st, *w, *x, M, EPI_STORE, dev_out, (int)w->N, nullptr, PC_OTHER);
 }
 
 
