@@ -93,11 +93,12 @@ int ev_model_create(const ev_config* cfg, ev_model** out);
 int ev_model_set_weight(ev_model*, int kind, int layer, const void* dev_bf16, long rows, long cols,
                         void* stream);
 
-/* Returns device pointers (owned by the library, valid until destroy) to the E4M3 codes [rows][cols]
- * and fp32 scales [rows] of a quantized matrix (kinds 1..8).  Q/K/V (and GATE/UP) are views into
- * fused storage: rows are contiguous per kind. */
-int ev_model_get_quantized(ev_model*, int kind, int layer, const uint8_t** dev_codes,
-                           const float** dev_scales, long* rows, long* cols);
+/* Copies a quantized matrix (kinds 1..8) out of the library: E4M3 codes row-major [rows][cols] into
+ * dev_codes_out and fp32 per-output-channel scales [rows] into dev_scales_out (both caller-owned device
+ * buffers).  Internally the codes live in the GEMM's tiled, swizzled HBM layout; this call un-tiles.
+ * rows/cols must equal the matrix shape.  Q/K/V (and GATE/UP) are sub-ranges of fused storage. */
+int ev_model_get_quantized(ev_model*, int kind, int layer, uint8_t* dev_codes_out, float* dev_scales_out,
+                           long rows, long cols, void* stream);
 
 /* Static activation scales (act_scale_mode 1; "Static quantization sets scales offline
  * from activation statistics collected on calibration data"; DESIGN.md R-static): runs

@@ -50,7 +50,7 @@ _P = C.c_void_p
 SIGNATURES = {
     "ev_model_create": (C.c_int, [C.POINTER(ev_config), C.POINTER(_P)]),
     "ev_model_set_weight": (C.c_int, [_P, C.c_int, C.c_int, _P, C.c_long, C.c_long, _P]),
-    "ev_model_get_quantized": (C.c_int, [_P, C.c_int, C.c_int, C.POINTER(_P), C.POINTER(_P), C.POINTER(C.c_long), C.POINTER(C.c_long)]),
+    "ev_model_get_quantized": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_long, C.c_long, _P]),
     "ev_model_calibrate": (C.c_int, [_P, _P, C.c_int, _P, _P]),
     "ev_model_get_static_scales": (C.c_int, [_P, _P]),
     "ev_model_set_static_scales": (C.c_int, [_P, _P]),
@@ -116,13 +116,6 @@ def ev_launch_count(reset=False):
     return load_library().ev_launch_count(1 if reset else 0)
 
 
-class _DevView:
-    """Zero-copy view of library-owned device memory (CUDA array interface)."""
-
-    def __init__(self, ptr, shape, typestr):
-        self.__cuda_array_interface__ = dict(shape=tuple(shape), typestr=typestr, data=(int(ptr), False), version=2)
-
-
 class Model:
     """ev_model handle."""
 
@@ -145,14 +138,14 @@ class Model:
                                             rows, cols, _stream()))
 
     def ev_model_get_quantized(self, kind, layer):
-        """-> (codes uint8 [rows, cols], scales float32 [rows]) as torch CUDA tensors (copies)."""
+        """-> (codes uint8 [rows, cols] row-major, scales float32 [rows]) as torch CUDA tensors."""
         import torch
-        codes, scales, rows, cols = C.c_void_p(), C.c_void_p(), C.c_long(), C.c_long()
-        _check(self.lib.ev_model_get_quantized(self.h, EV_W[kind], layer, C.byref(codes), C.byref(scales),
-                                               C.byref(rows), C.byref(cols)))
-        torch.cuda.current_stream().synchronize()
-        out_c = torch.as_tensor(_DevView(codes.value, (rows.value, cols.value), "|u1"), device="cuda").clone()
-        out_s = torch.as_tensor(_DevView(scales.value, (rows.value,), "<f4"), device="cuda").clone()
+        sh, H, F = self.shape, self.shape.hidden, self.shape.ffn
+        rows, cols = {"wq": (sh.q_dim, H), "wk": (sh.kv_dim, H), "wv": (sh.kv_dim, H), "wo": (H, sh.q_dim), "wgate": (F, H),
+                      "wup": (F, H), "wdown": (H, F), "lm_head": (sh.vocab, H)}[kind]
+        out_c = torch.empty((rows, cols), dtype=torch.uint8, device="cuda")
+        out_s = torch.empty((rows,), dtype=torch.float32, device="cuda")
+        _check(self.lib.ev_model_get_quantized(self.h, EV_W[kind], layer, _ptr(out_c), _ptr(out_s), rows, cols, _stream()))
         return out_c, out_s
 
     def ev_model_calibrate(self, hidden_f32, want_layer_inputs=False):

@@ -77,8 +77,8 @@ int make_tmap(CUtensorMap* tm, const void* base, long rows, long cols, int box_r
     return EV_OK;
 }
 
-constexpr int N_TOK_VARIANTS = 5;
-const int kTokVariants[N_TOK_VARIANTS] = {16, 32, 64, 128, 256};
+constexpr int GEMM_MAX_SPLIT_TILES = 4096;
+constexpr int N_TOK_VARIANTS = 16;  // token-tile sizes 16, 32, ..., 256
 
 struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, with one TMA map per token-tile size
     uint8_t* codes = nullptr;
@@ -87,11 +87,11 @@ struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, 
     CUtensorMap tm[N_TOK_VARIANTS];
 };
 
-struct QMat {  // a quantized weight matrix [N][K]
-    uint8_t* codes = nullptr;
-    float* scale = nullptr;
+struct QMat {  // a quantized weight matrix [N][K], codes in the GEMM's tiled HBM layout (ev_gemm.cuh)
+    uint8_t* codes = nullptr;  // [n_tiles][total_kb][16 KiB]
+    float* scale = nullptr;    // [N]
     long N = 0, K = 0;
-    CUtensorMap tm;
+    int n_tiles = 0, total_kb = 0;
 };
 
 struct LayerW {
@@ -129,6 +129,7 @@ struct ev_model {
     long split_rows_budget = 0;
     float* splitk_partial = nullptr;
     long splitk_floats = 0;
+    int* tile_counter = nullptr;
     // tree state
     int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
     unsigned long long *anc = nullptr, *argmax_keys = nullptr;
@@ -197,84 +198,91 @@ int alloc_actbuf(ev_model* m, ActBuf* b, long K) {
     EV_TRY(dev_alloc(m, &b->codes, (size_t)m->M_pad * K));
     EV_TRY(dev_alloc(m, &b->scale, (size_t)m->M_pad));
     cudaMemset(b->codes, 0, (size_t)m->M_pad * K);
-    for (int i = 0; i < N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&b->tm[i], b->codes, m->M_pad, K, kTokVariants[i]));
+    for (int i = 0; i < N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&b->tm[i], b->codes, m->M_pad, K, 16 * (i + 1)));
     return EV_OK;
 }
 
 int alloc_qmat(ev_model* m, QMat* q, long N, long K) {
     q->N = N;
     q->K = K;
-    EV_TRY(dev_alloc(m, &q->codes, (size_t)N * K));
+    q->n_tiles = (int)((N + GEMM_WROWS - 1) / GEMM_WROWS);
+    q->total_kb = (int)((K + GEMM_BK - 1) / GEMM_BK);
+    const size_t bytes = (size_t)q->n_tiles * q->total_kb * GEMM_WTILE;
+    EV_TRY(dev_alloc(m, &q->codes, bytes));
     EV_TRY(dev_alloc(m, &q->scale, (size_t)N));
-    EV_TRY(make_tmap(&q->tm, q->codes, N, K, GEMM_WROWS));
-    return EV_OK;
-}
-
-template <int TOK, int EPI>
-int launch_gemm_inst(cudaStream_t st, const CUtensorMap& tmW, const CUtensorMap& tmX, const GemmArgs& a, int splits) {
-    using S = GemmSmem<TOK>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<TOK, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL));
-        attr_set = true;
-    }
-    dim3 grid((a.N + GEMM_WROWS - 1) / GEMM_WROWS, (a.M + TOK - 1) / TOK, splits);
-    gemm_e4m3_kernel<TOK, EPI><<<grid, GEMM_THREADS, S::TOTAL, st>>>(tmW, tmX, a);
-    LAUNCH_CHECK();
+    if (cudaMemset(q->codes, 0, bytes) != cudaSuccess) return fail(EV_ECUDA, "memset");  // K / N padding stays zero
     return EV_OK;
 }
 
 template <int EPI>
-int launch_gemm_epi(cudaStream_t st, const CUtensorMap& tmW, const ActBuf& x, const GemmArgs& a, int splits) {
-    int v = N_TOK_VARIANTS - 1;
-    for (int i = 0; i < N_TOK_VARIANTS; ++i)
-        if (a.M <= kTokVariants[i]) { v = i; break; }
-    switch (v) {
-        case 0: return launch_gemm_inst<16, EPI>(st, tmW, x.tm[0], a, splits);
-        case 1: return launch_gemm_inst<32, EPI>(st, tmW, x.tm[1], a, splits);
-        case 2: return launch_gemm_inst<64, EPI>(st, tmW, x.tm[2], a, splits);
-        case 3: return launch_gemm_inst<128, EPI>(st, tmW, x.tm[3], a, splits);
-        default: return launch_gemm_inst<256, EPI>(st, tmW, x.tm[4], a, splits);
+int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int grid, int smem) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        attr_set = true;
     }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(GEMM_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;  // PDL: weight prefetch overlaps the previous kernel
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_e4m3_kernel<EPI>, tmX, a));
+    ++g_launches;
+    return EV_OK;
 }
 
 // y = x . W^T with scales; epi: EPI_STORE / EPI_RESID (in place on out) / EPI_ARGMAX
 int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, float* out, int ldo,
                unsigned long long* keys, int prof_cls) {
     ProfScope prof_scope(m, st, prof_cls);
-    GemmArgs a;
-    a.M = M; a.N = (int)w.N; a.K = (int)w.K;
-    a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
-    a.partial = nullptr; a.argmax_keys = keys;
-    const int total_kb = (int)((w.K + GEMM_BK - 1) / GEMM_BK);
-    a.kb_per_split = total_kb;
     if (m->naive_gemm && epi != EPI_ARGMAX) {
-        dim3 grid((a.N + 127) / 128, M);
-        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, a.N, a.K, a.sx, a.sw, out, ldo, epi == EPI_RESID);
+        dim3 grid((unsigned)((w.N + 127) / 128), M);
+        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, (int)w.N, (int)w.K, w.total_kb, x.scale, w.scale, out, ldo,
+                                                     epi == EPI_RESID);
         LAUNCH_CHECK();
         return EV_OK;
     }
-    int splits = 1;
-    const int tiles = (a.N + GEMM_WROWS - 1) / GEMM_WROWS;
-    if (m->use_splitk && epi != EPI_ARGMAX && M <= 256 && tiles * 2 <= m->num_sms && total_kb >= 8) {
-        splits = std::min(std::min(m->num_sms / tiles, total_kb / 4), 8);
-        a.kb_per_split = (total_kb + splits - 1) / splits;
-        splits = (total_kb + a.kb_per_split - 1) / a.kb_per_split;
-        if ((long)splits * M * a.N > m->splitk_floats) splits = 1, a.kb_per_split = total_kb;
+    GemmArgs a;
+    a.M = M; a.N = (int)w.N; a.total_kb = w.total_kb; a.n_tiles = w.n_tiles;
+    a.m_tiles = (M + 255) / 256;
+    a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
+    const int stage_bytes = GEMM_WTILE + a.tok * GEMM_BK;
+    a.stages = std::min(GEMM_MAX_STAGES, GEMM_SMEM_BUDGET / stage_bytes);
+    a.W = w.codes; a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
+    a.partial = m->splitk_partial; a.tile_counter = m->tile_counter; a.argmax_keys = keys;
+    // split K when the tiles alone cannot fill the SMs evenly: pick the split count with the best wave efficiency
+    const int G = m->num_sms;
+    const int tiles = a.n_tiles * a.m_tiles;
+    int best = 1;
+    if (m->use_splitk && a.m_tiles == 1 && tiles <= GEMM_MAX_SPLIT_TILES) {
+        double best_score = 0.0;
+        for (int ks = 1; ks <= 8 && ks * 4 <= std::max(4, a.total_kb); ++ks) {
+            const int kbs = (a.total_kb + ks - 1) / ks;
+            const int eff_ks = (a.total_kb + kbs - 1) / kbs;
+            if (eff_ks != ks) continue;
+            if ((long)tiles * ks * a.tok * GEMM_WROWS > m->splitk_floats) break;
+            const long items = (long)tiles * ks;
+            const long rounds = (items + G - 1) / G;
+            const double score = (double)items / (double)(rounds * G) / (1.0 + 0.03 * (ks - 1));
+            if (score > best_score + 1e-9) { best_score = score; best = ks; }
+        }
     }
-    if (splits > 1) {
-        a.partial = m->splitk_partial;
-        EV_TRY(launch_gemm_epi<EPI_PARTIAL>(st, w.tm, x, a, splits));
-        const long total = (long)M * a.N;
-        const int blocks = (int)std::min<long>((total + 255) / 256, 148 * 8);
-        splitk_finish_kernel<<<blocks, 256, 0, st>>>(m->splitk_partial, splits, M, a.N, a.sx, a.sw, out, ldo, epi == EPI_RESID);
-        LAUNCH_CHECK();
-        return EV_OK;
-    }
+    a.k_splits = best;
+    a.kb_per_split = (a.total_kb + best - 1) / best;
+    const int items = tiles * a.k_splits;
+    const int grid = std::min(items, G);
+    const int smem = a.stages * stage_bytes + 512 + 1024;
+    const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
     switch (epi) {
-        case EPI_STORE: return launch_gemm_epi<EPI_STORE>(st, w.tm, x, a, 1);
-        case EPI_RESID: return launch_gemm_epi<EPI_RESID>(st, w.tm, x, a, 1);
-        case EPI_ARGMAX: return launch_gemm_epi<EPI_ARGMAX>(st, w.tm, x, a, 1);
+        case EPI_STORE: return launch_gemm<EPI_STORE>(st, tmX, a, grid, smem);
+        case EPI_RESID: return launch_gemm<EPI_RESID>(st, tmX, a, grid, smem);
+        case EPI_ARGMAX: return launch_gemm<EPI_ARGMAX>(st, tmX, a, grid, smem);
     }
     return fail(EV_EINVAL, "bad epilogue");
 }
@@ -497,7 +505,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, dev);
-    m->use_splitk = getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) != 0;
+    m->use_splitk = !(getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) == 0);  // on by default
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;
@@ -520,8 +528,10 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->split_rows_budget = std::max<long>(2L * m->M_cap, 4096);
     A(dev_alloc(m, &m->o_part, (size_t)m->split_rows_budget * m->q_dim));
     A(dev_alloc(m, &m->ml_part, (size_t)m->split_rows_budget * cfg->n_q_heads * 2));
-    m->splitk_floats = 8L * std::min(m->M_cap, 256) * std::max<long>(m->qkv_dim, H);
+    m->splitk_floats = 16L << 20;  // 64 MiB of fp32 split-K partials
     A(dev_alloc(m, &m->splitk_partial, (size_t)m->splitk_floats));
+    A(dev_alloc(m, &m->tile_counter, (size_t)GEMM_MAX_SPLIT_TILES));
+    if (rc == EV_OK) cudaMemset(m->tile_counter, 0, GEMM_MAX_SPLIT_TILES * sizeof(int));
     A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
@@ -574,8 +584,8 @@ int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, 
     auto shape_is = [&](long r, long k) { return rows == r && cols == k; };
     auto bad_shape = [&]() { return fail(EV_EINVAL, "weight shape does not match the model config"); };
     auto quant = [&](QMat& q, long row_off) -> int {
-        quantize_weight_rows_kernel<<<(unsigned)rows, EW_THREADS, 0, st>>>((const __nv_bfloat16*)dev_bf16, cols,
-                                                                          q.codes + row_off * q.K, q.scale + row_off);
+        quantize_weight_rows_kernel<<<(unsigned)rows, EW_THREADS, 0, st>>>((const __nv_bfloat16*)dev_bf16, cols, q.codes, q.total_kb,
+                                                                          row_off, q.scale);
         LAUNCH_CHECK();
         return EV_OK;
     };
@@ -610,8 +620,9 @@ int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, 
     return EV_OK;
 }
 
-int ev_model_get_quantized(ev_model* m, int kind, int layer, const uint8_t** codes, const float** scales, long* rows, long* cols) {
-    if (!m || !codes || !scales) return fail(EV_EINVAL, "null argument");
+int ev_model_get_quantized(ev_model* m, int kind, int layer, uint8_t* dev_codes_out, float* dev_scales_out, long rows, long cols,
+                           void* stream) {
+    if (!m || !dev_codes_out || !dev_scales_out) return fail(EV_EINVAL, "null argument");
     if (kind >= EV_W_Q && kind <= EV_W_DOWN && (layer < 0 || layer >= m->cfg.n_layers)) return fail(EV_EINVAL, "layer out of range");
     const long F = m->cfg.ffn;
     QMat* q = nullptr;
@@ -627,10 +638,11 @@ int ev_model_get_quantized(ev_model* m, int kind, int layer, const uint8_t** cod
         case EV_W_LM_HEAD: q = &m->lm; n = q->N; break;
         default: return fail(EV_EINVAL, "kind is not a quantized matrix");
     }
-    *codes = q->codes + off * q->K;
-    *scales = q->scale + off;
-    if (rows) *rows = n;
-    if (cols) *cols = q->K;
+    if (rows != n || cols != q->K) return fail(EV_EINVAL, "rows/cols do not match the matrix");
+    cudaStream_t st = (cudaStream_t)stream;
+    untile_weight_kernel<<<(unsigned)n, 256, 0, st>>>(q->codes, q->total_kb, off, n, q->K, dev_codes_out);
+    LAUNCH_CHECK();
+    CUDA_TRY(cudaMemcpyAsync(dev_scales_out, q->scale + off, (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
     return EV_OK;
 }
 

@@ -55,14 +55,6 @@ __device__ __forceinline__ void mma_bf16(float* d, const uint32_t* a, uint32_t b
         : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
-// x = hi + lo with hi = bf16(x), lo = bf16(x - hi); packs two values (first in the low half)
-__device__ __forceinline__ void split2(float x0, float x1, uint32_t& hi, uint32_t& lo) {
-    const __nv_bfloat16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
-    const __nv_bfloat16 l0 = __float2bfloat16_rn(x0 - __bfloat162float(h0));
-    const __nv_bfloat16 l1 = __float2bfloat16_rn(x1 - __bfloat162float(h1));
-    hi = (uint32_t)__bfloat16_as_ushort(h0) | ((uint32_t)__bfloat16_as_ushort(h1) << 16);
-    lo = (uint32_t)__bfloat16_as_ushort(l0) | ((uint32_t)__bfloat16_as_ushort(l1) << 16);
-}
 // x = hi + mid + lo exactly (8 + 8 + 8 significand bits)
 __device__ __forceinline__ void split3(float x0, float x1, uint32_t& hi, uint32_t& mid, uint32_t& lo) {
     const __nv_bfloat16 h0 = __float2bfloat16_rn(x0), h1 = __float2bfloat16_rn(x1);
@@ -234,15 +226,18 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
             m0 = mn0; m1 = mn1;
             l0 *= c0; l1 *= c1;
 #pragma unroll
-            for (int i = 0; i < D / 8; ++i) { o[i][0] *= c0; o[i][1] *= c0; o[i][2] *= c1; o[i][3] *= c1; }
-#pragma unroll
             for (int nt = 0; nt < ATT_CH / 8; ++nt) {
                 s[nt][0] = expf(s[nt][0] - mu0); s[nt][1] = expf(s[nt][1] - mu0);
                 s[nt][2] = expf(s[nt][2] - mu1); s[nt][3] = expf(s[nt][3] - mu1);
                 l0 += s[nt][0] + s[nt][1];
                 l1 += s[nt][2] + s[nt][3];
             }
-            // ---- O += P V ----
+            // ---- O += P V: the chunk's product is accumulated from zero inside the tensor core and added to
+            // the running output with ONE rounded fp32 add per chunk (long chains of tensor-core accumulation
+            // truncate: 16k keys in one chain cost ~2e-5 relative) ----
+            float oc[D / 8][4];
+#pragma unroll
+            for (int i = 0; i < D / 8; ++i) { oc[i][0] = oc[i][1] = oc[i][2] = oc[i][3] = 0.f; }
 #pragma unroll
             for (int kt2 = 0; kt2 < ATT_CH / 16; ++kt2) {
                 uint32_t pp[3][4];  // hi | mid | lo
@@ -258,10 +253,15 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                     ldsm_x4_trans(vs + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
 #pragma unroll
                     for (int part = 2; part >= 0; --part) {
-                        mma_bf16(o[2 * np], pp[part], b0, b1);
-                        mma_bf16(o[2 * np + 1], pp[part], b2, b3);
+                        mma_bf16(oc[2 * np], pp[part], b0, b1);
+                        mma_bf16(oc[2 * np + 1], pp[part], b2, b3);
                     }
                 }
+            }
+#pragma unroll
+            for (int i = 0; i < D / 8; ++i) {
+                o[i][0] = fmaf(o[i][0], c0, oc[i][0]); o[i][1] = fmaf(o[i][1], c0, oc[i][1]);
+                o[i][2] = fmaf(o[i][2], c1, oc[i][2]); o[i][3] = fmaf(o[i][3], c1, oc[i][3]);
             }
         }
         __syncthreads();
@@ -298,6 +298,7 @@ struct MergeArgs {
     QuantOut q;
 };
 __global__ void __launch_bounds__(EW_THREADS) attn_merge_quant_kernel(MergeArgs a) {
+    pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
     __shared__ float red[EW_THREADS / 32];
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;

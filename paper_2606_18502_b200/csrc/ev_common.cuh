@@ -150,6 +150,13 @@ __host__ __device__ constexpr uint32_t umma_idesc_e4m3(int M, int N) {
            ((uint32_t)(M >> 4) << 24);
 }
 
+// ---- programmatic dependent launch -----------------------------------------------------------------
+// A kernel launched with the programmatic-serialization attribute may begin while its predecessor
+// runs; it must execute pdl_wait() before touching anything the predecessor wrote.  A predecessor
+// calls pdl_launch_dependents() as early as possible so the dependent's prologue overlaps it.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- cp.async (Ampere-style, for the paged KV gathers) ------------------------------------------
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");

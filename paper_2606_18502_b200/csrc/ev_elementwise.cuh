@@ -23,10 +23,12 @@ __device__ __forceinline__ float block_max(float v, float* red) {
 }
 
 // ---- K1: per-output-channel absmax -> scale, E4M3 codes --------------------------------------
-// one CTA per output channel (row); cols % 8 == 0
+// one CTA per output channel (row); cols % 8 == 0.  Codes are written straight into the GEMM's HBM
+// layout: [n/128][k/128] tiles of 128 rows x 128 bytes, 16 KiB contiguous, 128-byte swizzled
+// (ev_gemm.cuh); row_off = first row of this matrix inside fused storage (QKV, gate|up).
 __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const __nv_bfloat16* __restrict__ w, long cols,
-                                                                          uint8_t* __restrict__ codes,
-                                                                          float* __restrict__ scales) {
+                                                                          uint8_t* __restrict__ codes_tiled, int total_kb,
+                                                                          long row_off, float* __restrict__ scales) {
     __shared__ float red[EW_THREADS / 32];
     const long row = blockIdx.x;
     const uint4* src = reinterpret_cast<const uint4*>(w + row * cols);
@@ -43,8 +45,10 @@ __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const 
     }
     amax = block_max(amax, red);
     const float s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
-    if (threadIdx.x == 0) scales[row] = s;
-    uint2* dst = reinterpret_cast<uint2*>(codes + row * cols);
+    const long n = row_off + row;
+    if (threadIdx.x == 0) scales[n] = s;
+    const int r = (int)(n & 127);
+    uint8_t* trow = codes_tiled + (size_t)(n >> 7) * total_kb * 16384;
     for (int i = threadIdx.x; i < nvec; i += EW_THREADS) {
         uint4 v = __ldg(src + i);
         const uint32_t u[4] = {v.x, v.y, v.z, v.w};
@@ -57,7 +61,9 @@ __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const 
         uint2 o;
         o.x = e4m3x4(f[0], f[1], f[2], f[3]);
         o.y = e4m3x4(f[4], f[5], f[6], f[7]);
-        dst[i] = o;
+        const int k = i * 8, c = k & 127;
+        const int off = r * 128 + ((((c >> 4) ^ (r & 7)) << 4) | (c & 15));
+        *reinterpret_cast<uint2*>(trow + (size_t)(k >> 7) * 16384 + off) = o;
     }
 }
 
@@ -168,6 +174,7 @@ __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut
 __global__ void __launch_bounds__(EW_THREADS) rmsnorm_quant_kernel(const float* __restrict__ h, int H,
                                                                    const __nv_bfloat16* __restrict__ gain, float eps,
                                                                    QuantOut q) {
+    pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
     __shared__ float red[EW_THREADS / 32];
     __shared__ double dred[EW_THREADS / 32];
     const int m = blockIdx.x;
@@ -194,6 +201,7 @@ __global__ void __launch_bounds__(EW_THREADS) rmsnorm_quant_kernel(const float* 
 
 // plain per-token quantization of fp32 rows (attention output uses the fused merge kernel instead)
 __global__ void __launch_bounds__(EW_THREADS) quantize_rows_kernel(const float* __restrict__ x, int K, QuantOut q) {
+    pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
     __shared__ float red[EW_THREADS / 32];
     const int m = blockIdx.x;
     const float* row = x + (size_t)m * K;
@@ -206,6 +214,7 @@ __device__ __forceinline__ float swiglu_f(float g, float u) {
     return mul_rn(div_rn(g, add_rn(1.0f, expf(-g))), u);
 }
 __global__ void __launch_bounds__(EW_THREADS) swiglu_quant_kernel(const float* __restrict__ gu, int F, QuantOut q) {
+    pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
     __shared__ float red[EW_THREADS / 32];
     const int m = blockIdx.x;
     const float* g = gu + (size_t)m * 2 * F;
