@@ -77,7 +77,6 @@ int make_tmap(CUtensorMap* tm, const void* base, long rows, long cols, int box_r
     return EV_OK;
 }
 
-constexpr int GEMM_MAX_SPLIT_TILES = 4096;
 constexpr int N_TOK_VARIANTS = 16;  // token-tile sizes 16, 32, ..., 256
 
 struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, with one TMA map per token-tile size
@@ -123,13 +122,12 @@ struct ev_model {
     ActBuf xq, aq, tq;
     float* qkv = nullptr;
     float* attn = nullptr;
-    float* gu = nullptr;
     float* o_part = nullptr;
     float* ml_part = nullptr;
     long split_rows_budget = 0;
-    float* splitk_partial = nullptr;
-    long splitk_floats = 0;
-    int* tile_counter = nullptr;
+    float* lin_out = nullptr;   // raw GEMM output [splits][M][N], consumed by the next element-wise kernel
+    long lin_floats = 0;
+    unsigned long long* dbg_ts = nullptr;
     // tree state
     int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
     unsigned long long *anc = nullptr, *argmax_keys = nullptr;
@@ -141,6 +139,7 @@ struct ev_model {
     int num_sms = 148;
     bool use_splitk = false, naive_gemm = false;
     bool profile = false;
+    int gemm_dbg = 0, gemm_stages = 0;
     std::vector<ProfRec> prof;
     size_t prof_used = 0;
     std::vector<void*> allocs;
@@ -237,14 +236,18 @@ int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int 
     return EV_OK;
 }
 
-// y = x . W^T with scales; epi: EPI_STORE / EPI_RESID (in place on out) / EPI_ARGMAX
-int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, float* out, int ldo,
+// one W8A8 linear.  epi == EPI_RAW: raw accumulators go to m->lin_out as [splits][M][N]; *lin describes them for
+// the consumer kernel.  epi == EPI_ARGMAX (LM head): scales applied, argmax keys updated, optional logits.
+int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, LinOut* lin, float* logits,
                unsigned long long* keys, int prof_cls) {
     ProfScope prof_scope(m, st, prof_cls);
-    if (m->naive_gemm && epi != EPI_ARGMAX) {
+    if (lin) {
+        lin->p = m->lin_out; lin->splits = 1; lin->ld = (int)w.N; lin->split_stride = (long)M * w.N;
+        lin->sx = x.scale; lin->sw = w.scale;
+    }
+    if (m->naive_gemm && epi == EPI_RAW) {
         dim3 grid((unsigned)((w.N + 127) / 128), M);
-        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, (int)w.N, (int)w.K, w.total_kb, x.scale, w.scale, out, ldo,
-                                                     epi == EPI_RESID);
+        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, (int)w.N, (int)w.K, w.total_kb, m->lin_out, (int)w.N);
         LAUNCH_CHECK();
         return EV_OK;
     }
@@ -254,37 +257,39 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
     const int stage_bytes = GEMM_WTILE + a.tok * GEMM_BK;
     a.stages = std::min(GEMM_MAX_STAGES, GEMM_SMEM_BUDGET / stage_bytes);
-    a.W = w.codes; a.sx = x.scale; a.sw = w.scale; a.out = out; a.ldo = ldo;
-    a.partial = m->splitk_partial; a.tile_counter = m->tile_counter; a.argmax_keys = keys;
-    // split K when the tiles alone cannot fill the SMs evenly: pick the split count with the best wave efficiency
+    if (a.stages < 2) return fail(EV_EINVAL, "token tile too large");
+    if (m->gemm_stages > 0) a.stages = std::min(a.stages, m->gemm_stages);
+    a.W = w.codes; a.sx = x.scale; a.sw = w.scale; a.argmax_keys = keys;
+    a.out = (epi == EPI_RAW) ? m->lin_out : logits;
+    a.ldo = (int)w.N;
+    a.dbg = m->gemm_dbg;
+    a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
+    // split K when the tiles alone cannot fill the SMs evenly: pick the split count with the best wave efficiency.
+    // Splits cost nothing in the GEMM (each writes its own slab); the consumer reads `splits` values per element.
     const int G = m->num_sms;
     const int tiles = a.n_tiles * a.m_tiles;
     int best = 1;
-    if (m->use_splitk && a.m_tiles == 1 && tiles <= GEMM_MAX_SPLIT_TILES) {
+    if (m->use_splitk && epi == EPI_RAW && a.m_tiles == 1) {
         double best_score = 0.0;
         for (int ks = 1; ks <= 8 && ks * 4 <= std::max(4, a.total_kb); ++ks) {
             const int kbs = (a.total_kb + ks - 1) / ks;
-            const int eff_ks = (a.total_kb + kbs - 1) / kbs;
-            if (eff_ks != ks) continue;
-            if ((long)tiles * ks * a.tok * GEMM_WROWS > m->splitk_floats) break;
+            if ((a.total_kb + kbs - 1) / kbs != ks) continue;
+            if ((long)ks * M * a.N > m->lin_floats) break;
             const long items = (long)tiles * ks;
             const long rounds = (items + G - 1) / G;
-            const double score = (double)items / (double)(rounds * G) / (1.0 + 0.03 * (ks - 1));
+            const double score = (double)items / (double)(rounds * G) / (1.0 + 0.02 * (ks - 1));
             if (score > best_score + 1e-9) { best_score = score; best = ks; }
         }
     }
     a.k_splits = best;
     a.kb_per_split = (a.total_kb + best - 1) / best;
+    if (lin) lin->splits = best;
     const int items = tiles * a.k_splits;
     const int grid = std::min(items, G);
-    const int smem = a.stages * stage_bytes + 512 + 1024;
+    const int smem = a.stages * stage_bytes + 512 + 2048 + 8192 + 1024;  // stages + barriers + sx staging + argmax keys + alignment slack
     const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
-    switch (epi) {
-        case EPI_STORE: return launch_gemm<EPI_STORE>(st, tmX, a, grid, smem);
-        case EPI_RESID: return launch_gemm<EPI_RESID>(st, tmX, a, grid, smem);
-        case EPI_ARGMAX: return launch_gemm<EPI_ARGMAX>(st, tmX, a, grid, smem);
-    }
-    return fail(EV_EINVAL, "bad epilogue");
+    if (epi == EPI_RAW) return launch_gemm<EPI_RAW>(st, tmX, a, grid, smem);
+    return launch_gemm<EPI_ARGMAX>(st, tmX, a, grid, smem);
 }
 
 QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
@@ -361,27 +366,41 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     int split_len = (int)round_up((max_keys + n_splits - 1) / n_splits, ATT_CH);
     n_splits = (max_keys + split_len - 1) / split_len;
 
+    LinOut pend;           // raw output of the last O / down GEMM, not yet added to the residual stream
+    pend.p = nullptr;
+    LinOut none;
+    none.p = nullptr; none.splits = 0; none.ld = 0; none.split_stride = 0; none.sx = nullptr; none.sw = nullptr;
+    pend = none;
+    auto materialize = [&]() -> int {  // h += pending (only for debug taps; the fast path fuses this into RMSNorm)
+        if (!pend.p) return EV_OK;
+        apply_pending_kernel<<<M, 256, 0, st>>>(m->h, H, pend);
+        LAUNCH_CHECK();
+        pend = none;
+        return EV_OK;
+    };
+    const bool lockstep = ovr && !in->override_first_only;
     for (int l = 0; l < cfg.n_layers; ++l) {
         LayerW& w = m->layers[l];
         const bool tap = (out->tap_layer == l);
-        if (ovr && !in->override_first_only && l > 0) EV_TRY(copy_f32(st, ovr + (size_t)l * M * H, m->h, (long)M * H));
+        if (lockstep && l > 0) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)l * M * H, m->h, (long)M * H)); }
         // --- attention block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
+            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
             LAUNCH_CHECK();
+            pend = none;
         }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sx) EV_TRY(copy_f32(st, m->xq.scale, out->dev_tap_sx, M));
-        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_STORE, m->qkv, m->qkv_dim, nullptr, PC_GEMM_QKV));
         RopeArgs ra;
-        ra.qkv = m->qkv; ra.ld = m->qkv_dim; ra.Hq = cfg.n_q_heads; ra.Hkv = cfg.n_kv_heads; ra.D = D; ra.T = T;
+        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_RAW, &ra.lin, nullptr, nullptr, PC_GEMM_QKV));
+        ra.qkv_out = m->qkv; ra.ld = m->qkv_dim; ra.Hq = cfg.n_q_heads; ra.Hkv = cfg.n_kv_heads; ra.D = D; ra.T = T;
         ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
         ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
         ra.pool = c->pool + (size_t)l * c->layer_stride;
         {
             ProfScope ps(m, st, PC_ROPE_KV);
-            rope_kvwrite_kernel<<<M, EW_THREADS, 0, st>>>(ra);
+            rope_kvwrite_kernel<<<M, ROPE_THREADS, 0, st>>>(ra);
             LAUNCH_CHECK();
         }
         if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
@@ -408,31 +427,36 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         if (tap && out->dev_tap_attn) EV_TRY(copy_f32(st, m->attn, out->dev_tap_attn, (long)M * m->q_dim));
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
-        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RESID, m->h, H, nullptr, PC_GEMM_O));
-        if (tap && out->dev_tap_hmid) EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H));
+        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_O));
+        if (tap && out->dev_tap_hmid) { EV_TRY(materialize()); EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H)); }
         // --- MLP block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
+            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
             LAUNCH_CHECK();
+            pend = none;
         }
-        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_STORE, m->gu, 2 * F, nullptr, PC_GEMM_GATEUP));
-        if (tap && out->dev_tap_gu) EV_TRY(copy_f32(st, m->gu, out->dev_tap_gu, (long)M * 2 * F));
+        LinOut gul;
+        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_RAW, &gul, nullptr, nullptr, PC_GEMM_GATEUP));
         {
             ProfScope ps(m, st, PC_SWIGLU);
-            swiglu_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->gu, F, quant_out(m, m->tq, 4 * l + 3));
+            swiglu_quant_kernel<<<M, SWI_THREADS, 0, st>>>(gul, F, (tap ? out->dev_tap_gu : nullptr), quant_out(m, m->tq, 4 * l + 3));
             LAUNCH_CHECK();
         }
         if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
-        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RESID, m->h, H, nullptr, PC_GEMM_DOWN));
-        if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H));
+        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_DOWN));
+        if (out->dev_hidden) { EV_TRY(materialize()); EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H)); }
     }
     if (need_lm) {
-        if (ovr && !in->override_first_only) EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H));
-        rmsnorm_quant_kernel<<<M, EW_THREADS, 0, st>>>(m->h, H, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers));
-        LAUNCH_CHECK();
-        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, out->dev_logits, cfg.vocab, m->argmax_keys, PC_GEMM_LM));
+        if (lockstep) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H)); }
+        {
+            ProfScope ps(m, st, PC_NORM_QUANT);
+            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers));
+            LAUNCH_CHECK();
+            pend = none;
+        }
+        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM));
     }
     AcceptArgs ac;
     ac.B = B; ac.T = T; ac.commit = in->commit; ac.force_all = in->force_accept_all;
@@ -506,6 +530,8 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, dev);
     m->use_splitk = !(getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) == 0);  // on by default
+    m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
+    m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;
@@ -524,14 +550,15 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(alloc_actbuf(m, &m->tq, F));
     A(dev_alloc(m, &m->qkv, (size_t)m->M_pad * m->qkv_dim));
     A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
-    A(dev_alloc(m, &m->gu, (size_t)m->M_pad * 2 * F));
     m->split_rows_budget = std::max<long>(2L * m->M_cap, 4096);
     A(dev_alloc(m, &m->o_part, (size_t)m->split_rows_budget * m->q_dim));
     A(dev_alloc(m, &m->ml_part, (size_t)m->split_rows_budget * cfg->n_q_heads * 2));
-    m->splitk_floats = 16L << 20;  // 64 MiB of fp32 split-K partials
-    A(dev_alloc(m, &m->splitk_partial, (size_t)m->splitk_floats));
-    A(dev_alloc(m, &m->tile_counter, (size_t)GEMM_MAX_SPLIT_TILES));
-    if (rc == EV_OK) cudaMemset(m->tile_counter, 0, GEMM_MAX_SPLIT_TILES * sizeof(int));
+    {
+        const long widest = std::max<long>(std::max<long>(2 * F, m->qkv_dim), H);
+        m->lin_floats = std::max<long>((long)m->M_pad * widest, 8L * std::min(m->M_pad, 256) * widest);
+    }
+    A(dev_alloc(m, &m->lin_out, (size_t)m->lin_floats));
+    A(dev_alloc(m, &m->dbg_ts, (size_t)1024 * 8));
     A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
@@ -975,9 +1002,13 @@ int ev_op_linear(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, c
     CUDA_TRY(cudaMemcpyAsync(x->scale, dev_sx, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
     if (kind == EV_W_LM_HEAD) {
         CUDA_TRY(cudaMemsetAsync(m->argmax_keys, 0, (size_t)M * 8, st));
-        return run_linear(m, st, *w, *x, M, EPI_ARGMAX, dev_out, (int)w->N, m->argmax_keys, PC_OTHER);
+        return run_linear(m, st, *w, *x, M, EPI_ARGMAX, nullptr, dev_out, m->argmax_keys, PC_OTHER);
     }
-    return run_linear(m, st, *w, *x, M, EPI_STORE, dev_out, (int)w->N, nullptr, PC_OTHER);
+    LinOut lin;
+    EV_TRY(run_linear(m, st, *w, *x, M, EPI_RAW, &lin, nullptr, nullptr, PC_OTHER));
+    materialize_linear_kernel<<<M, 256, 0, st>>>(dev_out, (int)w->N, lin);
+    LAUNCH_CHECK();
+    return EV_OK;
 }
 
 
@@ -1036,6 +1067,15 @@ int ev_profile_read(ev_model* m, double* host_ms_by_class, long* host_count_by_c
         host_count_by_class[c] += 1;
     }
     m->prof_used = 0;
+    return EV_OK;
+}
+
+// bring-up: copies the per-CTA GEMM phase timestamps of the last launch (EV_GEMM_DBG & 16) to the host
+int ev_debug_gemm_timestamps(ev_model* m, unsigned long long* host_out, int n_ctas) {
+    if (!m || !host_out) return fail(EV_EINVAL, "null argument");
+    CUDA_TRY(cudaDeviceSynchronize());
+    if (n_ctas > 128) n_ctas = 128;
+    CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts, (size_t)n_ctas * 8 * 8, cudaMemcpyDeviceToHost));
     return EV_OK;
 }
 

@@ -150,6 +150,45 @@ __host__ __device__ constexpr uint32_t umma_idesc_e4m3(int M, int N) {
            ((uint32_t)(M >> 4) << 24);
 }
 
+// ---- output of a W8A8 linear as its consumer sees it ------------------------------------------------
+// The layer GEMMs write raw fp32 accumulators, one [M][ld] slab per K-split; the consumer forms
+//   y[m][n] = (((p_0 + p_1) + ...) + p_{S-1}) * s_x[m] * s_w[n]        (fixed order: deterministic)
+// with single rounded fp32 operations, exactly the epilogue the method defines (DESIGN.md R-accum).
+struct LinOut {
+    const float* p;      // [splits][M][ld]
+    int splits, ld;
+    long split_stride;   // M * ld
+    const float* sx;     // [M]
+    const float* sw;     // [N]
+};
+__device__ __forceinline__ float lin_acc(const LinOut& o, size_t idx) {
+    float acc = __ldcg(o.p + idx);
+    for (int s = 1; s < o.splits; ++s) acc = __fadd_rn(acc, __ldcg(o.p + (size_t)s * o.split_stride + idx));
+    return acc;
+}
+__device__ __forceinline__ float lin_value(const LinOut& o, int m, int n, float sxm) {
+    return __fmul_rn(__fmul_rn(lin_acc(o, (size_t)m * o.ld + n), sxm), __ldg(o.sw + n));
+}
+
+// four consecutive channels n..n+3 (n % 4 == 0, ld % 4 == 0): 16-byte loads, all splits in flight together
+__device__ __forceinline__ float4 lin_value4(const LinOut& o, int m, int n, float sxm) {
+    const size_t idx = (size_t)m * o.ld + n;
+    float4 acc = __ldcg(reinterpret_cast<const float4*>(o.p + idx));
+    float4 t[7];
+#pragma unroll
+    for (int s = 1; s < 8; ++s)
+        if (s < o.splits) t[s - 1] = __ldcg(reinterpret_cast<const float4*>(o.p + (size_t)s * o.split_stride + idx));
+#pragma unroll
+    for (int s = 1; s < 8; ++s)
+        if (s < o.splits) {
+            acc.x = __fadd_rn(acc.x, t[s - 1].x); acc.y = __fadd_rn(acc.y, t[s - 1].y);
+            acc.z = __fadd_rn(acc.z, t[s - 1].z); acc.w = __fadd_rn(acc.w, t[s - 1].w);
+        }
+    const float4 w = __ldg(reinterpret_cast<const float4*>(o.sw + n));
+    return make_float4(__fmul_rn(__fmul_rn(acc.x, sxm), w.x), __fmul_rn(__fmul_rn(acc.y, sxm), w.y),
+                       __fmul_rn(__fmul_rn(acc.z, sxm), w.z), __fmul_rn(__fmul_rn(acc.w, sxm), w.w));
+}
+
 // ---- programmatic dependent launch -----------------------------------------------------------------
 // A kernel launched with the programmatic-serialization attribute may begin while its predecessor
 // runs; it must execute pdl_wait() before touching anything the predecessor wrote.  A predecessor

@@ -10,15 +10,15 @@ namespace ev {
 
 constexpr int EW_THREADS = 256;
 
+// red: >= blockDim.x / 32 floats of shared memory
 __device__ __forceinline__ float block_max(float v, float* red) {
     v = warp_max(v);
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = blockDim.x >> 5;
     __syncthreads();
     if (l == 0) red[w] = v;
     __syncthreads();
     float r = red[0];
-#pragma unroll
-    for (int i = 1; i < EW_THREADS / 32; ++i) r = fmaxf(r, red[i]);
+    for (int i = 1; i < nw; ++i) r = fmaxf(r, red[i]);
     return r;
 }
 
@@ -170,61 +170,139 @@ __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut
         dst[i >> 2] = e4m3x4(div_rn(val(i), s), div_rn(val(i + 1), s), div_rn(val(i + 2), s), div_rn(val(i + 3), s));
 }
 
-// ---- K3: RMSNorm + quantize; one CTA per token; H % 4 == 0 --------------------------------------
-__global__ void __launch_bounds__(EW_THREADS) rmsnorm_quant_kernel(const float* __restrict__ h, int H,
-                                                                   const __nv_bfloat16* __restrict__ gain, float eps,
-                                                                   QuantOut q) {
+// row held in registers: thread t owns float4 number t + k*blockDim.x (k < NV4) of the row
+template <int NV4>
+__device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int K, const QuantOut& q, float* red) {
+    const int nthr = blockDim.x;
+    float amax = 0.f;
+#pragma unroll
+    for (int k = 0; k < NV4; ++k)
+        if ((threadIdx.x + k * nthr) * 4 < K)
+            amax = fmaxf(amax, fmaxf(fmaxf(fabsf(v[k].x), fabsf(v[k].y)), fmaxf(fabsf(v[k].z), fabsf(v[k].w))));
+    amax = block_max(amax, red);
+    float s;
+    if (q.static_scale) s = *q.static_scale;
+    else s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
+    if (threadIdx.x == 0) {
+        q.sx[m] = s;
+        if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
+    }
+    uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
+#pragma unroll
+    for (int k = 0; k < NV4; ++k) {
+        const int i4 = threadIdx.x + k * nthr;
+        if (i4 * 4 < K) dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
+    }
+}
+
+// ---- K3: (residual += pending linear output) + RMSNorm + quantize; one CTA of 256 threads per token;
+// H % 4 == 0 and H <= 4096.  `pend` is the raw output of the previous O / down GEMM (LinOut, ev_common.cuh) or
+// has p == null; the updated residual stream is written back to h. ----
+constexpr int NORM_THREADS = 256;
+constexpr int NORM_NV4 = 4;
+__global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
+                                                                     const __nv_bfloat16* __restrict__ gain, float eps,
+                                                                     QuantOut q) {
     pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
-    __shared__ float red[EW_THREADS / 32];
-    __shared__ double dred[EW_THREADS / 32];
+    __shared__ float red[NORM_THREADS / 32];
+    __shared__ double dred[NORM_THREADS / 32];
     const int m = blockIdx.x;
-    const float* x = h + (size_t)m * H;
+    float* x = h + (size_t)m * H;
+    float4 v[NORM_NV4];
+    const float sxm = pend.p ? __ldg(pend.sx + m) : 0.f;
     double acc = 0.0;  // mean of squares accumulated in fp64, rounded once (DESIGN.md R-accum)
-    for (int i = threadIdx.x * 4; i < H; i += EW_THREADS * 4) {
-        const float4 v = *reinterpret_cast<const float4*>(x + i);
-        acc += (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z + (double)v.w * v.w;
+#pragma unroll
+    for (int k = 0; k < NORM_NV4; ++k) {
+        const int i = (threadIdx.x + k * NORM_THREADS) * 4;
+        v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < H) {
+            v[k] = *reinterpret_cast<const float4*>(x + i);
+            if (pend.p) {
+                const float4 y = lin_value4(pend, m, i, sxm);
+                v[k] = make_float4(add_rn(v[k].x, y.x), add_rn(v[k].y, y.y), add_rn(v[k].z, y.z), add_rn(v[k].w, y.w));
+                *reinterpret_cast<float4*>(x + i) = v[k];
+            }
+            acc += (double)v[k].x * v[k].x + (double)v[k].y * v[k].y + (double)v[k].z * v[k].z + (double)v[k].w * v[k].w;
+        }
     }
     acc = warp_sum(acc);
     if ((threadIdx.x & 31) == 0) dred[threadIdx.x >> 5] = acc;
     __syncthreads();
     double tot = 0.0;
 #pragma unroll
-    for (int i = 0; i < EW_THREADS / 32; ++i) tot += dred[i];
+    for (int i = 0; i < NORM_THREADS / 32; ++i) tot += dred[i];
     const float ms = (float)(tot / (double)H);
     const float r = div_rn(1.0f, sqrtf(add_rn(ms, eps)));
-    auto val = [&](int i) -> float {
-        const float g = gain ? __bfloat162float(gain[i]) : 1.0f;
-        return mul_rn(mul_rn(x[i], r), g);
-    };
-    quantize_row(m, H, val, q, red);
+#pragma unroll
+    for (int k = 0; k < NORM_NV4; ++k) {
+        const int i = (threadIdx.x + k * NORM_THREADS) * 4;
+        if (i < H) {
+            float4 g = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (gain) g = make_float4(__bfloat162float(gain[i]), __bfloat162float(gain[i + 1]), __bfloat162float(gain[i + 2]),
+                                      __bfloat162float(gain[i + 3]));
+            v[k] = make_float4(mul_rn(mul_rn(v[k].x, r), g.x), mul_rn(mul_rn(v[k].y, r), g.y), mul_rn(mul_rn(v[k].z, r), g.z),
+                               mul_rn(mul_rn(v[k].w, r), g.w));
+        }
+    }
+    quantize_regs<NORM_NV4>(v, m, H, q, red);
 }
 
-// plain per-token quantization of fp32 rows (attention output uses the fused merge kernel instead)
+// residual += pending linear output, nothing else (debug taps / end of a prefill pass)
+__global__ void __launch_bounds__(256) apply_pending_kernel(float* __restrict__ h, int H, LinOut pend) {
+    const int m = blockIdx.x;
+    const float sxm = __ldg(pend.sx + m);
+    for (int i = threadIdx.x; i < H; i += 256) h[(size_t)m * H + i] = add_rn(h[(size_t)m * H + i], lin_value(pend, m, i, sxm));
+}
+// y = linear output with its scales (ev_op_linear)
+__global__ void __launch_bounds__(256) materialize_linear_kernel(float* __restrict__ out, int N, LinOut lin) {
+    const int m = blockIdx.x;
+    const float sxm = __ldg(lin.sx + m);
+    for (int i = threadIdx.x; i < N; i += 256) out[(size_t)m * N + i] = lin_value(lin, m, i, sxm);
+}
+
+// plain per-token quantization of fp32 rows (ev_op_quantize_rows)
 __global__ void __launch_bounds__(EW_THREADS) quantize_rows_kernel(const float* __restrict__ x, int K, QuantOut q) {
-    pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
     __shared__ float red[EW_THREADS / 32];
     const int m = blockIdx.x;
     const float* row = x + (size_t)m * K;
     quantize_row(m, K, [&](int i) -> float { return row[i]; }, q, red);
 }
 
-// ---- K6: SwiGLU + quantize; gu = [M][2F] (gate | up); one CTA per token; F % 4 == 0 -------------
+// ---- K6: SwiGLU + quantize on the raw gate|up GEMM output (LinOut, ld = 2F: gate | up); one CTA of 512
+// threads per token, the row of F values lives in registers; F % 4 == 0 and F <= 16384. ----
 __device__ __forceinline__ float swiglu_f(float g, float u) {
     // t = (g / (1 + exp(-g))) * u, fp32 ops in this order; expf is the full-range libdevice one
     return mul_rn(div_rn(g, add_rn(1.0f, expf(-g))), u);
 }
-__global__ void __launch_bounds__(EW_THREADS) swiglu_quant_kernel(const float* __restrict__ gu, int F, QuantOut q) {
-    pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
-    __shared__ float red[EW_THREADS / 32];
+constexpr int SWI_THREADS = 512;
+constexpr int SWI_NV4 = 8;
+__global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, int F, float* __restrict__ gu_tap, QuantOut q) {
+    pdl_launch_dependents();  // the down-projection GEMM may start prefetching its weights now
+    __shared__ float red[SWI_THREADS / 32];
     const int m = blockIdx.x;
-    const float* g = gu + (size_t)m * 2 * F;
-    const float* u = g + F;
-    quantize_row(m, F, [&](int i) -> float { return swiglu_f(g[i], u[i]); }, q, red);
+    const float sxm = __ldg(gu.sx + m);
+    float4 v[SWI_NV4];
+#pragma unroll
+    for (int k = 0; k < SWI_NV4; ++k) {
+        const int i = (threadIdx.x + k * SWI_THREADS) * 4;
+        v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < F) {
+            const float4 g = lin_value4(gu, m, i, sxm), u = lin_value4(gu, m, F + i, sxm);
+            if (gu_tap) {
+                *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + i) = g;
+                *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + F + i) = u;
+            }
+            v[k] = make_float4(swiglu_f(g.x, u.x), swiglu_f(g.y, u.y), swiglu_f(g.z, u.z), swiglu_f(g.w, u.w));
+        }
+    }
+    quantize_regs<SWI_NV4>(v, m, F, q, red);
 }
 
-// ---- K4: RoPE (positions = L + depth) on q, k in place (fp32) + K,V -> bf16 pages ----------------
+// ---- K4: RoPE (positions = L + depth) on q, k of the raw QKV GEMM output + K,V -> bf16 pages; q, k, v are
+// also written as fp32 to qkv_out [M][ld] (q feeds attention).  One CTA of 512 threads per token. ----
 struct RopeArgs {
-    float* qkv;           // [M][ld]; q heads, then k heads, then v heads
+    LinOut lin;           // raw QKV output, ld = (Hq + 2 Hkv) * D
+    float* qkv_out;       // [M][ld]
     int ld, Hq, Hkv, D, T;
     const int32_t* pos;   // [M]
     const float2* cs;     // [max_pos][D/2] (cos, sin) built on the host in fp64
@@ -235,11 +313,13 @@ struct RopeArgs {
     int max_pages, page_size;
     __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D]
 };
-__global__ void __launch_bounds__(EW_THREADS) rope_kvwrite_kernel(RopeArgs a) {
+constexpr int ROPE_THREADS = 512;
+__global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) {
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
     const int D = a.D, D2 = D / 2;
-    float* row = a.qkv + (size_t)m * a.ld;
+    const float sxm = __ldg(a.lin.sx + m);
+    float* __restrict__ row = a.qkv_out + (size_t)m * a.ld;
     const float2* cs = a.cs + (size_t)a.pos[m] * D2;
     const bool write = node < a.nn_eff[b];
     __nv_bfloat16* kdst = nullptr;
@@ -251,27 +331,35 @@ __global__ void __launch_bounds__(EW_THREADS) rope_kvwrite_kernel(RopeArgs a) {
         kdst = a.pool + base;
         vdst = a.pool + base + (size_t)a.Hkv * a.page_size * D;
     }
-    const int n_rot = (a.Hq + a.Hkv) * D2;
-    for (int i = threadIdx.x; i < n_rot; i += EW_THREADS) {
-        const int head = i / D2, j = i % D2;
-        float* x = row + head * D;
-        const float2 c = cs[j];
-        const float lo = x[j], hi = x[j + D2];
-        const float rlo = sub_rn(mul_rn(lo, c.x), mul_rn(hi, c.y));
-        const float rhi = add_rn(mul_rn(hi, c.x), mul_rn(lo, c.y));
-        x[j] = rlo;
-        x[j + D2] = rhi;
+    const int n_rot4 = (a.Hq + a.Hkv) * D2 / 4;  // groups of 4 rotation pairs
+    for (int i = threadIdx.x; i < n_rot4; i += ROPE_THREADS) {
+        const int head = (i * 4) / D2, j = (i * 4) % D2;
+        const float4 lo = lin_value4(a.lin, m, head * D + j, sxm), hi = lin_value4(a.lin, m, head * D + j + D2, sxm);
+        const float4 c01 = __ldg(reinterpret_cast<const float4*>(cs + j)), c23 = __ldg(reinterpret_cast<const float4*>(cs + j + 2));
+        float4 rlo, rhi;  // (cos, sin) pairs: c01 = (c0, s0, c1, s1), c23 = (c2, s2, c3, s3)
+        rlo.x = sub_rn(mul_rn(lo.x, c01.x), mul_rn(hi.x, c01.y)); rhi.x = add_rn(mul_rn(hi.x, c01.x), mul_rn(lo.x, c01.y));
+        rlo.y = sub_rn(mul_rn(lo.y, c01.z), mul_rn(hi.y, c01.w)); rhi.y = add_rn(mul_rn(hi.y, c01.z), mul_rn(lo.y, c01.w));
+        rlo.z = sub_rn(mul_rn(lo.z, c23.x), mul_rn(hi.z, c23.y)); rhi.z = add_rn(mul_rn(hi.z, c23.x), mul_rn(lo.z, c23.y));
+        rlo.w = sub_rn(mul_rn(lo.w, c23.z), mul_rn(hi.w, c23.w)); rhi.w = add_rn(mul_rn(hi.w, c23.z), mul_rn(lo.w, c23.w));
+        *reinterpret_cast<float4*>(row + head * D + j) = rlo;
+        *reinterpret_cast<float4*>(row + head * D + j + D2) = rhi;
         if (head >= a.Hq && write) {
             __nv_bfloat16* kd = kdst + (size_t)(head - a.Hq) * a.page_size * D;
-            kd[j] = __float2bfloat16_rn(rlo);
-            kd[j + D2] = __float2bfloat16_rn(rhi);
+            __nv_bfloat162 p0 = __floats2bfloat162_rn(rlo.x, rlo.y), p1 = __floats2bfloat162_rn(rlo.z, rlo.w);
+            __nv_bfloat162 p2 = __floats2bfloat162_rn(rhi.x, rhi.y), p3 = __floats2bfloat162_rn(rhi.z, rhi.w);
+            *reinterpret_cast<uint2*>(kd + j) = make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
+            *reinterpret_cast<uint2*>(kd + j + D2) = make_uint2(*reinterpret_cast<uint32_t*>(&p2), *reinterpret_cast<uint32_t*>(&p3));
         }
     }
-    if (write) {
-        const float* v = row + (a.Hq + a.Hkv) * D;
-        for (int i = threadIdx.x; i < a.Hkv * D; i += EW_THREADS) {
-            const int head = i / D, j = i % D;
-            vdst[(size_t)head * a.page_size * D + j] = __float2bfloat16_rn(v[i]);
+    const int voff = (a.Hq + a.Hkv) * D;
+    for (int i = threadIdx.x; i < a.Hkv * D / 4; i += ROPE_THREADS) {
+        const int head = (i * 4) / D, j = (i * 4) % D;
+        const float4 v = lin_value4(a.lin, m, voff + i * 4, sxm);
+        *reinterpret_cast<float4*>(row + voff + i * 4) = v;
+        if (write) {
+            __nv_bfloat162 p0 = __floats2bfloat162_rn(v.x, v.y), p1 = __floats2bfloat162_rn(v.z, v.w);
+            *reinterpret_cast<uint2*>(vdst + (size_t)head * a.page_size * D + j) =
+                make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
         }
     }
 }

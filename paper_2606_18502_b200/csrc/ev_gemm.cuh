@@ -20,8 +20,11 @@
 // Persistent CTAs (grid = min(#SMs, work items)); a work item is (n_tile, m_tile, k_split), k_split
 // fastest.  Warp roles (192 threads): warp 0 = TMA producer, warp 1 = TMEM owner + MMA issuer,
 // warps 2..5 = epilogue.  Two TMEM accumulators alternate so the epilogue of item i overlaps the
-// main loop of item i+1.  Split-K (few tiles, small M) is deterministic: every split writes its raw
-// fp32 partial, the split that arrives last at the tile's counter sums ALL partials in split order.
+// main loop of item i+1.  The epilogue of the layer GEMMs is deliberately trivial: raw fp32 accumulators
+// go to out[split][m][n]; the kernel that consumes them (RMSNorm / RoPE / SwiGLU, each of which reads
+// every element exactly once) sums the K-splits in split order and applies s_x[m] * s_w[n] (+ residual).
+// That makes split-K free of any fix-up pass, fence or atomic, and deterministic (LinOut, ev_common.cuh).
+// Only the LM head applies its scales here, because it reduces to an argmax in the epilogue.
 // Programmatic dependent launch: barrier setup, TMEM allocation and the first STAGES weight tiles
 // are issued BEFORE griddepcontrol.wait (weights do not depend on the previous kernel), so the
 // weight stream of this GEMM starts while the previous (element-wise) kernel is still running.
@@ -30,7 +33,7 @@
 
 namespace ev {
 
-enum GemmEpi { EPI_STORE = 0, EPI_RESID = 1, EPI_ARGMAX = 2 };
+enum GemmEpi { EPI_RAW = 0, EPI_ARGMAX = 2 };
 
 constexpr int GEMM_THREADS = 192;
 constexpr int GEMM_BK = 128;          // bytes (= E4M3 elements) of K per stage: one swizzle row
@@ -48,11 +51,11 @@ struct GemmArgs {
     const uint8_t* W;   // tiled + swizzled codes: [n_tiles][total_kb][16 KiB]
     const float* sx;    // [M]
     const float* sw;    // [N]
-    float* out;         // [M][ldo]; EPI_RESID: out += y in place; EPI_ARGMAX: optional logits
+    float* out;         // EPI_RAW: [k_splits][M][ldo] raw accumulators; EPI_ARGMAX: optional logits [M][ldo]
     int ldo;
-    float* partial;     // split-K: [tile][split][tok][128] raw fp32
-    int* tile_counter;  // split-K: [tile], zero on entry and on exit
     unsigned long long* argmax_keys;  // EPI_ARGMAX: [M] packed (ordered logit, ~index)
+    unsigned long long* ts;  // bring-up: per-CTA phase timestamps [grid][8] (globaltimer ns), or null
+    int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads
 };
 
 // byte offset of element (row r, byte c) inside a 16 KiB weight tile (128-byte swizzle)
@@ -80,6 +83,27 @@ __device__ __forceinline__ void tmem_dealloc_rt(uint32_t taddr, uint32_t ncols) 
 }
 __device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
+__device__ __forceinline__ void bulk_load_plain(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void load_w(int dbg, uint8_t* dst, const uint8_t* src, uint64_t* bar, uint64_t pol) {
+    if (dbg & 8) return;
+    const int parts = (dbg & 2) ? 4 : 1;
+    const uint32_t bytes = GEMM_WROWS * GEMM_BK / parts;
+    for (int i = 0; i < parts; ++i) {
+        if (dbg & 1) bulk_load_plain(dst + i * bytes, src + i * bytes, bytes, bar);
+        else bulk_load(dst + i * bytes, src + i * bytes, bytes, bar, pol);
+    }
+}
+__device__ __forceinline__ void load_x(int dbg, uint8_t* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, uint64_t pol) {
+    if (dbg & 8) return;
+    if (dbg & 1) tma_load_2d(dst, tm, bar, c0, c1);
+    else tma_load_2d_hint(dst, tm, bar, c0, c1, pol);
+}
+__device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
+#define TS(i) do { if (a.ts) a.ts[blockIdx.x * 8 + (i)] = gtimer(); } while (0)
 struct GemmItem { int n_tile, m_tile, split, tile, kb0, nkb; };
 __device__ __forceinline__ GemmItem gemm_item(const GemmArgs& a, int w) {
     GemmItem it;
@@ -103,57 +127,59 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     uint64_t* tmem_full_bar = empty_bar + GEMM_MAX_STAGES;   // [2]
     uint64_t* tmem_empty_bar = tmem_full_bar + 2;            // [2]
     uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(tmem_empty_bar + 2);
-    int* flag_smem = reinterpret_cast<int*>(tmem_base_smem + 1);
+    float* sx_smem = reinterpret_cast<float*>(tmem_base_smem + 4);  // [2][256] per-token scales of the current / next item
+    unsigned long long* keys_smem = reinterpret_cast<unsigned long long*>(sx_smem + 512);  // [4 warps][256] argmax keys
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) TS(0);
     const int total_items = a.n_tiles * a.m_tiles * a.k_splits;
     uint32_t tmem_cols = 32;
     while ((int)tmem_cols < 2 * a.tok) tmem_cols <<= 1;
 
+    // ---- prologue.  The producer thread initialises the barriers and immediately starts the weight stream of
+    // its first work item (weights do not depend on the previous kernel: this runs before griddepcontrol.wait,
+    // i.e. while the previous kernel is still executing when launched with programmatic serialization). ----
+    int pre = 0;
+    GemmItem it0 = gemm_item(a, min((int)blockIdx.x, total_items - 1));
     if (warp == 0 && lane == 0) {
-        tma_prefetch_desc(&tmX);
         for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], 4); }
         fence_barrier_init();
+        pre = min(a.stages, it0.nkb);
+        const uint8_t* wsrc = a.W + ((size_t)it0.n_tile * a.total_kb + it0.kb0) * GEMM_WTILE;
+        for (int i = 0; i < pre; ++i) {
+            if (a.dbg & 8) mbar_arrive(&full_bar[i]); else mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
+            if (!(a.dbg & 8)) bulk_load_plain(smem + i * stage_bytes, wsrc + (size_t)i * GEMM_WTILE, GEMM_WTILE, &full_bar[i]);
+        }
+        tma_prefetch_desc(&tmX);
+        TS(2);
     }
     if (warp == 1) tmem_alloc_rt(tmem_base_smem, tmem_cols);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
+    if (threadIdx.x == 0) TS(1);
 
     if (warp == 0) {
         if (lane == 0) {  // ===== producer: weights by linear bulk copy, activations by 2-D TMA =====
             const uint64_t pol_w = policy_evict_first();   // weights are streamed once per step
             const uint64_t pol_x = policy_evict_last();    // activations are re-read by every tile
-            int s = 0;
-            uint32_t ph = 0;
-            int w = blockIdx.x;
-            int pre = 0;
-            GemmItem it0;
-            if (w < total_items) {  // weight tiles of the first item: no dependency on the previous kernel
-                it0 = gemm_item(a, w);
-                pre = min(a.stages, it0.nkb);
-                for (int i = 0; i < pre; ++i) {
-                    mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
-                    bulk_load(smem + i * stage_bytes, a.W + ((size_t)it0.n_tile * a.total_kb + it0.kb0 + i) * GEMM_WTILE,
-                              GEMM_WTILE, &full_bar[i], pol_w);
-                }
-            }
-            pdl_wait();  // activations (and everything the epilogue reads) come from the previous kernel
+            pdl_wait();  // activations come from the previous kernel
+            TS(3);
             for (int i = 0; i < pre; ++i)
-                tma_load_2d_hint(smem + i * stage_bytes + GEMM_WTILE, &tmX, &full_bar[i], (it0.kb0 + i) * GEMM_BK,
-                                 it0.m_tile * a.tok, pol_x);
-            s = pre;
+                load_x(a.dbg, smem + i * stage_bytes + GEMM_WTILE, &tmX, &full_bar[i], (it0.kb0 + i) * GEMM_BK, it0.m_tile * a.tok, pol_x);
+            int s = pre;
+            uint32_t ph = 0;
             if (s == a.stages) { s = 0; ph ^= 1; }
-            for (; w < total_items; w += gridDim.x) {
+            for (int w = blockIdx.x; w < total_items; w += gridDim.x) {
                 const GemmItem it = gemm_item(a, w);
                 for (int kb = (w == (int)blockIdx.x ? pre : 0); kb < it.nkb; ++kb) {
                     mbar_wait(&empty_bar[s], ph ^ 1);
-                    mbar_arrive_expect_tx(&full_bar[s], stage_bytes);
+                    if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], stage_bytes);
                     uint8_t* st = smem + s * stage_bytes;
-                    bulk_load(st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, GEMM_WTILE, &full_bar[s], pol_w);
-                    tma_load_2d_hint(st + GEMM_WTILE, &tmX, &full_bar[s], (it.kb0 + kb) * GEMM_BK, it.m_tile * a.tok, pol_x);
+                    load_w(a.dbg, st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, &full_bar[s], pol_w);
+                    load_x(a.dbg, st + GEMM_WTILE, &tmX, &full_bar[s], (it.kb0 + kb) * GEMM_BK, it.m_tile * a.tok, pol_x);
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
             }
@@ -176,124 +202,105 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     const uint32_t wa = smem_u32(smem + s * stage_bytes);
                     const uint64_t adesc = umma_desc_k128(wa);
                     const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
+                    if (!(a.dbg & 4)) {
 #pragma unroll
-                    for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
-                        umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                        for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
+                            umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                    }
                     umma_commit(&empty_bar[s]);
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
                 umma_commit(&tmem_full_bar[buf]);
+                if (n_it == 0) TS(4);
             }
         }
     } else {  // ===== epilogue: warps 2..5; warp w may touch TMEM lanes 32*(w%4) .. +31 =====
         pdl_wait();
         const int q = warp & 3;
         const int et = (int)threadIdx.x - 64;  // 0..127 among the epilogue threads
+        const int n_loc = q * 32 + lane;
         int n_it = 0;
         for (int w = blockIdx.x; w < total_items; w += gridDim.x, ++n_it) {
             const GemmItem it = gemm_item(a, w);
             const int buf = n_it & 1;
-            const int n_loc = q * 32 + lane;
             const int n = it.n_tile * GEMM_WROWS + n_loc;
             const int m0 = it.m_tile * a.tok;
             const bool n_ok = n < a.N;
-            const float swn = n_ok ? a.sw[n] : 0.f;
+            constexpr int GC = 32;                    // columns (tokens) handled per register group
+            const int n_groups = (a.tok + GC - 1) / GC;
+            float swn = 0.f;
+            float* sxs = sx_smem + buf * 256;
+            if (EPI == EPI_ARGMAX) {  // scales are fetched BEFORE waiting for the MMAs
+                swn = n_ok ? __ldg(a.sw + n) : 0.f;
+                for (int i = et; i < a.tok; i += 128) sxs[i] = (m0 + i < a.M) ? __ldg(a.sx + m0 + i) : 0.f;
+                epi_bar_sync();
+            }
             mbar_wait(&tmem_full_bar[buf], (n_it >> 1) & 1);
             tc_fence_after();
+            if (n_it == 0 && et == 0) TS(5);
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * a.tok);
-            const int n_chunks = a.tok / 16;
-            bool reduce_here = true;
-            float* part = nullptr;
-            if (a.k_splits > 1) {
-                // ---- split-K: publish the raw partial, last arriver reduces all of them in split order ----
-                part = a.partial + (size_t)it.tile * a.k_splits * a.tok * GEMM_WROWS;
-                float* mine = part + (size_t)it.split * a.tok * GEMM_WROWS;
-                for (int c = 0; c < n_chunks; ++c) {
-                    uint32_t v[16];
-                    tmem_ld16(t_addr + (uint32_t)(c * 16), v);
-                    tmem_ld_wait();
+            float* outp = a.out + (size_t)it.split * a.M * a.ldo;
+            for (int g = 0; g < n_groups; ++g) {
+                uint32_t v[GC];
+                tmem_ld16(t_addr + (uint32_t)(g * GC), v);
+                if (g * GC + 16 < a.tok) tmem_ld16(t_addr + (uint32_t)(g * GC + 16), v + 16);
+                tmem_ld_wait();
+                if (g == n_groups - 1) {  // accumulator fully read: hand it back to the MMA warp
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&tmem_empty_bar[buf]);
+                }
+                if (EPI == EPI_ARGMAX) {
+                    // per token: max over the tile's 128 channels of (ordered logit, ~index); warp shuffle, then the 4
+                    // warps meet in shared memory and ONE atomicMax per (token, tile) goes to global memory
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) mine[(size_t)(c * 16 + j) * GEMM_WROWS + n_loc] = __uint_as_float(v[j]);
+                    for (int j = 0; j < GC; ++j) {
+                        const int col = g * GC + j;
+                        const int m = m0 + col;
+                        const float y = mul_rn(mul_rn(__uint_as_float(v[j]), sxs[col < a.tok ? col : 0]), swn);
+                        unsigned long long key = (n_ok && col < a.tok && m < a.M) ? (((unsigned long long)ordered_bits(y) << 32) | (0xFFFFFFFFu - (uint32_t)n)) : 0ull;
+#pragma unroll
+                        for (int o = 16; o > 0; o >>= 1) {
+                            const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+                            key = other > key ? other : key;
+                        }
+                        if (lane == 0 && col < a.tok) keys_smem[q * 256 + col] = key;
+                        if (n_ok && col < a.tok && m < a.M && a.out) __stcs(a.out + (size_t)m * a.ldo + n, y);
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < GC; ++j) {
+                        const int col = g * GC + j;
+                        const int m = m0 + col;
+                        if (n_ok && col < a.tok && m < a.M) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
+                    }
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&tmem_empty_bar[buf]);
-                __threadfence();
-                epi_bar_sync();
-                if (et == 0) {
-                    const int old = atomicAdd(a.tile_counter + it.tile, 1);
-                    *flag_smem = (old == a.k_splits - 1);
-                    if (old == a.k_splits - 1) a.tile_counter[it.tile] = 0;  // ready for the next launch
-                }
-                epi_bar_sync();
-                reduce_here = *flag_smem != 0;
-                epi_bar_sync();  // flag is rewritten by the next item
-                if (reduce_here) __threadfence();
             }
-            if (reduce_here) {
-                for (int c = 0; c < n_chunks; ++c) {
-                    float acc[16];
-                    if (a.k_splits > 1) {
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) acc[j] = __ldcg(part + (size_t)(c * 16 + j) * GEMM_WROWS + n_loc);
-                        for (int sp = 1; sp < a.k_splits; ++sp) {
-                            const float* ps = part + (size_t)sp * a.tok * GEMM_WROWS;
-#pragma unroll
-                            for (int j = 0; j < 16; ++j) acc[j] = add_rn(acc[j], __ldcg(ps + (size_t)(c * 16 + j) * GEMM_WROWS + n_loc));
-                        }
-                    } else {
-                        uint32_t v[16];
-                        tmem_ld16(t_addr + (uint32_t)(c * 16), v);
-                        tmem_ld_wait();
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) acc[j] = __uint_as_float(v[j]);
-                        if (c == n_chunks - 1) {  // accumulator fully read: hand it back to the MMA warp
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) mbar_arrive(&tmem_empty_bar[buf]);
-                        }
-                    }
-                    const int mc = m0 + c * 16;
-                    if (mc >= a.M) continue;  // warp-uniform
-                    const int m_lane = mc + (lane & 15);
-                    const float sx_lane = (m_lane < a.M) ? __ldg(a.sx + m_lane) : 0.f;
-                    float res[16];
-                    if (EPI == EPI_RESID) {
-#pragma unroll
-                        for (int j = 0; j < 16; ++j) res[j] = (n_ok && mc + j < a.M) ? __ldcg(a.out + (size_t)(mc + j) * a.ldo + n) : 0.f;
-                    }
-#pragma unroll
-                    for (int j = 0; j < 16; ++j) {
-                        const float sxm = __shfl_sync(0xffffffffu, sx_lane, j);
-                        const int m = mc + j;
-                        const float y = mul_rn(mul_rn(acc[j], sxm), swn);
-                        if (EPI == EPI_ARGMAX) {
-                            unsigned long long key = (n_ok && m < a.M) ? (((unsigned long long)ordered_bits(y) << 32) | (0xFFFFFFFFu - (uint32_t)n)) : 0ull;
-#pragma unroll
-                            for (int o = 16; o > 0; o >>= 1) {
-                                const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
-                                key = other > key ? other : key;
-                            }
-                            if (lane == 0 && m < a.M) atomicMax(a.argmax_keys + m, key);
-                            if (n_ok && m < a.M && a.out) __stcs(a.out + (size_t)m * a.ldo + n, y);
-                        } else if (n_ok && m < a.M) {
-                            a.out[(size_t)m * a.ldo + n] = (EPI == EPI_RESID) ? add_rn(res[j], y) : y;
-                        }
+            if (EPI == EPI_ARGMAX) {
+                epi_bar_sync();
+                for (int col = et; col < a.tok; col += 128) {
+                    const int m = m0 + col;
+                    if (m < a.M) {
+                        unsigned long long k0 = keys_smem[col], k1 = keys_smem[256 + col], k2 = keys_smem[512 + col], k3 = keys_smem[768 + col];
+                        k0 = k1 > k0 ? k1 : k0; k2 = k3 > k2 ? k3 : k2; k0 = k2 > k0 ? k2 : k0;
+                        atomicMax(a.argmax_keys + m, k0);
                     }
                 }
+                epi_bar_sync();  // keys_smem is rewritten by the next item
             }
         }
+        if (et == 0) TS(6);
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc_rt(tmem_base, tmem_cols);
+    if (threadIdx.x == 32) TS(7);
 }
 
-// debug / bring-up reference: same contraction on CUDA cores from the tiled weight layout
-// (exact products, fp32 accumulation).  Used only when EV_NAIVE_GEMM=1 to bisect tensor-core issues.
+// debug / bring-up reference: same contraction on CUDA cores from the tiled weight layout (exact products,
+// fp32 accumulation), raw output like EPI_RAW.  Used only when EV_NAIVE_GEMM=1 to bisect tensor-core issues.
 __global__ void __launch_bounds__(128) gemm_e4m3_naive_kernel(const uint8_t* __restrict__ X, const uint8_t* __restrict__ Wt,
-                                                              int M, int N, int K, int total_kb, const float* sx,
-                                                              const float* sw, float* out, int ldo, int add_resid) {
+                                                              int M, int N, int K, int total_kb, float* out, int ldo) {
     const int n = blockIdx.x * 128 + threadIdx.x, m = blockIdx.y;
     if (n >= N) return;
     float acc = 0.f;
@@ -303,9 +310,7 @@ __global__ void __launch_bounds__(128) gemm_e4m3_naive_kernel(const uint8_t* __r
         const __half_raw hw = __nv_cvt_fp8_to_halfraw(wc, __NV_E4M3);
         acc = fmaf(__half2float(__half(hx)), __half2float(__half(hw)), acc);
     }
-    const float y = mul_rn(mul_rn(acc, sx[m]), sw[n]);
-    float* p = out + (size_t)m * ldo + n;
-    *p = add_resid ? add_rn(*p, y) : y;
+    out[(size_t)m * ldo + n] = acc;
 }
 
 // tiled+swizzled codes -> row-major [rows][cols] (ev_model_get_quantized)
