@@ -357,10 +357,11 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     int n_splits;
     {
         const long base = (long)B * cfg.n_kv_heads * row_groups;
-        long want = (2L * m->num_sms + base - 1) / base;
+        long want = std::max(1L, (long)m->num_sms / base);  // one wave of CTAs
         const long chunks = (max_keys + ATT_CH - 1) / ATT_CH;
         want = std::max(1L, std::min(want, chunks));
         want = std::min(want, std::max(1L, m->split_rows_budget / M));
+        want = std::min(want, 64L);  // merge kernel's shared-memory table
         n_splits = (int)want;
     }
     int split_len = (int)round_up((max_keys + n_splits - 1) / n_splits, ATT_CH);
@@ -410,6 +411,8 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         aa.page_size = cfg.page_size; aa.seq_slots = in->dev_seq_slots; aa.Lsnap = m->Lsnap; aa.nn_eff = m->nn_eff;
         aa.anc = m->anc; aa.split_len = split_len; aa.n_splits = n_splits; aa.scale = 1.0f / sqrtf((float)D);
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
+        aa.ts = (m->gemm_dbg & 32) ? m->dbg_ts + 512 : nullptr;
+        if (aa.ts && l == 1) fprintf(stderr, "[attn] grid (%d,%d,%d) split_len %d\n", n_splits, cfg.n_kv_heads * row_groups, B, split_len);
         dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
@@ -417,14 +420,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         }
         MergeArgs ma;
         ma.T = T; ma.Hq = cfg.n_q_heads; ma.D = D; ma.n_splits = n_splits; ma.split_len = split_len;
-        ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part; ma.attn = m->attn;
+        ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part;
+        ma.attn = (tap && out->dev_tap_attn) ? out->dev_tap_attn : nullptr;
         ma.q = quant_out(m, m->aq, 4 * l + 1);
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
-            attn_merge_quant_kernel<<<M, EW_THREADS, 0, st>>>(ma);
+            attn_merge_quant_kernel<<<M, MERGE_THREADS, (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st>>>(ma);
             LAUNCH_CHECK();
         }
-        if (tap && out->dev_tap_attn) EV_TRY(copy_f32(st, m->attn, out->dev_tap_attn, (long)M * m->q_dim));
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
         EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_O));
@@ -510,6 +513,8 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     if (cfg->head_dim != 64 && cfg->head_dim != 128) return fail(EV_EINVAL, "head_dim must be 64 or 128");
     if (cfg->n_q_heads % cfg->n_kv_heads) return fail(EV_EINVAL, "n_q_heads must be a multiple of n_kv_heads");
     if (cfg->hidden % 16 || cfg->ffn % 16) return fail(EV_EINVAL, "hidden and ffn must be multiples of 16 (TMA row pitch)");
+    if (cfg->hidden > 4096 || cfg->ffn > 16384 || cfg->n_q_heads * cfg->head_dim > 4096)
+        return fail(EV_EINVAL, "hidden <= 4096, ffn <= 16384, n_q_heads*head_dim <= 4096 (register-resident rows)");
     if (cfg->page_size < 1 || cfg->page_size > 256) return fail(EV_EINVAL, "page_size out of range");
     if (cfg->max_tree_nodes < 1 || cfg->max_tree_nodes > EV_MAX_TREE_NODES) return fail(EV_EINVAL, "max_tree_nodes must be 1..64");
     if (cfg->max_batch < 1 || cfg->max_ctx < 1) return fail(EV_EINVAL, "max_batch / max_ctx must be positive");
@@ -1075,6 +1080,10 @@ int ev_debug_gemm_timestamps(ev_model* m, unsigned long long* host_out, int n_ct
     if (!m || !host_out) return fail(EV_EINVAL, "null argument");
     CUDA_TRY(cudaDeviceSynchronize());
     if (n_ctas > 128) n_ctas = 128;
+    if (n_ctas < 0) {  // attention timestamps
+        CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts + 512, 16 * 8, cudaMemcpyDeviceToHost));
+        return EV_OK;
+    }
     CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts, (size_t)n_ctas * 8 * 8, cudaMemcpyDeviceToHost));
     return EV_OK;
 }

@@ -38,6 +38,7 @@ struct AttnArgs {
     float scale;                // 1/sqrt(D)
     float* o_part;              // [M][Hq][n_splits][D]
     float* ml_part;             // [M][Hq][n_splits][2]  (running max, running sum)
+    unsigned long long* ts;     // bring-up: phase timestamps of CTA (0,0,0), or null
 };
 
 __device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
@@ -50,7 +51,7 @@ __device__ __forceinline__ void ldsm_x4_trans(uint32_t addr, uint32_t& r0, uint3
 }
 // D(16x8, fp32) += A(16x16 bf16, row) * B(16x8 bf16, col)
 __device__ __forceinline__ void mma_bf16(float* d, const uint32_t* a, uint32_t b0, uint32_t b1) {
-    asm volatile(
+    asm(
         "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
         : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -71,8 +72,10 @@ __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsr
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(sz) : "memory");
 }
 
+#define ATS(i) do { if (a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); a.ts[i] = t_; } } while (0)
 template <int D>
 __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnArgs a) {
+    ATS(0);
     constexpr int ROWB = D * 2;           // bytes per key row
     constexpr int CPR = ROWB / 16;        // 16-byte chunks per row
     constexpr int TILE = ATT_CH * ROWB;   // bytes per K (or V) tile
@@ -83,15 +86,16 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
     const int b = blockIdx.z;
-    const int nn = a.nn_eff[b];
-    if (nn == 0) return;
+    const int nn = a.nn_eff[b];     // the three scalars are loaded together, before the first branch
     const int L = a.Lsnap[b];
+    const int seq_slot = a.seq_slots[b];
+    if (nn == 0) return;
     const int n_keys = L + nn;
     const int k_begin = split * a.split_len;
     if (k_begin >= n_keys) return;
     const int k_end = min(k_begin + a.split_len, n_keys);
     const int n_chunks = (k_end - k_begin + ATT_CH - 1) / ATT_CH;
-    const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+    const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int R = a.T * a.G;
@@ -128,6 +132,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
         }
         __syncwarp();
     }
+    ATS(1);
 
     // ---- page gather: chunk ch -> stage ----
     auto load_chunk = [&](int stage, int ch) {
@@ -163,6 +168,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
             cp_async_wait<0>();
         }
         __syncthreads();
+        if (ch < 4) ATS(2 + 2 * ch);
         if (active) {
             const uint32_t ks = smem_u32(att_smem + (ch & 1) * 2 * TILE);
             const uint32_t vs = ks + TILE;
@@ -186,15 +192,20 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                     }
                 }
 #pragma unroll
-                for (int nt = 0; nt < ATT_CH / 8; ++nt) {
-                    const int r = nt * 8 + (lane & 7);
-                    const int c = kp * 4 + (lane >> 3);
-                    uint32_t b0, b1, b2, b3;
-                    ldsm_x4(ks + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
+                for (int nt4 = 0; nt4 < ATT_CH / 32; ++nt4) {  // four n-tiles at a time: four independent accumulator chains
+                    uint32_t bk[4][4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int r = (nt4 * 4 + u) * 8 + (lane & 7);
+                        const int c = kp * 4 + (lane >> 3);
+                        ldsm_x4(ks + r * ROWB + ((c ^ (r & 7)) * 16), bk[u][0], bk[u][1], bk[u][2], bk[u][3]);
+                    }
 #pragma unroll
                     for (int part = 2; part >= 0; --part) {  // smallest parts first
-                        mma_bf16(s[nt], qa[0][part], b0, b1);
-                        mma_bf16(s[nt], qa[1][part], b2, b3);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) mma_bf16(s[nt4 * 4 + u], qa[0][part], bk[u][0], bk[u][1]);
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) mma_bf16(s[nt4 * 4 + u], qa[1][part], bk[u][2], bk[u][3]);
                     }
                 }
             }
@@ -247,14 +258,20 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                 split3(s[2 * kt2 + 1][2], s[2 * kt2 + 1][3], pp[0][3], pp[1][3], pp[2][3]);
                 const int r = kt2 * 16 + ((lane >> 3) & 1) * 8 + (lane & 7);
 #pragma unroll
-                for (int np = 0; np < D / 16; ++np) {
-                    const int c = np * 2 + (lane >> 4);
-                    uint32_t b0, b1, b2, b3;
-                    ldsm_x4_trans(vs + r * ROWB + ((c ^ (r & 7)) * 16), b0, b1, b2, b3);
+                for (int np2 = 0; np2 < D / 32; ++np2) {  // four n-tiles (32 dims) at a time: four independent chains
+                    uint32_t bv[2][4];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int c = (np2 * 2 + u) * 2 + (lane >> 4);
+                        ldsm_x4_trans(vs + r * ROWB + ((c ^ (r & 7)) * 16), bv[u][0], bv[u][1], bv[u][2], bv[u][3]);
+                    }
 #pragma unroll
                     for (int part = 2; part >= 0; --part) {
-                        mma_bf16(oc[2 * np], pp[part], b0, b1);
-                        mma_bf16(oc[2 * np + 1], pp[part], b2, b3);
+#pragma unroll
+                        for (int u = 0; u < 2; ++u) {
+                            mma_bf16(oc[(np2 * 2 + u) * 2], pp[part], bv[u][0], bv[u][1]);
+                            mma_bf16(oc[(np2 * 2 + u) * 2 + 1], pp[part], bv[u][2], bv[u][3]);
+                        }
                     }
                 }
             }
@@ -264,6 +281,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                 o[i][2] = fmaf(o[i][2], c1, oc[i][2]); o[i][3] = fmaf(o[i][3], c1, oc[i][3]);
             }
         }
+        if (ch < 4) ATS(3 + 2 * ch);
         __syncthreads();
     }
     if (!active) return;
@@ -285,50 +303,87 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
         for (int i = 0; i < D / 8; ++i) *reinterpret_cast<float2*>(op + i * 8) = make_float2(o[i][2], o[i][3]);
         if ((lane & 3) == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m1, l1);
     }
+    ATS(10);
 }
 
 // ---- merge of the key splits (fixed order 0..ns-1) + per-token absmax + E4M3 quantize -----------
+// One CTA of 512 threads per token.  Phase 1 stages the (max, sum) pairs of all heads x splits in shared
+// memory, phase 2 turns them into softmax weights w[h][s] = exp(m_s - max) and the denominator per head,
+// phase 3 forms out = (sum_s w_s O_s) / den with all S partial loads of a thread in flight at once; the
+// merged row stays in registers for the quantizer.
 struct MergeArgs {
     int T, Hq, D, n_splits, split_len;
     const int32_t* Lsnap;
     const int32_t* nn_eff;
     const float* o_part;
     const float* ml_part;
-    float* attn;   // [M][Hq*D] fp32 merged output (workspace; also the debug tap)
+    float* attn;   // optional [M][Hq*D] fp32 merged output (debug tap) or null
     QuantOut q;
 };
-__global__ void __launch_bounds__(EW_THREADS) attn_merge_quant_kernel(MergeArgs a) {
+constexpr int MERGE_THREADS = 512;
+constexpr int MERGE_NV4 = 2;   // Hq*D <= 4096
+__global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeArgs a) {
     pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
-    __shared__ float red[EW_THREADS / 32];
+    extern __shared__ float msm[];             // w[Hq][S] | l[Hq][S] | den[Hq]
+    __shared__ float red[MERGE_THREADS / 32];
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
     const int nn = a.nn_eff[b];
-    const int K = a.Hq * a.D;
-    float* out = a.attn + (size_t)m * K;
+    const int K = a.Hq * a.D, S = a.n_splits;
     const bool valid = node < nn;
     const int ns = valid ? (a.Lsnap[b] + nn + a.split_len - 1) / a.split_len : 0;
-    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4) {
-        float4 r = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (valid) {
-            const int h = i / a.D, d = i % a.D;
-            const size_t pi = ((size_t)m * a.Hq + h) * a.n_splits;
-            float mx = -INFINITY;
-            for (int s = 0; s < ns; ++s) mx = fmaxf(mx, a.ml_part[(pi + s) * 2]);
-            float den = 0.f;
-            float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
-            for (int s = 0; s < ns; ++s) {
-                const float2 ml = *reinterpret_cast<const float2*>(a.ml_part + (pi + s) * 2);
-                const float w = (ml.x == -INFINITY) ? 0.f : expf(ml.x - mx);
-                const float4 ov = *reinterpret_cast<const float4*>(a.o_part + (pi + s) * a.D + d);
-                den += w * ml.y;
-                num.x += w * ov.x; num.y += w * ov.y; num.z += w * ov.z; num.w += w * ov.w;
-            }
-            r = make_float4(div_rn(num.x, den), div_rn(num.y, den), div_rn(num.z, den), div_rn(num.w, den));
-        }
-        *reinterpret_cast<float4*>(out + i) = r;
+    float* w = msm;
+    float* ls = msm + a.Hq * S;
+    float* den = ls + a.Hq * S;
+    for (int i = threadIdx.x; i < a.Hq * S; i += MERGE_THREADS) {
+        const int h = i / S, sp = i % S;
+        float2 ml = make_float2(-INFINITY, 0.f);
+        if (sp < ns) ml = __ldcg(reinterpret_cast<const float2*>(a.ml_part + (((size_t)m * a.Hq + h) * S + sp) * 2));
+        w[i] = ml.x;
+        ls[i] = ml.y;
     }
     __syncthreads();
-    quantize_row(m, K, [&](int i) -> float { return out[i]; }, a.q, red);
+    if ((int)threadIdx.x < a.Hq) {
+        const int h = threadIdx.x;
+        float mx = -INFINITY;
+        for (int sp = 0; sp < ns; ++sp) mx = fmaxf(mx, w[h * S + sp]);
+        float d = 0.f;
+        for (int sp = 0; sp < ns; ++sp) {
+            const float ms = w[h * S + sp];
+            const float wt = (ms == -INFINITY) ? 0.f : expf(ms - mx);
+            w[h * S + sp] = wt;
+            d += wt * ls[h * S + sp];
+        }
+        den[h] = d;
+    }
+    __syncthreads();
+    float4 v[MERGE_NV4];
+#pragma unroll
+    for (int k = 0; k < MERGE_NV4; ++k) {
+        const int i = (threadIdx.x + k * MERGE_THREADS) * 4;
+        v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (i < K && valid) {
+            const int h = i / a.D, d = i % a.D;
+            const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * a.D + d;
+            float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int s0 = 0; s0 < ns; s0 += 8) {
+                float4 t[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (s0 + u < ns) t[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)(s0 + u) * a.D));
+#pragma unroll
+                for (int u = 0; u < 8; ++u)
+                    if (s0 + u < ns) {
+                        const float wt = w[h * S + s0 + u];
+                        num.x += wt * t[u].x; num.y += wt * t[u].y; num.z += wt * t[u].z; num.w += wt * t[u].w;
+                    }
+            }
+            const float dn = den[h];
+            v[k] = make_float4(div_rn(num.x, dn), div_rn(num.y, dn), div_rn(num.z, dn), div_rn(num.w, dn));
+        }
+        if (i < K && a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
+    }
+    quantize_regs<MERGE_NV4>(v, m, K, a.q, red);
 }
 
 }  // namespace ev
