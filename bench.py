@@ -184,6 +184,23 @@ def oracle_sample(spec, steps, warmup, log):
                        f"{t_layer:.2f}s/layer, LM head {t_lm:.2f}s")
 
 
+# ------------------------------------------------------------------------------------------ multi-rank host logic
+
+def max_over_ranks(x, dist, device):
+    """Replicas only: the one cross-rank exchange is the MAX of a timing."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank, world, ms_per_step):
+    """Aggregate throughput of `world` independent replicas that each process units_per_rank per step."""
+    return world * units_per_rank / (ms_per_step * 1e-3)
+
+
 # ------------------------------------------------------------------------------------------ main
 
 def main():
@@ -263,10 +280,7 @@ def main():
     launches = ev.ev_launch_count()
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dist, "cuda")
     ms_step = ms / args.steps
     acc = buf.accept_len.cpu().numpy()
     assert (buf.status.cpu().numpy() == 0).all(), "a sequence was rejected during the timed steps"
@@ -314,10 +328,7 @@ def main():
         cache.ev_cache_set_lens(slots, L0)
         ev.ev_verify_host(model, cache, host)      # synchronises internally
     e2e_ms = 1e3 * (time.perf_counter() - t0)
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     assert np.array_equal(host["accept_len"].numpy(), acc)
     emitted = int((acc + 1).sum())
     if rank != 0:
@@ -327,7 +338,7 @@ def main():
         r = oracle_sample(spec, 4, 1, log)
         cpu = {"value": round(r["value"], 3), "unit": "tree-tokens/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
     line = {
-        "metric": METRIC, "value": round(world * B * T / (ms_step * 1e-3), 1), "unit": "tree-tokens/s", "n_gpus": world,
+        "metric": METRIC, "value": round(whole_job_rate(B * T, world, ms_step), 1), "unit": "tree-tokens/s", "n_gpus": world,
         "steps": args.steps, "warmup": warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "e4m3 x e4m3 -> f32 (bf16 KV, f32 residual)", "data": "synthetic",
         "config": {"workload": spec.name, "batch_per_gpu": B, "tree_nodes": T, "context": L0 if B <= 4 else [min(L0), max(L0)],
@@ -340,7 +351,7 @@ def main():
                           "weight_bytes": work["weight_bytes"], "kv_bytes": work["kv_bytes"], "flops": work["flops"]},
         "roofline": roofline,
         "cpu_baseline": cpu,
-        "e2e": {"value": round(world * B * T / (e2e_ms / args.steps * 1e-3), 1), "unit": "tree-tokens/s",
+        "e2e": {"value": round(whole_job_rate(B * T, world, e2e_ms / args.steps), 1), "unit": "tree-tokens/s",
                 "ms_per_step": round(e2e_ms / args.steps, 4), "h2d_bytes_per_step": (2 * B * T + B) * 4,
                 "d2h_bytes_per_step": (2 * B * T + 3 * B) * 4},
         "gpu_launches": int(launches), "clocks": clocks,
