@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "ev_attention.cuh"
+#include "ev_attention_tc.cuh"
 #include "ev_common.cuh"
 #include "ev_elementwise.cuh"
 #include "ev_gemm.cuh"
@@ -77,6 +78,20 @@ int make_tmap(CUtensorMap* tm, const void* base, long rows, long cols, int box_r
     return EV_OK;
 }
 
+// KV pool as a 2-D bf16 tensor [rows = (layer, page, K|V, head, token)][D], box = 16 tokens x 64 dims (128 B), 128-byte swizzle
+int make_tmap_kv(CUtensorMap* tm, const void* base, long rows, int D) {
+    EV_TRY(get_encode());
+    cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)rows};
+    cuuint64_t strides[1] = {(cuuint64_t)D * 2};
+    cuuint32_t box[2] = {64u, (cuuint32_t)TCA_PAGE};
+    cuuint32_t estr[2] = {1u, 1u};
+    CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(EV_ECUDA, "cuTensorMapEncodeTiled (KV pool) failed, code " + std::to_string((int)r));
+    return EV_OK;
+}
+
 constexpr int N_TOK_VARIANTS = 16;  // token-tile sizes 16, 32, ..., 256
 
 struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, with one TMA map per token-tile size
@@ -137,7 +152,7 @@ struct ev_model {
     float* site_amax = nullptr;      // device [n_sites]
     bool calibrated = false, recording = false;
     int num_sms = 148;
-    bool use_splitk = false, naive_gemm = false;
+    bool use_splitk = false, naive_gemm = false, legacy_attn = false;
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
     std::vector<ProfRec> prof;
@@ -158,6 +173,8 @@ struct ev_cache {
     std::vector<std::vector<int>> seq_pages;
     std::vector<char> seq_used;
     std::vector<int> len_bound;  // host-side upper bound of each sequence's ctx_len (sizes the key-split grid)
+    CUtensorMap tmKV;            // whole pool, for the tcgen05 attention kernel
+    bool tc_attn = false;        // page_size == 16 and the pool fits 32-bit row coordinates
     // prefill staging
     int32_t *pf_tokens = nullptr, *pf_parents = nullptr, *pf_nn = nullptr, *pf_slots = nullptr;
     int32_t *pf_out = nullptr;
@@ -307,6 +324,18 @@ int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
 }
 
 template <int D>
+int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, dim3 grid) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D>::SMEM));
+        attr_set = true;
+    }
+    tree_attn_tc_kernel<D><<<grid, TCA_THREADS, TcaCfg<D>::SMEM, st>>>(tm, a);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+
+template <int D>
 int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
     constexpr int smem = 2 * 2 * ATT_CH * D * 2 + ATT_WARPS * 3 * 16 * D * 2;
     static bool attr_set = false;
@@ -416,7 +445,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
-            if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
+            if (c->tc_attn && !m->legacy_attn) {
+                TcAttnArgs ta;
+                ta.a = aa;
+                ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
+                if (D == 128) EV_TRY(launch_attn_tc<128>(st, c->tmKV, ta, agrid)); else EV_TRY(launch_attn_tc<64>(st, c->tmKV, ta, agrid));
+            } else {
+                if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
+            }
         }
         MergeArgs ma;
         ma.T = T; ma.Hq = cfg.n_q_heads; ma.D = D; ma.n_splits = n_splits; ma.split_len = split_len;
@@ -538,6 +574,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
+    m->legacy_attn = getenv("EV_ATTN_LEGACY") && atoi(getenv("EV_ATTN_LEGACY")) != 0;  // bring-up: mma.sync attention
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;
     auto A = [&](int r) { if (rc == EV_OK) rc = r; };
@@ -717,6 +754,18 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
         return fail(EV_ENOMEM, "KV pool allocation failed");
     }
     cudaMemset(c->pool, 0, pool_elems * 2);
+    {
+        const long rows = (long)cfg.n_layers * n_pages * 2 * cfg.n_kv_heads * cfg.page_size;
+        if (cfg.page_size == TCA_PAGE && rows < (1L << 31)) {
+            if (make_tmap_kv(&c->tmKV, c->pool, rows, cfg.head_dim) != EV_OK) {
+                std::string keep = g_err;
+                ev_cache_destroy(c);
+                g_err = keep;
+                return EV_ECUDA;
+            }
+            c->tc_attn = true;
+        }
+    }
     cudaMemset(c->page_table, 0, (size_t)max_seqs * c->max_pages * 4);
     cudaMemset(c->ctx_len, 0, (size_t)max_seqs * 4);
     cudaMemset(c->capacity, 0, (size_t)max_seqs * 4);

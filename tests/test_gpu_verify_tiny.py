@@ -247,46 +247,71 @@ def test_status_codes_and_rejected_sequences(setup):
         cache.ev_cache_add_seq(100000)
 
 
-def test_gpu_speculative_loop_is_lossless_vs_oracle_greedy(setup):
-    """PAPER.md:92 on the GPU: the multi-step speculative loop (planted + random drafts) emits the oracle's
-    greedy sequence; positions after a sub-1e-3 top-2 gap are void."""
+def test_gpu_speculative_loop_is_lossless_teacher_forced(setup):
+    """PAPER.md:92 on the GPU: a multi-step speculative loop (planted + random drafts).  Multi-step free-running
+    comparison is not a fixed-tolerance statement (one E4M3 code flip moves a logit by up to ~0.05 sigma and the
+    sequences then diverge for good: DESIGN.md section 5), so the oracle is teacher-forced with the GPU's history:
+    at every step it verifies the SAME tree on a cache holding the SAME tokens, and every token the GPU emits must be
+    the oracle's argmax at that node -- literally where the oracle's top-2 gap >= 1e-3 AND the two sides' logits agree
+    within the 2e-2 sigma tolerance; a mismatch is only admissible where the oracle's margin between the two tokens is
+    below twice that logit tolerance (both sides within tolerance of each other), and at most 2 of the 24 positions.
+    Then the GPU's own token-by-token greedy decode of the emitted sequence must reproduce it (tree-verify logits ==
+    decode logits on the GPU), same admissibility rule."""
     from gpu_helpers import import_oracle_kv, run_verify
     spec, gm, om, ev = setup
     V = spec.model.vocab
     rng = np.random.default_rng(21)
     L, n_tok = 40, 24
     ids = rng.integers(0, V, L).astype(np.int32)
-    oc = _oracle_ctx(om, ids, cap=128)
-    # oracle greedy + its top-2 gaps
-    greedy, gaps, tok = [], [], 11
-    for _ in range(n_tok):
-        lg, _ = vo.forward_tree(om, oc, 0, np.array([tok]), np.array([-1]))
-        oc.ctx_len[0] += 1
-        s = np.sort(lg[0])
-        gaps.append(s[-1] - s[-2])
-        tok = int(np.argmax(lg[0]))
-        greedy.append(tok)
-    first_void = next((i for i, g in enumerate(gaps) if g < GAP), n_tok)
+    oc = _oracle_ctx(om, ids, cap=160)
+    greedy = vo.decode_greedy(om, _oracle_ctx(om, ids, cap=160), 0, 11, n_tok)   # only used to plant good drafts
     cache = ev.Cache(gm, 64, 4)
-    slot = cache.ev_cache_add_seq(128)
+    slot = cache.ev_cache_add_seq(160)
     import_oracle_kv(cache, slot, _oracle_ctx(om, ids), 0, L, 2)
     parents = wl.tree_parents(12, (3, 2, 2))
-    emitted, root, steps = [], 11, 0
-    buf = ev.VerifyBuffers(gm, 1, 12, want_logits=False, want_hidden=False)
+    emitted, root, steps, soft = [], 11, 0, 0
+    buf = ev.VerifyBuffers(gm, 1, 12, want_logits=True, want_hidden=False)
+    sigma = None
     while len(emitted) < n_tok:
         toks = rng.integers(0, V, 12).astype(np.int32)
         toks[0] = root
         cur, pos = 0, len(emitted)
-        for c in range(1, 12):          # plant the true continuation down the first-child chain
+        for c in range(1, 12):          # plant a plausible continuation down the first-child chain
             if parents[c] == cur and pos < n_tok and rng.random() < 0.8:
                 toks[c] = greedy[pos]
                 cur, pos = c, pos + 1
+        ref = vo.verify(om, oc, 0, toks, parents, commit=False)
+        sigma = sigma or float(ref["logits"].std())
         run_verify(gm, cache, [slot], toks[None], parents[None], commit=True, buf=buf)
         a = int(buf.accept_len.cpu()[0])
+        path = buf.accept_nodes.cpu().numpy()[0, :a + 1].tolist()
         out = buf.out_tokens.cpu().numpy()[0, :a + 1].tolist()
+        assert path[0] == 0 and all(parents[path[k + 1]] == path[k] for k in range(a))
+        assert out[:a] == [int(toks[c]) for c in path[1:]]
+        for k, node in enumerate(path):     # the token emitted after `node` must be the target argmax there
+            lg = ref["logits"][node]
+            top = int(np.argmax(lg))
+            if out[k] != top:
+                assert lg[top] - lg[out[k]] < 2 * TOL_LOGIT_SIGMA * sigma, (steps, k, lg[top] - lg[out[k]])
+                soft += 1
+        vo.kv_compact(oc, 0, path)          # oracle cache follows the GPU's accepted path
         emitted += out
         root = out[-1]
         steps += 1
-    n = min(first_void, n_tok)
-    assert emitted[:n] == greedy[:n]
+    assert soft <= 2, soft
     assert steps < n_tok, "speculation should accept drafts"
+    # GPU token-by-token greedy decode, teacher-forced on the emitted sequence, reproduces it
+    cache2 = ev.Cache(gm, 64, 4)
+    slot2 = cache2.ev_cache_add_seq(160)
+    import_oracle_kv(cache2, slot2, _oracle_ctx(om, ids), 0, L, 2)
+    one = ev.VerifyBuffers(gm, 1, 1, want_logits=True, want_hidden=False)
+    tok, soft2 = 11, 0
+    for i in range(n_tok):
+        run_verify(gm, cache2, [slot2], np.array([[tok]], np.int32), np.array([[-1]], np.int32), commit=True, buf=one)
+        lg = one.logits.cpu().numpy()[0]
+        top = int(np.argmax(lg))
+        if top != emitted[i]:
+            assert lg[top] - lg[emitted[i]] < 2 * TOL_LOGIT_SIGMA * sigma, (i, lg[top] - lg[emitted[i]])
+            soft2 += 1
+        tok = emitted[i]
+    assert soft2 <= 2, soft2
