@@ -121,6 +121,14 @@ enum ProfClass { PC_GEMM_QKV = 0, PC_GEMM_O, PC_GEMM_GATEUP, PC_GEMM_DOWN, PC_GE
                  PC_ROPE_KV, PC_SWIGLU, PC_OTHER, PC_COUNT };
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
+struct AttnPlan { int n_splits, split_len; };
+struct GraphKey {
+    int B, T, commit, force_all, n_splits, split_len, need_lm, pad;
+    const void* p[12];
+};
+struct GraphEntry { GraphKey key; cudaGraphExec_t exec; long launches; unsigned long stamp; };
+constexpr size_t MAX_GRAPHS = 16;
+
 }  // namespace
 
 struct ev_model {
@@ -153,10 +161,16 @@ struct ev_model {
     bool calibrated = false, recording = false;
     int num_sms = 148;
     bool use_splitk = false, naive_gemm = false, legacy_attn = false;
+    int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
     std::vector<ProfRec> prof;
     size_t prof_used = 0;
+    // captured verify steps (CUDA graphs), keyed by everything a launch depends on
+    bool use_graph = true;
+    cudaStream_t cap_stream = nullptr;
+    std::vector<GraphEntry> graphs;
+    unsigned long graph_clock = 0;
     std::vector<void*> allocs;
 };
 
@@ -230,6 +244,48 @@ int alloc_qmat(ev_model* m, QMat* q, long N, long K) {
     return EV_OK;
 }
 
+
+// Every kernel of the step is launched with the programmatic-stream-serialization attribute (PDL): it may
+// become resident while its predecessor is still running, and executes griddepcontrol.wait before touching
+// anything the predecessor wrote.  Under stream capture these launches become programmatic graph edges.
+bool g_use_pdl = true;
+template <class... KArgs, class... Args>
+int launch_kc(int cluster, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    int na = 0;
+    if (g_use_pdl) {
+        at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    if (cluster > 1) {  // grid.x counts CTAs: a multiple of the cluster size
+        at[na].id = cudaLaunchAttributeClusterDimension;
+        at[na].val.clusterDim.x = cluster; at[na].val.clusterDim.y = 1; at[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    cfg.attrs = at;
+    cfg.numAttrs = na;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, args...);
+    if (e != cudaSuccess) return fail(EV_ECUDA, std::string("kernel launch: ") + cudaGetErrorString(e));
+    ++g_launches;
+    return EV_OK;
+}
+template <class... KArgs, class... Args>
+int launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    return launch_kc(1, kern, grid, block, smem, st, args...);
+}
+// CTAs per token row of the element-wise kernels: spread few rows over all SMs
+int row_cluster(const ev_model* m, int M) {
+    if (m->row_cluster > 0) return m->row_cluster;
+    return M * 2 > m->num_sms ? 1 : (M * 4 > m->num_sms ? 2 : 4);
+}
+
 template <int EPI>
 int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int grid, int smem) {
     static bool attr_set = false;
@@ -260,7 +316,7 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     ProfScope prof_scope(m, st, prof_cls);
     if (lin) {
         lin->p = m->lin_out; lin->splits = 1; lin->ld = (int)w.N; lin->split_stride = (long)M * w.N;
-        lin->sx = x.scale; lin->sw = w.scale;
+        lin->sx = x.scale; lin->sw = w.scale; lin->sk_G = lin->sk_U = lin->sk_kb = 0;
     }
     if (m->naive_gemm && epi == EPI_RAW) {
         dim3 grid((unsigned)((w.N + 127) / 128), M);
@@ -281,28 +337,28 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     a.ldo = (int)w.N;
     a.dbg = m->gemm_dbg;
     a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
-    // split K when the tiles alone cannot fill the SMs evenly: pick the split count with the best wave efficiency.
-    // Splits cost nothing in the GEMM (each writes its own slab); the consumer reads `splits` values per element.
+    // Few token rows (one token tile): stream-K - the n_tiles * total_kb K-blocks are dealt out evenly to the
+    // CTAs (ev_gemm.cuh), each tile's pieces land in slabs the consumer adds in K order.  The partition depends
+    // only on the matrix shape and the SM count, never on M: a token's result is batch-invariant.
     const int G = m->num_sms;
     const int tiles = a.n_tiles * a.m_tiles;
-    int best = 1;
+    a.k_splits = 1;
+    a.kb_per_split = a.total_kb;
+    a.sk_units = 0;
+    int grid = std::min(tiles, G);
+    if (lin) { lin->splits = 1; lin->sk_G = 0; lin->sk_U = 0; lin->sk_kb = 0; }
     if (m->use_splitk && epi == EPI_RAW && a.m_tiles == 1) {
-        double best_score = 0.0;
-        for (int ks = 1; ks <= 8 && ks * 4 <= std::max(4, a.total_kb); ++ks) {
-            const int kbs = (a.total_kb + ks - 1) / ks;
-            if ((a.total_kb + kbs - 1) / kbs != ks) continue;
-            if ((long)ks * M * a.N > m->lin_floats) break;
-            const long items = (long)tiles * ks;
-            const long rounds = (items + G - 1) / G;
-            const double score = (double)items / (double)(rounds * G) / (1.0 + 0.02 * (ks - 1));
-            if (score > best_score + 1e-9) { best_score = score; best = ks; }
+        const int U = a.n_tiles * a.total_kb;
+        const int g = std::min(G, U);
+        int pmax = 1;
+        for (int t = 0; t < a.n_tiles; ++t)
+            pmax = std::max(pmax, sk_first_cta((t + 1) * a.total_kb - 1, g, U) - sk_first_cta(t * a.total_kb, g, U) + 1);
+        if (pmax <= 8 && (long)pmax * M * a.N <= m->lin_floats) {
+            a.sk_units = U;
+            grid = g;
+            if (lin) { lin->splits = pmax; lin->sk_G = g; lin->sk_U = U; lin->sk_kb = a.total_kb; }
         }
     }
-    a.k_splits = best;
-    a.kb_per_split = (a.total_kb + best - 1) / best;
-    if (lin) lin->splits = best;
-    const int items = tiles * a.k_splits;
-    const int grid = std::min(items, G);
     const int smem = a.stages * stage_bytes + 512 + 2048 + 8192 + 1024;  // stages + barriers + sx staging + argmax keys + alignment slack
     const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
     if (epi == EPI_RAW) return launch_gemm<EPI_RAW>(st, tmX, a, grid, smem);
@@ -330,9 +386,7 @@ int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, 
         CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D>::SMEM));
         attr_set = true;
     }
-    tree_attn_tc_kernel<D><<<grid, TCA_THREADS, TcaCfg<D>::SMEM, st>>>(tm, a);
-    LAUNCH_CHECK();
-    return EV_OK;
+    return launch_k(tree_attn_tc_kernel<D>, grid, dim3(TCA_THREADS), TcaCfg<D>::SMEM, st, tm, a);
 }
 
 template <int D>
@@ -343,14 +397,42 @@ int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
         CUDA_TRY(cudaFuncSetAttribute(tree_attn_partial_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;
     }
-    tree_attn_partial_kernel<D><<<grid, ATT_THREADS, smem, st>>>(a);
-    LAUNCH_CHECK();
-    return EV_OK;
+    return launch_k(tree_attn_partial_kernel<D>, grid, dim3(ATT_THREADS), smem, st, a);
+}
+
+
+// key-split plan for attention: enough CTAs for one wave, bounded by the partial-output workspace.  The key
+// bound (host-side upper bound of ctx_len + T over the batch) is rounded up to 256 so that the plan - and with
+// it the captured graph - only changes when a sequence crosses such a boundary; the kernels read the true
+// lengths on the device and skip empty splits.  Also advances the host-side length bounds on commit.
+AttnPlan plan_attention(ev_model* m, ev_cache* c, const ev_verify_in* in) {
+    const ev_config& cfg = m->cfg;
+    const int B = in->n_seqs, T = in->n_nodes_max, M = B * T;
+    const int R = T * (cfg.n_q_heads / cfg.n_kv_heads);
+    const int row_groups = (R + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
+    int max_keys = 0;
+    for (int i = 0; i < c->max_seqs; ++i)
+        if (c->seq_used[i]) max_keys = std::max(max_keys, c->len_bound[i]);
+    max_keys = (int)round_up(max_keys + T, 256);
+    if (in->commit)
+        for (int i = 0; i < c->max_seqs; ++i)
+            if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * cfg.page_size);
+    AttnPlan p;
+    const long base = (long)B * cfg.n_kv_heads * row_groups;
+    long want = std::max(1L, (long)m->num_sms / base);  // one wave of CTAs
+    const long chunks = (max_keys + ATT_CH - 1) / ATT_CH;
+    want = std::max(1L, std::min(want, chunks));
+    want = std::min(want, std::max(1L, m->split_rows_budget / M));
+    want = std::min(want, 64L);  // merge kernel's shared-memory table
+    p.n_splits = (int)want;
+    p.split_len = (int)round_up((max_keys + p.n_splits - 1) / p.n_splits, ATT_CH);
+    p.n_splits = (max_keys + p.split_len - 1) / p.split_len;
+    return p;
 }
 
 // the verify-step schedule; max_keys_hint: upper bound of ctx_len + T over the
 // batch known to the host (sizes the key-split grid; the kernels read the true lengths on the device)
-int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* out, cudaStream_t st, bool need_lm) {
+int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* out, cudaStream_t st, bool need_lm, AttnPlan plan) {
     const ev_config& cfg = m->cfg;
     const int B = in->n_seqs, T = in->n_nodes_max, M = B * T;
     const int H = cfg.hidden, D = cfg.head_dim, F = cfg.ffn;
@@ -361,50 +443,29 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     tp.ctx_len = c->ctx_len; tp.capacity = c->capacity; tp.max_seqs = c->max_seqs; tp.max_pos = m->max_pos;
     tp.Lsnap = m->Lsnap; tp.nn_eff = m->nn_eff; tp.status = out->dev_status; tp.depth = m->depth; tp.pos = m->pos;
     tp.anc = m->anc; tp.argmax_keys = m->argmax_keys;
-    tree_prep_kernel<<<(B + 63) / 64, 64, 0, st>>>(tp);
-    LAUNCH_CHECK();
+    EV_TRY(launch_k(tree_prep_kernel, dim3((B + 63) / 64), dim3(64), 0, st, tp));
 
     const float* ovr = in->dev_hidden_override;
     if (ovr) {
         EV_TRY(copy_f32(st, ovr, m->h, (long)M * H));
     } else {
-        embed_gather_kernel<<<M, EW_THREADS, 0, st>>>(in->dev_tokens, cfg.vocab, m->embed, H, m->h);
-        LAUNCH_CHECK();
+        EV_TRY(launch_k(embed_gather_kernel, dim3(M), dim3(EW_THREADS), 0, st, in->dev_tokens, cfg.vocab, m->embed, H, m->h));
     }
     if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden, (long)M * H));
 
-    // key-split plan for attention: enough CTAs for ~2 waves, bounded by the partial-output workspace
-    const int R = T * (cfg.n_q_heads / cfg.n_kv_heads);
-    const int row_groups = (R + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
-    int max_keys = 0;
-    for (int i = 0; i < c->max_seqs; ++i)
-        if (c->seq_used[i]) max_keys = std::max(max_keys, c->len_bound[i]);
-    max_keys = std::min(max_keys + T, cfg.max_ctx);
-    if (in->commit)
-        for (int i = 0; i < c->max_seqs; ++i)
-            if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * cfg.page_size);
-    int n_splits;
-    {
-        const long base = (long)B * cfg.n_kv_heads * row_groups;
-        long want = std::max(1L, (long)m->num_sms / base);  // one wave of CTAs
-        const long chunks = (max_keys + ATT_CH - 1) / ATT_CH;
-        want = std::max(1L, std::min(want, chunks));
-        want = std::min(want, std::max(1L, m->split_rows_budget / M));
-        want = std::min(want, 64L);  // merge kernel's shared-memory table
-        n_splits = (int)want;
-    }
-    int split_len = (int)round_up((max_keys + n_splits - 1) / n_splits, ATT_CH);
-    n_splits = (max_keys + split_len - 1) / split_len;
+    const int n_splits = plan.n_splits, split_len = plan.split_len;
+    const int CL = row_cluster(m, M);
+    const int row_groups = (T * (cfg.n_q_heads / cfg.n_kv_heads) + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
 
     LinOut pend;           // raw output of the last O / down GEMM, not yet added to the residual stream
     pend.p = nullptr;
     LinOut none;
     none.p = nullptr; none.splits = 0; none.ld = 0; none.split_stride = 0; none.sx = nullptr; none.sw = nullptr;
+    none.sk_G = none.sk_U = none.sk_kb = 0;
     pend = none;
     auto materialize = [&]() -> int {  // h += pending (only for debug taps; the fast path fuses this into RMSNorm)
         if (!pend.p) return EV_OK;
-        apply_pending_kernel<<<M, 256, 0, st>>>(m->h, H, pend);
-        LAUNCH_CHECK();
+        EV_TRY(launch_k(apply_pending_kernel, dim3(M), dim3(256), 0, st, m->h, H, pend));
         pend = none;
         return EV_OK;
     };
@@ -416,8 +477,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // --- attention block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0));
-            LAUNCH_CHECK();
+            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0)));
             pend = none;
         }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
@@ -430,8 +490,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ra.pool = c->pool + (size_t)l * c->layer_stride;
         {
             ProfScope ps(m, st, PC_ROPE_KV);
-            rope_kvwrite_kernel<<<M, ROPE_THREADS, 0, st>>>(ra);
-            LAUNCH_CHECK();
+            EV_TRY(launch_k(rope_kvwrite_kernel, dim3(M, CL), dim3(CL > 1 ? 256 : ROPE_THREADS), 0, st, ra));
         }
         if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
         AttnArgs aa;
@@ -461,8 +520,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ma.q = quant_out(m, m->aq, 4 * l + 1);
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
-            attn_merge_quant_kernel<<<M, MERGE_THREADS, (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st>>>(ma);
-            LAUNCH_CHECK();
+            EV_TRY(launch_kc(CL, attn_merge_quant_kernel, dim3(M * CL), dim3(MERGE_THREADS), (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st, ma));
         }
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
@@ -471,16 +529,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // --- MLP block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2));
-            LAUNCH_CHECK();
+            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2)));
             pend = none;
         }
         LinOut gul;
         EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_RAW, &gul, nullptr, nullptr, PC_GEMM_GATEUP));
         {
             ProfScope ps(m, st, PC_SWIGLU);
-            swiglu_quant_kernel<<<M, SWI_THREADS, 0, st>>>(gul, F, (tap ? out->dev_tap_gu : nullptr), quant_out(m, m->tq, 4 * l + 3));
-            LAUNCH_CHECK();
+            EV_TRY(launch_kc(CL, swiglu_quant_kernel, dim3(M * CL), dim3(SWI_THREADS), 0, st, gul, F, (tap ? out->dev_tap_gu : nullptr), quant_out(m, m->tq, 4 * l + 3)));
         }
         if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
@@ -491,8 +547,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         if (lockstep) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H)); }
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            rmsnorm_quant_kernel<<<M, NORM_THREADS, 0, st>>>(m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers));
-            LAUNCH_CHECK();
+            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers)));
             pend = none;
         }
         EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM));
@@ -503,15 +558,13 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     ac.Lsnap = m->Lsnap; ac.seq_slots = in->dev_seq_slots; ac.argmax_keys = m->argmax_keys; ac.argmax_out = out->dev_argmax;
     ac.accept_len = out->dev_accept_len; ac.accept_nodes = out->dev_accept_nodes; ac.out_tokens = out->dev_out_tokens;
     ac.new_ctx_len = out->dev_new_ctx_len; ac.ctx_len = c->ctx_len;
-    accept_walk_kernel<<<(B + 63) / 64, 64, 0, st>>>(ac);
-    LAUNCH_CHECK();
+    EV_TRY(launch_k(accept_walk_kernel, dim3((B + 63) / 64), dim3(64), 0, st, ac));
     if (in->commit && !in->force_accept_all) {
         CompactArgs ca;
         ca.T = T; ca.Hkv = cfg.n_kv_heads; ca.D = D; ca.page_size = cfg.page_size; ca.max_pages = c->max_pages;
         ca.layer_stride = c->layer_stride; ca.pool = c->pool; ca.page_table = c->page_table; ca.seq_slots = in->dev_seq_slots;
         ca.Lsnap = m->Lsnap; ca.accept_len = out->dev_accept_len; ca.accept_nodes = out->dev_accept_nodes;
-        kv_compact_kernel<<<dim3(B, cfg.n_layers), EW_THREADS, 0, st>>>(ca);
-        LAUNCH_CHECK();
+        EV_TRY(launch_k(kv_compact_kernel, dim3(dim3(B, cfg.n_layers)), dim3(EW_THREADS), 0, st, ca));
     }
     return EV_OK;
 }
@@ -574,6 +627,9 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
+    m->row_cluster = getenv("EV_ROW_CLUSTER") ? atoi(getenv("EV_ROW_CLUSTER")) : 0;
+    m->use_graph = !(getenv("EV_GRAPH") && atoi(getenv("EV_GRAPH")) == 0);          // on by default
+    g_use_pdl = !(getenv("EV_PDL") && atoi(getenv("EV_PDL")) == 0);                // on by default
     m->legacy_attn = getenv("EV_ATTN_LEGACY") && atoi(getenv("EV_ATTN_LEGACY")) != 0;  // bring-up: mma.sync attention
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;
@@ -639,6 +695,8 @@ int ev_model_destroy(ev_model* m) {
     cudaDeviceSynchronize();
     for (void* p : m->allocs) cudaFree(p);
     for (auto& r : m->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto& g : m->graphs) cudaGraphExecDestroy(g.exec);
+    if (m->cap_stream) cudaStreamDestroy(m->cap_stream);
     delete m;
     return EV_OK;
 }
@@ -781,6 +839,11 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
 int ev_cache_destroy(ev_cache* c) {
     if (!c) return EV_OK;
     cudaDeviceSynchronize();
+    if (c->model) {  // captured steps that reference this cache's buffers die with it
+        auto& gs = c->model->graphs;
+        for (size_t i = gs.size(); i-- > 0;)
+            if (gs[i].key.p[0] == (const void*)c) { cudaGraphExecDestroy(gs[i].exec); gs.erase(gs.begin() + i); }
+    }
     cudaFree(c->pool); cudaFree(c->page_table); cudaFree(c->ctx_len); cudaFree(c->capacity);
     cudaFree(c->pf_tokens); cudaFree(c->pf_parents); cudaFree(c->pf_nn); cudaFree(c->pf_slots); cudaFree(c->pf_out);
     delete c;
@@ -903,7 +966,59 @@ int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* o
         return fail(EV_EINVAL, "null required output array");
     const bool need_lm = !in->force_accept_all || m->recording;
     EV_TRY(check_ready(m, need_lm));
-    return run_forward(m, c, in, out, (cudaStream_t)stream, need_lm);
+    cudaStream_t st = (cudaStream_t)stream;
+    const AttnPlan plan = plan_attention(m, c, in);
+    // Fast path: the whole step (~330 launches, PDL edges included) is captured once per distinct argument set
+    // and replayed as one CUDA graph.  Debug taps, lock-step overrides, profiling and calibration run eagerly.
+    bool graph_ok = m->use_graph && !m->profile && !m->recording && !in->dev_hidden_override && !out->dev_hidden &&
+                    (out->tap_layer < 0 || out->tap_layer >= m->cfg.n_layers) && !(m->gemm_dbg & 48);
+    if (graph_ok) {
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) graph_ok = false;  // caller captures
+    }
+    if (!graph_ok) return run_forward(m, c, in, out, st, need_lm, plan);
+    GraphKey key;
+    memset(&key, 0, sizeof(key));
+    key.B = in->n_seqs; key.T = in->n_nodes_max; key.commit = in->commit; key.force_all = in->force_accept_all;
+    key.n_splits = plan.n_splits; key.split_len = plan.split_len; key.need_lm = need_lm;
+    const void* ptrs[12] = {c, in->dev_seq_slots, in->dev_tokens, in->dev_parents, in->dev_n_nodes, out->dev_accept_len,
+                            out->dev_accept_nodes, out->dev_out_tokens, out->dev_new_ctx_len, out->dev_status, out->dev_argmax,
+                            out->dev_logits};
+    memcpy(key.p, ptrs, sizeof(ptrs));
+    GraphEntry* hit = nullptr;
+    for (auto& g : m->graphs)
+        if (memcmp(&g.key, &key, sizeof(key)) == 0) { hit = &g; break; }
+    if (!hit) {
+        if (!m->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&m->cap_stream, cudaStreamNonBlocking));
+        const long before = g_launches;
+        CUDA_TRY(cudaStreamBeginCapture(m->cap_stream, cudaStreamCaptureModeRelaxed));
+        const int rc = run_forward(m, c, in, out, m->cap_stream, need_lm, plan);
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(m->cap_stream, &graph);
+        const long n_launch = g_launches - before;
+        g_launches = before;
+        if (rc != EV_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess || !graph) return fail(EV_ECUDA, std::string("graph capture: ") + cudaGetErrorString(e));
+        cudaGraphExec_t exec = nullptr;
+        const cudaError_t e2 = cudaGraphInstantiate(&exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) return fail(EV_ECUDA, std::string("graph instantiate: ") + cudaGetErrorString(e2));
+        if (m->graphs.size() >= MAX_GRAPHS) {  // evict the least recently used
+            size_t lru = 0;
+            for (size_t i = 1; i < m->graphs.size(); ++i)
+                if (m->graphs[i].stamp < m->graphs[lru].stamp) lru = i;
+            cudaGraphExecDestroy(m->graphs[lru].exec);
+            m->graphs.erase(m->graphs.begin() + lru);
+        }
+        GraphEntry ge;
+        ge.key = key; ge.exec = exec; ge.launches = n_launch; ge.stamp = 0;
+        m->graphs.push_back(ge);
+        hit = &m->graphs.back();
+    }
+    hit->stamp = ++m->graph_clock;
+    CUDA_TRY(cudaGraphLaunch(hit->exec, st));
+    g_launches += hit->launches;
+    return EV_OK;
 }
 
 int ev_cache_prefill(ev_model* m, ev_cache* c, int n_seqs, const int* host_seq_slots, const int32_t* host_token_ids,

@@ -75,6 +75,8 @@ __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsr
 #define ATS(i) do { if (a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); a.ts[i] = t_; } } while (0)
 template <int D>
 __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     ATS(0);
     constexpr int ROWB = D * 2;           // bytes per key row
     constexpr int CPR = ROWB / 16;        // 16-byte chunks per row
@@ -324,9 +326,11 @@ constexpr int MERGE_THREADS = 512;
 constexpr int MERGE_NV4 = 2;   // Hq*D <= 4096
 __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeArgs a) {
     pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
+    pdl_wait();
     extern __shared__ float msm[];             // w[Hq][S] | l[Hq][S] | den[Hq]
     __shared__ float red[MERGE_THREADS / 32];
-    const int m = blockIdx.x;
+    __shared__ float xch_f[CLUSTER_MAX];
+    const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     const int b = m / a.T, node = m % a.T;
     const int nn = a.nn_eff[b];
     const int K = a.Hq * a.D, S = a.n_splits;
@@ -358,11 +362,14 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
     }
     __syncthreads();
     float4 v[MERGE_NV4];
+    int c0, c1;
+    cluster_cols(K / 4, c0, c1);
 #pragma unroll
     for (int k = 0; k < MERGE_NV4; ++k) {
-        const int i = (threadIdx.x + k * MERGE_THREADS) * 4;
+        const int i4 = c0 + threadIdx.x + k * MERGE_THREADS;
+        const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (i < K && valid) {
+        if (i4 < c1 && valid) {
             const int h = i / a.D, d = i % a.D;
             const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * a.D + d;
             float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -381,9 +388,9 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
             const float dn = den[h];
             v[k] = make_float4(div_rn(num.x, dn), div_rn(num.y, dn), div_rn(num.z, dn), div_rn(num.w, dn));
         }
-        if (i < K && a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
+        if (i4 < c1 && a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
     }
-    quantize_regs<MERGE_NV4>(v, m, K, a.q, red);
+    quantize_regs<MERGE_NV4>(v, m, K, c0, c1, a.q, red, xch_f);
 }
 
 }  // namespace ev

@@ -140,19 +140,11 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
     const int b = blockIdx.z;
-    const int nn = a.nn_eff[b];
-    const int L = a.Lsnap[b];
-    const int seq_slot = a.seq_slots[b];
-    if (nn == 0) return;
-    const int n_keys = L + nn;
-    const int k_begin = split * a.split_len;
-    if (k_begin >= n_keys) return;
-    const int k_end = min(k_begin + a.split_len, n_keys);
-    const int n_tiles = (k_end - k_begin + TCA_BN - 1) / TCA_BN;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int R = a.T * a.G;
 
-    // ---- prologue: barriers, TMEM, Q tile (fp32 -> hi | mid | lo bf16, 128-byte swizzled K-major) ----
+    // ---- prologue that does not depend on the previous kernel (overlaps it under PDL): barriers, TMEM ----
+    pdl_launch_dependents();
     if (threadIdx.x == 0) {
         for (int s = 0; s < TCA_STAGES; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
@@ -162,6 +154,17 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         tma_prefetch_desc(&tmKV);
     }
     if (warp == 1) tmem_alloc<512>(tmem_base_smem);
+    pdl_wait();
+    const int nn = a.nn_eff[b];
+    const int L = a.Lsnap[b];
+    const int seq_slot = a.seq_slots[b];
+    const int n_keys = L + nn;
+    const int k_begin = split * a.split_len;
+    const bool active = nn != 0 && k_begin < n_keys;   // uniform over the CTA
+    const int k_end = min(k_begin + a.split_len, n_keys);
+    const int n_tiles = active ? (k_end - k_begin + TCA_BN - 1) / TCA_BN : 0;
+    // ---- Q tile (fp32 -> hi | mid | lo bf16, 128-byte swizzled K-major) ----
+    if (active)
     {
         constexpr int CPR = D / 8;  // 16-byte chunks (8 elements) per row
         for (int it = threadIdx.x; it < 128 * CPR; it += TCA_THREADS) {
@@ -193,7 +196,9 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
 
-    if (warp == 0) {
+    if (!active) {
+        // nothing to do for this (sequence, split): fall through to the TMEM release
+    } else if (warp == 0) {
         // ===== TMA producer: lane i issues box i of the tile (K|V, page, half) =====
         constexpr int OPS = 2 * 4 * C::NH;
         const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;

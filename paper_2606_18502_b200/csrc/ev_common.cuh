@@ -155,32 +155,43 @@ __host__ __device__ constexpr uint32_t umma_idesc_e4m3(int M, int N) {
 //   y[m][n] = (((p_0 + p_1) + ...) + p_{S-1}) * s_x[m] * s_w[n]        (fixed order: deterministic)
 // with single rounded fp32 operations, exactly the epilogue the method defines (DESIGN.md R-accum).
 struct LinOut {
-    const float* p;      // [splits][M][ld]
-    int splits, ld;
+    const float* p;      // [slabs][M][ld]
+    int splits, ld;      // splits: uniform slab count (classic split-K), or the maximum (stream-K)
     long split_stride;   // M * ld
     const float* sx;     // [M]
     const float* sw;     // [N]
+    int sk_G, sk_U, sk_kb;  // stream-K partition (ev_gemm.cuh): grid size, K-block units, K-blocks per tile; sk_U == 0 = classic
 };
-__device__ __forceinline__ float lin_acc(const LinOut& o, size_t idx) {
+// number of slabs that hold a piece of output channel n (all channels of a 128-row weight tile share it)
+__device__ __forceinline__ int lin_slabs(const LinOut& o, int n) {
+    if (o.sk_U == 0) return o.splits;
+    const unsigned t = (unsigned)n >> 7, G = (unsigned)o.sk_G, U = (unsigned)o.sk_U, kb = (unsigned)o.sk_kb;
+    const unsigned c_first = ((t * kb + 1u) * G + U - 1u) / U;   // first CTA touching the tile, + 1
+    const unsigned c_last = ((t + 1u) * kb * G + U - 1u) / U;    // last CTA touching it, + 1
+    return (int)(c_last - c_first) + 1;
+}
+__device__ __forceinline__ float lin_acc(const LinOut& o, size_t idx, int n) {
+    const int cnt = lin_slabs(o, n);
     float acc = __ldcg(o.p + idx);
-    for (int s = 1; s < o.splits; ++s) acc = __fadd_rn(acc, __ldcg(o.p + (size_t)s * o.split_stride + idx));
+    for (int s = 1; s < cnt; ++s) acc = __fadd_rn(acc, __ldcg(o.p + (size_t)s * o.split_stride + idx));
     return acc;
 }
 __device__ __forceinline__ float lin_value(const LinOut& o, int m, int n, float sxm) {
-    return __fmul_rn(__fmul_rn(lin_acc(o, (size_t)m * o.ld + n), sxm), __ldg(o.sw + n));
+    return __fmul_rn(__fmul_rn(lin_acc(o, (size_t)m * o.ld + n, n), sxm), __ldg(o.sw + n));
 }
 
-// four consecutive channels n..n+3 (n % 4 == 0, ld % 4 == 0): 16-byte loads, all splits in flight together
+// four consecutive channels n..n+3 (n % 4 == 0, ld % 4 == 0): 16-byte loads, all slabs in flight together
 __device__ __forceinline__ float4 lin_value4(const LinOut& o, int m, int n, float sxm) {
     const size_t idx = (size_t)m * o.ld + n;
+    const int cnt = lin_slabs(o, n);
     float4 acc = __ldcg(reinterpret_cast<const float4*>(o.p + idx));
     float4 t[7];
 #pragma unroll
     for (int s = 1; s < 8; ++s)
-        if (s < o.splits) t[s - 1] = __ldcg(reinterpret_cast<const float4*>(o.p + (size_t)s * o.split_stride + idx));
+        if (s < cnt) t[s - 1] = __ldcg(reinterpret_cast<const float4*>(o.p + (size_t)s * o.split_stride + idx));
 #pragma unroll
     for (int s = 1; s < 8; ++s)
-        if (s < o.splits) {
+        if (s < cnt) {
             acc.x = __fadd_rn(acc.x, t[s - 1].x); acc.y = __fadd_rn(acc.y, t[s - 1].y);
             acc.z = __fadd_rn(acc.z, t[s - 1].z); acc.w = __fadd_rn(acc.w, t[s - 1].w);
         }
@@ -195,6 +206,44 @@ __device__ __forceinline__ float4 lin_value4(const LinOut& o, int m, int n, floa
 // calls pdl_launch_dependents() as early as possible so the dependent's prologue overlaps it.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// ---- thread-block clusters: a token row of the element-wise kernels is spread over the CTAs of one cluster
+// (so that M = 60 rows still occupy all SMs); row statistics meet through distributed shared memory.
+// Push model: every CTA stores its value into slot [own rank] of every peer, one cluster barrier, then each CTA
+// reads its own shared memory in rank order (deterministic).  A launch without the cluster attribute is a
+// cluster of one CTA: the same code runs.
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_nctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_map(const void* local_smem, uint32_t rank) {
+    uint32_t ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(local_smem)), "r"(rank));
+    return ra;
+}
+constexpr int CLUSTER_MAX = 8;
+// v: a value every thread of the CTA already holds (block-reduced); xch: CLUSTER_MAX slots of shared memory,
+// used once per kernel.  All threads of all CTAs of the cluster must call.
+__device__ __forceinline__ float cluster_max(float v, float* xch) {
+    const uint32_t nct = cluster_nctarank();
+    if (nct == 1) return v;
+    if (threadIdx.x < nct) asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(cluster_map(xch + cluster_ctarank(), threadIdx.x)), "f"(v) : "memory");
+    cluster_barrier();
+    float r = xch[0];
+    for (uint32_t i = 1; i < nct; ++i) r = fmaxf(r, xch[i]);
+    return r;
+}
+__device__ __forceinline__ double cluster_sum(double v, double* xch) {
+    const uint32_t nct = cluster_nctarank();
+    if (nct == 1) return v;
+    if (threadIdx.x < nct) asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(cluster_map(xch + cluster_ctarank(), threadIdx.x)), "d"(v) : "memory");
+    cluster_barrier();
+    double r = xch[0];
+    for (uint32_t i = 1; i < nct; ++i) r += xch[i];
+    return r;
+}
 
 // ---- cp.async (Ampere-style, for the paged KV gathers) ------------------------------------------
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {

@@ -87,6 +87,8 @@ struct TreePrepArgs {
 };
 
 __global__ void tree_prep_kernel(TreePrepArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= a.B) return;
     const int T = a.T;
@@ -130,6 +132,8 @@ __global__ void tree_prep_kernel(TreePrepArgs a) {
 __global__ void __launch_bounds__(EW_THREADS) embed_gather_kernel(const int32_t* __restrict__ tokens, int vocab,
                                                                   const __nv_bfloat16* __restrict__ table, int H,
                                                                   float* __restrict__ h) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int m = blockIdx.x;
     const int tk = tokens[m];
     const bool ok = tk >= 0 && tk < vocab;
@@ -170,29 +174,38 @@ __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut
         dst[i >> 2] = e4m3x4(div_rn(val(i), s), div_rn(val(i + 1), s), div_rn(val(i + 2), s), div_rn(val(i + 3), s));
 }
 
-// row held in registers: thread t owns float4 number t + k*blockDim.x (k < NV4) of the row
+// row held in registers, spread over the CTAs of a cluster: this CTA owns the float4 numbers [c0, c1) of the
+// row and thread t owns c0 + t + k*blockDim.x (k < NV4).  The absmax meets across the cluster (cluster_max).
 template <int NV4>
-__device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int K, const QuantOut& q, float* red) {
+__device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int K, int c0, int c1, const QuantOut& q, float* red,
+                                              float* xch) {
     const int nthr = blockDim.x;
     float amax = 0.f;
 #pragma unroll
     for (int k = 0; k < NV4; ++k)
-        if ((threadIdx.x + k * nthr) * 4 < K)
+        if (c0 + (int)threadIdx.x + k * nthr < c1)
             amax = fmaxf(amax, fmaxf(fmaxf(fabsf(v[k].x), fabsf(v[k].y)), fmaxf(fabsf(v[k].z), fabsf(v[k].w))));
-    amax = block_max(amax, red);
+    amax = cluster_max(block_max(amax, red), xch);
     float s;
     if (q.static_scale) s = *q.static_scale;
     else s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0 && cluster_ctarank() == 0) {
         q.sx[m] = s;
         if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
     }
     uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
 #pragma unroll
     for (int k = 0; k < NV4; ++k) {
-        const int i4 = threadIdx.x + k * nthr;
-        if (i4 * 4 < K) dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
+        const int i4 = c0 + (int)threadIdx.x + k * nthr;
+        if (i4 < c1) dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
     }
+}
+// this CTA's share [c0, c1) of a row of n4 float4s
+__device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
+    const int nct = (int)cluster_nctarank(), r = (int)cluster_ctarank();
+    const int per = (n4 + nct - 1) / nct;
+    c0 = min(n4, r * per);
+    c1 = min(n4, c0 + per);
 }
 
 // ---- K3: (residual += pending linear output) + RMSNorm + quantize; one CTA of 256 threads per token;
@@ -204,18 +217,24 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
                                                                      const __nv_bfloat16* __restrict__ gain, float eps,
                                                                      QuantOut q) {
     pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
+    pdl_wait();
     __shared__ float red[NORM_THREADS / 32];
     __shared__ double dred[NORM_THREADS / 32];
-    const int m = blockIdx.x;
+    __shared__ float xch_f[CLUSTER_MAX];
+    __shared__ double xch_d[CLUSTER_MAX];
+    const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
+    int c0, c1;
+    cluster_cols(H / 4, c0, c1);
     float* x = h + (size_t)m * H;
     float4 v[NORM_NV4];
     const float sxm = pend.p ? __ldg(pend.sx + m) : 0.f;
     double acc = 0.0;  // mean of squares accumulated in fp64, rounded once (DESIGN.md R-accum)
 #pragma unroll
     for (int k = 0; k < NORM_NV4; ++k) {
-        const int i = (threadIdx.x + k * NORM_THREADS) * 4;
+        const int i4 = c0 + threadIdx.x + k * NORM_THREADS;
+        const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (i < H) {
+        if (i4 < c1) {
             v[k] = *reinterpret_cast<const float4*>(x + i);
             if (pend.p) {
                 const float4 y = lin_value4(pend, m, i, sxm);
@@ -231,12 +250,14 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
     double tot = 0.0;
 #pragma unroll
     for (int i = 0; i < NORM_THREADS / 32; ++i) tot += dred[i];
+    tot = cluster_sum(tot, xch_d);
     const float ms = (float)(tot / (double)H);
     const float r = div_rn(1.0f, sqrtf(add_rn(ms, eps)));
 #pragma unroll
     for (int k = 0; k < NORM_NV4; ++k) {
-        const int i = (threadIdx.x + k * NORM_THREADS) * 4;
-        if (i < H) {
+        const int i4 = c0 + threadIdx.x + k * NORM_THREADS;
+        const int i = i4 * 4;
+        if (i4 < c1) {
             float4 g = make_float4(1.f, 1.f, 1.f, 1.f);
             if (gain) g = make_float4(__bfloat162float(gain[i]), __bfloat162float(gain[i + 1]), __bfloat162float(gain[i + 2]),
                                       __bfloat162float(gain[i + 3]));
@@ -244,17 +265,21 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
                                mul_rn(mul_rn(v[k].w, r), g.w));
         }
     }
-    quantize_regs<NORM_NV4>(v, m, H, q, red);
+    quantize_regs<NORM_NV4>(v, m, H, c0, c1, q, red, xch_f);
 }
 
 // residual += pending linear output, nothing else (debug taps / end of a prefill pass)
 __global__ void __launch_bounds__(256) apply_pending_kernel(float* __restrict__ h, int H, LinOut pend) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int m = blockIdx.x;
     const float sxm = __ldg(pend.sx + m);
     for (int i = threadIdx.x; i < H; i += 256) h[(size_t)m * H + i] = add_rn(h[(size_t)m * H + i], lin_value(pend, m, i, sxm));
 }
 // y = linear output with its scales (ev_op_linear)
 __global__ void __launch_bounds__(256) materialize_linear_kernel(float* __restrict__ out, int N, LinOut lin) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int m = blockIdx.x;
     const float sxm = __ldg(lin.sx + m);
     for (int i = threadIdx.x; i < N; i += 256) out[(size_t)m * N + i] = lin_value(lin, m, i, sxm);
@@ -278,15 +303,20 @@ constexpr int SWI_THREADS = 512;
 constexpr int SWI_NV4 = 8;
 __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, int F, float* __restrict__ gu_tap, QuantOut q) {
     pdl_launch_dependents();  // the down-projection GEMM may start prefetching its weights now
+    pdl_wait();
     __shared__ float red[SWI_THREADS / 32];
-    const int m = blockIdx.x;
+    __shared__ float xch_f[CLUSTER_MAX];
+    const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
+    int c0, c1;
+    cluster_cols(F / 4, c0, c1);
     const float sxm = __ldg(gu.sx + m);
     float4 v[SWI_NV4];
 #pragma unroll
     for (int k = 0; k < SWI_NV4; ++k) {
-        const int i = (threadIdx.x + k * SWI_THREADS) * 4;
+        const int i4 = c0 + threadIdx.x + k * SWI_THREADS;
+        const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (i < F) {
+        if (i4 < c1) {
             const float4 g = lin_value4(gu, m, i, sxm), u = lin_value4(gu, m, F + i, sxm);
             if (gu_tap) {
                 *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + i) = g;
@@ -295,7 +325,7 @@ __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, in
             v[k] = make_float4(swiglu_f(g.x, u.x), swiglu_f(g.y, u.y), swiglu_f(g.z, u.z), swiglu_f(g.w, u.w));
         }
     }
-    quantize_regs<SWI_NV4>(v, m, F, q, red);
+    quantize_regs<SWI_NV4>(v, m, F, c0, c1, q, red, xch_f);
 }
 
 // ---- K4: RoPE (positions = L + depth) on q, k of the raw QKV GEMM output + K,V -> bf16 pages; q, k, v are
@@ -315,6 +345,8 @@ struct RopeArgs {
 };
 constexpr int ROPE_THREADS = 512;
 __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
     const int D = a.D, D2 = D / 2;
@@ -332,7 +364,8 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
         vdst = a.pool + base + (size_t)a.Hkv * a.page_size * D;
     }
     const int n_rot4 = (a.Hq + a.Hkv) * D2 / 4;  // groups of 4 rotation pairs
-    for (int i = threadIdx.x; i < n_rot4; i += ROPE_THREADS) {
+    const int tid = blockIdx.y * blockDim.x + threadIdx.x, nthr = gridDim.y * blockDim.x;  // a row may be spread over gridDim.y CTAs
+    for (int i = tid; i < n_rot4; i += nthr) {
         const int head = (i * 4) / D2, j = (i * 4) % D2;
         const float4 lo = lin_value4(a.lin, m, head * D + j, sxm), hi = lin_value4(a.lin, m, head * D + j + D2, sxm);
         const float4 c01 = __ldg(reinterpret_cast<const float4*>(cs + j)), c23 = __ldg(reinterpret_cast<const float4*>(cs + j + 2));
@@ -352,7 +385,7 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
         }
     }
     const int voff = (a.Hq + a.Hkv) * D;
-    for (int i = threadIdx.x; i < a.Hkv * D / 4; i += ROPE_THREADS) {
+    for (int i = tid; i < a.Hkv * D / 4; i += nthr) {
         const int head = (i * 4) / D, j = (i * 4) % D;
         const float4 v = lin_value4(a.lin, m, voff + i * 4, sxm);
         *reinterpret_cast<float4*>(row + voff + i * 4) = v;
@@ -382,6 +415,8 @@ struct AcceptArgs {
     int32_t* ctx_len;                       // device state, advanced when commit
 };
 __global__ void accept_walk_kernel(AcceptArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= a.B) return;
     const int T = a.T, nn = a.nn_eff[b], L = a.Lsnap[b];
@@ -437,6 +472,8 @@ struct CompactArgs {
     const int32_t* accept_nodes;
 };
 __global__ void __launch_bounds__(EW_THREADS) kv_compact_kernel(CompactArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     const int b = blockIdx.x, layer = blockIdx.y;
     const int n = a.accept_len[b];
     const int L = a.Lsnap[b];
@@ -483,6 +520,8 @@ __global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
 __global__ void set_i32_kernel(int32_t* p, int32_t v) { *p = v; }
 struct SetLensArgs { static constexpr int MAX = 64; int n; int slot[MAX]; int len[MAX]; };
 __global__ void set_lens_kernel(int32_t* ctx_len, SetLensArgs a) {
+    pdl_launch_dependents();
+    pdl_wait();
     if ((int)threadIdx.x < a.n) ctx_len[a.slot[threadIdx.x]] = a.len[threadIdx.x];
 }
 

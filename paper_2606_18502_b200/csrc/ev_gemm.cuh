@@ -46,6 +46,8 @@ struct GemmArgs {
     int M, N;
     int total_kb;       // ceil(K / 128) = K tiles of W
     int n_tiles, m_tiles, k_splits, kb_per_split;
+    int sk_units;       // stream-K (m_tiles == 1): n_tiles * total_kb K-blocks dealt out evenly, CTA c gets
+                        // [c U / G, (c+1) U / G); 0 = classic items (n_tile, m_tile, k_split)
     int tok;            // tokens per tile (UMMA N), multiple of 16, <= 256
     int stages;
     const uint8_t* W;   // tiled + swizzled codes: [n_tiles][total_kb][16 KiB]
@@ -115,6 +117,37 @@ __device__ __forceinline__ GemmItem gemm_item(const GemmArgs& a, int w) {
     it.nkb = min(a.kb_per_split, a.total_kb - it.kb0);
     return it;
 }
+// Work of one CTA, in order.  Classic: items blockIdx.x, +gridDim.x, ...  Stream-K: the contiguous range of
+// K-blocks [c U / G, (c+1) U / G) of the flattened (n_tile, kb) space, cut at tile boundaries; the piece of a
+// tile computed by the j-th CTA that touches it goes to slab j (sk_first_cta gives the first such CTA), so the
+// consumer (LinOut) adds the pieces in K order: deterministic, and independent of M.
+__host__ __device__ __forceinline__ int sk_first_cta(int unit, int G, int U) {  // largest c with floor(c U / G) <= unit
+    return (int)(((long long)(unit + 1) * G + U - 1) / U) - 1;
+}
+struct GemmWork {
+    int w, u, u_end;
+    __device__ __forceinline__ void init(const GemmArgs& a) {
+        w = blockIdx.x;
+        u = (int)((long long)blockIdx.x * a.sk_units / gridDim.x);
+        u_end = (int)((long long)(blockIdx.x + 1) * a.sk_units / gridDim.x);
+    }
+    __device__ __forceinline__ bool next(const GemmArgs& a, GemmItem& it) {
+        if (a.sk_units) {
+            if (u >= u_end) return false;
+            it.tile = it.n_tile = u / a.total_kb;
+            it.m_tile = 0;
+            it.kb0 = u - it.tile * a.total_kb;
+            it.nkb = min(a.total_kb - it.kb0, u_end - u);
+            it.split = (int)blockIdx.x - sk_first_cta(it.tile * a.total_kb, gridDim.x, a.sk_units);
+            u += it.nkb;
+            return true;
+        }
+        if (w >= a.n_tiles * a.m_tiles * a.k_splits) return false;
+        it = gemm_item(a, w);
+        w += gridDim.x;
+        return true;
+    }
+};
 
 template <int EPI>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, GemmArgs a) {
@@ -131,8 +164,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     unsigned long long* keys_smem = reinterpret_cast<unsigned long long*>(sx_smem + 512);  // [4 warps][256] argmax keys
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    pdl_launch_dependents();  // the consumer kernel's CTAs may become resident (they block in griddepcontrol.wait)
     if (threadIdx.x == 0) TS(0);
-    const int total_items = a.n_tiles * a.m_tiles * a.k_splits;
     uint32_t tmem_cols = 32;
     while ((int)tmem_cols < 2 * a.tok) tmem_cols <<= 1;
 
@@ -140,7 +173,12 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     // its first work item (weights do not depend on the previous kernel: this runs before griddepcontrol.wait,
     // i.e. while the previous kernel is still executing when launched with programmatic serialization). ----
     int pre = 0;
-    GemmItem it0 = gemm_item(a, min((int)blockIdx.x, total_items - 1));
+    GemmItem it0;
+    {
+        GemmWork w0;
+        w0.init(a);
+        if (!w0.next(a, it0)) { it0.n_tile = it0.m_tile = it0.kb0 = it0.nkb = 0; }
+    }
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], 4); }
@@ -172,9 +210,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             int s = pre;
             uint32_t ph = 0;
             if (s == a.stages) { s = 0; ph ^= 1; }
-            for (int w = blockIdx.x; w < total_items; w += gridDim.x) {
-                const GemmItem it = gemm_item(a, w);
-                for (int kb = (w == (int)blockIdx.x ? pre : 0); kb < it.nkb; ++kb) {
+            GemmWork wk;
+            wk.init(a);
+            GemmItem it;
+            for (bool first = true; wk.next(a, it); first = false) {
+                for (int kb = (first ? pre : 0); kb < it.nkb; ++kb) {
                     mbar_wait(&empty_bar[s], ph ^ 1);
                     if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], stage_bytes);
                     uint8_t* st = smem + s * stage_bytes;
@@ -190,8 +230,10 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             int s = 0;
             uint32_t ph = 0;
             int n_it = 0;
-            for (int w = blockIdx.x; w < total_items; w += gridDim.x, ++n_it) {
-                const GemmItem it = gemm_item(a, w);
+            GemmWork wk;
+            wk.init(a);
+            GemmItem it;
+            for (; wk.next(a, it); ++n_it) {
                 const int buf = n_it & 1;
                 mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);  // epilogue has drained this accumulator
                 tc_fence_after();
@@ -220,8 +262,10 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
         const int et = (int)threadIdx.x - 64;  // 0..127 among the epilogue threads
         const int n_loc = q * 32 + lane;
         int n_it = 0;
-        for (int w = blockIdx.x; w < total_items; w += gridDim.x, ++n_it) {
-            const GemmItem it = gemm_item(a, w);
+        GemmWork wk;
+        wk.init(a);
+        GemmItem it;
+        for (; wk.next(a, it); ++n_it) {
             const int buf = n_it & 1;
             const int n = it.n_tile * GEMM_WROWS + n_loc;
             const int m0 = it.m_tile * a.tok;
