@@ -69,6 +69,7 @@ SIGNATURES = {
     "ev_verify_host": (C.c_int, [_P, _P, C.c_int, C.c_int, _P, _P, _P, _P, C.c_int, _P, _P, _P, _P, _P, _P]),
     "ev_profile_enable": (C.c_int, [_P, C.c_int]),
     "ev_profile_read": (C.c_int, [_P, _P, _P, C.c_int]),
+    "ev_profile_trace": (C.c_int, [_P, _P, C.c_int, _P]),
     "ev_op_linear": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
     "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
     "ev_last_error": (C.c_char_p, []),
@@ -201,6 +202,14 @@ class Model:
         cnt = (C.c_long * n)()
         _check(self.lib.ev_profile_read(self.h, ms, cnt, n))
         return {k: (ms[i], cnt[i]) for i, k in enumerate(self.PROFILE_CLASSES)}
+
+    def ev_profile_trace(self, max_entries=1024):
+        """-> list of (t_enter, t_past_wait_first, t_exit, t_past_wait_last, 4 phase marks) in ns per traced launch of the
+        last verify step (needs EV_TRACE=1 in the environment when the model was created)."""
+        buf = (C.c_ulonglong * (8 * max_entries))()
+        n = C.c_int(0)
+        _check(self.lib.ev_profile_trace(self.h, buf, max_entries, C.byref(n)))
+        return [tuple(buf[8 * i + j] for j in range(8)) for i in range(n.value)]
 
     def ev_model_destroy(self):
         if self.h:

@@ -122,6 +122,7 @@ enum ProfClass { PC_GEMM_QKV = 0, PC_GEMM_O, PC_GEMM_GATEUP, PC_GEMM_DOWN, PC_GE
 struct ProfRec { cudaEvent_t a, b; int cls; };
 
 struct AttnPlan { int n_splits, split_len; };
+constexpr int TRACE_CAP = 1024;
 struct GraphKey {
     int B, T, commit, force_all, n_splits, split_len, need_lm, pad;
     const void* p[12];
@@ -151,6 +152,8 @@ struct ev_model {
     float* lin_out = nullptr;   // raw GEMM output [splits][M][N], consumed by the next element-wise kernel
     long lin_floats = 0;
     unsigned long long* dbg_ts = nullptr;
+    unsigned long long* trace = nullptr;   // EV_TRACE=1: [TRACE_CAP][4] step trace, see ev_profile_trace
+    int n_traced = 0;
     // tree state
     int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
     unsigned long long *anc = nullptr, *argmax_keys = nullptr;
@@ -164,6 +167,9 @@ struct ev_model {
     int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
+    // L2 weight stream (PfPlanner): on for token counts <= l2pf_max_m; bytes the stream may run ahead / per launch
+    int l2pf_max_m = 0;
+    long l2pf_cap = 88L << 20, l2pf_maxq = 40L << 20;
     std::vector<ProfRec> prof;
     size_t prof_used = 0;
     // captured verify steps (CUDA graphs), keyed by everything a launch depends on
@@ -280,11 +286,31 @@ template <class... KArgs, class... Args>
 int launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     return launch_kc(1, kern, grid, block, smem, st, args...);
 }
-// CTAs per token row of the element-wise kernels: spread few rows over all SMs
-int row_cluster(const ev_model* m, int M) {
-    if (m->row_cluster > 0) return m->row_cluster;
-    return M * 2 > m->num_sms ? 1 : (M * 4 > m->num_sms ? 2 : 4);
+// Shape of a row kernel launch (RMSNorm / SwiGLU / attention merge; ev_elementwise.cuh): cl CTAs of ROW_THREADS
+// threads per token row (one cluster), nv4 float4s per thread.  Few rows are spread over many CTAs so that they
+// still occupy every SM (cl up to 8); many rows keep nv4 <= 4 so that several CTAs stay resident per SM.
+struct RowPlan { int cl, nv4; };
+int pow2_ceil(long x) { int p = 1; while (p < x) p <<= 1; return p; }
+RowPlan row_plan(const ev_model* m, int M, int row_floats, int cl_par_max = CLUSTER_MAX) {
+    const long row4 = (row_floats + 3) / 4;
+    int cl_par = 1;
+    while (cl_par < cl_par_max && (long)M * cl_par * 2 <= 4L * m->num_sms) cl_par <<= 1;
+    cl_par = std::min(cl_par, pow2_ceil((row4 + ROW_THREADS - 1) / ROW_THREADS));
+    const int cl_need = pow2_ceil((row4 + 4L * ROW_THREADS - 1) / (4L * ROW_THREADS));
+    RowPlan p;
+    p.cl = std::max(cl_par, cl_need);
+    if (m->row_cluster > 0) p.cl = std::max(pow2_ceil(m->row_cluster), cl_need);
+    p.cl = std::min(p.cl, CLUSTER_MAX);
+    p.nv4 = pow2_ceil((row4 + (long)ROW_THREADS * p.cl - 1) / ((long)ROW_THREADS * p.cl));
+    return p;
 }
+#define ROW_DISPATCH(plan, KERN, ...)                                                                          \
+    do {                                                                                                       \
+        if ((plan).nv4 == 1) EV_TRY(launch_kc((plan).cl, KERN<1>, __VA_ARGS__));                               \
+        else if ((plan).nv4 == 2) EV_TRY(launch_kc((plan).cl, KERN<2>, __VA_ARGS__));                          \
+        else if ((plan).nv4 == 4) EV_TRY(launch_kc((plan).cl, KERN<4>, __VA_ARGS__));                          \
+        else return fail(EV_EINVAL, "row too long for the row kernels");                                       \
+    } while (0)
 
 template <int EPI>
 int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int grid, int smem) {
@@ -309,10 +335,83 @@ int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int 
     return EV_OK;
 }
 
+template <int MAXS>
+int launch_swiglu_s(ev_model* m, cudaStream_t st, bool smem_form, RowPlan rp, int M, const LinOut& gu, int F, float* tap, const QuantOut& q,
+                    const L2Prefetch& pf) {
+    if (smem_form) {
+        static bool attr_set = false;
+        if (!attr_set) {
+            CUDA_TRY(cudaFuncSetAttribute(swiglu_quant_smem_kernel<MAXS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+            attr_set = true;
+        }
+        return launch_k(swiglu_quant_smem_kernel<MAXS>, dim3(M), dim3(SWI_THREADS), (size_t)F * 4, st, gu, F, tap, q, pf);
+    }
+    if (rp.nv4 == 1) return launch_kc(rp.cl, swiglu_quant_kernel<1, MAXS>, dim3(M * rp.cl), dim3(SWI_THREADS), 0, st, gu, F, tap, q, pf);
+    if (rp.nv4 == 2) return launch_kc(rp.cl, swiglu_quant_kernel<2, MAXS>, dim3(M * rp.cl), dim3(SWI_THREADS), 0, st, gu, F, tap, q, pf);
+    if (rp.nv4 == 4) return launch_kc(rp.cl, swiglu_quant_kernel<4, MAXS>, dim3(M * rp.cl), dim3(SWI_THREADS), 0, st, gu, F, tap, q, pf);
+    return fail(EV_EINVAL, "row too long for the row kernels");
+}
+int launch_swiglu(ev_model* m, cudaStream_t st, bool smem_form, RowPlan rp, int M, const LinOut& gu, int F, float* tap, const QuantOut& q,
+                  const L2Prefetch& pf) {
+    if (gu.splits <= 1) return launch_swiglu_s<1>(m, st, smem_form, rp, M, gu, F, tap, q, pf);
+    if (gu.splits <= 3) return launch_swiglu_s<3>(m, st, smem_form, rp, M, gu, F, tap, q, pf);
+    return launch_swiglu_s<8>(m, st, smem_form, rp, M, gu, F, tap, q, pf);
+}
+
+// Host side of the L2 weight stream (L2Prefetch, ev_common.cuh).  segs = the weight matrices of the step in
+// the order the GEMMs consume them.  Every kernel launch of the step takes the next slice: at most `maxq`
+// bytes, and never more than `cap` bytes ahead of the start of the most recently launched GEMM's weights
+// (that GEMM may still be reading them when the slice is issued, one PDL stage early).
+struct PfPlanner {
+    std::vector<std::pair<const uint8_t*, size_t>> segs;
+    std::vector<size_t> start;   // prefix sums, start[i] = first stream byte of segs[i]; start.back() = total
+    size_t cursor = 0;           // stream bytes already covered (prefetched, or read directly by their GEMM)
+    int next_gemm = 0;
+    size_t cap = 0, maxq = 0;
+    bool on = false;
+    unsigned long long* trace = nullptr;  // step trace (ev_profile_trace): 4 slots per launch, in launch order
+    int n_traced = 0, trace_cap = 0;
+    void add(const uint8_t* p, size_t n) {
+        if (start.empty()) start.push_back(0);
+        segs.push_back({p, n});
+        start.push_back(start.back() + n);
+    }
+    L2Prefetch take(bool is_gemm) {
+        L2Prefetch pf;
+        pf.p[0] = pf.p[1] = nullptr; pf.n[0] = pf.n[1] = 0;
+        pf.trace = (trace && n_traced < trace_cap) ? trace + TRACE_SLOTS * (size_t)n_traced++ : nullptr;
+        if (!on || segs.empty()) return pf;
+        if (is_gemm && next_gemm < (int)segs.size()) {  // this GEMM reads its own weights: nothing of them is left to prefetch
+            cursor = std::max(cursor, start[next_gemm + 1]);
+            ++next_gemm;
+        }
+        const size_t consumed = start[std::max(0, next_gemm - 1)];
+        const size_t ahead = cursor - std::min(cursor, consumed);
+        if (ahead >= cap) return pf;
+        size_t quota = std::min(maxq, cap - ahead);
+        quota -= quota % L2PF_CHUNK;
+        int piece = 0;
+        while (quota > 0 && piece < 2 && cursor < start.back()) {
+            int si = (int)(std::upper_bound(start.begin(), start.end(), cursor) - start.begin()) - 1;
+            const size_t off = cursor - start[si];
+            size_t n = std::min(quota, segs[si].second - off);
+            n -= n % L2PF_CHUNK;
+            if (n == 0) { cursor = start[si + 1]; continue; }
+            pf.p[piece] = segs[si].first + off;
+            pf.n[piece] = (unsigned)n;
+            ++piece;
+            cursor += n;
+            quota -= n;
+            if (segs[si].second - off - n < L2PF_CHUNK) cursor = start[si + 1];
+        }
+        return pf;
+    }
+};
+
 // one W8A8 linear.  epi == EPI_RAW: raw accumulators go to m->lin_out as [splits][M][N]; *lin describes them for
 // the consumer kernel.  epi == EPI_ARGMAX (LM head): scales applied, argmax keys updated, optional logits.
 int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, LinOut* lin, float* logits,
-               unsigned long long* keys, int prof_cls) {
+               unsigned long long* keys, int prof_cls, PfPlanner* pfp = nullptr, const void* warm1 = nullptr, int warm1_bytes = 0) {
     ProfScope prof_scope(m, st, prof_cls);
     if (lin) {
         lin->p = m->lin_out; lin->splits = 1; lin->ld = (int)w.N; lin->split_stride = (long)M * w.N;
@@ -335,6 +434,10 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     a.W = w.codes; a.sx = x.scale; a.sw = w.scale; a.argmax_keys = keys;
     a.out = (epi == EPI_RAW) ? m->lin_out : logits;
     a.ldo = (int)w.N;
+    a.pf.p[0] = a.pf.p[1] = nullptr; a.pf.n[0] = a.pf.n[1] = 0; a.pf.trace = nullptr;
+    a.warm[0] = (epi == EPI_RAW) ? w.scale : nullptr; a.warm_bytes[0] = (epi == EPI_RAW) ? (int)(w.N * sizeof(float)) : 0;
+    a.warm[1] = warm1; a.warm_bytes[1] = warm1 ? warm1_bytes : 0;
+    if (pfp) a.pf = pfp->take(true);
     a.dbg = m->gemm_dbg;
     a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
     // Few token rows (one token tile): stream-K - the n_tiles * total_kb K-blocks are dealt out evenly to the
@@ -453,8 +556,25 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     }
     if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden, (long)M * H));
 
+    // L2 weight stream: the step's weight matrices in consumption order (PfPlanner)
+    PfPlanner pfp;
+    pfp.on = M <= m->l2pf_max_m && !m->profile && !m->naive_gemm;
+    pfp.cap = (size_t)m->l2pf_cap; pfp.maxq = (size_t)m->l2pf_maxq;
+    pfp.trace = m->trace; pfp.trace_cap = TRACE_CAP;
+    if (pfp.on) {
+        auto qbytes = [](const QMat& q) { return (size_t)q.n_tiles * q.total_kb * GEMM_WTILE; };
+        for (int l = 0; l < cfg.n_layers; ++l) {
+            LayerW& w = m->layers[l];
+            pfp.add(w.qkv.codes, qbytes(w.qkv)); pfp.add(w.o.codes, qbytes(w.o));
+            pfp.add(w.gu.codes, qbytes(w.gu)); pfp.add(w.down.codes, qbytes(w.down));
+        }
+        if (need_lm) pfp.add(m->lm.codes, qbytes(m->lm));
+    }
+
     const int n_splits = plan.n_splits, split_len = plan.split_len;
-    const int CL = row_cluster(m, M);
+    const RowPlan rp_h = row_plan(m, M, H), rp_f = row_plan(m, M, F, 4), rp_q = row_plan(m, M, m->q_dim);
+    const bool swi_smem = M > 2 * m->num_sms && (size_t)F * 4 <= 160 * 1024;   // many rows: one CTA per row, row staged in smem
+    const int rope_gy = (long)M * 4 <= 4L * m->num_sms ? 4 : 2;
     const int row_groups = (T * (cfg.n_q_heads / cfg.n_kv_heads) + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
 
     LinOut pend;           // raw output of the last O / down GEMM, not yet added to the residual stream
@@ -477,20 +597,21 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // --- attention block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0)));
+            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0), pfp.take(false));
             pend = none;
         }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sx) EV_TRY(copy_f32(st, m->xq.scale, out->dev_tap_sx, M));
         RopeArgs ra;
-        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_RAW, &ra.lin, nullptr, nullptr, PC_GEMM_QKV));
+        EV_TRY(run_linear(m, st, w.qkv, m->xq, M, EPI_RAW, &ra.lin, nullptr, nullptr, PC_GEMM_QKV, &pfp));
         ra.qkv_out = m->qkv; ra.ld = m->qkv_dim; ra.Hq = cfg.n_q_heads; ra.Hkv = cfg.n_kv_heads; ra.D = D; ra.T = T;
         ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
         ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
         ra.pool = c->pool + (size_t)l * c->layer_stride;
+        ra.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ROPE_KV);
-            EV_TRY(launch_k(rope_kvwrite_kernel, dim3(M, CL), dim3(CL > 1 ? 256 : ROPE_THREADS), 0, st, ra));
+            EV_TRY(launch_k(rope_kvwrite_kernel, dim3(M, rope_gy), dim3(ROPE_THREADS), 0, st, ra));
         }
         if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
         AttnArgs aa;
@@ -508,6 +629,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                 TcAttnArgs ta;
                 ta.a = aa;
                 ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
+                ta.pf = pfp.take(false);
                 if (D == 128) EV_TRY(launch_attn_tc<128>(st, c->tmKV, ta, agrid)); else EV_TRY(launch_attn_tc<64>(st, c->tmKV, ta, agrid));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
@@ -518,40 +640,43 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part;
         ma.attn = (tap && out->dev_tap_attn) ? out->dev_tap_attn : nullptr;
         ma.q = quant_out(m, m->aq, 4 * l + 1);
+        ma.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
-            EV_TRY(launch_kc(CL, attn_merge_quant_kernel, dim3(M * CL), dim3(MERGE_THREADS), (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st, ma));
+            ROW_DISPATCH(rp_q, attn_merge_quant_kernel, dim3(M * rp_q.cl), dim3(MERGE_THREADS), (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st, ma);
         }
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
-        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_O));
+        EV_TRY(run_linear(m, st, w.o, m->aq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_O, &pfp, w.g2, H * 2));
         if (tap && out->dev_tap_hmid) { EV_TRY(materialize()); EV_TRY(copy_f32(st, m->h, out->dev_tap_hmid, (long)M * H)); }
         // --- MLP block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2)));
+            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2), pfp.take(false));
             pend = none;
         }
         LinOut gul;
-        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_RAW, &gul, nullptr, nullptr, PC_GEMM_GATEUP));
+        EV_TRY(run_linear(m, st, w.gu, m->xq, M, EPI_RAW, &gul, nullptr, nullptr, PC_GEMM_GATEUP, &pfp));
         {
             ProfScope ps(m, st, PC_SWIGLU);
-            EV_TRY(launch_kc(CL, swiglu_quant_kernel, dim3(M * CL), dim3(SWI_THREADS), 0, st, gul, F, (tap ? out->dev_tap_gu : nullptr), quant_out(m, m->tq, 4 * l + 3)));
+            EV_TRY(launch_swiglu(m, st, swi_smem, rp_f, M, gul, F, (tap ? out->dev_tap_gu : nullptr), quant_out(m, m->tq, 4 * l + 3), pfp.take(false)));
         }
         if (tap && out->dev_tap_tq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_tq, m->tq.codes, (size_t)M * F, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_st) EV_TRY(copy_f32(st, m->tq.scale, out->dev_tap_st, M));
-        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_DOWN));
+        EV_TRY(run_linear(m, st, w.down, m->tq, M, EPI_RAW, &pend, nullptr, nullptr, PC_GEMM_DOWN, &pfp,
+                          (l + 1 < cfg.n_layers) ? m->layers[l + 1].g1 : m->gf, H * 2));
         if (out->dev_hidden) { EV_TRY(materialize()); EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H)); }
     }
     if (need_lm) {
         if (lockstep) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H)); }
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            EV_TRY(launch_kc(CL, rmsnorm_quant_kernel, dim3(M * CL), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers)));
+            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers), pfp.take(false));
             pend = none;
         }
-        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM));
+        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM, &pfp));
     }
+    m->n_traced = pfp.n_traced;
     AcceptArgs ac;
     ac.B = B; ac.T = T; ac.commit = in->commit; ac.force_all = in->force_accept_all;
     ac.tokens = in->dev_tokens; ac.parents = in->dev_parents; ac.nn_eff = m->nn_eff; ac.status = out->dev_status;
@@ -626,6 +751,9 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->use_splitk = !(getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) == 0);  // on by default
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
+    if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
+    if (getenv("EV_L2PF_CAP_MB")) m->l2pf_cap = (long)atoi(getenv("EV_L2PF_CAP_MB")) << 20;
+    if (getenv("EV_L2PF_MAXQ_MB")) m->l2pf_maxq = (long)atoi(getenv("EV_L2PF_MAXQ_MB")) << 20;
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
     m->row_cluster = getenv("EV_ROW_CLUSTER") ? atoi(getenv("EV_ROW_CLUSTER")) : 0;
     m->use_graph = !(getenv("EV_GRAPH") && atoi(getenv("EV_GRAPH")) == 0);          // on by default
@@ -657,6 +785,10 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     }
     A(dev_alloc(m, &m->lin_out, (size_t)m->lin_floats));
     A(dev_alloc(m, &m->dbg_ts, (size_t)1024 * 8));
+    if (getenv("EV_TRACE") && atoi(getenv("EV_TRACE")) != 0) {
+        A(dev_alloc(m, &m->trace, (size_t)TRACE_CAP * TRACE_SLOTS));
+        cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8);
+    }
     A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
@@ -1240,6 +1372,19 @@ int ev_profile_read(ev_model* m, double* host_ms_by_class, long* host_count_by_c
 }
 
 // bring-up: copies the per-CTA GEMM phase timestamps of the last launch (EV_GEMM_DBG & 16) to the host
+int ev_profile_trace(ev_model* m, unsigned long long* host_out, int max_entries, int* n_out) {
+    if (!m || !host_out || !n_out) return fail(EV_EINVAL, "null argument");
+    if (!m->trace) return fail(EV_ESTATE, "step trace is off (create the model with EV_TRACE=1 in the environment)");
+    CUDA_TRY(cudaDeviceSynchronize());
+    const int n = std::min(std::min(max_entries, m->n_traced), TRACE_CAP);
+    CUDA_TRY(cudaMemcpy(host_out, m->trace, (size_t)n * TRACE_SLOTS * 8, cudaMemcpyDeviceToHost));
+    for (int i = 0; i < n; ++i)
+        for (int j = 2; j < TRACE_SLOTS; ++j) host_out[TRACE_SLOTS * i + j] = ~host_out[TRACE_SLOTS * i + j];
+    CUDA_TRY(cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8));
+    *n_out = n;
+    return EV_OK;
+}
+
 int ev_debug_gemm_timestamps(ev_model* m, unsigned long long* host_out, int n_ctas) {
     if (!m || !host_out) return fail(EV_EINVAL, "null argument");
     CUDA_TRY(cudaDeviceSynchronize());

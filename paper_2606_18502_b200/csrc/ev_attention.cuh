@@ -321,12 +321,15 @@ struct MergeArgs {
     const float* ml_part;
     float* attn;   // optional [M][Hq*D] fp32 merged output (debug tap) or null
     QuantOut q;
+    L2Prefetch pf;
 };
-constexpr int MERGE_THREADS = 512;
-constexpr int MERGE_NV4 = 2;   // Hq*D <= 4096
+constexpr int MERGE_THREADS = 256;   // = ROW_THREADS (ev_elementwise.cuh): Hq * D <= 4 * 256 * NV4 * cluster size
+template <int MERGE_NV4>
 __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeArgs a) {
     pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
+    l2_prefetch_issue(a.pf);
     pdl_wait();
+    trace_past_wait(a.pf);
     extern __shared__ float msm[];             // w[Hq][S] | l[Hq][S] | den[Hq]
     __shared__ float red[MERGE_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
@@ -391,6 +394,7 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
         if (i4 < c1 && a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
     }
     quantize_regs<MERGE_NV4>(v, m, K, c0, c1, a.q, red, xch_f);
+    trace_exit(a.pf);
 }
 
 }  // namespace ev

@@ -116,6 +116,7 @@ __device__ __forceinline__ void split3_pack(float x0, float x1, uint32_t& hi, ui
 struct TcAttnArgs {
     AttnArgs a;       // same fields as the legacy kernel (pool pointer unused here)
     int row0;         // first row of this layer in the pool tensor map: layer * n_pages * 2 * Hkv * 16
+    L2Prefetch pf;
 };
 
 template <int D>
@@ -145,6 +146,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
 
     // ---- prologue that does not depend on the previous kernel (overlaps it under PDL): barriers, TMEM ----
     pdl_launch_dependents();
+    l2_prefetch_issue(ta.pf);
     if (threadIdx.x == 0) {
         for (int s = 0; s < TCA_STAGES; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
@@ -155,6 +157,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     }
     if (warp == 1) tmem_alloc<512>(tmem_base_smem);
     pdl_wait();
+    trace_past_wait(ta.pf);
     const int nn = a.nn_eff[b];
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
@@ -362,6 +365,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<512>(tmem_base);
+    trace_exit(ta.pf);
 }
 
 }  // namespace ev

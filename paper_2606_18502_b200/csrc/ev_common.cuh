@@ -180,17 +180,19 @@ __device__ __forceinline__ float lin_value(const LinOut& o, int m, int n, float 
     return __fmul_rn(__fmul_rn(lin_acc(o, (size_t)m * o.ld + n, n), sxm), __ldg(o.sw + n));
 }
 
-// four consecutive channels n..n+3 (n % 4 == 0, ld % 4 == 0): 16-byte loads, all slabs in flight together
+// four consecutive channels n..n+3 (n % 4 == 0, ld % 4 == 0): 16-byte loads, all slabs in flight together.
+// MAXS = compile-time bound of the slab count (o.splits <= MAXS): bounds the registers held for loads in flight.
+template <int MAXS = 8>
 __device__ __forceinline__ float4 lin_value4(const LinOut& o, int m, int n, float sxm) {
     const size_t idx = (size_t)m * o.ld + n;
-    const int cnt = lin_slabs(o, n);
+    const int cnt = MAXS == 1 ? 1 : lin_slabs(o, n);
     float4 acc = __ldcg(reinterpret_cast<const float4*>(o.p + idx));
-    float4 t[7];
+    float4 t[MAXS > 1 ? MAXS - 1 : 1];
 #pragma unroll
-    for (int s = 1; s < 8; ++s)
+    for (int s = 1; s < MAXS; ++s)
         if (s < cnt) t[s - 1] = __ldcg(reinterpret_cast<const float4*>(o.p + (size_t)s * o.split_stride + idx));
 #pragma unroll
-    for (int s = 1; s < 8; ++s)
+    for (int s = 1; s < MAXS; ++s)
         if (s < cnt) {
             acc.x = __fadd_rn(acc.x, t[s - 1].x); acc.y = __fadd_rn(acc.y, t[s - 1].y);
             acc.z = __fadd_rn(acc.z, t[s - 1].z); acc.w = __fadd_rn(acc.w, t[s - 1].w);
@@ -206,6 +208,54 @@ __device__ __forceinline__ float4 lin_value4(const LinOut& o, int m, int n, floa
 // calls pdl_launch_dependents() as early as possible so the dependent's prologue overlaps it.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// ---- weight stream -> L2 ahead of use ---------------------------------------------------------------
+// At small M the step is bound by streaming 7.5 GB of weights, but the chain of short dependent kernels
+// between the GEMMs (norm, RoPE, attention, merge, SwiGLU) leaves HBM idle most of the time.  Every kernel
+// of the step therefore carries one slice of the upcoming GEMMs' weights and, before griddepcontrol.wait,
+// asks the L2 to fetch it (cp.async.bulk.prefetch.L2: fire and forget, no registers, no shared memory).
+// The 126 MB L2 becomes the staging buffer of a continuous weight stream; the host (PfPlanner, ev_api.cu)
+// bounds how far the stream may run ahead of the GEMM that is consuming it.
+struct L2Prefetch {
+    const uint8_t* p[2];   // up to two pieces (a slice may straddle two matrices); 16-byte aligned
+    unsigned n[2];         // bytes, multiples of L2PF_CHUNK
+    unsigned long long* trace;  // null, or this launch's TRACE_SLOTS step-trace slots (ev_profile_trace): min over CTAs of
+                                // t_enter, t_past_wait, ~t_exit, ~t_past_wait (globaltimer ns; memset 0xFF = empty)
+};
+__device__ __forceinline__ void trace_mark(const L2Prefetch& pf, int slot, bool complement) {
+    if (pf.trace && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        atomicMin(pf.trace + slot, complement ? ~t : t);
+    }
+}
+__device__ __forceinline__ void trace_past_wait(const L2Prefetch& pf) { trace_mark(pf, 1, false); trace_mark(pf, 3, true); }
+__device__ __forceinline__ void trace_exit(const L2Prefetch& pf) { trace_mark(pf, 2, true); }
+// bring-up: phase k (0..3) reached by the LAST CTA (slots 4..7 hold ~t)
+__device__ __forceinline__ void trace_phase(const L2Prefetch& pf, int k) { trace_mark(pf, 4 + k, true); }
+constexpr int TRACE_SLOTS = 8;
+// same, but ordered after the instruction that produced `dep` (e.g. a load)
+__device__ __forceinline__ void trace_phase_dep(const L2Prefetch& pf, int k, float dep) {
+    if (pf.trace && threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("{\n\t.reg .f32 d;\n\tmov.f32 d, %1;\n\tmov.u64 %0, %%globaltimer;\n\t}" : "=l"(t) : "f"(dep));
+        atomicMin(pf.trace + 4 + k, ~t);
+    }
+}
+constexpr unsigned L2PF_CHUNK = 8192;
+__device__ __forceinline__ void l2_prefetch_issue(const L2Prefetch& pf, unsigned first_thread = 0) {
+    trace_mark(pf, 0, false);
+    const unsigned lane = threadIdx.x - first_thread;   // the 32 threads [first_thread, +32) issue
+    if (lane >= 32u || (pf.n[0] | pf.n[1]) == 0) return;
+    const unsigned cta = blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z);
+    const unsigned ncta = gridDim.x * gridDim.y * gridDim.z;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const unsigned chunks = pf.n[s] / L2PF_CHUNK;
+        for (unsigned i = cta * 32u + lane; i < chunks; i += ncta * 32u)
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf.p[s] + (size_t)i * L2PF_CHUNK), "r"(L2PF_CHUNK) : "memory");
+    }
+}
 
 // ---- thread-block clusters: a token row of the element-wise kernels is spread over the CTAs of one cluster
 // (so that M = 60 rows still occupy all SMs); row statistics meet through distributed shared memory.

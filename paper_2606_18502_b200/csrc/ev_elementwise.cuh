@@ -210,14 +210,18 @@ __device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
 
 // ---- K3: (residual += pending linear output) + RMSNorm + quantize; one CTA of 256 threads per token;
 // H % 4 == 0 and H <= 4096.  `pend` is the raw output of the previous O / down GEMM (LinOut, ev_common.cuh) or
-// has p == null; the updated residual stream is written back to h. ----
-constexpr int NORM_THREADS = 256;
-constexpr int NORM_NV4 = 4;
+// has p == null; the updated residual stream is written back to h.  H <= 4 * ROW_THREADS * NV4 * cluster size. ----
+// Row kernels (RMSNorm, SwiGLU, attention merge): ROW_THREADS threads per CTA, a row spread over the CTAs of a
+// cluster, NV4 float4s per thread in registers (instantiated for 1, 2, 4; the host picks cluster size and NV4 from
+// the token count so that few rows still fill the machine and many rows keep several CTAs per SM: row_plan()).
+constexpr int ROW_THREADS = 256;
+constexpr int NORM_THREADS = ROW_THREADS;
+template <int NORM_NV4>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
                                                                      const __nv_bfloat16* __restrict__ gain, float eps,
-                                                                     QuantOut q) {
+                                                                     QuantOut q, L2Prefetch pf) {
     pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
-    pdl_wait();
+    l2_prefetch_issue(pf);
     __shared__ float red[NORM_THREADS / 32];
     __shared__ double dred[NORM_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
@@ -225,6 +229,15 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     int c0, c1;
     cluster_cols(H / 4, c0, c1);
+    uint2 gbits[NORM_NV4];   // gains (bf16 x 4) do not depend on the previous kernel: fetched before the wait
+#pragma unroll
+    for (int k = 0; k < NORM_NV4; ++k) {
+        const int i4 = c0 + threadIdx.x + k * NORM_THREADS;
+        gbits[k] = make_uint2(0x3F803F80u, 0x3F803F80u);  // 1.0, 1.0
+        if (gain && i4 < c1) gbits[k] = __ldg(reinterpret_cast<const uint2*>(gain + i4 * 4));
+    }
+    pdl_wait();
+    trace_past_wait(pf);
     float* x = h + (size_t)m * H;
     float4 v[NORM_NV4];
     const float sxm = pend.p ? __ldg(pend.sx + m) : 0.f;
@@ -258,14 +271,14 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
         const int i4 = c0 + threadIdx.x + k * NORM_THREADS;
         const int i = i4 * 4;
         if (i4 < c1) {
-            float4 g = make_float4(1.f, 1.f, 1.f, 1.f);
-            if (gain) g = make_float4(__bfloat162float(gain[i]), __bfloat162float(gain[i + 1]), __bfloat162float(gain[i + 2]),
-                                      __bfloat162float(gain[i + 3]));
+            const float4 g = make_float4(__uint_as_float(gbits[k].x << 16), __uint_as_float(gbits[k].x & 0xFFFF0000u),
+                                         __uint_as_float(gbits[k].y << 16), __uint_as_float(gbits[k].y & 0xFFFF0000u));
             v[k] = make_float4(mul_rn(mul_rn(v[k].x, r), g.x), mul_rn(mul_rn(v[k].y, r), g.y), mul_rn(mul_rn(v[k].z, r), g.z),
                                mul_rn(mul_rn(v[k].w, r), g.w));
         }
     }
     quantize_regs<NORM_NV4>(v, m, H, c0, c1, q, red, xch_f);
+    trace_exit(pf);
 }
 
 // residual += pending linear output, nothing else (debug taps / end of a prefill pass)
@@ -294,16 +307,19 @@ __global__ void __launch_bounds__(EW_THREADS) quantize_rows_kernel(const float* 
 }
 
 // ---- K6: SwiGLU + quantize on the raw gate|up GEMM output (LinOut, ld = 2F: gate | up); one CTA of 512
-// threads per token, the row of F values lives in registers; F % 4 == 0 and F <= 16384. ----
+// threads per token, the row of F values lives in registers; F % 4 == 0 and F <= 4 * ROW_THREADS * NV4 * cluster size. ----
 __device__ __forceinline__ float swiglu_f(float g, float u) {
     // t = (g / (1 + exp(-g))) * u, fp32 ops in this order; expf is the full-range libdevice one
     return mul_rn(div_rn(g, add_rn(1.0f, expf(-g))), u);
 }
-constexpr int SWI_THREADS = 512;
-constexpr int SWI_NV4 = 8;
-__global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, int F, float* __restrict__ gu_tap, QuantOut q) {
+constexpr int SWI_THREADS = ROW_THREADS;
+template <int SWI_NV4, int MAXS>
+__global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, int F, float* __restrict__ gu_tap, QuantOut q,
+                                                                   L2Prefetch pf) {
     pdl_launch_dependents();  // the down-projection GEMM may start prefetching its weights now
+    l2_prefetch_issue(pf);
     pdl_wait();
+    trace_past_wait(pf);
     __shared__ float red[SWI_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
@@ -317,7 +333,7 @@ __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, in
         const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
         if (i4 < c1) {
-            const float4 g = lin_value4(gu, m, i, sxm), u = lin_value4(gu, m, F + i, sxm);
+            const float4 g = lin_value4<MAXS>(gu, m, i, sxm), u = lin_value4<MAXS>(gu, m, F + i, sxm);
             if (gu_tap) {
                 *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + i) = g;
                 *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + F + i) = u;
@@ -326,6 +342,49 @@ __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_kernel(LinOut gu, in
         }
     }
     quantize_regs<SWI_NV4>(v, m, F, c0, c1, q, red, xch_f);
+    trace_exit(pf);
+}
+
+// Many rows (M > ~2 rows per SM): one CTA per token, no cluster; the row of F SwiGLU values is staged in shared
+// memory (4 F bytes) between the absmax pass and the quantize pass, so a thread holds only a few values in
+// registers and several CTAs stay resident per SM (the register-resident form above runs one CTA per SM at F = 14336).
+template <int MAXS>
+__global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_smem_kernel(LinOut gu, int F, float* __restrict__ gu_tap, QuantOut q,
+                                                                        L2Prefetch pf) {
+    extern __shared__ float4 swi_row[];   // [F / 4]
+    __shared__ float red[SWI_THREADS / 32];
+    pdl_launch_dependents();
+    pdl_wait();
+    trace_past_wait(pf);
+    const int m = blockIdx.x;
+    const int n4 = F / 4;
+    const float sxm = __ldg(gu.sx + m);
+    float amax = 0.f;
+    for (int i4 = threadIdx.x; i4 < n4; i4 += SWI_THREADS) {
+        const int i = i4 * 4;
+        const float4 g = lin_value4<MAXS>(gu, m, i, sxm), u = lin_value4<MAXS>(gu, m, F + i, sxm);
+        if (gu_tap) {
+            *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + i) = g;
+            *reinterpret_cast<float4*>(gu_tap + (size_t)m * 2 * F + F + i) = u;
+        }
+        const float4 t = make_float4(swiglu_f(g.x, u.x), swiglu_f(g.y, u.y), swiglu_f(g.z, u.z), swiglu_f(g.w, u.w));
+        swi_row[i4] = t;
+        amax = fmaxf(amax, fmaxf(fmaxf(fabsf(t.x), fabsf(t.y)), fmaxf(fabsf(t.z), fabsf(t.w))));
+    }
+    amax = block_max(amax, red);   // contains the __syncthreads that publishes swi_row
+    float s;
+    if (q.static_scale) s = *q.static_scale;
+    else s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
+    if (threadIdx.x == 0) {
+        q.sx[m] = s;
+        if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
+    }
+    uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * F);
+    for (int i4 = threadIdx.x; i4 < n4; i4 += SWI_THREADS) {
+        const float4 t = swi_row[i4];   // written by this same thread
+        dst[i4] = e4m3x4(div_rn(t.x, s), div_rn(t.y, s), div_rn(t.z, s), div_rn(t.w, s));
+    }
+    trace_exit(pf);
 }
 
 // ---- K4: RoPE (positions = L + depth) on q, k of the raw QKV GEMM output + K,V -> bf16 pages; q, k, v are
@@ -342,11 +401,14 @@ struct RopeArgs {
     const int32_t* page_table; // [max_seqs][max_pages]
     int max_pages, page_size;
     __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D]
+    L2Prefetch pf;
 };
-constexpr int ROPE_THREADS = 512;
+constexpr int ROPE_THREADS = 256;
 __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) {
     pdl_launch_dependents();
+    l2_prefetch_issue(a.pf);
     pdl_wait();
+    trace_past_wait(a.pf);
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
     const int D = a.D, D2 = D / 2;
@@ -395,6 +457,7 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
                 make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
         }
     }
+    trace_exit(a.pf);
 }
 
 // ---- K8 finalize + K9 greedy acceptance walk + ctx_len update: one thread per sequence ---------

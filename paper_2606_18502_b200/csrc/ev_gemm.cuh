@@ -57,6 +57,9 @@ struct GemmArgs {
     int ldo;
     unsigned long long* argmax_keys;  // EPI_ARGMAX: [M] packed (ordered logit, ~index)
     unsigned long long* ts;  // bring-up: per-CTA phase timestamps [grid][8] (globaltimer ns), or null
+    L2Prefetch pf;      // slice of the weight stream of the GEMMs that follow (ev_common.cuh)
+    const void* warm[2];   // per-layer constants the CONSUMER kernel will read first thing after its wait (this
+    int warm_bytes[2];     // matrix's s_w, the next RMSNorm's gain): touched here so they are L2 hits there
     int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads
 };
 
@@ -165,6 +168,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     pdl_launch_dependents();  // the consumer kernel's CTAs may become resident (they block in griddepcontrol.wait)
+    l2_prefetch_issue(a.pf, 64);  // warp 2 (an epilogue warp, idle until the first accumulator is ready)
+    if (warp >= 2) {  // epilogue warps are idle until the first accumulator is ready: one 128-byte line per thread
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+            for (int ln = blockIdx.x * 128 + (int)threadIdx.x - 64; ln * 128 < a.warm_bytes[s]; ln += gridDim.x * 128) {
+                unsigned tmp;
+                asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(tmp) : "l"(reinterpret_cast<const char*>(a.warm[s]) + (size_t)ln * 128));
+            }
+    }
     if (threadIdx.x == 0) TS(0);
     uint32_t tmem_cols = 32;
     while ((int)tmem_cols < 2 * a.tok) tmem_cols <<= 1;
@@ -204,6 +216,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             const uint64_t pol_w = policy_evict_first();   // weights are streamed once per step
             const uint64_t pol_x = policy_evict_last();    // activations are re-read by every tile
             pdl_wait();  // activations come from the previous kernel
+            trace_past_wait(a.pf);
             TS(3);
             for (int i = 0; i < pre; ++i)
                 load_x(a.dbg, smem + i * stage_bytes + GEMM_WTILE, &tmX, &full_bar[i], (it0.kb0 + i) * GEMM_BK, it0.m_tile * a.tok, pol_x);
@@ -339,6 +352,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     __syncthreads();
     if (warp == 1) tmem_dealloc_rt(tmem_base, tmem_cols);
     if (threadIdx.x == 32) TS(7);
+    trace_exit(a.pf);
 }
 
 // debug / bring-up reference: same contraction on CUDA cores from the tiled weight layout (exact products,
