@@ -164,6 +164,7 @@ struct ev_model {
     bool calibrated = false, recording = false;
     int num_sms = 148;
     bool use_splitk = false, naive_gemm = false, legacy_attn = false;
+    int attn_dbg = 0;
     int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
@@ -630,6 +631,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                 ta.a = aa;
                 ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
                 ta.pf = pfp.take(false);
+                ta.dbg = m->attn_dbg;
                 if (D == 128) EV_TRY(launch_attn_tc<128>(st, c->tmKV, ta, agrid)); else EV_TRY(launch_attn_tc<64>(st, c->tmKV, ta, agrid));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
@@ -758,6 +760,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->row_cluster = getenv("EV_ROW_CLUSTER") ? atoi(getenv("EV_ROW_CLUSTER")) : 0;
     m->use_graph = !(getenv("EV_GRAPH") && atoi(getenv("EV_GRAPH")) == 0);          // on by default
     g_use_pdl = !(getenv("EV_PDL") && atoi(getenv("EV_PDL")) == 0);                // on by default
+    m->attn_dbg = getenv("EV_ATTN_DBG") ? atoi(getenv("EV_ATTN_DBG")) : 0;
     m->legacy_attn = getenv("EV_ATTN_LEGACY") && atoi(getenv("EV_ATTN_LEGACY")) != 0;  // bring-up: mma.sync attention
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;

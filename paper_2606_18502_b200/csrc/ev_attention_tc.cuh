@@ -8,10 +8,15 @@
 //                   (the pool's 4 KiB (page, K|V, head) blocks are read in place through one 2-D tensor map)
 //   MMA thread    : S[j&1]  = Q . K_j^T   (tcgen05.mma kind::f16, A = Q from smem, B = K tile, D in TMEM)
 //                   Oc      = P[j&1] . V_j (A = P from TMEM, B = V tile MN-major, D in TMEM, from zero)
-//   8 softmax warps (thread = one query row x half of the tile's keys / half of d):
-//                   S -> registers (tcgen05.ld), scale, tree mask, online max (halves meet in smem),
-//                   p = 2^((s-m) log2 e), P -> TMEM (tcgen05.st); then Oc -> registers and
-//                   O = O * exp(m_old - m_new) + Oc with ONE rounded fp32 operation per tile.
+//   8 softmax warps (thread = one query row x half of the tile's keys):
+//                   S -> registers (tcgen05.ld), tree mask, online max (the two halves of a row meet in shared
+//                   memory behind a 64-thread named barrier), p = 2^(s k - m k), k = log2(e)/sqrt(d), one FFMA +
+//                   one MUFU per key, P -> hi|mid|lo bf16 -> TMEM (tcgen05.st); publishes the tile's rescale
+//                   factor c = exp(m_old - m_new) in shared memory
+//   8 correction warps (thread = one query row x half of d): Oc -> registers and
+//                   O = O * c + Oc with ONE rounded fp32 operation per tile, concurrently with the softmax of
+//                   the next tile (the two used to be serial in the same threads: 3,700 cycles per tile against
+//                   a tensor floor of 1,536; profiles/r1_attention_v2.md).
 // Precision (DESIGN.md section 6 "attention precision"): Q and P are fp32 values split into hi+mid+lo bf16
 // parts (3 x 8 significand bits: exact), K and V are bf16, so every product is exact; the tensor core only
 // accumulates (smallest parts first).  The running output lives in registers, not in TMEM, because long
@@ -22,9 +27,10 @@
 
 namespace ev {
 
-constexpr int TCA_THREADS = 320;  // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 softmax / correction
+constexpr int TCA_THREADS = 576;  // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 softmax, warps 10..17 correction
 constexpr int TCA_BN = 64;        // keys per tile (= ATT_CH: the split plan is shared with the legacy kernel)
-constexpr int TCA_STAGES = 3;
+constexpr int TCA_KS = 4;        // K ring depth (a K tile is released by Q.K^T, early)
+constexpr int TCA_VS = 3;        // V ring depth (a V tile is released by P.V)
 constexpr int TCA_PAGE = 16;      // tokens per page this kernel is built for
 
 template <int D>
@@ -34,14 +40,18 @@ struct TcaCfg {
     static constexpr int Q_BYTES = 3 * Q_PART;
     static constexpr int KV_HALF = TCA_BN * 128;         // 8 KiB: 64 keys x 128 B
     static constexpr int K_BYTES = NH * KV_HALF;
-    static constexpr int STAGE = 2 * K_BYTES;            // K tile | V tile
     static constexpr int BAR_BYTES = 256;
-    static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128) * 4;  // max exchange (double buffered) + sum exchange
-    static constexpr int SMEM = 1024 + Q_BYTES + TCA_STAGES * STAGE + BAR_BYTES + XCH_BYTES;
+    static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
+    static constexpr int SMEM = 1024 + Q_BYTES + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;
     // TMEM columns
-    static constexpr int TS = 0;            // S[2]: 2 x 64 fp32 columns
-    static constexpr int TP = 128;          // P[2][3 parts]: 32 columns each (64 bf16 pairs)
-    static constexpr int TO = 320;          // O chunk: D fp32 columns
+    // S[2] and P[2] share two 96-column regions: S(j) = 64 fp32 columns, P(j) = 3 parts x 32 columns (64 bf16
+    // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that); that
+    // frees room for TWO O chunks, so P.V of tile j+1 does not wait for the correction warps to read chunk j.
+    static constexpr int TS = 0;
+    static constexpr int TP = 0;
+    static constexpr int SP = 96;           // columns per S/P region
+    static constexpr int TO = 192;          // O chunks: 2 x D fp32 columns
+    static_assert(TO + 2 * D <= 512, "TMEM budget");
     static constexpr int DH = D / 2;        // output columns per softmax warpgroup
 };
 
@@ -95,6 +105,17 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
         "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
         : "memory");
 }
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]),
+                 "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
+__device__ __forceinline__ void pair_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ bool elect_one() {  // one lane of a converged warp
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -102,20 +123,25 @@ __device__ __forceinline__ float ex2_approx(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// (x0, x1) -> packed bf16 pairs hi, mid, lo with x = hi + mid + lo exactly (x0 in the low half)
+// (x0, x1) -> packed bf16 pairs hi, mid, lo with x = hi + mid + lo exactly (x0 in the low half).  The parts are
+// cut by TRUNCATION (mask the low 16 bits), not by cvt.rn: the three parts still sum to x exactly (the
+// remainder after taking the top 8 significand bits has at most 16, then at most 8 significant bits), and the
+// work stays on the ALU/FMA pipes: F2FP shares the quarter-rate XU pipe with the softmax's MUFU.EX2 and was the
+// bottleneck of the softmax warps (profiles/r1_attention_v2.md).
 __device__ __forceinline__ void split3_pack(float x0, float x1, uint32_t& hi, uint32_t& mid, uint32_t& lo) {
-    uint32_t h, m, l;
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(h) : "f"(x1), "f"(x0));
-    const float r0 = x0 - __uint_as_float(h << 16), r1 = x1 - __uint_as_float(h & 0xFFFF0000u);
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(m) : "f"(r1), "f"(r0));
-    const float t0 = r0 - __uint_as_float(m << 16), t1 = r1 - __uint_as_float(m & 0xFFFF0000u);
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(l) : "f"(t1), "f"(t0));
-    hi = h; mid = m; lo = l;
+    const uint32_t u0 = __float_as_uint(x0), u1 = __float_as_uint(x1);
+    hi = __byte_perm(u0, u1, 0x7632);
+    const float r0 = x0 - __uint_as_float(u0 & 0xFFFF0000u), r1 = x1 - __uint_as_float(u1 & 0xFFFF0000u);
+    const uint32_t v0 = __float_as_uint(r0), v1 = __float_as_uint(r1);
+    mid = __byte_perm(v0, v1, 0x7632);
+    const float t0 = r0 - __uint_as_float(v0 & 0xFFFF0000u), t1 = r1 - __uint_as_float(v1 & 0xFFFF0000u);
+    lo = __byte_perm(__float_as_uint(t0), __float_as_uint(t1), 0x7632);
 }
 
 struct TcAttnArgs {
     AttnArgs a;       // same fields as the legacy kernel (pool pointer unused here)
     int row0;         // first row of this layer in the pool tensor map: layer * n_pages * 2 * Hkv * 16
+    int dbg;          // bring-up experiments (EV_ATTN_DBG): 1 no KV loads, 2 no MMAs, 4 no O-chunk reads
     L2Prefetch pf;
 };
 
@@ -126,17 +152,20 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     extern __shared__ uint8_t tca_smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tca_smem_raw) + 1023) & ~(uintptr_t)1023);
     uint8_t* q_s = smem;                                  // [3 parts][NH][128 rows][128 B]
-    uint8_t* kv_s = smem + C::Q_BYTES;                    // [STAGES][K: NH x 8 KiB | V: NH x 8 KiB]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(kv_s + TCA_STAGES * C::STAGE);
-    uint64_t* kv_full = bars;                             // [STAGES]
-    uint64_t* kv_empty = bars + TCA_STAGES;               // [STAGES]
-    uint64_t* s_full = bars + 2 * TCA_STAGES;             // [2]
+    uint8_t* kv_s = smem + C::Q_BYTES;                    // K ring [KS][NH x 8 KiB] | V ring [VS][NH x 8 KiB]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(kv_s + (TCA_KS + TCA_VS) * C::K_BYTES);
+    uint64_t* k_full = bars;                              // [KS]
+    uint64_t* k_empty = k_full + TCA_KS;                  // [KS]
+    uint64_t* v_full = k_empty + TCA_KS;                  // [VS]
+    uint64_t* v_empty = v_full + TCA_VS;                  // [VS]
+    uint64_t* s_full = v_empty + TCA_VS;                  // [2]
     uint64_t* p_full = s_full + 2;                        // [2]
-    uint64_t* o_full = p_full + 2;                        // [1]
-    uint64_t* o_empty = o_full + 1;                       // [1]
-    uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(o_empty + 1);
+    uint64_t* o_full = p_full + 2;                        // [2]
+    uint64_t* o_empty = o_full + 2;                       // [2]
+    uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(o_empty + 2);
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
     float* xsum = xmax + 2 * 2 * 128;                     // [2 wg][128]
+    float* xc = xsum + 2 * 128;                           // [8 tiles][128] rescale factor of tile j at [j & 7]
 
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
@@ -148,10 +177,10 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     pdl_launch_dependents();
     l2_prefetch_issue(ta.pf);
     if (threadIdx.x == 0) {
-        for (int s = 0; s < TCA_STAGES; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
+        for (int s = 0; s < TCA_KS; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
+        for (int s = 0; s < TCA_VS; ++s) { mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
-        mbar_init(o_full, 1);
-        mbar_init(o_empty, 8);
+        for (int i = 0; i < 2; ++i) { mbar_init(&o_full[i], 1); mbar_init(&o_empty[i], 8); }
         fence_barrier_init();
         tma_prefetch_desc(&tmKV);
     }
@@ -206,50 +235,92 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         constexpr int OPS = 2 * 4 * C::NH;
         const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;
         const int kv = lane / (4 * C::NH), pg = (lane / C::NH) & 3, half = lane % C::NH;
-        for (int j = 0; j < n_tiles; ++j) {
-            const int s = j % TCA_STAGES;
-            int pid = 0;
-            if (lane < OPS) pid = pt[min((k_begin + j * TCA_BN) / TCA_PAGE + pg, a.max_pages - 1)];
-            mbar_wait(&kv_empty[s], ((j / TCA_STAGES) & 1) ^ 1);
-            if (lane == 0) mbar_arrive_expect_tx(&kv_full[s], C::STAGE);
-            __syncwarp();
+        // K and V tiles travel in separate rings: a K tile is released as soon as Q.K^T of its tile has run, a V
+        // tile only after P.V, one tile later; the K stream runs one tile ahead of the V stream.  Page ids are
+        // looked up one iteration ahead (off the critical path).  An L2 look-ahead (cp.async.bulk.prefetch.tensor
+        // of tile j + 8) was tried and removed: the 16 extra 2-KiB boxes per tile go through the same TMA unit as
+        // the loads and made IT the bottleneck (period 3,080 -> 2,380 cycles per tile without; profiles/r1_attention_v2.md).
+        auto box_row = [&](int j) {
+            const int pid = pt[min((k_begin + j * TCA_BN) / TCA_PAGE + pg, a.max_pages - 1)];
+            return ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE;
+        };
+        const bool ld_on = !(ta.dbg & 1);
+        // lanes [0, OPS/2) carry K boxes of tile jk, lanes [OPS/2, OPS) V boxes of tile jv = jk - 1
+        const int dst_off = half * C::KV_HALF + pg * (TCA_PAGE * 128);
+        int row_next = (lane < OPS) ? box_row(0) : 0;    // K lanes: tile 0; V lanes: tile 0 (used one iteration later)
+        int row_cur = row_next;
+        for (int it = 0; it <= n_tiles; ++it) {
+            const int jk = it, jv = it - 1;
+            const int jmine = kv ? jv : jk;
             if (lane < OPS) {
-                uint8_t* dst = kv_s + s * C::STAGE + kv * C::K_BYTES + half * C::KV_HALF + pg * (TCA_PAGE * 128);
-                tma_load_2d(dst, &tmKV, &kv_full[s], half * 64, ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE);
+                row_cur = row_next;
+                if (jmine + 1 < n_tiles) row_next = box_row(jmine + 1);
+            }
+            if (jk < n_tiles) {
+                const int sk = jk % TCA_KS;
+                mbar_wait(&k_empty[sk], ((jk / TCA_KS) & 1) ^ 1);
+                if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&k_full[sk], C::K_BYTES); else mbar_arrive(&k_full[sk]); }
+                __syncwarp();
+                if (lane < OPS / 2 && ld_on) tma_load_2d(kv_s + sk * C::K_BYTES + dst_off, &tmKV, &k_full[sk], half * 64, row_cur);
+            }
+            if (jv >= 0) {
+                const int sv = jv % TCA_VS;
+                mbar_wait(&v_empty[sv], ((jv / TCA_VS) & 1) ^ 1);
+                if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&v_full[sv], C::K_BYTES); else mbar_arrive(&v_full[sv]); }
+                __syncwarp();
+                if (lane >= OPS / 2 && lane < OPS && ld_on)
+                    tma_load_2d(kv_s + (TCA_KS + sv) * C::K_BYTES + dst_off, &tmKV, &v_full[sv], half * 64, row_cur);
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {
-            // ===== MMA issuer =====
-            constexpr uint32_t idesc_qk = umma_idesc_bf16(128, TCA_BN, 0);
-            constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 1);
-            const uint32_t q_addr = smem_u32(q_s);
-            auto issue_pv = [&](int i) {
-                const int s = i % TCA_STAGES;
-                mbar_wait(&p_full[i & 1], (i >> 1) & 1);
-                if (i >= 1) mbar_wait(o_empty, (i - 1) & 1);
-                tc_fence_after();
-                const uint32_t v_addr = smem_u32(kv_s + s * C::STAGE + C::K_BYTES);
-                const uint64_t vdesc = umma_desc_mn128(v_addr, C::KV_HALF, 1024);
-                bool first = true;
+        // ===== MMA issuer.  The WHOLE warp runs the loop (so addresses and descriptors are provably warp-uniform and
+        // live in uniform registers); one elected lane issues.  Under `if (lane == 0)` the compiler wrapped every
+        // tcgen05.mma in an ELECT / R2UR / BRA.U.ANY loop: ~100 cycles per instruction, 36 instructions per tile,
+        // which made this thread - not the tensor pipe, not the softmax - the bottleneck (profiles/r1_attention_v2.md).
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(128, TCA_BN, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 1);
+        const bool leader = elect_one();
+        const bool do_mma = !(ta.dbg & 2);
+        const uint32_t q_addr = smem_u32(q_s);
+        const uint32_t kv_addr = smem_u32(kv_s);
+        const bool mts = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;
+        long long mt_p = 0, mt_o = 0, mt_kv = 0;
+        auto issue_pv = [&](int i) {
+            const int s = i % TCA_VS;
+            mbar_wait(&v_full[s], (i / TCA_VS) & 1);
+            const long long t0_ = mts ? clock64() : 0;
+            mbar_wait(&p_full[i & 1], (i >> 1) & 1);
+            const long long t1_ = mts ? clock64() : 0;
+            mbar_wait(&o_empty[i & 1], ((i >> 1) & 1) ^ 1);   // the correction warps have read chunk i - 2
+            if (mts) { const long long t2_ = clock64(); mt_p += t1_ - t0_; mt_o += t2_ - t1_; }
+            tc_fence_after();
+            const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, C::KV_HALF, 1024);
+            const uint32_t d_addr = tmem_base + C::TO + (i & 1) * D;
+            const uint32_t p_addr = tmem_base + C::TP + (i & 1) * C::SP;
+            if (leader && do_mma) {
 #pragma unroll
                 for (int part = 2; part >= 0; --part) {
 #pragma unroll
-                    for (int t = 0; t < TCA_BN / 16; ++t) {
-                        umma_bf16_ts(tmem_base + C::TO, tmem_base + C::TP + (i & 1) * 96 + part * 32 + t * 8,
-                                     vdesc + (uint64_t)(t * (16 * 128 >> 4)), idesc_pv, first ? 0u : 1u);
-                        first = false;
-                    }
+                    for (int t = 0; t < TCA_BN / 16; ++t)
+                        umma_bf16_ts(d_addr, p_addr + part * 32 + t * 8, vdesc + (uint64_t)(t * (16 * 128 >> 4)), idesc_pv,
+                                     (part == 2 && t == 0) ? 0u : 1u);
                 }
-                umma_commit(&kv_empty[s]);
-                umma_commit(o_full);
-            };
-            for (int j = 0; j < n_tiles; ++j) {
-                const int s = j % TCA_STAGES;
-                mbar_wait(&kv_full[s], (j / TCA_STAGES) & 1);
-                tc_fence_after();
-                const uint32_t k_addr = smem_u32(kv_s + s * C::STAGE);
-                bool first = true;
+            }
+            if (leader) {
+                umma_commit(&v_empty[s]);
+                umma_commit(&o_full[i & 1]);
+            }
+            __syncwarp();
+        };
+        for (int j = 0; j < n_tiles; ++j) {
+            const int s = j % TCA_KS;
+            const long long t0_ = mts ? clock64() : 0;
+            mbar_wait(&k_full[s], (j / TCA_KS) & 1);
+            if (mts) mt_kv += clock64() - t0_;
+            tc_fence_after();
+            const uint32_t k_addr = kv_addr + s * C::K_BYTES;
+            const uint32_t s_addr = tmem_base + C::TS + (j & 1) * C::SP;
+            if (leader && do_mma) {
 #pragma unroll
                 for (int part = 2; part >= 0; --part) {
 #pragma unroll
@@ -257,20 +328,23 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                         const uint64_t adesc = umma_desc_k128(q_addr + part * C::Q_PART + h * (128 * 128));
                         const uint64_t bdesc = umma_desc_k128(k_addr + h * C::KV_HALF);
 #pragma unroll
-                        for (int ks = 0; ks < 4; ++ks) {  // UMMA K = 16 bf16 = 32 B
-                            umma_bf16_ss(tmem_base + C::TS + (j & 1) * TCA_BN, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, first ? 0u : 1u);
-                            first = false;
-                        }
+                        for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 bf16 = 32 B
+                            umma_bf16_ss(s_addr, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, (part == 2 && h == 0 && ks == 0) ? 0u : 1u);
                     }
                 }
-                umma_commit(&s_full[j & 1]);
-                if (j >= 1) issue_pv(j - 1);
             }
-            issue_pv(n_tiles - 1);
+            if (leader) {
+                umma_commit(&k_empty[s]);
+                umma_commit(&s_full[j & 1]);
+            }
+            __syncwarp();
+            if (j >= 1) issue_pv(j - 1);
         }
-    } else {
-        // ===== softmax / correction: thread = (row, warpgroup); wg handles keys [32 wg, +32) of a tile and
-        // output columns [DH wg, +DH).  Warp w may touch TMEM lanes 32 (w % 4) .. +31. =====
+        issue_pv(n_tiles - 1);
+        if (mts && leader) { a.ts[14] = (unsigned long long)mt_p; a.ts[15] = (unsigned long long)(mt_kv + (mt_o << 32)); }
+    } else if (warp < 10) {
+        // ===== softmax: thread = (row, wg); wg handles keys [32 wg, +32) of every tile.  Warp w may touch TMEM
+        // lanes 32 (w % 4) .. +31; the two warps of a row quarter meet behind named barrier 1 + (w % 4). =====
         const int wg = (warp - 2) >> 2;
         const int r = (warp & 3) * 32 + lane;
         const int row = rg * 128 + r;
@@ -279,87 +353,127 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const unsigned long long anc = valid ? a.anc[b * a.T + node] : 1ull;
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
-        float o[C::DH];
-#pragma unroll
-        for (int i = 0; i < C::DH; ++i) o[i] = 0.f;
-        float m_run = -INFINITY, l_run = 0.f, c_prev = 0.f;
+        float m_run = -INFINITY, l_run = 0.f;
 
-        auto correct = [&](int i) {  // O = O * c_prev + Oc(i)
-            mbar_wait(o_full, i & 1);
-            tc_fence_after();
-#pragma unroll
-            for (int cb = 0; cb < C::DH / 32; ++cb) {
-                uint32_t ov[32];
-                tmem_ld32(lane_addr + C::TO + wg * C::DH + cb * 32, ov);
-                tmem_ld_wait();
-                if (cb == C::DH / 32 - 1) {
-                    tc_fence_before();
-                    __syncwarp();
-                    if (lane == 0) mbar_arrive(o_empty);
-                }
-#pragma unroll
-                for (int e = 0; e < 32; ++e) o[cb * 32 + e] = fmaf(o[cb * 32 + e], c_prev, __uint_as_float(ov[e]));
-            }
-        };
-
+        const bool tsw = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;  // bring-up: phase cycles of one warp
+        long long tph[5] = {0, 0, 0, 0, 0}, tq = tsw ? clock64() : 0;
+#define TPH(k) do { if (tsw) { const long long t_ = clock64(); tph[k] += t_ - tq; tq = t_; } } while (0)
         for (int j = 0; j < n_tiles; ++j) {
             mbar_wait(&s_full[j & 1], (j >> 1) & 1);
             tc_fence_after();
+            TPH(0);
             uint32_t sv[32];
-            tmem_ld32(lane_addr + C::TS + (j & 1) * TCA_BN + wg * 32, sv);
+            tmem_ld32(lane_addr + C::TS + (j & 1) * C::SP + wg * 32, sv);
             tmem_ld_wait();
+            TPH(1);
             const int kb = k_begin + j * TCA_BN + wg * 32;
-            const bool need_mask = kb + 32 > L;   // tile half touches tree keys or the end of the key range
-            float mx = -INFINITY;
 #pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                float v = mul_rn(__uint_as_float(sv[e]), a.scale);
-                if (need_mask) {
+            for (int e = 0; e < 32; ++e) sv[e] = __float_as_uint(mul_rn(__uint_as_float(sv[e]), a.scale));  // s = (q.k) / sqrt(d), rounded as the method states
+            if (kb + 32 > L) {   // tile half touches tree keys or the end of the key range (warp-uniform)
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
                     const int kidx = kb + e;
                     const bool ok = kidx < k_end && (kidx < L || ((anc >> (kidx - L)) & 1ull));
-                    if (!ok) v = -INFINITY;
+                    if (!ok) sv[e] = 0xFF800000u;  // -inf
                 }
-                sv[e] = __float_as_uint(v);
-                mx = fmaxf(mx, v);
             }
+            float mx0 = fmaxf(__uint_as_float(sv[0]), __uint_as_float(sv[1])), mx1 = fmaxf(__uint_as_float(sv[2]), __uint_as_float(sv[3]));
+#pragma unroll
+            for (int e = 4; e < 32; e += 2) {
+                mx0 = fmaxf(mx0, __uint_as_float(sv[e]));
+                mx1 = fmaxf(mx1, __uint_as_float(sv[e + 1]));
+            }
+            float mx = fmaxf(mx0, mx1);
             xmax[((j & 1) * 2 + wg) * 128 + r] = mx;
-            softmax_bar_sync();
+            pair_bar_sync(1 + (warp & 3));
             mx = fmaxf(mx, xmax[((j & 1) * 2 + (wg ^ 1)) * 128 + r]);
+            TPH(2);
             const float mn = fmaxf(m_run, mx);
             const float mu = (mn == -INFINITY) ? 0.f : mn;
             const float c = ex2_approx((m_run - mu) * LOG2E);  // 2^-inf = 0 on the first tile
             m_run = mn;
-            float ls = 0.f;
-            uint32_t ph[16], pm[16], pl[16];
+            if (wg == 0) xc[(j & 7) * 128 + r] = c;
+            const float nmk = -mu * LOG2E;
+            float ls0 = 0.f, ls1 = 0.f;
+            const uint32_t p_addr = lane_addr + C::TP + (j & 1) * C::SP + wg * 16;
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                const float p0 = ex2_approx((__uint_as_float(sv[2 * e]) - mu) * LOG2E);
-                const float p1 = ex2_approx((__uint_as_float(sv[2 * e + 1]) - mu) * LOG2E);
-                ls += p0 + p1;
-                split3_pack(p0, p1, ph[e], pm[e], pl[e]);
+            for (int h = 0; h < 2; ++h) {
+                uint32_t ph[8], pm[8], pl[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const float p0 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e]), LOG2E, nmk));
+                    const float p1 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e + 1]), LOG2E, nmk));
+                    ls0 += p0;
+                    ls1 += p1;
+                    split3_pack(p0, p1, ph[e], pm[e], pl[e]);
+                }
+                tmem_st8(p_addr + h * 8, ph);
+                tmem_st8(p_addr + 32 + h * 8, pm);
+                tmem_st8(p_addr + 64 + h * 8, pl);
             }
-            l_run = fmaf(l_run, c, ls);
-            const uint32_t p_addr = lane_addr + C::TP + (j & 1) * 96 + wg * 16;
-            tmem_st16(p_addr, ph);
-            tmem_st16(p_addr + 32, pm);
-            tmem_st16(p_addr + 64, pl);
+            l_run = fmaf(l_run, c, ls0 + ls1);
+            TPH(3);
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&p_full[j & 1]);
-            if (j >= 1) correct(j - 1);
-            c_prev = c;
+            TPH(4);
         }
-        correct(n_tiles - 1);
-        // ---- partial result of this split: O (unnormalised), running max, running sum ----
+        if (tsw && lane == 0) {
+            if (warp == 2) {
+                for (int k = 0; k < 5; ++k) a.ts[k] = (unsigned long long)tph[k];
+                a.ts[5] = (unsigned long long)n_tiles;
+            }
+            a.ts[6 + warp - 2] = (unsigned long long)(tph[1] + tph[2] + tph[3] + tph[4]);
+        }
+#undef TPH
+        // ---- running max and sum of this split ----
         xsum[wg * 128 + r] = l_run;
-        softmax_bar_sync();
+        pair_bar_sync(1 + (warp & 3));
+        if (valid && wg == 0) {
+            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
+            *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m_run, l_run + xsum[128 + r]);
+        }
+    } else {
+        // ===== correction: thread = (row, half of d).  O = O * c(i) + Oc(i), one rounded fp32 operation per tile;
+        // c(i) was published by the softmax warps before they released P(i), which Oc(i) depends on. =====
+        const int hh = (warp - 10) >> 2;
+        const int r = (warp & 3) * 32 + lane;
+        const int row = rg * 128 + r;
+        const int node = row / a.G, gi = row % a.G;
+        const bool valid = row < R && node < nn;
+        const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
+        float o[C::DH];
+#pragma unroll
+        for (int i = 0; i < C::DH; ++i) o[i] = 0.f;
+        for (int i = 0; i < n_tiles; ++i) {
+            mbar_wait(&o_full[i & 1], (i >> 1) & 1);
+            tc_fence_after();
+            const float c = xc[(i & 7) * 128 + r];
+#pragma unroll
+            for (int cb = 0; cb < C::DH / 16; ++cb) {
+                uint32_t ov[16];
+                if (!(ta.dbg & 4)) {
+                    tmem_ld16(lane_addr + C::TO + (i & 1) * D + hh * C::DH + cb * 16, ov);
+                    tmem_ld_wait();
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) ov[e] = 0;
+                }
+                if (cb == C::DH / 16 - 1) {
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&o_empty[i & 1]);
+                }
+#pragma unroll
+                for (int e = 0; e < 16; ++e) o[cb * 16 + e] = fmaf(o[cb * 16 + e], c, __uint_as_float(ov[e]));
+            }
+        }
         if (valid) {
             const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
-            float* op = a.o_part + pi * D + wg * C::DH;
+            float* op = a.o_part + pi * D + hh * C::DH;
 #pragma unroll
             for (int i = 0; i < C::DH; i += 4) *reinterpret_cast<float4*>(op + i) = make_float4(o[i], o[i + 1], o[i + 2], o[i + 3]);
-            if (wg == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m_run, l_run + xsum[128 + r]);
         }
     }
     tc_fence_before();
