@@ -171,6 +171,7 @@ struct ev_model {
     // L2 weight stream (PfPlanner): on for token counts <= l2pf_max_m; bytes the stream may run ahead / per launch
     int l2pf_max_m = 0;
     long l2pf_cap = 88L << 20, l2pf_maxq = 40L << 20;
+    unsigned l2pf_mask = 0xFFFFFFFFu;
     std::vector<ProfRec> prof;
     size_t prof_used = 0;
     // captured verify steps (CUDA graphs), keyed by everything a launch depends on
@@ -313,6 +314,23 @@ RowPlan row_plan(const ev_model* m, int M, int row_floats, int cl_par_max = CLUS
         else return fail(EV_EINVAL, "row too long for the row kernels");                                       \
     } while (0)
 
+// row kernels that consume a LinOut: also instantiated for the slab-count bound (1 / 3 / 8) so that the
+// no-split case (M > 256) does not issue seven predicated-off slab loads and adds per element
+#define ROW_DISPATCH_S(plan, splits, KERN, ...)                                                                \
+    do {                                                                                                       \
+        const int s_ = (splits);                                                                               \
+        if (s_ <= 1) ROW_DISPATCH_S1(plan, 1, KERN, __VA_ARGS__);                                              \
+        else if (s_ <= 3) ROW_DISPATCH_S1(plan, 3, KERN, __VA_ARGS__);                                         \
+        else ROW_DISPATCH_S1(plan, 8, KERN, __VA_ARGS__);                                                      \
+    } while (0)
+#define ROW_DISPATCH_S1(plan, S, KERN, ...)                                                                    \
+    do {                                                                                                       \
+        if ((plan).nv4 == 1) EV_TRY(launch_kc((plan).cl, KERN<1, S>, __VA_ARGS__));                            \
+        else if ((plan).nv4 == 2) EV_TRY(launch_kc((plan).cl, KERN<2, S>, __VA_ARGS__));                       \
+        else if ((plan).nv4 == 4) EV_TRY(launch_kc((plan).cl, KERN<4, S>, __VA_ARGS__));                       \
+        else return fail(EV_EINVAL, "row too long for the row kernels");                                       \
+    } while (0)
+
 template <int EPI>
 int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int grid, int smem) {
     static bool attr_set = false;
@@ -370,6 +388,8 @@ struct PfPlanner {
     int next_gemm = 0;
     size_t cap = 0, maxq = 0;
     bool on = false;
+    unsigned mask = 0xFFFFFFFFu;   // which launches of a layer may issue (bit = position in the layer's 10-kernel sequence:
+    int n_take = 0, per_layer = 10, n_layer_launches = 0;   // norm1 qkv rope attn merge o norm2 gu swiglu down; bit 10 = final norm / LM head)
     unsigned long long* trace = nullptr;  // step trace (ev_profile_trace): 4 slots per launch, in launch order
     int n_traced = 0, trace_cap = 0;
     void add(const uint8_t* p, size_t n) {
@@ -386,6 +406,9 @@ struct PfPlanner {
             cursor = std::max(cursor, start[next_gemm + 1]);
             ++next_gemm;
         }
+        const int pos = n_take < n_layer_launches ? n_take % per_layer : per_layer;
+        ++n_take;
+        if (!((mask >> pos) & 1u)) return pf;
         const size_t consumed = start[std::max(0, next_gemm - 1)];
         const size_t ahead = cursor - std::min(cursor, consumed);
         if (ahead >= cap) return pf;
@@ -562,6 +585,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     pfp.on = M <= m->l2pf_max_m && !m->profile && !m->naive_gemm;
     pfp.cap = (size_t)m->l2pf_cap; pfp.maxq = (size_t)m->l2pf_maxq;
     pfp.trace = m->trace; pfp.trace_cap = TRACE_CAP;
+    pfp.mask = m->l2pf_mask; pfp.n_layer_launches = 10 * cfg.n_layers;
     if (pfp.on) {
         auto qbytes = [](const QMat& q) { return (size_t)q.n_tiles * q.total_kb * GEMM_WTILE; };
         for (int l = 0; l < cfg.n_layers; ++l) {
@@ -598,7 +622,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // --- attention block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0), pfp.take(false));
+            ROW_DISPATCH_S(rp_h, pend.p ? pend.splits : 1, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g1, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 0), pfp.take(false));
             pend = none;
         }
         if (tap && out->dev_tap_xq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_xq, m->xq.codes, (size_t)M * H, cudaMemcpyDeviceToDevice, st));
@@ -612,7 +636,9 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ra.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ROPE_KV);
-            EV_TRY(launch_k(rope_kvwrite_kernel, dim3(M, rope_gy), dim3(ROPE_THREADS), 0, st, ra));
+            if (ra.lin.splits <= 1) EV_TRY(launch_k(rope_kvwrite_kernel<1>, dim3(M, rope_gy), dim3(ROPE_THREADS), 0, st, ra));
+            else if (ra.lin.splits <= 3) EV_TRY(launch_k(rope_kvwrite_kernel<3>, dim3(M, rope_gy), dim3(ROPE_THREADS), 0, st, ra));
+            else EV_TRY(launch_k(rope_kvwrite_kernel<8>, dim3(M, rope_gy), dim3(ROPE_THREADS), 0, st, ra));
         }
         if (tap && out->dev_tap_qkv) EV_TRY(copy_f32(st, m->qkv, out->dev_tap_qkv, (long)M * m->qkv_dim));
         AttnArgs aa;
@@ -654,7 +680,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // --- MLP block ---
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2), pfp.take(false));
+            ROW_DISPATCH_S(rp_h, pend.p ? pend.splits : 1, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, w.g2, cfg.rms_eps, quant_out(m, m->xq, 4 * l + 2), pfp.take(false));
             pend = none;
         }
         LinOut gul;
@@ -673,7 +699,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         if (lockstep) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H)); }
         {
             ProfScope ps(m, st, PC_NORM_QUANT);
-            ROW_DISPATCH(rp_h, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers), pfp.take(false));
+            ROW_DISPATCH_S(rp_h, pend.p ? pend.splits : 1, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers), pfp.take(false));
             pend = none;
         }
         EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM, &pfp));
@@ -754,6 +780,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
     if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
+    if (getenv("EV_L2PF_MASK")) m->l2pf_mask = (unsigned)strtoul(getenv("EV_L2PF_MASK"), nullptr, 0);
     if (getenv("EV_L2PF_CAP_MB")) m->l2pf_cap = (long)atoi(getenv("EV_L2PF_CAP_MB")) << 20;
     if (getenv("EV_L2PF_MAXQ_MB")) m->l2pf_maxq = (long)atoi(getenv("EV_L2PF_MAXQ_MB")) << 20;
     m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;

@@ -216,7 +216,7 @@ __device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
 // the token count so that few rows still fill the machine and many rows keep several CTAs per SM: row_plan()).
 constexpr int ROW_THREADS = 256;
 constexpr int NORM_THREADS = ROW_THREADS;
-template <int NORM_NV4>
+template <int NORM_NV4, int MAXS>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
                                                                      const __nv_bfloat16* __restrict__ gain, float eps,
                                                                      QuantOut q, L2Prefetch pf) {
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
         if (i4 < c1) {
             v[k] = *reinterpret_cast<const float4*>(x + i);
             if (pend.p) {
-                const float4 y = lin_value4(pend, m, i, sxm);
+                const float4 y = lin_value4<MAXS>(pend, m, i, sxm);
                 v[k] = make_float4(add_rn(v[k].x, y.x), add_rn(v[k].y, y.y), add_rn(v[k].z, y.z), add_rn(v[k].w, y.w));
                 *reinterpret_cast<float4*>(x + i) = v[k];
             }
@@ -404,6 +404,7 @@ struct RopeArgs {
     L2Prefetch pf;
 };
 constexpr int ROPE_THREADS = 256;
+template <int MAXS>
 __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) {
     pdl_launch_dependents();
     l2_prefetch_issue(a.pf);
@@ -429,7 +430,7 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
     const int tid = blockIdx.y * blockDim.x + threadIdx.x, nthr = gridDim.y * blockDim.x;  // a row may be spread over gridDim.y CTAs
     for (int i = tid; i < n_rot4; i += nthr) {
         const int head = (i * 4) / D2, j = (i * 4) % D2;
-        const float4 lo = lin_value4(a.lin, m, head * D + j, sxm), hi = lin_value4(a.lin, m, head * D + j + D2, sxm);
+        const float4 lo = lin_value4<MAXS>(a.lin, m, head * D + j, sxm), hi = lin_value4<MAXS>(a.lin, m, head * D + j + D2, sxm);
         const float4 c01 = __ldg(reinterpret_cast<const float4*>(cs + j)), c23 = __ldg(reinterpret_cast<const float4*>(cs + j + 2));
         float4 rlo, rhi;  // (cos, sin) pairs: c01 = (c0, s0, c1, s1), c23 = (c2, s2, c3, s3)
         rlo.x = sub_rn(mul_rn(lo.x, c01.x), mul_rn(hi.x, c01.y)); rhi.x = add_rn(mul_rn(hi.x, c01.x), mul_rn(lo.x, c01.y));
@@ -449,7 +450,7 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
     const int voff = (a.Hq + a.Hkv) * D;
     for (int i = tid; i < a.Hkv * D / 4; i += nthr) {
         const int head = (i * 4) / D, j = (i * 4) % D;
-        const float4 v = lin_value4(a.lin, m, voff + i * 4, sxm);
+        const float4 v = lin_value4<MAXS>(a.lin, m, voff + i * 4, sxm);
         *reinterpret_cast<float4*>(row + voff + i * 4) = v;
         if (write) {
             __nv_bfloat162 p0 = __floats2bfloat162_rn(v.x, v.y), p1 = __floats2bfloat162_rn(v.z, v.w);

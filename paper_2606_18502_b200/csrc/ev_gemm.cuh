@@ -308,22 +308,27 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     if (lane == 0) mbar_arrive(&tmem_empty_bar[buf]);
                 }
                 if (EPI == EPI_ARGMAX) {
-                    // per token: max over the tile's 128 channels of (ordered logit, ~index); warp shuffle, then the 4
-                    // warps meet in shared memory and ONE atomicMax per (token, tile) goes to global memory
+                    // per token: max over the tile's 128 channels of (ordered logit, ~index).  Two warp-wide integer
+                    // reductions per token (redux.sync: max of the ordered logit bits, then min of the channel index
+                    // among the lanes that hold that maximum = lowest id on ties) instead of a 5-round shuffle tree
+                    // on 64-bit keys (the shuffle tree made the LM head's epilogue, not its MMAs, the bound at M = 832);
+                    // lane j keeps token j's key, then the 4 warps meet in shared memory and ONE atomicMax per
+                    // (token, tile) goes to global memory
+                    uint32_t kmx = 0u, kmn = 0xFFFFFFFFu;
 #pragma unroll
                     for (int j = 0; j < GC; ++j) {
                         const int col = g * GC + j;
                         const int m = m0 + col;
                         const float y = mul_rn(mul_rn(__uint_as_float(v[j]), sxs[col < a.tok ? col : 0]), swn);
-                        unsigned long long key = (n_ok && col < a.tok && m < a.M) ? (((unsigned long long)ordered_bits(y) << 32) | (0xFFFFFFFFu - (uint32_t)n)) : 0ull;
-#pragma unroll
-                        for (int o = 16; o > 0; o >>= 1) {
-                            const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
-                            key = other > key ? other : key;
-                        }
-                        if (lane == 0 && col < a.tok) keys_smem[q * 256 + col] = key;
-                        if (n_ok && col < a.tok && m < a.M && a.out) __stcs(a.out + (size_t)m * a.ldo + n, y);
+                        const bool ok = n_ok && col < a.tok && m < a.M;
+                        const uint32_t ob = ok ? ordered_bits(y) : 0u;      // ordered_bits of a non-NaN value is never 0
+                        const uint32_t mx = __reduce_max_sync(0xffffffffu, ob);
+                        const uint32_t mn = __reduce_min_sync(0xffffffffu, (ok && ob == mx) ? (uint32_t)n : 0xFFFFFFFFu);
+                        if (lane == j) { kmx = mx; kmn = mn; }
+                        if (ok && a.out) __stcs(a.out + (size_t)m * a.ldo + n, y);
                     }
+                    if (g * GC + lane < a.tok)   // no valid lane: (0, ~0xFFFFFFFF) = key 0, below every real key
+                        keys_smem[q * 256 + g * GC + lane] = ((unsigned long long)kmx << 32) | (0xFFFFFFFFu - kmn);
                 } else {
 #pragma unroll
                     for (int j = 0; j < GC; ++j) {
