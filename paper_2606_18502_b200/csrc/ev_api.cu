@@ -78,14 +78,18 @@ int make_tmap(CUtensorMap* tm, const void* base, long rows, long cols, int box_r
     return EV_OK;
 }
 
-// KV pool as a 2-D bf16 tensor [rows = (layer, page, K|V, head, token)][D], box = 16 tokens x 64 dims (128 B), 128-byte swizzle
+// KV pool as a 4-D tensor of 2-byte elements over its rows = (layer, page, K|V, head, token) of D elements:
+// (64 elements of a 128-byte half row, 8 rows of a swizzle group, D/64 half rows, rows/8 groups).  A box of
+// (64, 8, D/64, 2) is one whole 16-token (page, K|V, head) block - 4 KiB contiguous in HBM at D = 128 - and lands
+// in shared memory as [group][half][8 rows x 128 B]: every 1-KiB swizzle atom whole, 8-row groups of one half
+// D/64 KiB apart (the UMMA stride byte offset).  One TMA instruction per block instead of one per half block.
 int make_tmap_kv(CUtensorMap* tm, const void* base, long rows, int D) {
     EV_TRY(get_encode());
-    cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)rows};
-    cuuint64_t strides[1] = {(cuuint64_t)D * 2};
-    cuuint32_t box[2] = {64u, (cuuint32_t)TCA_PAGE};
-    cuuint32_t estr[2] = {1u, 1u};
-    CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+    cuuint64_t dims[4] = {64u, 8u, (cuuint64_t)(D / 64), (cuuint64_t)(rows / 8)};
+    cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128u, (cuuint64_t)D * 2 * 8};
+    cuuint32_t box[4] = {64u, 8u, (cuuint32_t)(D / 64), (cuuint32_t)(TCA_PAGE / 8)};
+    cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    CUresult r = g_encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 4, const_cast<void*>(base), dims, strides, box, estr,
                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(EV_ECUDA, "cuTensorMapEncodeTiled (KV pool) failed, code " + std::to_string((int)r));
@@ -168,6 +172,7 @@ struct ev_model {
     int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
+    bool gemm_mc = true;   // multicast CTA pairs for the many-row GEMMs (EV_GEMM_MC=0 turns them off)
     // L2 weight stream (PfPlanner): on for token counts <= l2pf_max_m; bytes the stream may run ahead / per launch
     int l2pf_max_m = 0;
     long l2pf_cap = 88L << 20, l2pf_maxq = 40L << 20;
@@ -197,6 +202,7 @@ struct ev_cache {
     std::vector<int> len_bound;  // host-side upper bound of each sequence's ctx_len (sizes the key-split grid)
     CUtensorMap tmKV;            // whole pool, for the tcgen05 attention kernel
     bool tc_attn = false;        // page_size == 16 and the pool fits 32-bit row coordinates
+    bool kv_f16 = false;         // the pool keeps the bf16-rounded K/V values in binary16 containers (tcgen05 attention; ev_common.cuh)
     // prefill staging
     int32_t *pf_tokens = nullptr, *pf_parents = nullptr, *pf_nn = nullptr, *pf_slots = nullptr;
     int32_t *pf_out = nullptr;
@@ -332,7 +338,7 @@ RowPlan row_plan(const ev_model* m, int M, int row_floats, int cl_par_max = CLUS
     } while (0)
 
 template <int EPI>
-int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int grid, int smem) {
+int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const CUtensorMap& tmXh, const GemmArgs& a, int grid, int smem) {
     static bool attr_set = false;
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
@@ -344,12 +350,17 @@ int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const GemmArgs& a, int 
     cfg.blockDim = dim3(GEMM_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute at[1];
+    cudaLaunchAttribute at[2];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;  // PDL: weight prefetch overlaps the previous kernel
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_e4m3_kernel<EPI>, tmX, a));
+    if (a.mc) {  // multicast pairs: clusters of 2 CTAs along x
+        at[1].id = cudaLaunchAttributeClusterDimension;
+        at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+        cfg.numAttrs = 2;
+    }
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_e4m3_kernel<EPI>, tmX, tmXh, a));
     ++g_launches;
     return EV_OK;
 }
@@ -464,32 +475,49 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     if (pfp) a.pf = pfp->take(true);
     a.dbg = m->gemm_dbg;
     a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
-    // Few token rows (one token tile): stream-K - the n_tiles * total_kb K-blocks are dealt out evenly to the
-    // CTAs (ev_gemm.cuh), each tile's pieces land in slabs the consumer adds in K order.  The partition depends
-    // only on the matrix shape and the SM count, never on M: a token's result is batch-invariant.
+    // Multicast pairs (many token rows: several token tiles): the GEMM is then bound by the L2 -> SM fill of its
+    // operand tiles (16 KiB of W + tok x 128 B of X per K-block and CTA).  Adjacent n tiles of the same token tile
+    // run as a cluster of two CTAs; each fetches half of the token tile and the TMA unit multicasts it to both, so
+    // the pair behaves like one 256 x tok tile: a third less L2 traffic per flop.
     const int G = m->num_sms;
-    const int tiles = a.n_tiles * a.m_tiles;
+    a.mc = 0; a.tok_h0 = a.tok;
+    if (m->gemm_mc && a.m_tiles >= 2 && a.n_tiles % 2 == 0 && a.tok >= 32) {
+        a.mc = 1;
+        a.tok_h0 = 16 * ((a.tok / 16 + 1) / 2);
+    }
+    const int nmul = a.mc ? 2 : 1;                       // n tiles per scheduling unit
+    const int Gc = a.mc ? G / 2 : G;                     // CTAs, or CTA pairs
+    const int tiles = (a.n_tiles / nmul) * a.m_tiles;    // (n tile or pair of n tiles, token tile)
     a.k_splits = 1;
     a.kb_per_split = a.total_kb;
     a.sk_units = 0;
-    int grid = std::min(tiles, G);
+    int grid = nmul * std::min(tiles, Gc);
     if (lin) { lin->splits = 1; lin->sk_G = 0; lin->sk_U = 0; lin->sk_kb = 0; }
-    if (m->use_splitk && epi == EPI_RAW && a.m_tiles == 1) {
-        const int U = a.n_tiles * a.total_kb;
-        const int g = std::min(G, U);
+    // Stream-K (one token tile): the n_tiles * total_kb K-blocks are dealt out evenly to the CTAs (ev_gemm.cuh); each
+    // tile's pieces land in slabs the consumer adds in K order.  The partition depends only on the matrix shape and
+    // the SM count, never on M: a token's result is batch-invariant.  (Tried for several token tiles too, where
+    // whole tiles leave a partial last wave - 896 tiles on 148 CTAs: the GEMMs did not get faster and the consumers
+    // paid for the second slab: config[2] 17.2 -> 19.3 ms; the kernel keeps the generality, the plan does not use it.)
+    if (m->use_splitk && epi == EPI_RAW) {
+        const int U = tiles * a.total_kb;
+        const int g = std::min(Gc, U);
+        const bool worth = a.m_tiles == 1;
         int pmax = 1;
-        for (int t = 0; t < a.n_tiles; ++t)
+        for (int t = 0; t < tiles && worth; ++t)
             pmax = std::max(pmax, sk_first_cta((t + 1) * a.total_kb - 1, g, U) - sk_first_cta(t * a.total_kb, g, U) + 1);
-        if (pmax <= 8 && (long)pmax * M * a.N <= m->lin_floats) {
+        if (worth && pmax <= 8 && (long)pmax * M * a.N <= m->lin_floats) {
             a.sk_units = U;
-            grid = g;
-            if (lin) { lin->splits = pmax; lin->sk_G = g; lin->sk_U = U; lin->sk_kb = a.total_kb; }
+            grid = nmul * g;
+            if (lin) {
+                lin->splits = pmax; lin->sk_G = g; lin->sk_U = U; lin->sk_kb = a.total_kb;
+            }
         }
     }
     const int smem = a.stages * stage_bytes + 512 + 2048 + 8192 + 1024;  // stages + barriers + sx staging + argmax keys + alignment slack
-    const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
-    if (epi == EPI_RAW) return launch_gemm<EPI_RAW>(st, tmX, a, grid, smem);
-    return launch_gemm<EPI_ARGMAX>(st, tmX, a, grid, smem);
+    const CUtensorMap& tmX = x.tm[(a.mc ? a.tok_h0 : a.tok) / 16 - 1];
+    const CUtensorMap& tmXh = x.tm[(a.mc ? a.tok - a.tok_h0 : a.tok) / 16 - 1];
+    if (epi == EPI_RAW) return launch_gemm<EPI_RAW>(st, tmX, tmXh, a, grid, smem);
+    return launch_gemm<EPI_ARGMAX>(st, tmX, tmXh, a, grid, smem);
 }
 
 QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
@@ -633,6 +661,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ra.pos = m->pos; ra.cs = m->rope_cs; ra.seq_slots = in->dev_seq_slots; ra.Lsnap = m->Lsnap; ra.nn_eff = m->nn_eff;
         ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
         ra.pool = c->pool + (size_t)l * c->layer_stride;
+        ra.kv_f16 = c->kv_f16;
         ra.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ROPE_KV);
@@ -652,7 +681,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
-            if (c->tc_attn && !m->legacy_attn) {
+            if (c->kv_f16) {
                 TcAttnArgs ta;
                 ta.a = aa;
                 ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
@@ -779,6 +808,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->use_splitk = !(getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) == 0);  // on by default
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
+    m->gemm_mc = !(getenv("EV_GEMM_MC") && atoi(getenv("EV_GEMM_MC")) == 0);
     if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
     if (getenv("EV_L2PF_MASK")) m->l2pf_mask = (unsigned)strtoul(getenv("EV_L2PF_MASK"), nullptr, 0);
     if (getenv("EV_L2PF_CAP_MB")) m->l2pf_cap = (long)atoi(getenv("EV_L2PF_CAP_MB")) << 20;
@@ -984,6 +1014,7 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
                 return EV_ECUDA;
             }
             c->tc_attn = true;
+            c->kv_f16 = !m->legacy_attn;
         }
     }
     cudaMemset(c->page_table, 0, (size_t)max_seqs * c->max_pages * 4);
@@ -1102,7 +1133,7 @@ static int dense_copy(ev_cache* c, int slot, int lb, int le, int n_tokens, void*
     DenseCopyArgs a;
     a.Hkv = cfg.n_kv_heads; a.D = cfg.head_dim; a.page_size = cfg.page_size; a.n_tokens = n_tokens; a.layer_begin = lb;
     a.layer_stride = c->layer_stride; a.pool = c->pool; a.page_row = c->page_table + (size_t)slot * c->max_pages;
-    a.dense = (__nv_bfloat16*)dense; a.to_dense = to_dense;
+    a.dense = (__nv_bfloat16*)dense; a.to_dense = to_dense; a.kv_f16 = c->kv_f16;
     dense_copy_kernel<<<dim3(n_tokens, le - lb), 128, 0, st>>>(a);
     LAUNCH_CHECK();
     return EV_OK;

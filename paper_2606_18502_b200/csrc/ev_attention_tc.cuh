@@ -4,24 +4,32 @@
 // rows = tree nodes x GQA group; partial (O, max, sum) per split, merged by attn_merge_quant_kernel.
 //
 // Data flow per 64-key tile j (a CTA walks its key range tile by tile):
-//   TMA warp      : 4 pages x {K,V} x {d-halves} boxes of 16 tokens x 64 dims -> 128-byte-swizzled smem
-//                   (the pool's 4 KiB (page, K|V, head) blocks are read in place through one 2-D tensor map)
+//   TMA warp      : 4 pages x {K,V} boxes, each a whole (page, K|V, head) block of 16 tokens x D -> 128-byte-swizzled
+//                   smem as [page][8-token group][d half][8 x 128 B] (read in place through one 4-D tensor map)
 //   MMA thread    : S[j&1]  = Q . K_j^T   (tcgen05.mma kind::f16, A = Q from smem, B = K tile, D in TMEM)
 //                   Oc      = P[j&1] . V_j (A = P from TMEM, B = V tile MN-major, D in TMEM, from zero)
 //   8 softmax warps (thread = one query row x half of the tile's keys):
 //                   S -> registers (tcgen05.ld), tree mask, online max (the two halves of a row meet in shared
 //                   memory behind a 64-thread named barrier), p = 2^(s k - m k), k = log2(e)/sqrt(d), one FFMA +
-//                   one MUFU per key, P -> hi|mid|lo bf16 -> TMEM (tcgen05.st); publishes the tile's rescale
+//                   one MUFU per key, P -> hi|lo fp16 -> TMEM (tcgen05.st); publishes the tile's rescale
 //                   factor c = exp(m_old - m_new) in shared memory
 //   8 correction warps (thread = one query row x half of d): Oc -> registers and
 //                   O = O * c + Oc with ONE rounded fp32 operation per tile, concurrently with the softmax of
 //                   the next tile (the two used to be serial in the same threads: 3,700 cycles per tile against
 //                   a tensor floor of 1,536; profiles/r1_attention_v2.md).
-// Precision (DESIGN.md section 6 "attention precision"): Q and P are fp32 values split into hi+mid+lo bf16
-// parts (3 x 8 significand bits: exact), K and V are bf16, so every product is exact; the tensor core only
-// accumulates (smallest parts first).  The running output lives in registers, not in TMEM, because long
-// tensor-core accumulation chains truncate.
+// Precision (DESIGN.md section 6 "attention precision"): Q and P are fp32 values split into hi+lo fp16 parts
+// (2 x 11 significand bits: x = hi + lo to 2^-22 relative, the size of one fp32 rounding of the sum), K and V
+// are bf16 VALUES in binary16 containers (ev_common.cuh "KV pool containers"): kind::f16 wants A and B in the same
+// format (fp16 A with bf16 B is an illegal instruction on sm_100a; converting the tiles in shared memory inside
+// this kernel made the converting warps the bottleneck), so rope_kvwrite_kernel and the import path store them
+// that way.  Every product is then exact (11 + 8 bits) and the tensor core only accumulates (small parts first).  Both are
+// scaled by a power of two before the split so that the lo parts stay out of fp16's subnormals: Q by 2^6 (undone
+// exactly in the 1/sqrt(d) multiply), P by 2^15 (p <= 1; the row sum and the running output carry the factor and
+// drop it, exactly, when the partial is written).  The first version used three bf16 parts (exact, 3x the
+// tensor work): the tensor pipe bounded the kernel at batch 32.  The running output lives in registers, not in
+// TMEM, because long tensor-core accumulation chains truncate.
 #pragma once
+#include <cuda_fp16.h>
 #include "ev_common.cuh"
 #include "ev_attention.cuh"
 
@@ -29,28 +37,30 @@ namespace ev {
 
 constexpr int TCA_THREADS = 576;  // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 softmax, warps 10..17 correction
 constexpr int TCA_BN = 64;        // keys per tile (= ATT_CH: the split plan is shared with the legacy kernel)
-constexpr int TCA_KS = 4;        // K ring depth (a K tile is released by Q.K^T, early)
-constexpr int TCA_VS = 3;        // V ring depth (a V tile is released by P.V)
+constexpr int TCA_KS = 5;        // K ring depth (a K tile is released by Q.K^T, early)
+constexpr int TCA_VS = 4;        // V ring depth (a V tile is released by P.V)
 constexpr int TCA_PAGE = 16;      // tokens per page this kernel is built for
 
 template <int D>
 struct TcaCfg {
     static constexpr int NH = D / 64;                    // 128-byte (64-element) halves of a head row
     static constexpr int Q_PART = NH * 128 * 128;        // bytes of one bf16 part of the 128 x D query tile
-    static constexpr int Q_BYTES = 3 * Q_PART;
+    static constexpr int Q_BYTES = 2 * Q_PART;
     static constexpr int KV_HALF = TCA_BN * 128;         // 8 KiB: 64 keys x 128 B
     static constexpr int K_BYTES = NH * KV_HALF;
+    static constexpr int SBO = NH * 1024;               // 8-token groups of one d half: [page][group][half][1 KiB]
+    static constexpr int PAGE_BYTES = 2 * SBO;          // one 16-token (page, K|V, head) block
     static constexpr int BAR_BYTES = 256;
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
     static constexpr int SMEM = 1024 + Q_BYTES + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;
     // TMEM columns
-    // S[2] and P[2] share two 96-column regions: S(j) = 64 fp32 columns, P(j) = 3 parts x 32 columns (64 bf16
+    // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
     // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that); that
     // frees room for TWO O chunks, so P.V of tile j+1 does not wait for the correction warps to read chunk j.
     static constexpr int TS = 0;
     static constexpr int TP = 0;
-    static constexpr int SP = 96;           // columns per S/P region
-    static constexpr int TO = 192;          // O chunks: 2 x D fp32 columns
+    static constexpr int SP = 64;           // columns per S/P region
+    static constexpr int TO = 128;          // O chunks: 2 x D fp32 columns
     static_assert(TO + 2 * D <= 512, "TMEM budget");
     static constexpr int DH = D / 2;        // output columns per softmax warpgroup
 };
@@ -71,10 +81,10 @@ __device__ __forceinline__ void umma_bf16_ts(uint32_t d_tmem, uint32_t a_tmem, u
         "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// instruction descriptor, kind::f16: D fp32, A = B = bf16, A K-major, B K-major (0) or MN-major (1)
-__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int b_mn_major) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
-           ((uint32_t)(M >> 4) << 24);
+// instruction descriptor, kind::f16: D fp32 (bit 4), A format bits 7..9 = B format bits 10..12 = fp16 (0),
+// A K-major, B K-major (0) or MN-major (1)
+__host__ __device__ constexpr uint32_t umma_idesc_f16(int M, int N, int b_mn_major) {
+    return (1u << 4) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
 }
 // MN-major operand tile, 128-byte swizzle: 64 contiguous elements along MN per 128-byte row, rows = K index,
 // 8-row groups SBO apart, next 64 elements along MN LBO apart
@@ -111,11 +121,6 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t* v) {
                  : "memory");
 }
 __device__ __forceinline__ void pair_bar_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
-__device__ __forceinline__ bool elect_one() {  // one lane of a converged warp
-    uint32_t pred;
-    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
-    return pred != 0;
-}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void softmax_bar_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) {
@@ -123,20 +128,17 @@ __device__ __forceinline__ float ex2_approx(float x) {
     asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// (x0, x1) -> packed bf16 pairs hi, mid, lo with x = hi + mid + lo exactly (x0 in the low half).  The parts are
-// cut by TRUNCATION (mask the low 16 bits), not by cvt.rn: the three parts still sum to x exactly (the
-// remainder after taking the top 8 significand bits has at most 16, then at most 8 significant bits), and the
-// work stays on the ALU/FMA pipes: F2FP shares the quarter-rate XU pipe with the softmax's MUFU.EX2 and was the
-// bottleneck of the softmax warps (profiles/r1_attention_v2.md).
-__device__ __forceinline__ void split3_pack(float x0, float x1, uint32_t& hi, uint32_t& mid, uint32_t& lo) {
-    const uint32_t u0 = __float_as_uint(x0), u1 = __float_as_uint(x1);
-    hi = __byte_perm(u0, u1, 0x7632);
-    const float r0 = x0 - __uint_as_float(u0 & 0xFFFF0000u), r1 = x1 - __uint_as_float(u1 & 0xFFFF0000u);
-    const uint32_t v0 = __float_as_uint(r0), v1 = __float_as_uint(r1);
-    mid = __byte_perm(v0, v1, 0x7632);
-    const float t0 = r0 - __uint_as_float(v0 & 0xFFFF0000u), t1 = r1 - __uint_as_float(v1 & 0xFFFF0000u);
-    lo = __byte_perm(__float_as_uint(t0), __float_as_uint(t1), 0x7632);
+// (x0, x1) -> packed fp16 pairs hi, lo with x = hi + lo up to 2^-22 |x| (x0 in the low half): hi = RN16(x),
+// lo = RN16(x - hi); x - hi is exact in fp32.  |x| must stay below 65504 (the callers scale: see the header).
+__device__ __forceinline__ void split2_pack(float x0, float x1, uint32_t& hi, uint32_t& lo) {
+    const __half2 h = __floats2half2_rn(x0, x1);
+    const float2 hf = __half22float2(h);
+    const __half2 l = __floats2half2_rn(x0 - hf.x, x1 - hf.y);
+    hi = *reinterpret_cast<const uint32_t*>(&h);
+    lo = *reinterpret_cast<const uint32_t*>(&l);
 }
+constexpr float TCA_QSCALE = 64.f;        // 2^6
+constexpr float TCA_PSCALE_LOG2 = 15.f;   // P is scaled by 2^15
 
 struct TcAttnArgs {
     AttnArgs a;       // same fields as the legacy kernel (pool pointer unused here)
@@ -151,7 +153,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const AttnArgs& a = ta.a;
     extern __shared__ uint8_t tca_smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tca_smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint8_t* q_s = smem;                                  // [3 parts][NH][128 rows][128 B]
+    uint8_t* q_s = smem;                                  // [2 parts][NH][128 rows][128 B]
     uint8_t* kv_s = smem + C::Q_BYTES;                    // K ring [KS][NH x 8 KiB] | V ring [VS][NH x 8 KiB]
     uint64_t* bars = reinterpret_cast<uint64_t*>(kv_s + (TCA_KS + TCA_VS) * C::K_BYTES);
     uint64_t* k_full = bars;                              // [KS]
@@ -195,7 +197,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const bool active = nn != 0 && k_begin < n_keys;   // uniform over the CTA
     const int k_end = min(k_begin + a.split_len, n_keys);
     const int n_tiles = active ? (k_end - k_begin + TCA_BN - 1) / TCA_BN : 0;
-    // ---- Q tile (fp32 -> hi | mid | lo bf16, 128-byte swizzled K-major) ----
+    // ---- Q tile (fp32 x 2^6 -> hi | lo fp16, 128-byte swizzled K-major) ----
     if (active)
     {
         constexpr int CPR = D / 8;  // 16-byte chunks (8 elements) per row
@@ -212,14 +214,13 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
 #pragma unroll
                 for (int i = 0; i < 8; ++i) x[i] = 0.f;
             }
-            uint32_t h[4], m[4], l[4];
+            uint32_t h[4], l[4];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) split3_pack(x[2 * i], x[2 * i + 1], h[i], m[i], l[i]);
+            for (int i = 0; i < 4; ++i) split2_pack(x[2 * i] * TCA_QSCALE, x[2 * i + 1] * TCA_QSCALE, h[i], l[i]);
             const int half = c >> 3, cc = c & 7;
             const int off = half * (128 * 128) + r * 128 + ((cc ^ (r & 7)) << 4);
             *reinterpret_cast<uint4*>(q_s + off) = make_uint4(h[0], h[1], h[2], h[3]);
-            *reinterpret_cast<uint4*>(q_s + C::Q_PART + off) = make_uint4(m[0], m[1], m[2], m[3]);
-            *reinterpret_cast<uint4*>(q_s + 2 * C::Q_PART + off) = make_uint4(l[0], l[1], l[2], l[3]);
+            *reinterpret_cast<uint4*>(q_s + C::Q_PART + off) = make_uint4(l[0], l[1], l[2], l[3]);
         }
     }
     fence_proxy_async();   // generic-proxy smem writes (Q) -> visible to the tensor core's async proxy
@@ -227,26 +228,27 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
+    trace_phase(ta.pf, 0);   // Q tile staged
 
     if (!active) {
         // nothing to do for this (sequence, split): fall through to the TMEM release
     } else if (warp == 0) {
         // ===== TMA producer: lane i issues box i of the tile (K|V, page, half) =====
-        constexpr int OPS = 2 * 4 * C::NH;
+        constexpr int OPS = 2 * 4;
         const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;
-        const int kv = lane / (4 * C::NH), pg = (lane / C::NH) & 3, half = lane % C::NH;
+        const int kv = lane >> 2, pg = lane & 3;
         // K and V tiles travel in separate rings: a K tile is released as soon as Q.K^T of its tile has run, a V
         // tile only after P.V, one tile later; the K stream runs one tile ahead of the V stream.  Page ids are
         // looked up one iteration ahead (off the critical path).  An L2 look-ahead (cp.async.bulk.prefetch.tensor
-        // of tile j + 8) was tried and removed: the 16 extra 2-KiB boxes per tile go through the same TMA unit as
-        // the loads and made IT the bottleneck (period 3,080 -> 2,380 cycles per tile without; profiles/r1_attention_v2.md).
+        // of tile j + 8) was tried and removed: the extra boxes go through the same TMA unit as the loads and made
+        // IT the bottleneck (profiles/r1_attention_v2.md); for the same reason a block is ONE box, not one per half.
         auto box_row = [&](int j) {
             const int pid = pt[min((k_begin + j * TCA_BN) / TCA_PAGE + pg, a.max_pages - 1)];
-            return ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE;
+            return (ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE) >> 3;   // 8-row group index
         };
         const bool ld_on = !(ta.dbg & 1);
         // lanes [0, OPS/2) carry K boxes of tile jk, lanes [OPS/2, OPS) V boxes of tile jv = jk - 1
-        const int dst_off = half * C::KV_HALF + pg * (TCA_PAGE * 128);
+        const int dst_off = pg * C::PAGE_BYTES;
         int row_next = (lane < OPS) ? box_row(0) : 0;    // K lanes: tile 0; V lanes: tile 0 (used one iteration later)
         int row_cur = row_next;
         for (int it = 0; it <= n_tiles; ++it) {
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 mbar_wait(&k_empty[sk], ((jk / TCA_KS) & 1) ^ 1);
                 if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&k_full[sk], C::K_BYTES); else mbar_arrive(&k_full[sk]); }
                 __syncwarp();
-                if (lane < OPS / 2 && ld_on) tma_load_2d(kv_s + sk * C::K_BYTES + dst_off, &tmKV, &k_full[sk], half * 64, row_cur);
+                if (lane < OPS / 2 && ld_on) tma_load_4d(kv_s + sk * C::K_BYTES + dst_off, &tmKV, &k_full[sk], 0, 0, 0, row_cur);
             }
             if (jv >= 0) {
                 const int sv = jv % TCA_VS;
@@ -269,7 +271,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&v_full[sv], C::K_BYTES); else mbar_arrive(&v_full[sv]); }
                 __syncwarp();
                 if (lane >= OPS / 2 && lane < OPS && ld_on)
-                    tma_load_2d(kv_s + (TCA_KS + sv) * C::K_BYTES + dst_off, &tmKV, &v_full[sv], half * 64, row_cur);
+                    tma_load_4d(kv_s + (TCA_KS + sv) * C::K_BYTES + dst_off, &tmKV, &v_full[sv], 0, 0, 0, row_cur);
             }
         }
     } else if (warp == 1) {
@@ -277,8 +279,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         // live in uniform registers); one elected lane issues.  Under `if (lane == 0)` the compiler wrapped every
         // tcgen05.mma in an ELECT / R2UR / BRA.U.ANY loop: ~100 cycles per instruction, 36 instructions per tile,
         // which made this thread - not the tensor pipe, not the softmax - the bottleneck (profiles/r1_attention_v2.md).
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(128, TCA_BN, 0);
-        constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 1);
+        constexpr uint32_t idesc_qk = umma_idesc_f16(128, TCA_BN, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_f16(128, D, 1);
         const bool leader = elect_one();
         const bool do_mma = !(ta.dbg & 2);
         const uint32_t q_addr = smem_u32(q_s);
@@ -294,16 +296,16 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             mbar_wait(&o_empty[i & 1], ((i >> 1) & 1) ^ 1);   // the correction warps have read chunk i - 2
             if (mts) { const long long t2_ = clock64(); mt_p += t1_ - t0_; mt_o += t2_ - t1_; }
             tc_fence_after();
-            const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, C::KV_HALF, 1024);
+            const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
             const uint32_t d_addr = tmem_base + C::TO + (i & 1) * D;
             const uint32_t p_addr = tmem_base + C::TP + (i & 1) * C::SP;
             if (leader && do_mma) {
 #pragma unroll
-                for (int part = 2; part >= 0; --part) {
+                for (int part = 1; part >= 0; --part) {
 #pragma unroll
                     for (int t = 0; t < TCA_BN / 16; ++t)
-                        umma_bf16_ts(d_addr, p_addr + part * 32 + t * 8, vdesc + (uint64_t)(t * (16 * 128 >> 4)), idesc_pv,
-                                     (part == 2 && t == 0) ? 0u : 1u);
+                        umma_bf16_ts(d_addr, p_addr + part * 32 + t * 8, vdesc + (uint64_t)(t * (C::PAGE_BYTES >> 4)), idesc_pv,
+                                     (part == 1 && t == 0) ? 0u : 1u);
                 }
             }
             if (leader) {
@@ -322,14 +324,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const uint32_t s_addr = tmem_base + C::TS + (j & 1) * C::SP;
             if (leader && do_mma) {
 #pragma unroll
-                for (int part = 2; part >= 0; --part) {
+                for (int part = 1; part >= 0; --part) {
 #pragma unroll
                     for (int h = 0; h < C::NH; ++h) {
                         const uint64_t adesc = umma_desc_k128(q_addr + part * C::Q_PART + h * (128 * 128));
-                        const uint64_t bdesc = umma_desc_k128(k_addr + h * C::KV_HALF);
+                        const uint64_t bdesc = umma_desc_k128(k_addr + h * 1024, C::SBO);
 #pragma unroll
                         for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 bf16 = 32 B
-                            umma_bf16_ss(s_addr, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, (part == 2 && h == 0 && ks == 0) ? 0u : 1u);
+                            umma_bf16_ss(s_addr, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, (part == 1 && h == 0 && ks == 0) ? 0u : 1u);
                     }
                 }
             }
@@ -353,7 +355,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const unsigned long long anc = valid ? a.anc[b * a.T + node] : 1ull;
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
-        float m_run = -INFINITY, l_run = 0.f;
+        float m_run = -INFINITY, l_run = 0.f;   // l_run carries P's factor 2^15
+        const float qk_scale = a.scale * (1.f / TCA_QSCALE);
 
         const bool tsw = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;  // bring-up: phase cycles of one warp
         long long tph[5] = {0, 0, 0, 0, 0}, tq = tsw ? clock64() : 0;
@@ -361,6 +364,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         for (int j = 0; j < n_tiles; ++j) {
             mbar_wait(&s_full[j & 1], (j >> 1) & 1);
             tc_fence_after();
+            if (j == 0 && threadIdx.x == 64) trace_phase_any(ta.pf, 1);   // first S tile ready
             TPH(0);
             uint32_t sv[32];
             tmem_ld32(lane_addr + C::TS + (j & 1) * C::SP + wg * 32, sv);
@@ -368,7 +372,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             TPH(1);
             const int kb = k_begin + j * TCA_BN + wg * 32;
 #pragma unroll
-            for (int e = 0; e < 32; ++e) sv[e] = __float_as_uint(mul_rn(__uint_as_float(sv[e]), a.scale));  // s = (q.k) / sqrt(d), rounded as the method states
+            for (int e = 0; e < 32; ++e) sv[e] = __float_as_uint(mul_rn(__uint_as_float(sv[e]), qk_scale));  // s = (q.k) / sqrt(d), rounded as the method states (2^6 of Q taken out exactly)
             if (kb + 32 > L) {   // tile half touches tree keys or the end of the key range (warp-uniform)
 #pragma unroll
                 for (int e = 0; e < 32; ++e) {
@@ -393,23 +397,22 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const float c = ex2_approx((m_run - mu) * LOG2E);  // 2^-inf = 0 on the first tile
             m_run = mn;
             if (wg == 0) xc[(j & 7) * 128 + r] = c;
-            const float nmk = -mu * LOG2E;
+            const float nmk = fmaf(-mu, LOG2E, TCA_PSCALE_LOG2);   // p' = 2^15 p
             float ls0 = 0.f, ls1 = 0.f;
             const uint32_t p_addr = lane_addr + C::TP + (j & 1) * C::SP + wg * 16;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                uint32_t ph[8], pm[8], pl[8];
+                uint32_t ph[8], pl[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
                     const float p0 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e]), LOG2E, nmk));
                     const float p1 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e + 1]), LOG2E, nmk));
                     ls0 += p0;
                     ls1 += p1;
-                    split3_pack(p0, p1, ph[e], pm[e], pl[e]);
+                    split2_pack(p0, p1, ph[e], pl[e]);
                 }
                 tmem_st8(p_addr + h * 8, ph);
-                tmem_st8(p_addr + 32 + h * 8, pm);
-                tmem_st8(p_addr + 64 + h * 8, pl);
+                tmem_st8(p_addr + 32 + h * 8, pl);
             }
             l_run = fmaf(l_run, c, ls0 + ls1);
             TPH(3);
@@ -427,7 +430,9 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             a.ts[6 + warp - 2] = (unsigned long long)(tph[1] + tph[2] + tph[3] + tph[4]);
         }
 #undef TPH
+        if (threadIdx.x == 64) trace_phase_any(ta.pf, 2);   // softmax of the last tile done
         // ---- running max and sum of this split ----
+        l_run *= exp2f(-TCA_PSCALE_LOG2);   // exact
         xsum[wg * 128 + r] = l_run;
         pair_bar_sync(1 + (warp & 3));
         if (valid && wg == 0) {
@@ -473,8 +478,11 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
             float* op = a.o_part + pi * D + hh * C::DH;
 #pragma unroll
+            for (int i = 0; i < C::DH; ++i) o[i] *= exp2f(-TCA_PSCALE_LOG2);   // P's factor 2^15, exact
+#pragma unroll
             for (int i = 0; i < C::DH; i += 4) *reinterpret_cast<float4*>(op + i) = make_float4(o[i], o[i + 1], o[i + 2], o[i + 3]);
         }
+        if (threadIdx.x == 320) trace_phase_any(ta.pf, 3);   // partial output written
     }
     tc_fence_before();
     __syncthreads();

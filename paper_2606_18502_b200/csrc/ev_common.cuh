@@ -76,6 +76,13 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* m
         "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
         : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(
+            smem_u32(smem_dst)),
+        "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        : "memory");
+}
 __device__ __forceinline__ void tma_load_2d_hint(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1,
                                                  uint64_t policy) {
     asm volatile(
@@ -119,6 +126,27 @@ __device__ __forceinline__ void umma_f8(uint32_t d_tmem, uint64_t a_desc, uint64
         : "memory");
 }
 // all previously issued tcgen05.mma of this thread arrive on the mbarrier when complete
+// KV pool containers.  K and V are ROUNDED to bf16 (the method's rounding point, DESIGN.md R-round).  A cache read by
+// the tcgen05 attention kernel keeps those bf16 values in binary16 containers (same 2 bytes per element): kind::f16
+// wants both MMA operands in one format and Q / P are split into fp16 parts.  bf16 -> fp16 is exact for
+// 2^-17 <= |x| <= 65504, keeps 2^-25 absolute below, and saturates above (no inf can enter the pool).
+__device__ __forceinline__ uint32_t bf16x2_to_f16x2(uint32_t w) {
+    uint32_t r;
+    asm("cvt.rn.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(__uint_as_float(w & 0xFFFF0000u)), "f"(__uint_as_float(w << 16)));
+    return r;
+}
+__device__ __forceinline__ uint32_t f16x2_to_bf16x2(uint32_t w) {   // exact for values that came from bf16
+    float lo, hi;
+    asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.f32.f16 %0, l;\n\tcvt.f32.f16 %1, h;\n\t}" : "=f"(lo), "=f"(hi) : "r"(w));
+    uint32_t r;
+    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+__device__ __forceinline__ bool elect_one() {  // one lane of a converged warp
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void umma_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
@@ -135,11 +163,11 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 
 // K-major operand tile in shared memory, 128-byte rows, SWIZZLE_128B (the layout TMA writes with
 // CU_TENSOR_MAP_SWIZZLE_128B): 8-row groups are 1024 B apart (SBO), version 1, layout type 2.
-__device__ __forceinline__ uint64_t umma_desc_k128(uint32_t smem_addr) {
+__device__ __forceinline__ uint64_t umma_desc_k128(uint32_t smem_addr, uint32_t sbo = 1024) {
     uint64_t d = 0;
     d |= (uint64_t)((smem_addr & 0x3FFFFu) >> 4);  // start address, 16-B units
     d |= (uint64_t)1 << 16;                        // leading byte offset (unused for swizzled K-major)
-    d |= (uint64_t)(1024 >> 4) << 32;              // stride byte offset
+    d |= (uint64_t)(sbo >> 4) << 32;               // stride byte offset
     d |= (uint64_t)1 << 46;                        // descriptor version (Blackwell)
     d |= (uint64_t)2 << 61;                        // SWIZZLE_128B
     return d;
@@ -234,6 +262,14 @@ __device__ __forceinline__ void trace_exit(const L2Prefetch& pf) { trace_mark(pf
 // bring-up: phase k (0..3) reached by the LAST CTA (slots 4..7 hold ~t)
 __device__ __forceinline__ void trace_phase(const L2Prefetch& pf, int k) { trace_mark(pf, 4 + k, true); }
 constexpr int TRACE_SLOTS = 8;
+// same, from whichever thread calls (the caller selects one thread)
+__device__ __forceinline__ void trace_phase_any(const L2Prefetch& pf, int k) {
+    if (pf.trace) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        atomicMin(pf.trace + 4 + k, ~t);
+    }
+}
 // same, but ordered after the instruction that produced `dep` (e.g. a load)
 __device__ __forceinline__ void trace_phase_dep(const L2Prefetch& pf, int k, float dep) {
     if (pf.trace && threadIdx.x == 0) {

@@ -401,6 +401,7 @@ struct RopeArgs {
     const int32_t* page_table; // [max_seqs][max_pages]
     int max_pages, page_size;
     __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D]
+    int kv_f16;                // pool keeps the bf16-rounded values in binary16 containers (ev_common.cuh)
     L2Prefetch pf;
 };
 constexpr int ROPE_THREADS = 256;
@@ -443,8 +444,11 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
             __nv_bfloat16* kd = kdst + (size_t)(head - a.Hq) * a.page_size * D;
             __nv_bfloat162 p0 = __floats2bfloat162_rn(rlo.x, rlo.y), p1 = __floats2bfloat162_rn(rlo.z, rlo.w);
             __nv_bfloat162 p2 = __floats2bfloat162_rn(rhi.x, rhi.y), p3 = __floats2bfloat162_rn(rhi.z, rhi.w);
-            *reinterpret_cast<uint2*>(kd + j) = make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
-            *reinterpret_cast<uint2*>(kd + j + D2) = make_uint2(*reinterpret_cast<uint32_t*>(&p2), *reinterpret_cast<uint32_t*>(&p3));
+            uint32_t w0 = *reinterpret_cast<uint32_t*>(&p0), w1 = *reinterpret_cast<uint32_t*>(&p1);
+            uint32_t w2 = *reinterpret_cast<uint32_t*>(&p2), w3 = *reinterpret_cast<uint32_t*>(&p3);
+            if (a.kv_f16) { w0 = bf16x2_to_f16x2(w0); w1 = bf16x2_to_f16x2(w1); w2 = bf16x2_to_f16x2(w2); w3 = bf16x2_to_f16x2(w3); }
+            *reinterpret_cast<uint2*>(kd + j) = make_uint2(w0, w1);
+            *reinterpret_cast<uint2*>(kd + j + D2) = make_uint2(w2, w3);
         }
     }
     const int voff = (a.Hq + a.Hkv) * D;
@@ -454,8 +458,9 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
         *reinterpret_cast<float4*>(row + voff + i * 4) = v;
         if (write) {
             __nv_bfloat162 p0 = __floats2bfloat162_rn(v.x, v.y), p1 = __floats2bfloat162_rn(v.z, v.w);
-            *reinterpret_cast<uint2*>(vdst + (size_t)head * a.page_size * D + j) =
-                make_uint2(*reinterpret_cast<uint32_t*>(&p0), *reinterpret_cast<uint32_t*>(&p1));
+            uint32_t w0 = *reinterpret_cast<uint32_t*>(&p0), w1 = *reinterpret_cast<uint32_t*>(&p1);
+            if (a.kv_f16) { w0 = bf16x2_to_f16x2(w0); w1 = bf16x2_to_f16x2(w1); }
+            *reinterpret_cast<uint2*>(vdst + (size_t)head * a.page_size * D + j) = make_uint2(w0, w1);
         }
     }
     trace_exit(a.pf);
@@ -565,8 +570,9 @@ struct DenseCopyArgs {
     long layer_stride;
     __nv_bfloat16* pool;
     const int32_t* page_row;   // this sequence's page-table row
-    __nv_bfloat16* dense;      // [layer][2][Hkv][n_tokens][D]
+    __nv_bfloat16* dense;      // [layer][2][Hkv][n_tokens][D], always bf16
     int to_dense;
+    int kv_f16;                // pool container (ev_common.cuh)
 };
 __global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
     const int t = blockIdx.x, li = blockIdx.y;
@@ -577,7 +583,15 @@ __global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
         const int kvh = i / vec_per_head, c = i % vec_per_head;
         uint4* p = reinterpret_cast<uint4*>(pool + pbase + (size_t)kvh * a.page_size * a.D + (size_t)c * 8);
         uint4* d = reinterpret_cast<uint4*>(a.dense + (((size_t)li * 2 * a.Hkv + kvh) * a.n_tokens + t) * a.D + (size_t)c * 8);
-        if (a.to_dense) *d = *p; else *p = *d;
+        if (a.to_dense) {
+            uint4 v = *p;
+            if (a.kv_f16) { v.x = f16x2_to_bf16x2(v.x); v.y = f16x2_to_bf16x2(v.y); v.z = f16x2_to_bf16x2(v.z); v.w = f16x2_to_bf16x2(v.w); }
+            *d = v;
+        } else {
+            uint4 v = *d;
+            if (a.kv_f16) { v.x = bf16x2_to_f16x2(v.x); v.y = bf16x2_to_f16x2(v.y); v.z = bf16x2_to_f16x2(v.z); v.w = bf16x2_to_f16x2(v.w); }
+            *p = v;
+        }
     }
 }
 

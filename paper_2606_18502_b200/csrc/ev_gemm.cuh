@@ -46,8 +46,8 @@ struct GemmArgs {
     int M, N;
     int total_kb;       // ceil(K / 128) = K tiles of W
     int n_tiles, m_tiles, k_splits, kb_per_split;
-    int sk_units;       // stream-K (m_tiles == 1): n_tiles * total_kb K-blocks dealt out evenly, CTA c gets
-                        // [c U / G, (c+1) U / G); 0 = classic items (n_tile, m_tile, k_split)
+    int sk_units;       // stream-K: U = tiles * total_kb K-blocks dealt out evenly (tile = n_tile * m_tiles + m_tile, or the
+                        // same over PAIRS of n tiles with mc), CTA (pair) c gets [c U / G, (c+1) U / G); 0 = classic items
     int tok;            // tokens per tile (UMMA N), multiple of 16, <= 256
     int stages;
     const uint8_t* W;   // tiled + swizzled codes: [n_tiles][total_kb][16 KiB]
@@ -61,6 +61,8 @@ struct GemmArgs {
     const void* warm[2];   // per-layer constants the CONSUMER kernel will read first thing after its wait (this
     int warm_bytes[2];     // matrix's s_w, the next RMSNorm's gain): touched here so they are L2 hits there
     int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads
+    int mc;             // 1 = CTA pairs (cluster of 2) share the token tile: see "multicast pairs" below
+    int tok_h0;         // mc: token rows loaded (and multicast) by cluster rank 0; rank 1 loads the other tok - tok_h0
 };
 
 // byte offset of element (row r, byte c) inside a 16 KiB weight tile (128-byte swizzle)
@@ -91,6 +93,22 @@ __device__ __forceinline__ void epi_bar_sync() { asm volatile("bar.sync 1, 128;"
 __device__ __forceinline__ void bulk_load_plain(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
                  "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// 2-D tile load delivered to the same shared-memory offset of every CTA in cta_mask; each destination CTA's
+// mbarrier (same offset) receives the complete_tx of the bytes written into it
+__device__ __forceinline__ void tma_load_2d_mc(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1, uint16_t cta_mask,
+                                               uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint "
+        "[%0], [%1, {%3, %4}], [%2], %5, %6;" ::"r"(smem_u32(smem_dst)),
+        "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "h"(cta_mask), "l"(policy)
+        : "memory");
+}
+// all previously issued tcgen05.mma of this thread arrive on the mbarrier at this offset in every CTA of cta_mask
+__device__ __forceinline__ void umma_commit_mc(uint64_t* bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+                 "h"(cta_mask)
                  : "memory");
 }
 __device__ __forceinline__ void load_w(int dbg, uint8_t* dst, const uint8_t* src, uint64_t* bar, uint64_t pol) {
@@ -129,31 +147,54 @@ __host__ __device__ __forceinline__ int sk_first_cta(int unit, int G, int U) {  
 }
 struct GemmWork {
     int w, u, u_end;
+    // c / G: this CTA's index and the CTA count, or - multicast pairs - the pair's index and the pair count
     __device__ __forceinline__ void init(const GemmArgs& a) {
-        w = blockIdx.x;
-        u = (int)((long long)blockIdx.x * a.sk_units / gridDim.x);
-        u_end = (int)((long long)(blockIdx.x + 1) * a.sk_units / gridDim.x);
+        const int c = a.mc ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, G = a.mc ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+        w = c;
+        u = (int)((long long)c * a.sk_units / G);
+        u_end = (int)((long long)(c + 1) * a.sk_units / G);
     }
     __device__ __forceinline__ bool next(const GemmArgs& a, GemmItem& it) {
+        const int c = a.mc ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, G = a.mc ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+        const int rank = a.mc ? (int)(blockIdx.x & 1) : 0, nmul = a.mc ? 2 : 1;   // pairs: tile = (pair of n tiles, m tile)
         if (a.sk_units) {
             if (u >= u_end) return false;
-            it.tile = it.n_tile = u / a.total_kb;
-            it.m_tile = 0;
+            it.tile = u / a.total_kb;
+            it.m_tile = it.tile % a.m_tiles;
+            it.n_tile = nmul * (it.tile / a.m_tiles) + rank;
             it.kb0 = u - it.tile * a.total_kb;
             it.nkb = min(a.total_kb - it.kb0, u_end - u);
-            it.split = (int)blockIdx.x - sk_first_cta(it.tile * a.total_kb, gridDim.x, a.sk_units);
+            it.split = c - sk_first_cta(it.tile * a.total_kb, G, a.sk_units);
             u += it.nkb;
+            return true;
+        }
+        if (a.mc) {  // pair item = (pair of adjacent n tiles, m tile), m fastest; this CTA takes n tile 2 * pair + rank
+            if (w >= (a.n_tiles >> 1) * a.m_tiles) return false;
+            it.split = 0;
+            it.tile = w;
+            it.m_tile = w % a.m_tiles;
+            it.n_tile = 2 * (w / a.m_tiles) + rank;
+            it.kb0 = 0;
+            it.nkb = a.total_kb;
+            w += G;
             return true;
         }
         if (w >= a.n_tiles * a.m_tiles * a.k_splits) return false;
         it = gemm_item(a, w);
-        w += gridDim.x;
+        w += G;
         return true;
+    }
+    // K-blocks this CTA (pair) processes in total
+    __device__ __forceinline__ long total_kb_iters(const GemmArgs& a) const {
+        const int c = a.mc ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, G = a.mc ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+        if (a.sk_units) return (long)((long long)(c + 1) * a.sk_units / G - (long long)c * a.sk_units / G);
+        const int items = (a.mc ? (a.n_tiles >> 1) : a.n_tiles) * a.m_tiles * a.k_splits;
+        return c < items ? (long)((items - c + G - 1) / G) * a.kb_per_split : 0;
     }
 };
 
 template <int EPI>
-__global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, GemmArgs a) {
+__global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmXh, GemmArgs a) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
     const int x_bytes = a.tok * GEMM_BK;
@@ -192,7 +233,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
         if (!w0.next(a, it0)) { it0.n_tile = it0.m_tile = it0.kb0 = it0.nkb = 0; }
     }
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); }
+        for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], a.mc ? 2 : 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], 4); }
         fence_barrier_init();
         pre = min(a.stages, it0.nkb);
@@ -207,6 +248,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     if (warp == 1) tmem_alloc_rt(tmem_base_smem, tmem_cols);
     tc_fence_before();
     __syncthreads();
+    if (a.mc) cluster_barrier();   // the peer's barriers exist before any multicast load or commit targets them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
     if (threadIdx.x == 0) TS(1);
@@ -218,8 +260,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             pdl_wait();  // activations come from the previous kernel
             trace_past_wait(a.pf);
             TS(3);
-            for (int i = 0; i < pre; ++i)
-                load_x(a.dbg, smem + i * stage_bytes + GEMM_WTILE, &tmX, &full_bar[i], (it0.kb0 + i) * GEMM_BK, it0.m_tile * a.tok, pol_x);
+            // multicast pairs: this CTA fetches only its half of the token tile and the TMA unit delivers it to the
+            // same stage of BOTH CTAs of the cluster (each CTA's full barrier counts the bytes that land in it)
+            const int rank = (int)(blockIdx.x & 1);
+            const int mc_r0 = rank ? a.tok_h0 : 0;
+            auto ld_x = [&](uint8_t* st, uint64_t* bar, int kb_abs, int m_tile) {
+                if (a.mc) tma_load_2d_mc(st + GEMM_WTILE + mc_r0 * GEMM_BK, rank ? &tmXh : &tmX, bar, kb_abs * GEMM_BK, m_tile * a.tok + mc_r0, (uint16_t)3, pol_x);
+                else load_x(a.dbg, st + GEMM_WTILE, &tmX, bar, kb_abs * GEMM_BK, m_tile * a.tok, pol_x);
+            };
+            for (int i = 0; i < pre; ++i) ld_x(smem + i * stage_bytes, &full_bar[i], it0.kb0 + i, it0.m_tile);
             int s = pre;
             uint32_t ph = 0;
             if (s == a.stages) { s = 0; ph ^= 1; }
@@ -232,20 +281,29 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], stage_bytes);
                     uint8_t* st = smem + s * stage_bytes;
                     load_w(a.dbg, st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, &full_bar[s], pol_w);
-                    load_x(a.dbg, st + GEMM_WTILE, &tmX, &full_bar[s], (it.kb0 + kb) * GEMM_BK, it.m_tile * a.tok, pol_x);
+                    ld_x(st, &full_bar[s], it.kb0 + kb, it.m_tile);
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
-        if (lane == 0) {  // ===== MMA issuer =====
+        {   // ===== MMA issuer.  The WHOLE warp runs the loop and one elected lane issues: addresses and descriptors are
+            // then provably warp-uniform and stay in uniform registers.  Under `if (lane == 0)` the compiler wrapped
+            // every tcgen05.mma and commit in an ELECT / R2UR.BROADCAST / BRA.U.ANY loop (~100 cycles each, five per
+            // K-block: more than the 416 cycles of tensor work of a 208-token K-block). =====
+            const bool leader = elect_one();
             const uint32_t idesc = umma_idesc_e4m3(GEMM_WROWS, a.tok);
+            const uint32_t smem_base = smem_u32(smem);
             int s = 0;
             uint32_t ph = 0;
             int n_it = 0;
             GemmWork wk;
             wk.init(a);
             GemmItem it;
+            // multicast pairs: a stage may be refilled (by either CTA's half load) only when BOTH CTAs have consumed it,
+            // so the release goes to both CTAs' empty barriers (count 2).  The releases of the last `stages` K-blocks
+            // are never waited for; they stay local so that nothing is in flight towards a peer that may have exited.
+            long mc_left = a.mc ? wk.total_kb_iters(a) : 0;
             for (; wk.next(a, it); ++n_it) {
                 const int buf = n_it & 1;
                 mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);  // epilogue has drained this accumulator
@@ -254,19 +312,27 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                 for (int kb = 0; kb < it.nkb; ++kb) {
                     mbar_wait(&full_bar[s], ph);
                     tc_fence_after();
-                    const uint32_t wa = smem_u32(smem + s * stage_bytes);
+                    const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
                     const uint64_t adesc = umma_desc_k128(wa);
                     const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
-                    if (!(a.dbg & 4)) {
+                    if (leader) {
+                        if (!(a.dbg & 4)) {
 #pragma unroll
-                        for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
-                            umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                            for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
+                                umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                        }
+                        if (a.mc && mc_left > a.stages) umma_commit_mc(&empty_bar[s], (uint16_t)3);
+                        else umma_commit(&empty_bar[s]);
                     }
-                    umma_commit(&empty_bar[s]);
+                    __syncwarp();
+                    --mc_left;
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
-                umma_commit(&tmem_full_bar[buf]);
-                if (n_it == 0) TS(4);
+                if (leader) {
+                    umma_commit(&tmem_full_bar[buf]);
+                    if (n_it == 0) TS(4);
+                }
+                __syncwarp();
             }
         }
     } else {  // ===== epilogue: warps 2..5; warp w may touch TMEM lanes 32*(w%4) .. +31 =====
@@ -355,6 +421,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     }
     tc_fence_before();
     __syncthreads();
+    if (a.mc) cluster_barrier();   // no CTA of the pair exits while the other may still multicast into it
     if (warp == 1) tmem_dealloc_rt(tmem_base, tmem_cols);
     if (threadIdx.x == 32) TS(7);
     trace_exit(a.pf);

@@ -93,6 +93,34 @@ def test_fp8_gemm_tiny_shapes(tiny_gpu, kind, M):
     assert np.max(np.abs(got - ref)) <= 1e-5 * np.max(np.abs(ref)) + 1e-7
 
 
+@pytest.fixture(scope="module")
+def tiny_gpu_many_rows():
+    from gpu_helpers import gpu_model
+    return gpu_model(wl.TINY, 0, max_batch=13, max_tree_nodes=64, max_ctx=512, random_gains=True)
+
+
+@pytest.mark.parametrize("kind,M", [("wq", 257), ("wq", 300), ("wq", 832), ("wo", 512), ("wo", 831), ("wgate", 300),
+                                    ("wdown", 640), ("lm_head", 300), ("lm_head", 832)])
+def test_fp8_gemm_many_rows(tiny_gpu_many_rows, kind, M):
+    """M > 256: several token tiles, no split-K.  Even numbers of 128-channel tiles (QKV 4, O 2, down 2, LM head 8)
+    run as multicast CTA pairs (each CTA fetches half of the token tile for both; odd halves at M = 300 / 831);
+    gate|up (11 tiles, ragged) takes the single-CTA path.  LM head: logits and the argmax keys' epilogue."""
+    shape = wl.TINY
+    K = {"wq": 256, "wo": 256, "wgate": 256, "wdown": 688, "lm_head": 256}[kind]
+    rng = np.random.default_rng(M + 17)
+    x = rng.standard_normal((M, K)).astype(np.float32)
+    xq, sx = vo.quantize_rows(x)
+    names = {"wq": ("wq", "wk", "wv"), "wgate": ("wgate", "wup")}.get(kind, (kind,))
+    ws = [vo.quantize_weight(wl.weight_matrix_bf16(shape, 0, k, 0)) for k in names]
+    wq = np.concatenate([w[0] for w in ws])
+    sw = np.concatenate([w[1] for w in ws])
+    ref = vo.linear(xq, sx, wq, sw)
+    got = tiny_gpu_many_rows.ev_op_linear(kind, 0, torch.from_numpy(xq).cuda(), torch.from_numpy(sx).cuda()).cpu().numpy()
+    assert got.shape == ref.shape
+    assert rel_l2(got, ref) < 1e-5, (kind, M, rel_l2(got, ref))
+    assert np.max(np.abs(got - ref)) <= 1e-5 * np.max(np.abs(ref)) + 1e-7
+
+
 def test_fp8_gemm_accumulation_error_at_8b_k():
     """tcgen05 kind::f8f6f4 fp32 accumulation vs exact sums at K = 4096 and 14336 (SURVEY H2):
     reported, and bounded at 2^-18 relative to the mean |y|."""
