@@ -103,6 +103,8 @@ struct ActBuf {  // an E4M3 activation buffer [rows_pad][K] + per-token scales, 
     float* scale = nullptr;
     long K = 0;
     CUtensorMap tm[N_TOK_VARIANTS];
+    CUtensorMap tmh[N_TOK_VARIANTS];   // half tiles (8, 16, ..., 128 rows): one CTA's share of a CTA pair's token tile
+    CUtensorMap* tms_dev = nullptr;    // device copy: box heights 8, 16, ..., 256 rows (the balanced partition picks per item)
 };
 
 struct QMat {  // a quantized weight matrix [N][K], codes in the GEMM's tiled HBM layout (ev_gemm.cuh)
@@ -172,7 +174,8 @@ struct ev_model {
     int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
     int gemm_dbg = 0, gemm_stages = 0;
-    bool gemm_mc = true;   // multicast CTA pairs for the many-row GEMMs (EV_GEMM_MC=0 turns them off)
+    bool gemm_bal = true, gemm_bal_all = false;  // balanced partition of the many-row LM head (EV_GEMM_BAL=0: never, 2: every GEMM)
+    bool gemm_mc = true;   // CTA pairs (tcgen05 cta_group::2) for the many-row GEMMs (EV_GEMM_MC=0 turns them off)
     // L2 weight stream (PfPlanner): on for token counts <= l2pf_max_m; bytes the stream may run ahead / per launch
     int l2pf_max_m = 0;
     long l2pf_cap = 88L << 20, l2pf_maxq = 40L << 20;
@@ -243,6 +246,11 @@ int alloc_actbuf(ev_model* m, ActBuf* b, long K) {
     EV_TRY(dev_alloc(m, &b->scale, (size_t)m->M_pad));
     cudaMemset(b->codes, 0, (size_t)m->M_pad * K);
     for (int i = 0; i < N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&b->tm[i], b->codes, m->M_pad, K, 16 * (i + 1)));
+    for (int i = 0; i < N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&b->tmh[i], b->codes, m->M_pad, K, 8 * (i + 1)));
+    CUtensorMap all[2 * N_TOK_VARIANTS];
+    for (int i = 0; i < 2 * N_TOK_VARIANTS; ++i) EV_TRY(make_tmap(&all[i], b->codes, m->M_pad, K, 8 * (i + 1)));
+    EV_TRY(dev_alloc(m, &b->tms_dev, (size_t)2 * N_TOK_VARIANTS));
+    CUDA_TRY(cudaMemcpy(b->tms_dev, all, sizeof(all), cudaMemcpyHostToDevice));
     return EV_OK;
 }
 
@@ -337,11 +345,11 @@ RowPlan row_plan(const ev_model* m, int M, int row_floats, int cl_par_max = CLUS
         else return fail(EV_EINVAL, "row too long for the row kernels");                                       \
     } while (0)
 
-template <int EPI>
+template <int EPI, bool PAIR>
 int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const CUtensorMap& tmXh, const GemmArgs& a, int grid, int smem) {
     static bool attr_set = false;
     if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<EPI, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_set = true;
     }
     cudaLaunchConfig_t cfg;
@@ -355,12 +363,12 @@ int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const CUtensorMap& tmXh
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    if (a.mc) {  // multicast pairs: clusters of 2 CTAs along x
+    if (PAIR) {  // CTA pairs: clusters of 2 CTAs along x
         at[1].id = cudaLaunchAttributeClusterDimension;
         at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
         cfg.numAttrs = 2;
     }
-    CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_e4m3_kernel<EPI>, tmX, tmXh, a));
+    CUDA_TRY(cudaLaunchKernelEx(&cfg, gemm_e4m3_kernel<EPI, PAIR>, tmX, tmXh, a));
     ++g_launches;
     return EV_OK;
 }
@@ -462,7 +470,17 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     a.M = M; a.N = (int)w.N; a.total_kb = w.total_kb; a.n_tiles = w.n_tiles;
     a.m_tiles = (M + 255) / 256;
     a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
-    const int stage_bytes = GEMM_WTILE + a.tok * GEMM_BK;
+    // balanced partition (ev_gemm.cuh, GemmArgs::bal): several token tiles -> items of up to 256 tokens cut from an even deal.
+    // Used for the LM head (1002 n tiles: 27 items per CTA pair, 588 -> 548 us at M = 832).  The layer GEMMs have 1-6
+    // items per pair; there the extra partial items (a 32-token item costs as much W traffic as a 208-token one)
+    // outweigh the partial last wave: O 26 -> 33 us, down 54 -> 82 us, gate|up 98 -> 104 us (EV_GEMM_BAL=2 forces it).
+    a.bal = (m->gemm_bal && a.m_tiles >= 2 && (epi == EPI_ARGMAX || m->gemm_bal_all)) ? 1 : 0;
+    a.bal_blocks = (M + 15) / 16;
+    a.tms = x.tms_dev;
+    if (a.bal) a.tok = 256;   // the largest item: sizes the stages and the two accumulators
+    // CTA pairs (ev_gemm.cuh): several token tiles and an even number of 128-channel tiles
+    a.mc = (m->gemm_mc && a.m_tiles >= 2 && a.n_tiles % 2 == 0) ? 1 : 0;
+    const int stage_bytes = GEMM_WTILE + (a.mc ? a.tok / 2 : a.tok) * GEMM_BK;
     a.stages = std::min(GEMM_MAX_STAGES, GEMM_SMEM_BUDGET / stage_bytes);
     if (a.stages < 2) return fail(EV_EINVAL, "token tile too large");
     if (m->gemm_stages > 0) a.stages = std::min(a.stages, m->gemm_stages);
@@ -475,23 +493,14 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     if (pfp) a.pf = pfp->take(true);
     a.dbg = m->gemm_dbg;
     a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
-    // Multicast pairs (many token rows: several token tiles): the GEMM is then bound by the L2 -> SM fill of its
-    // operand tiles (16 KiB of W + tok x 128 B of X per K-block and CTA).  Adjacent n tiles of the same token tile
-    // run as a cluster of two CTAs; each fetches half of the token tile and the TMA unit multicasts it to both, so
-    // the pair behaves like one 256 x tok tile: a third less L2 traffic per flop.
     const int G = m->num_sms;
-    a.mc = 0; a.tok_h0 = a.tok;
-    if (m->gemm_mc && a.m_tiles >= 2 && a.n_tiles % 2 == 0 && a.tok >= 32) {
-        a.mc = 1;
-        a.tok_h0 = 16 * ((a.tok / 16 + 1) / 2);
-    }
     const int nmul = a.mc ? 2 : 1;                       // n tiles per scheduling unit
     const int Gc = a.mc ? G / 2 : G;                     // CTAs, or CTA pairs
     const int tiles = (a.n_tiles / nmul) * a.m_tiles;    // (n tile or pair of n tiles, token tile)
     a.k_splits = 1;
     a.kb_per_split = a.total_kb;
     a.sk_units = 0;
-    int grid = nmul * std::min(tiles, Gc);
+    int grid = nmul * std::min(a.bal ? (a.n_tiles / nmul) * a.bal_blocks : tiles, Gc);
     if (lin) { lin->splits = 1; lin->sk_G = 0; lin->sk_U = 0; lin->sk_kb = 0; }
     // Stream-K (one token tile): the n_tiles * total_kb K-blocks are dealt out evenly to the CTAs (ev_gemm.cuh); each
     // tile's pieces land in slabs the consumer adds in K order.  The partition depends only on the matrix shape and
@@ -514,10 +523,10 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
         }
     }
     const int smem = a.stages * stage_bytes + 512 + 2048 + 8192 + 1024;  // stages + barriers + sx staging + argmax keys + alignment slack
-    const CUtensorMap& tmX = x.tm[(a.mc ? a.tok_h0 : a.tok) / 16 - 1];
-    const CUtensorMap& tmXh = x.tm[(a.mc ? a.tok - a.tok_h0 : a.tok) / 16 - 1];
-    if (epi == EPI_RAW) return launch_gemm<EPI_RAW>(st, tmX, tmXh, a, grid, smem);
-    return launch_gemm<EPI_ARGMAX>(st, tmX, tmXh, a, grid, smem);
+    const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
+    const CUtensorMap& tmXh = x.tmh[a.tok / 16 - 1];
+    if (epi == EPI_RAW) return a.mc ? launch_gemm<EPI_RAW, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_RAW, false>(st, tmX, tmXh, a, grid, smem);
+    return a.mc ? launch_gemm<EPI_ARGMAX, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_ARGMAX, false>(st, tmX, tmXh, a, grid, smem);
 }
 
 QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
@@ -809,6 +818,8 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
     m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
     m->gemm_mc = !(getenv("EV_GEMM_MC") && atoi(getenv("EV_GEMM_MC")) == 0);
+    m->gemm_bal = !(getenv("EV_GEMM_BAL") && atoi(getenv("EV_GEMM_BAL")) == 0);
+    m->gemm_bal_all = getenv("EV_GEMM_BAL") && atoi(getenv("EV_GEMM_BAL")) == 2;
     if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
     if (getenv("EV_L2PF_MASK")) m->l2pf_mask = (unsigned)strtoul(getenv("EV_L2PF_MASK"), nullptr, 0);
     if (getenv("EV_L2PF_CAP_MB")) m->l2pf_cap = (long)atoi(getenv("EV_L2PF_CAP_MB")) << 20;

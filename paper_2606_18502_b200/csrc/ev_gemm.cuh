@@ -61,8 +61,14 @@ struct GemmArgs {
     const void* warm[2];   // per-layer constants the CONSUMER kernel will read first thing after its wait (this
     int warm_bytes[2];     // matrix's s_w, the next RMSNorm's gain): touched here so they are L2 hits there
     int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads
-    int mc;             // 1 = CTA pairs (cluster of 2) share the token tile: see "multicast pairs" below
-    int tok_h0;         // mc: token rows loaded (and multicast) by cluster rank 0; rank 1 loads the other tok - tok_h0
+    int bal;            // balanced partition (several token tiles): the (n unit, 16-token block) space, n unit major, is dealt
+                        // out evenly to the CTAs (CTA pairs); a CTA's contiguous range is cut at n-unit boundaries and into
+                        // items of <= 256 tokens, so token tiles differ in size from item to item (GemmItem::tok) and no
+                        // CTA idles in a partial last wave (896 tiles on 148 CTAs = 6.05 waves cost 7).  0 = uniform tiles
+    int bal_blocks;     // 16-token blocks per n unit = ceil(M / 16)
+    const CUtensorMap* tms;   // bal: activation tensor maps in global memory, box heights 8, 16, ..., 256 rows ([h / 8 - 1])
+    int mc;             // 1 = CTA pairs (cluster of 2, tcgen05 cta_group::2): one 256-channel x tok MMA per pair, each CTA
+                        // stages its own 128 channels of W and HALF of the token tile (see "CTA pairs" below)
 };
 
 // byte offset of element (row r, byte c) inside a 16 KiB weight tile (128-byte swizzle)
@@ -95,21 +101,36 @@ __device__ __forceinline__ void bulk_load_plain(void* smem_dst, const void* gsrc
                  "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-// 2-D tile load delivered to the same shared-memory offset of every CTA in cta_mask; each destination CTA's
-// mbarrier (same offset) receives the complete_tx of the bytes written into it
-__device__ __forceinline__ void tma_load_2d_mc(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1, uint16_t cta_mask,
-                                               uint64_t policy) {
+// ---- CTA pairs (cta_group::2) ----
+__device__ __forceinline__ void tmem_alloc_rt2(uint32_t* smem_result, uint32_t ncols) {   // one warp of EACH CTA of the pair
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_result)), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_rt2(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// D[tmem, 256 lanes over the pair] (+)= A[smem of both CTAs, 128 rows each] * B[smem of both CTAs, N/2 rows each]
+__device__ __forceinline__ void umma_f8_2cta(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate) {
     asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster.L2::cache_hint "
-        "[%0], [%1, {%3, %4}], [%2], %5, %6;" ::"r"(smem_u32(smem_dst)),
-        "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "h"(cta_mask), "l"(policy)
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f8f6f4 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
-// all previously issued tcgen05.mma of this thread arrive on the mbarrier at this offset in every CTA of cta_mask
-__device__ __forceinline__ void umma_commit_mc(uint64_t* bar, uint16_t cta_mask) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
-                 "h"(cta_mask)
+// all previously issued tcgen05.mma of this thread arrive on the mbarrier at this offset in BOTH CTAs of the pair
+__device__ __forceinline__ void umma_commit_2cta(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(smem_u32(bar)),
+                 "h"((uint16_t)3)
                  : "memory");
+}
+// arrive on the mbarrier at the same offset in CTA `rank` of the cluster
+__device__ __forceinline__ void mbar_arrive_remote(uint64_t* bar, uint32_t rank) {
+    // default (CTA-scope) semantics on purpose: the cluster-scope release / acquire forms compile to MEMBAR.ALL.GPU and
+    // CCTL.IVALL around every arrive / wait (the pair ran at HALF the single-CTA speed with them).  What travels
+    // through these barriers is ordered by the barriers' own completion: TMA-written shared memory read by the
+    // tensor core, and tcgen05.ld -> tcgen05.fence::before_thread_sync -> arrive on the epilogue side.
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_map(bar, rank)) : "memory");
 }
 __device__ __forceinline__ void load_w(int dbg, uint8_t* dst, const uint8_t* src, uint64_t* bar, uint64_t pol) {
     if (dbg & 8) return;
@@ -127,7 +148,7 @@ __device__ __forceinline__ void load_x(int dbg, uint8_t* dst, const CUtensorMap*
 }
 __device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
 #define TS(i) do { if (a.ts) a.ts[blockIdx.x * 8 + (i)] = gtimer(); } while (0)
-struct GemmItem { int n_tile, m_tile, split, tile, kb0, nkb; };
+struct GemmItem { int n_tile, m_tile, split, tile, kb0, nkb, m0, tok; };   // m0, tok: first token row and token count of the item
 __device__ __forceinline__ GemmItem gemm_item(const GemmArgs& a, int w) {
     GemmItem it;
     it.split = w % a.k_splits;
@@ -136,6 +157,8 @@ __device__ __forceinline__ GemmItem gemm_item(const GemmArgs& a, int w) {
     it.n_tile = it.tile / a.m_tiles;
     it.kb0 = it.split * a.kb_per_split;
     it.nkb = min(a.kb_per_split, a.total_kb - it.kb0);
+    it.m0 = it.m_tile * a.tok;
+    it.tok = a.tok;
     return it;
 }
 // Work of one CTA, in order.  Classic: items blockIdx.x, +gridDim.x, ...  Stream-K: the contiguous range of
@@ -151,12 +174,26 @@ struct GemmWork {
     __device__ __forceinline__ void init(const GemmArgs& a) {
         const int c = a.mc ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, G = a.mc ? (int)(gridDim.x >> 1) : (int)gridDim.x;
         w = c;
-        u = (int)((long long)c * a.sk_units / G);
-        u_end = (int)((long long)(c + 1) * a.sk_units / G);
+        const long long U = a.bal ? (long long)(a.n_tiles / (a.mc ? 2 : 1)) * a.bal_blocks : a.sk_units;
+        u = (int)((long long)c * U / G);
+        u_end = (int)((long long)(c + 1) * U / G);
     }
     __device__ __forceinline__ bool next(const GemmArgs& a, GemmItem& it) {
         const int c = a.mc ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, G = a.mc ? (int)(gridDim.x >> 1) : (int)gridDim.x;
         const int rank = a.mc ? (int)(blockIdx.x & 1) : 0, nmul = a.mc ? 2 : 1;   // pairs: tile = (pair of n tiles, m tile)
+        if (a.bal) {   // u, u_end: 16-token blocks of the flattened (n unit, block) space
+            if (u >= u_end) return false;
+            const int p = u / a.bal_blocks, b0 = u - p * a.bal_blocks;
+            const int len = min(u_end, (p + 1) * a.bal_blocks) - u;    // what is left of this CTA's piece of n unit p
+            const int n_items = (len + 15) >> 4;                        // items of <= 16 blocks, as even as possible
+            const int chunk = (len + n_items - 1) / n_items;
+            it.tile = p; it.m_tile = 0; it.split = 0;
+            it.n_tile = nmul * p + rank;
+            it.kb0 = 0; it.nkb = a.total_kb;
+            it.m0 = b0 * 16; it.tok = chunk * 16;
+            u += chunk;
+            return true;
+        }
         if (a.sk_units) {
             if (u >= u_end) return false;
             it.tile = u / a.total_kb;
@@ -165,6 +202,7 @@ struct GemmWork {
             it.kb0 = u - it.tile * a.total_kb;
             it.nkb = min(a.total_kb - it.kb0, u_end - u);
             it.split = c - sk_first_cta(it.tile * a.total_kb, G, a.sk_units);
+            it.m0 = it.m_tile * a.tok; it.tok = a.tok;
             u += it.nkb;
             return true;
         }
@@ -176,6 +214,7 @@ struct GemmWork {
             it.n_tile = 2 * (w / a.m_tiles) + rank;
             it.kb0 = 0;
             it.nkb = a.total_kb;
+            it.m0 = it.m_tile * a.tok; it.tok = a.tok;
             w += G;
             return true;
         }
@@ -193,15 +232,26 @@ struct GemmWork {
     }
 };
 
-template <int EPI>
+// PAIR: the kernel contains cta_group::2 instructions and must be launched in clusters of 2 (a.mc == PAIR)
+template <int EPI, bool PAIR>
 __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmXh, GemmArgs a) {
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    const int x_bytes = a.tok * GEMM_BK;
+    // CTA pairs (many token rows; PAIR = a.mc): the pair runs ONE tcgen05.mma.cta_group::2 of 256 channels x tok tokens per
+    // K step.  Each CTA stages its own 128 channels of W and HALF of the token tile; the tensor cores read both
+    // halves across the pair.  Per K-block a CTA then receives 16 KiB + tok/2 x 128 B instead of 16 KiB + tok x 128 B:
+    // a third less L2 -> SM traffic per flop and 6 instead of 4 stages in flight at tok = 208, which is what bounded
+    // the single-CTA form (tensor pipe 61 % busy; multicasting the token tile to both CTAs changed nothing, because
+    // every CTA still had to RECEIVE the whole tile).  Rank 0 issues the MMAs and commits to both CTAs' barriers;
+    // rank 1's MMA warp only relays "my stage has landed" to rank 0; each CTA's epilogue drains its own 128 lanes.
+    const int rank = PAIR ? (int)(blockIdx.x & 1) : 0;
+    const int x_rows = PAIR ? a.tok / 2 : a.tok;
+    const int x_bytes = x_rows * GEMM_BK;
     const int stage_bytes = GEMM_WTILE + x_bytes;
     uint64_t* full_bar = reinterpret_cast<uint64_t*>(smem + a.stages * stage_bytes);
     uint64_t* empty_bar = full_bar + GEMM_MAX_STAGES;
-    uint64_t* tmem_full_bar = empty_bar + GEMM_MAX_STAGES;   // [2]
+    uint64_t* peer_full_bar = empty_bar + GEMM_MAX_STAGES;    // rank 0: rank 1's stage has landed
+    uint64_t* tmem_full_bar = peer_full_bar + GEMM_MAX_STAGES;   // [2]
     uint64_t* tmem_empty_bar = tmem_full_bar + 2;            // [2]
     uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(tmem_empty_bar + 2);
     float* sx_smem = reinterpret_cast<float*>(tmem_base_smem + 4);  // [2][256] per-token scales of the current / next item
@@ -230,25 +280,26 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     {
         GemmWork w0;
         w0.init(a);
-        if (!w0.next(a, it0)) { it0.n_tile = it0.m_tile = it0.kb0 = it0.nkb = 0; }
+        if (!w0.next(a, it0)) { it0.n_tile = it0.m_tile = it0.kb0 = it0.nkb = it0.m0 = 0; it0.tok = a.tok; }
     }
     if (warp == 0 && lane == 0) {
-        for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], a.mc ? 2 : 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], 4); }
+        for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); mbar_init(&peer_full_bar[s], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], PAIR ? 8 : 4); }
         fence_barrier_init();
         pre = min(a.stages, it0.nkb);
         const uint8_t* wsrc = a.W + ((size_t)it0.n_tile * a.total_kb + it0.kb0) * GEMM_WTILE;
+        const uint32_t tx0 = GEMM_WTILE + (PAIR ? it0.tok / 2 : it0.tok) * GEMM_BK;   // W tile + this CTA's token rows of the item
         for (int i = 0; i < pre; ++i) {
-            if (a.dbg & 8) mbar_arrive(&full_bar[i]); else mbar_arrive_expect_tx(&full_bar[i], stage_bytes);
+            if (a.dbg & 8) mbar_arrive(&full_bar[i]); else mbar_arrive_expect_tx(&full_bar[i], tx0);
             if (!(a.dbg & 8)) bulk_load_plain(smem + i * stage_bytes, wsrc + (size_t)i * GEMM_WTILE, GEMM_WTILE, &full_bar[i]);
         }
         tma_prefetch_desc(&tmX);
         TS(2);
     }
-    if (warp == 1) tmem_alloc_rt(tmem_base_smem, tmem_cols);
+    if (warp == 1) { if (PAIR) tmem_alloc_rt2(tmem_base_smem, tmem_cols); else tmem_alloc_rt(tmem_base_smem, tmem_cols); }
     tc_fence_before();
     __syncthreads();
-    if (a.mc) cluster_barrier();   // the peer's barriers exist before any multicast load or commit targets them
+    if (PAIR) cluster_barrier();   // the peer's barriers exist before any commit or relayed arrive targets them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
     if (threadIdx.x == 0) TS(1);
@@ -260,15 +311,13 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             pdl_wait();  // activations come from the previous kernel
             trace_past_wait(a.pf);
             TS(3);
-            // multicast pairs: this CTA fetches only its half of the token tile and the TMA unit delivers it to the
-            // same stage of BOTH CTAs of the cluster (each CTA's full barrier counts the bytes that land in it)
-            const int rank = (int)(blockIdx.x & 1);
-            const int mc_r0 = rank ? a.tok_h0 : 0;
-            auto ld_x = [&](uint8_t* st, uint64_t* bar, int kb_abs, int m_tile) {
-                if (a.mc) tma_load_2d_mc(st + GEMM_WTILE + mc_r0 * GEMM_BK, rank ? &tmXh : &tmX, bar, kb_abs * GEMM_BK, m_tile * a.tok + mc_r0, (uint16_t)3, pol_x);
-                else load_x(a.dbg, st + GEMM_WTILE, &tmX, bar, kb_abs * GEMM_BK, m_tile * a.tok, pol_x);
+            // pairs: this CTA fetches only its half of the item's token rows (rows rank * tok / 2 ...), into its own stage
+            auto ld_x = [&](uint8_t* st, uint64_t* bar, int kb_abs, const GemmItem& item) {
+                const int rows = PAIR ? item.tok / 2 : item.tok;
+                const CUtensorMap* tm = a.bal ? a.tms + (rows / 8 - 1) : (PAIR ? &tmXh : &tmX);
+                load_x(a.dbg, st + GEMM_WTILE, tm, bar, kb_abs * GEMM_BK, item.m0 + rank * rows, pol_x);
             };
-            for (int i = 0; i < pre; ++i) ld_x(smem + i * stage_bytes, &full_bar[i], it0.kb0 + i, it0.m_tile);
+            for (int i = 0; i < pre; ++i) ld_x(smem + i * stage_bytes, &full_bar[i], it0.kb0 + i, it0);
             int s = pre;
             uint32_t ph = 0;
             if (s == a.stages) { s = 0; ph ^= 1; }
@@ -276,12 +325,13 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             wk.init(a);
             GemmItem it;
             for (bool first = true; wk.next(a, it); first = false) {
+                const uint32_t tx = GEMM_WTILE + (PAIR ? it.tok / 2 : it.tok) * GEMM_BK;
                 for (int kb = (first ? pre : 0); kb < it.nkb; ++kb) {
                     mbar_wait(&empty_bar[s], ph ^ 1);
-                    if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], stage_bytes);
+                    if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], tx);
                     uint8_t* st = smem + s * stage_bytes;
                     load_w(a.dbg, st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, &full_bar[s], pol_w);
-                    ld_x(st, &full_bar[s], it.kb0 + kb, it.m_tile);
+                    ld_x(st, &full_bar[s], it.kb0 + kb, it);
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
             }
@@ -292,7 +342,6 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             // every tcgen05.mma and commit in an ELECT / R2UR.BROADCAST / BRA.U.ANY loop (~100 cycles each, five per
             // K-block: more than the 416 cycles of tensor work of a 208-token K-block). =====
             const bool leader = elect_one();
-            const uint32_t idesc = umma_idesc_e4m3(GEMM_WROWS, a.tok);
             const uint32_t smem_base = smem_u32(smem);
             int s = 0;
             uint32_t ph = 0;
@@ -300,39 +349,55 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             GemmWork wk;
             wk.init(a);
             GemmItem it;
-            // multicast pairs: a stage may be refilled (by either CTA's half load) only when BOTH CTAs have consumed it,
-            // so the release goes to both CTAs' empty barriers (count 2).  The releases of the last `stages` K-blocks
-            // are never waited for; they stay local so that nothing is in flight towards a peer that may have exited.
-            long mc_left = a.mc ? wk.total_kb_iters(a) : 0;
-            for (; wk.next(a, it); ++n_it) {
-                const int buf = n_it & 1;
-                mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);  // epilogue has drained this accumulator
-                tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(buf * a.tok);
-                for (int kb = 0; kb < it.nkb; ++kb) {
-                    mbar_wait(&full_bar[s], ph);
+            if (rank == 1) {
+                // pair, rank 1: no MMAs here; tell rank 0 when a stage of THIS CTA has landed
+                for (; wk.next(a, it); ++n_it) {
+                    for (int kb = 0; kb < it.nkb; ++kb) {
+                        mbar_wait(&full_bar[s], ph);
+                        if (leader) mbar_arrive_remote(&peer_full_bar[s], 0);
+                        __syncwarp();
+                        if (++s == a.stages) { s = 0; ph ^= 1; }
+                    }
+                }
+            } else {
+                for (; wk.next(a, it); ++n_it) {
+                    const int buf = n_it & 1;
+                    // epilogue (of both CTAs of a pair) has drained this accumulator
+                    if (PAIR) mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);
+                    else mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);
                     tc_fence_after();
-                    const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
-                    const uint64_t adesc = umma_desc_k128(wa);
-                    const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
-                    if (leader) {
-                        if (!(a.dbg & 4)) {
+                    const uint32_t idesc = umma_idesc_e4m3(PAIR ? 2 * GEMM_WROWS : GEMM_WROWS, it.tok);
+                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * a.tok);
+                    for (int kb = 0; kb < it.nkb; ++kb) {
+                        mbar_wait(&full_bar[s], ph);
+                        if (PAIR) mbar_wait(&peer_full_bar[s], ph);
+                        tc_fence_after();
+                        const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
+                        const uint64_t adesc = umma_desc_k128(wa);
+                        const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
+                        if (leader) {
+                            if (!(a.dbg & 4)) {
+                                if (PAIR) {
 #pragma unroll
-                            for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
-                                umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                                    for (int k = 0; k < GEMM_BK / 32; ++k)
+                                        umma_f8_2cta(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                                } else {
+#pragma unroll
+                                    for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
+                                        umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                                }
+                            }
+                            if (PAIR) umma_commit_2cta(&empty_bar[s]); else umma_commit(&empty_bar[s]);
                         }
-                        if (a.mc && mc_left > a.stages) umma_commit_mc(&empty_bar[s], (uint16_t)3);
-                        else umma_commit(&empty_bar[s]);
+                        __syncwarp();
+                        if (++s == a.stages) { s = 0; ph ^= 1; }
+                    }
+                    if (leader) {
+                        if (PAIR) umma_commit_2cta(&tmem_full_bar[buf]); else umma_commit(&tmem_full_bar[buf]);
+                        if (n_it == 0) TS(4);
                     }
                     __syncwarp();
-                    --mc_left;
-                    if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
-                if (leader) {
-                    umma_commit(&tmem_full_bar[buf]);
-                    if (n_it == 0) TS(4);
-                }
-                __syncwarp();
             }
         }
     } else {  // ===== epilogue: warps 2..5; warp w may touch TMEM lanes 32*(w%4) .. +31 =====
@@ -347,15 +412,15 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
         for (; wk.next(a, it); ++n_it) {
             const int buf = n_it & 1;
             const int n = it.n_tile * GEMM_WROWS + n_loc;
-            const int m0 = it.m_tile * a.tok;
+            const int m0 = it.m0, tok = it.tok;
             const bool n_ok = n < a.N;
             constexpr int GC = 32;                    // columns (tokens) handled per register group
-            const int n_groups = (a.tok + GC - 1) / GC;
+            const int n_groups = (tok + GC - 1) / GC;
             float swn = 0.f;
             float* sxs = sx_smem + buf * 256;
             if (EPI == EPI_ARGMAX) {  // scales are fetched BEFORE waiting for the MMAs
                 swn = n_ok ? __ldg(a.sw + n) : 0.f;
-                for (int i = et; i < a.tok; i += 128) sxs[i] = (m0 + i < a.M) ? __ldg(a.sx + m0 + i) : 0.f;
+                for (int i = et; i < tok; i += 128) sxs[i] = (m0 + i < a.M) ? __ldg(a.sx + m0 + i) : 0.f;
                 epi_bar_sync();
             }
             mbar_wait(&tmem_full_bar[buf], (n_it >> 1) & 1);
@@ -366,12 +431,12 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             for (int g = 0; g < n_groups; ++g) {
                 uint32_t v[GC];
                 tmem_ld16(t_addr + (uint32_t)(g * GC), v);
-                if (g * GC + 16 < a.tok) tmem_ld16(t_addr + (uint32_t)(g * GC + 16), v + 16);
+                if (g * GC + 16 < tok) tmem_ld16(t_addr + (uint32_t)(g * GC + 16), v + 16);
                 tmem_ld_wait();
                 if (g == n_groups - 1) {  // accumulator fully read: hand it back to the MMA warp
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&tmem_empty_bar[buf]);
+                    if (lane == 0) { if (rank == 0) mbar_arrive(&tmem_empty_bar[buf]); else mbar_arrive_remote(&tmem_empty_bar[buf], 0); }
                 }
                 if (EPI == EPI_ARGMAX) {
                     // per token: max over the tile's 128 channels of (ordered logit, ~index).  Two warp-wide integer
@@ -385,28 +450,28 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     for (int j = 0; j < GC; ++j) {
                         const int col = g * GC + j;
                         const int m = m0 + col;
-                        const float y = mul_rn(mul_rn(__uint_as_float(v[j]), sxs[col < a.tok ? col : 0]), swn);
-                        const bool ok = n_ok && col < a.tok && m < a.M;
+                        const float y = mul_rn(mul_rn(__uint_as_float(v[j]), sxs[col < tok ? col : 0]), swn);
+                        const bool ok = n_ok && col < tok && m < a.M;
                         const uint32_t ob = ok ? ordered_bits(y) : 0u;      // ordered_bits of a non-NaN value is never 0
                         const uint32_t mx = __reduce_max_sync(0xffffffffu, ob);
                         const uint32_t mn = __reduce_min_sync(0xffffffffu, (ok && ob == mx) ? (uint32_t)n : 0xFFFFFFFFu);
                         if (lane == j) { kmx = mx; kmn = mn; }
                         if (ok && a.out) __stcs(a.out + (size_t)m * a.ldo + n, y);
                     }
-                    if (g * GC + lane < a.tok)   // no valid lane: (0, ~0xFFFFFFFF) = key 0, below every real key
+                    if (g * GC + lane < tok)   // no valid lane: (0, ~0xFFFFFFFF) = key 0, below every real key
                         keys_smem[q * 256 + g * GC + lane] = ((unsigned long long)kmx << 32) | (0xFFFFFFFFu - kmn);
                 } else {
 #pragma unroll
                     for (int j = 0; j < GC; ++j) {
                         const int col = g * GC + j;
                         const int m = m0 + col;
-                        if (n_ok && col < a.tok && m < a.M) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
+                        if (n_ok && col < tok && m < a.M) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
                     }
                 }
             }
             if (EPI == EPI_ARGMAX) {
                 epi_bar_sync();
-                for (int col = et; col < a.tok; col += 128) {
+                for (int col = et; col < tok; col += 128) {
                     const int m = m0 + col;
                     if (m < a.M) {
                         unsigned long long k0 = keys_smem[col], k1 = keys_smem[256 + col], k2 = keys_smem[512 + col], k3 = keys_smem[768 + col];
@@ -421,8 +486,8 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     }
     tc_fence_before();
     __syncthreads();
-    if (a.mc) cluster_barrier();   // no CTA of the pair exits while the other may still multicast into it
-    if (warp == 1) tmem_dealloc_rt(tmem_base, tmem_cols);
+    if (PAIR) cluster_barrier();   // no CTA of the pair exits (or frees its TMEM) while the pair's MMAs or arrives may still target it
+    if (warp == 1) { if (PAIR) tmem_dealloc_rt2(tmem_base, tmem_cols); else tmem_dealloc_rt(tmem_base, tmem_cols); }
     if (threadIdx.x == 32) TS(7);
     trace_exit(a.pf);
 }
