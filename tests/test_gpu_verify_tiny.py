@@ -315,3 +315,37 @@ def test_gpu_speculative_loop_is_lossless_teacher_forced(setup):
             soft2 += 1
         tok = emitted[i]
     assert soft2 <= 2, soft2
+
+
+def test_kv_pool_container_round_trip(setup):
+    """The pool keeps the bf16-rounded K/V VALUES in binary16 containers when the tcgen05 attention kernel reads it
+    (DESIGN.md section 6 "KV pool containers"); the C ABI stays bf16.  import -> export must return every bf16
+    value with 2^-17 <= |x| <= 65504 bit for bit (zeros included), values below within 2^-25, and values above
+    65504 saturated to the largest binary16, 65504, which reads back as bf16 65536 (never inf / NaN: a zero
+    probability times inf would poison an output row)."""
+    spec, gm, om, ev = setup
+    from gpu_helpers import bits_to_bf16_cuda, export_kv_bits
+    shape = spec.model
+    n_tok = 40
+    rng = np.random.default_rng(7)
+    n = shape.n_layers * 2 * shape.n_kv_heads * n_tok * shape.head_dim
+    # bf16 bit patterns: random signs / exponents 2^-17 .. 2^15 / 7-bit mantissas, then planted special values
+    exp = rng.integers(127 - 17, 127 + 15, size=n, dtype=np.uint16)
+    bits = (rng.integers(0, 2, size=n, dtype=np.uint16) << 15) | (exp << 7) | rng.integers(0, 128, size=n, dtype=np.uint16)
+    bits[:8] = [0x0000, 0x8000, 0x477F, 0xC77F, 0x3F80, 0x3380, 0x4780, 0x7F00]   # +-0, +-65280, 1, 2^-24, 65536, 1.7e38
+    tiny = rng.integers(0, 2, size=64, dtype=np.uint16) << 15 | (rng.integers(60, 127 - 17, size=64, dtype=np.uint16) << 7)
+    bits[8:72] = tiny
+    dense = bits.reshape(shape.n_layers, 2, shape.n_kv_heads, n_tok, shape.head_dim)
+    cache = ev.Cache(gm, n_pages=16, max_seqs=2)
+    slot = cache.ev_cache_add_seq(64)
+    cache.ev_cache_import_seq(slot, 0, shape.n_layers, bits_to_bf16_cuda(dense), set_len=True)
+    back = export_kv_bits(cache, slot, 0, shape.n_layers, n_tok).reshape(-1)
+    f_in = (bits.astype(np.uint32) << 16).view(np.float32)
+    f_out = (back.astype(np.uint32) << 16).view(np.float32)
+    assert np.all(np.isfinite(f_out))
+    in_range = (np.abs(f_in) >= 2.0 ** -17) & (np.abs(f_in) <= 65504.0) | (f_in == 0.0)
+    assert np.array_equal(back[in_range], bits[in_range])
+    small = np.abs(f_in) < 2.0 ** -17
+    assert np.max(np.abs(f_out[small] - f_in[small])) <= 2.0 ** -25
+    big = np.abs(f_in) > 65504.0
+    assert big.sum() >= 2 and np.all(np.abs(f_out[big]) == 65536.0) and np.array_equal(np.sign(f_out[big]), np.sign(f_in[big]))
