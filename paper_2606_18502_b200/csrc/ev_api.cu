@@ -161,6 +161,7 @@ struct ev_model {
     unsigned long long* trace = nullptr;   // EV_TRACE=1: [TRACE_CAP][4] step trace, see ev_profile_trace
     int n_traced = 0;
     // tree state
+    int32_t *attn_order = nullptr;
     int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
     unsigned long long *anc = nullptr, *argmax_keys = nullptr;
     // static activation scales
@@ -606,7 +607,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     tp.seq_slots = in->dev_seq_slots; tp.tokens = in->dev_tokens; tp.parents = in->dev_parents; tp.n_nodes = in->dev_n_nodes;
     tp.ctx_len = c->ctx_len; tp.capacity = c->capacity; tp.max_seqs = c->max_seqs; tp.max_pos = m->max_pos;
     tp.Lsnap = m->Lsnap; tp.nn_eff = m->nn_eff; tp.status = out->dev_status; tp.depth = m->depth; tp.pos = m->pos;
-    tp.anc = m->anc; tp.argmax_keys = m->argmax_keys;
+    tp.anc = m->anc; tp.argmax_keys = m->argmax_keys; tp.order = m->attn_order;
     EV_TRY(launch_k(tree_prep_kernel, dim3((B + 63) / 64), dim3(64), 0, st, tp));
 
     const float* ovr = in->dev_hidden_override;
@@ -682,7 +683,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         AttnArgs aa;
         aa.q = m->qkv; aa.q_ld = m->qkv_dim; aa.T = T; aa.G = cfg.n_q_heads / cfg.n_kv_heads; aa.Hq = cfg.n_q_heads;
         aa.Hkv = cfg.n_kv_heads; aa.pool = ra.pool; aa.page_table = c->page_table; aa.max_pages = c->max_pages;
-        aa.page_size = cfg.page_size; aa.seq_slots = in->dev_seq_slots; aa.Lsnap = m->Lsnap; aa.nn_eff = m->nn_eff;
+        aa.page_size = cfg.page_size; aa.seq_slots = in->dev_seq_slots; aa.Lsnap = m->Lsnap; aa.nn_eff = m->nn_eff; aa.order = m->attn_order;
         aa.anc = m->anc; aa.split_len = split_len; aa.n_splits = n_splits; aa.scale = 1.0f / sqrtf((float)D);
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
         aa.ts = (m->gemm_dbg & 32) ? m->dbg_ts + 512 : nullptr;
@@ -862,6 +863,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     }
     A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
+    A(dev_alloc(m, &m->attn_order, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
     A(dev_alloc(m, &m->pos, (size_t)m->M_cap));
     A(dev_alloc(m, &m->anc, (size_t)m->M_cap));

@@ -32,6 +32,7 @@ struct AttnArgs {
     const int32_t* seq_slots;   // [B]
     const int32_t* Lsnap;       // [B]
     const int32_t* nn_eff;      // [B]
+    const int32_t* order;       // [B] grid z -> sequence (longest context first); null = identity
     const unsigned long long* anc;  // [B][T]
     int split_len;              // keys per split, multiple of ATT_CH
     int n_splits;               // grid.x

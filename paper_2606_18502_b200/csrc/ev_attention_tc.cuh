@@ -54,13 +54,17 @@ struct TcaCfg {
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
     static constexpr int SMEM = 1024 + Q_BYTES + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;
     // TMEM columns
-    // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
-    // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that); that
-    // frees room for TWO O chunks, so P.V of tile j+1 does not wait for the correction warps to read chunk j.
+    // S[3] and P[3] share three 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
+    // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that).  THREE
+    // regions: Q.K^T(j+2) is issued before P.V(j), so S(j+1) is long finished when the softmax warps get to it (with
+    // two regions Q.K^T(j+1) could only follow P.V(j-1): every tile paid a softmax -> MMA -> softmax round trip,
+    // 1,750 cycles per tile against 1,280 of tensor work).  TWO O chunks, so P.V of tile j+1 does not wait for the
+    // correction warps to read chunk j.
+    static constexpr int NSP = 3;
     static constexpr int TS = 0;
     static constexpr int TP = 0;
     static constexpr int SP = 64;           // columns per S/P region
-    static constexpr int TO = 128;          // O chunks: 2 x D fp32 columns
+    static constexpr int TO = NSP * SP;     // O chunks: 2 x D fp32 columns
     static_assert(TO + 2 * D <= 512, "TMEM budget");
     static constexpr int DH = D / 2;        // output columns per softmax warpgroup
 };
@@ -160,9 +164,9 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     uint64_t* k_empty = k_full + TCA_KS;                  // [KS]
     uint64_t* v_full = k_empty + TCA_KS;                  // [VS]
     uint64_t* v_empty = v_full + TCA_VS;                  // [VS]
-    uint64_t* s_full = v_empty + TCA_VS;                  // [2]
-    uint64_t* p_full = s_full + 2;                        // [2]
-    uint64_t* o_full = p_full + 2;                        // [2]
+    uint64_t* s_full = v_empty + TCA_VS;                  // [3]
+    uint64_t* p_full = s_full + C::NSP;                   // [3]
+    uint64_t* o_full = p_full + C::NSP;                   // [2]
     uint64_t* o_empty = o_full + 2;                       // [2]
     uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(o_empty + 2);
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
@@ -171,7 +175,6 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
 
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
-    const int b = blockIdx.z;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int R = a.T * a.G;
 
@@ -181,7 +184,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     if (threadIdx.x == 0) {
         for (int s = 0; s < TCA_KS; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
         for (int s = 0; s < TCA_VS; ++s) { mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
+        for (int i = 0; i < C::NSP; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
         for (int i = 0; i < 2; ++i) { mbar_init(&o_full[i], 1); mbar_init(&o_empty[i], 8); }
         fence_barrier_init();
         tma_prefetch_desc(&tmKV);
@@ -193,6 +196,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const uint32_t tmem_base = *tmem_base_smem;
     pdl_wait();
     trace_past_wait(ta.pf);
+    const int b = a.order ? a.order[blockIdx.z] : (int)blockIdx.z;
     const int nn = a.nn_eff[b];
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
@@ -295,14 +299,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const int s = i % TCA_VS;
             mbar_wait(&v_full[s], (i / TCA_VS) & 1);
             const long long t0_ = mts ? clock64() : 0;
-            mbar_wait(&p_full[i & 1], (i >> 1) & 1);
+            mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
             const long long t1_ = mts ? clock64() : 0;
             mbar_wait(&o_empty[i & 1], ((i >> 1) & 1) ^ 1);   // the correction warps have read chunk i - 2
             if (mts) { const long long t2_ = clock64(); mt_p += t1_ - t0_; mt_o += t2_ - t1_; }
             tc_fence_after();
             const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
             const uint32_t d_addr = tmem_base + C::TO + (i & 1) * D;
-            const uint32_t p_addr = tmem_base + C::TP + (i & 1) * C::SP;
+            const uint32_t p_addr = tmem_base + C::TP + (i % C::NSP) * C::SP;
             if (leader && do_mma) {
 #pragma unroll
                 for (int part = 1; part >= 0; --part) {
@@ -318,14 +322,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             }
             __syncwarp();
         };
-        for (int j = 0; j < n_tiles; ++j) {
+        auto issue_qk = [&](int j) {
             const int s = j % TCA_KS;
             const long long t0_ = mts ? clock64() : 0;
             mbar_wait(&k_full[s], (j / TCA_KS) & 1);
             if (mts) mt_kv += clock64() - t0_;
             tc_fence_after();
             const uint32_t k_addr = kv_addr + s * C::K_BYTES;
-            const uint32_t s_addr = tmem_base + C::TS + (j & 1) * C::SP;
+            const uint32_t s_addr = tmem_base + C::TS + (j % C::NSP) * C::SP;
             if (leader && do_mma) {
 #pragma unroll
                 for (int part = 1; part >= 0; --part) {
@@ -334,19 +338,25 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                         const uint64_t adesc = umma_desc_k128(q_addr + part * C::Q_PART + h * (128 * 128));
                         const uint64_t bdesc = umma_desc_k128(k_addr + h * 1024, C::SBO);
 #pragma unroll
-                        for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 bf16 = 32 B
+                        for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 elements = 32 B
                             umma_bf16_ss(s_addr, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, (part == 1 && h == 0 && ks == 0) ? 0u : 1u);
                     }
                 }
             }
             if (leader) {
                 umma_commit(&k_empty[s]);
-                umma_commit(&s_full[j & 1]);
+                umma_commit(&s_full[j % C::NSP]);
             }
             __syncwarp();
-            if (j >= 1) issue_pv(j - 1);
+        };
+        // Q.K^T runs two tiles ahead of P.V: S(j+2) goes into the region P(j-1) was read from by P.V(j-1), issued one
+        // iteration earlier (the tensor pipe executes in issue order)
+        issue_qk(0);
+        if (n_tiles > 1) issue_qk(1);
+        for (int j = 0; j < n_tiles; ++j) {
+            if (j + 2 < n_tiles) issue_qk(j + 2);
+            issue_pv(j);
         }
-        issue_pv(n_tiles - 1);
         if (mts && leader) { a.ts[14] = (unsigned long long)mt_p; a.ts[15] = (unsigned long long)(mt_kv + (mt_o << 32)); }
     } else if (warp < 10) {
         // ===== softmax: thread = (row, wg); wg handles keys [32 wg, +32) of every tile.  Warp w may touch TMEM
@@ -356,6 +366,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const int row = rg * 128 + r;
         const int node = row / a.G, gi = row % a.G;
         const bool valid = row < R && node < nn;
+        const bool warp_valid = __any_sync(0xffffffffu, valid);   // the same for both warps of a row quarter
         const unsigned long long anc = valid ? a.anc[b * a.T + node] : 1ull;
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
@@ -366,12 +377,18 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         long long tph[5] = {0, 0, 0, 0, 0}, tq = tsw ? clock64() : 0;
 #define TPH(k) do { if (tsw) { const long long t_ = clock64(); tph[k] += t_ - tq; tq = t_; } } while (0)
         for (int j = 0; j < n_tiles; ++j) {
-            mbar_wait(&s_full[j & 1], (j >> 1) & 1);
+            mbar_wait(&s_full[j % C::NSP], (j / C::NSP) & 1);
             tc_fence_after();
+            if (!warp_valid) {   // no live row in this warp (chain drafts: 16 of 128 rows): keep the barrier protocol only
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
+                continue;
+            }
             if (j == 0 && threadIdx.x == 64) trace_phase_any(ta.pf, 1);   // first S tile ready
             TPH(0);
             uint32_t sv[32];
-            tmem_ld32(lane_addr + C::TS + (j & 1) * C::SP + wg * 32, sv);
+            tmem_ld32(lane_addr + C::TS + (j % C::NSP) * C::SP + wg * 32, sv);
             tmem_ld_wait();
             TPH(1);
             const int kb = k_begin + j * TCA_BN + wg * 32;
@@ -403,7 +420,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             if (wg == 0) xc[(j & 7) * 128 + r] = c;
             const float nmk = fmaf(-mu, LOG2E, TCA_PSCALE_LOG2);   // p' = 2^15 p
             float ls0 = 0.f, ls1 = 0.f;
-            const uint32_t p_addr = lane_addr + C::TP + (j & 1) * C::SP + wg * 16;
+            const uint32_t p_addr = lane_addr + C::TP + (j % C::NSP) * C::SP + wg * 16;
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 uint32_t ph[8], pl[8];
@@ -423,7 +440,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&p_full[j & 1]);
+            if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
             TPH(4);
         }
         if (tsw && lane == 0) {
@@ -438,7 +455,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         // ---- running max and sum of this split ----
         l_run *= exp2f(-TCA_PSCALE_LOG2);   // exact
         xsum[wg * 128 + r] = l_run;
-        pair_bar_sync(1 + (warp & 3));
+        if (warp_valid) pair_bar_sync(1 + (warp & 3));
         if (valid && wg == 0) {
             const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
             *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m_run, l_run + xsum[128 + r]);
@@ -451,6 +468,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const int row = rg * 128 + r;
         const int node = row / a.G, gi = row % a.G;
         const bool valid = row < R && node < nn;
+        const bool warp_valid = __any_sync(0xffffffffu, valid);
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         float o[C::DH];
 #pragma unroll
@@ -458,6 +476,12 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         for (int i = 0; i < n_tiles; ++i) {
             mbar_wait(&o_full[i & 1], (i >> 1) & 1);
             tc_fence_after();
+            if (!warp_valid) {   // no live row in this warp: release the chunk, nothing to add
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&o_empty[i & 1]);
+                continue;
+            }
             const float c = xc[(i & 7) * 128 + r];
 #pragma unroll
             for (int cb = 0; cb < C::DH / 16; ++cb) {

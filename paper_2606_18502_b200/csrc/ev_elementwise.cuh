@@ -79,6 +79,7 @@ struct TreePrepArgs {
     int max_seqs, max_pos;
     int32_t* Lsnap;            // [B] context length at entry
     int32_t* nn_eff;           // [B] nodes in use (0 when the sequence is rejected)
+    int32_t* order;            // [B] sequences by decreasing context length (attention CTAs start the longest first)
     int32_t* status;           // [B]
     int32_t* depth;            // [B][T]
     int32_t* pos;              // [B][T] RoPE position = L + depth
@@ -114,6 +115,16 @@ __global__ void tree_prep_kernel(TreePrepArgs a) {
     a.status[b] = st;
     a.Lsnap[b] = L;
     a.nn_eff[b] = st ? 0 : nn;
+    {   // rank of this sequence by decreasing context length (ties by index): the attention grid walks sequences in
+        // this order, so with mixed lengths (config[3]: 1,024..8,192) the long CTAs start first and the tail is short
+        int rank = 0;
+        for (int o = 0; o < a.B; ++o) {
+            const int so = a.seq_slots[o];
+            const int Lo = (so < 0 || so >= a.max_seqs) ? 0 : a.ctx_len[so];
+            rank += (Lo > L || (Lo == L && o < b)) ? 1 : 0;
+        }
+        a.order[rank] = b;
+    }
     for (int i = 0; i < T; ++i) {
         int d = 0;
         unsigned long long m = 1ull;  // padding / rejected rows see the root only
