@@ -60,7 +60,7 @@ struct GemmArgs {
     L2Prefetch pf;      // slice of the weight stream of the GEMMs that follow (ev_common.cuh)
     const void* warm[2];   // per-layer constants the CONSUMER kernel will read first thing after its wait (this
     int warm_bytes[2];     // matrix's s_w, the next RMSNorm's gain): touched here so they are L2 hits there
-    int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads
+    int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads, 64 skip stores
     int bal;            // balanced partition (several token tiles): the (n unit, 16-token block) space, n unit major, is dealt
                         // out evenly to the CTAs (CTA pairs); a CTA's contiguous range is cut at n-unit boundaries and into
                         // items of <= 256 tokens, so token tiles differ in size from item to item (GemmItem::tok) and no
@@ -465,7 +465,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     for (int j = 0; j < GC; ++j) {
                         const int col = g * GC + j;
                         const int m = m0 + col;
-                        if (n_ok && col < tok && m < a.M) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
+                        if (n_ok && col < tok && m < a.M && !(a.dbg & 64)) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
                     }
                 }
             }
