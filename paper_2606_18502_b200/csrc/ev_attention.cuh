@@ -343,6 +343,24 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
     float* w = msm;
     float* ls = msm + a.Hq * S;
     float* den = ls + a.Hq * S;
+    // The partial outputs of the first NB splits are requested BEFORE the split weights are computed (they only need
+    // ns): the (max, sum) round trip, the two CTA barriers and the exps then run under the loads instead of in front
+    // of them.  One float4 per thread (few tokens, rows spread over a cluster): 12 splits in flight; else 4.
+    constexpr int NB = MERGE_NV4 == 1 ? 12 : 4;
+    float4 v[MERGE_NV4];
+    int c0, c1;
+    cluster_cols(K / 4, c0, c1);
+    float4 t0[NB];
+    {
+        const int i4 = c0 + threadIdx.x;
+        const int i = i4 * 4;
+        if (i4 < c1 && valid) {
+            const float* op = a.o_part + ((size_t)m * a.Hq + i / a.D) * S * a.D + i % a.D;
+#pragma unroll
+            for (int u = 0; u < NB; ++u)
+                if (u < ns) t0[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)u * a.D));
+        }
+    }
     for (int i = threadIdx.x; i < a.Hq * S; i += MERGE_THREADS) {
         const int h = i / S, sp = i % S;
         float2 ml = make_float2(-INFINITY, 0.f);
@@ -365,9 +383,6 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
         den[h] = d;
     }
     __syncthreads();
-    float4 v[MERGE_NV4];
-    int c0, c1;
-    cluster_cols(K / 4, c0, c1);
 #pragma unroll
     for (int k = 0; k < MERGE_NV4; ++k) {
         const int i4 = c0 + threadIdx.x + k * MERGE_THREADS;
@@ -377,13 +392,23 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
             const int h = i / a.D, d = i % a.D;
             const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * a.D + d;
             float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
-            for (int s0 = 0; s0 < ns; s0 += 8) {
-                float4 t[8];
+            int s_done = 0;
+            if (k == 0) {   // the splits requested up front
 #pragma unroll
-                for (int u = 0; u < 8; ++u)
+                for (int u = 0; u < NB; ++u)
+                    if (u < ns) {
+                        const float wt = w[h * S + u];
+                        num.x += wt * t0[u].x; num.y += wt * t0[u].y; num.z += wt * t0[u].z; num.w += wt * t0[u].w;
+                    }
+                s_done = NB;
+            }
+            for (int s0 = s_done; s0 < ns; s0 += 4) {   // splits are added in index order, whatever the batching
+                float4 t[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
                     if (s0 + u < ns) t[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)(s0 + u) * a.D));
 #pragma unroll
-                for (int u = 0; u < 8; ++u)
+                for (int u = 0; u < 4; ++u)
                     if (s0 + u < ns) {
                         const float wt = w[h * S + s0 + u];
                         num.x += wt * t[u].x; num.y += wt * t[u].y; num.z += wt * t[u].z; num.w += wt * t[u].w;
