@@ -1463,6 +1463,10 @@ int ev_debug_gemm_timestamps(ev_model* m, unsigned long long* host_out, int n_ct
     if (!m || !host_out) return fail(EV_EINVAL, "null argument");
     CUDA_TRY(cudaDeviceSynchronize());
     if (n_ctas > 128) n_ctas = 128;
+    if (n_ctas == -2) {  // attention: (start, end, SM id) of up to 512 CTAs
+        CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts + 1024, 3 * 512 * 8, cudaMemcpyDeviceToHost));
+        return EV_OK;
+    }
     if (n_ctas < 0) {  // attention timestamps
         CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts + 512, 16 * 8, cudaMemcpyDeviceToHost));
         return EV_OK;

@@ -197,6 +197,16 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     pdl_wait();
     trace_past_wait(ta.pf);
     const int b = a.order ? a.order[blockIdx.z] : (int)blockIdx.z;
+    // bring-up (EV_GEMM_DBG=32): per-CTA start / end / SM id at ts[512 + 3 cta ..] (ev_debug_gemm_timestamps(-2))
+    const int cta_lin = (int)(blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
+    if (a.ts && threadIdx.x == 0 && cta_lin < 512) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        a.ts[512 + 3 * cta_lin] = t;
+        a.ts[512 + 3 * cta_lin + 2] = smid;
+    }
     const int nn = a.nn_eff[b];
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
@@ -515,6 +525,11 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<512>(tmem_base);
+    if (a.ts && threadIdx.x == 0 && cta_lin < 512) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        a.ts[512 + 3 * cta_lin + 1] = t;
+    }
     trace_exit(ta.pf);
 }
 
