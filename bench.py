@@ -333,6 +333,18 @@ def main():
     emitted = int((acc + 1).sum())
     if rank != 0:
         return
+    # static scales (config[4]): the clip rate PAPER.md:140 reports, from the quantizers' own counters over one step
+    clip = None
+    if spec.act_scale_mode == 1:
+        model.ev_model_get_clip_counts(reset=True)
+        step()
+        torch.cuda.synchronize()
+        cc = model.ev_model_get_clip_counts(reset=True)
+        sh = spec.model
+        per_layer = B * T * (2 * sh.hidden + sh.n_q_heads * sh.head_dim + sh.ffn)   # qkv_in, gateup_in, o_in, down_in
+        n_el = sh.n_layers * per_layer + B * T * sh.hidden
+        clip = {"clipped": int(cc.sum()), "quantized_elements": int(n_el), "rate": float(cc.sum()) / n_el,
+                "def": "activation elements with |x| > 448 * s_site over one verify step (PAPER.md:140)"}
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         r = oracle_sample(spec, 4, 1, log)
@@ -357,6 +369,8 @@ def main():
         "gpu_launches": int(launches), "clocks": clocks,
         "attention": {"ms_per_step": round(attn_ms / args.steps, 4), "kv_gbs": round(work["kv_bytes"] * args.steps / max(attn_ms, 1e-9) / 1e6, 1)},
     }
+    if clip is not None:
+        line["clip_rate"] = clip
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -116,6 +116,13 @@ int ev_model_calibrate(ev_model*, const float* dev_hidden, int n_tok, float* dev
 int ev_model_get_static_scales(ev_model*, float* host_out);
 /* Overrides them (same order); used to replay externally calibrated scales. */
 int ev_model_set_static_scales(ev_model*, const float* host_in);
+/* Clip counters (Fig. 4 "clip rate"): with static scales
+ * (act_scale_mode == 1) every activation quantizer counts the elements it saturates, |x| > 448 * s_site,
+ * per site, in the order of ev_model_get_static_scales, accumulated over all calls since the last reset
+ * (calibration passes do not count).  Copies the 4*n_layers+1 counters to host_out (host memory owned by the
+ * caller); reset != 0 zeroes them afterwards.  Synchronous (waits for the device).  All zero in dynamic
+ * mode.  Returns EV_EINVAL on null arguments. */
+int ev_model_get_clip_counts(ev_model*, unsigned long long* host_out, int reset);
 
 int ev_model_destroy(ev_model*);
 

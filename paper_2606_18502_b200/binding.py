@@ -54,6 +54,7 @@ SIGNATURES = {
     "ev_model_calibrate": (C.c_int, [_P, _P, C.c_int, _P, _P]),
     "ev_model_get_static_scales": (C.c_int, [_P, _P]),
     "ev_model_set_static_scales": (C.c_int, [_P, _P]),
+    "ev_model_get_clip_counts": (C.c_int, [_P, _P, C.c_int]),
     "ev_model_destroy": (C.c_int, [_P]),
     "ev_cache_create": (C.c_int, [_P, C.c_long, C.c_int, C.POINTER(_P)]),
     "ev_cache_add_seq": (C.c_int, [_P, C.c_int, _P, C.POINTER(C.c_int)]),
@@ -162,6 +163,12 @@ class Model:
         import numpy as np
         out = np.empty(4 * self.cfg.n_layers + 1, dtype=np.float32)
         _check(self.lib.ev_model_get_static_scales(self.h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def ev_model_get_clip_counts(self, reset=False):
+        import numpy as np
+        out = np.zeros(4 * self.cfg.n_layers + 1, dtype=np.uint64)
+        _check(self.lib.ev_model_get_clip_counts(self.h, out.ctypes.data_as(C.c_void_p), 1 if reset else 0))
         return out
 
     def ev_model_set_static_scales(self, scales):

@@ -168,6 +168,7 @@ struct ev_model {
     int n_sites = 0;
     float* static_scales = nullptr;  // device [n_sites]
     float* site_amax = nullptr;      // device [n_sites]
+    unsigned long long* clip_counts = nullptr;  // device [n_sites]: elements clipped by the static scales since the last reset
     bool calibrated = false, recording = false;
     int num_sms = 148;
     bool use_splitk = false, naive_gemm = false, legacy_attn = false;
@@ -536,6 +537,7 @@ QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
     q.sx = b.scale;
     q.static_scale = (m->cfg.act_scale_mode == 1 && !m->recording) ? m->static_scales + site : nullptr;
     q.site_amax = m->recording ? m->site_amax + site : nullptr;
+    q.clip_count = q.static_scale ? m->clip_counts + site : nullptr;
     return q;
 }
 
@@ -870,6 +872,8 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->argmax_keys, (size_t)m->M_cap));
     A(dev_alloc(m, &m->static_scales, (size_t)m->n_sites));
     A(dev_alloc(m, &m->site_amax, (size_t)m->n_sites));
+    A(dev_alloc(m, &m->clip_counts, (size_t)m->n_sites));
+    cudaMemset(m->clip_counts, 0, (size_t)m->n_sites * 8);
     A(dev_alloc(m, &m->rope_cs, (size_t)m->max_pos * (cfg->head_dim / 2)));
     if (rc == EV_OK) {
         // RoPE table: angle = p * theta^(-2j/d) in fp64, cos/sin rounded to fp32 (DESIGN.md R-rope)
@@ -982,6 +986,13 @@ int ev_model_get_static_scales(ev_model* m, float* host_out) {
     if (!m || !host_out) return fail(EV_EINVAL, "null argument");
     if (!m->calibrated) return fail(EV_ESTATE, "not calibrated");
     CUDA_TRY(cudaMemcpy(host_out, m->static_scales, m->n_sites * sizeof(float), cudaMemcpyDeviceToHost));
+    return EV_OK;
+}
+int ev_model_get_clip_counts(ev_model* m, unsigned long long* host_out, int reset) {
+    if (!m || !host_out) return fail(EV_EINVAL, "null argument");
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(host_out, m->clip_counts, m->n_sites * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    if (reset) CUDA_TRY(cudaMemset(m->clip_counts, 0, m->n_sites * sizeof(unsigned long long)));
     return EV_OK;
 }
 int ev_model_set_static_scales(ev_model* m, const float* host_in) {
@@ -1345,7 +1356,7 @@ int ev_op_quantize_rows(ev_model* m, const float* dev_x, int M, int K, float sta
     if (!m || !dev_x || !dev_codes || !dev_sx || M < 1 || K < 4 || K % 4) return fail(EV_EINVAL, "bad argument");
     cudaStream_t st = (cudaStream_t)stream;
     QuantOut q;
-    q.codes = dev_codes; q.sx = dev_sx; q.static_scale = nullptr; q.site_amax = nullptr;
+    q.codes = dev_codes; q.sx = dev_sx; q.static_scale = nullptr; q.site_amax = nullptr; q.clip_count = nullptr;
     if (static_scale > 0.f) {
         CUDA_TRY(cudaMemcpyAsync(m->site_amax, &static_scale, 4, cudaMemcpyHostToDevice, st));
         CUDA_TRY(cudaStreamSynchronize(st));

@@ -163,7 +163,18 @@ struct QuantOut {
     float* sx;                 // [M]
     const float* static_scale; // null = dynamic per-token
     float* site_amax;          // null, or calibration accumulator (atomicMax on the float's bits)
+    unsigned long long* clip_count;  // null, or (static scales) this site's count of elements with |x| > 448 s: the
+                                     // clipping PAPER.md:140 measures ("clip rate"); SURVEY section 8(f)-1
 };
+// adds this thread's count of clipped elements to the site counter: one atomic per warp that saw any
+__device__ __forceinline__ void clip_add(const QuantOut& q, unsigned cnt) {
+    if (!q.clip_count) return;   // uniform
+    const unsigned tot = __reduce_add_sync(0xffffffffu, cnt);
+    if (tot && (threadIdx.x & 31) == 0) atomicAdd(q.clip_count, (unsigned long long)tot);
+}
+__device__ __forceinline__ unsigned clip4(float x0, float x1, float x2, float x3, float thr) {
+    return (unsigned)(fabsf(x0) > thr) + (unsigned)(fabsf(x1) > thr) + (unsigned)(fabsf(x2) > thr) + (unsigned)(fabsf(x3) > thr);
+}
 
 template <class F>
 __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut& q, float* red) {
@@ -181,8 +192,13 @@ __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut
         if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
     }
     uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
-    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4)
+    const float thr = mul_rn(448.0f, s);
+    unsigned clipped = 0;
+    for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4) {
         dst[i >> 2] = e4m3x4(div_rn(val(i), s), div_rn(val(i + 1), s), div_rn(val(i + 2), s), div_rn(val(i + 3), s));
+        clipped += clip4(val(i), val(i + 1), val(i + 2), val(i + 3), thr);
+    }
+    clip_add(q, clipped);
 }
 
 // row held in registers, spread over the CTAs of a cluster: this CTA owns the float4 numbers [c0, c1) of the
@@ -205,11 +221,17 @@ __device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int
         if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
     }
     uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
+    const float thr = mul_rn(448.0f, s);
+    unsigned clipped = 0;
 #pragma unroll
     for (int k = 0; k < NV4; ++k) {
         const int i4 = c0 + (int)threadIdx.x + k * nthr;
-        if (i4 < c1) dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
+        if (i4 < c1) {
+            dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
+            clipped += clip4(v[k].x, v[k].y, v[k].z, v[k].w, thr);
+        }
     }
+    clip_add(q, clipped);
 }
 // this CTA's share [c0, c1) of a row of n4 float4s
 __device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
@@ -391,10 +413,14 @@ __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_smem_kernel(LinOut g
         if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
     }
     uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * F);
+    const float thr = mul_rn(448.0f, s);
+    unsigned clipped = 0;
     for (int i4 = threadIdx.x; i4 < n4; i4 += SWI_THREADS) {
         const float4 t = swi_row[i4];   // written by this same thread
         dst[i4] = e4m3x4(div_rn(t.x, s), div_rn(t.y, s), div_rn(t.z, s), div_rn(t.w, s));
+        clipped += clip4(t.x, t.y, t.z, t.w, thr);
     }
+    clip_add(q, clipped);
     trace_exit(pf);
 }
 

@@ -349,3 +349,47 @@ def test_kv_pool_container_round_trip(setup):
     assert np.max(np.abs(f_out[small] - f_in[small])) <= 2.0 ** -25
     big = np.abs(f_in) > 65504.0
     assert big.sum() >= 2 and np.all(np.abs(f_out[big]) == 65536.0) and np.array_equal(np.sign(f_out[big]), np.sign(f_in[big]))
+
+
+def test_static_scales_clip_counters_match_oracle():
+    """SURVEY 8(f)-1 / PAPER.md:140 ("clip rate"): with static per-site scales every activation quantizer counts
+    the elements it saturates (|x| > 448 s).  Scales = half of the oracle's calibrated ones, so thousands of
+    elements clip; the GPU's counters (ev_model_get_clip_counts) must reproduce the oracle's counts for one verify
+    step: exactly at layer 0's first site (its input is the embedding: no accumulated rounding), and within 1 %
+    (+2) elsewhere - both sides run free, an element within rounding of the threshold may fall either way."""
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import gpu_model, import_oracle_kv, run_verify
+    spec = wl.CONFIGS[0]
+    shape = spec.model
+    om = oracle_model(shape, spec.seed, act_scale_mode=1)
+    rng = np.random.default_rng(11)
+    rec = vo.calibrate(om, rng.standard_normal((64, shape.hidden)).astype(np.float32))
+    sites = ("qkv_in", "o_in", "gateup_in", "down_in")
+    scales = np.empty(4 * shape.n_layers + 1, dtype=np.float32)
+    for l in range(shape.n_layers):
+        for j, site in enumerate(sites):
+            scales[4 * l + j] = np.float32(0.5) * om.static[(site, l)]
+            om.static[(site, l)] = scales[4 * l + j]
+    scales[-1] = np.float32(0.5) * om.static[("lm_in", 0)]
+    om.static[("lm_in", 0)] = scales[-1]
+    gm = gpu_model(shape, spec.seed, max_batch=2, max_tree_nodes=16, max_ctx=512, act_scale_mode=1)
+    gm.ev_model_set_static_scales(scales)
+
+    ids = wl.context_ids(spec, 0, spec.ctx_len)
+    oc = _oracle_ctx(om, ids)                       # oracle prefill, static scales
+    parents = np.array([-1, 0, 0, 1, 1, 2, 3, 3, 4, 6, 6, 9], dtype=np.int32)
+    toks = wl.draft_tokens_uniform(spec, parents, 0)
+    cache = ev.Cache(gm, 64, 2)
+    slot = cache.ev_cache_add_seq(256)
+    import_oracle_kv(cache, slot, oc, 0, spec.ctx_len, shape.n_layers)
+    gm.ev_model_get_clip_counts(reset=True)
+    om.clip_counts = {}
+    vo.verify(om, oc, 0, toks, parents, commit=False)
+    run_verify(gm, cache, [slot], toks[None], parents[None], commit=False)
+    got = gm.ev_model_get_clip_counts(reset=True)
+    want = np.array([om.clip_counts.get((site, l), 0) for l in range(shape.n_layers) for site in sites] +
+                    [om.clip_counts.get(("lm_in", 0), 0)], dtype=np.int64)
+    assert want.sum() > 100, want                   # the halved scales do clip
+    assert int(got[0]) == int(want[0])
+    assert np.all(np.abs(got.astype(np.int64) - want) <= 2 + want // 100), (got, want)
+    assert gm.ev_model_get_clip_counts().sum() == 0  # reset worked
