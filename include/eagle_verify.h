@@ -71,6 +71,9 @@ typedef struct {
     int max_batch;        /* B upper bound per ev_verify call */
     int max_tree_nodes;   /* T upper bound, <= EV_MAX_TREE_NODES */
     int max_ctx;          /* upper bound on ctx_len + tree nodes of any sequence (RoPE table) */
+    int weight_scale_mode; /* 0 = one E4M3 scale per output channel (BASELINE.json:north_star); 1 = one scale per
+                            * weight matrix, absmax / 448 over the whole matrix ("per-tensor";
+                            * SURVEY section 8(f)-1; each of Q, K, V, gate, up keeps its own scale) */
 } ev_config;
 
 typedef enum {

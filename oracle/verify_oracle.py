@@ -73,19 +73,29 @@ def _matmul64(a, bt):
 
 # ----------------------------------------------------------------------------- quantization
 
-def quantize_weight(w_bf16_bits):
-    """Per-output-channel absmax E4M3 quantization of a [N_out, K] bf16 matrix.
-    BASELINE.json:configs[0] "E4M3 per-output-channel absmax scales"; PAPER.md:98 "min-max".
-    s_w[n] = max_k |W[n,k]| / 448 (fp32 IEEE division; 1 for an all-zero row);
-    Wq[n,k] = encode(W[n,k] / s_w[n]) (fp32 IEEE division).  DESIGN.md R-quant."""
+def quantize_weight(w_bf16_bits, per_tensor=False):
+    """Absmax E4M3 quantization of a [N_out, K] bf16 matrix.
+    Per output channel (default; BASELINE.json:configs[0] "E4M3 per-output-channel absmax scales";
+    PAPER.md:98 "min-max"): s_w[n] = max_k |W[n,k]| / 448 (fp32 IEEE division; 1 for an all-zero row);
+    Wq[n,k] = encode(W[n,k] / s_w[n]) (fp32 IEEE division).  DESIGN.md R-quant.
+    per_tensor=True ("per-tensor"; DESIGN.md R-pertensor): ONE scale per
+    matrix, s_w = max_{n,k} |W[n,k]| / 448, returned replicated over the N_out channels."""
+    w_bf16_bits = np.asarray(w_bf16_bits)
+    t_amax = None
+    if per_tensor:
+        t_amax = F32(0.0)
+        for r0 in range(0, w_bf16_bits.shape[0], 4096):
+            t_amax = max(t_amax, F32(np.max(np.abs(bf16_bits_to_f32(w_bf16_bits[r0:r0 + 4096])))))
+
     def rows(block):
         w = bf16_bits_to_f32(block)
         amax = np.max(np.abs(w), axis=1).astype(F32)
+        if t_amax is not None:
+            amax = np.full_like(amax, t_amax)
         s = (amax / F32(448.0)).astype(F32)
         s = np.where(amax == 0, F32(1.0), s).astype(F32)
         return e4m3.encode((w / s[:, None]).astype(F32)), s
 
-    w_bf16_bits = np.asarray(w_bf16_bits)
     n = w_bf16_bits.shape[0]
     if w_bf16_bits.size < (1 << 22):
         return rows(w_bf16_bits)
@@ -229,11 +239,12 @@ class OracleModel:
     input quantization and are three independent per-output-channel matrices, likewise gate/up
     (DESIGN.md R-quant).  Embedding and RMSNorm gains stay bf16 (R-embed)."""
 
-    def __init__(self, shape, act_scale_mode=0, accum="exact"):
+    def __init__(self, shape, act_scale_mode=0, accum="exact", weight_scale_mode=0):
         for f in ("n_layers", "hidden", "n_q_heads", "n_kv_heads", "head_dim", "ffn", "vocab",
                   "rms_eps", "rope_theta"):
             setattr(self, f, getattr(shape, f))
         self.act_scale_mode = act_scale_mode
+        self.weight_scale_mode = weight_scale_mode   # 0 per output channel, 1 per tensor (each matrix its own scale)
         self.accum = accum
         self.w = {}          # (kind, layer) -> (codes, scales)
         self.embed = None    # bf16 bits [V, H]
@@ -247,7 +258,7 @@ class OracleModel:
         elif kind in ("norm1", "norm2", "normf"):
             self.gain[(kind, layer)] = bf16_bits_to_f32(bf16_bits)
         else:
-            self.w[(kind, layer)] = quantize_weight(bf16_bits)
+            self.w[(kind, layer)] = quantize_weight(bf16_bits, per_tensor=self.weight_scale_mode == 1)
 
     def set_quantized(self, kind, layer, codes, scales):
         self.w[(kind, layer)] = (np.ascontiguousarray(codes, dtype=np.uint8), np.ascontiguousarray(scales, dtype=F32))

@@ -168,6 +168,7 @@ struct ev_model {
     int n_sites = 0;
     float* static_scales = nullptr;  // device [n_sites]
     float* site_amax = nullptr;      // device [n_sites]
+    float* w_amax = nullptr;         // device scalar: absmax of the matrix being quantized (per-tensor weight scales)
     unsigned long long* clip_counts = nullptr;  // device [n_sites]: elements clipped by the static scales since the last reset
     bool calibrated = false, recording = false;
     int num_sms = 148;
@@ -802,6 +803,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     if (cfg->max_tree_nodes < 1 || cfg->max_tree_nodes > EV_MAX_TREE_NODES) return fail(EV_EINVAL, "max_tree_nodes must be 1..64");
     if (cfg->max_batch < 1 || cfg->max_ctx < 1) return fail(EV_EINVAL, "max_batch / max_ctx must be positive");
     if (cfg->act_scale_mode != 0 && cfg->act_scale_mode != 1) return fail(EV_EINVAL, "act_scale_mode must be 0 or 1");
+    if (cfg->weight_scale_mode != 0 && cfg->weight_scale_mode != 1) return fail(EV_EINVAL, "weight_scale_mode must be 0 or 1");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(EV_ECUDA, "no CUDA device");
     ev_model* m = new ev_model();
@@ -872,6 +874,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->argmax_keys, (size_t)m->M_cap));
     A(dev_alloc(m, &m->static_scales, (size_t)m->n_sites));
     A(dev_alloc(m, &m->site_amax, (size_t)m->n_sites));
+    A(dev_alloc(m, &m->w_amax, (size_t)1));
     A(dev_alloc(m, &m->clip_counts, (size_t)m->n_sites));
     cudaMemset(m->clip_counts, 0, (size_t)m->n_sites * 8);
     A(dev_alloc(m, &m->rope_cs, (size_t)m->max_pos * (cfg->head_dim / 2)));
@@ -920,8 +923,17 @@ int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, 
     auto shape_is = [&](long r, long k) { return rows == r && cols == k; };
     auto bad_shape = [&]() { return fail(EV_EINVAL, "weight shape does not match the model config"); };
     auto quant = [&](QMat& q, long row_off) -> int {
+        const float* t_amax = nullptr;
+        if (c.weight_scale_mode == 1) {   // per-tensor: the matrix's absmax first (cols % 8 == 0: rows * cols / 8 uint4s)
+            CUDA_TRY(cudaMemsetAsync(m->w_amax, 0, sizeof(float), st));
+            const long n8 = rows * cols / 8;
+            tensor_absmax_bf16_kernel<<<(unsigned)std::min<long>((n8 + 255) / 256, 4L * m->num_sms), 256, 0, st>>>(
+                (const __nv_bfloat16*)dev_bf16, n8, m->w_amax);
+            LAUNCH_CHECK();
+            t_amax = m->w_amax;
+        }
         quantize_weight_rows_kernel<<<(unsigned)rows, EW_THREADS, 0, st>>>((const __nv_bfloat16*)dev_bf16, cols, q.codes, q.total_kb,
-                                                                          row_off, q.scale);
+                                                                          row_off, q.scale, t_amax);
         LAUNCH_CHECK();
         return EV_OK;
     };

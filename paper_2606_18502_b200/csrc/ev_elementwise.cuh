@@ -22,13 +22,32 @@ __device__ __forceinline__ float block_max(float v, float* red) {
     return r;
 }
 
+// absmax of a bf16 matrix (per-tensor weight scales): atomicMax on the bits of a non-negative float; *out zeroed before
+__global__ void __launch_bounds__(256) tensor_absmax_bf16_kernel(const __nv_bfloat16* __restrict__ w, long n8, float* __restrict__ out) {
+    __shared__ float red[8];
+    const uint4* src = reinterpret_cast<const uint4*>(w);
+    float amax = 0.f;
+    for (long i = blockIdx.x * 256L + threadIdx.x; i < n8; i += (long)gridDim.x * 256) {
+        const uint4 v = __ldg(src + i);
+        const uint32_t u[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            amax = fmaxf(amax, fabsf(__uint_as_float(u[j] << 16)));
+            amax = fmaxf(amax, fabsf(__uint_as_float(u[j] & 0xFFFF0000u)));
+        }
+    }
+    amax = block_max(amax, red);
+    if (threadIdx.x == 0) atomicMax(reinterpret_cast<int*>(out), __float_as_int(amax));
+}
+
 // ---- K1: per-output-channel absmax -> scale, E4M3 codes --------------------------------------
 // one CTA per output channel (row); cols % 8 == 0.  Codes are written straight into the GEMM's HBM
 // layout: [n/128][k/128] tiles of 128 rows x 128 bytes, 16 KiB contiguous, 128-byte swizzled
 // (ev_gemm.cuh); row_off = first row of this matrix inside fused storage (QKV, gate|up).
 __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const __nv_bfloat16* __restrict__ w, long cols,
                                                                           uint8_t* __restrict__ codes_tiled, int total_kb,
-                                                                          long row_off, float* __restrict__ scales) {
+                                                                          long row_off, float* __restrict__ scales,
+                                                                          const float* __restrict__ tensor_amax) {
     __shared__ float red[EW_THREADS / 32];
     const long row = blockIdx.x;
     const uint4* src = reinterpret_cast<const uint4*>(w + row * cols);
@@ -44,6 +63,7 @@ __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const 
         }
     }
     amax = block_max(amax, red);
+    if (tensor_amax) amax = *tensor_amax;   // per-tensor mode: the whole matrix's absmax (tensor_absmax_bf16_kernel)
     const float s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
     const long n = row_off + row;
     if (threadIdx.x == 0) scales[n] = s;

@@ -9,11 +9,11 @@ LAYER_KINDS = ("wq", "wk", "wv", "wo", "wgate", "wup", "wdown")
 
 
 def oracle_model(shape, seed, random_gains=False, act_scale_mode=0, accum="exact", layers=None,
-                 with_lm_head=True, device="cpu", weight_fn=None):
+                 with_lm_head=True, device="cpu", weight_fn=None, weight_scale_mode=0):
     """weight_fn(kind, layer) -> uint16 bits overrides the generator (8B shapes: tensors drawn on
     the GPU and copied to the host)."""
     get = weight_fn or (lambda kind, layer: wl.weight_matrix_bf16(shape, seed, kind, layer))
-    m = vo.OracleModel(shape, act_scale_mode=act_scale_mode, accum=accum)
+    m = vo.OracleModel(shape, act_scale_mode=act_scale_mode, accum=accum, weight_scale_mode=weight_scale_mode)
     m.set_weight("embed", 0, get("embed", 0))
     for layer in (range(shape.n_layers) if layers is None else layers):
         for kind in LAYER_KINDS:

@@ -155,3 +155,35 @@ def test_fp8_gemm_accumulation_error_at_8b_k():
     print("GEMM accumulation vs exact:", report)
     for kind in ("wq", "wdown"):
         assert report[kind][0] < 1e-5 and report[kind][1] < 2.0 ** -18, report
+
+
+def test_per_tensor_weight_scales_bit_exact_and_verify_parity():
+    """weight_scale_mode = 1 (PAPER.md:98 per-tensor min-max): codes and (replicated) scales of every
+    matrix equal the oracle's bit for bit; one verify step on the tiny config stays within the north_star bars."""
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import gpu_model, import_oracle_kv, run_verify
+    from helpers import oracle_model, fresh_cache
+    spec = wl.CONFIGS[0]
+    shape = spec.model
+    gm = gpu_model(shape, spec.seed, max_batch=2, max_tree_nodes=16, max_ctx=512, weight_scale_mode=1)
+    for kind, layer in (("wq", 0), ("wk", 1), ("wv", 0), ("wo", 1), ("wgate", 0), ("wup", 1), ("wdown", 0), ("lm_head", 0)):
+        bits = wl.weight_matrix_bf16(shape, spec.seed, kind, layer)
+        codes_o, s_o = vo.quantize_weight(bits, per_tensor=True)
+        codes_g, s_g = gm.ev_model_get_quantized(kind, layer)
+        assert np.array_equal(s_g.cpu().numpy(), s_o), kind
+        assert np.array_equal(codes_g.cpu().numpy(), codes_o), kind
+    om = oracle_model(shape, spec.seed, weight_scale_mode=1)
+    oc = fresh_cache(om, 256)
+    vo.prefill(om, oc, 0, wl.context_ids(spec, 0, spec.ctx_len))
+    parents = wl.chain_parents(spec.n_nodes)
+    toks = wl.draft_tokens_uniform(spec, parents, 0)
+    cache = ev.Cache(gm, 64, 2)
+    slot = cache.ev_cache_add_seq(256)
+    import_oracle_kv(cache, slot, oc, 0, spec.ctx_len, shape.n_layers)
+    res = vo.verify(om, oc, 0, toks, parents, commit=False, want_hidden=True)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None], commit=False)
+    hid = buf.hidden.cpu().numpy()
+    for l, h_ref in enumerate(res["hidden"]):
+        assert rel_l2(hid[l, :spec.n_nodes], h_ref) <= 1e-2
+    lg = buf.logits.cpu().numpy()[:spec.n_nodes]
+    assert np.max(np.abs(lg - res["logits"])) <= 2e-2 * float(res["logits"].std())

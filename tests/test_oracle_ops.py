@@ -192,3 +192,39 @@ def test_p12_static_mode_clip_count_equals_saturated_codes():
     assert 100 < n_clip and np.count_nonzero(sat & (np.abs(x) > np.float32(1.75))) == n_clip
     deq = e4m3.decode(codes) * float(s)
     assert np.max(np.abs(deq)) == 1.75
+
+
+def test_per_tensor_weight_quantizer_pins():
+    """SURVEY 8(f)-1 / PAPER.md:98, 140: per-tensor min-max weight scales.  Pinned without retyping the formula:
+    (i) a matrix on the E4M3 grid times ONE power of two quantizes losslessly with s = 2^k on every channel;
+    (ii) the row that holds the matrix absmax gets the same codes as under per-channel scales, every other row's
+    per-channel scale is <= the tensor scale; (iii) every code is the E4M3 value nearest to w / s, found by
+    exhaustive search over the 256 codes (ties to the even code); (iv) an all-zero matrix has scale 1."""
+    rng = np.random.default_rng(5)
+    t = e4m3.decode_table()
+    finite = t[~np.isnan(t)]
+    w = (rng.choice(finite, size=(16, 64)) * 2.0 ** -7).astype(np.float32)
+    w[3, 5] = np.float32(448.0 * 2.0 ** -7)
+    bits = wl.f32_to_bf16_bits(w)
+    codes, s = vo.quantize_weight(bits, per_tensor=True)
+    assert np.all(s == np.float32(2.0 ** -7))
+    assert np.array_equal(e4m3.decode(codes) * 2.0 ** -7, w.astype(np.float64))
+
+    bits = wl.weight_matrix_bf16(wl.TINY, 0, "wq", 0)
+    wf = wl.bf16_bits_to_f32(bits)
+    codes_t, s_t = vo.quantize_weight(bits, per_tensor=True)
+    codes_c, s_c = vo.quantize_weight(bits)
+    r, _ = np.unravel_index(np.argmax(np.abs(wf)), wf.shape)
+    assert np.all(s_t == s_t[0]) and s_t[0] == s_c[r] and np.all(s_c <= s_t[0])
+    assert np.array_equal(codes_t[r], codes_c[r])
+    # exhaustive nearest-code search on a sample of elements (fp64 distances; ties -> even code)
+    vals = t.astype(np.float64)
+    idx = rng.choice(wf.size, size=400, replace=False)
+    x = (wf.reshape(-1)[idx] / s_t[0]).astype(np.float32).astype(np.float64)
+    for xi, ci in zip(x, codes_t.reshape(-1)[idx]):
+        d = np.abs(vals - xi)
+        d[np.isnan(d)] = np.inf
+        best = np.flatnonzero(d == d.min())
+        assert ci in best and (len(best) == 1 or ci % 2 == 0 or vals[ci] == xi), (xi, ci, best)
+    z, sz = vo.quantize_weight(np.zeros((4, 16), dtype=np.uint16), per_tensor=True)
+    assert np.all(sz == 1.0) and np.all(z == 0)
