@@ -216,7 +216,7 @@ __device__ __forceinline__ void quantize_row(int m, int K, F val, const QuantOut
     unsigned clipped = 0;
     for (int i = threadIdx.x * 4; i < K; i += EW_THREADS * 4) {
         dst[i >> 2] = e4m3x4(div_rn(val(i), s), div_rn(val(i + 1), s), div_rn(val(i + 2), s), div_rn(val(i + 3), s));
-        clipped += clip4(val(i), val(i + 1), val(i + 2), val(i + 3), thr);
+        if (q.clip_count) clipped += clip4(val(i), val(i + 1), val(i + 2), val(i + 3), thr);
     }
     clip_add(q, clipped);
 }
@@ -248,7 +248,7 @@ __device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int
         const int i4 = c0 + (int)threadIdx.x + k * nthr;
         if (i4 < c1) {
             dst[i4] = e4m3x4(div_rn(v[k].x, s), div_rn(v[k].y, s), div_rn(v[k].z, s), div_rn(v[k].w, s));
-            clipped += clip4(v[k].x, v[k].y, v[k].z, v[k].w, thr);
+            if (q.clip_count) clipped += clip4(v[k].x, v[k].y, v[k].z, v[k].w, thr);
         }
     }
     clip_add(q, clipped);
@@ -438,7 +438,7 @@ __global__ void __launch_bounds__(SWI_THREADS) swiglu_quant_smem_kernel(LinOut g
     for (int i4 = threadIdx.x; i4 < n4; i4 += SWI_THREADS) {
         const float4 t = swi_row[i4];   // written by this same thread
         dst[i4] = e4m3x4(div_rn(t.x, s), div_rn(t.y, s), div_rn(t.z, s), div_rn(t.w, s));
-        clipped += clip4(t.x, t.y, t.z, t.w, thr);
+        if (q.clip_count) clipped += clip4(t.x, t.y, t.z, t.w, thr);
     }
     clip_add(q, clipped);
     trace_exit(pf);
