@@ -393,3 +393,43 @@ def test_static_scales_clip_counters_match_oracle():
     assert int(got[0]) == int(want[0])
     assert np.all(np.abs(got.astype(np.int64) - want) <= 2 + want // 100), (got, want)
     assert gm.ev_model_get_clip_counts().sum() == 0  # reset worked
+
+
+def test_edge_contexts_empty_tile_boundaries_and_max_tree(setup):
+    """Degenerate and boundary shapes of the attention / KV path: an EMPTY context (L = 0: only tree keys), contexts one
+    below / exactly on / one above the 64-key tile and 16-token page boundaries, and the largest tree the ABI takes
+    (T = EV_MAX_TREE_NODES = 64: every bit of the 64-bit ancestor masks in use, a random topology)."""
+    from gpu_helpers import import_oracle_kv, run_verify
+    spec, gm, om, ev = setup
+    V = spec.model.vocab
+    rng = np.random.default_rng(23)
+    T = 64
+    parents = np.array([-1] + [int(rng.integers(0, i)) for i in range(1, T)], dtype=np.int32)   # random tree, node 63 used
+    ctxs = [0, 63, 64, 129]
+    cache = ev.Cache(gm, 80, 4)
+    slots, ocs = [], []
+    toks = rng.integers(0, V, (4, T)).astype(np.int32)
+    for b, L in enumerate(ctxs):
+        oc = fresh_cache(om, 256)
+        if L:
+            vo.prefill(om, oc, 0, rng.integers(0, V, L).astype(np.int32))
+        slot = cache.ev_cache_add_seq(L + T)
+        if L:
+            import_oracle_kv(cache, slot, oc, 0, L, spec.model.n_layers)
+        slots.append(slot)
+        ocs.append(oc)
+    buf = run_verify(gm, cache, slots, toks, np.tile(parents, (4, 1)), commit=True)
+    assert buf.status.cpu().tolist() == [0, 0, 0, 0]
+    hid = buf.hidden.cpu().numpy().reshape(3, 4, T, -1)
+    lg = buf.logits.cpu().numpy().reshape(4, T, -1)
+    for b, L in enumerate(ctxs):
+        res = vo.verify(om, ocs[b], 0, toks[b], parents, commit=True, want_hidden=True)
+        for l in range(3):
+            assert rel_l2(hid[l, b], res["hidden"][l]) <= TOL_HIDDEN, (L, l)
+        assert np.max(np.abs(lg[b] - res["logits"])) <= TOL_LOGIT_SIGMA * res["logits"].std(), L
+        srt = np.sort(res["logits"], axis=1)
+        if ((srt[:, -1] - srt[:, -2]) >= GAP).all():
+            a = res["accept_len"]
+            assert buf.accept_len.cpu().numpy()[b] == a
+            assert buf.accept_nodes.cpu().numpy()[b, :a + 1].tolist() == res["path"]
+            assert cache.ev_cache_get_len(slots[b]) == L + a + 1
