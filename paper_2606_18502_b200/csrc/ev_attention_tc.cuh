@@ -6,7 +6,7 @@
 // Data flow per 64-key tile j (a CTA walks its key range tile by tile):
 //   TMA warp      : 4 pages x {K,V} boxes, each a whole (page, K|V, head) block of 16 tokens x D -> 128-byte-swizzled
 //                   smem as [page][8-token group][d half][8 x 128 B] (read in place through one 4-D tensor map)
-//   MMA thread    : S[j&1]  = Q . K_j^T   (tcgen05.mma kind::f16, A = Q from smem, B = K tile, D in TMEM)
+//   MMA thread    : S[j&1]  = Q . K_j^T   (tcgen05.mma kind::f16, A = Q from TMEM, B = K tile, D in TMEM)
 //                   Oc      = P[j&1] . V_j (A = P from TMEM, B = V tile MN-major, D in TMEM, from zero)
 //   8 softmax warps (thread = one query row x half of the tile's keys):
 //                   S -> registers (tcgen05.ld), tree mask, online max (the two halves of a row meet in shared
@@ -37,8 +37,8 @@ namespace ev {
 
 constexpr int TCA_THREADS = 576;  // warp 0 TMA producer, warp 1 MMA issuer, warps 2..9 softmax, warps 10..17 correction
 constexpr int TCA_BN = 64;        // keys per tile (= ATT_CH: the split plan is shared with the legacy kernel)
-constexpr int TCA_KS = 5;        // K ring depth (a K tile is released by Q.K^T, early)
-constexpr int TCA_VS = 4;        // V ring depth (a V tile is released by P.V)
+constexpr int TCA_KS = 6;        // K ring depth (a K tile is released by Q.K^T, early)
+constexpr int TCA_VS = 5;        // V ring depth (a V tile is released by P.V)
 constexpr int TCA_PAGE = 16;      // tokens per page this kernel is built for
 
 template <int D>
@@ -52,20 +52,22 @@ struct TcaCfg {
     static constexpr int PAGE_BYTES = 2 * SBO;          // one 16-token (page, K|V, head) block
     static constexpr int BAR_BYTES = 256;
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
-    static constexpr int SMEM = 1024 + Q_BYTES + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;
+    static constexpr int SMEM = 1024 + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;   // Q lives in TMEM
     // TMEM columns
-    // S[3] and P[3] share three 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
-    // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that).  THREE
-    // regions: Q.K^T(j+2) is issued before P.V(j), so S(j+1) is long finished when the softmax warps get to it (with
-    // two regions Q.K^T(j+1) could only follow P.V(j-1): every tile paid a softmax -> MMA -> softmax round trip,
-    // 1,750 cycles per tile against 1,280 of tensor work).  TWO O chunks, so P.V of tile j+1 does not wait for the
-    // correction warps to read chunk j.
-    static constexpr int NSP = 3;
+    // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
+    // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that).  (Three
+    // regions with Q.K^T two tiles ahead measured the same: the tensor pipe, not the S hand-off, set the period.)
+    // TWO O chunks, so P.V of tile j+1 does not wait for the correction warps to read chunk j.  The Q tile (hi | lo
+    // fp16 parts, D/2 columns of pairs each) sits in TMEM too and is the A operand of Q.K^T straight from there:
+    // from shared memory every N = 64 MMA read 4 KiB of Q + 2 KiB of K, 48 cycles against 32 of math.
+    static constexpr int NSP = 2;
+    static constexpr int NO = 2;            // O chunks in TMEM
     static constexpr int TS = 0;
     static constexpr int TP = 0;
     static constexpr int SP = 64;           // columns per S/P region
     static constexpr int TO = NSP * SP;     // O chunks: 2 x D fp32 columns
-    static_assert(TO + 2 * D <= 512, "TMEM budget");
+    static constexpr int TQ = TO + NO * D;  // Q: 2 parts x D/2 columns
+    static_assert(TQ + D <= 512, "TMEM budget");
     static constexpr int DH = D / 2;        // output columns per softmax warpgroup
 };
 
@@ -157,8 +159,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const AttnArgs& a = ta.a;
     extern __shared__ uint8_t tca_smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tca_smem_raw) + 1023) & ~(uintptr_t)1023);
-    uint8_t* q_s = smem;                                  // [2 parts][NH][128 rows][128 B]
-    uint8_t* kv_s = smem + C::Q_BYTES;                    // K ring [KS][NH x 8 KiB] | V ring [VS][NH x 8 KiB]
+    uint8_t* kv_s = smem;                                 // K ring [KS][NH x 8 KiB] | V ring [VS][NH x 8 KiB]
     uint64_t* bars = reinterpret_cast<uint64_t*>(kv_s + (TCA_KS + TCA_VS) * C::K_BYTES);
     uint64_t* k_full = bars;                              // [KS]
     uint64_t* k_empty = k_full + TCA_KS;                  // [KS]
@@ -215,37 +216,38 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const bool active = nn != 0 && k_begin < n_keys;   // uniform over the CTA
     const int k_end = min(k_begin + a.split_len, n_keys);
     const int n_tiles = active ? (k_end - k_begin + TCA_BN - 1) / TCA_BN : 0;
-    // ---- Q tile (fp32 x 2^6 -> hi | lo fp16, 128-byte swizzled K-major) ----
-    // Warps 1..17 stage Q and meet behind named barrier 5; warp 0 goes straight to its K/V loads, which then run
-    // under the Q staging instead of after it (the staging is ~1.5 us of a 15 us launch at batch 1).
-    if (active && warp != 0)
-    {
-        constexpr int CPR = D / 8;  // 16-byte chunks (8 elements) per row
-        for (int it = threadIdx.x - 32; it < 128 * CPR; it += TCA_THREADS - 32) {
-            const int r = it / CPR, c = it % CPR;
-            const int row = rg * 128 + r;
-            const int node = row / a.G, gi = row % a.G;
-            float x[8];
-            if (row < R && node < nn) {
-                const float* qp = a.q + (size_t)(b * a.T + node) * a.q_ld + (size_t)(kvh * a.G + gi) * D + c * 8;
-                const float4 u0 = *reinterpret_cast<const float4*>(qp), u1 = *reinterpret_cast<const float4*>(qp + 4);
-                x[0] = u0.x; x[1] = u0.y; x[2] = u0.z; x[3] = u0.w; x[4] = u1.x; x[5] = u1.y; x[6] = u1.z; x[7] = u1.w;
-            } else {
+    // ---- Q tile -> TMEM (fp32 x 2^6 -> hi | lo fp16 pairs).  Softmax and correction threads stage it: a warp owns the
+    // TMEM lanes of its 32 rows.  Warps 1..17 meet behind named barrier 5; warp 0 goes straight to its K/V
+    // loads, which run under the staging (~1.5 us of a 15 us launch at batch 1). ----
+    if (active && warp >= 2) {
+        // softmax AND correction warps: thread = (row, quarter of d); every load is issued before the first split
+        const int qd = (warp - 2) >> 2;   // 0..3
+        const int r = (warp & 3) * 32 + lane;
+        const int row = rg * 128 + r;
+        const int node = row / a.G, gi = row % a.G;
+        const bool valid = row < R && node < nn;
+        const float* qp = a.q + (size_t)(b * a.T + (valid ? node : 0)) * a.q_ld + (size_t)(kvh * a.G + (valid ? gi : 0)) * D + qd * (D / 4);
+        const uint32_t q_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + C::TQ + qd * (D / 8);
+        float4 u[D / 16];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) x[i] = 0.f;
+        for (int i = 0; i < D / 16; ++i) u[i] = valid ? *reinterpret_cast<const float4*>(qp + i * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int g = 0; g < D / 64; ++g) {   // 16 elements = 8 columns of pairs per group
+            uint32_t h[8], l[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                split2_pack(u[4 * g + i].x * TCA_QSCALE, u[4 * g + i].y * TCA_QSCALE, h[2 * i], l[2 * i]);
+                split2_pack(u[4 * g + i].z * TCA_QSCALE, u[4 * g + i].w * TCA_QSCALE, h[2 * i + 1], l[2 * i + 1]);
             }
-            uint32_t h[4], l[4];
-#pragma unroll
-            for (int i = 0; i < 4; ++i) split2_pack(x[2 * i] * TCA_QSCALE, x[2 * i + 1] * TCA_QSCALE, h[i], l[i]);
-            const int half = c >> 3, cc = c & 7;
-            const int off = half * (128 * 128) + r * 128 + ((cc ^ (r & 7)) << 4);
-            *reinterpret_cast<uint4*>(q_s + off) = make_uint4(h[0], h[1], h[2], h[3]);
-            *reinterpret_cast<uint4*>(q_s + C::Q_PART + off) = make_uint4(l[0], l[1], l[2], l[3]);
+            tmem_st8(q_addr + g * 8, h);
+            tmem_st8(q_addr + D / 2 + g * 8, l);
         }
+        tmem_st_wait();
+        tc_fence_before();
     }
     if (warp != 0) {
-        fence_proxy_async();   // generic-proxy smem writes (Q) -> visible to the tensor core's async proxy
         asm volatile("bar.sync 5, %0;" ::"n"(TCA_THREADS - 32) : "memory");
+        tc_fence_after();
     }
 
     if (!active) {
@@ -256,8 +258,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;
         const int kv = lane >> 2, pg = lane & 3;
         // K and V tiles travel in separate rings: a K tile is released as soon as Q.K^T of its tile has run, a V
-        // tile only after P.V, one tile later; the K stream runs one tile ahead of the V stream.  Page ids are
-        // looked up one iteration ahead (off the critical path).  An L2 look-ahead (cp.async.bulk.prefetch.tensor
+        // tile only after P.V.  Page ids are looked up one iteration ahead (off the critical path).  An L2 look-ahead (cp.async.bulk.prefetch.tensor
         // of tile j + 8) was tried and removed: the extra boxes go through the same TMA unit as the loads and made
         // IT the bottleneck (profiles/r1_attention_v2.md); for the same reason a block is ONE box, not one per half.
         auto box_row = [&](int j) {
@@ -265,31 +266,25 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             return (ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE) >> 3;   // 8-row group index
         };
         const bool ld_on = !(ta.dbg & 1);
-        // lanes [0, OPS/2) carry K boxes of tile jk, lanes [OPS/2, OPS) V boxes of tile jv = jk - 1
+        // Lanes 0..3 stream the K tiles, lanes 4..7 the V tiles, as two INDEPENDENT loops (divergent lanes of one warp):
+        // each stream runs as far ahead as its own ring allows.  In one common loop a full V ring (V tiles are
+        // released by P.V, two tiles behind Q.K^T) also held back the K loads, and the MMA warp waited ~420 cycles per
+        // tile for K.  The lane that owns page 0 arms the tile's full barrier (arrive + expected bytes); a box of
+        // another lane may complete first - the phase still cannot complete before that arrive.
         const int dst_off = pg * C::PAGE_BYTES;
-        int row_next = (lane < OPS) ? box_row(0) : 0;    // K lanes: tile 0; V lanes: tile 0 (used one iteration later)
-        int row_cur = row_next;
-        for (int it = 0; it <= n_tiles; ++it) {
-            const int jk = it, jv = it - 1;
-            const int jmine = kv ? jv : jk;
-            if (lane < OPS) {
-                row_cur = row_next;
-                if (jmine + 1 < n_tiles) row_next = box_row(jmine + 1);
-            }
-            if (jk < n_tiles) {
-                const int sk = jk % TCA_KS;
-                mbar_wait(&k_empty[sk], ((jk / TCA_KS) & 1) ^ 1);
-                if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&k_full[sk], C::K_BYTES); else mbar_arrive(&k_full[sk]); }
-                __syncwarp();
-                if (lane < OPS / 2 && ld_on) tma_load_4d(kv_s + sk * C::K_BYTES + dst_off, &tmKV, &k_full[sk], 0, 0, 0, row_cur);
-            }
-            if (jv >= 0) {
-                const int sv = jv % TCA_VS;
-                mbar_wait(&v_empty[sv], ((jv / TCA_VS) & 1) ^ 1);
-                if (lane == 0) { if (ld_on) mbar_arrive_expect_tx(&v_full[sv], C::K_BYTES); else mbar_arrive(&v_full[sv]); }
-                __syncwarp();
-                if (lane >= OPS / 2 && lane < OPS && ld_on)
-                    tma_load_4d(kv_s + (TCA_KS + sv) * C::K_BYTES + dst_off, &tmKV, &v_full[sv], 0, 0, 0, row_cur);
+        if (lane < OPS) {
+            uint64_t* full = kv ? v_full : k_full;
+            uint64_t* empty = kv ? v_empty : k_empty;
+            const int depth = kv ? TCA_VS : TCA_KS;
+            uint8_t* ring = kv_s + (kv ? TCA_KS * C::K_BYTES : 0);
+            int row_next = box_row(0);
+            for (int j = 0; j < n_tiles; ++j) {
+                const int row_cur = row_next;
+                if (j + 1 < n_tiles) row_next = box_row(j + 1);
+                const int sl = j % depth;
+                mbar_wait(&empty[sl], ((j / depth) & 1) ^ 1);
+                if (pg == 0) { if (ld_on) mbar_arrive_expect_tx(&full[sl], C::K_BYTES); else mbar_arrive(&full[sl]); }
+                if (ld_on) tma_load_4d(ring + sl * C::K_BYTES + dst_off, &tmKV, &full[sl], 0, 0, 0, row_cur);
             }
         }
     } else if (warp == 1) {
@@ -301,7 +296,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         constexpr uint32_t idesc_pv = umma_idesc_f16(128, D, 1);
         const bool leader = elect_one();
         const bool do_mma = !(ta.dbg & 2);
-        const uint32_t q_addr = smem_u32(q_s);
+        const uint32_t q_tmem = tmem_base + C::TQ;
         const uint32_t kv_addr = smem_u32(kv_s);
         const bool mts = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;
         long long mt_p = 0, mt_o = 0, mt_kv = 0;
@@ -311,11 +306,11 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const long long t0_ = mts ? clock64() : 0;
             mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
             const long long t1_ = mts ? clock64() : 0;
-            mbar_wait(&o_empty[i & 1], ((i >> 1) & 1) ^ 1);   // the correction warps have read chunk i - 2
+            mbar_wait(&o_empty[i % C::NO], ((i / C::NO) & 1) ^ 1);   // the correction warps have read chunk i - NO
             if (mts) { const long long t2_ = clock64(); mt_p += t1_ - t0_; mt_o += t2_ - t1_; }
             tc_fence_after();
             const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
-            const uint32_t d_addr = tmem_base + C::TO + (i & 1) * D;
+            const uint32_t d_addr = tmem_base + C::TO + (i % C::NO) * D;
             const uint32_t p_addr = tmem_base + C::TP + (i % C::NSP) * C::SP;
             if (leader && do_mma) {
 #pragma unroll
@@ -328,7 +323,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             }
             if (leader) {
                 umma_commit(&v_empty[s]);
-                umma_commit(&o_full[i & 1]);
+                umma_commit(&o_full[i % C::NO]);
             }
             __syncwarp();
         };
@@ -345,11 +340,11 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 for (int part = 1; part >= 0; --part) {
 #pragma unroll
                     for (int h = 0; h < C::NH; ++h) {
-                        const uint64_t adesc = umma_desc_k128(q_addr + part * C::Q_PART + h * (128 * 128));
                         const uint64_t bdesc = umma_desc_k128(k_addr + h * 1024, C::SBO);
 #pragma unroll
-                        for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 elements = 32 B
-                            umma_bf16_ss(s_addr, adesc + 2 * ks, bdesc + 2 * ks, idesc_qk, (part == 1 && h == 0 && ks == 0) ? 0u : 1u);
+                        for (int ks = 0; ks < 4; ++ks)  // UMMA K = 16 elements: 8 TMEM columns of Q pairs, 32 B of a K row
+                            umma_bf16_ts(s_addr, q_tmem + part * (D / 2) + (h * 4 + ks) * 8, bdesc + 2 * ks, idesc_qk,
+                                         (part == 1 && h == 0 && ks == 0) ? 0u : 1u);
                     }
                 }
             }
@@ -359,12 +354,12 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             }
             __syncwarp();
         };
-        // Q.K^T runs two tiles ahead of P.V: S(j+2) goes into the region P(j-1) was read from by P.V(j-1), issued one
-        // iteration earlier (the tensor pipe executes in issue order)
-        issue_qk(0);
-        if (n_tiles > 1) issue_qk(1);
+        // Q.K^T runs NSP - 1 tiles ahead of P.V: S(j + NSP - 1) goes into the region P(j-1) was read from by P.V(j-1),
+        // issued one iteration earlier (the tensor pipe executes in issue order)
+        constexpr int LA = C::NSP - 1;   // S/P regions - 1 tiles of look-ahead
+        for (int j = 0; j < min(LA, n_tiles); ++j) issue_qk(j);
         for (int j = 0; j < n_tiles; ++j) {
-            if (j + 2 < n_tiles) issue_qk(j + 2);
+            if (j + LA < n_tiles) issue_qk(j + LA);
             issue_pv(j);
         }
         if (mts && leader) { a.ts[14] = (unsigned long long)mt_p; a.ts[15] = (unsigned long long)(mt_kv + (mt_o << 32)); }
@@ -484,12 +479,12 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
 #pragma unroll
         for (int i = 0; i < C::DH; ++i) o[i] = 0.f;
         for (int i = 0; i < n_tiles; ++i) {
-            mbar_wait(&o_full[i & 1], (i >> 1) & 1);
+            mbar_wait(&o_full[i % C::NO], (i / C::NO) & 1);
             tc_fence_after();
             if (!warp_valid) {   // no live row in this warp: release the chunk, nothing to add
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&o_empty[i & 1]);
+                if (lane == 0) mbar_arrive(&o_empty[i % C::NO]);
                 continue;
             }
             const float c = xc[(i & 7) * 128 + r];
@@ -497,7 +492,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             for (int cb = 0; cb < C::DH / 16; ++cb) {
                 uint32_t ov[16];
                 if (!(ta.dbg & 4)) {
-                    tmem_ld16(lane_addr + C::TO + (i & 1) * D + hh * C::DH + cb * 16, ov);
+                    tmem_ld16(lane_addr + C::TO + (i % C::NO) * D + hh * C::DH + cb * 16, ov);
                     tmem_ld_wait();
                 } else {
 #pragma unroll
@@ -506,7 +501,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 if (cb == C::DH / 16 - 1) {
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&o_empty[i & 1]);
+                    if (lane == 0) mbar_arrive(&o_empty[i % C::NO]);
                 }
 #pragma unroll
                 for (int e = 0; e < 16; ++e) o[cb * 16 + e] = fmaf(o[cb * 16 + e], c, __uint_as_float(ov[e]));
