@@ -74,6 +74,10 @@ typedef struct {
     int weight_scale_mode; /* 0 = one E4M3 scale per output channel (BASELINE.json:north_star); 1 = one scale per
                             * weight matrix, absmax / 448 over the whole matrix ("per-tensor";
                             * SURVEY section 8(f)-1; each of Q, K, V, gate, up keeps its own scale) */
+    int attn_chunk;        /* keys per attention chunk: 0 = default (1024), else a multiple of 64.  A node's key set is reduced in
+                            * chunks aligned to ABSOLUTE key positions plus a short tail, so its
+                            * result does not depend on batch, tree or GPU; the chunk length is part of the model's arithmetic:
+                            * two models with different attn_chunk agree only to fp32 rounding */
 } ev_config;
 
 typedef enum {

@@ -25,7 +25,8 @@ class ev_config(C.Structure):
     _fields_ = [("n_layers", C.c_int), ("hidden", C.c_int), ("n_q_heads", C.c_int), ("n_kv_heads", C.c_int),
                 ("head_dim", C.c_int), ("ffn", C.c_int), ("vocab", C.c_int), ("rms_eps", C.c_float),
                 ("rope_theta", C.c_float), ("page_size", C.c_int), ("act_scale_mode", C.c_int),
-                ("max_batch", C.c_int), ("max_tree_nodes", C.c_int), ("max_ctx", C.c_int), ("weight_scale_mode", C.c_int)]
+                ("max_batch", C.c_int), ("max_tree_nodes", C.c_int), ("max_ctx", C.c_int), ("weight_scale_mode", C.c_int),
+                ("attn_chunk", C.c_int)]
 
 
 class ev_verify_in(C.Structure):
@@ -121,11 +122,12 @@ def ev_launch_count(reset=False):
 class Model:
     """ev_model handle."""
 
-    def __init__(self, shape, max_batch, max_tree_nodes, max_ctx, page_size=16, act_scale_mode=0, weight_scale_mode=0):
+    def __init__(self, shape, max_batch, max_tree_nodes, max_ctx, page_size=16, act_scale_mode=0, weight_scale_mode=0,
+                 attn_chunk=0):
         self.lib = load_library()
         self.cfg = ev_config(shape.n_layers, shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim,
                              shape.ffn, shape.vocab, shape.rms_eps, shape.rope_theta, page_size, act_scale_mode,
-                             max_batch, max_tree_nodes, max_ctx, weight_scale_mode)
+                             max_batch, max_tree_nodes, max_ctx, weight_scale_mode, attn_chunk)
         self.shape = shape
         h = C.c_void_p()
         _check(self.lib.ev_model_create(C.byref(self.cfg), C.byref(h)))

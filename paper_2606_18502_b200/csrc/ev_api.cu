@@ -154,16 +154,16 @@ struct ev_model {
     float* attn = nullptr;
     float* o_part = nullptr;
     float* ml_part = nullptr;
-    long split_rows_budget = 0;
     float* lin_out = nullptr;   // raw GEMM output [splits][M][N], consumed by the next element-wise kernel
     long lin_floats = 0;
-    unsigned long long* dbg_ts = nullptr;
     unsigned long long* trace = nullptr;   // EV_TRACE=1: [TRACE_CAP][4] step trace, see ev_profile_trace
     int n_traced = 0;
     // tree state
     int32_t *attn_order = nullptr;
     int32_t *Lsnap = nullptr, *nn_eff = nullptr, *depth = nullptr, *pos = nullptr;
-    unsigned long long *anc = nullptr, *argmax_keys = nullptr;
+    unsigned long long *anc = nullptr, *anc_bulk = nullptr, *argmax_keys = nullptr;
+    int32_t *erow = nullptr, *kend_row = nullptr, *kend_seq = nullptr;   // bulk / tail cut of every row's key set (tree_prep_kernel)
+    int attn_chunk = 1024, n_chunks_max = 1;   // keys per attention chunk (cfg.attn_chunk); chunk columns the partial workspace holds
     // static activation scales
     int n_sites = 0;
     float* static_scales = nullptr;  // device [n_sites]
@@ -172,14 +172,10 @@ struct ev_model {
     unsigned long long* clip_counts = nullptr;  // device [n_sites]: elements clipped by the static scales since the last reset
     bool calibrated = false, recording = false;
     int num_sms = 148;
-    bool use_splitk = false, naive_gemm = false, legacy_attn = false;
-    int attn_dbg = 0;
+    int cut_pairs = 74;   // pieces of the canonical K cuts of every layer matrix (ev_gemm.cuh): a constant of the library, NOT the
+                          // SM count of the device, so results do not change with the GPU the model runs on (148 SMs = 74 pairs)
     int row_cluster = 0;  // EV_ROW_CLUSTER override (bring-up)
     bool profile = false;
-    int gemm_dbg = 0, gemm_stages = 0;
-    bool gemm_bal = true, gemm_bal_all = false;  // balanced partition of the many-row LM head (EV_GEMM_BAL=0: never, 2: every GEMM)
-    int attn_splits = 0;   // EV_ATTN_SPLITS: key splits per (sequence, head, row group); 0 = one wave of CTAs
-    bool gemm_mc = true;   // CTA pairs (tcgen05 cta_group::2) for the many-row GEMMs (EV_GEMM_MC=0 turns them off)
     // L2 weight stream (PfPlanner): on for token counts <= l2pf_max_m; bytes the stream may run ahead / per launch
     int l2pf_max_m = 0;
     long l2pf_cap = 88L << 20, l2pf_maxq = 40L << 20;
@@ -192,6 +188,7 @@ struct ev_model {
     std::vector<GraphEntry> graphs;
     unsigned long graph_clock = 0;
     std::vector<void*> allocs;
+    std::vector<ev_cache*> caches;   // caches created on this model (their model pointer is cleared if the model dies first)
 };
 
 struct ev_cache {
@@ -261,7 +258,7 @@ int alloc_actbuf(ev_model* m, ActBuf* b, long K) {
 int alloc_qmat(ev_model* m, QMat* q, long N, long K) {
     q->N = N;
     q->K = K;
-    q->n_tiles = (int)((N + GEMM_WROWS - 1) / GEMM_WROWS);
+    q->n_tiles = (int)round_up((N + GEMM_WROWS - 1) / GEMM_WROWS, 2);   // whole PAIRS of 128-channel tiles (canonical K cuts, CTA pairs)
     q->total_kb = (int)((K + GEMM_BK - 1) / GEMM_BK);
     const size_t bytes = (size_t)q->n_tiles * q->total_kb * GEMM_WTILE;
     EV_TRY(dev_alloc(m, &q->codes, bytes));
@@ -359,7 +356,7 @@ int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const CUtensorMap& tmXh
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(GEMM_THREADS);
+    cfg.blockDim = dim3(gemm_threads<EPI, PAIR>());
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute at[2];
@@ -455,8 +452,12 @@ struct PfPlanner {
     }
 };
 
-// one W8A8 linear.  epi == EPI_RAW: raw accumulators go to m->lin_out as [splits][M][N]; *lin describes them for
+// one W8A8 linear.  epi == EPI_RAW: raw accumulators go to m->lin_out as [slabs][M][N]; *lin describes them for
 // the consumer kernel.  epi == EPI_ARGMAX (LM head): scales applied, argmax keys updated, optional logits.
+// Two forms (ev_gemm.cuh), both cutting K at the matrix's canonical cuts (cut_G = m->cut_pairs pieces over the
+// flattened (pair tile, K-block) space), so a token's result does not depend on how many tokens share the launch:
+//   M <= 256 (one token tile): stream-K over CTA pairs of single CTAs, piece c = work of pair c, slabs added by the consumer;
+//   M  > 256: cta_group::2 pairs own whole (pair tile, token tile) items, running fp32 sum over the pieces in the epilogue.
 int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int M, int epi, LinOut* lin, float* logits,
                unsigned long long* keys, int prof_cls, PfPlanner* pfp = nullptr, const void* warm1 = nullptr, int warm1_bytes = 0) {
     ProfScope prof_scope(m, st, prof_cls);
@@ -464,30 +465,22 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
         lin->p = m->lin_out; lin->splits = 1; lin->ld = (int)w.N; lin->split_stride = (long)M * w.N;
         lin->sx = x.scale; lin->sw = w.scale; lin->sk_G = lin->sk_U = lin->sk_kb = 0;
     }
-    if (m->naive_gemm && epi == EPI_RAW) {
-        dim3 grid((unsigned)((w.N + 127) / 128), M);
-        gemm_e4m3_naive_kernel<<<grid, 128, 0, st>>>(x.codes, w.codes, M, (int)w.N, (int)w.K, w.total_kb, m->lin_out, (int)w.N);
-        LAUNCH_CHECK();
-        return EV_OK;
-    }
     GemmArgs a;
-    a.M = M; a.N = (int)w.N; a.total_kb = w.total_kb; a.n_tiles = w.n_tiles;
+    a.M = M; a.N = (int)w.N; a.total_kb = w.total_kb; a.n_tiles = w.n_tiles;   // n_tiles is even (alloc_qmat)
     a.m_tiles = (M + 255) / 256;
     a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
+    const bool pair = a.m_tiles >= 2;   // cta_group::2 kernel
     // balanced partition (ev_gemm.cuh, GemmArgs::bal): several token tiles -> items of up to 256 tokens cut from an even deal.
     // Used for the LM head (1002 n tiles: 27 items per CTA pair, 588 -> 548 us at M = 832).  The layer GEMMs have 1-6
     // items per pair; there the extra partial items (a 32-token item costs as much W traffic as a 208-token one)
-    // outweigh the partial last wave: O 26 -> 33 us, down 54 -> 82 us, gate|up 98 -> 104 us (EV_GEMM_BAL=2 forces it).
-    a.bal = (m->gemm_bal && a.m_tiles >= 2 && (epi == EPI_ARGMAX || m->gemm_bal_all)) ? 1 : 0;
+    // outweigh the partial last wave: O 26 -> 33 us, down 54 -> 82 us, gate|up 98 -> 104 us.
+    a.bal = (pair && epi == EPI_ARGMAX) ? 1 : 0;
     a.bal_blocks = (M + 15) / 16;
     a.tms = x.tms_dev;
     if (a.bal) a.tok = 256;   // the largest item: sizes the stages and the two accumulators
-    // CTA pairs (ev_gemm.cuh): several token tiles and an even number of 128-channel tiles
-    a.mc = (m->gemm_mc && a.m_tiles >= 2 && a.n_tiles % 2 == 0) ? 1 : 0;
-    const int stage_bytes = GEMM_WTILE + (a.mc ? a.tok / 2 : a.tok) * GEMM_BK;
+    const int stage_bytes = GEMM_WTILE + (pair ? a.tok / 2 : a.tok) * GEMM_BK;
     a.stages = std::min(GEMM_MAX_STAGES, GEMM_SMEM_BUDGET / stage_bytes);
     if (a.stages < 2) return fail(EV_EINVAL, "token tile too large");
-    if (m->gemm_stages > 0) a.stages = std::min(a.stages, m->gemm_stages);
     a.W = w.codes; a.sx = x.scale; a.sw = w.scale; a.argmax_keys = keys;
     a.out = (epi == EPI_RAW) ? m->lin_out : logits;
     a.ldo = (int)w.N;
@@ -495,42 +488,36 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     a.warm[0] = (epi == EPI_RAW) ? w.scale : nullptr; a.warm_bytes[0] = (epi == EPI_RAW) ? (int)(w.N * sizeof(float)) : 0;
     a.warm[1] = warm1; a.warm_bytes[1] = warm1 ? warm1_bytes : 0;
     if (pfp) a.pf = pfp->take(true);
-    a.dbg = m->gemm_dbg;
-    a.ts = (m->gemm_dbg & 16) ? m->dbg_ts : nullptr;
-    const int G = m->num_sms;
-    const int nmul = a.mc ? 2 : 1;                       // n tiles per scheduling unit
-    const int Gc = a.mc ? G / 2 : G;                     // CTAs, or CTA pairs
-    const int tiles = (a.n_tiles / nmul) * a.m_tiles;    // (n tile or pair of n tiles, token tile)
     a.k_splits = 1;
     a.kb_per_split = a.total_kb;
     a.sk_units = 0;
-    int grid = nmul * std::min(a.bal ? (a.n_tiles / nmul) * a.bal_blocks : tiles, Gc);
-    if (lin) { lin->splits = 1; lin->sk_G = 0; lin->sk_U = 0; lin->sk_kb = 0; }
-    // Stream-K (one token tile): the n_tiles * total_kb K-blocks are dealt out evenly to the CTAs (ev_gemm.cuh); each
-    // tile's pieces land in slabs the consumer adds in K order.  The partition depends only on the matrix shape and
-    // the SM count, never on M: a token's result is batch-invariant.  (Tried for several token tiles too, where
-    // whole tiles leave a partial last wave - 896 tiles on 148 CTAs: the GEMMs did not get faster and the consumers
-    // paid for the second slab: config[2] 17.2 -> 19.3 ms; the kernel keeps the generality, the plan does not use it.)
-    if (m->use_splitk && epi == EPI_RAW) {
-        const int U = tiles * a.total_kb;
-        const int g = std::min(Gc, U);
-        const bool worth = a.m_tiles == 1;
-        int pmax = 1;
-        for (int t = 0; t < tiles && worth; ++t)
-            pmax = std::max(pmax, sk_first_cta((t + 1) * a.total_kb - 1, g, U) - sk_first_cta(t * a.total_kb, g, U) + 1);
-        if (worth && pmax <= 8 && (long)pmax * M * a.N <= m->lin_floats) {
-            a.sk_units = U;
-            grid = nmul * g;
-            if (lin) {
-                lin->splits = pmax; lin->sk_G = g; lin->sk_U = U; lin->sk_kb = a.total_kb;
-            }
-        }
+    a.cut_G = a.cut_U = 0;
+    const int n_pairs = a.n_tiles / 2;
+    const int U = n_pairs * a.total_kb;             // K-block units of the (pair tile, K-block) space
+    const int cutG = std::min(std::min(m->cut_pairs, U), 7 * n_pairs);   // canonical pieces: matrix shape and a model constant only; <= 8 pieces per tile
+    int pmax = 1;                                   // most pieces any pair tile is cut into
+    for (int t = 0; t < n_pairs; ++t)
+        pmax = std::max(pmax, sk_first_cta((t + 1) * a.total_kb - 1, cutG, U) - sk_first_cta(t * a.total_kb, cutG, U) + 1);
+    int grid;
+    if (epi == EPI_ARGMAX) {          // LM head: whole K per item, no cuts
+        a.mc = pair ? 1 : 0;
+        grid = pair ? 2 * std::min(n_pairs * a.bal_blocks, m->num_sms / 2) : std::min(a.n_tiles, m->num_sms);
+    } else if (!pair) {               // stream-K: piece c = CTAs 2c, 2c+1
+        if (pmax > 8 || (long)pmax * M * a.N > m->lin_floats) return fail(EV_EINVAL, "K cuts: more than 8 pieces per tile or slab workspace too small");
+        a.mc = 1;
+        a.sk_units = U;
+        grid = 2 * cutG;
+        if (lin) { lin->splits = pmax; lin->sk_G = cutG; lin->sk_U = U; lin->sk_kb = a.total_kb; }
+    } else {                          // CTA pairs, whole items, running sum over the same pieces
+        a.mc = 1;
+        a.cut_G = cutG; a.cut_U = U;
+        grid = 2 * std::min(n_pairs * a.m_tiles, m->num_sms / 2);
     }
     const int smem = a.stages * stage_bytes + 512 + 2048 + 8192 + 1024;  // stages + barriers + sx staging + argmax keys + alignment slack
     const CUtensorMap& tmX = x.tm[a.tok / 16 - 1];
     const CUtensorMap& tmXh = x.tmh[a.tok / 16 - 1];
-    if (epi == EPI_RAW) return a.mc ? launch_gemm<EPI_RAW, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_RAW, false>(st, tmX, tmXh, a, grid, smem);
-    return a.mc ? launch_gemm<EPI_ARGMAX, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_ARGMAX, false>(st, tmX, tmXh, a, grid, smem);
+    if (epi == EPI_RAW) return pair ? launch_gemm<EPI_RAW, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_RAW, false>(st, tmX, tmXh, a, grid, smem);
+    return pair ? launch_gemm<EPI_ARGMAX, true>(st, tmX, tmXh, a, grid, smem) : launch_gemm<EPI_ARGMAX, false>(st, tmX, tmXh, a, grid, smem);
 }
 
 QuantOut quant_out(ev_model* m, ActBuf& b, int site) {
@@ -570,36 +557,22 @@ int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
 }
 
 
-// key-split plan for attention: enough CTAs for one wave, bounded by the partial-output workspace.  The key
-// bound (host-side upper bound of ctx_len + T over the batch) is rounded up to 256 so that the plan - and with
-// it the captured graph - only changes when a sequence crosses such a boundary; the kernels read the true
-// lengths on the device and skip empty splits.  Also advances the host-side length bounds on commit.
+// Attention grid: n_chunks chunk columns of cfg.attn_chunk keys each (ev_attention.cuh).  The chunk length is a constant
+// of the model - which keys share a chunk never depends on the batch - so the plan only says how many chunk columns the
+// grid has: enough for the longest sequence the host knows of (len_bound, an upper bound of ctx_len; the kernels read the
+// true lengths on the device, CTAs of empty chunks leave at once, and tree_prep rejects a sequence the grid does not cover).
 AttnPlan plan_attention(ev_model* m, ev_cache* c, const ev_verify_in* in) {
-    const ev_config& cfg = m->cfg;
-    const int B = in->n_seqs, T = in->n_nodes_max, M = B * T;
-    const int R = T * (cfg.n_q_heads / cfg.n_kv_heads);
-    const int row_groups = (R + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
+    const int T = in->n_nodes_max;
     int max_keys = 0;
     for (int i = 0; i < c->max_seqs; ++i)
         if (c->seq_used[i]) max_keys = std::max(max_keys, c->len_bound[i]);
-    max_keys = (int)round_up(max_keys + T, 256);
-    if (in->commit)
+    max_keys += T;
+    if (in->commit)   // the host does not see which nodes are accepted: every sequence may grow by T (ev_verify_host and ev_cache_get_len tighten the bound)
         for (int i = 0; i < c->max_seqs; ++i)
-            if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * cfg.page_size);
+            if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * m->cfg.page_size);
     AttnPlan p;
-    const long base = (long)B * cfg.n_kv_heads * row_groups;
-    // one wave of CTAs, on ~90 % of the SMs: at config[1] (base = 16) 8 splits of 5 tiles on 112 SMs ran the attention
-    // in 18.8 us against 20.9 us for 9 splits of 4 tiles on 144 SMs (EV_ATTN_SPLITS sweep, 4..9): the SMs left free
-    // take the CTAs of the kernels launched behind it (programmatic dependent launch)
-    long want = std::max(1L, (long)(m->num_sms * 9 / 10) / base);
-    const long chunks = (max_keys + ATT_CH - 1) / ATT_CH;
-    want = std::max(1L, std::min(want, chunks));
-    want = std::min(want, std::max(1L, m->split_rows_budget / M));
-    if (m->attn_splits > 0) want = std::min<long>(m->attn_splits, chunks);   // EV_ATTN_SPLITS (bring-up sweep)
-    want = std::min(want, 64L);  // merge kernel's shared-memory table
-    p.n_splits = (int)want;
-    p.split_len = (int)round_up((max_keys + p.n_splits - 1) / p.n_splits, ATT_CH);
-    p.n_splits = (max_keys + p.split_len - 1) / p.split_len;
+    p.split_len = m->attn_chunk;
+    p.n_splits = std::min(m->n_chunks_max, std::max(1, (max_keys + p.split_len - 1) / p.split_len));
     return p;
 }
 
@@ -616,6 +589,8 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     tp.ctx_len = c->ctx_len; tp.capacity = c->capacity; tp.max_seqs = c->max_seqs; tp.max_pos = m->max_pos;
     tp.Lsnap = m->Lsnap; tp.nn_eff = m->nn_eff; tp.status = out->dev_status; tp.depth = m->depth; tp.pos = m->pos;
     tp.anc = m->anc; tp.argmax_keys = m->argmax_keys; tp.order = m->attn_order;
+    tp.anc_bulk = m->anc_bulk; tp.erow = m->erow; tp.kend_row = m->kend_row; tp.kend_seq = m->kend_seq;
+    tp.max_keys = plan.n_splits * plan.split_len;
     EV_TRY(launch_k(tree_prep_kernel, dim3((B + 63) / 64), dim3(64), 0, st, tp));
 
     const float* ovr = in->dev_hidden_override;
@@ -628,7 +603,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
 
     // L2 weight stream: the step's weight matrices in consumption order (PfPlanner)
     PfPlanner pfp;
-    pfp.on = M <= m->l2pf_max_m && !m->profile && !m->naive_gemm;
+    pfp.on = M <= m->l2pf_max_m && !m->profile;
     pfp.cap = (size_t)m->l2pf_cap; pfp.maxq = (size_t)m->l2pf_maxq;
     pfp.trace = m->trace; pfp.trace_cap = TRACE_CAP;
     pfp.mask = m->l2pf_mask; pfp.n_layer_launches = 10 * cfg.n_layers;
@@ -692,10 +667,9 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         aa.q = m->qkv; aa.q_ld = m->qkv_dim; aa.T = T; aa.G = cfg.n_q_heads / cfg.n_kv_heads; aa.Hq = cfg.n_q_heads;
         aa.Hkv = cfg.n_kv_heads; aa.pool = ra.pool; aa.page_table = c->page_table; aa.max_pages = c->max_pages;
         aa.page_size = cfg.page_size; aa.seq_slots = in->dev_seq_slots; aa.Lsnap = m->Lsnap; aa.nn_eff = m->nn_eff; aa.order = m->attn_order;
-        aa.anc = m->anc; aa.split_len = split_len; aa.n_splits = n_splits; aa.scale = 1.0f / sqrtf((float)D);
+        aa.anc_bulk = m->anc_bulk; aa.erow = m->erow; aa.kend_seq = m->kend_seq;
+        aa.chunk = split_len; aa.n_chunks = n_splits; aa.scale = 1.0f / sqrtf((float)D);
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
-        aa.ts = (m->gemm_dbg & 32) ? m->dbg_ts + 512 : nullptr;
-        if (aa.ts && l == 1) fprintf(stderr, "[attn] grid (%d,%d,%d) split_len %d\n", n_splits, cfg.n_kv_heads * row_groups, B, split_len);
         dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
@@ -704,21 +678,23 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                 ta.a = aa;
                 ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
                 ta.pf = pfp.take(false);
-                ta.dbg = m->attn_dbg;
                 if (D == 128) EV_TRY(launch_attn_tc<128>(st, c->tmKV, ta, agrid)); else EV_TRY(launch_attn_tc<64>(st, c->tmKV, ta, agrid));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
             }
         }
         MergeArgs ma;
-        ma.T = T; ma.Hq = cfg.n_q_heads; ma.D = D; ma.n_splits = n_splits; ma.split_len = split_len;
-        ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.o_part = m->o_part; ma.ml_part = m->ml_part;
+        ma.T = T; ma.Hq = cfg.n_q_heads; ma.Hkv = cfg.n_kv_heads; ma.D = D; ma.n_chunks = n_splits; ma.chunk = split_len;
+        ma.Lsnap = m->Lsnap; ma.nn_eff = m->nn_eff; ma.seq_slots = in->dev_seq_slots; ma.erow = m->erow; ma.kend_row = m->kend_row;
+        ma.anc = m->anc; ma.anc_bulk = m->anc_bulk; ma.o_part = m->o_part; ma.ml_part = m->ml_part;
+        ma.qkv = m->qkv; ma.q_ld = m->qkv_dim; ma.pool = ra.pool; ma.page_table = c->page_table; ma.max_pages = c->max_pages;
+        ma.page_size = cfg.page_size; ma.kv_f16 = c->kv_f16 ? 1 : 0; ma.scale = aa.scale;
         ma.attn = (tap && out->dev_tap_attn) ? out->dev_tap_attn : nullptr;
         ma.q = quant_out(m, m->aq, 4 * l + 1);
         ma.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
-            ROW_DISPATCH(rp_q, attn_merge_quant_kernel, dim3(M * rp_q.cl), dim3(MERGE_THREADS), (size_t)(2 * n_splits + 1) * cfg.n_q_heads * sizeof(float), st, ma);
+            ROW_DISPATCH(rp_q, attn_merge_quant_kernel, dim3(M * rp_q.cl), dim3(MERGE_THREADS), 0, st, ma);
         }
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
@@ -809,6 +785,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     if (cfg->max_batch < 1 || cfg->max_ctx < 1) return fail(EV_EINVAL, "max_batch / max_ctx must be positive");
     if (cfg->act_scale_mode != 0 && cfg->act_scale_mode != 1) return fail(EV_EINVAL, "act_scale_mode must be 0 or 1");
     if (cfg->weight_scale_mode != 0 && cfg->weight_scale_mode != 1) return fail(EV_EINVAL, "weight_scale_mode must be 0 or 1");
+    if (cfg->attn_chunk < 0 || cfg->attn_chunk % 64) return fail(EV_EINVAL, "attn_chunk must be 0 (default 1024) or a multiple of 64");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(EV_ECUDA, "no CUDA device");
     ev_model* m = new ev_model();
@@ -824,23 +801,15 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, dev);
-    m->use_splitk = !(getenv("EV_SPLITK") && atoi(getenv("EV_SPLITK")) == 0);  // on by default
-    m->gemm_dbg = getenv("EV_GEMM_DBG") ? atoi(getenv("EV_GEMM_DBG")) : 0;
-    m->gemm_stages = getenv("EV_GEMM_STAGES") ? atoi(getenv("EV_GEMM_STAGES")) : 0;
-    m->gemm_mc = !(getenv("EV_GEMM_MC") && atoi(getenv("EV_GEMM_MC")) == 0);
-    if (getenv("EV_ATTN_SPLITS")) m->attn_splits = atoi(getenv("EV_ATTN_SPLITS"));
-    m->gemm_bal = !(getenv("EV_GEMM_BAL") && atoi(getenv("EV_GEMM_BAL")) == 0);
-    m->gemm_bal_all = getenv("EV_GEMM_BAL") && atoi(getenv("EV_GEMM_BAL")) == 2;
+#ifdef EV_BRINGUP   // bring-up builds only (-DEV_BRINGUP): the shipped library reads no environment variable
     if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
     if (getenv("EV_L2PF_MASK")) m->l2pf_mask = (unsigned)strtoul(getenv("EV_L2PF_MASK"), nullptr, 0);
     if (getenv("EV_L2PF_CAP_MB")) m->l2pf_cap = (long)atoi(getenv("EV_L2PF_CAP_MB")) << 20;
     if (getenv("EV_L2PF_MAXQ_MB")) m->l2pf_maxq = (long)atoi(getenv("EV_L2PF_MAXQ_MB")) << 20;
-    m->naive_gemm = getenv("EV_NAIVE_GEMM") && atoi(getenv("EV_NAIVE_GEMM")) != 0;
     m->row_cluster = getenv("EV_ROW_CLUSTER") ? atoi(getenv("EV_ROW_CLUSTER")) : 0;
     m->use_graph = !(getenv("EV_GRAPH") && atoi(getenv("EV_GRAPH")) == 0);          // on by default
     g_use_pdl = !(getenv("EV_PDL") && atoi(getenv("EV_PDL")) == 0);                // on by default
-    m->attn_dbg = getenv("EV_ATTN_DBG") ? atoi(getenv("EV_ATTN_DBG")) : 0;
-    m->legacy_attn = getenv("EV_ATTN_LEGACY") && atoi(getenv("EV_ATTN_LEGACY")) != 0;  // bring-up: mma.sync attention
+#endif
     const long H = cfg->hidden, F = cfg->ffn, V = cfg->vocab;
     int rc = EV_OK;
     auto A = [&](int r) { if (rc == EV_OK) rc = r; };
@@ -858,16 +827,21 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(alloc_actbuf(m, &m->tq, F));
     A(dev_alloc(m, &m->qkv, (size_t)m->M_pad * m->qkv_dim));
     A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
-    m->split_rows_budget = std::max<long>(2L * m->M_cap, 4096);
-    A(dev_alloc(m, &m->o_part, (size_t)m->split_rows_budget * m->q_dim));
-    A(dev_alloc(m, &m->ml_part, (size_t)m->split_rows_budget * cfg->n_q_heads * 2));
+    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : 1024;
+    m->n_chunks_max = (cfg->max_ctx + m->attn_chunk - 1) / m->attn_chunk;
+    A(dev_alloc(m, &m->o_part, (size_t)m->M_cap * m->n_chunks_max * m->q_dim));
+    A(dev_alloc(m, &m->ml_part, (size_t)m->M_cap * m->n_chunks_max * cfg->n_q_heads * 2));
     {
         const long widest = std::max<long>(std::max<long>(2 * F, m->qkv_dim), H);
         m->lin_floats = std::max<long>((long)m->M_pad * widest, 8L * std::min(m->M_pad, 256) * widest);
     }
     A(dev_alloc(m, &m->lin_out, (size_t)m->lin_floats));
-    A(dev_alloc(m, &m->dbg_ts, (size_t)1024 * 8));
-    if (getenv("EV_TRACE") && atoi(getenv("EV_TRACE")) != 0) {
+#ifdef EV_BRINGUP
+    const bool want_trace = getenv("EV_TRACE") && atoi(getenv("EV_TRACE")) != 0;
+#else
+    const bool want_trace = false;
+#endif
+    if (want_trace) {
         A(dev_alloc(m, &m->trace, (size_t)TRACE_CAP * TRACE_SLOTS));
         cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8);
     }
@@ -877,6 +851,10 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->depth, (size_t)m->M_cap));
     A(dev_alloc(m, &m->pos, (size_t)m->M_cap));
     A(dev_alloc(m, &m->anc, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->anc_bulk, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->erow, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->kend_row, (size_t)m->M_cap));
+    A(dev_alloc(m, &m->kend_seq, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->argmax_keys, (size_t)m->M_cap));
     A(dev_alloc(m, &m->static_scales, (size_t)m->n_sites));
     A(dev_alloc(m, &m->site_amax, (size_t)m->n_sites));
@@ -908,6 +886,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     return EV_OK;
 }
 
+static void ev_cache_detach(ev_cache* c) { c->model = nullptr; }
 int ev_model_destroy(ev_model* m) {
     if (!m) return EV_OK;
     cudaDeviceSynchronize();
@@ -915,6 +894,7 @@ int ev_model_destroy(ev_model* m) {
     for (auto& r : m->prof) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto& g : m->graphs) cudaGraphExecDestroy(g.exec);
     if (m->cap_stream) cudaStreamDestroy(m->cap_stream);
+    for (ev_cache* c : m->caches) ev_cache_detach(c);
     delete m;
     return EV_OK;
 }
@@ -1056,7 +1036,7 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
                 return EV_ECUDA;
             }
             c->tc_attn = true;
-            c->kv_f16 = !m->legacy_attn;
+            c->kv_f16 = true;
         }
     }
     cudaMemset(c->page_table, 0, (size_t)max_seqs * c->max_pages * 4);
@@ -1067,6 +1047,7 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
     c->seq_pages.resize(max_seqs);
     c->seq_used.assign(max_seqs, 0);
     c->len_bound.assign(max_seqs, 0);
+    m->caches.push_back(c);
     *out = c;
     return EV_OK;
 }
@@ -1075,6 +1056,8 @@ int ev_cache_destroy(ev_cache* c) {
     if (!c) return EV_OK;
     cudaDeviceSynchronize();
     if (c->model) {  // captured steps that reference this cache's buffers die with it
+        auto& cs = c->model->caches;
+        cs.erase(std::remove(cs.begin(), cs.end(), c), cs.end());
         auto& gs = c->model->graphs;
         for (size_t i = gs.size(); i-- > 0;)
             if (gs[i].key.p[0] == (const void*)c) { cudaGraphExecDestroy(gs[i].exec); gs.erase(gs.begin() + i); }
@@ -1206,7 +1189,7 @@ int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* o
     // Fast path: the whole step (~330 launches, PDL edges included) is captured once per distinct argument set
     // and replayed as one CUDA graph.  Debug taps, lock-step overrides, profiling and calibration run eagerly.
     bool graph_ok = m->use_graph && !m->profile && !m->recording && !in->dev_hidden_override && !out->dev_hidden &&
-                    (out->tap_layer < 0 || out->tap_layer >= m->cfg.n_layers) && !(m->gemm_dbg & 48);
+                    (out->tap_layer < 0 || out->tap_layer >= m->cfg.n_layers);
     if (graph_ok) {
         cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
         if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) graph_ok = false;  // caller captures
@@ -1449,6 +1432,11 @@ int ev_verify_host(ev_model* m, ev_cache* c, int n_seqs, int n_nodes, const int3
     CUDA_TRY(cudaMemcpyAsync(host_accept_nodes, o.dev_accept_nodes, BT * 4, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(host_out_tokens, o.dev_out_tokens, BT * 4, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
+    if (commit)   // the true new lengths are on the host now: tighten the bounds plan_attention advanced by T
+        for (int i = 0; i < n_seqs; ++i) {
+            const int s = host_seq_slots[i];
+            if (s >= 0 && s < c->max_seqs && c->seq_used[s] && host_status[i] == 0) c->len_bound[s] = host_new_ctx_len[i];
+        }
     return EV_OK;
 }
 
@@ -1485,22 +1473,6 @@ int ev_profile_trace(ev_model* m, unsigned long long* host_out, int max_entries,
         for (int j = 2; j < TRACE_SLOTS; ++j) host_out[TRACE_SLOTS * i + j] = ~host_out[TRACE_SLOTS * i + j];
     CUDA_TRY(cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8));
     *n_out = n;
-    return EV_OK;
-}
-
-int ev_debug_gemm_timestamps(ev_model* m, unsigned long long* host_out, int n_ctas) {
-    if (!m || !host_out) return fail(EV_EINVAL, "null argument");
-    CUDA_TRY(cudaDeviceSynchronize());
-    if (n_ctas > 128) n_ctas = 128;
-    if (n_ctas == -2) {  // attention: (start, end, SM id) of up to 512 CTAs
-        CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts + 1024, 3 * 512 * 8, cudaMemcpyDeviceToHost));
-        return EV_OK;
-    }
-    if (n_ctas < 0) {  // attention timestamps
-        CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts + 512, 16 * 8, cudaMemcpyDeviceToHost));
-        return EV_OK;
-    }
-    CUDA_TRY(cudaMemcpy(host_out, m->dbg_ts, (size_t)n_ctas * 8 * 8, cudaMemcpyDeviceToHost));
     return EV_OK;
 }
 

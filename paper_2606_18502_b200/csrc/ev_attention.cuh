@@ -1,19 +1,31 @@
 // K5: tree-masked GQA attention over the paged bf16 KV cache ("tree attention";
-// BASELINE.json:north_star (2)), split over the key axis, + K7: merge of the splits fused with the
-// per-token absmax / E4M3 quantization that feeds the O projection.
+// BASELINE.json:north_star (2)), + K7: merge fused with the per-token absmax / E4M3 quantization that feeds
+// the O projection.
 //
-// One CTA = (sequence b, kv head, group of 8 row tiles, key split).  The query rows of one kv head
-// are the T nodes x G query heads that share it (row = node*G + g), 16 rows per warp.  Keys are the
-// L committed context slots followed by the T tree slots L..L+T-1 (written by the RoPE/KV-write
-// kernel just before); a tree key j is visible to node i iff j is an ancestor-or-self of i (bit j
-// of anc[i]).  Pages are gathered with 16-byte cp.async into XOR-swizzled shared memory (each
-// (page, K|V, head) block is page_size*D*2 contiguous bytes), double buffered; Q.K^T and P.V run on
-// the tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with Q and P each split into
-// hi + mid + lo bf16 parts: 3 x 8 significand bits represent an fp32 value exactly, K and V are bf16
-// already, so every product is exact and only the fp32 accumulation rounds (DESIGN.md section 6
-// "attention precision": a 2-way split left 2^-17 errors that flip E4M3 codes downstream);
-// the online softmax is done in fp32 registers with warp shuffles across the 4 lanes of a row.
+// Batch-invariant reduction order (speculative verification must emit exactly what plain decoding
+// emits, so a node's attention output may not depend on the tree or batch it is verified in).  A node at position
+// p = L + depth attends to positions [0, p].  The key set is cut the same way wherever the node appears:
+//   BULK  = positions [0, p - ATT_TAIL_R), in CHUNKS of `chunk` keys aligned to absolute positions (chunk j = keys
+//           [j chunk, (j+1) chunk)); each chunk is an online softmax over 64-key tiles from a fresh state, on the tensor
+//           cores (tree_attn_tc_kernel, or tree_attn_partial_kernel below for page sizes other than 16);
+//   TAIL  = the last ATT_TAIL_R + 1 positions (youngest cached tokens, then the node's nearest ancestors in depth
+//           order, itself last), scored key by key in fp32 by the merge kernel;
+//   MERGE = out = (sum_j w_j O_j + sum_t e_t v_t) / (sum_j w_j l_j + sum_t e_t), chunks in index order, then the tail
+//           keys in position order, w_j = exp(m_j - M), e_t = exp(s_t - M), M = the overall maximum.
+// For trees no deeper than ATT_TAIL_R the bulk lies inside the committed context: which tree slots the ancestors sit
+// in, how many nodes and sequences share the launch and how many CTAs there are no longer enter the arithmetic.
+// Deeper trees (prefill chains) put the older ancestors into the bulk by slot (anc_bulk); chains stay invariant
+// because a chain's slots are its positions.
+//
+// tree_attn_partial_kernel: one CTA = (sequence b, kv head, group of 8 row tiles, chunk).  The query rows of one kv
+// head are the T nodes x G query heads that share it (row = node*G + g), 16 rows per warp.  Pages are gathered with
+// 16-byte cp.async into XOR-swizzled shared memory (each (page, K|V, head) block is page_size*D*2 contiguous bytes),
+// double buffered; Q.K^T and P.V run on the tensor cores (mma.sync m16n8k16 bf16, fp32 accumulate) with Q and P each
+// split into hi + mid + lo bf16 parts: 3 x 8 significand bits represent an fp32 value exactly, K and V are bf16
+// already, so every product is exact and only the fp32 accumulation rounds; the online softmax is done in fp32
+// registers with warp shuffles across the 4 lanes of a row.
 #pragma once
+#include <cuda_fp16.h>
 #include "ev_common.cuh"
 #include "ev_elementwise.cuh"
 
@@ -21,7 +33,7 @@ namespace ev {
 
 constexpr int ATT_THREADS = 256;
 constexpr int ATT_WARPS = 8;
-constexpr int ATT_CH = 64;  // keys per pipeline chunk
+constexpr int ATT_CH = 64;  // keys per pipeline tile
 
 struct AttnArgs {
     const float* q;       // qkv buffer after RoPE; q head h of row m at q[m*q_ld + h*D]
@@ -33,14 +45,19 @@ struct AttnArgs {
     const int32_t* Lsnap;       // [B]
     const int32_t* nn_eff;      // [B]
     const int32_t* order;       // [B] grid z -> sequence (longest context first); null = identity
-    const unsigned long long* anc;  // [B][T]
-    int split_len;              // keys per split, multiple of ATT_CH
-    int n_splits;               // grid.x
+    const unsigned long long* anc_bulk;  // [B][T] tree slots among the row's bulk keys (tree_prep_kernel)
+    const int32_t* erow;        // [B][T] cached positions below erow[row] are bulk keys of the row
+    const int32_t* kend_seq;    // [B] one past the last bulk key slot of the sequence
+    int chunk;                  // keys per chunk, multiple of ATT_CH: a constant of the model, NOT a function of the batch
+    int n_chunks;               // grid.x = chunks the grid covers; stride of the partial arrays
     float scale;                // 1/sqrt(D)
-    float* o_part;              // [M][Hq][n_splits][D]
-    float* ml_part;             // [M][Hq][n_splits][2]  (running max, running sum)
-    unsigned long long* ts;     // bring-up: phase timestamps of CTA (0,0,0), or null
+    float* o_part;              // [M][Hq][n_chunks][D]
+    float* ml_part;             // [M][Hq][n_chunks][2]  (running max, running sum)
 };
+// bulk membership of key slot kidx for a row (erow e, tree bits ab) of a sequence with L cached tokens
+__device__ __forceinline__ bool bulk_key(int kidx, int L, int e, unsigned long long ab) {
+    return kidx < L ? kidx < e : (kidx - L < 64 && ((ab >> (kidx - L)) & 1ull));
+}
 
 __device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
     asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
@@ -73,12 +90,10 @@ __device__ __forceinline__ void cp_async16_zfill(void* smem_dst, const void* gsr
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(smem_u32(smem_dst)), "l"(gsrc), "r"(sz) : "memory");
 }
 
-#define ATS(i) do { if (a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && threadIdx.x == 0) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); a.ts[i] = t_; } } while (0)
 template <int D>
 __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnArgs a) {
     pdl_launch_dependents();
     pdl_wait();
-    ATS(0);
     constexpr int ROWB = D * 2;           // bytes per key row
     constexpr int CPR = ROWB / 16;        // 16-byte chunks per row
     constexpr int TILE = ATT_CH * ROWB;   // bytes per K (or V) tile
@@ -89,14 +104,14 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
     const int b = blockIdx.z;
-    const int nn = a.nn_eff[b];     // the three scalars are loaded together, before the first branch
+    const int nn = a.nn_eff[b];     // the scalars are loaded together, before the first branch
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
+    const int n_keys = a.kend_seq[b];
     if (nn == 0) return;
-    const int n_keys = L + nn;
-    const int k_begin = split * a.split_len;
+    const int k_begin = split * a.chunk;
     if (k_begin >= n_keys) return;
-    const int k_end = min(k_begin + a.split_len, n_keys);
+    const int k_end = min(k_begin + a.chunk, n_keys);
     const int n_chunks = (k_end - k_begin + ATT_CH - 1) / ATT_CH;
     const int32_t* pt = a.page_table + (size_t)seq_slot * a.max_pages;
 
@@ -107,7 +122,8 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     const int row0 = rt * 16 + (lane >> 2), row1 = row0 + 8;
     const int node0 = row0 / a.G, g0 = row0 % a.G, node1 = row1 / a.G, g1 = row1 % a.G;
     const bool v0 = active && row0 < R && node0 < nn, v1 = active && row1 < R && node1 < nn;
-    const unsigned long long anc0 = v0 ? a.anc[b * a.T + node0] : 0ull, anc1 = v1 ? a.anc[b * a.T + node1] : 0ull;
+    const unsigned long long anc0 = v0 ? a.anc_bulk[b * a.T + node0] : 0ull, anc1 = v1 ? a.anc_bulk[b * a.T + node1] : 0ull;
+    const int e0 = v0 ? a.erow[b * a.T + node0] : 0, e1 = v1 ? a.erow[b * a.T + node1] : 0;
 
     // ---- Q rows -> this warp's shared-memory tiles, split hi/mid/lo (A operand, read by ldmatrix) ----
     const uint32_t qs = smem_u32(att_smem + 4 * TILE + warp * 3 * QTILE);
@@ -135,7 +151,6 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
         }
         __syncwarp();
     }
-    ATS(1);
 
     // ---- page gather: chunk ch -> stage ----
     auto load_chunk = [&](int stage, int ch) {
@@ -171,7 +186,6 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
             cp_async_wait<0>();
         }
         __syncthreads();
-        if (ch < 4) ATS(2 + 2 * ch);
         if (active) {
             const uint32_t ks = smem_u32(att_smem + (ch & 1) * 2 * TILE);
             const uint32_t vs = ks + TILE;
@@ -213,7 +227,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                 }
             }
             // ---- scale, mask, row max ----
-            const bool need_mask = kbase + ATT_CH > L;  // chunk touches tree keys or the split end
+            const bool need_mask = kbase + ATT_CH > L - ATT_TAIL_R;  // tile reaches the end of some row's bulk
             float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
             for (int nt = 0; nt < ATT_CH / 8; ++nt) {
@@ -222,8 +236,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                     float v = mul_rn(s[nt][e], a.scale);
                     if (need_mask) {
                         const int kidx = kbase + nt * 8 + (lane & 3) * 2 + (e & 1);
-                        const unsigned long long am = (e < 2) ? anc0 : anc1;
-                        const bool ok = kidx < k_end && (kidx < L || ((am >> (kidx - L)) & 1ull));
+                        const bool ok = kidx < k_end && bulk_key(kidx, L, (e < 2) ? e0 : e1, (e < 2) ? anc0 : anc1);
                         if (!ok) v = -INFINITY;
                     }
                     s[nt][e] = v;
@@ -284,7 +297,6 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
                 o[i][2] = fmaf(o[i][2], c1, oc[i][2]); o[i][3] = fmaf(o[i][3], c1, oc[i][3]);
             }
         }
-        if (ch < 4) ATS(3 + 2 * ch);
         __syncthreads();
     }
     if (!active) return;
@@ -293,37 +305,59 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     l1 += __shfl_xor_sync(0xffffffffu, l1, 1);
     l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
     if (row0 < R) {
-        const size_t pi = ((size_t)(b * a.T + node0) * a.Hq + kvh * a.G + g0) * a.n_splits + split;
+        const size_t pi = ((size_t)(b * a.T + node0) * a.Hq + kvh * a.G + g0) * a.n_chunks + split;
         float* op = a.o_part + pi * D + (lane & 3) * 2;
 #pragma unroll
         for (int i = 0; i < D / 8; ++i) *reinterpret_cast<float2*>(op + i * 8) = make_float2(o[i][0], o[i][1]);
         if ((lane & 3) == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m0, l0);
     }
     if (row1 < R) {
-        const size_t pi = ((size_t)(b * a.T + node1) * a.Hq + kvh * a.G + g1) * a.n_splits + split;
+        const size_t pi = ((size_t)(b * a.T + node1) * a.Hq + kvh * a.G + g1) * a.n_chunks + split;
         float* op = a.o_part + pi * D + (lane & 3) * 2;
 #pragma unroll
         for (int i = 0; i < D / 8; ++i) *reinterpret_cast<float2*>(op + i * 8) = make_float2(o[i][2], o[i][3]);
         if ((lane & 3) == 0) *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m1, l1);
     }
-    ATS(10);
 }
 
-// ---- merge of the key splits (fixed order 0..ns-1) + per-token absmax + E4M3 quantize -----------
-// One CTA of 512 threads per token.  Phase 1 stages the (max, sum) pairs of all heads x splits in shared
-// memory, phase 2 turns them into softmax weights w[h][s] = exp(m_s - max) and the denominator per head,
-// phase 3 forms out = (sum_s w_s O_s) / den with all S partial loads of a thread in flight at once; the
-// merged row stays in registers for the quantizer.
+// ---- tail keys + merge of the chunks (fixed order) + per-token absmax + E4M3 quantize ---------------
+// One cluster of MERGE_THREADS-thread CTAs per token row; a thread owns float4s of the row, i.e. 4 output dims of one
+// query head, and the D/4 consecutive lanes that share a head form one reduction group (aligned: the CTA's first
+// float4 is a multiple of 32).  Per head: (1) the tail keys - cached slots [erow, L) then the row's own ancestors in
+// the tail, in position order - are scored in fp32: partial dot of 4 dims per lane (one fixed FMA chain), xor-butterfly
+// over the group (every lane ends with the same bits), times 1/sqrt(d); (2) the chunk partials (max, sum, O) of the
+// bulk are read in chunk order; (3) out = (sum_j w_j O_j + sum_t e_t v_t) / (sum_j w_j l_j + sum_t e_t).  The merged
+// row stays in registers for the quantizer.  Nothing here depends on the cluster size or on how many rows there are.
+constexpr int ATT_TAIL_MAX = ATT_TAIL_R + 1;
 struct MergeArgs {
-    int T, Hq, D, n_splits, split_len;
+    int T, Hq, Hkv, D, n_chunks, chunk;
     const int32_t* Lsnap;
     const int32_t* nn_eff;
+    const int32_t* seq_slots;
+    const int32_t* erow;
+    const int32_t* kend_row;
+    const unsigned long long* anc;
+    const unsigned long long* anc_bulk;
     const float* o_part;
     const float* ml_part;
+    const float* qkv;      // rotated q (fp32): head h of row m at qkv[m * q_ld + h * D]
+    int q_ld;
+    const __nv_bfloat16* pool;   // this layer
+    const int32_t* page_table;
+    int max_pages, page_size, kv_f16;
+    float scale;
     float* attn;   // optional [M][Hq*D] fp32 merged output (debug tap) or null
     QuantOut q;
     L2Prefetch pf;
 };
+__device__ __forceinline__ float4 kv_load4(const __nv_bfloat16* p, int kv_f16) {   // 4 consecutive K or V elements as fp32
+    const uint2 w = *reinterpret_cast<const uint2*>(p);
+    if (kv_f16) {
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&w.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&w.y));
+        return make_float4(a.x, a.y, b.x, b.y);
+    }
+    return make_float4(__uint_as_float(w.x << 16), __uint_as_float(w.x & 0xFFFF0000u), __uint_as_float(w.y << 16), __uint_as_float(w.y & 0xFFFF0000u));
+}
 constexpr int MERGE_THREADS = 256;   // = ROW_THREADS (ev_elementwise.cuh): Hq * D <= 4 * 256 * NV4 * cluster size
 template <int MERGE_NV4>
 __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeArgs a) {
@@ -331,93 +365,109 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
     l2_prefetch_issue(a.pf);
     pdl_wait();
     trace_past_wait(a.pf);
-    extern __shared__ float msm[];             // w[Hq][S] | l[Hq][S] | den[Hq]
     __shared__ float red[MERGE_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     const int b = m / a.T, node = m % a.T;
     const int nn = a.nn_eff[b];
-    const int K = a.Hq * a.D, S = a.n_splits;
+    const int K = a.Hq * a.D, S = a.n_chunks, D = a.D;
     const bool valid = node < nn;
-    const int ns = valid ? (a.Lsnap[b] + nn + a.split_len - 1) / a.split_len : 0;
-    float* w = msm;
-    float* ls = msm + a.Hq * S;
-    float* den = ls + a.Hq * S;
-    // The partial outputs of the first NB splits are requested BEFORE the split weights are computed (they only need
-    // ns): the (max, sum) round trip, the two CTA barriers and the exps then run under the loads instead of in front
-    // of them.  One float4 per thread (few tokens, rows spread over a cluster): 12 splits in flight; else 4.
-    constexpr int NB = MERGE_NV4 == 1 ? 12 : 4;
+    const int L = a.Lsnap[b];
+    const int e = valid ? a.erow[m] : 0;
+    const int ns = valid ? (a.kend_row[m] + a.chunk - 1) / a.chunk : 0;
+    // tail keys, in position order: n_ctx cached slots e .. L-1, then the ancestors of the tail (lowest node index = lowest depth first)
+    const int n_ctx = valid ? min(max(0, L - e), ATT_TAIL_MAX) : 0;
+    const unsigned long long anc_tail = valid ? (a.anc[m] & ~a.anc_bulk[m]) : 0ull;
+    const int nt = min(n_ctx + __popcll(anc_tail), ATT_TAIL_MAX);
+    const int32_t* pt = a.page_table + (size_t)(valid ? a.seq_slots[b] : 0) * a.max_pages;
+    const size_t kv_stride = (size_t)a.Hkv * a.page_size * D;   // K block -> V block of a page
+    const int G = a.Hq / a.Hkv;
+    const int gl = D / 4;   // lanes per head group (32 or 16)
     float4 v[MERGE_NV4];
     int c0, c1;
     cluster_cols(K / 4, c0, c1);
-    float4 t0[NB];
-    {
-        const int i4 = c0 + threadIdx.x;
-        const int i = i4 * 4;
-        if (i4 < c1 && valid) {
-            const float* op = a.o_part + ((size_t)m * a.Hq + i / a.D) * S * a.D + i % a.D;
-#pragma unroll
-            for (int u = 0; u < NB; ++u)
-                if (u < ns) t0[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)u * a.D));
-        }
-    }
-    for (int i = threadIdx.x; i < a.Hq * S; i += MERGE_THREADS) {
-        const int h = i / S, sp = i % S;
-        float2 ml = make_float2(-INFINITY, 0.f);
-        if (sp < ns) ml = __ldcg(reinterpret_cast<const float2*>(a.ml_part + (((size_t)m * a.Hq + h) * S + sp) * 2));
-        w[i] = ml.x;
-        ls[i] = ml.y;
-    }
-    __syncthreads();
-    if ((int)threadIdx.x < a.Hq) {
-        const int h = threadIdx.x;
-        float mx = -INFINITY;
-        for (int sp = 0; sp < ns; ++sp) mx = fmaxf(mx, w[h * S + sp]);
-        float d = 0.f;
-        for (int sp = 0; sp < ns; ++sp) {
-            const float ms = w[h * S + sp];
-            const float wt = (ms == -INFINITY) ? 0.f : expf(ms - mx);
-            w[h * S + sp] = wt;
-            d += wt * ls[h * S + sp];
-        }
-        den[h] = d;
-    }
-    __syncthreads();
 #pragma unroll
     for (int k = 0; k < MERGE_NV4; ++k) {
         const int i4 = c0 + threadIdx.x + k * MERGE_THREADS;
         const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (i4 < c1 && valid) {
-            const int h = i / a.D, d = i % a.D;
-            const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * a.D + d;
-            float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
-            int s_done = 0;
-            if (k == 0) {   // the splits requested up front
+        const bool on = i4 < c1 && valid;      // uniform over a head group (D / 4 lanes, aligned)
+        const int h = on ? i / D : 0, d = on ? i % D : 0;
+        const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * D + d;
+        const float* mlp = a.ml_part + ((size_t)m * a.Hq + h) * S * 2;
+        // chunk partials are requested first: the tail scoring below runs under these loads
+        constexpr int NB = 4;
+        float4 t0[NB];
+        float2 ml0[NB];
 #pragma unroll
-                for (int u = 0; u < NB; ++u)
-                    if (u < ns) {
-                        const float wt = w[h * S + u];
-                        num.x += wt * t0[u].x; num.y += wt * t0[u].y; num.z += wt * t0[u].z; num.w += wt * t0[u].w;
-                    }
-                s_done = NB;
+        for (int u = 0; u < NB; ++u)
+            if (on && u < ns) { t0[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)u * D)); ml0[u] = __ldcg(reinterpret_cast<const float2*>(mlp + 2 * u)); }
+        // (1) tail scores
+        float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (on) q4 = *reinterpret_cast<const float4*>(a.qkv + (size_t)m * a.q_ld + i);
+        const int kvh = h / G;
+        float ts[ATT_TAIL_MAX];
+        float4 tv[ATT_TAIL_MAX];
+        unsigned long long at = anc_tail;
+#pragma unroll
+        for (int u = 0; u < ATT_TAIL_MAX; ++u) {
+            float part = 0.f;
+            tv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+            int sl = e + u;
+            if (u >= n_ctx && u < nt) { sl = L + __ffsll((long long)at) - 1; at &= at - 1; }
+            if (on && u < nt) {
+                const __nv_bfloat16* kp = a.pool + (size_t)pt[sl / a.page_size] * 2 * kv_stride + ((size_t)kvh * a.page_size + sl % a.page_size) * D + d;
+                const float4 k4 = kv_load4(kp, a.kv_f16);
+                tv[u] = kv_load4(kp + kv_stride, a.kv_f16);
+                part = fmaf(q4.w, k4.w, fmaf(q4.z, k4.z, fmaf(q4.y, k4.y, __fmul_rn(q4.x, k4.x))));
             }
-            for (int s0 = s_done; s0 < ns; s0 += 4) {   // splits are added in index order, whatever the batching
+            for (int o = gl >> 1; o > 0; o >>= 1) part = __fadd_rn(part, __shfl_xor_sync(0xffffffffu, part, o));
+            ts[u] = mul_rn(part, a.scale);
+        }
+        if (on) {
+            // (2) overall maximum: chunk maxima, then tail scores
+            float mx = -INFINITY;
+#pragma unroll
+            for (int u = 0; u < NB; ++u)
+                if (u < ns) mx = fmaxf(mx, ml0[u].x);
+            for (int j = NB; j < ns; ++j) mx = fmaxf(mx, __ldcg(mlp + 2 * j));
+#pragma unroll
+            for (int u = 0; u < ATT_TAIL_MAX; ++u)
+                if (u < nt) mx = fmaxf(mx, ts[u]);
+            // (3) weighted sums, chunks in index order then the tail in position order
+            float den = 0.f;
+            float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int u = 0; u < NB; ++u)
+                if (u < ns) {
+                    const float wt = (ml0[u].x == -INFINITY) ? 0.f : expf(ml0[u].x - mx);
+                    den = fmaf(wt, ml0[u].y, den);
+                    num.x = fmaf(wt, t0[u].x, num.x); num.y = fmaf(wt, t0[u].y, num.y); num.z = fmaf(wt, t0[u].z, num.z); num.w = fmaf(wt, t0[u].w, num.w);
+                }
+            for (int s0 = NB; s0 < ns; s0 += 4) {
                 float4 t[4];
+                float2 ml[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (s0 + u < ns) t[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)(s0 + u) * a.D));
+                    if (s0 + u < ns) { t[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)(s0 + u) * D)); ml[u] = __ldcg(reinterpret_cast<const float2*>(mlp + 2 * (s0 + u))); }
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
                     if (s0 + u < ns) {
-                        const float wt = w[h * S + s0 + u];
-                        num.x += wt * t[u].x; num.y += wt * t[u].y; num.z += wt * t[u].z; num.w += wt * t[u].w;
+                        const float wt = (ml[u].x == -INFINITY) ? 0.f : expf(ml[u].x - mx);
+                        den = fmaf(wt, ml[u].y, den);
+                        num.x = fmaf(wt, t[u].x, num.x); num.y = fmaf(wt, t[u].y, num.y); num.z = fmaf(wt, t[u].z, num.z); num.w = fmaf(wt, t[u].w, num.w);
                     }
             }
-            const float dn = den[h];
-            v[k] = make_float4(div_rn(num.x, dn), div_rn(num.y, dn), div_rn(num.z, dn), div_rn(num.w, dn));
+#pragma unroll
+            for (int u = 0; u < ATT_TAIL_MAX; ++u)
+                if (u < nt) {
+                    const float et = expf(ts[u] - mx);
+                    den = __fadd_rn(den, et);
+                    num.x = fmaf(et, tv[u].x, num.x); num.y = fmaf(et, tv[u].y, num.y); num.z = fmaf(et, tv[u].z, num.z); num.w = fmaf(et, tv[u].w, num.w);
+                }
+            v[k] = make_float4(div_rn(num.x, den), div_rn(num.y, den), div_rn(num.z, den), div_rn(num.w, den));
+            if (a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
         }
-        if (i4 < c1 && a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
     }
     quantize_regs<MERGE_NV4>(v, m, K, c0, c1, a.q, red, xch_f);
     trace_exit(a.pf);

@@ -147,9 +147,8 @@ constexpr float TCA_QSCALE = 64.f;        // 2^6
 constexpr float TCA_PSCALE_LOG2 = 15.f;   // P is scaled by 2^15
 
 struct TcAttnArgs {
-    AttnArgs a;       // same fields as the legacy kernel (pool pointer unused here)
+    AttnArgs a;       // same fields as tree_attn_partial_kernel (pool pointer unused here)
     int row0;         // first row of this layer in the pool tensor map: layer * n_pages * 2 * Hkv * 16
-    int dbg;          // bring-up experiments (EV_ATTN_DBG): 1 no KV loads, 2 no MMAs, 4 no O-chunk reads
     L2Prefetch pf;
 };
 
@@ -198,23 +197,13 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     pdl_wait();
     trace_past_wait(ta.pf);
     const int b = a.order ? a.order[blockIdx.z] : (int)blockIdx.z;
-    // bring-up (EV_GEMM_DBG=32): per-CTA start / end / SM id at ts[512 + 3 cta ..] (ev_debug_gemm_timestamps(-2))
-    const int cta_lin = (int)(blockIdx.x + gridDim.x * (blockIdx.y + gridDim.y * blockIdx.z));
-    if (a.ts && threadIdx.x == 0 && cta_lin < 512) {
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        a.ts[512 + 3 * cta_lin] = t;
-        a.ts[512 + 3 * cta_lin + 2] = smid;
-    }
     const int nn = a.nn_eff[b];
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
-    const int n_keys = L + nn;
-    const int k_begin = split * a.split_len;
+    const int n_keys = a.kend_seq[b];                  // one past the last bulk key slot of the sequence (tree_prep_kernel)
+    const int k_begin = split * a.chunk;               // chunks sit at absolute key positions: batch-invariant (ev_attention.cuh)
     const bool active = nn != 0 && k_begin < n_keys;   // uniform over the CTA
-    const int k_end = min(k_begin + a.split_len, n_keys);
+    const int k_end = min(k_begin + a.chunk, n_keys);
     const int n_tiles = active ? (k_end - k_begin + TCA_BN - 1) / TCA_BN : 0;
     // ---- Q tile -> TMEM (fp32 x 2^6 -> hi | lo fp16 pairs).  Softmax and correction threads stage it: a warp owns the
     // TMEM lanes of its 32 rows.  Warps 1..17 meet behind named barrier 5; warp 0 goes straight to its K/V
@@ -265,7 +254,6 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             const int pid = pt[min((k_begin + j * TCA_BN) / TCA_PAGE + pg, a.max_pages - 1)];
             return (ta.row0 + ((pid * 2 + kv) * a.Hkv + kvh) * TCA_PAGE) >> 3;   // 8-row group index
         };
-        const bool ld_on = !(ta.dbg & 1);
         // Lanes 0..3 stream the K tiles, lanes 4..7 the V tiles, as two INDEPENDENT loops (divergent lanes of one warp):
         // each stream runs as far ahead as its own ring allows.  In one common loop a full V ring (V tiles are
         // released by P.V, two tiles behind Q.K^T) also held back the K loads, and the MMA warp waited ~420 cycles per
@@ -283,8 +271,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 if (j + 1 < n_tiles) row_next = box_row(j + 1);
                 const int sl = j % depth;
                 mbar_wait(&empty[sl], ((j / depth) & 1) ^ 1);
-                if (pg == 0) { if (ld_on) mbar_arrive_expect_tx(&full[sl], C::K_BYTES); else mbar_arrive(&full[sl]); }
-                if (ld_on) tma_load_4d(ring + sl * C::K_BYTES + dst_off, &tmKV, &full[sl], 0, 0, 0, row_cur);
+                if (pg == 0) mbar_arrive_expect_tx(&full[sl], C::K_BYTES);
+                tma_load_4d(ring + sl * C::K_BYTES + dst_off, &tmKV, &full[sl], 0, 0, 0, row_cur);
             }
         }
     } else if (warp == 1) {
@@ -295,19 +283,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         constexpr uint32_t idesc_qk = umma_idesc_f16(128, TCA_BN, 0);
         constexpr uint32_t idesc_pv = umma_idesc_f16(128, D, 1);
         const bool leader = elect_one();
-        const bool do_mma = !(ta.dbg & 2);
+        constexpr bool do_mma = true;
         const uint32_t q_tmem = tmem_base + C::TQ;
         const uint32_t kv_addr = smem_u32(kv_s);
-        const bool mts = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;
-        long long mt_p = 0, mt_o = 0, mt_kv = 0;
         auto issue_pv = [&](int i) {
             const int s = i % TCA_VS;
             mbar_wait(&v_full[s], (i / TCA_VS) & 1);
-            const long long t0_ = mts ? clock64() : 0;
             mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
-            const long long t1_ = mts ? clock64() : 0;
             mbar_wait(&o_empty[i % C::NO], ((i / C::NO) & 1) ^ 1);   // the correction warps have read chunk i - NO
-            if (mts) { const long long t2_ = clock64(); mt_p += t1_ - t0_; mt_o += t2_ - t1_; }
             tc_fence_after();
             const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
             const uint32_t d_addr = tmem_base + C::TO + (i % C::NO) * D;
@@ -329,9 +312,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         };
         auto issue_qk = [&](int j) {
             const int s = j % TCA_KS;
-            const long long t0_ = mts ? clock64() : 0;
             mbar_wait(&k_full[s], (j / TCA_KS) & 1);
-            if (mts) mt_kv += clock64() - t0_;
             tc_fence_after();
             const uint32_t k_addr = kv_addr + s * C::K_BYTES;
             const uint32_t s_addr = tmem_base + C::TS + (j % C::NSP) * C::SP;
@@ -362,7 +343,6 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             if (j + LA < n_tiles) issue_qk(j + LA);
             issue_pv(j);
         }
-        if (mts && leader) { a.ts[14] = (unsigned long long)mt_p; a.ts[15] = (unsigned long long)(mt_kv + (mt_o << 32)); }
     } else if (warp < 10) {
         // ===== softmax: thread = (row, wg); wg handles keys [32 wg, +32) of every tile.  Warp w may touch TMEM
         // lanes 32 (w % 4) .. +31; the two warps of a row quarter meet behind named barrier 1 + (w % 4). =====
@@ -372,15 +352,13 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const int node = row / a.G, gi = row % a.G;
         const bool valid = row < R && node < nn;
         const bool warp_valid = __any_sync(0xffffffffu, valid);   // the same for both warps of a row quarter
-        const unsigned long long anc = valid ? a.anc[b * a.T + node] : 1ull;
+        const unsigned long long ab = valid ? a.anc_bulk[b * a.T + node] : 0ull;   // tree slots among this row's bulk keys
+        const int erow = valid ? a.erow[b * a.T + node] : 0;                       // cached positions below erow are bulk keys
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
         float m_run = -INFINITY, l_run = 0.f;   // l_run carries P's factor 2^15
         const float qk_scale = a.scale * (1.f / TCA_QSCALE);
 
-        const bool tsw = a.ts && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0;  // bring-up: phase cycles of one warp
-        long long tph[5] = {0, 0, 0, 0, 0}, tq = tsw ? clock64() : 0;
-#define TPH(k) do { if (tsw) { const long long t_ = clock64(); tph[k] += t_ - tq; tq = t_; } } while (0)
         for (int j = 0; j < n_tiles; ++j) {
             mbar_wait(&s_full[j % C::NSP], (j / C::NSP) & 1);
             tc_fence_after();
@@ -390,22 +368,16 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
                 continue;
             }
-            if (j == 0 && threadIdx.x == 64) trace_phase_any(ta.pf, 1);   // first S tile ready
-            TPH(0);
             uint32_t sv[32];
             tmem_ld32(lane_addr + C::TS + (j % C::NSP) * C::SP + wg * 32, sv);
             tmem_ld_wait();
-            TPH(1);
             const int kb = k_begin + j * TCA_BN + wg * 32;
 #pragma unroll
             for (int e = 0; e < 32; ++e) sv[e] = __float_as_uint(mul_rn(__uint_as_float(sv[e]), qk_scale));  // s = (q.k) / sqrt(d), rounded as the method states (2^6 of Q taken out exactly)
-            if (kb + 32 > L) {   // tile half touches tree keys or the end of the key range (warp-uniform)
+            if (kb + 32 > L - ATT_TAIL_R) {   // tile half reaches the end of some row's bulk (warp-uniform)
 #pragma unroll
-                for (int e = 0; e < 32; ++e) {
-                    const int kidx = kb + e;
-                    const bool ok = kidx < k_end && (kidx < L || ((anc >> (kidx - L)) & 1ull));
-                    if (!ok) sv[e] = 0xFF800000u;  // -inf
-                }
+                for (int e = 0; e < 32; ++e)
+                    if (!bulk_key(kb + e, L, erow, ab)) sv[e] = 0xFF800000u;  // -inf
             }
             float mx0 = fmaxf(__uint_as_float(sv[0]), __uint_as_float(sv[1])), mx1 = fmaxf(__uint_as_float(sv[2]), __uint_as_float(sv[3]));
 #pragma unroll
@@ -417,7 +389,6 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             xmax[((j & 1) * 2 + wg) * 128 + r] = mx;
             pair_bar_sync(1 + (warp & 3));
             mx = fmaxf(mx, xmax[((j & 1) * 2 + (wg ^ 1)) * 128 + r]);
-            TPH(2);
             const float mn = fmaxf(m_run, mx);
             const float mu = (mn == -INFINITY) ? 0.f : mn;
             const float c = ex2_approx((m_run - mu) * LOG2E);  // 2^-inf = 0 on the first tile
@@ -441,28 +412,17 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 tmem_st8(p_addr + 32 + h * 8, pl);
             }
             l_run = fmaf(l_run, c, ls0 + ls1);
-            TPH(3);
             tmem_st_wait();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
-            TPH(4);
         }
-        if (tsw && lane == 0) {
-            if (warp == 2) {
-                for (int k = 0; k < 5; ++k) a.ts[k] = (unsigned long long)tph[k];
-                a.ts[5] = (unsigned long long)n_tiles;
-            }
-            a.ts[6 + warp - 2] = (unsigned long long)(tph[1] + tph[2] + tph[3] + tph[4]);
-        }
-#undef TPH
-        if (threadIdx.x == 64) trace_phase_any(ta.pf, 2);   // softmax of the last tile done
         // ---- running max and sum of this split ----
         l_run *= exp2f(-TCA_PSCALE_LOG2);   // exact
         xsum[wg * 128 + r] = l_run;
         if (warp_valid) pair_bar_sync(1 + (warp & 3));
         if (valid && wg == 0) {
-            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
+            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_chunks + split;
             *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m_run, l_run + xsum[128 + r]);
         }
     } else {
@@ -491,13 +451,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
 #pragma unroll
             for (int cb = 0; cb < C::DH / 16; ++cb) {
                 uint32_t ov[16];
-                if (!(ta.dbg & 4)) {
-                    tmem_ld16(lane_addr + C::TO + (i % C::NO) * D + hh * C::DH + cb * 16, ov);
-                    tmem_ld_wait();
-                } else {
-#pragma unroll
-                    for (int e = 0; e < 16; ++e) ov[e] = 0;
-                }
+                tmem_ld16(lane_addr + C::TO + (i % C::NO) * D + hh * C::DH + cb * 16, ov);
+                tmem_ld_wait();
                 if (cb == C::DH / 16 - 1) {
                     tc_fence_before();
                     __syncwarp();
@@ -508,23 +463,17 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             }
         }
         if (valid) {
-            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_splits + split;
+            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_chunks + split;
             float* op = a.o_part + pi * D + hh * C::DH;
 #pragma unroll
             for (int i = 0; i < C::DH; ++i) o[i] *= exp2f(-TCA_PSCALE_LOG2);   // P's factor 2^15, exact
 #pragma unroll
             for (int i = 0; i < C::DH; i += 4) *reinterpret_cast<float4*>(op + i) = make_float4(o[i], o[i + 1], o[i + 2], o[i + 3]);
         }
-        if (threadIdx.x == 320) trace_phase_any(ta.pf, 3);   // partial output written
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<512>(tmem_base);
-    if (a.ts && threadIdx.x == 0 && cta_lin < 512) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        a.ts[512 + 3 * cta_lin + 1] = t;
-    }
     trace_exit(ta.pf);
 }
 

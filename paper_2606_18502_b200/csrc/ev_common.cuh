@@ -188,12 +188,12 @@ struct LinOut {
     long split_stride;   // M * ld
     const float* sx;     // [M]
     const float* sw;     // [N]
-    int sk_G, sk_U, sk_kb;  // stream-K partition (ev_gemm.cuh): grid size, K-block units, K-blocks per tile; sk_U == 0 = classic
+    int sk_G, sk_U, sk_kb;  // canonical K cuts (ev_gemm.cuh): CTA pairs, K-block units, K-blocks per tile; sk_U == 0 = no cuts
 };
-// number of slabs that hold a piece of output channel n (all channels of a 128-row weight tile share it)
+// number of slabs that hold a piece of output channel n (all channels of a PAIR of 128-row weight tiles share it)
 __device__ __forceinline__ int lin_slabs(const LinOut& o, int n) {
     if (o.sk_U == 0) return o.splits;
-    const unsigned t = (unsigned)n >> 7, G = (unsigned)o.sk_G, U = (unsigned)o.sk_U, kb = (unsigned)o.sk_kb;
+    const unsigned t = (unsigned)n >> 8, G = (unsigned)o.sk_G, U = (unsigned)o.sk_U, kb = (unsigned)o.sk_kb;
     const unsigned c_first = ((t * kb + 1u) * G + U - 1u) / U;   // first CTA touching the tile, + 1
     const unsigned c_last = ((t + 1u) * kb * G + U - 1u) / U;    // last CTA touching it, + 1
     return (int)(c_last - c_first) + 1;

@@ -88,6 +88,13 @@ __global__ void __launch_bounds__(EW_THREADS) quantize_weight_rows_kernel(const 
 }
 
 // ---- tree bookkeeping: one thread per sequence -----------------------------------------------
+// Besides depths, positions and ancestor masks this kernel fixes how every node's key set is cut for attention
+// (ev_attention_tc.cuh, "batch-invariant reduction order"): a node at position p = L + depth attends to positions
+// [0, p].  The BULK [0, p - ATT_TAIL_R) goes through the tensor-core kernel in chunks aligned to absolute positions;
+// the TAIL (the last ATT_TAIL_R + 1 positions: the youngest cached tokens and the node's nearest ancestors, itself
+// included) is added key by key in position order by the merge kernel.  For trees of depth <= ATT_TAIL_R the bulk
+// lies entirely in the committed context, so a node's result does not depend on the tree it arrived in.
+constexpr int ATT_TAIL_R = 8;
 struct TreePrepArgs {
     int B, T, vocab, page_size;
     const int32_t* seq_slots;  // [B]
@@ -97,6 +104,7 @@ struct TreePrepArgs {
     const int32_t* ctx_len;    // [max_seqs] (device state)
     const int32_t* capacity;   // [max_seqs] tokens
     int max_seqs, max_pos;
+    int max_keys;              // keys the attention grid of this step covers (n_chunks * chunk): longer sequences are rejected
     int32_t* Lsnap;            // [B] context length at entry
     int32_t* nn_eff;           // [B] nodes in use (0 when the sequence is rejected)
     int32_t* order;            // [B] sequences by decreasing context length (attention CTAs start the longest first)
@@ -104,6 +112,10 @@ struct TreePrepArgs {
     int32_t* depth;            // [B][T]
     int32_t* pos;              // [B][T] RoPE position = L + depth
     unsigned long long* anc;   // [B][T] ancestor-or-self bit masks
+    unsigned long long* anc_bulk;  // [B][T] ancestors that belong to the bulk (depth < own depth - ATT_TAIL_R); 0 for shallow trees
+    int32_t* erow;             // [B][T] cached positions below erow are bulk keys of the row: max(0, L + depth - ATT_TAIL_R)
+    int32_t* kend_row;         // [B][T] one past the row's last bulk key slot
+    int32_t* kend_seq;         // [B] max over the sequence's rows
     unsigned long long* argmax_keys;  // [B*T] reset to 0 here
 };
 
@@ -117,20 +129,20 @@ __global__ void tree_prep_kernel(TreePrepArgs a) {
     const int slot = a.seq_slots[b];
     int nn = a.n_nodes ? a.n_nodes[b] : T;
     int L = 0;
+    if (nn < 1 || nn > T) { st |= 1; nn = 0; }   // checked before anything is indexed by it
     if (slot < 0 || slot >= a.max_seqs) {
         st |= 4;
     } else {
         L = a.ctx_len[slot];
-        if (nn < 1 || nn > T) st |= 1;
-        else if (L + nn > a.capacity[slot] || L + nn > a.max_pos) st |= 4;
+        if (L + nn > a.capacity[slot] || L + nn > a.max_pos || L + nn > a.max_keys) st |= 4;
+        for (int o = 0; o < b; ++o)   // two rows of one batch on the same sequence would race on its KV slots: the later one is rejected
+            if (a.seq_slots[o] == slot) st |= 4;
     }
-    if (!(st & 1)) {
-        for (int i = 0; i < nn; ++i) {
-            const int p = a.parents[b * T + i];
-            const int tk = a.tokens[b * T + i];
-            if (tk < 0 || tk >= a.vocab) st |= 2;
-            if (i == 0 ? (p != -1) : (p < 0 || p >= i)) { st |= 1; break; }
-        }
+    for (int i = 0; i < nn; ++i) {
+        const int p = a.parents[b * T + i];
+        const int tk = a.tokens[b * T + i];
+        if (tk < 0 || tk >= a.vocab) st |= 2;
+        if (i == 0 ? (p != -1) : (p < 0 || p >= i)) { st |= 1; break; }
     }
     a.status[b] = st;
     a.Lsnap[b] = L;
@@ -145,18 +157,30 @@ __global__ void tree_prep_kernel(TreePrepArgs a) {
         }
         a.order[rank] = b;
     }
+    int kend = 0;
     for (int i = 0; i < T; ++i) {
         int d = 0;
-        unsigned long long m = 1ull;  // padding / rejected rows see the root only
+        unsigned long long m = 1ull, mb = 0ull;  // padding / rejected rows see the root only
+        int e = 0, ke = 0;
         if (!st && i < nn) {
             const int p = a.parents[b * T + i];
             if (i > 0) { d = a.depth[b * T + p] + 1; m = a.anc[b * T + p] | (1ull << i); }
+            e = max(0, L + d - ATT_TAIL_R);
+            if (d > ATT_TAIL_R)
+                for (int j = 0; j < i; ++j)
+                    if (((m >> j) & 1ull) && a.depth[b * T + j] < d - ATT_TAIL_R) mb |= 1ull << j;
+            ke = mb ? L + (63 - __clzll((long long)mb)) + 1 : min(L, e);
         }
         a.depth[b * T + i] = d;
         a.pos[b * T + i] = L + d;
         a.anc[b * T + i] = m;
+        a.anc_bulk[b * T + i] = mb;
+        a.erow[b * T + i] = e;
+        a.kend_row[b * T + i] = ke;
+        kend = max(kend, ke);
         a.argmax_keys[b * T + i] = 0ull;
     }
+    a.kend_seq[b] = kend;
 }
 
 // ---- K11: embedding gather: residual stream (fp32) <- bf16 rows --------------------------------
@@ -256,7 +280,7 @@ __device__ __forceinline__ void quantize_regs(const float4 (&v)[NV4], int m, int
 // this CTA's share [c0, c1) of a row of n4 float4s
 __device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
     const int nct = (int)cluster_nctarank(), r = (int)cluster_ctarank();
-    const int per = (n4 + nct - 1) / nct;
+    const int per = ((n4 + nct - 1) / nct + 31) & ~31;   // whole 32-float4 segments: a warp's float4s never straddle two CTAs' shares
     c0 = min(n4, r * per);
     c1 = min(n4, c0 + per);
 }
@@ -269,6 +293,7 @@ __device__ __forceinline__ void cluster_cols(int n4, int& c0, int& c1) {
 // the token count so that few rows still fill the machine and many rows keep several CTAs per SM: row_plan()).
 constexpr int ROW_THREADS = 256;
 constexpr int NORM_THREADS = ROW_THREADS;
+constexpr int NORM_SEG_MAX = 32;   // 128-element segments of a row: hidden <= 4096
 template <int NORM_NV4, int MAXS>
 __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
                                                                      const __nv_bfloat16* __restrict__ gain, float eps,
@@ -276,9 +301,8 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
     pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
     l2_prefetch_issue(pf);
     __shared__ float red[NORM_THREADS / 32];
-    __shared__ double dred[NORM_THREADS / 32];
+    __shared__ double seg[NORM_SEG_MAX];   // segment sums of the whole row, in segment order (every CTA of the cluster gets all of them)
     __shared__ float xch_f[CLUSTER_MAX];
-    __shared__ double xch_d[CLUSTER_MAX];
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     int c0, c1;
     cluster_cols(H / 4, c0, c1);
@@ -294,12 +318,17 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
     float* x = h + (size_t)m * H;
     float4 v[NORM_NV4];
     const float sxm = pend.p ? __ldg(pend.sx + m) : 0.f;
-    double acc = 0.0;  // mean of squares accumulated in fp64, rounded once (DESIGN.md R-accum)
+    // Mean of squares in fp64, rounded once (DESIGN.md R-accum), in ONE fixed order whatever the cluster size and the
+    // float4s per thread: the row is cut into segments of 32 float4s (128 elements); a segment always belongs to one
+    // warp in one k-iteration, which sums it with an xor butterfly; the segment sums are then added in segment order.
+    const int nseg = (H / 4 + 31) / 32;
+    const uint32_t nct = cluster_nctarank();
 #pragma unroll
     for (int k = 0; k < NORM_NV4; ++k) {
         const int i4 = c0 + threadIdx.x + k * NORM_THREADS;
         const int i = i4 * 4;
         v[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+        double acc = 0.0;
         if (i4 < c1) {
             v[k] = *reinterpret_cast<const float4*>(x + i);
             if (pend.p) {
@@ -307,16 +336,19 @@ __global__ void __launch_bounds__(NORM_THREADS) rmsnorm_quant_kernel(float* __re
                 v[k] = make_float4(add_rn(v[k].x, y.x), add_rn(v[k].y, y.y), add_rn(v[k].z, y.z), add_rn(v[k].w, y.w));
                 *reinterpret_cast<float4*>(x + i) = v[k];
             }
-            acc += (double)v[k].x * v[k].x + (double)v[k].y * v[k].y + (double)v[k].z * v[k].z + (double)v[k].w * v[k].w;
+            acc = (((double)v[k].x * v[k].x + (double)v[k].y * v[k].y) + (double)v[k].z * v[k].z) + (double)v[k].w * v[k].w;
+        }
+        acc = warp_sum(acc);
+        const int w4 = i4 - (int)(threadIdx.x & 31);   // the warp's first float4 (warp-uniform); every segment has exactly one owner
+        const int sg = w4 >> 5;
+        if ((threadIdx.x & 31) == 0 && w4 < c1) {
+            if (nct == 1) seg[sg] = acc;
+            else for (uint32_t r = 0; r < nct; ++r) asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(cluster_map(seg + sg, r)), "d"(acc) : "memory");
         }
     }
-    acc = warp_sum(acc);
-    if ((threadIdx.x & 31) == 0) dred[threadIdx.x >> 5] = acc;
-    __syncthreads();
+    if (nct > 1) cluster_barrier(); else __syncthreads();
     double tot = 0.0;
-#pragma unroll
-    for (int i = 0; i < NORM_THREADS / 32; ++i) tot += dred[i];
-    tot = cluster_sum(tot, xch_d);
+    for (int i = 0; i < nseg; ++i) tot += seg[i];
     const float ms = (float)(tot / (double)H);
     const float r = div_rn(1.0f, sqrtf(add_rn(ms, eps)));
 #pragma unroll

@@ -25,6 +25,15 @@
 // every element exactly once) sums the K-splits in split order and applies s_x[m] * s_w[n] (+ residual).
 // That makes split-K free of any fix-up pass, fence or atomic, and deterministic (LinOut, ev_common.cuh).
 // Only the LM head applies its scales here, because it reduces to an argmax in the epilogue.
+// Canonical K cuts (batch invariance: verification must reproduce plain decoding bit for bit, so a token's
+// result may not depend on how many other tokens share the launch).  Every layer matrix has ONE fixed set of K cuts,
+// a function of its shape and of the model constant `cut_G` only: the K-blocks of the flattened (pair of 128-channel
+// tiles, K-block) space are dealt out evenly to cut_G pieces, piece c = [floor(c U / G), floor((c+1) U / G)); each
+// piece is accumulated from zero inside the tensor core and the pieces of a tile are added in K order with single
+// rounded fp32 additions.  Few rows (one token tile): piece c IS the work of CTA pair c (stream-K), the pieces land
+// in slabs the consumer adds (LinOut).  Many rows: a CTA pair owns whole (pair tile, token tile) items, switches the
+// TMEM accumulator at the same cuts and its epilogue warps keep the running fp32 sum in registers - same additions,
+// same order, one slab.  The LM head is never cut (1002 tiles).
 // Programmatic dependent launch: barrier setup, TMEM allocation and the first STAGES weight tiles
 // are issued BEFORE griddepcontrol.wait (weights do not depend on the previous kernel), so the
 // weight stream of this GEMM starts while the previous (element-wise) kernel is still running.
@@ -35,7 +44,9 @@ namespace ev {
 
 enum GemmEpi { EPI_RAW = 0, EPI_ARGMAX = 2 };
 
-constexpr int GEMM_THREADS = 192;
+constexpr int GEMM_THREADS = 192;        // warp 0 TMA, warp 1 MMA, 4 epilogue warps
+constexpr int GEMM_THREADS_SUM = 320;    // the running-sum epilogue (CTA pairs, raw output): 8 epilogue warps
+template <int EPI, bool PAIR> constexpr int gemm_threads() { return (PAIR && EPI == 0) ? GEMM_THREADS_SUM : GEMM_THREADS; }
 constexpr int GEMM_BK = 128;          // bytes (= E4M3 elements) of K per stage: one swizzle row
 constexpr int GEMM_WROWS = 128;       // output channels per tile = UMMA M
 constexpr int GEMM_WTILE = GEMM_WROWS * GEMM_BK;  // 16 KiB
@@ -56,19 +67,20 @@ struct GemmArgs {
     float* out;         // EPI_RAW: [k_splits][M][ldo] raw accumulators; EPI_ARGMAX: optional logits [M][ldo]
     int ldo;
     unsigned long long* argmax_keys;  // EPI_ARGMAX: [M] packed (ordered logit, ~index)
-    unsigned long long* ts;  // bring-up: per-CTA phase timestamps [grid][8] (globaltimer ns), or null
     L2Prefetch pf;      // slice of the weight stream of the GEMMs that follow (ev_common.cuh)
     const void* warm[2];   // per-layer constants the CONSUMER kernel will read first thing after its wait (this
     int warm_bytes[2];     // matrix's s_w, the next RMSNorm's gain): touched here so they are L2 hits there
-    int dbg;            // bring-up experiments (EV_GEMM_DBG): 1 no L2 hints, 2 W in 4 copies, 4 skip MMA, 8 skip loads, 64 skip stores
     int bal;            // balanced partition (several token tiles): the (n unit, 16-token block) space, n unit major, is dealt
                         // out evenly to the CTAs (CTA pairs); a CTA's contiguous range is cut at n-unit boundaries and into
                         // items of <= 256 tokens, so token tiles differ in size from item to item (GemmItem::tok) and no
                         // CTA idles in a partial last wave (896 tiles on 148 CTAs = 6.05 waves cost 7).  0 = uniform tiles
     int bal_blocks;     // 16-token blocks per n unit = ceil(M / 16)
     const CUtensorMap* tms;   // bal: activation tensor maps in global memory, box heights 8, 16, ..., 256 rows ([h / 8 - 1])
-    int mc;             // 1 = CTA pairs (cluster of 2, tcgen05 cta_group::2): one 256-channel x tok MMA per pair, each CTA
-                        // stages its own 128 channels of W and HALF of the token tile (see "CTA pairs" below)
+    int mc;             // 1 = work is indexed by PAIRS of CTAs (pair c = CTAs 2c, 2c+1; CTA rank r takes n tile 2 p + r of pair
+                        // tile p).  The PAIR kernel (cluster of 2, tcgen05 cta_group::2) runs one 256-channel x tok MMA per pair,
+                        // each CTA staging its own 128 channels of W and HALF of the token tile (see "CTA pairs" below); the
+                        // single-CTA kernel uses the same indexing for stream-K so that both share the canonical K cuts
+    int cut_G, cut_U;   // canonical K cuts for whole-tile items (PAIR kernel, raw output): pieces, K-block units; cut_U == 0 = none
 };
 
 // byte offset of element (row r, byte c) inside a 16 KiB weight tile (128-byte swizzle)
@@ -132,22 +144,6 @@ __device__ __forceinline__ void mbar_arrive_remote(uint64_t* bar, uint32_t rank)
     // tensor core, and tcgen05.ld -> tcgen05.fence::before_thread_sync -> arrive on the epilogue side.
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_map(bar, rank)) : "memory");
 }
-__device__ __forceinline__ void load_w(int dbg, uint8_t* dst, const uint8_t* src, uint64_t* bar, uint64_t pol) {
-    if (dbg & 8) return;
-    const int parts = (dbg & 2) ? 4 : 1;
-    const uint32_t bytes = GEMM_WROWS * GEMM_BK / parts;
-    for (int i = 0; i < parts; ++i) {
-        if (dbg & 1) bulk_load_plain(dst + i * bytes, src + i * bytes, bytes, bar);
-        else bulk_load(dst + i * bytes, src + i * bytes, bytes, bar, pol);
-    }
-}
-__device__ __forceinline__ void load_x(int dbg, uint8_t* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, uint64_t pol) {
-    if (dbg & 8) return;
-    if (dbg & 1) tma_load_2d(dst, tm, bar, c0, c1);
-    else tma_load_2d_hint(dst, tm, bar, c0, c1, pol);
-}
-__device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define TS(i) do { if (a.ts) a.ts[blockIdx.x * 8 + (i)] = gtimer(); } while (0)
 struct GemmItem { int n_tile, m_tile, split, tile, kb0, nkb, m0, tok; };   // m0, tok: first token row and token count of the item
 __device__ __forceinline__ GemmItem gemm_item(const GemmArgs& a, int w) {
     GemmItem it;
@@ -232,12 +228,19 @@ struct GemmWork {
     }
 };
 
-// PAIR: the kernel contains cta_group::2 instructions and must be launched in clusters of 2 (a.mc == PAIR)
+// chunk ends of a whole-tile item under the canonical K cuts: the K-blocks [kb, *end) of pair tile p that belong to piece cc
+__device__ __forceinline__ int cut_end(const GemmArgs& a, int p, int cc) {
+    return min(a.total_kb, (int)((long long)(cc + 1) * a.cut_U / a.cut_G) - p * a.total_kb);
+}
+
+// PAIR: the kernel contains cta_group::2 instructions and must be launched in clusters of 2 (a.mc == 1)
 template <int EPI, bool PAIR>
-__global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmXh, GemmArgs a) {
+__global__ void __launch_bounds__((gemm_threads<EPI, PAIR>()), 1) gemm_e4m3_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmXh, GemmArgs a) {
+    constexpr bool SUM = PAIR && EPI == EPI_RAW;   // running-sum epilogue: 8 epilogue warps, canonical K cuts inside an item
+    constexpr int EPI_WARPS = SUM ? 8 : 4;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-    // CTA pairs (many token rows; PAIR = a.mc): the pair runs ONE tcgen05.mma.cta_group::2 of 256 channels x tok tokens per
+    // CTA pairs (many token rows; PAIR): the pair runs ONE tcgen05.mma.cta_group::2 of 256 channels x tok tokens per
     // K step.  Each CTA stages its own 128 channels of W and HALF of the token tile; the tensor cores read both
     // halves across the pair.  Per K-block a CTA then receives 16 KiB + tok/2 x 128 B instead of 16 KiB + tok x 128 B:
     // a third less L2 -> SM traffic per flop and 6 instead of 4 stages in flight at tok = 208, which is what bounded
@@ -263,12 +266,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     if (warp >= 2) {  // epilogue warps are idle until the first accumulator is ready: one 128-byte line per thread
 #pragma unroll
         for (int s = 0; s < 2; ++s)
-            for (int ln = blockIdx.x * 128 + (int)threadIdx.x - 64; ln * 128 < a.warm_bytes[s]; ln += gridDim.x * 128) {
+            for (int ln = blockIdx.x * (32 * EPI_WARPS) + (int)threadIdx.x - 64; ln * 128 < a.warm_bytes[s]; ln += gridDim.x * (32 * EPI_WARPS)) {
                 unsigned tmp;
                 asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(tmp) : "l"(reinterpret_cast<const char*>(a.warm[s]) + (size_t)ln * 128));
             }
     }
-    if (threadIdx.x == 0) TS(0);
     uint32_t tmem_cols = 32;
     while ((int)tmem_cols < 2 * a.tok) tmem_cols <<= 1;
 
@@ -284,17 +286,16 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     }
     if (warp == 0 && lane == 0) {
         for (int s = 0; s < a.stages; ++s) { mbar_init(&full_bar[s], 1); mbar_init(&empty_bar[s], 1); mbar_init(&peer_full_bar[s], 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], PAIR ? 8 : 4); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&tmem_full_bar[i], 1); mbar_init(&tmem_empty_bar[i], (PAIR ? 2 : 1) * EPI_WARPS); }
         fence_barrier_init();
         pre = min(a.stages, it0.nkb);
         const uint8_t* wsrc = a.W + ((size_t)it0.n_tile * a.total_kb + it0.kb0) * GEMM_WTILE;
         const uint32_t tx0 = GEMM_WTILE + (PAIR ? it0.tok / 2 : it0.tok) * GEMM_BK;   // W tile + this CTA's token rows of the item
         for (int i = 0; i < pre; ++i) {
-            if (a.dbg & 8) mbar_arrive(&full_bar[i]); else mbar_arrive_expect_tx(&full_bar[i], tx0);
-            if (!(a.dbg & 8)) bulk_load_plain(smem + i * stage_bytes, wsrc + (size_t)i * GEMM_WTILE, GEMM_WTILE, &full_bar[i]);
+            mbar_arrive_expect_tx(&full_bar[i], tx0);
+            bulk_load_plain(smem + i * stage_bytes, wsrc + (size_t)i * GEMM_WTILE, GEMM_WTILE, &full_bar[i]);
         }
         tma_prefetch_desc(&tmX);
-        TS(2);
     }
     if (warp == 1) { if (PAIR) tmem_alloc_rt2(tmem_base_smem, tmem_cols); else tmem_alloc_rt(tmem_base_smem, tmem_cols); }
     tc_fence_before();
@@ -302,7 +303,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
     if (PAIR) cluster_barrier();   // the peer's barriers exist before any commit or relayed arrive targets them
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
-    if (threadIdx.x == 0) TS(1);
+    const bool cuts = SUM && a.cut_U > 0;
 
     if (warp == 0) {
         if (lane == 0) {  // ===== producer: weights by linear bulk copy, activations by 2-D TMA =====
@@ -310,12 +311,11 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             const uint64_t pol_x = policy_evict_last();    // activations are re-read by every tile
             pdl_wait();  // activations come from the previous kernel
             trace_past_wait(a.pf);
-            TS(3);
             // pairs: this CTA fetches only its half of the item's token rows (rows rank * tok / 2 ...), into its own stage
             auto ld_x = [&](uint8_t* st, uint64_t* bar, int kb_abs, const GemmItem& item) {
                 const int rows = PAIR ? item.tok / 2 : item.tok;
                 const CUtensorMap* tm = a.bal ? a.tms + (rows / 8 - 1) : (PAIR ? &tmXh : &tmX);
-                load_x(a.dbg, st + GEMM_WTILE, tm, bar, kb_abs * GEMM_BK, item.m0 + rank * rows, pol_x);
+                tma_load_2d_hint(st + GEMM_WTILE, tm, bar, kb_abs * GEMM_BK, item.m0 + rank * rows, pol_x);
             };
             for (int i = 0; i < pre; ++i) ld_x(smem + i * stage_bytes, &full_bar[i], it0.kb0 + i, it0);
             int s = pre;
@@ -328,9 +328,9 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                 const uint32_t tx = GEMM_WTILE + (PAIR ? it.tok / 2 : it.tok) * GEMM_BK;
                 for (int kb = (first ? pre : 0); kb < it.nkb; ++kb) {
                     mbar_wait(&empty_bar[s], ph ^ 1);
-                    if (a.dbg & 8) mbar_arrive(&full_bar[s]); else mbar_arrive_expect_tx(&full_bar[s], tx);
+                    mbar_arrive_expect_tx(&full_bar[s], tx);
                     uint8_t* st = smem + s * stage_bytes;
-                    load_w(a.dbg, st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, &full_bar[s], pol_w);
+                    bulk_load(st, a.W + ((size_t)it.n_tile * a.total_kb + it.kb0 + kb) * GEMM_WTILE, GEMM_WTILE, &full_bar[s], pol_w);
                     ld_x(st, &full_bar[s], it.kb0 + kb, it);
                     if (++s == a.stages) { s = 0; ph ^= 1; }
                 }
@@ -345,13 +345,12 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             const uint32_t smem_base = smem_u32(smem);
             int s = 0;
             uint32_t ph = 0;
-            int n_it = 0;
             GemmWork wk;
             wk.init(a);
             GemmItem it;
             if (rank == 1) {
                 // pair, rank 1: no MMAs here; tell rank 0 when a stage of THIS CTA has landed
-                for (; wk.next(a, it); ++n_it) {
+                while (wk.next(a, it)) {
                     for (int kb = 0; kb < it.nkb; ++kb) {
                         mbar_wait(&full_bar[s], ph);
                         if (leader) mbar_arrive_remote(&peer_full_bar[s], 0);
@@ -360,44 +359,95 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     }
                 }
             } else {
-                for (; wk.next(a, it); ++n_it) {
-                    const int buf = n_it & 1;
-                    // epilogue (of both CTAs of a pair) has drained this accumulator
-                    if (PAIR) mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);
-                    else mbar_wait(&tmem_empty_bar[buf], ((n_it >> 1) & 1) ^ 1);
-                    tc_fence_after();
+                int n_acc = 0;   // accumulators handed to the epilogue so far (one per item, or one per K piece of an item)
+                while (wk.next(a, it)) {
                     const uint32_t idesc = umma_idesc_e4m3(PAIR ? 2 * GEMM_WROWS : GEMM_WROWS, it.tok);
-                    const uint32_t d_tmem = tmem_base + (uint32_t)(buf * a.tok);
-                    for (int kb = 0; kb < it.nkb; ++kb) {
-                        mbar_wait(&full_bar[s], ph);
-                        if (PAIR) mbar_wait(&peer_full_bar[s], ph);
+                    const int p = it.n_tile >> 1;
+                    int cc = cuts ? sk_first_cta(p * a.total_kb, a.cut_G, a.cut_U) : 0;
+                    for (int kb = 0; kb < it.nkb; ++cc, ++n_acc) {
+                        const int kb_end = cuts ? cut_end(a, p, cc) : it.nkb;
+                        const int buf = n_acc & 1;
+                        mbar_wait(&tmem_empty_bar[buf], ((n_acc >> 1) & 1) ^ 1);   // the epilogue (of both CTAs of a pair) has drained this accumulator
                         tc_fence_after();
-                        const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
-                        const uint64_t adesc = umma_desc_k128(wa);
-                        const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
-                        if (leader) {
-                            if (!(a.dbg & 4)) {
+                        const uint32_t d_tmem = tmem_base + (uint32_t)(buf * a.tok);
+                        for (const int kb0 = kb; kb < kb_end; ++kb) {
+                            mbar_wait(&full_bar[s], ph);
+                            if (PAIR) mbar_wait(&peer_full_bar[s], ph);
+                            tc_fence_after();
+                            const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
+                            const uint64_t adesc = umma_desc_k128(wa);
+                            const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
+                            if (leader) {
                                 if (PAIR) {
 #pragma unroll
                                     for (int k = 0; k < GEMM_BK / 32; ++k)
-                                        umma_f8_2cta(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                                        umma_f8_2cta(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, ((kb - kb0) | k) != 0);
+                                    umma_commit_2cta(&empty_bar[s]);
                                 } else {
 #pragma unroll
                                     for (int k = 0; k < GEMM_BK / 32; ++k)  // UMMA K = 32 E4M3 elements = 2 x 16 B
-                                        umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+                                        umma_f8(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, ((kb - kb0) | k) != 0);
+                                    umma_commit(&empty_bar[s]);
                                 }
                             }
-                            if (PAIR) umma_commit_2cta(&empty_bar[s]); else umma_commit(&empty_bar[s]);
+                            __syncwarp();
+                            if (++s == a.stages) { s = 0; ph ^= 1; }
                         }
+                        if (leader) { if (PAIR) umma_commit_2cta(&tmem_full_bar[buf]); else umma_commit(&tmem_full_bar[buf]); }
                         __syncwarp();
-                        if (++s == a.stages) { s = 0; ph ^= 1; }
                     }
-                    if (leader) {
-                        if (PAIR) umma_commit_2cta(&tmem_full_bar[buf]); else umma_commit(&tmem_full_bar[buf]);
-                        if (n_it == 0) TS(4);
-                    }
-                    __syncwarp();
                 }
+            }
+        }
+    } else if (SUM) {
+        // ===== running-sum epilogue (CTA pairs, raw output): warps 2..9; warp w may touch TMEM lanes 32*(w%4) .. +31 and
+        // takes one half of the item's token columns.  Every K piece of the item arrives as a fresh accumulator; the
+        // pieces are added in K order with single rounded fp32 additions - the additions the consumer of the stream-K
+        // slabs performs (lin_acc, ev_common.cuh) - and the item's sum is stored once. =====
+        pdl_wait();
+        const int q = warp & 3, half = (warp - 2) >> 2;
+        const int n_loc = q * 32 + lane;
+        int n_acc = 0;
+        GemmWork wk;
+        wk.init(a);
+        GemmItem it;
+        while (wk.next(a, it)) {
+            const int n = it.n_tile * GEMM_WROWS + n_loc;
+            const int ch = ((it.tok + 31) >> 5) << 4;            // columns per half, multiple of 16, <= 128
+            const int c_lo = half * ch;
+            const int ncols = max(0, min(it.tok, c_lo + ch) - c_lo);
+            const int p = it.n_tile >> 1;
+            int cc = cuts ? sk_first_cta(p * a.total_kb, a.cut_G, a.cut_U) : 0;
+            float acc[128];
+            bool first = true;
+            for (int kb = 0; kb < it.nkb; ++cc, ++n_acc, first = false) {
+                kb = cuts ? cut_end(a, p, cc) : it.nkb;
+                const int buf = n_acc & 1;
+                mbar_wait(&tmem_full_bar[buf], (n_acc >> 1) & 1);
+                tc_fence_after();
+                const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * a.tok + c_lo);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) {   // 32 columns per batch of loads
+                    uint32_t v[32];
+#pragma unroll
+                    for (int u = 0; u < 2; ++u)
+                        if (g * 32 + u * 16 < ncols) tmem_ld16(t_addr + (uint32_t)(g * 32 + u * 16), v + u * 16);
+                    tmem_ld_wait();
+                    if (g == 3) {  // accumulator fully read: hand it back to the MMA warp
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) { if (rank == 0) mbar_arrive(&tmem_empty_bar[buf]); else mbar_arrive_remote(&tmem_empty_bar[buf], 0); }
+                    }
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (g * 32 + (j & ~15) < ncols) acc[g * 32 + j] = first ? __uint_as_float(v[j]) : __fadd_rn(acc[g * 32 + j], __uint_as_float(v[j]));
+                }
+            }
+            if (n < a.N) {
+                float* outp = a.out + (size_t)(it.m0 + c_lo) * a.ldo + n;
+#pragma unroll
+                for (int j = 0; j < 128; ++j)
+                    if (j < ncols && it.m0 + c_lo + j < a.M) outp[(size_t)j * a.ldo] = acc[j];
             }
         }
     } else {  // ===== epilogue: warps 2..5; warp w may touch TMEM lanes 32*(w%4) .. +31 =====
@@ -425,7 +475,6 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
             }
             mbar_wait(&tmem_full_bar[buf], (n_it >> 1) & 1);
             tc_fence_after();
-            if (n_it == 0 && et == 0) TS(5);
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * a.tok);
             float* outp = a.out + (size_t)it.split * a.M * a.ldo;
             for (int g = 0; g < n_groups; ++g) {
@@ -465,7 +514,7 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                     for (int j = 0; j < GC; ++j) {
                         const int col = g * GC + j;
                         const int m = m0 + col;
-                        if (n_ok && col < tok && m < a.M && !(a.dbg & 64)) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
+                        if (n_ok && col < tok && m < a.M) outp[(size_t)m * a.ldo + n] = __uint_as_float(v[j]);
                     }
                 }
             }
@@ -482,30 +531,12 @@ __global__ void __launch_bounds__(GEMM_THREADS, 1) gemm_e4m3_kernel(const __grid
                 epi_bar_sync();  // keys_smem is rewritten by the next item
             }
         }
-        if (et == 0) TS(6);
     }
     tc_fence_before();
     __syncthreads();
     if (PAIR) cluster_barrier();   // no CTA of the pair exits (or frees its TMEM) while the pair's MMAs or arrives may still target it
     if (warp == 1) { if (PAIR) tmem_dealloc_rt2(tmem_base, tmem_cols); else tmem_dealloc_rt(tmem_base, tmem_cols); }
-    if (threadIdx.x == 32) TS(7);
     trace_exit(a.pf);
-}
-
-// debug / bring-up reference: same contraction on CUDA cores from the tiled weight layout (exact products,
-// fp32 accumulation), raw output like EPI_RAW.  Used only when EV_NAIVE_GEMM=1 to bisect tensor-core issues.
-__global__ void __launch_bounds__(128) gemm_e4m3_naive_kernel(const uint8_t* __restrict__ X, const uint8_t* __restrict__ Wt,
-                                                              int M, int N, int K, int total_kb, float* out, int ldo) {
-    const int n = blockIdx.x * 128 + threadIdx.x, m = blockIdx.y;
-    if (n >= N) return;
-    float acc = 0.f;
-    for (int k = 0; k < K; ++k) {
-        const uint8_t wc = Wt[((size_t)(n >> 7) * total_kb + (k >> 7)) * GEMM_WTILE + wtile_offset(n & 127, k & 127)];
-        const __half_raw hx = __nv_cvt_fp8_to_halfraw(X[(size_t)m * K + k], __NV_E4M3);
-        const __half_raw hw = __nv_cvt_fp8_to_halfraw(wc, __NV_E4M3);
-        acc = fmaf(__half2float(__half(hx)), __half2float(__half(hw)), acc);
-    }
-    out[(size_t)m * ldo + n] = acc;
 }
 
 // tiled+swizzled codes -> row-major [rows][cols] (ev_model_get_quantized)

@@ -149,3 +149,119 @@ def test_config3_b64_mixed_context_chain3_full_size():
 
 def test_config4_b8_L16384_tree60_static_scales_full_size():
     _run_config(wl.CONFIGS[4], sample_layers=[0, 16], sample_seqs=[7])
+
+
+# ---- GPU self-consistency at 8B shape ("guaranteeing to preserve accuracy"):
+# the GPU speculative loop emits exactly the tokens of GPU token-by-token greedy decoding, bit for bit.  Holds by
+# construction: every contraction's reduction order is a function of the token's own data (canonical K cuts of the
+# GEMMs, attention chunks at absolute key positions + per-row tail, segment-ordered RMSNorm sums).
+
+def _rank0_chain(parents):
+    """nodes whose every ancestor-or-self is the lowest-index child of its parent, by depth (root excluded)."""
+    first_child = {}
+    for i in range(1, len(parents)):
+        first_child.setdefault(int(parents[i]), i)
+    chain, cur = [], 0
+    while cur in first_child:
+        cur = first_child[cur]
+        chain.append(cur)
+    return chain
+
+
+def _lossless(spec, B, ctx, n_steps=8, planted_p=0.7):
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import run_verify
+    shape = spec.model
+    T = spec.n_nodes
+    parents = wl.chain_parents(T) if spec.tree_caps is None else wl.tree_parents(T, spec.tree_caps)
+    depth = int(wl.tree_depths(parents).max())
+    n_greedy = n_steps * (depth + 1) + depth + 1
+    model = ev.Model(shape, max_batch=2 * B, max_tree_nodes=64, max_ctx=int(max(ctx)) + n_greedy + 80, page_size=spec.page_size,
+                     act_scale_mode=spec.act_scale_mode)
+    for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
+        model.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
+    if spec.act_scale_mode == 1:
+        model.ev_model_calibrate(torch.from_numpy(wl.calibration_hidden(spec)).cuda())
+    cap = [int(L) + n_greedy + 72 for L in ctx]
+    cache = ev.Cache(model, 2 * sum(c // spec.page_size + 2 for c in cap) + cap[0] // spec.page_size + 2, 2 * B + 1)
+    s_slots = [cache.ev_cache_add_seq(c) for c in cap]     # speculative decoding
+    g_slots = [cache.ev_cache_add_seq(c) for c in cap]     # plain greedy decoding
+    ids = [wl.context_ids(spec, b, int(ctx[b])) for b in range(B)]
+    cache.ev_cache_prefill(s_slots + g_slots, ids + ids)
+    rng = np.random.default_rng(spec.seed + 77)
+    roots = rng.integers(0, shape.vocab, size=B).astype(np.int32)
+    # --- plain greedy: one token per sequence per step (M = B rows; sequence 0 also alone, M = 1: batch invariance)
+    greedy = np.zeros((B, n_greedy), dtype=np.int32)
+    tok = roots.copy()
+    one = np.full((B, 1), -1, dtype=np.int32)
+    for s in range(n_greedy):
+        buf = run_verify(model, cache, g_slots, tok[:, None], one, commit=True, want_logits=False, want_hidden=False)
+        assert (buf.status.cpu().numpy() == 0).all()
+        tok = buf.out_tokens.cpu().numpy()[:, 0].astype(np.int32)
+        greedy[:, s] = tok
+    # --- speculative loop with planted drafts
+    chain = _rank0_chain(parents)
+    emitted = [[] for _ in range(B)]
+    root = roots.copy()
+    total_acc = 0
+    for s in range(n_steps):
+        tokens = np.zeros((B, T), dtype=np.int32)
+        for b in range(B):
+            tk = rng.integers(0, shape.vocab, size=T).astype(np.int32)
+            tk[0] = root[b]
+            e = len(emitted[b])
+            for d, node in enumerate(chain):
+                if rng.random() < planted_p:
+                    tk[node] = greedy[b, e + d]
+            for i in range(1, T):      # siblings distinct (DESIGN.md R-tokens)
+                sib = [tk[j] for j in range(1, i) if parents[j] == parents[i]]
+                while tk[i] in sib:
+                    tk[i] = (tk[i] + 1) % shape.vocab
+            tokens[b] = tk
+        buf = run_verify(model, cache, s_slots, tokens, np.tile(parents, (B, 1)), commit=True, want_logits=False, want_hidden=False)
+        assert (buf.status.cpu().numpy() == 0).all()
+        acc = buf.accept_len.cpu().numpy()
+        outs = buf.out_tokens.cpu().numpy()
+        for b in range(B):
+            a = int(acc[b])
+            emitted[b] += outs[b, :a + 1].tolist()
+            root[b] = outs[b, a]
+            total_acc += a
+    for b in range(B):
+        n = len(emitted[b])
+        assert emitted[b] == greedy[b, :n].tolist(), (b, emitted[b], greedy[b, :n].tolist())
+    # the planted drafts were accepted about as often as planted (1 + sum p^d emitted per step; loose lower bound)
+    assert total_acc >= 0.5 * B * n_steps * planted_p, total_acc
+    # compacted cache == cache of plain decoding, bit for bit (all layers), for sequence 0
+    n0 = int(ctx[0]) + len(emitted[0])
+    a = cache.ev_cache_export_seq(s_slots[0], 0, shape.n_layers, n0)
+    g = cache.ev_cache_export_seq(g_slots[0], 0, shape.n_layers, n0)
+    assert torch.equal(a.view(torch.int16), g.view(torch.int16))
+    # sequence 0 decoded ALONE (M = 1) gives the same tokens as in the batch of B
+    if B > 1:
+        solo = cache.ev_cache_add_seq(cap[0])
+        cache.ev_cache_prefill([solo], [ids[0]])
+        tok1 = roots[:1].copy()
+        for s in range(8):
+            buf = run_verify(model, cache, [solo], tok1[:, None], one[:1], commit=True, want_logits=False, want_hidden=False)
+            tok1 = buf.out_tokens.cpu().numpy()[:, 0].astype(np.int32)
+            assert int(tok1[0]) == int(greedy[0, s]), s
+    print(f"lossless {spec.name}: {sum(len(e) for e in emitted)} tokens emitted in {n_steps} steps x {B} sequences, {total_acc} drafts accepted")
+
+
+def test_config1_gpu_speculative_equals_gpu_greedy():
+    _lossless(wl.CONFIGS[1], 1, [2048])
+
+
+def test_config2_gpu_speculative_equals_gpu_greedy():
+    _lossless(wl.CONFIGS[2], 4, [4096, 4096, 4096, 4096])
+
+
+def test_config3_gpu_speculative_equals_gpu_greedy():
+    spec = wl.CONFIGS[3]
+    ctx = wl.context_lengths(spec)
+    _lossless(spec, 4, [int(ctx[0]), int(ctx[1]), int(ctx.min()), int(ctx.max())])
+
+
+def test_config4_gpu_speculative_equals_gpu_greedy():
+    _lossless(wl.CONFIGS[4], 2, [16384, 16384])

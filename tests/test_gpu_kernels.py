@@ -104,7 +104,7 @@ def tiny_gpu_many_rows():
 def test_fp8_gemm_many_rows(tiny_gpu_many_rows, kind, M):
     """M > 256: several token tiles, no split-K.  Even numbers of 128-channel tiles (QKV 4, O 2, down 2, LM head 8)
     run as multicast CTA pairs (each CTA fetches half of the token tile for both; odd halves at M = 300 / 831);
-    gate|up (11 tiles, ragged) takes the single-CTA path.  LM head: logits and the argmax keys' epilogue."""
+    gate|up (11 tiles, ragged, stored as 12) too.  LM head: logits and the argmax keys' epilogue."""
     shape = wl.TINY
     K = {"wq": 256, "wo": 256, "wgate": 256, "wdown": 688, "lm_head": 256}[kind]
     rng = np.random.default_rng(M + 17)
@@ -129,8 +129,6 @@ def test_fp8_gemm_accumulation_error_at_8b_k():
     shape = wl.ModelShape("k8b", 1, 4096, 4, 2, 128, 14336, 1024, 1e-5, 5e5)
     m = ev.Model(shape, 1, 64, 128)
     rng = np.random.default_rng(0)
-    for kind, K, N in (("wo", 512, 4096), ("wdown", 14336, 4096), ("wq", 4096, 1024)):
-        pass
     # O-proj has K = q_dim = 512 here; use QKV (K = 4096) and down (K = 14336)
     report = {}
     for kind, K in (("wq", 4096), ("wdown", 14336)):
@@ -187,3 +185,45 @@ def test_per_tensor_weight_scales_bit_exact_and_verify_parity():
         assert rel_l2(hid[l, :spec.n_nodes], h_ref) <= 1e-2
     lg = buf.logits.cpu().numpy()[:spec.n_nodes]
     assert np.max(np.abs(lg - res["logits"])) <= 2e-2 * float(res["logits"].std())
+
+
+def test_fp8_gemm_batch_invariant_and_exact_at_8b_k():
+    """A token's linear output may not depend on how many tokens share the launch (PAPER.md:92 losslessness needs
+    verify == decode; DESIGN.md section 6 "canonical K cuts"): rows computed at M = 1, 16, 60, 256 (stream-K slabs,
+    single CTAs) equal, bit for bit, the same rows inside an M = 832 launch (cta_group::2 pairs with the running-sum
+    epilogue), at 8B K (4096 / 14336) for QKV, O, gate|up, down and the LM head, wherever the row sits in the batch.
+    The M = 832 pair path and the balanced LM head are also held to the <= 1e-5 GEMM bar against the oracle's exact
+    sums on sampled rows x all channels."""
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import bf16_cuda_to_bits
+    shape = wl.ModelShape("k8b1", 1, 4096, 32, 8, 128, 14336, 8192, 1e-5, 5e5)
+    m = ev.Model(shape, 32, 32, 256)
+    host = {}
+    for kind in ("embed", "wq", "wk", "wv", "wo", "wgate", "wup", "wdown", "lm_head"):
+        w = wl.weight_matrix_bf16(shape, 7, kind, 0, device="cuda")
+        m.ev_model_set_weight(kind, 0, w)
+        if kind != "embed":
+            host[kind] = bf16_cuda_to_bits(w)
+    g = torch.Generator(device="cuda")
+    g.manual_seed(1)
+    rows = [0, 59, 207, 208, 415, 831]
+    for kind, K, names in (("lm_head", 4096, ("lm_head",)), ("wq", 4096, ("wq", "wk", "wv")), ("wo", 4096, ("wo",)),
+                           ("wgate", 4096, ("wgate", "wup")), ("wdown", 14336, ("wdown",))):
+        x = torch.randn((832, K), generator=g, device="cuda") * torch.exp(torch.randn((832, 1), generator=g, device="cuda"))
+        codes, sx = m.ev_op_quantize_rows(x)
+        y_big = m.ev_op_linear(kind, 0, codes, sx).clone()
+        for M in (1, 16, 60, 256):
+            y = m.ev_op_linear(kind, 0, codes[:M].contiguous(), sx[:M].contiguous())
+            assert torch.equal(y, y_big[:M]), (kind, M, int((y != y_big[:M]).sum()))
+        perm = torch.arange(832, device="cuda").roll(300)
+        y_p = m.ev_op_linear(kind, 0, codes[perm].contiguous(), sx[perm].contiguous())
+        assert torch.equal(y_p, y_big[perm]), kind
+        y_mid = m.ev_op_linear(kind, 0, codes[100:400].contiguous(), sx[100:400].contiguous())   # M = 300: two token tiles of 160
+        assert torch.equal(y_mid, y_big[100:400]), kind
+        ws = [vo.quantize_weight(host[k]) for k in names]
+        wq = np.concatenate([w[0] for w in ws])
+        sw = np.concatenate([w[1] for w in ws])
+        ref = vo.linear(codes[rows].cpu().numpy(), sx[rows].cpu().numpy(), wq, sw)
+        got = y_big[rows].cpu().numpy()
+        assert rel_l2(got, ref) < 1e-5, (kind, rel_l2(got, ref))
+        assert np.max(np.abs(got - ref)) <= 1e-5 * np.max(np.abs(ref)) + 1e-7, kind
