@@ -123,24 +123,66 @@ def quantize_rows(x, static_scale=None):
     return codes, s
 
 
+ACCUM_MODES = ("exact", "f32", "f32perm", "f32seq")
+
+
+def _perm_k(K):
+    """The fixed permutation of the K axis used by accum="f32perm" (seeded by K only)."""
+    return np.random.Generator(np.random.PCG64(np.random.SeedSequence([0x5EED, K]))).permutation(K)
+
+
 def linear(xq, s_x, wq, s_w, accum="exact", n_block=8192):
     """W8A8 linear, DESIGN.md R-accum:
     y[m,n] = fp32( sum_k decode(xq[m,k]) * decode(wq[n,k]) ) * s_x[m] * s_w[n],
     the sum exact (fp64) and rounded once, the two scales applied left to right in fp32.
-    accum="f32" replaces the exact sum by a library fp32 matmul (noise-floor study only).
+    The other accumulation modes exist for the noise-floor study only (SURVEY section 8(c)-6 item 1, 8(c)-7 `--accum`;
+    DESIGN.md R-noise): they are what an honest fp32-accumulating implementation may compute instead of the exact sum:
+      "f32"     a library fp32 GEMM (its own blocked summation order);
+      "f32perm" the same library GEMM with the K axis of both operands permuted by one fixed permutation (a second,
+                unrelated fp32 summation order);
+      "f32seq"  strictly sequential fp32 accumulation over k ascending (slow: small cases and pins).
     The loop over n_block output channels bounds memory; it splits no reduction."""
+    assert accum in ACCUM_MODES, accum
     M, K = xq.shape
     N = wq.shape[0]
     x64 = _LUT64[xq]
     y = np.empty((M, N), dtype=F32)
+    perm = _perm_k(K) if accum == "f32perm" else None
     for n0 in range(0, N, n_block):
         w64 = _LUT64[wq[n0:n0 + n_block]]
         if accum == "exact":
             acc = _matmul64(x64, w64).astype(F32)
-        else:
+        elif accum == "f32":
             acc = (x64.astype(F32) @ w64.astype(F32).T).astype(F32)
+        elif accum == "f32perm":
+            acc = (np.ascontiguousarray(x64[:, perm].astype(F32)) @ np.ascontiguousarray(w64[:, perm].astype(F32)).T).astype(F32)
+        else:
+            x32, w32 = x64.astype(F32), w64.astype(F32)
+            acc = np.zeros((M, w32.shape[0]), dtype=F32)
+            for k in range(K):    # every product is exact in fp32; one rounded fp32 addition per k
+                acc = (acc + x32[:, k, None] * w32[None, :, k]).astype(F32)
         y[:, n0:n0 + n_block] = (acc * s_x[:, None].astype(F32)) * s_w[None, n0:n0 + n_block].astype(F32)
     return y
+
+
+# ----------------------------------------------------------------------------- perturbation injection
+
+ROUND_MODES = {"bf16": 8, "tf32": 11, "split16": 16}   # significand bits kept (implicit one included)
+ROUND_SITES = ("resid", "prequant", "qp")
+
+
+def round_sig(x, bits):
+    """fp32 -> nearest value with `bits` significand bits (round to nearest, ties to even), as fp32.  bits = 8 is bf16,
+    11 is tf32's operand precision, 16 is what a hi+lo pair of bf16 holds.  Used ONLY by the perturbation-injection
+    switches (SURVEY section 8(c)-6/7 `--round <site>:bf16|tf32|split16`; DESIGN.md R-noise); the default oracle never
+    rounds anywhere but at the E4M3 quantizers and the bf16 K/V."""
+    drop = 24 - bits
+    u = np.ascontiguousarray(x, dtype=F32).view(np.uint32)
+    if drop <= 0:
+        return u.view(F32).copy()
+    lsb = (u >> np.uint32(drop)) & np.uint32(1)
+    r = (u + np.uint32((1 << (drop - 1)) - 1) + lsb) & np.uint32((0xFFFFFFFF << drop) & 0xFFFFFFFF)
+    return r.view(F32)
 
 
 # ----------------------------------------------------------------------------- element ops
@@ -201,7 +243,7 @@ def node_depths(parents):
     return d
 
 
-def tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents):
+def tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents, qp_bits=None):
     """Tree attention: node i attends to the L committed context positions and to
     its own ancestors-or-self among the tree nodes; GQA: q-head h uses kv-head h // (Hq/Hkv).
     q [T,Hq,d] fp32; k_*/v_* hold bf16 values (as fp32): ctx [L,Hkv,d], tree [T,Hkv,d].
@@ -210,6 +252,8 @@ def tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents):
     T, Hq, d = q.shape
     Hkv = k_tree.shape[1]
     G = Hq // Hkv
+    if qp_bits is not None:      # perturbation injection "qp": Q and P rounded as a tensor-core attention would hold them
+        q = round_sig(q, qp_bits)
     scale = (F32(1.0) / np.sqrt(F32(d))).astype(F32)
     anc = ancestor_mask(parents)
     out = np.empty((T, Hq, d), dtype=F32)
@@ -224,6 +268,8 @@ def tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents):
             m = np.max(s, axis=1, keepdims=True)
             p = np.exp((s - m).astype(F32).astype(np.float64)).astype(F32)
             l = np.sum(p.astype(np.float64), axis=1).astype(F32)
+            if qp_bits is not None:
+                p = round_sig(p, qp_bits)
             o = (p.astype(np.float64) @ vals).astype(F32)
             out[:, h, :] = (o / l[:, None]).astype(F32)
     return out.reshape(T, Hq * d)
@@ -246,6 +292,7 @@ class OracleModel:
         self.act_scale_mode = act_scale_mode
         self.weight_scale_mode = weight_scale_mode   # 0 per output channel, 1 per tensor (each matrix its own scale)
         self.accum = accum
+        self.inject = {}     # perturbation injection: site in ROUND_SITES -> significand bits (empty = none, the default)
         self.w = {}          # (kind, layer) -> (codes, scales)
         self.embed = None    # bf16 bits [V, H]
         self.gain = {}       # ("norm1"|"norm2", layer) / ("normf", 0) -> fp32 [H]
@@ -267,7 +314,20 @@ class OracleModel:
         g = self.gain.get((kind, layer))
         return g if g is not None else np.ones(self.hidden, dtype=F32)
 
+    def set_round(self, spec):
+        """spec: "" or "<site>:<mode>[,<site>:<mode>...]" with site in ROUND_SITES, mode in ROUND_MODES."""
+        self.inject = {}
+        for item in filter(None, (spec or "").split(",")):
+            site, mode = item.split(":")
+            assert site in ROUND_SITES and mode in ROUND_MODES, item
+            self.inject[site] = ROUND_MODES[mode]
+
+    def _inj(self, x, site):
+        b = self.inject.get(site)
+        return x if b is None else round_sig(x, b)
+
     def _quant(self, x, site, layer, record=None):
+        x = self._inj(x, "prequant")
         if record is not None:   # calibration pass: dynamic scales, remember per-site absmax
             record[(site, layer)] = max(record.get((site, layer), 0.0), float(np.max(np.abs(x))))
             return quantize_rows(x)
@@ -367,16 +427,16 @@ def layer_forward(model, layer, h, cache, seq, L, parents, record=None, taps=Non
     cache.write(layer, seq, [L + i for i in range(T)], k, v)          # rounds to bf16
     k_ctx, v_ctx = cache.read(layer, seq, 0, L)
     k_tree, v_tree = cache.read(layer, seq, L, L + T)
-    attn = tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents)
+    attn = tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents, qp_bits=model.inject.get("qp"))
     aq, sa = model._quant(attn, "o_in", layer, record)
-    h = (h + model._lin(aq, sa, "wo", layer)).astype(F32)
+    h = model._inj((h + model._lin(aq, sa, "wo", layer)).astype(F32), "resid")
     x2 = rmsnorm(h, model._gain("norm2", layer), model.rms_eps)
     x2q, s2 = model._quant(x2, "gateup_in", layer, record)
     g = model._lin(x2q, s2, "wgate", layer)
     u = model._lin(x2q, s2, "wup", layer)
     t = swiglu(g, u)
     tq, st = model._quant(t, "down_in", layer, record)
-    h_out = (h + model._lin(tq, st, "wdown", layer)).astype(F32)
+    h_out = model._inj((h + model._lin(tq, st, "wdown", layer)).astype(F32), "resid")
     if taps is not None:
         taps.update(dict(x=x, xq=xq, sx=sx, q=q, k=k, v=v, attn=attn, aq=aq, sa=sa, h_mid=h,
                          x2q=x2q, s2=s2, g=g, u=u, t=t, tq=tq, st=st))

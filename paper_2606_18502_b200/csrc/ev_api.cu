@@ -670,7 +670,10 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         aa.anc_bulk = m->anc_bulk; aa.erow = m->erow; aa.kend_seq = m->kend_seq;
         aa.chunk = split_len; aa.n_chunks = n_splits; aa.scale = 1.0f / sqrtf((float)D);
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
-        dim3 agrid(n_splits, cfg.n_kv_heads * row_groups, B);
+        // chunks per CTA (tcgen05 kernel): about four CTAs per SM-slot over the launch; a scheduling choice only
+        const long units = (long)B * cfg.n_kv_heads * row_groups;
+        aa.cpg = c->kv_f16 ? (int)std::min<long>(n_splits, std::max<long>(1, units * n_splits / (4L * m->num_sms))) : 1;
+        dim3 agrid((n_splits + aa.cpg - 1) / aa.cpg, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
             if (c->kv_f16) {
@@ -827,7 +830,9 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(alloc_actbuf(m, &m->tq, F));
     A(dev_alloc(m, &m->qkv, (size_t)m->M_pad * m->qkv_dim));
     A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
-    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : 1024;
+    // default chunk length: short for models built for one or two sequences (every chunk is its own CTA: latency), long
+    // for batched serving (fewer partial outputs per row); a function of the config only, hence fixed for the model's life
+    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : (cfg->max_batch <= 2 ? 256 : (cfg->max_ctx <= 10240 ? 1024 : 2048));
     m->n_chunks_max = (cfg->max_ctx + m->attn_chunk - 1) / m->attn_chunk;
     A(dev_alloc(m, &m->o_part, (size_t)m->M_cap * m->n_chunks_max * m->q_dim));
     A(dev_alloc(m, &m->ml_part, (size_t)m->M_cap * m->n_chunks_max * cfg->n_q_heads * 2));

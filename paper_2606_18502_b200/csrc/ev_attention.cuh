@@ -49,7 +49,8 @@ struct AttnArgs {
     const int32_t* erow;        // [B][T] cached positions below erow[row] are bulk keys of the row
     const int32_t* kend_seq;    // [B] one past the last bulk key slot of the sequence
     int chunk;                  // keys per chunk, multiple of ATT_CH: a constant of the model, NOT a function of the batch
-    int n_chunks;               // grid.x = chunks the grid covers; stride of the partial arrays
+    int n_chunks;               // chunks the grid covers; stride of the partial arrays
+    int cpg;                    // consecutive chunks one CTA walks (grid.x = ceil(n_chunks / cpg)); a scheduling choice, no effect on results
     float scale;                // 1/sqrt(D)
     float* o_part;              // [M][Hq][n_chunks][D]
     float* ml_part;             // [M][Hq][n_chunks][2]  (running max, running sum)
@@ -109,7 +110,7 @@ __global__ void __launch_bounds__(ATT_THREADS, 1) tree_attn_partial_kernel(AttnA
     const int seq_slot = a.seq_slots[b];
     const int n_keys = a.kend_seq[b];
     if (nn == 0) return;
-    const int k_begin = split * a.chunk;
+    const int k_begin = split * a.chunk;   // this kernel: one chunk per CTA (cpg == 1)
     if (k_begin >= n_keys) return;
     const int k_end = min(k_begin + a.chunk, n_keys);
     const int n_chunks = (k_end - k_begin + ATT_CH - 1) / ATT_CH;
@@ -350,23 +351,23 @@ struct MergeArgs {
     QuantOut q;
     L2Prefetch pf;
 };
-__device__ __forceinline__ float4 kv_load4(const __nv_bfloat16* p, int kv_f16) {   // 4 consecutive K or V elements as fp32
-    const uint2 w = *reinterpret_cast<const uint2*>(p);
+constexpr int MERGE_THREADS = 256;   // = ROW_THREADS (ev_elementwise.cuh): Hq * D <= 4 * 256 * NV4 * cluster size
+__device__ __forceinline__ float4 kv_cvt4(uint2 w, int kv_f16) {   // 4 consecutive K or V elements (raw pool bits) as fp32
     if (kv_f16) {
         const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&w.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&w.y));
         return make_float4(a.x, a.y, b.x, b.y);
     }
     return make_float4(__uint_as_float(w.x << 16), __uint_as_float(w.x & 0xFFFF0000u), __uint_as_float(w.y << 16), __uint_as_float(w.y & 0xFFFF0000u));
 }
-constexpr int MERGE_THREADS = 256;   // = ROW_THREADS (ev_elementwise.cuh): Hq * D <= 4 * 256 * NV4 * cluster size
 template <int MERGE_NV4>
-__global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeArgs a) {
+__global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(MergeArgs a) {
     pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
     l2_prefetch_issue(a.pf);
     pdl_wait();
     trace_past_wait(a.pf);
     __shared__ float red[MERGE_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
+    __shared__ long long tbase[ATT_TAIL_MAX];   // element offset of the tail key's K row (kv head 0, dim 0) in this layer's pool
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     const int b = m / a.T, node = m % a.T;
     const int nn = a.nn_eff[b];
@@ -378,9 +379,24 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
     // tail keys, in position order: n_ctx cached slots e .. L-1, then the ancestors of the tail (lowest node index = lowest depth first)
     const int n_ctx = valid ? min(max(0, L - e), ATT_TAIL_MAX) : 0;
     const unsigned long long anc_tail = valid ? (a.anc[m] & ~a.anc_bulk[m]) : 0ull;
+#ifdef EXP_NOTAIL
+    const int nt = 0;
+#else
     const int nt = min(n_ctx + __popcll(anc_tail), ATT_TAIL_MAX);
-    const int32_t* pt = a.page_table + (size_t)(valid ? a.seq_slots[b] : 0) * a.max_pages;
+#endif
     const size_t kv_stride = (size_t)a.Hkv * a.page_size * D;   // K block -> V block of a page
+    if ((int)threadIdx.x < nt) {
+        const int u = threadIdx.x;
+        int sl = e + u;
+        if (u >= n_ctx) {   // the (u - n_ctx)-th set bit of anc_tail
+            unsigned long long at = anc_tail;
+            for (int i = n_ctx; i < u; ++i) at &= at - 1;
+            sl = L + __ffsll((long long)at) - 1;
+        }
+        const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+        tbase[u] = (long long)((size_t)pt[sl / a.page_size] * 2 * kv_stride + (size_t)(sl % a.page_size) * D);
+    }
+    __syncthreads();
     const int G = a.Hq / a.Hkv;
     const int gl = D / 4;   // lanes per head group (32 or 16)
     float4 v[MERGE_NV4];
@@ -395,32 +411,32 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
         const int h = on ? i / D : 0, d = on ? i % D : 0;
         const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * D + d;
         const float* mlp = a.ml_part + ((size_t)m * a.Hq + h) * S * 2;
-        // chunk partials are requested first: the tail scoring below runs under these loads
+        // every load of this float4 is requested before the first use: chunk partials, q, the tail keys' K and V
         constexpr int NB = 4;
         float4 t0[NB];
         float2 ml0[NB];
+        uint2 kr[ATT_TAIL_MAX], vr[ATT_TAIL_MAX];
+        float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        const size_t hoff = (size_t)(h / G) * a.page_size * D + d;
+#pragma unroll
+        for (int u = 0; u < ATT_TAIL_MAX; ++u) {
+            kr[u] = make_uint2(0u, 0u); vr[u] = make_uint2(0u, 0u);
+            if (on && u < nt) {
+                const __nv_bfloat16* kp = a.pool + tbase[u] + hoff;
+                kr[u] = *reinterpret_cast<const uint2*>(kp);              // L1-cached: the G query heads of a kv head read the same rows
+                vr[u] = *reinterpret_cast<const uint2*>(kp + kv_stride);
+            }
+        }
+        if (on) q4 = *reinterpret_cast<const float4*>(a.qkv + (size_t)m * a.q_ld + i);
 #pragma unroll
         for (int u = 0; u < NB; ++u)
             if (on && u < ns) { t0[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)u * D)); ml0[u] = __ldcg(reinterpret_cast<const float2*>(mlp + 2 * u)); }
-        // (1) tail scores
-        float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (on) q4 = *reinterpret_cast<const float4*>(a.qkv + (size_t)m * a.q_ld + i);
-        const int kvh = h / G;
+        // (1) tail scores: fixed FMA chain over the lane's 4 dims, xor butterfly over the head group, times 1/sqrt(d)
         float ts[ATT_TAIL_MAX];
-        float4 tv[ATT_TAIL_MAX];
-        unsigned long long at = anc_tail;
 #pragma unroll
         for (int u = 0; u < ATT_TAIL_MAX; ++u) {
-            float part = 0.f;
-            tv[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-            int sl = e + u;
-            if (u >= n_ctx && u < nt) { sl = L + __ffsll((long long)at) - 1; at &= at - 1; }
-            if (on && u < nt) {
-                const __nv_bfloat16* kp = a.pool + (size_t)pt[sl / a.page_size] * 2 * kv_stride + ((size_t)kvh * a.page_size + sl % a.page_size) * D + d;
-                const float4 k4 = kv_load4(kp, a.kv_f16);
-                tv[u] = kv_load4(kp + kv_stride, a.kv_f16);
-                part = fmaf(q4.w, k4.w, fmaf(q4.z, k4.z, fmaf(q4.y, k4.y, __fmul_rn(q4.x, k4.x))));
-            }
+            const float4 k4 = kv_cvt4(kr[u], a.kv_f16);
+            float part = fmaf(q4.w, k4.w, fmaf(q4.z, k4.z, fmaf(q4.y, k4.y, __fmul_rn(q4.x, k4.x))));
             for (int o = gl >> 1; o > 0; o >>= 1) part = __fadd_rn(part, __shfl_xor_sync(0xffffffffu, part, o));
             ts[u] = mul_rn(part, a.scale);
         }
@@ -462,8 +478,9 @@ __global__ void __launch_bounds__(MERGE_THREADS) attn_merge_quant_kernel(MergeAr
             for (int u = 0; u < ATT_TAIL_MAX; ++u)
                 if (u < nt) {
                     const float et = expf(ts[u] - mx);
+                    const float4 v4 = kv_cvt4(vr[u], a.kv_f16);
                     den = __fadd_rn(den, et);
-                    num.x = fmaf(et, tv[u].x, num.x); num.y = fmaf(et, tv[u].y, num.y); num.z = fmaf(et, tv[u].z, num.z); num.w = fmaf(et, tv[u].w, num.w);
+                    num.x = fmaf(et, v4.x, num.x); num.y = fmaf(et, v4.y, num.y); num.z = fmaf(et, v4.z, num.z); num.w = fmaf(et, v4.w, num.w);
                 }
             v[k] = make_float4(div_rn(num.x, den), div_rn(num.y, den), div_rn(num.z, den), div_rn(num.w, den));
             if (a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];

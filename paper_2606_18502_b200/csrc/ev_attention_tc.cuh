@@ -201,9 +201,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     const int L = a.Lsnap[b];
     const int seq_slot = a.seq_slots[b];
     const int n_keys = a.kend_seq[b];                  // one past the last bulk key slot of the sequence (tree_prep_kernel)
-    const int k_begin = split * a.chunk;               // chunks sit at absolute key positions: batch-invariant (ev_attention.cuh)
+    // This CTA walks a.cpg consecutive chunks; chunks sit at absolute key positions and each is reduced from a fresh
+    // softmax state (batch-invariant, ev_attention.cuh), so how many chunks a CTA takes changes no result: the K/V
+    // stream and the MMAs simply run on across chunk boundaries, the softmax / correction warps restart their state.
+    const int chunk0 = split * a.cpg;
+    const int tpc = a.chunk / TCA_BN;                  // tiles per chunk
+    const int k_begin = chunk0 * a.chunk;
     const bool active = nn != 0 && k_begin < n_keys;   // uniform over the CTA
-    const int k_end = min(k_begin + a.chunk, n_keys);
+    const int k_end = min(k_begin + a.cpg * a.chunk, n_keys);
     const int n_tiles = active ? (k_end - k_begin + TCA_BN - 1) / TCA_BN : 0;
     // ---- Q tile -> TMEM (fp32 x 2^6 -> hi | lo fp16 pairs).  Softmax and correction threads stage it: a warp owns the
     // TMEM lanes of its 32 rows.  Warps 1..17 meet behind named barrier 5; warp 0 goes straight to its K/V
@@ -359,6 +364,10 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         float m_run = -INFINITY, l_run = 0.f;   // l_run carries P's factor 2^15
         const float qk_scale = a.scale * (1.f / TCA_QSCALE);
 
+        // (max, sum) of a finished chunk go to its partial slot (the two halves of a row meet in shared memory) and the
+        // state restarts: t_left counts the tiles left in the current chunk
+        float2* mlp = reinterpret_cast<float2*>(a.ml_part) + ((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0;
+        int t_left = tpc;
         for (int j = 0; j < n_tiles; ++j) {
             mbar_wait(&s_full[j % C::NSP], (j / C::NSP) & 1);
             tc_fence_after();
@@ -416,14 +425,14 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
-        }
-        // ---- running max and sum of this split ----
-        l_run *= exp2f(-TCA_PSCALE_LOG2);   // exact
-        xsum[wg * 128 + r] = l_run;
-        if (warp_valid) pair_bar_sync(1 + (warp & 3));
-        if (valid && wg == 0) {
-            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_chunks + split;
-            *reinterpret_cast<float2*>(a.ml_part + pi * 2) = make_float2(m_run, l_run + xsum[128 + r]);
+            if (--t_left == 0 || j == n_tiles - 1) {   // chunk finished (CTA-uniform)
+                xsum[wg * 128 + r] = l_run * exp2f(-TCA_PSCALE_LOG2);   // exact
+                pair_bar_sync(1 + (warp & 3));
+                if (valid && wg == 0) *mlp = make_float2(m_run, xsum[r] + xsum[128 + r]);
+                ++mlp;
+                m_run = -INFINITY; l_run = 0.f;
+                t_left = tpc;
+            }
         }
     } else {
         // ===== correction: thread = (row, half of d).  O = O * c(i) + Oc(i), one rounded fp32 operation per tile;
@@ -438,6 +447,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         float o[C::DH];
 #pragma unroll
         for (int i = 0; i < C::DH; ++i) o[i] = 0.f;
+        float* op = a.o_part + (((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0) * D + hh * C::DH;
+        int t_left = tpc;
         for (int i = 0; i < n_tiles; ++i) {
             mbar_wait(&o_full[i % C::NO], (i / C::NO) & 1);
             tc_fence_after();
@@ -447,6 +458,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 if (lane == 0) mbar_arrive(&o_empty[i % C::NO]);
                 continue;
             }
+            const bool last = --t_left == 0 || i == n_tiles - 1;   // the key chunk ends with this tile (CTA-uniform)
             const float c = xc[(i & 7) * 128 + r];
 #pragma unroll
             for (int cb = 0; cb < C::DH / 16; ++cb) {
@@ -460,15 +472,18 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                 }
 #pragma unroll
                 for (int e = 0; e < 16; ++e) o[cb * 16 + e] = fmaf(o[cb * 16 + e], c, __uint_as_float(ov[e]));
+                if (last) {   // the chunk's partial output goes out (P's factor 2^15 taken out exactly), fresh accumulator
+                    if (valid) {
+#pragma unroll
+                        for (int e = 0; e < 16; e += 4)
+                            *reinterpret_cast<float4*>(op + cb * 16 + e) = make_float4(o[cb * 16 + e] * exp2f(-TCA_PSCALE_LOG2), o[cb * 16 + e + 1] * exp2f(-TCA_PSCALE_LOG2),
+                                                                                       o[cb * 16 + e + 2] * exp2f(-TCA_PSCALE_LOG2), o[cb * 16 + e + 3] * exp2f(-TCA_PSCALE_LOG2));
+                    }
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) o[cb * 16 + e] = 0.f;
+                }
             }
-        }
-        if (valid) {
-            const size_t pi = ((size_t)(b * a.T + node) * a.Hq + kvh * a.G + gi) * a.n_chunks + split;
-            float* op = a.o_part + pi * D + hh * C::DH;
-#pragma unroll
-            for (int i = 0; i < C::DH; ++i) o[i] *= exp2f(-TCA_PSCALE_LOG2);   // P's factor 2^15, exact
-#pragma unroll
-            for (int i = 0; i < C::DH; i += 4) *reinterpret_cast<float4*>(op + i) = make_float4(o[i], o[i + 1], o[i + 2], o[i + 3]);
+            if (last) { op += D; t_left = tpc; }
         }
     }
     tc_fence_before();
