@@ -37,6 +37,31 @@ def peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, source="fallback")  # B200_PROFILING.md fallback
 
 
+def fp8_peak_probe(torch):
+    """Dense E4M3 tensor peak of THIS GPU, measured the way MEASURED_PEAKS.json measures its bf16 figure:
+    an 8192^3 E4M3 matmul through torch._scaled_mm, best of 10 (burst).  A probe outside the product path: it only sets
+    the FLOP roofline's denominator.  Falls back to 2 x the measured bf16 burst when the probe is unavailable."""
+    try:
+        a = torch.randn(8192, 8192, device="cuda").to(torch.float8_e4m3fn)
+        b = torch.randn(8192, 8192, device="cuda").to(torch.float8_e4m3fn).t()
+        one = torch.tensor(1.0, device="cuda")
+        for _ in range(3):
+            torch._scaled_mm(a, b, scale_a=one, scale_b=one, out_dtype=torch.bfloat16)
+        best = 1e9
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            torch._scaled_mm(a, b, scale_a=one, scale_b=one, out_dtype=torch.bfloat16)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        del a, b
+        torch.cuda.empty_cache()
+        return 2 * 8192 ** 3 / (best * 1e-3), "measured: torch._scaled_mm 8192^3 E4M3, best of 10 (probe outside the product path)"
+    except Exception as e:  # pragma: no cover
+        return 2 * peaks()["bf16_tflops"] * 1e12, f"2 x bf16 burst (E4M3 probe unavailable: {type(e).__name__})"
+
+
 # ------------------------------------------------------------------------------------------ workload
 
 def tree_of(spec):
@@ -86,12 +111,41 @@ class ClockSampler(threading.Thread):
         return dict(sm_mhz=sm[len(sm) // 2], sm_max_mhz=float(self.rows[0][2]), reasons=reasons, samples=len(self.rows))
 
 
-def build_gpu_workload(spec, steps_total, torch, ev, log):
+def rank0_chain(parents):
+    """the nodes reached from the root by always taking the lowest-index child, by depth"""
+    first_child = {}
+    for i in range(1, len(parents)):
+        first_child.setdefault(int(parents[i]), i)
+    chain, cur = [], 0
+    while cur in first_child:
+        cur = first_child[cur]
+        chain.append(cur)
+    return chain
+
+
+def plant(spec, parents, b, root, greedy_next, coins):
+    """Draft tokens of one tree (DESIGN.md R-tokens): uniform ids with distinct siblings, the root given, and on the rank-0
+    chain the GPU's own greedy continuation with probability 0.7 per depth (config[3]'s rule): coins[d] < 0.7 plants."""
+    tk = wl.draft_tokens_uniform(spec, parents, b)
+    tk[0] = root
+    for d, node in enumerate(rank0_chain(parents)):
+        if coins[d] < 0.7:
+            tk[node] = greedy_next[d]
+    for i in range(1, len(tk)):        # planting may have collided with a sibling
+        sib = [tk[j] for j in range(1, i) if parents[j] == parents[i]]
+        while tk[i] in sib:
+            tk[i] = (tk[i] + 1) % spec.model.vocab
+    return tk
+
+
+def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0):
     shape = spec.model
     B, T = spec.batch, spec.n_nodes
     parents = tree_of(spec)
     ctx = wl.context_lengths(spec)
-    max_ctx = int(ctx.max()) + 64 + 8
+    D0 = int(wl.tree_depths(parents).max())
+    grow = loop_steps * (D0 + 1) + D0 + 1 if loop_steps else 0     # tokens a sustained loop may append
+    max_ctx = int(ctx.max()) + 64 + 8 + grow
     t0 = time.time()
     model = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=max_ctx, page_size=spec.page_size,
                      act_scale_mode=spec.act_scale_mode)
@@ -103,9 +157,9 @@ def build_gpu_workload(spec, steps_total, torch, ev, log):
         calib = torch.from_numpy(wl.calibration_hidden(spec)).cuda()
         model.ev_model_calibrate(calib)
         log("calibrated static activation scales")
-    pages = sum((int(L) + 64 + spec.page_size - 1) // spec.page_size + 1 for L in ctx)
+    pages = sum((int(L) + 64 + grow + spec.page_size - 1) // spec.page_size + 1 for L in ctx)
     cache = ev.Cache(model, pages, B)
-    slots = [cache.ev_cache_add_seq(int(L) + 64) for L in ctx]
+    slots = [cache.ev_cache_add_seq(int(L) + 64 + grow) for L in ctx]
     t0 = time.time()
     cache.ev_cache_prefill(slots, [wl.context_ids(spec, b, int(ctx[b])) for b in range(B)])
     torch.cuda.synchronize()
@@ -113,11 +167,12 @@ def build_gpu_workload(spec, steps_total, torch, ev, log):
     # drafts: GPU greedy continuation planted on the rank-0 chain w.p. 0.7 (config[3]'s rule), else uniform ids
     depth = wl.tree_depths(parents)
     D = int(depth.max())
+    n_greedy = max(D, grow)
     root = np.array([wl.draft_tokens_uniform(spec, parents, b)[0] for b in range(B)], dtype=np.int32)
-    greedy = np.zeros((B, D), dtype=np.int32)
+    greedy = np.zeros((B, n_greedy), dtype=np.int32)
     one = ev.VerifyBuffers(model, B, 1, want_argmax=True)
     cur = root.copy()
-    for d in range(D):
+    for d in range(n_greedy):
         one.set_inputs(slots, cur[:, None], np.full((B, 1), -1, np.int32))
         ev.ev_verify(model, cache, one, commit=True)
         torch.cuda.synchronize()
@@ -125,20 +180,14 @@ def build_gpu_workload(spec, steps_total, torch, ev, log):
         greedy[:, d] = cur
     cache.ev_cache_set_lens(slots, [int(L) for L in ctx])
     tokens = np.zeros((B, T), dtype=np.int32)
-    first_child = {}
-    for i in range(1, T):
-        first_child.setdefault(int(parents[i]), i)
+    planted = np.zeros(B, dtype=np.int64)     # drafts that verification must accept if it reproduces greedy decoding
     for b in range(B):
-        tk = wl.draft_tokens_uniform(spec, parents, b)
         coins = wl.gen.match_coins(spec, b, D)
-        node = 0
-        while node in first_child:
-            c = first_child[node]
-            if coins[depth[c] - 1] < 0.7:
-                tk[c] = greedy[b, depth[c] - 1]
-            node = c
-        tokens[b] = tk
-    return dict(model=model, cache=cache, slots=slots, ctx=ctx, parents=parents, tokens=tokens)
+        tokens[b] = plant(spec, parents, b, root[b], greedy[b], coins)
+        hit = coins[:len(rank0_chain(parents))] < 0.7
+        planted[b] = int(np.argmin(hit)) if not hit.all() else len(hit)
+    return dict(model=model, cache=cache, slots=slots, ctx=ctx, parents=parents, tokens=tokens, greedy=greedy, root=root,
+                planted=planted)
 
 
 # ------------------------------------------------------------------------------------------ oracle arm
@@ -203,49 +252,10 @@ def whole_job_rate(units_per_rank, world, ms_per_step):
 
 # ------------------------------------------------------------------------------------------ main
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--impl", default="ours")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    spec = wl.CONFIGS[args.config]
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    log = lambda s: print(f"[bench r{rank}] {s}", file=sys.stderr, flush=True)  # noqa: E731
-    warmup = max(args.warmup, 3)
-
-    if args.impl == "reference":
-        if rank != 0:
-            return
-        r = oracle_sample(spec, min(args.steps, 10), min(warmup, 2), log)
-        line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": "tree-tokens/s", "n_gpus": args.gpus,
-                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 elementwise (E4M3 W8A8 emulated)",
-                "data": "synthetic", "config": {"workload": spec.name, "batch": spec.batch, "tree_nodes": spec.n_nodes},
-                "cpu_baseline": {"value": r["value"], "unit": "tree-tokens/s", "cores": r["cores"], "kind": "oracle",
-                                 "sample": r["sample"]},
-                "e2e": {"value": r["value"], "unit": "tree-tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
-        print(json.dumps(line), flush=True)
-        return
-
-    import torch
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
-    torch.cuda.set_device(local_rank)
-    import paper_2606_18502_b200 as ev
-    from paper_2606_18502_b200 import build
-    build.build()
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    wk = build_gpu_workload(spec, warmup + args.steps, torch, ev, log)
+def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, steps, with_cpu, fp8_peak):
+    """Builds the workload of one config, times `steps` verify steps (device events), the per-class pass, the end-to-end
+    leg through ev_verify_host and - with --loop - the sustained closed loop.  Returns the JSON line as a dict."""
+    wk = build_gpu_workload(spec, warmup + steps, torch, ev, log, loop_steps=args.loop)
     model, cache, slots, ctx, parents, tokens = (wk[k] for k in ("model", "cache", "slots", "ctx", "parents", "tokens"))
     B, T = tokens.shape
     L0 = [int(x) for x in ctx]
@@ -271,7 +281,7 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.profiler.start()          # no-op unless run under ncu --profile-from-start off
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     e1.record()
     torch.cuda.synchronize()
@@ -281,13 +291,15 @@ def main():
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop()
     ms = max_over_ranks(ms, dist, "cuda")
-    ms_step = ms / args.steps
+    ms_step = ms / steps
     acc = buf.accept_len.cpu().numpy()
     assert (buf.status.cpu().numpy() == 0).all(), "a sequence was rejected during the timed steps"
+    # losslessness inside the bench: the drafts planted from the GPU's own greedy decode must be accepted
+    assert (acc >= wk["planted"]).all(), ("tree verification did not reproduce the GPU's greedy decode", acc.tolist(), wk["planted"].tolist())
 
     # per-kernel-class device time over a second pass of the same K steps (CUDA events on the launch stream)
     model.ev_profile_enable(True)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step()
     prof = model.ev_profile_read()
     model.ev_profile_enable(False)
@@ -298,19 +310,26 @@ def main():
     per_launch_us = {k: round(1e3 * v[0] / max(v[1], 1), 2) for k, v in prof.items()}
     attn_ms, attn_n = prof["tree_attention"]
     share = {k: round(v[0] / max(sum(x[0] for x in prof.values()), 1e-9), 4) for k, v in prof.items()}
-    gemm_gbs = work["weight_bytes"] * args.steps / (gemm_ms * 1e-3) / 1e9
+    gemm_gbs = work["weight_bytes"] * steps / (gemm_ms * 1e-3) / 1e9
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(spec.name, {}).get("gemm_dram_bytes_per_launch")
-    roofline = {"bound": "hbm", "kernel": "gemm_e4m3_kernel (tcgen05 FP8 W8A8 linears)", "achieved": round(gemm_gbs, 1),
-                "peak": pk["hbm_gbs"], "peak_source": pk["source"] + " (MEASURED_PEAKS.json hbm_gbs)" if pk["source"] == "measured" else "fallback (B200_PROFILING.md)",
-                "unit": "GB/s", "frac": round(gemm_gbs / pk["hbm_gbs"], 4),
-                "bytes_per_launch": work["weight_bytes"] / (gemm_n / args.steps), "launches_per_step": gemm_n // args.steps,
-                "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic, "time_share_by_class": share,
-                "avg_launch_us_by_class": per_launch_us}
-    fp8_peak = 2 * pk["bf16_tflops"] * 1e12
-    t_roof = max((work["weight_bytes"] + work["kv_bytes"]) / (pk["hbm_gbs"] * 1e9), work["flops"] / fp8_peak)
+    peak_src = pk["source"] + " (MEASURED_PEAKS.json hbm_gbs)" if pk["source"] == "measured" else "fallback (B200_PROFILING.md)"
+    lin_flops = B * T * spec.model.linear_flops_per_token()
+    hbm_bound = work["weight_bytes"] / (pk["hbm_gbs"] * 1e9) >= lin_flops / fp8_peak[0]
+    if hbm_bound:     # few rows: the GEMMs stream the weights once per step
+        roofline = {"bound": "hbm", "kernel": "gemm_e4m3_kernel (tcgen05 FP8 W8A8 linears)", "achieved": round(gemm_gbs, 1),
+                    "peak": pk["hbm_gbs"], "peak_source": peak_src, "unit": "GB/s", "frac": round(gemm_gbs / pk["hbm_gbs"], 4),
+                    "bytes_per_launch": work["weight_bytes"] / (gemm_n / steps)}
+    else:             # many rows: the same kernels are bound by the FP8 tensor pipe
+        tf = lin_flops * steps / (gemm_ms * 1e-3) / 1e12
+        roofline = {"bound": "tensor", "kernel": "gemm_e4m3_kernel (tcgen05 FP8 W8A8 linears)", "achieved": round(tf, 1),
+                    "peak": round(fp8_peak[0] / 1e12, 1), "peak_source": fp8_peak[1], "unit": "TFLOP/s", "frac": round(tf * 1e12 / fp8_peak[0], 4),
+                    "flops_per_launch": lin_flops / (gemm_n / steps)}
+    roofline.update({"launches_per_step": gemm_n // steps, "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic,
+                     "time_share_by_class": share, "avg_launch_us_by_class": per_launch_us})
+    t_roof = max((work["weight_bytes"] + work["kv_bytes"]) / (pk["hbm_gbs"] * 1e9), work["flops"] / fp8_peak[0])
 
     # end to end: host (pinned) buffers through the C ABI, copies inside the timed region
     host = {k: torch.empty(s, dtype=torch.int32).pin_memory() for k, s in
@@ -324,15 +343,57 @@ def main():
         ev.ev_verify_host(model, cache, host)
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         cache.ev_cache_set_lens(slots, L0)
         ev.ev_verify_host(model, cache, host)      # synchronises internally
     e2e_ms = 1e3 * (time.perf_counter() - t0)
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     assert np.array_equal(host["accept_len"].numpy(), acc)
     emitted = int((acc + 1).sum())
+
+    # sustained closed loop (--loop K): commit = 1, no rewind, every sequence advances by its own a + 1 per step; the drafts
+    # of the next step are planted (p = 0.7 per depth) from the greedy stream at the position the sequence has reached -
+    # the role a drafter plays - on the host, between steps, inside the timed region; results come back through
+    # ev_verify_host, which also tells the library the true new lengths.
+    loop = None
+    if args.loop > 0:
+        greedy, D = wk["greedy"], int(wl.tree_depths(parents).max())
+        rng = np.random.default_rng(spec.seed + 991)
+        cache.ev_cache_set_lens(slots, L0)
+        pos = np.zeros(B, dtype=np.int64)           # tokens emitted so far
+        root = wk["root"].copy()
+        tot_emit = tot_acc = 0
+        caps_at = []
+        barrier()
+        ev.ev_capture_count(reset=True)
+        t0 = time.perf_counter()
+        for s in range(args.loop):
+            tk = np.stack([plant(spec, parents, b, root[b], greedy[b, pos[b]:pos[b] + D], rng.random(D)) for b in range(B)])
+            host["tokens"].copy_(torch.from_numpy(tk))
+            ev.ev_verify_host(model, cache, host)
+            a = host["accept_len"].numpy().astype(np.int64)
+            out = host["out_tokens"].numpy()
+            assert (host["status"].numpy() == 0).all()
+            for b in range(B):
+                assert out[b, :a[b] + 1].tolist() == greedy[b, pos[b]:pos[b] + a[b] + 1].tolist(), "sustained loop left the greedy sequence"
+                root[b] = out[b, a[b]]
+            pos += a + 1
+            tot_emit += int((a + 1).sum())
+            tot_acc += int(a.sum())
+            if ev.ev_capture_count(reset=True):
+                caps_at.append(s)
+        loop_ms = 1e3 * (time.perf_counter() - t0)
+        loop_ms = max_over_ranks(loop_ms, dist, "cuda")
+        loop = {"steps": args.loop, "ms_per_step": round(loop_ms / args.loop, 4),
+                "tree_tokens_per_s": round(whole_job_rate(B * T, world, loop_ms / args.loop), 1),
+                "emitted_tokens_per_s": round(world * tot_emit / (loop_ms * 1e-3), 1),
+                "accepted_tokens_per_s": round(world * tot_acc / (loop_ms * 1e-3), 1),
+                "mean_emitted_per_step": round(tot_emit / (B * args.loop), 3), "graph_captures_at_steps": caps_at,
+                "vs_rewound_e2e": round((e2e_ms / steps) / (loop_ms / args.loop), 4),
+                "def": "commit=1, no rewind, ctx advances by a+1; host plants the next drafts from the GPU greedy stream between steps; "
+                       "every emitted token checked against that stream"}
     if rank != 0:
-        return
+        return None
     # static scales (config[4]): the clip rate PAPER.md:140 reports, from the quantizers' own counters over one step
     clip = None
     if spec.act_scale_mode == 1:
@@ -346,32 +407,111 @@ def main():
         clip = {"clipped": int(cc.sum()), "quantized_elements": int(n_el), "rate": float(cc.sum()) / n_el,
                 "def": "activation elements with |x| > 448 * s_site over one verify step (PAPER.md:140)"}
     cpu = None
-    if not args.no_cpu_baseline and world == 1:
+    if with_cpu and world == 1:
         r = oracle_sample(spec, 4, 1, log)
         cpu = {"value": round(r["value"], 3), "unit": "tree-tokens/s", "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
     line = {
         "metric": METRIC, "value": round(whole_job_rate(B * T, world, ms_step), 1), "unit": "tree-tokens/s", "n_gpus": world,
-        "steps": args.steps, "warmup": warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "e4m3 x e4m3 -> f32 (bf16 KV, f32 residual)", "data": "synthetic",
         "config": {"workload": spec.name, "batch_per_gpu": B, "tree_nodes": T, "context": L0 if B <= 4 else [min(L0), max(L0)],
-                   "cache_state": "cold: 7.5 GB of weights + KV exceed the 126 MB L2 every step", "replicas": world},
+                   "cache_state": "cold: 7.5 GB of weights + KV exceed the 126 MB L2 every step", "replicas": world,
+                   "attn_chunk": "library default for this max_batch / max_ctx (ev_config.attn_chunk = 0)"},
         "accepted_tokens_per_s": round(world * int(acc.sum()) / (ms_step * 1e-3), 1),
         "emitted_tokens_per_s": round(world * emitted / (ms_step * 1e-3), 1),
         "mean_emitted_per_step": round(emitted / B, 3),
+        "planted_emitted_per_step": round(float((wk["planted"] + 1).mean()), 3),
         "step_roofline": {"ideal_ms": round(1e3 * t_roof, 4), "frac": round(1e3 * t_roof / ms_step, 4),
-                          "def": "max((weight+KV bytes)/HBM, FLOPs/FP8 peak); FP8 peak = 2 x measured bf16 burst",
+                          "def": "max((weight+KV bytes)/HBM, FLOPs/FP8 peak)", "fp8_peak_tflops": round(fp8_peak[0] / 1e12, 1),
+                          "fp8_peak_source": fp8_peak[1], "hbm_gbs": pk["hbm_gbs"],
                           "weight_bytes": work["weight_bytes"], "kv_bytes": work["kv_bytes"], "flops": work["flops"]},
         "roofline": roofline,
         "cpu_baseline": cpu,
-        "e2e": {"value": round(whole_job_rate(B * T, world, e2e_ms / args.steps), 1), "unit": "tree-tokens/s",
-                "ms_per_step": round(e2e_ms / args.steps, 4), "h2d_bytes_per_step": (2 * B * T + B) * 4,
+        "e2e": {"value": round(whole_job_rate(B * T, world, e2e_ms / steps), 1), "unit": "tree-tokens/s",
+                "ms_per_step": round(e2e_ms / steps, 4), "h2d_bytes_per_step": (2 * B * T + B) * 4,
                 "d2h_bytes_per_step": (2 * B * T + 3 * B) * 4},
         "gpu_launches": int(launches), "clocks": clocks,
-        "attention": {"ms_per_step": round(attn_ms / args.steps, 4), "kv_gbs": round(work["kv_bytes"] * args.steps / max(attn_ms, 1e-9) / 1e6, 1)},
+        "attention": {"ms_per_step": round(attn_ms / steps, 4), "kv_gbs": round(work["kv_bytes"] * steps / max(attn_ms, 1e-9) / 1e6, 1)},
     }
+    if loop is not None:
+        line["sustained_loop"] = loop
     if clip is not None:
         line["clip_rate"] = clip
-    print(json.dumps(line), flush=True)
+    del buf, cache, model
+    torch.cuda.empty_cache()
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--loop", type=int, default=0, help="also run a sustained closed loop of this many committed steps")
+    ap.add_argument("--also", default="auto", help="configs whose short line is added under 'also' (default: 2 = batch 32 "
+                                                   "when the headline config 1 runs on one GPU; 'none' to skip)")
+    args = ap.parse_args()
+    spec = wl.CONFIGS[args.config]
+    if args.impl != "reference" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # N independent replicas, one process per GPU: start them the way the driver would
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    log = lambda s: print(f"[bench r{rank}] {s}", file=sys.stderr, flush=True)  # noqa: E731
+    warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        r = oracle_sample(spec, min(args.steps, 10), min(warmup, 2), log)
+        line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": "tree-tokens/s", "n_gpus": args.gpus,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate / f32 elementwise (E4M3 W8A8 emulated)",
+                "data": "synthetic", "config": {"workload": spec.name, "batch_per_gpu": spec.batch, "tree_nodes": spec.n_nodes},
+                "cpu_baseline": {"value": r["value"], "unit": "tree-tokens/s", "cores": r["cores"], "kind": "oracle",
+                                 "sample": r["sample"]},
+                "e2e": {"value": r["value"], "unit": "tree-tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line), flush=True)
+        return
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local_rank)
+    import paper_2606_18502_b200 as ev
+    from paper_2606_18502_b200 import build
+    build.build()
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    fp8_peak = fp8_peak_probe(torch)
+    log(f"FP8 tensor peak: {fp8_peak[0] / 1e12:.0f} TFLOP/s ({fp8_peak[1]})")
+    line = measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, args.steps, not args.no_cpu_baseline, fp8_peak)
+    also = [2] if (args.also == "auto" and args.config == 1 and world == 1) else \
+        [int(x) for x in args.also.split(",") if x.strip().isdigit()] if args.also not in ("auto", "none") else []
+    if also:   # north_star names batch 1 AND batch 32: the batch-32 config rides along as a short line
+        args.loop = 0
+        extra = {}
+        for c in also:
+            l2 = measure(wl.CONFIGS[c], args, torch, ev, dist, rank, world, local_rank, log, 3, min(args.steps, 8), False, fp8_peak)
+            if l2 is not None:
+                extra[wl.CONFIGS[c].name] = {k: l2[k] for k in ("value", "unit", "ms_per_step", "steps", "config", "mean_emitted_per_step",
+                                                                   "planted_emitted_per_step", "emitted_tokens_per_s", "step_roofline", "roofline", "e2e", "clocks", "attention")}
+        if line is not None:
+            line["also"] = extra
+    if rank == 0:
+        print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
 

@@ -248,6 +248,10 @@ int ev_profile_trace(ev_model*, unsigned long long* host_out, int max_entries, i
 const char* ev_last_error(void);
 /* kernels launched by the calling thread's library calls since the last reset */
 long ev_launch_count(int reset);
+/* verify steps captured into a CUDA graph by the calling thread's ev_verify calls since the last reset: the first call with a
+ * new (batch, tree size, buffer set, attention chunk-column count) captures and instantiates (host work, ~ms); every later
+ * call with the same set replays.  A steady decode loop captures once per chunk-column boundary a sequence crosses. */
+long ev_capture_count(int reset);
 int ev_version(void);
 
 #ifdef __cplusplus

@@ -3,6 +3,6 @@
 The product is the C-ABI library declared in include/eagle_verify.h (hand-written CUDA kernels
 in csrc/).  This package only marshals arguments; it never imports oracle/."""
 from .binding import (  # noqa: F401
-    Cache, EvError, Model, VerifyBuffers, ev_last_error, ev_launch_count, ev_verify, ev_verify_host, load_library,
+    Cache, EvError, Model, VerifyBuffers, ev_last_error, ev_launch_count, ev_capture_count, ev_verify, ev_verify_host, load_library,
     LIB_PATH, SIGNATURES,
 )

@@ -76,6 +76,7 @@ SIGNATURES = {
     "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
     "ev_last_error": (C.c_char_p, []),
     "ev_launch_count": (C.c_long, [C.c_int]),
+    "ev_capture_count": (C.c_long, [C.c_int]),
     "ev_version": (C.c_int, []),
 }
 
@@ -113,6 +114,10 @@ def _stream():
 
 def ev_last_error():
     return load_library().ev_last_error().decode()
+
+
+def ev_capture_count(reset=False):
+    return int(load_library().ev_capture_count(1 if reset else 0))
 
 
 def ev_launch_count(reset=False):

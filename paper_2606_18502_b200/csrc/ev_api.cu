@@ -24,6 +24,7 @@ namespace {
 
 thread_local std::string g_err;
 thread_local long g_launches = 0;
+thread_local long g_captures = 0;
 
 int fail(int code, const std::string& msg) {
     g_err = msg;
@@ -771,7 +772,12 @@ long ev_launch_count(int reset) {
     if (reset) g_launches = 0;
     return v;
 }
-int ev_version(void) { return 1; }
+long ev_capture_count(int reset) {
+    long v = g_captures;
+    if (reset) g_captures = 0;
+    return v;
+}
+int ev_version(void) { return 2; }
 
 int ev_model_create(const ev_config* cfg, ev_model** out) {
     if (!cfg || !out) return fail(EV_EINVAL, "null argument");
@@ -1214,6 +1220,7 @@ int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* o
     if (!hit) {
         if (!m->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&m->cap_stream, cudaStreamNonBlocking));
         const long before = g_launches;
+        ++g_captures;
         CUDA_TRY(cudaStreamBeginCapture(m->cap_stream, cudaStreamCaptureModeRelaxed));
         const int rc = run_forward(m, c, in, out, m->cap_stream, need_lm, plan);
         cudaGraph_t graph = nullptr;
