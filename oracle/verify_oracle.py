@@ -348,9 +348,16 @@ class OracleKV:
     """Paged bf16 KV cache (BASELINE.json:configs[2] "bf16 paged KV cache with 16-token pages").
     pool[layer] is uint16 [n_pages, 2(K|V), Hkv, page_size, d]; a sequence owns a list of physical
     pages; token slot t lives in page_table[seq][t // page_size] at offset t % page_size.
-    Layers are allocated on first touch so sampled-layer checks at 8B shape stay small."""
+    Layers are allocated on first touch so sampled-layer checks at 8B shape stay small.
+    kv_dtype="e4m3" ("quantizing the KV cache to FP8 halves the storage compared to FP16/BF16"; SURVEY section
+    8(f)-2; DESIGN.md R-kv8): the pool holds E4M3 codes (one byte per element) and K, V are quantized with STATIC per-tensor
+    scales - one for the K cache and one for the V cache of each layer, set by calibrate() as absmax / 448 over the
+    calibration tokens (the paper's static min-max PTQ): code = E4M3_sat(x / s) on write (values beyond 448 s saturate),
+    value = fp32(decode(code) * s) on read.  The scales live in model.static under ("k_cache", layer), ("v_cache", layer)."""
 
-    def __init__(self, model, n_pages, page_size=16, page_order=None):
+    def __init__(self, model, n_pages, page_size=16, page_order=None, kv_dtype="bf16"):
+        assert kv_dtype in ("bf16", "e4m3")
+        self.kv_dtype, self.model = kv_dtype, model
         self.Hkv, self.d, self.page_size, self.n_pages = model.n_kv_heads, model.head_dim, page_size, n_pages
         self.pool = {}
         self.free = list(range(n_pages)) if page_order is None else list(page_order)
@@ -359,8 +366,29 @@ class OracleKV:
 
     def _layer(self, layer):
         if layer not in self.pool:
-            self.pool[layer] = np.zeros((self.n_pages, 2, self.Hkv, self.page_size, self.d), dtype=np.uint16)
+            self.pool[layer] = np.zeros((self.n_pages, 2, self.Hkv, self.page_size, self.d),
+                                        dtype=np.uint16 if self.kv_dtype == "bf16" else np.uint8)
         return self.pool[layer]
+
+    def bytes_per_token(self):
+        """cache storage per token per layer"""
+        return 2 * self.Hkv * self.d * (2 if self.kv_dtype == "bf16" else 1)
+
+    def _scales(self, layer):
+        return F32(self.model.static[("k_cache", layer)]), F32(self.model.static[("v_cache", layer)])
+
+    def _encode(self, layer, k, v):
+        """fp32 K, V -> the pool's storage bits"""
+        if self.kv_dtype == "bf16":
+            return f32_to_bf16_bits(k), f32_to_bf16_bits(v)
+        sk, sv = self._scales(layer)
+        return e4m3.encode((np.asarray(k, dtype=F32) / sk).astype(F32)), e4m3.encode((np.asarray(v, dtype=F32) / sv).astype(F32))
+
+    def _decode(self, layer, kb, vb):
+        if self.kv_dtype == "bf16":
+            return bf16_bits_to_f32(kb), bf16_bits_to_f32(vb)
+        sk, sv = self._scales(layer)
+        return (e4m3.decode(kb).astype(F32) * sk).astype(F32), (e4m3.decode(vb).astype(F32) * sv).astype(F32)
 
     def add_seq(self, seq, capacity_tokens):
         n = -(-capacity_tokens // self.page_size)
@@ -372,22 +400,30 @@ class OracleKV:
         return len(self.page_table[seq]) * self.page_size
 
     def write(self, layer, seq, slots, k, v):
-        """k, v: fp32 [n, Hkv, d]; stored rounded to bf16."""
+        """k, v: fp32 [n, Hkv, d]; stored rounded to bf16 (or quantized to E4M3, kv_dtype)."""
         pool = self._layer(layer)
-        kb, vb = f32_to_bf16_bits(k), f32_to_bf16_bits(v)
+        kb, vb = self._encode(layer, k, v)
         for i, t in enumerate(slots):
             pg, off = self.page_table[seq][t // self.page_size], t % self.page_size
             pool[pg, 0, :, off, :] = kb[i]
             pool[pg, 1, :, off, :] = vb[i]
 
     def read(self, layer, seq, start, stop):
-        """-> K, V as fp32 [stop-start, Hkv, d] (bf16 values)."""
+        """-> K, V as fp32 [stop-start, Hkv, d] (the stored values: bf16, or dequantized E4M3)."""
         pool = self._layer(layer)
         slots = np.arange(start, stop)
         pages = np.asarray(self.page_table[seq], dtype=np.int64)[slots // self.page_size]
         offs = slots % self.page_size
         blk = pool[pages, :, :, offs, :]            # [n, 2, Hkv, d]
-        return bf16_bits_to_f32(blk[:, 0]), bf16_bits_to_f32(blk[:, 1])
+        return self._decode(layer, blk[:, 0], blk[:, 1])
+
+    def read_bits(self, layer, seq, start, stop):
+        """-> the stored bits of K, V: [stop-start, Hkv, d] uint16 (bf16) or uint8 (E4M3 codes)"""
+        pool = self._layer(layer)
+        slots = np.arange(start, stop)
+        pages = np.asarray(self.page_table[seq], dtype=np.int64)[slots // self.page_size]
+        blk = pool[pages, :, :, slots % self.page_size, :]
+        return blk[:, 0], blk[:, 1]
 
     def move(self, seq, src_slot, dst_slot):
         for pool in self.pool.values():
@@ -396,16 +432,19 @@ class OracleKV:
             pool[pd, :, :, od, :] = pool[ps, :, :, os_, :]
 
     def export_dense(self, layer, seq, n_tokens):
-        """-> uint16 [2, Hkv, n_tokens, d] (the layout of the library's export, per layer)."""
-        k, v = self.read(layer, seq, 0, n_tokens)
-        return np.stack([f32_to_bf16_bits(k).transpose(1, 0, 2), f32_to_bf16_bits(v).transpose(1, 0, 2)])
+        """-> stored bits [2, Hkv, n_tokens, d] (the layout of the library's export, per layer)."""
+        kb, vb = self.read_bits(layer, seq, 0, n_tokens)
+        return np.stack([kb.transpose(1, 0, 2), vb.transpose(1, 0, 2)])
 
     def import_dense(self, layer, seq, dense_bits):
-        """dense_bits uint16 [2, Hkv, n, d] -> slots 0..n-1 of seq (DESIGN.md R-kv-input)."""
+        """dense_bits (stored bits) [2, Hkv, n, d] -> slots 0..n-1 of seq (DESIGN.md R-kv-input)."""
         n = dense_bits.shape[2]
-        k = bf16_bits_to_f32(dense_bits[0].transpose(1, 0, 2))
-        v = bf16_bits_to_f32(dense_bits[1].transpose(1, 0, 2))
-        self.write(layer, seq, range(n), k, v)
+        pool = self._layer(layer)
+        kb, vb = dense_bits[0].transpose(1, 0, 2), dense_bits[1].transpose(1, 0, 2)
+        for t in range(n):
+            pg, off = self.page_table[seq][t // self.page_size], t % self.page_size
+            pool[pg, 0, :, off, :] = kb[t]
+            pool[pg, 1, :, off, :] = vb[t]
 
 
 # ----------------------------------------------------------------------------- forward
@@ -424,7 +463,10 @@ def layer_forward(model, layer, h, cache, seq, L, parents, record=None, taps=Non
     v = model._lin(xq, sx, "wv", layer).reshape(T, Hkv, d)
     cos, sin = rope_cos_sin(L + depth, d, model.rope_theta)
     q, k = apply_rope(q, cos, sin), apply_rope(k, cos, sin)
-    cache.write(layer, seq, [L + i for i in range(T)], k, v)          # rounds to bf16
+    if record is not None:   # calibration pass: per-tensor absmax of what the cache stores (FP8 KV scales, DESIGN.md R-kv8)
+        record[("k_cache", layer)] = max(record.get(("k_cache", layer), 0.0), float(np.max(np.abs(k))))
+        record[("v_cache", layer)] = max(record.get(("v_cache", layer), 0.0), float(np.max(np.abs(v))))
+    cache.write(layer, seq, [L + i for i in range(T)], k, v)          # rounds to bf16 (or quantizes to E4M3)
     k_ctx, v_ctx = cache.read(layer, seq, 0, L)
     k_tree, v_tree = cache.read(layer, seq, L, L + T)
     attn = tree_attention(q, k_ctx, v_ctx, k_tree, v_tree, parents, qp_bits=model.inject.get("qp"))

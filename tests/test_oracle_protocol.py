@@ -133,7 +133,7 @@ def test_calibrate_replay_clips_nothing_and_hits_the_top_code_at_every_site():
     lands on +-448 (code 0x7E / 0xFE).  Fails for a scale of absmax/240, for an absmax taken at the wrong tensor and
     for a mislabelled site (a smaller site's scale clips, a larger one never reaches the top code)."""
     m, calib, rec = _calibrated()
-    assert set(rec) == {(s, l) for l in range(MICRO.n_layers) for s in vo.SITES} | {("lm_in", 0)}
+    assert set(rec) == {(s, l) for l in range(MICRO.n_layers) for s in vo.SITES + ("k_cache", "v_cache")} | {("lm_in", 0)}
     assert set(m.static) == set(rec)
     n = calib.shape[0]
     dyn = oracle_model(MICRO, seed=31, random_gains=True, act_scale_mode=0)     # same weights, dynamic scales
@@ -207,3 +207,98 @@ def test_calibrate_scale_is_absmax_over_all_tokens_not_the_last_chunk():
     vo.calibrate(m2, np.delete(calib, tok, axis=0))
     assert m2.static[("qkv_in", 0)] < m.static[("qkv_in", 0)]
     assert m.static[("qkv_in", 0)] == np.float32(np.float32(np.max(np.abs(x))) / np.float32(448.0))
+
+
+# ---- FP8 (E4M3) KV cache (DESIGN.md R-kv8) --------------------------------------
+
+def _fp8kv_model(seed=61):
+    m = oracle_model(MICRO, seed=seed, random_gains=True)
+    calib = np.random.default_rng(seed + 1).standard_normal((40, MICRO.hidden)).astype(np.float32)
+    vo.calibrate(m, calib)          # act_scale_mode 0: activations stay dynamic, only the cache scales are used
+    return m
+
+
+def test_fp8_kv_storage_halves_and_grid_values_round_trip():
+    m = _fp8kv_model()
+    c8 = vo.OracleKV(m, 4, 16, kv_dtype="e4m3")
+    c16 = vo.OracleKV(m, 4, 16)
+    assert 2 * c8.bytes_per_token() == c16.bytes_per_token()            # "halves the storage"
+    c8.add_seq(0, 32)
+    sk, sv = m.static[("k_cache", 1)], m.static[("v_cache", 1)]
+    assert sk > 0 and sv > 0 and sk != sv
+    codes = np.arange(256, dtype=np.uint8)
+    codes = codes[(codes & 0x7F) != 0x7F][: 2 * MICRO.n_kv_heads * MICRO.head_dim].reshape(2, MICRO.n_kv_heads, MICRO.head_dim)
+    k = (e4m3.decode(codes[0]).astype(np.float32) * sk).astype(np.float32)[None]
+    v = (e4m3.decode(codes[1]).astype(np.float32) * sv).astype(np.float32)[None]
+    c8.write(1, 0, [5], k, v)
+    kb, vb = c8.read_bits(1, 0, 5, 6)
+    kk, vv = c8.read(1, 0, 5, 6)
+    # values on the scaled E4M3 grid survive the cache bit for bit (x / s lands exactly on the grid when s is the scale used)
+    assert np.array_equal(kk, k) and np.array_equal(vv, v)
+    assert np.array_equal(kb[0] & 0x7F, codes[0] & 0x7F) or np.array_equal(e4m3.decode(kb[0]), e4m3.decode(codes[0]))
+    # anything else is rounded to within half an E4M3 step (2^-4 relative) or saturates at 448 s
+    rng = np.random.default_rng(3)
+    x = (rng.standard_normal((6, MICRO.n_kv_heads, MICRO.head_dim)) * float(sk) * 100).astype(np.float32)
+    c8.write(1, 0, range(6, 12), x, x)
+    kk, _ = c8.read(1, 0, 6, 12)
+    inr = np.abs(x) <= 448 * sk
+    assert np.all(np.abs(kk[inr] - x[inr]) <= np.maximum(np.abs(x[inr]) * 2.0 ** -4, float(sk) * 2.0 ** -10))
+    assert np.all(np.abs(kk[~inr]) == np.float32(448.0) * sk)
+
+
+def test_fp8_kv_invariants_chain_equals_decode_and_losslessness():
+    """Rows stay independent with an FP8 cache (static scales): chain == token-by-token decode bit for bit (P4), tree nodes ==
+    per-path recomputation (P5), speculative loop == greedy (P6) - and the FP8 model is a different model from
+    the bf16-cache one, within the size of the cache's quantization step."""
+    m = _fp8kv_model()
+    ids = np.random.default_rng(70).integers(0, MICRO.vocab, size=20).astype(np.int32)
+
+    def cache8(n=64):
+        c = vo.OracleKV(m, n // 16 + 2, 16, kv_dtype="e4m3")
+        c.add_seq(0, n)
+        return c
+    ca = cache8()
+    vo.prefill(m, ca, 0, ids)
+    chain = np.random.default_rng(71).integers(0, MICRO.vocab, size=5).astype(np.int32)
+    lg_chain, _ = vo.forward_tree(m, ca, 0, chain, wl.chain_parents(5))
+    cb = cache8()
+    vo.prefill(m, cb, 0, ids)
+    for i, t in enumerate(chain):
+        lg, _ = vo.forward_tree(m, cb, 0, np.array([t]), np.array([-1]))
+        cb.ctx_len[0] += 1
+        assert np.array_equal(lg[0], lg_chain[i]), i
+    # tree: every node == the last token of its root path run as a chain
+    par = np.array([-1, 0, 0, 1, 1, 2, 3], dtype=np.int32)
+    toks = np.random.default_rng(72).integers(0, MICRO.vocab, size=7).astype(np.int32)
+    cc = cache8()
+    vo.prefill(m, cc, 0, ids)
+    lg_tree, _ = vo.forward_tree(m, cc, 0, toks, par)
+    for i in range(7):
+        path = [i]
+        while par[path[-1]] >= 0:
+            path.append(int(par[path[-1]]))
+        path = path[::-1]
+        cd = cache8()
+        vo.prefill(m, cd, 0, ids)
+        lg, _ = vo.forward_tree(m, cd, 0, toks[path], wl.chain_parents(len(path)))
+        assert np.array_equal(lg[-1], lg_tree[i]), i
+    # losslessness: speculative loop with planted drafts == plain greedy
+    cg = cache8(96)
+    vo.prefill(m, cg, 0, ids)
+    greedy = vo.decode_greedy(m, cg, 0, 7, 16)
+    cs = cache8(96)
+    vo.prefill(m, cs, 0, ids)
+    out, root, rng = [], 7, np.random.default_rng(73)
+    while len(out) < 10:
+        e = len(out)
+        tk = np.array([root] + [greedy[e + d] if rng.random() < 0.7 else int(rng.integers(0, MICRO.vocab)) for d in range(3)], dtype=np.int32)
+        r = vo.verify(m, cs, 0, tk, wl.chain_parents(4))
+        out += r["out_tokens"]
+        root = r["out_tokens"][-1]
+    assert out == greedy[:len(out)]
+    # against the bf16 cache: a different model, close (E4M3 step 2^-4 on K and V only)
+    c16 = fresh_cache(m, 64)
+    vo.prefill(m, c16, 0, ids)
+    lg16, _ = vo.forward_tree(m, c16, 0, chain, wl.chain_parents(5))
+    rel = np.linalg.norm(lg_chain - lg16) / np.linalg.norm(lg16)
+    assert 1e-4 < rel < 0.3, rel

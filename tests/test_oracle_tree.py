@@ -280,7 +280,7 @@ def test_calibration_static_scales(micro):
     m = oracle_model(MICRO, seed=11, random_gains=True, act_scale_mode=1)
     calib = np.random.default_rng(17).standard_normal((48, MICRO.hidden)).astype(np.float32)
     rec = vo.calibrate(m, calib)
-    assert len(rec) == 4 * MICRO.n_layers + 1 and all(v > 0 for v in rec.values())
+    assert len(rec) == 6 * MICRO.n_layers + 1 and all(v > 0 for v in rec.values())   # 4 activation sites + K, V cache per layer; LM head input
     # with static scales from the very batch it is run on, nothing clips and the forward runs
     cache = fresh_cache(m, 64)
     ids = _ctx(MICRO, 12, seed=18)
