@@ -78,6 +78,12 @@ typedef struct {
                             * chunks aligned to ABSOLUTE key positions plus a short tail, so its
                             * result does not depend on batch, tree or GPU; the chunk length is part of the model's arithmetic:
                             * two models with different attn_chunk agree only to fp32 rounding */
+    int kv_dtype;          /* 0 = bf16 KV cache (BASELINE.json configs; values rounded to bf16, held in IEEE binary16 containers: exact for
+                            * 2^-17 <= |x| <= 65504, 2^-25 absolute below, saturating above); 1 = FP8 (E4M3) KV cache, one byte per
+                            * element ("quantizing the KV cache to FP8 halves the storage"): K (after
+                            * RoPE) and V are stored as E4M3_sat(x / s) with ONE static scale per layer for K and one for V, set by
+                            * ev_model_calibrate (absmax over the calibration tokens / 448) or ev_model_set_kv_scales; needs page_size
+                            * 16 and head_dim 128 */
 } ev_config;
 
 typedef enum {
@@ -123,6 +129,10 @@ int ev_model_calibrate(ev_model*, const float* dev_hidden, int n_tok, float* dev
 int ev_model_get_static_scales(ev_model*, float* host_out);
 /* Overrides them (same order); used to replay externally calibrated scales. */
 int ev_model_set_static_scales(ev_model*, const float* host_in);
+/* FP8 KV cache scales (kv_dtype 1): 2*n_layers floats, (K, V) per layer.  get: after calibration; set: replays external scales
+ * (all > 0).  Both synchronous host calls; set drops the captured CUDA graphs. */
+int ev_model_get_kv_scales(ev_model*, float* host_out);
+int ev_model_set_kv_scales(ev_model*, const float* host_in);
 /* Clip counters (Fig. 4 "clip rate"): with static scales
  * (act_scale_mode == 1) every activation quantizer counts the elements it saturates, |x| > 448 * s_site,
  * per site, in the order of ev_model_get_static_scales, accumulated over all calls since the last reset
@@ -136,7 +146,9 @@ int ev_model_destroy(ev_model*);
 /* ---- paged bf16 KV cache ------------------------------------------------------------------- */
 
 /* Pool of n_pages pages; each page holds page_size tokens for all layers.
- * Device layout: [layer][page][K|V][kv_head][page_size][head_dim] bf16. */
+ * Device layout: [layer][page][K|V][kv_head][page_size][head_dim], 2 bytes per element (bf16 VALUES in IEEE binary16
+ * containers when page_size is 16 - the tcgen05 attention kernel's operand format, see ev_config.kv_dtype - plain bf16
+ * otherwise) or 1 byte per element (E4M3 codes, kv_dtype 1). */
 int ev_cache_create(ev_model*, long n_pages, int max_seqs, ev_cache** out);
 
 /* Reserves ceil(capacity_tokens / page_size) pages for a new sequence (ctx_len = 0) and returns
@@ -154,8 +166,8 @@ int ev_cache_prefill(ev_model*, ev_cache*, int n_seqs, const int* host_seq_slots
                      const int32_t* host_token_ids, const int* host_lens, void* stream);
 
 /* Dense export/import of one sequence's first n_tokens slots for layers [layer_begin, layer_end):
- * dev_dense: [layer][K|V][kv_head][n_tokens][head_dim] bf16.  import also sets ctx_len = n_tokens
- * when set_len != 0. */
+ * dev_dense: [layer][K|V][kv_head][n_tokens][head_dim] bf16 (kv_dtype 1: uint8 E4M3 codes).  import also sets
+ * ctx_len = n_tokens when set_len != 0. */
 int ev_cache_export_seq(ev_cache*, int seq_slot, int layer_begin, int layer_end, int n_tokens,
                         void* dev_dense, void* stream);
 int ev_cache_import_seq(ev_cache*, int seq_slot, int layer_begin, int layer_end, int n_tokens,

@@ -26,7 +26,7 @@ class ev_config(C.Structure):
                 ("head_dim", C.c_int), ("ffn", C.c_int), ("vocab", C.c_int), ("rms_eps", C.c_float),
                 ("rope_theta", C.c_float), ("page_size", C.c_int), ("act_scale_mode", C.c_int),
                 ("max_batch", C.c_int), ("max_tree_nodes", C.c_int), ("max_ctx", C.c_int), ("weight_scale_mode", C.c_int),
-                ("attn_chunk", C.c_int)]
+                ("attn_chunk", C.c_int), ("kv_dtype", C.c_int)]
 
 
 class ev_verify_in(C.Structure):
@@ -55,6 +55,8 @@ SIGNATURES = {
     "ev_model_calibrate": (C.c_int, [_P, _P, C.c_int, _P, _P]),
     "ev_model_get_static_scales": (C.c_int, [_P, _P]),
     "ev_model_set_static_scales": (C.c_int, [_P, _P]),
+    "ev_model_get_kv_scales": (C.c_int, [_P, _P]),
+    "ev_model_set_kv_scales": (C.c_int, [_P, _P]),
     "ev_model_get_clip_counts": (C.c_int, [_P, _P, C.c_int]),
     "ev_model_destroy": (C.c_int, [_P]),
     "ev_cache_create": (C.c_int, [_P, C.c_long, C.c_int, C.POINTER(_P)]),
@@ -128,11 +130,11 @@ class Model:
     """ev_model handle."""
 
     def __init__(self, shape, max_batch, max_tree_nodes, max_ctx, page_size=16, act_scale_mode=0, weight_scale_mode=0,
-                 attn_chunk=0):
+                 attn_chunk=0, kv_dtype=0):
         self.lib = load_library()
         self.cfg = ev_config(shape.n_layers, shape.hidden, shape.n_q_heads, shape.n_kv_heads, shape.head_dim,
                              shape.ffn, shape.vocab, shape.rms_eps, shape.rope_theta, page_size, act_scale_mode,
-                             max_batch, max_tree_nodes, max_ctx, weight_scale_mode, attn_chunk)
+                             max_batch, max_tree_nodes, max_ctx, weight_scale_mode, attn_chunk, kv_dtype)
         self.shape = shape
         h = C.c_void_p()
         _check(self.lib.ev_model_create(C.byref(self.cfg), C.byref(h)))
@@ -171,6 +173,18 @@ class Model:
         out = np.empty(4 * self.cfg.n_layers + 1, dtype=np.float32)
         _check(self.lib.ev_model_get_static_scales(self.h, out.ctypes.data_as(C.c_void_p)))
         return out
+
+    def ev_model_get_kv_scales(self):
+        import numpy as np
+        out = np.zeros(2 * self.cfg.n_layers, dtype=np.float32)
+        _check(self.lib.ev_model_get_kv_scales(self.h, out.ctypes.data_as(C.c_void_p)))
+        return out
+
+    def ev_model_set_kv_scales(self, scales):
+        import numpy as np
+        s = np.ascontiguousarray(scales, dtype=np.float32)
+        assert s.shape == (2 * self.cfg.n_layers,)
+        _check(self.lib.ev_model_set_kv_scales(self.h, s.ctypes.data_as(C.c_void_p)))
 
     def ev_model_get_clip_counts(self, reset=False):
         import numpy as np
@@ -272,7 +286,8 @@ class Cache:
 
     def ev_cache_export_seq(self, slot, layer_begin, layer_end, n_tokens):
         import torch
-        out = torch.empty(self._dense_shape(layer_begin, layer_end, n_tokens), dtype=torch.bfloat16, device="cuda")
+        dt = torch.uint8 if self.model.cfg.kv_dtype == 1 else torch.bfloat16      # kv_dtype 1: the E4M3 codes themselves
+        out = torch.empty(self._dense_shape(layer_begin, layer_end, n_tokens), dtype=dt, device="cuda")
         _check(self.lib.ev_cache_export_seq(self.h, slot, layer_begin, layer_end, n_tokens, _ptr(out), _stream()))
         return out
 

@@ -172,6 +172,10 @@ struct ev_model {
     float* w_amax = nullptr;         // device scalar: absmax of the matrix being quantized (per-tensor weight scales)
     unsigned long long* clip_counts = nullptr;  // device [n_sites]: elements clipped by the static scales since the last reset
     bool calibrated = false, recording = false;
+    // FP8 KV cache (cfg.kv_dtype 1): static per-tensor scales of every layer's K and V cache, [2 * n_layers] = (K, V) per layer
+    float* kv_amax = nullptr;          // device: calibration accumulators
+    std::vector<float> kv_scales;      // host copy (kernel arguments)
+    bool kv_calibrated = false;
     int num_sms = 148;
     int cut_pairs = 74;   // pieces of the canonical K cuts of every layer matrix (ev_gemm.cuh): a constant of the library, NOT the
                           // SM count of the device, so results do not change with the GPU the model runs on (148 SMs = 74 pairs)
@@ -208,6 +212,8 @@ struct ev_cache {
     CUtensorMap tmKV;            // whole pool, for the tcgen05 attention kernel
     bool tc_attn = false;        // page_size == 16 and the pool fits 32-bit row coordinates
     bool kv_f16 = false;         // the pool keeps the bf16-rounded K/V values in binary16 containers (tcgen05 attention; ev_common.cuh)
+    bool kv_fp8 = false;         // the pool keeps E4M3 codes, one byte per element (cfg.kv_dtype 1)
+    int eb = 2;                  // bytes per pool element
     // prefill staging
     int32_t *pf_tokens = nullptr, *pf_parents = nullptr, *pf_nn = nullptr, *pf_slots = nullptr;
     int32_t *pf_out = nullptr;
@@ -536,14 +542,14 @@ int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
     return EV_OK;
 }
 
-template <int D>
+template <int D, bool FP8>
 int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, dim3 grid) {
     static bool attr_set = false;
     if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D>::SMEM));
+        CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D, FP8>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D, FP8>::SMEM));
         attr_set = true;
     }
-    return launch_k(tree_attn_tc_kernel<D>, grid, dim3(TCA_THREADS), TcaCfg<D>::SMEM, st, tm, a);
+    return launch_k(tree_attn_tc_kernel<D, FP8>, grid, dim3(TcaCfg<D, FP8>::THREADS), TcaCfg<D, FP8>::SMEM, st, tm, a);
 }
 
 template <int D>
@@ -656,6 +662,9 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ra.page_table = c->page_table; ra.max_pages = c->max_pages; ra.page_size = cfg.page_size;
         ra.pool = c->pool + (size_t)l * c->layer_stride;
         ra.kv_f16 = c->kv_f16;
+        ra.pool8 = c->kv_fp8 ? reinterpret_cast<uint8_t*>(c->pool) + (size_t)l * c->layer_stride : nullptr;
+        ra.k_scale = c->kv_fp8 ? m->kv_scales[2 * l] : 1.f; ra.v_scale = c->kv_fp8 ? m->kv_scales[2 * l + 1] : 1.f;
+        ra.kv_amax = m->recording ? m->kv_amax + 2 * l : nullptr;
         ra.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ROPE_KV);
@@ -673,16 +682,19 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         aa.o_part = m->o_part; aa.ml_part = m->ml_part;
         // chunks per CTA (tcgen05 kernel): about four CTAs per SM-slot over the launch; a scheduling choice only
         const long units = (long)B * cfg.n_kv_heads * row_groups;
-        aa.cpg = c->kv_f16 ? (int)std::min<long>(n_splits, std::max<long>(1, units * n_splits / (4L * m->num_sms))) : 1;
+        aa.cpg = (c->kv_f16 || c->kv_fp8) ? (int)std::min<long>(n_splits, std::max<long>(1, units * n_splits / (4L * m->num_sms))) : 1;
         dim3 agrid((n_splits + aa.cpg - 1) / aa.cpg, cfg.n_kv_heads * row_groups, B);
         {
             ProfScope ps(m, st, PC_ATTN);
-            if (c->kv_f16) {
+            if (c->kv_f16 || c->kv_fp8) {
                 TcAttnArgs ta;
                 ta.a = aa;
                 ta.row0 = (int)((long)l * c->n_pages * 2 * cfg.n_kv_heads * TCA_PAGE);
+                ta.pool8 = reinterpret_cast<const uint8_t*>(c->pool);
+                ta.k_scale = c->kv_fp8 ? m->kv_scales[2 * l] : 1.f; ta.v_scale = c->kv_fp8 ? m->kv_scales[2 * l + 1] : 1.f;
                 ta.pf = pfp.take(false);
-                if (D == 128) EV_TRY(launch_attn_tc<128>(st, c->tmKV, ta, agrid)); else EV_TRY(launch_attn_tc<64>(st, c->tmKV, ta, agrid));
+                if (c->kv_fp8) EV_TRY((launch_attn_tc<128, true>(st, c->tmKV, ta, agrid)));
+                else if (D == 128) EV_TRY((launch_attn_tc<128, false>(st, c->tmKV, ta, agrid))); else EV_TRY((launch_attn_tc<64, false>(st, c->tmKV, ta, agrid)));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
             }
@@ -693,6 +705,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ma.anc = m->anc; ma.anc_bulk = m->anc_bulk; ma.o_part = m->o_part; ma.ml_part = m->ml_part;
         ma.qkv = m->qkv; ma.q_ld = m->qkv_dim; ma.pool = ra.pool; ma.page_table = c->page_table; ma.max_pages = c->max_pages;
         ma.page_size = cfg.page_size; ma.kv_f16 = c->kv_f16 ? 1 : 0; ma.scale = aa.scale;
+        ma.pool8 = ra.pool8; ma.k_scale = ra.k_scale; ma.v_scale = ra.v_scale;
         ma.attn = (tap && out->dev_tap_attn) ? out->dev_tap_attn : nullptr;
         ma.q = quant_out(m, m->aq, 4 * l + 1);
         ma.pf = pfp.take(false);
@@ -741,12 +754,20 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     EV_TRY(launch_k(accept_walk_kernel, dim3((B + 63) / 64), dim3(64), 0, st, ac));
     if (in->commit && !in->force_accept_all) {
         CompactArgs ca;
-        ca.T = T; ca.Hkv = cfg.n_kv_heads; ca.D = D; ca.page_size = cfg.page_size; ca.max_pages = c->max_pages;
+        ca.eb = c->eb; ca.T = T; ca.Hkv = cfg.n_kv_heads; ca.D = D; ca.page_size = cfg.page_size; ca.max_pages = c->max_pages;
         ca.layer_stride = c->layer_stride; ca.pool = c->pool; ca.page_table = c->page_table; ca.seq_slots = in->dev_seq_slots;
         ca.Lsnap = m->Lsnap; ca.accept_len = out->dev_accept_len; ca.accept_nodes = out->dev_accept_nodes;
         EV_TRY(launch_k(kv_compact_kernel, dim3(dim3(B, cfg.n_layers)), dim3(EW_THREADS), 0, st, ca));
     }
     return EV_OK;
+}
+
+// captured steps bake kernel arguments (gain pointers, scales passed by value): any change of model state drops them
+void drop_graphs(ev_model* m) {
+    if (m->graphs.empty()) return;
+    cudaDeviceSynchronize();
+    for (auto& g : m->graphs) cudaGraphExecDestroy(g.exec);
+    m->graphs.clear();
 }
 
 int check_ready(ev_model* m, bool need_lm) {
@@ -758,6 +779,8 @@ int check_ready(ev_model* m, bool need_lm) {
     if (need_lm && !m->have_lm) return fail(EV_ESTATE, "lm_head not set");
     if (m->cfg.act_scale_mode == 1 && !m->calibrated && !m->recording)
         return fail(EV_ESTATE, "static activation scales: model not calibrated");
+    if (m->cfg.kv_dtype == 1 && !m->kv_calibrated && !m->recording)
+        return fail(EV_ESTATE, "FP8 KV cache: K/V scales not calibrated (ev_model_calibrate or ev_model_set_kv_scales)");
     return EV_OK;
 }
 
@@ -794,7 +817,9 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     if (cfg->max_batch < 1 || cfg->max_ctx < 1) return fail(EV_EINVAL, "max_batch / max_ctx must be positive");
     if (cfg->act_scale_mode != 0 && cfg->act_scale_mode != 1) return fail(EV_EINVAL, "act_scale_mode must be 0 or 1");
     if (cfg->weight_scale_mode != 0 && cfg->weight_scale_mode != 1) return fail(EV_EINVAL, "weight_scale_mode must be 0 or 1");
-    if (cfg->attn_chunk < 0 || cfg->attn_chunk % 64) return fail(EV_EINVAL, "attn_chunk must be 0 (default 1024) or a multiple of 64");
+    if (cfg->attn_chunk < 0 || cfg->attn_chunk % 64) return fail(EV_EINVAL, "attn_chunk must be 0 (default) or a multiple of 64");
+    if (cfg->kv_dtype != 0 && cfg->kv_dtype != 1) return fail(EV_EINVAL, "kv_dtype must be 0 (bf16) or 1 (E4M3)");
+    if (cfg->kv_dtype == 1 && (cfg->page_size != 16 || cfg->head_dim != 128)) return fail(EV_EINVAL, "kv_dtype 1 needs page_size 16 and head_dim 128");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(EV_ECUDA, "no CUDA device");
     ev_model* m = new ev_model();
@@ -871,6 +896,8 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->site_amax, (size_t)m->n_sites));
     A(dev_alloc(m, &m->w_amax, (size_t)1));
     A(dev_alloc(m, &m->clip_counts, (size_t)m->n_sites));
+    A(dev_alloc(m, &m->kv_amax, (size_t)2 * cfg->n_layers));
+    m->kv_scales.assign((size_t)2 * cfg->n_layers, 1.0f);
     cudaMemset(m->clip_counts, 0, (size_t)m->n_sites * 8);
     A(dev_alloc(m, &m->rope_cs, (size_t)m->max_pos * (cfg->head_dim / 2)));
     if (rc == EV_OK) {
@@ -955,7 +982,7 @@ int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, 
         case EV_W_NORM1: case EV_W_NORM2: case EV_W_NORMF: {
             if (!(shape_is(1, H) || shape_is(H, 1))) return bad_shape();
             __nv_bfloat16** dst = kind == EV_W_NORM1 ? &m->layers[layer].g1 : kind == EV_W_NORM2 ? &m->layers[layer].g2 : &m->gf;
-            if (!*dst) EV_TRY(dev_alloc(m, dst, (size_t)H));
+            if (!*dst) { EV_TRY(dev_alloc(m, dst, (size_t)H)); drop_graphs(m); }   // a graph captured before held a null gain pointer
             CUDA_TRY(cudaMemcpyAsync(*dst, dev_bf16, (size_t)H * 2, cudaMemcpyDeviceToDevice, st));
             return EV_OK;
         }
@@ -1010,20 +1037,42 @@ int ev_model_set_static_scales(ev_model* m, const float* host_in) {
     m->calibrated = true;
     return EV_OK;
 }
+int ev_model_get_kv_scales(ev_model* m, float* host_out) {
+    if (!m || !host_out) return fail(EV_EINVAL, "null argument");
+    if (!m->kv_calibrated) return fail(EV_ESTATE, "not calibrated");
+    memcpy(host_out, m->kv_scales.data(), m->kv_scales.size() * sizeof(float));
+    return EV_OK;
+}
+int ev_model_set_kv_scales(ev_model* m, const float* host_in) {
+    if (!m || !host_in) return fail(EV_EINVAL, "null argument");
+    for (size_t i = 0; i < m->kv_scales.size(); ++i)
+        if (!(host_in[i] > 0.f)) return fail(EV_EINVAL, "K/V cache scales must be positive");
+    memcpy(m->kv_scales.data(), host_in, m->kv_scales.size() * sizeof(float));
+    m->kv_calibrated = true;
+    drop_graphs(m);
+    return EV_OK;
+}
 
 // ---- cache ---------------------------------------------------------------------------------------
+static int cache_create(ev_model* m, long n_pages, int max_seqs, bool fp8, ev_cache** out);
 int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
+    if (!m) return fail(EV_EINVAL, "bad argument");
+    return cache_create(m, n_pages, max_seqs, m->cfg.kv_dtype == 1, out);
+}
+static int cache_create(ev_model* m, long n_pages, int max_seqs, bool fp8, ev_cache** out) {
     if (!m || !out || n_pages < 1 || max_seqs < 1) return fail(EV_EINVAL, "bad argument");
     *out = nullptr;
     ev_cache* c = new ev_cache();
     c->model = m;
+    c->kv_fp8 = fp8;
+    c->eb = fp8 ? 1 : 2;
     c->n_pages = n_pages;
     c->max_seqs = max_seqs;
     const ev_config& cfg = m->cfg;
     c->max_pages = (cfg.max_ctx + cfg.page_size - 1) / cfg.page_size;
     c->layer_stride = n_pages * 2L * cfg.n_kv_heads * cfg.page_size * cfg.head_dim;
     const size_t pool_elems = (size_t)cfg.n_layers * c->layer_stride;
-    bool ok = cudaMalloc((void**)&c->pool, pool_elems * 2) == cudaSuccess;
+    bool ok = cudaMalloc((void**)&c->pool, pool_elems * c->eb) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->page_table, (size_t)max_seqs * c->max_pages * 4) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->ctx_len, (size_t)max_seqs * 4) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->capacity, (size_t)max_seqs * 4) == cudaSuccess;
@@ -1036,7 +1085,7 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
         ev_cache_destroy(c);
         return fail(EV_ENOMEM, "KV pool allocation failed");
     }
-    cudaMemset(c->pool, 0, pool_elems * 2);
+    cudaMemset(c->pool, 0, pool_elems * c->eb);
     {
         const long rows = (long)cfg.n_layers * n_pages * 2 * cfg.n_kv_heads * cfg.page_size;
         if (cfg.page_size == TCA_PAGE && rows < (1L << 31)) {
@@ -1047,8 +1096,12 @@ int ev_cache_create(ev_model* m, long n_pages, int max_seqs, ev_cache** out) {
                 return EV_ECUDA;
             }
             c->tc_attn = true;
-            c->kv_f16 = true;
+            c->kv_f16 = !fp8;
         }
+    }
+    if (fp8 && !(c->tc_attn && cfg.head_dim == 128)) {
+        ev_cache_destroy(c);
+        return fail(EV_EINVAL, "kv_dtype 1 (FP8 KV cache) needs page_size 16 and head_dim 128");
     }
     cudaMemset(c->page_table, 0, (size_t)max_seqs * c->max_pages * 4);
     cudaMemset(c->ctx_len, 0, (size_t)max_seqs * 4);
@@ -1169,7 +1222,7 @@ static int dense_copy(ev_cache* c, int slot, int lb, int le, int n_tokens, void*
     DenseCopyArgs a;
     a.Hkv = cfg.n_kv_heads; a.D = cfg.head_dim; a.page_size = cfg.page_size; a.n_tokens = n_tokens; a.layer_begin = lb;
     a.layer_stride = c->layer_stride; a.pool = c->pool; a.page_row = c->page_table + (size_t)slot * c->max_pages;
-    a.dense = (__nv_bfloat16*)dense; a.to_dense = to_dense; a.kv_f16 = c->kv_f16;
+    a.dense = (__nv_bfloat16*)dense; a.to_dense = to_dense; a.kv_f16 = c->kv_f16; a.eb = c->eb;
     dense_copy_kernel<<<dim3(n_tokens, le - lb), 128, 0, st>>>(a);
     LAUNCH_CHECK();
     return EV_OK;
@@ -1313,12 +1366,13 @@ int ev_model_calibrate(ev_model* m, const float* dev_hidden, int n_tok, float* d
     const ev_config& cfg = m->cfg;
     const int T = cfg.max_tree_nodes, H = cfg.hidden;
     ev_cache* c = nullptr;
-    EV_TRY(ev_cache_create(m, (n_tok + cfg.page_size - 1) / cfg.page_size + 1, 1, &c));
+    EV_TRY(cache_create(m, (n_tok + cfg.page_size - 1) / cfg.page_size + 1, 1, false, &c));   // the calibration pass itself runs on a bf16 cache
     int slot = -1, rc = ev_cache_add_seq(c, n_tok, nullptr, &slot);
     float* taps = nullptr;
     if (rc == EV_OK && dev_layer_inputs && cudaMalloc((void**)&taps, (size_t)(cfg.n_layers + 1) * T * H * 4) != cudaSuccess)
         rc = fail(EV_ENOMEM, "calibration tap buffer");
     if (rc == EV_OK && cudaMemsetAsync(m->site_amax, 0, m->n_sites * 4, st) != cudaSuccess) rc = fail(EV_ECUDA, "memset");
+    if (rc == EV_OK && cudaMemsetAsync(m->kv_amax, 0, (size_t)2 * cfg.n_layers * 4, st) != cudaSuccess) rc = fail(EV_ECUDA, "memset");
     m->recording = true;
     std::vector<int32_t> tok(T, 0), par(T);
     for (int j = 0; j < T; ++j) par[j] = j - 1;
@@ -1355,6 +1409,13 @@ int ev_model_calibrate(ev_model* m, const float* dev_hidden, int n_tok, float* d
         for (int i = 0; i < m->n_sites; ++i) sc[i] = amax[i] > 0.f ? amax[i] / 448.0f : 1.0f;
         if (rc == EV_OK && cudaMemcpy(m->static_scales, sc.data(), m->n_sites * 4, cudaMemcpyHostToDevice) != cudaSuccess) rc = fail(EV_ECUDA, "H2D copy");
         if (rc == EV_OK) m->calibrated = true;
+        std::vector<float> kva((size_t)2 * cfg.n_layers);
+        if (rc == EV_OK && cudaMemcpy(kva.data(), m->kv_amax, kva.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess) rc = fail(EV_ECUDA, "D2H copy");
+        if (rc == EV_OK) {   // FP8 KV cache scales: per-tensor absmax of K (post-RoPE) and V over the calibration tokens / 448
+            for (size_t i = 0; i < kva.size(); ++i) m->kv_scales[i] = kva[i] > 0.f ? kva[i] / 448.0f : 1.0f;
+            m->kv_calibrated = true;
+        }
+        drop_graphs(m);
     }
     std::string keep = g_err;
     if (taps) cudaFree(taps);

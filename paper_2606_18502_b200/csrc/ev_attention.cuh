@@ -346,12 +346,20 @@ struct MergeArgs {
     const __nv_bfloat16* pool;   // this layer
     const int32_t* page_table;
     int max_pages, page_size, kv_f16;
+    const uint8_t* pool8;   // FP8 KV cache: this layer's pool as E4M3 codes (kv_dtype 1), or null
+    float k_scale, v_scale; // its static scales: value = fp32(decode(code) * s)
     float scale;
     float* attn;   // optional [M][Hq*D] fp32 merged output (debug tap) or null
     QuantOut q;
     L2Prefetch pf;
 };
 constexpr int MERGE_THREADS = 256;   // = ROW_THREADS (ev_elementwise.cuh): Hq * D <= 4 * 256 * NV4 * cluster size
+__device__ __forceinline__ float4 kv_cvt4_e4m3(uint32_t w, float s) {   // 4 E4M3 codes -> fp32(decode(code) * s)
+    const __half2_raw lo = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)(w & 0xFFFFu), __NV_E4M3);
+    const __half2_raw hi = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)(w >> 16), __NV_E4M3);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&lo)), b = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+    return make_float4(mul_rn(a.x, s), mul_rn(a.y, s), mul_rn(b.x, s), mul_rn(b.y, s));
+}
 __device__ __forceinline__ float4 kv_cvt4(uint2 w, int kv_f16) {   // 4 consecutive K or V elements (raw pool bits) as fp32
     if (kv_f16) {
         const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&w.x)), b = __half22float2(*reinterpret_cast<const __half2*>(&w.y));
@@ -422,9 +430,15 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
         for (int u = 0; u < ATT_TAIL_MAX; ++u) {
             kr[u] = make_uint2(0u, 0u); vr[u] = make_uint2(0u, 0u);
             if (on && u < nt) {
-                const __nv_bfloat16* kp = a.pool + tbase[u] + hoff;
-                kr[u] = *reinterpret_cast<const uint2*>(kp);              // L1-cached: the G query heads of a kv head read the same rows
-                vr[u] = *reinterpret_cast<const uint2*>(kp + kv_stride);
+                if (a.pool8) {   // one byte per element: 4 codes in the low word
+                    const uint8_t* kp = a.pool8 + tbase[u] + hoff;
+                    kr[u].x = *reinterpret_cast<const uint32_t*>(kp);
+                    vr[u].x = *reinterpret_cast<const uint32_t*>(kp + kv_stride);
+                } else {
+                    const __nv_bfloat16* kp = a.pool + tbase[u] + hoff;
+                    kr[u] = *reinterpret_cast<const uint2*>(kp);              // L1-cached: the G query heads of a kv head read the same rows
+                    vr[u] = *reinterpret_cast<const uint2*>(kp + kv_stride);
+                }
             }
         }
         if (on) q4 = *reinterpret_cast<const float4*>(a.qkv + (size_t)m * a.q_ld + i);
@@ -435,7 +449,7 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
         float ts[ATT_TAIL_MAX];
 #pragma unroll
         for (int u = 0; u < ATT_TAIL_MAX; ++u) {
-            const float4 k4 = kv_cvt4(kr[u], a.kv_f16);
+            const float4 k4 = a.pool8 ? kv_cvt4_e4m3(kr[u].x, a.k_scale) : kv_cvt4(kr[u], a.kv_f16);
             float part = fmaf(q4.w, k4.w, fmaf(q4.z, k4.z, fmaf(q4.y, k4.y, __fmul_rn(q4.x, k4.x))));
             for (int o = gl >> 1; o > 0; o >>= 1) part = __fadd_rn(part, __shfl_xor_sync(0xffffffffu, part, o));
             ts[u] = mul_rn(part, a.scale);
@@ -478,7 +492,7 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
             for (int u = 0; u < ATT_TAIL_MAX; ++u)
                 if (u < nt) {
                     const float et = expf(ts[u] - mx);
-                    const float4 v4 = kv_cvt4(vr[u], a.kv_f16);
+                    const float4 v4 = a.pool8 ? kv_cvt4_e4m3(vr[u].x, a.v_scale) : kv_cvt4(vr[u], a.kv_f16);
                     den = __fadd_rn(den, et);
                     num.x = fmaf(et, v4.x, num.x); num.y = fmaf(et, v4.y, num.y); num.z = fmaf(et, v4.z, num.z); num.w = fmaf(et, v4.w, num.w);
                 }

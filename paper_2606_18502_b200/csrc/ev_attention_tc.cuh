@@ -41,8 +41,17 @@ constexpr int TCA_KS = 6;        // K ring depth (a K tile is released by Q.K^T,
 constexpr int TCA_VS = 5;        // V ring depth (a V tile is released by P.V)
 constexpr int TCA_PAGE = 16;      // tokens per page this kernel is built for
 
-template <int D>
+// FP8 = the pool holds E4M3 codes (ev_config.kv_dtype 1; "quantizing the KV cache to FP8 halves the storage"):
+// raw 2-KiB page blocks arrive by linear bulk copies into raw rings, two extra warps (18: K, 19: V) turn each 64-key tile
+// into the fp16, 128-byte-swizzled tile the MMAs read (E4M3 -> fp16 is exact; the static per-tensor scales are applied in
+// fp32: K's in the score multiply, V's when the chunk's partial output is written), everything downstream is unchanged.
+template <int D, bool FP8 = false>
 struct TcaCfg {
+    static constexpr int KS = FP8 ? 4 : TCA_KS;          // fp16 K tiles in flight
+    static constexpr int VS = FP8 ? 4 : TCA_VS;          // fp16 V tiles in flight
+    static constexpr int RS = FP8 ? 4 : 0;               // raw E4M3 tiles in flight, per K and per V
+    static constexpr int RAW_BYTES = TCA_BN * D;         // one raw tile: 64 keys x D bytes
+    static constexpr int THREADS = FP8 ? TCA_THREADS + 64 : TCA_THREADS;
     static constexpr int NH = D / 64;                    // 128-byte (64-element) halves of a head row
     static constexpr int Q_PART = NH * 128 * 128;        // bytes of one bf16 part of the 128 x D query tile
     static constexpr int Q_BYTES = 2 * Q_PART;
@@ -50,9 +59,9 @@ struct TcaCfg {
     static constexpr int K_BYTES = NH * KV_HALF;
     static constexpr int SBO = NH * 1024;               // 8-token groups of one d half: [page][group][half][1 KiB]
     static constexpr int PAGE_BYTES = 2 * SBO;          // one 16-token (page, K|V, head) block
-    static constexpr int BAR_BYTES = 256;
+    static constexpr int BAR_BYTES = 512;
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
-    static constexpr int SMEM = 1024 + (TCA_KS + TCA_VS) * K_BYTES + BAR_BYTES + XCH_BYTES;   // Q lives in TMEM
+    static constexpr int SMEM = 1024 + (KS + VS) * K_BYTES + 2 * RS * RAW_BYTES + BAR_BYTES + XCH_BYTES;   // Q lives in TMEM
     // TMEM columns
     // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
     // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that).  (Three
@@ -149,17 +158,33 @@ constexpr float TCA_PSCALE_LOG2 = 15.f;   // P is scaled by 2^15
 struct TcAttnArgs {
     AttnArgs a;       // same fields as tree_attn_partial_kernel (pool pointer unused here)
     int row0;         // first row of this layer in the pool tensor map: layer * n_pages * 2 * Hkv * 16
+    const uint8_t* pool8;   // FP8: the whole pool as bytes (row r of D codes at pool8 + r * D)
+    float k_scale, v_scale; // FP8: this layer's static K / V cache scales (1 otherwise)
     L2Prefetch pf;
 };
+__device__ __forceinline__ void bulk_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+// 16 E4M3 codes (one 16-byte chunk) -> 16 fp16 values (two 16-byte chunks); exact
+__device__ __forceinline__ void e4m3x16_to_f16(const uint4& in, uint4& lo, uint4& hi) {
+    auto cv = [](uint32_t w, uint32_t& a, uint32_t& b) {
+        asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.rn.f16x2.e4m3x2 %0, l;\n\tcvt.rn.f16x2.e4m3x2 %1, h;\n\t}" : "=r"(a), "=r"(b) : "r"(w));
+    };
+    cv(in.x, lo.x, lo.y); cv(in.y, lo.z, lo.w); cv(in.z, hi.x, hi.y); cv(in.w, hi.z, hi.w);
+}
 
-template <int D>
-__global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
-    using C = TcaCfg<D>;
+template <int D, bool FP8>
+__global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
+    using C = TcaCfg<D, FP8>;
+    constexpr int TCA_KS = C::KS, TCA_VS = C::VS;         // ring depths of this variant (shadow the bf16 defaults)
     const AttnArgs& a = ta.a;
     extern __shared__ uint8_t tca_smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(tca_smem_raw) + 1023) & ~(uintptr_t)1023);
     uint8_t* kv_s = smem;                                 // K ring [KS][NH x 8 KiB] | V ring [VS][NH x 8 KiB]
-    uint64_t* bars = reinterpret_cast<uint64_t*>(kv_s + (TCA_KS + TCA_VS) * C::K_BYTES);
+    uint8_t* raw_s = kv_s + (TCA_KS + TCA_VS) * C::K_BYTES;   // FP8: raw K ring [RS][64 x D B] | raw V ring [RS][64 x D B]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(raw_s + 2 * C::RS * C::RAW_BYTES);
     uint64_t* k_full = bars;                              // [KS]
     uint64_t* k_empty = k_full + TCA_KS;                  // [KS]
     uint64_t* v_full = k_empty + TCA_KS;                  // [VS]
@@ -168,7 +193,9 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     uint64_t* p_full = s_full + C::NSP;                   // [3]
     uint64_t* o_full = p_full + C::NSP;                   // [2]
     uint64_t* o_empty = o_full + 2;                       // [2]
-    uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(o_empty + 2);
+    uint64_t* raw_full = o_empty + 2;                     // FP8: [2][RS] raw tile landed (K ring, then V ring)
+    uint64_t* raw_empty = raw_full + 8;                   // FP8: [2][RS] raw tile converted
+    uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(raw_empty + 8);
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
     float* xsum = xmax + 2 * 2 * 128;                     // [2 wg][128]
     float* xc = xsum + 2 * 128;                           // [8 tiles][128] rescale factor of tile j at [j & 7]
@@ -186,6 +213,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         for (int s = 0; s < TCA_VS; ++s) { mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
         for (int i = 0; i < C::NSP; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
         for (int i = 0; i < 2; ++i) { mbar_init(&o_full[i], 1); mbar_init(&o_empty[i], 8); }
+        if (FP8) for (int i = 0; i < 8; ++i) { mbar_init(&raw_full[i], 1); mbar_init(&raw_empty[i], 1); }   // [K|V][slot], stride 4
         fence_barrier_init();
         tma_prefetch_desc(&tmKV);
     }
@@ -213,7 +241,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
     // ---- Q tile -> TMEM (fp32 x 2^6 -> hi | lo fp16 pairs).  Softmax and correction threads stage it: a warp owns the
     // TMEM lanes of its 32 rows.  Warps 1..17 meet behind named barrier 5; warp 0 goes straight to its K/V
     // loads, which run under the staging (~1.5 us of a 15 us launch at batch 1). ----
-    if (active && warp >= 2) {
+    if (active && warp >= 2 && warp < 18) {
         // softmax AND correction warps: thread = (row, quarter of d); every load is issued before the first split
         const int qd = (warp - 2) >> 2;   // 0..3
         const int r = (warp & 3) * 32 + lane;
@@ -239,7 +267,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         tmem_st_wait();
         tc_fence_before();
     }
-    if (warp != 0) {
+    if (warp != 0 && warp < 18) {
         asm volatile("bar.sync 5, %0;" ::"n"(TCA_THREADS - 32) : "memory");
         tc_fence_after();
     }
@@ -265,7 +293,23 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         // tile for K.  The lane that owns page 0 arms the tile's full barrier (arrive + expected bytes); a box of
         // another lane may complete first - the phase still cannot complete before that arrive.
         const int dst_off = pg * C::PAGE_BYTES;
-        if (lane < OPS) {
+        if (FP8) {
+            // raw E4M3 page blocks: one linear 16-token x D-byte copy per (K|V, page) into the raw ring; lanes 0..3 stream K, 4..7 V
+            if (lane < OPS) {
+                uint64_t* full = raw_full + 4 * kv;
+                uint64_t* empty = raw_empty + 4 * kv;
+                uint8_t* ring = raw_s + kv * C::RS * C::RAW_BYTES;
+                int row_next = box_row(0);
+                for (int j = 0; j < n_tiles; ++j) {
+                    const int row_cur = row_next;
+                    if (j + 1 < n_tiles) row_next = box_row(j + 1);
+                    const int sl = j % C::RS;
+                    mbar_wait(&empty[sl], ((j / C::RS) & 1) ^ 1);
+                    if (pg == 0) mbar_arrive_expect_tx(&full[sl], C::RAW_BYTES);
+                    bulk_load_1d(ring + sl * C::RAW_BYTES + pg * (TCA_PAGE * D), ta.pool8 + (size_t)row_cur * 8 * D, TCA_PAGE * D, &full[sl]);
+                }
+            }
+        } else if (lane < OPS) {
             uint64_t* full = kv ? v_full : k_full;
             uint64_t* empty = kv ? v_empty : k_empty;
             const int depth = kv ? TCA_VS : TCA_KS;
@@ -348,6 +392,41 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
             if (j + LA < n_tiles) issue_qk(j + LA);
             issue_pv(j);
         }
+    } else if (warp >= 18) {
+        // ===== FP8 converters (warp 18: K tiles, warp 19: V tiles): raw [64 keys][D codes] -> fp16 tile in the layout the
+        // 4-D TMA box of the bf16 path produces: [8-key group][d half][8 rows x 128 B], 16-byte chunks XOR-swizzled by row =====
+        if (FP8 && warp < 20) {
+            const int kv = warp - 18;
+            uint64_t* rfull = raw_full + 4 * kv;
+            uint64_t* rempty = raw_empty + 4 * kv;
+            uint64_t* tfull = kv ? v_full : k_full;
+            uint64_t* tempty = kv ? v_empty : k_empty;
+            const int depth = kv ? TCA_VS : TCA_KS;
+            const uint8_t* raw = raw_s + kv * C::RS * C::RAW_BYTES;
+            uint8_t* ring = kv_s + (kv ? TCA_KS * C::K_BYTES : 0);
+            constexpr int CPR = D / 16;               // 16-code chunks per key row
+            for (int j = 0; j < n_tiles; ++j) {
+                const int rs = j % C::RS, ts = j % depth;
+                mbar_wait(&rfull[rs], (j / C::RS) & 1);
+                mbar_wait(&tempty[ts], ((j / depth) & 1) ^ 1);     // the MMAs that read this slot's previous tile have finished
+                const uint8_t* src = raw + rs * C::RAW_BYTES;
+                uint8_t* dst = ring + ts * C::K_BYTES;
+#pragma unroll 4
+                for (int c = lane; c < TCA_BN * CPR; c += 32) {
+                    const int r = c / CPR, j8 = c % CPR;           // key row, chunk of 16 dims
+                    const uint4 in = *reinterpret_cast<const uint4*>(src + r * D + j8 * 16);
+                    uint4 lo, hi;
+                    e4m3x16_to_f16(in, lo, hi);
+                    const int h = j8 >> 2, jj = (j8 & 3) * 2;      // d half (64 dims), first of the two 16-byte chunks inside the 128-byte row
+                    uint8_t* rowp = dst + (r >> 3) * C::SBO + h * 1024 + (r & 7) * 128;
+                    *reinterpret_cast<uint4*>(rowp + ((jj ^ (r & 7)) << 4)) = lo;
+                    *reinterpret_cast<uint4*>(rowp + (((jj + 1) ^ (r & 7)) << 4)) = hi;
+                }
+                fence_proxy_async();      // generic-proxy stores -> visible to the tensor core's async-proxy reads
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(&tfull[ts]); mbar_arrive(&rempty[rs]); }
+            }
+        }
     } else if (warp < 10) {
         // ===== softmax: thread = (row, wg); wg handles keys [32 wg, +32) of every tile.  Warp w may touch TMEM
         // lanes 32 (w % 4) .. +31; the two warps of a row quarter meet behind named barrier 1 + (w % 4). =====
@@ -362,7 +441,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
         float m_run = -INFINITY, l_run = 0.f;   // l_run carries P's factor 2^15
-        const float qk_scale = a.scale * (1.f / TCA_QSCALE);
+        const float qk_scale = FP8 ? mul_rn(a.scale * (1.f / TCA_QSCALE), ta.k_scale) : a.scale * (1.f / TCA_QSCALE);   // FP8: the K cache's static scale rides along
 
         // (max, sum) of a finished chunk go to its partial slot (the two halves of a row meet in shared memory) and the
         // state restarts: t_left counts the tiles left in the current chunk
@@ -449,6 +528,7 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
         for (int i = 0; i < C::DH; ++i) o[i] = 0.f;
         float* op = a.o_part + (((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0) * D + hh * C::DH;
         int t_left = tpc;
+        const float oscale = FP8 ? mul_rn(exp2f(-TCA_PSCALE_LOG2), ta.v_scale) : exp2f(-TCA_PSCALE_LOG2);   // P's 2^15 out (exact); FP8: V's static scale in
         for (int i = 0; i < n_tiles; ++i) {
             mbar_wait(&o_full[i % C::NO], (i / C::NO) & 1);
             tc_fence_after();
@@ -476,8 +556,8 @@ __global__ void __launch_bounds__(TCA_THREADS, 1) tree_attn_tc_kernel(const __gr
                     if (valid) {
 #pragma unroll
                         for (int e = 0; e < 16; e += 4)
-                            *reinterpret_cast<float4*>(op + cb * 16 + e) = make_float4(o[cb * 16 + e] * exp2f(-TCA_PSCALE_LOG2), o[cb * 16 + e + 1] * exp2f(-TCA_PSCALE_LOG2),
-                                                                                       o[cb * 16 + e + 2] * exp2f(-TCA_PSCALE_LOG2), o[cb * 16 + e + 3] * exp2f(-TCA_PSCALE_LOG2));
+                            *reinterpret_cast<float4*>(op + cb * 16 + e) = make_float4(o[cb * 16 + e] * oscale, o[cb * 16 + e + 1] * oscale,
+                                                                                       o[cb * 16 + e + 2] * oscale, o[cb * 16 + e + 3] * oscale);
                     }
 #pragma unroll
                     for (int e = 0; e < 16; ++e) o[cb * 16 + e] = 0.f;

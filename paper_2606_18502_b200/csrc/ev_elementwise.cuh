@@ -489,8 +489,11 @@ struct RopeArgs {
     const int32_t* nn_eff;     // [B]
     const int32_t* page_table; // [max_seqs][max_pages]
     int max_pages, page_size;
-    __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D]
+    __nv_bfloat16* pool;       // this layer: [page][2][Hkv][page_size][D] (2-byte elements; kv_mode 2: 1-byte E4M3 codes, see pool8)
     int kv_f16;                // pool keeps the bf16-rounded values in binary16 containers (ev_common.cuh)
+    uint8_t* pool8;            // kv_dtype 1 (FP8 KV cache): this layer's pool as E4M3 codes, or null
+    float k_scale, v_scale;    // its static per-tensor scales: code = E4M3_sat(x / s)
+    float* kv_amax;            // calibration: [2] running absmax of this layer's K (post-RoPE) and V (atomicMax on the bits), or null
     L2Prefetch pf;
 };
 constexpr int ROPE_THREADS = 256;
@@ -529,7 +532,16 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
         rlo.w = sub_rn(mul_rn(lo.w, c23.z), mul_rn(hi.w, c23.w)); rhi.w = add_rn(mul_rn(hi.w, c23.z), mul_rn(lo.w, c23.w));
         *reinterpret_cast<float4*>(row + head * D + j) = rlo;
         *reinterpret_cast<float4*>(row + head * D + j + D2) = rhi;
-        if (head >= a.Hq && write) {
+        if (head >= a.Hq && a.kv_amax) {
+            const float am = fmaxf(fmaxf(fmaxf(fabsf(rlo.x), fabsf(rlo.y)), fmaxf(fabsf(rlo.z), fabsf(rlo.w))),
+                                   fmaxf(fmaxf(fabsf(rhi.x), fabsf(rhi.y)), fmaxf(fabsf(rhi.z), fabsf(rhi.w))));
+            if (write) atomicMax(reinterpret_cast<int*>(a.kv_amax), __float_as_int(am));
+        }
+        if (head >= a.Hq && write && a.pool8) {
+            uint8_t* kd = a.pool8 + (kdst - a.pool) + (size_t)(head - a.Hq) * a.page_size * D;
+            *reinterpret_cast<uint32_t*>(kd + j) = e4m3x4(div_rn(rlo.x, a.k_scale), div_rn(rlo.y, a.k_scale), div_rn(rlo.z, a.k_scale), div_rn(rlo.w, a.k_scale));
+            *reinterpret_cast<uint32_t*>(kd + j + D2) = e4m3x4(div_rn(rhi.x, a.k_scale), div_rn(rhi.y, a.k_scale), div_rn(rhi.z, a.k_scale), div_rn(rhi.w, a.k_scale));
+        } else if (head >= a.Hq && write) {
             __nv_bfloat16* kd = kdst + (size_t)(head - a.Hq) * a.page_size * D;
             __nv_bfloat162 p0 = __floats2bfloat162_rn(rlo.x, rlo.y), p1 = __floats2bfloat162_rn(rlo.z, rlo.w);
             __nv_bfloat162 p2 = __floats2bfloat162_rn(rhi.x, rhi.y), p3 = __floats2bfloat162_rn(rhi.z, rhi.w);
@@ -545,7 +557,11 @@ __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) 
         const int head = (i * 4) / D, j = (i * 4) % D;
         const float4 v = lin_value4<MAXS>(a.lin, m, voff + i * 4, sxm);
         *reinterpret_cast<float4*>(row + voff + i * 4) = v;
-        if (write) {
+        if (a.kv_amax && write) atomicMax(reinterpret_cast<int*>(a.kv_amax + 1), __float_as_int(fmaxf(fmaxf(fabsf(v.x), fabsf(v.y)), fmaxf(fabsf(v.z), fabsf(v.w)))));
+        if (write && a.pool8) {
+            *reinterpret_cast<uint32_t*>(a.pool8 + (vdst - a.pool) + (size_t)head * a.page_size * D + j) =
+                e4m3x4(div_rn(v.x, a.v_scale), div_rn(v.y, a.v_scale), div_rn(v.z, a.v_scale), div_rn(v.w, a.v_scale));
+        } else if (write) {
             __nv_bfloat162 p0 = __floats2bfloat162_rn(v.x, v.y), p1 = __floats2bfloat162_rn(v.z, v.w);
             uint32_t w0 = *reinterpret_cast<uint32_t*>(&p0), w1 = *reinterpret_cast<uint32_t*>(&p1);
             if (a.kv_f16) { w0 = bf16x2_to_f16x2(w0); w1 = bf16x2_to_f16x2(w1); }
@@ -620,6 +636,7 @@ __global__ void accept_walk_kernel(AcceptArgs a) {
 // sources are never overwritten before they are read (path[j] >= j, strictly increasing), so all
 // moves of a sequence run in parallel.  grid (B, n_layers).
 struct CompactArgs {
+    int eb;             // bytes per pool element: 2 (bf16 / binary16 containers) or 1 (E4M3 codes)
     int T, Hkv, D, page_size, max_pages;
     long layer_stride;  // elements per layer in the pool
     __nv_bfloat16* pool;
@@ -636,8 +653,8 @@ __global__ void __launch_bounds__(EW_THREADS) kv_compact_kernel(CompactArgs a) {
     const int n = a.accept_len[b];
     const int L = a.Lsnap[b];
     const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
-    __nv_bfloat16* pool = a.pool + (size_t)layer * a.layer_stride;
-    const int vec_per_head = a.D / 8;              // uint4 = 8 bf16
+    uint8_t* pool = reinterpret_cast<uint8_t*>(a.pool) + (size_t)layer * a.layer_stride * a.eb;
+    const int vec_per_head = a.D * a.eb / 16;      // 16-byte vectors per (token, K|V, head) row
     const int per_tok = 2 * a.Hkv * vec_per_head;  // K|V x heads
     for (int j = 1; j <= n; ++j) {
         const int src_node = a.accept_nodes[b * a.T + j];
@@ -647,8 +664,8 @@ __global__ void __launch_bounds__(EW_THREADS) kv_compact_kernel(CompactArgs a) {
         const size_t dbase = (size_t)pt[ds / a.page_size] * 2 * a.Hkv * a.page_size * a.D + (size_t)(ds % a.page_size) * a.D;
         for (int i = threadIdx.x; i < per_tok; i += EW_THREADS) {
             const int kvh = i / vec_per_head, c = i % vec_per_head;  // kvh in [0, 2*Hkv)
-            const size_t off = (size_t)kvh * a.page_size * a.D + (size_t)c * 8;
-            *reinterpret_cast<uint4*>(pool + dbase + off) = *reinterpret_cast<const uint4*>(pool + sbase + off);
+            const size_t off = (size_t)kvh * a.page_size * a.D;
+            *reinterpret_cast<uint4*>(pool + (dbase + off) * a.eb + (size_t)c * 16) = *reinterpret_cast<const uint4*>(pool + (sbase + off) * a.eb + (size_t)c * 16);
         }
     }
 }
@@ -662,16 +679,17 @@ struct DenseCopyArgs {
     __nv_bfloat16* dense;      // [layer][2][Hkv][n_tokens][D], always bf16
     int to_dense;
     int kv_f16;                // pool container (ev_common.cuh)
+    int eb;                    // bytes per element: 2, or 1 (E4M3 codes: dense is then uint8 codes too)
 };
 __global__ void __launch_bounds__(128) dense_copy_kernel(DenseCopyArgs a) {
     const int t = blockIdx.x, li = blockIdx.y;
-    __nv_bfloat16* pool = a.pool + (size_t)(a.layer_begin + li) * a.layer_stride;
+    uint8_t* pool = reinterpret_cast<uint8_t*>(a.pool) + (size_t)(a.layer_begin + li) * a.layer_stride * a.eb;
     const size_t pbase = (size_t)a.page_row[t / a.page_size] * 2 * a.Hkv * a.page_size * a.D + (size_t)(t % a.page_size) * a.D;
-    const int vec_per_head = a.D / 8;
+    const int vec_per_head = a.D * a.eb / 16;
     for (int i = threadIdx.x; i < 2 * a.Hkv * vec_per_head; i += 128) {
         const int kvh = i / vec_per_head, c = i % vec_per_head;
-        uint4* p = reinterpret_cast<uint4*>(pool + pbase + (size_t)kvh * a.page_size * a.D + (size_t)c * 8);
-        uint4* d = reinterpret_cast<uint4*>(a.dense + (((size_t)li * 2 * a.Hkv + kvh) * a.n_tokens + t) * a.D + (size_t)c * 8);
+        uint4* p = reinterpret_cast<uint4*>(pool + (pbase + (size_t)kvh * a.page_size * a.D) * a.eb + (size_t)c * 16);
+        uint4* d = reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(a.dense) + ((((size_t)li * 2 * a.Hkv + kvh) * a.n_tokens + t) * a.D) * a.eb + (size_t)c * 16);
         if (a.to_dense) {
             uint4 v = *p;
             if (a.kv_f16) { v.x = f16x2_to_bf16x2(v.x); v.y = f16x2_to_bf16x2(v.y); v.z = f16x2_to_bf16x2(v.z); v.w = f16x2_to_bf16x2(v.w); }

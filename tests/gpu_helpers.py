@@ -16,11 +16,11 @@ def bf16_cuda_to_bits(t):
 
 
 def gpu_model(shape, seed, max_batch, max_tree_nodes, max_ctx, random_gains=False, act_scale_mode=0,
-              page_size=16, device_weights=False, keep=None, weight_scale_mode=0):
+              page_size=16, device_weights=False, keep=None, weight_scale_mode=0, kv_dtype=0, attn_chunk=0):
     """device_weights=True draws the matrices on the GPU (8B shapes); `keep` (dict) then receives
     host copies (uint16 bits) of the (kind, layer) pairs listed in keep['want'] for the oracle."""
     m = ev.Model(shape, max_batch, max_tree_nodes, max_ctx, page_size=page_size, act_scale_mode=act_scale_mode,
-                 weight_scale_mode=weight_scale_mode)
+                 weight_scale_mode=weight_scale_mode, kv_dtype=kv_dtype, attn_chunk=attn_chunk)
 
     def put(kind, layer):
         if device_weights:

@@ -1,0 +1,175 @@
+"""FP8 (E4M3) KV cache ("quantizing the KV cache to FP8 halves the storage"; DESIGN.md
+R-kv8): CUDA path (ev_config.kv_dtype = 1) vs the oracle's kv_dtype="e4m3" mode on the same seeded inputs - calibrated
+K/V scales, cache codes, per-kernel attention tap, free-running verify at the north_star tolerances, acceptance and
+compaction bit-exact, and the GPU's own losslessness (speculative loop == greedy decode) with the FP8 cache."""
+import numpy as np
+import pytest
+
+import workloads as wl
+from oracle import verify_oracle as vo
+from helpers import oracle_model, rel_l2
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+SHAPE = wl.ModelShape("kv8", 3, 512, 8, 2, 128, 1024, 2048, 1e-5, 1e4)
+SEED = 5
+
+
+@pytest.fixture(scope="module")
+def pair():
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import gpu_model
+    gm = gpu_model(SHAPE, SEED, max_batch=4, max_tree_nodes=64, max_ctx=1500, random_gains=True, kv_dtype=1)
+    om = oracle_model(SHAPE, SEED, random_gains=True)
+    calib = np.random.default_rng(SEED + 1).standard_normal((96, SHAPE.hidden)).astype(np.float32)
+    vo.calibrate(om, calib)
+    gm.ev_model_calibrate(torch.from_numpy(calib).cuda())
+    g = gm.ev_model_get_kv_scales()
+    o = np.array([om.static[(k, l)] for l in range(SHAPE.n_layers) for k in ("k_cache", "v_cache")], dtype=np.float32)
+    assert np.all(np.abs(g - o) <= 2e-3 * o), (g, o)          # the GPU's own calibration finds the oracle's scales
+    gm.ev_model_set_kv_scales(o)                               # from here on both sides are ONE model
+    return ev, gm, om
+
+
+def _ocache(om, n):
+    c = vo.OracleKV(om, n // 16 + 2, 16, kv_dtype="e4m3")
+    c.add_seq(0, n)
+    return c
+
+
+def test_fp8_kv_pool_is_half_the_bytes(pair):
+    ev, gm, om = pair
+    free0 = torch.cuda.mem_get_info()[0]
+    c8 = ev.Cache(gm, 4096, 1)
+    used8 = free0 - torch.cuda.mem_get_info()[0]
+    want = 4096 * SHAPE.n_layers * 2 * SHAPE.n_kv_heads * 16 * SHAPE.head_dim           # one byte per element
+    assert want <= used8 <= want + (8 << 20), (used8, want)
+    c8.ev_cache_destroy()
+
+
+def test_fp8_kv_verify_matches_oracle(pair):
+    ev, gm, om = pair
+    from gpu_helpers import run_verify
+    L, T = 333, 26
+    ids = np.random.default_rng(11).integers(0, SHAPE.vocab, size=L).astype(np.int32)
+    parents = wl.tree_parents(T, (4, 3, 2, 2, 1))
+    toks = np.random.default_rng(12).integers(0, SHAPE.vocab, size=T).astype(np.int32)
+    oc = _ocache(om, L + 64)
+    vo.prefill(om, oc, 0, ids)
+    cache = ev.Cache(gm, (L + 64) // 16 + 2, 1)
+    slot = cache.ev_cache_add_seq(L + 64)
+    # (b) the GPU prefills itself: its E4M3 cache codes against the oracle's
+    cache.ev_cache_prefill([slot], [ids])
+    g = cache.ev_cache_export_seq(slot, 0, SHAPE.n_layers, L).cpu().numpy()
+    o = np.stack([oc.export_dense(l, 0, L) for l in range(SHAPE.n_layers)])
+    assert g.dtype == np.uint8 and g.shape == o.shape
+    assert np.mean(g != o) <= 2e-3, np.mean(g != o)            # codes differ only where an upstream E4M3 code flipped
+    assert np.array_equal(g[0], o[0]) or np.mean(g[0] != o[0]) <= 1e-4
+    # (a) verify on the oracle's own cache codes, imported: free-running parity at the literal tolerances
+    cache.ev_cache_import_seq(slot, 0, SHAPE.n_layers, torch.from_numpy(o).cuda(), set_len=True)
+    assert np.array_equal(cache.ev_cache_export_seq(slot, 0, SHAPE.n_layers, L).cpu().numpy(), o)
+    res = vo.verify(om, oc, 0, toks, parents, commit=True, want_hidden=True)
+    taps = {}
+    # oracle per-kernel taps of layer 1 from the oracle's own layer input
+    oc2 = _ocache(om, L + 64)
+    for l in range(SHAPE.n_layers):
+        oc2.import_dense(l, 0, o[l])
+    oc2.ctx_len[0] = L
+    vo.layer_forward(om, 1, res["hidden"][1], oc2, 0, L, parents, taps=taps)
+    buf = run_verify(gm, cache, [slot], toks[None], parents[None], commit=True, tap_layer=1, hidden_override=None)
+    hid = buf.hidden.cpu().numpy()
+    for l, h in enumerate(res["hidden"]):
+        assert rel_l2(hid[l], h) <= 1e-2, (l, rel_l2(hid[l], h))
+    lg = buf.logits.cpu().numpy()
+    assert np.max(np.abs(lg - res["logits"])) <= 2e-2 * res["logits"].std()
+    srt = np.sort(res["logits"], axis=1)
+    if ((srt[:, -1] - srt[:, -2]) >= 1e-3).all():
+        a = res["accept_len"]
+        assert buf.accept_len.cpu().tolist() == [a]
+        assert buf.accept_nodes.cpu().numpy()[0, :a + 1].tolist() == res["path"]
+        assert buf.out_tokens.cpu().numpy()[0, :a + 1].tolist() == res["out_tokens"]
+        # compacted cache == the oracle's compacted cache, code for code
+        n = L + a + 1
+        gc = cache.ev_cache_export_seq(slot, 0, SHAPE.n_layers, n).cpu().numpy()
+        ocd = np.stack([oc.export_dense(l, 0, n) for l in range(SHAPE.n_layers)])
+        assert np.mean(gc != ocd) <= 2e-3
+
+
+def test_fp8_kv_attention_tap_lock_step(pair):
+    """attention output of one layer from the oracle's layer input and the oracle's cache codes: <= 1e-5 (exact products of
+    fp16 x E4M3-in-fp16 operands, fp32 sums; the static scales applied in fp32)"""
+    ev, gm, om = pair
+    from gpu_helpers import run_verify
+    L, T = 1100, 60            # more than one attention chunk of 1024
+    ids = np.random.default_rng(21).integers(0, SHAPE.vocab, size=L).astype(np.int32)
+    parents = wl.tree_parents(T, (4, 3, 2, 2, 1, 1))
+    toks = np.random.default_rng(22).integers(0, SHAPE.vocab, size=T).astype(np.int32)
+    oc = _ocache(om, L + 64)
+    vo.prefill(om, oc, 0, ids)
+    o = np.stack([oc.export_dense(l, 0, L) for l in range(SHAPE.n_layers)])
+    cache = ev.Cache(gm, (L + 64) // 16 + 2, 1)
+    slot = cache.ev_cache_add_seq(L + 64)
+    cache.ev_cache_import_seq(slot, 0, SHAPE.n_layers, torch.from_numpy(o).cuda(), set_len=True)
+    ref = vo.verify(om, oc, 0, toks, parents, commit=False, want_hidden=True)
+    hid_in = np.stack(ref["hidden"])                    # lock-step: every layer reads the oracle's input
+    for layer in (0, 2):
+        taps = {}
+        vo.layer_forward(om, layer, ref["hidden"][layer], oc, 0, L, parents, taps=taps)
+        buf = run_verify(gm, cache, [slot], toks[None], parents[None], commit=False, tap_layer=layer, hidden_override=hid_in)
+        t = {k: v.cpu().numpy() for k, v in buf.taps.items()}
+        assert rel_l2(t["attn"], taps["attn"]) <= 1e-5, (layer, rel_l2(t["attn"], taps["attn"]))
+        assert np.mean(t["aq"] != taps["aq"]) <= 1e-3
+        # appended tree K/V codes
+        g = cache.ev_cache_export_seq(slot, layer, layer + 1, L + T).cpu().numpy()[0][:, :, L:]
+        oo = oc.export_dense(layer, 0, L + T)[:, :, L:]
+        assert np.mean(g != oo) <= 2e-3
+
+
+def test_fp8_kv_gpu_speculative_equals_gpu_greedy(pair):
+    ev, gm, om = pair
+    from gpu_helpers import run_verify
+    B, T, L = 3, 26, 700
+    parents = wl.tree_parents(T, (4, 3, 2, 2, 1))
+    rng = np.random.default_rng(31)
+    ids = [rng.integers(0, SHAPE.vocab, size=L + 37 * b).astype(np.int32) for b in range(B)]
+    cache = ev.Cache(gm, 2 * B * ((L + 300) // 16 + 2), 2 * B)
+    s_slots = [cache.ev_cache_add_seq(L + 300) for _ in range(B)]
+    g_slots = [cache.ev_cache_add_seq(L + 300) for _ in range(B)]
+    cache.ev_cache_prefill(s_slots + g_slots, ids + ids)
+    roots = rng.integers(0, SHAPE.vocab, size=B).astype(np.int32)
+    n_greedy = 80
+    greedy = np.zeros((B, n_greedy), dtype=np.int32)
+    tok = roots.copy()
+    for s in range(n_greedy):
+        buf = run_verify(gm, cache, g_slots, tok[:, None], np.full((B, 1), -1, np.int32), commit=True, want_logits=False, want_hidden=False)
+        tok = buf.out_tokens.cpu().numpy()[:, 0].astype(np.int32)
+        greedy[:, s] = tok
+    first = {}
+    for i in range(1, T):
+        first.setdefault(int(parents[i]), i)
+    chain, cur = [], 0
+    while cur in first:
+        cur = first[cur]
+        chain.append(cur)
+    emitted = [[] for _ in range(B)]
+    root = roots.copy()
+    acc_total = 0
+    for step in range(10):
+        tokens = rng.integers(0, SHAPE.vocab, size=(B, T)).astype(np.int32)
+        for b in range(B):
+            tokens[b, 0] = root[b]
+            for d, node in enumerate(chain):
+                if rng.random() < 0.7:
+                    tokens[b, node] = greedy[b, len(emitted[b]) + d]
+        buf = run_verify(gm, cache, s_slots, tokens, np.tile(parents, (B, 1)), commit=True, want_logits=False, want_hidden=False)
+        acc, outs = buf.accept_len.cpu().numpy(), buf.out_tokens.cpu().numpy()
+        for b in range(B):
+            emitted[b] += outs[b, :acc[b] + 1].tolist()
+            root[b] = outs[b, acc[b]]
+            acc_total += int(acc[b])
+    for b in range(B):
+        assert emitted[b] == greedy[b, :len(emitted[b])].tolist(), b
+    assert acc_total >= 10
+    n0 = len(ids[0]) + len(emitted[0])
+    assert torch.equal(cache.ev_cache_export_seq(s_slots[0], 0, SHAPE.n_layers, n0), cache.ev_cache_export_seq(g_slots[0], 0, SHAPE.n_layers, n0))

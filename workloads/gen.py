@@ -5,7 +5,7 @@ import numpy as np
 
 # matrix kinds; ids are part of the seed derivation, do not renumber
 MATRIX_KINDS = {"embed": 0, "wq": 1, "wk": 2, "wv": 3, "wo": 4, "wgate": 5, "wup": 6,
-                "wdown": 7, "lm_head": 8}
+                "wdown": 7, "lm_head": 8, "d_fc": 9}
 _STREAM_WEIGHTS, _STREAM_INPUTS, _STREAM_CALIB = 0, 1, 2
 
 
@@ -14,7 +14,7 @@ def matrix_shape(shape, kind):
     H, F, V = shape.hidden, shape.ffn, shape.vocab
     return {"embed": (V, H), "wq": (shape.q_dim, H), "wk": (shape.kv_dim, H),
             "wv": (shape.kv_dim, H), "wo": (H, shape.q_dim), "wgate": (F, H), "wup": (F, H),
-            "wdown": (H, F), "lm_head": (V, H)}[kind]
+            "wdown": (H, F), "lm_head": (V, H), "d_fc": (H, 2 * H)}[kind]
 
 
 def f32_to_bf16_bits(x):
