@@ -68,12 +68,12 @@ def tree_of(spec):
     return wl.chain_parents(spec.n_nodes) if spec.tree_caps is None else wl.tree_parents(spec.n_nodes, spec.tree_caps)
 
 
-def algorithmic_work(spec, ctx_lens, parents):
+def algorithmic_work(spec, ctx_lens, parents, kv_fp8=False):
     """bytes = FP8 weight bytes + KV bytes of the context; FLOPs = linear + attention."""
     m = spec.model
     depth = wl.tree_depths(parents)
     B, T = len(ctx_lens), len(parents)
-    kv_bytes = m.kv_bytes_per_token() * int(np.sum(ctx_lens))
+    kv_bytes = m.kv_bytes_per_token() * int(np.sum(ctx_lens)) // (2 if kv_fp8 else 1)
     w_bytes = m.weight_bytes_fp8()
     lin = B * T * m.linear_flops_per_token()
     attn = m.attn_flops_per_token_pos() * int(sum(int(L) * T + int((depth + 1).sum()) for L in ctx_lens))
@@ -138,7 +138,7 @@ def plant(spec, parents, b, root, greedy_next, coins):
     return tk
 
 
-def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0):
+def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0, kv_fp8=False):
     shape = spec.model
     B, T = spec.batch, spec.n_nodes
     parents = tree_of(spec)
@@ -148,15 +148,15 @@ def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0):
     max_ctx = int(ctx.max()) + 64 + 8 + grow
     t0 = time.time()
     model = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=max_ctx, page_size=spec.page_size,
-                     act_scale_mode=spec.act_scale_mode)
+                     act_scale_mode=spec.act_scale_mode, kv_dtype=1 if kv_fp8 else 0)
     for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
         model.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
     torch.cuda.synchronize()
     log(f"weights quantized in {time.time() - t0:.1f}s")
-    if spec.act_scale_mode == 1:
-        calib = torch.from_numpy(wl.calibration_hidden(spec)).cuda()
+    if spec.act_scale_mode == 1 or kv_fp8:
+        calib = torch.from_numpy(wl.calibration_hidden(spec, None if spec.calib_tokens else 512)).cuda()
         model.ev_model_calibrate(calib)
-        log("calibrated static activation scales")
+        log("calibrated static scales (activations: config[4] only; K/V cache: --kv fp8)")
     pages = sum((int(L) + 64 + grow + spec.page_size - 1) // spec.page_size + 1 for L in ctx)
     cache = ev.Cache(model, pages, B)
     slots = [cache.ev_cache_add_seq(int(L) + 64 + grow) for L in ctx]
@@ -255,7 +255,8 @@ def whole_job_rate(units_per_rank, world, ms_per_step):
 def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, steps, with_cpu, fp8_peak):
     """Builds the workload of one config, times `steps` verify steps (device events), the per-class pass, the end-to-end
     leg through ev_verify_host and - with --loop - the sustained closed loop.  Returns the JSON line as a dict."""
-    wk = build_gpu_workload(spec, warmup + steps, torch, ev, log, loop_steps=args.loop)
+    kv_fp8 = args.kv == "fp8"
+    wk = build_gpu_workload(spec, warmup + steps, torch, ev, log, loop_steps=args.loop, kv_fp8=kv_fp8)
     model, cache, slots, ctx, parents, tokens = (wk[k] for k in ("model", "cache", "slots", "ctx", "parents", "tokens"))
     B, T = tokens.shape
     L0 = [int(x) for x in ctx]
@@ -303,7 +304,7 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
         step()
     prof = model.ev_profile_read()
     model.ev_profile_enable(False)
-    work = algorithmic_work(spec, ctx, parents)
+    work = algorithmic_work(spec, ctx, parents, kv_fp8)
     pk = peaks()
     gemm_ms = sum(v[0] for k, v in prof.items() if k.startswith("gemm_"))
     gemm_n = sum(v[1] for k, v in prof.items() if k.startswith("gemm_"))
@@ -413,10 +414,11 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
     line = {
         "metric": METRIC, "value": round(whole_job_rate(B * T, world, ms_step), 1), "unit": "tree-tokens/s", "n_gpus": world,
         "steps": steps, "warmup": warmup, "ms_per_step": round(ms_step, 4), "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "e4m3 x e4m3 -> f32 (bf16 KV, f32 residual)", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": f"e4m3 x e4m3 -> f32 ({'E4M3' if kv_fp8 else 'bf16'} KV, f32 residual)", "data": "synthetic",
         "config": {"workload": spec.name, "batch_per_gpu": B, "tree_nodes": T, "context": L0 if B <= 4 else [min(L0), max(L0)],
                    "cache_state": "cold: 7.5 GB of weights + KV exceed the 126 MB L2 every step", "replicas": world,
-                   "attn_chunk": "library default for this max_batch / max_ctx (ev_config.attn_chunk = 0)"},
+                   "attn_chunk": "library default for this max_batch / max_ctx (ev_config.attn_chunk = 0)",
+                   "kv_cache": "E4M3, static per-tensor scales (PAPER.md:98; ev_config.kv_dtype = 1)" if kv_fp8 else "bf16 (BASELINE.json configs)"},
         "accepted_tokens_per_s": round(world * int(acc.sum()) / (ms_step * 1e-3), 1),
         "emitted_tokens_per_s": round(world * emitted / (ms_step * 1e-3), 1),
         "mean_emitted_per_step": round(emitted / B, 3),
@@ -451,6 +453,7 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--loop", type=int, default=0, help="also run a sustained closed loop of this many committed steps")
+    ap.add_argument("--kv", default="bf16", choices=["bf16", "fp8"], help="KV cache: bf16 (the configs' format) or fp8 = E4M3 (PAPER.md:98, SURVEY 8(f)-2)")
     ap.add_argument("--also", default="auto", help="configs whose short line is added under 'also' (default: 2 = batch 32 "
                                                    "when the headline config 1 runs on one GPU; 'none' to skip)")
     args = ap.parse_args()

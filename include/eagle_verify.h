@@ -90,7 +90,9 @@ typedef enum {
     EV_W_EMBED = 0, /* [vocab][hidden] bf16, kept bf16 */
     EV_W_Q = 1, EV_W_K = 2, EV_W_V = 3, EV_W_O = 4, EV_W_GATE = 5, EV_W_UP = 6, EV_W_DOWN = 7,
     EV_W_LM_HEAD = 8,                    /* 1..8: quantized to E4M3 on arrival */
-    EV_W_NORM1 = 9, EV_W_NORM2 = 10, EV_W_NORMF = 11 /* RMSNorm gains [hidden] bf16; default 1.0 */
+    EV_W_NORM1 = 9, EV_W_NORM2 = 10, EV_W_NORMF = 11, /* RMSNorm gains [hidden] bf16; default 1.0 */
+    EV_W_DRAFT_FC = 12  /* draft models only: [hidden][2*hidden] bf16 -> E4M3, the EAGLE front end that maps
+                           [embedding ; predecessor feature] to the draft layer's input (no bias) */
 } ev_weight_kind;
 
 /* ---- model: quantize / calibrate weights -------------------------------------------------- */
@@ -196,6 +198,8 @@ typedef struct {
                                      its input from slice l instead of the previous layer's output
                                      (slice n_layers feeds the LM head); or NULL */
     int override_first_only;    /* 1 = only slice 0 (replaces the embedding) is read */
+    const float* dev_features;  /* draft models (EV_W_DRAFT_FC set): [B*T][hidden] predecessor feature of every node; the
+                                   layer-0 input is FC(Q8([embed(token) ; feature])) instead of the embedding; or NULL */
 } ev_verify_in;
 
 typedef struct {
@@ -217,6 +221,11 @@ typedef struct {
     float* dev_tap_hmid;                         /* residual after O-proj [M][hidden] */
     float* dev_tap_gu;                           /* gate|up GEMM output [M][2*ffn] */
     uint8_t* dev_tap_tq;  float* dev_tap_st;     /* SwiGLU + quant: [M][ffn] codes, [M] scales */
+    float* dev_final_hidden;    /* optional [B*T][hidden]: the residual stream after the last layer = the "feature" an EAGLE
+                                   drafter consumes (target) / predicts (draft model); graph-captured like the rest */
+    int32_t* dev_topk;          /* optional [B*T][topk]: the topk tokens with the largest logits per node, largest first,
+                                   ties to the lower id (tree expansion); topk <= 8 */
+    int topk;
 } ev_verify_out;
 
 /* One verify step for B sequences.  M = B*T rows are processed together by
@@ -233,6 +242,40 @@ int ev_verify_host(ev_model*, ev_cache*, int n_seqs, int n_nodes, const int32_t*
                    const int32_t* host_tokens, const int32_t* host_parents, const int32_t* host_n_nodes,
                    int commit, int32_t* host_accept_len, int32_t* host_accept_nodes,
                    int32_t* host_out_tokens, int32_t* host_new_ctx_len, int32_t* host_status, void* stream);
+
+/* ---- draft side (architecture from the EAGLE paper the paper cites) -----------
+ * A draft model is an ev_model with n_layers = 1 of the target's shape, its seven layer matrices, EV_W_DRAFT_FC, and the
+ * target's embedding / final norm / LM head (ev_model_share_head: pointers, no copy; the target must outlive the drafter).
+ * It keeps its own ev_cache.  Node p's input is [embed(token_p) ; feature_{p-1}]: committed positions use the TARGET's
+ * features (ev_draft_extend after every verify step), draft nodes the drafter's own prediction for their parent. */
+int ev_model_share_head(ev_model* drafter, ev_model* target);
+
+typedef struct {
+    int n_seqs, n_nodes;               /* B, T */
+    const int32_t* dev_seq_slots;      /* [B] slots in the drafter's cache */
+    const int32_t* host_parents;       /* [T] ONE static topology for the batch, nodes ordered by depth, parents[0] = -1 */
+    const int32_t* dev_root_tokens;    /* [B] last emitted token of every sequence */
+    const float* dev_root_feats;       /* [B][hidden] target feature preceding the root */
+    int32_t* dev_tokens;               /* out [B][T]: the drafted tree's tokens (node 0 = root) */
+    int32_t* dev_parents;              /* out [B][T]: the topology per sequence, as ev_verify takes it */
+} ev_draft_args;
+/* Expands the static tree level by level on the stream (no host sync): level d runs the drafter over the nodes of depth <= d
+ * (rows are independent given their ancestors, so re-running earlier levels changes nothing), takes every node's top-k
+ * tokens, and gives the child of rank r the parent's (r+1)-th best token and the parent's predicted feature.  The
+ * drafter's cache is NOT advanced (draft nodes are scratch).  A chain topology is greedy drafting. */
+int ev_draft_tree(ev_model* drafter, ev_cache* dcache, const ev_draft_args*, void* stream);
+/* Commits tokens to the drafter's cache with the given predecessor features: dev_tokens [B][T], dev_feats [B][T][hidden],
+ * dev_n [B] tokens in use per sequence (chains; every node kept; ctx_len += n). */
+int ev_draft_extend(ev_model* drafter, ev_cache* dcache, int n_seqs, int n_nodes, const int32_t* dev_seq_slots,
+                    const int32_t* dev_tokens, const float* dev_feats, const int32_t* dev_n, void* stream);
+/* After a target verify step: builds ev_draft_extend's inputs from the accepted path - row j <= a of sequence b holds the
+ * accepted node's token and the TARGET feature of the accepted node before it (row 0: dev_carry[b], the feature preceding the
+ * old root) - then dev_next_root[b] = the bonus token and dev_carry[b] = the feature of the last accepted node.  All device
+ * pointers: tokens/accept_nodes/out_tokens [B][T], accept_len [B], feat [B][T][hidden] (ev_verify_out.dev_final_hidden),
+ * carry [B][hidden], ext_tokens [B][T], ext_feats [B][T][hidden], ext_n [B], next_root [B]. */
+int ev_gather_accepted(int n_seqs, int n_nodes, int hidden, const int32_t* dev_tokens, const int32_t* dev_accept_len,
+                       const int32_t* dev_accept_nodes, const int32_t* dev_out_tokens, const float* dev_feat, float* dev_carry,
+                       int32_t* dev_ext_tokens, float* dev_ext_feats, int32_t* dev_ext_n, int32_t* dev_next_root, void* stream);
 
 /* ---- single operators (per-kernel parity tests; same kernels the step uses) ------------------ */
 

@@ -434,7 +434,7 @@ class OracleKV:
     def export_dense(self, layer, seq, n_tokens):
         """-> stored bits [2, Hkv, n_tokens, d] (the layout of the library's export, per layer)."""
         kb, vb = self.read_bits(layer, seq, 0, n_tokens)
-        return np.stack([kb.transpose(1, 0, 2), vb.transpose(1, 0, 2)])
+        return np.ascontiguousarray(np.stack([kb.transpose(1, 0, 2), vb.transpose(1, 0, 2)]))
 
     def import_dense(self, layer, seq, dense_bits):
         """dense_bits (stored bits) [2, Hkv, n, d] -> slots 0..n-1 of seq (DESIGN.md R-kv-input)."""

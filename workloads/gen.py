@@ -123,7 +123,8 @@ def match_coins(spec, seq, n):
     return _rng(spec.seed, _STREAM_INPUTS, 3, seq).random(n)
 
 
-def calibration_hidden(spec):
-    """config[4]: N(0,1) hidden states [calib_tokens, hidden], fp32."""
+def calibration_hidden(spec, n_tokens=None):
+    """config[4]: N(0,1) hidden states [calib_tokens, hidden], fp32.  n_tokens overrides the count for configs that state no
+    calibration batch (FP8 KV cache scales, DESIGN.md R-kv8: config[4]'s recipe, 512 tokens)."""
     return _rng(spec.seed, _STREAM_CALIB).standard_normal(
-        (spec.calib_tokens, spec.model.hidden), dtype=np.float32)
+        (n_tokens or spec.calib_tokens, spec.model.hidden), dtype=np.float32)
