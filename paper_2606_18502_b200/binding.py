@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libeagle_verify.so")
 
 EV_OK, EV_EINVAL, EV_ENOMEM, EV_ECAPACITY, EV_ECUDA, EV_ESTATE = 0, -1, -2, -3, -4, -5
-EV_W = dict(embed=0, wq=1, wk=2, wv=3, wo=4, wgate=5, wup=6, wdown=7, lm_head=8, norm1=9, norm2=10, normf=11)
+EV_W = dict(embed=0, wq=1, wk=2, wv=3, wo=4, wgate=5, wup=6, wdown=7, lm_head=8, norm1=9, norm2=10, normf=11, d_fc=12)
 EV_SEQ_BAD_TREE, EV_SEQ_BAD_TOKEN, EV_SEQ_OVER_CAPACITY = 1, 2, 4
 
 
@@ -33,7 +33,7 @@ class ev_verify_in(C.Structure):
     _fields_ = [("n_seqs", C.c_int), ("n_nodes_max", C.c_int), ("dev_seq_slots", C.c_void_p),
                 ("dev_tokens", C.c_void_p), ("dev_parents", C.c_void_p), ("dev_n_nodes", C.c_void_p),
                 ("commit", C.c_int), ("force_accept_all", C.c_int), ("dev_hidden_override", C.c_void_p),
-                ("override_first_only", C.c_int)]
+                ("override_first_only", C.c_int), ("dev_features", C.c_void_p)]
 
 
 class ev_verify_out(C.Structure):
@@ -43,7 +43,13 @@ class ev_verify_out(C.Structure):
                 ("dev_tap_xq", C.c_void_p), ("dev_tap_sx", C.c_void_p), ("dev_tap_qkv", C.c_void_p),
                 ("dev_tap_attn", C.c_void_p), ("dev_tap_aq", C.c_void_p), ("dev_tap_sa", C.c_void_p),
                 ("dev_tap_hmid", C.c_void_p), ("dev_tap_gu", C.c_void_p), ("dev_tap_tq", C.c_void_p),
-                ("dev_tap_st", C.c_void_p)]
+                ("dev_tap_st", C.c_void_p), ("dev_final_hidden", C.c_void_p), ("dev_topk", C.c_void_p), ("topk", C.c_int)]
+
+
+class ev_draft_args(C.Structure):
+    _fields_ = [("n_seqs", C.c_int), ("n_nodes", C.c_int), ("dev_seq_slots", C.c_void_p), ("host_parents", C.c_void_p),
+                ("dev_root_tokens", C.c_void_p), ("dev_root_feats", C.c_void_p), ("dev_tokens", C.c_void_p),
+                ("dev_parents", C.c_void_p)]
 
 
 # every symbol include/eagle_verify.h declares: name -> (restype, argtypes)
@@ -77,6 +83,10 @@ SIGNATURES = {
     "ev_op_linear": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
     "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
     "ev_last_error": (C.c_char_p, []),
+    "ev_model_share_head": (C.c_int, [_P, _P]),
+    "ev_draft_tree": (C.c_int, [_P, _P, C.POINTER(ev_draft_args), _P]),
+    "ev_draft_extend": (C.c_int, [_P, _P, C.c_int, C.c_int, _P, _P, _P, _P, _P]),
+    "ev_gather_accepted": (C.c_int, [C.c_int, C.c_int, C.c_int, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P]),
     "ev_launch_count": (C.c_long, [C.c_int]),
     "ev_capture_count": (C.c_long, [C.c_int]),
     "ev_version": (C.c_int, []),
@@ -324,7 +334,8 @@ class Cache:
 class VerifyBuffers:
     """Device buffers of one ev_verify call, allocated once and reused (no allocation per step)."""
 
-    def __init__(self, model, B, T, want_logits=False, want_hidden=False, want_argmax=True, tap_layer=-1):
+    def __init__(self, model, B, T, want_logits=False, want_hidden=False, want_argmax=True, tap_layer=-1,
+                 want_final_hidden=False, topk=0):
         import torch
         c = model.cfg
         i32 = dict(dtype=torch.int32, device="cuda")
@@ -342,6 +353,9 @@ class VerifyBuffers:
         self.logits = torch.empty((B * T, c.vocab), dtype=torch.float32, device="cuda") if want_logits else None
         self.hidden = torch.empty((c.n_layers + 1, B * T, c.hidden), dtype=torch.float32, device="cuda") if want_hidden else None
         self.hidden_override = None
+        self.features = None           # draft models: [B*T, hidden] fp32 predecessor features
+        self.final_hidden = torch.empty((B * T, c.hidden), dtype=torch.float32, device="cuda") if want_final_hidden else None
+        self.topk = torch.zeros((B * T, topk), **i32) if topk else None
         self.tap_layer = tap_layer
         self.taps = {}
         if tap_layer >= 0:
@@ -370,7 +384,7 @@ def ev_verify(model, cache, buf, commit=True, use_n_nodes=True, override_first_o
     vin = ev_verify_in(buf.B, buf.T, buf.seq_slots.data_ptr(), buf.tokens.data_ptr(), buf.parents.data_ptr(),
                        buf.n_nodes.data_ptr() if use_n_nodes else None, 1 if commit else 0, 0,
                        buf.hidden_override.data_ptr() if buf.hidden_override is not None else None,
-                       1 if override_first_only else 0)
+                       1 if override_first_only else 0, buf.features.data_ptr() if buf.features is not None else None)
     t = buf.taps
     g = lambda k: t[k].data_ptr() if k in t else None  # noqa: E731
     vout = ev_verify_out(buf.accept_len.data_ptr(), buf.accept_nodes.data_ptr(), buf.out_tokens.data_ptr(),
@@ -378,7 +392,9 @@ def ev_verify(model, cache, buf, commit=True, use_n_nodes=True, override_first_o
                          buf.argmax.data_ptr() if buf.argmax is not None else None,
                          buf.logits.data_ptr() if buf.logits is not None else None,
                          buf.hidden.data_ptr() if buf.hidden is not None else None, buf.tap_layer,
-                         g("xq"), g("sx"), g("qkv"), g("attn"), g("aq"), g("sa"), g("hmid"), g("gu"), g("tq"), g("st"))
+                         g("xq"), g("sx"), g("qkv"), g("attn"), g("aq"), g("sa"), g("hmid"), g("gu"), g("tq"), g("st"),
+                         buf.final_hidden.data_ptr() if buf.final_hidden is not None else None,
+                         buf.topk.data_ptr() if buf.topk is not None else None, buf.topk.shape[1] if buf.topk is not None else 0)
     _check(model.lib.ev_verify(model.h, cache.h, C.byref(vin), C.byref(vout), _stream()))
 
 
@@ -391,3 +407,35 @@ def ev_verify_host(model, cache, host, commit=True):
     _check(model.lib.ev_verify_host(model.h, cache.h, B, T, p("seq_slots"), p("tokens"), p("parents"), p("n_nodes"),
                                     1 if commit else 0, p("accept_len"), p("accept_nodes"), p("out_tokens"),
                                     p("new_ctx_len"), p("status"), _stream()))
+
+
+# ---- draft side (include/eagle_verify.h "draft side") ------------------------------------------------------------
+
+def ev_model_share_head(drafter, target):
+    _check(drafter.lib.ev_model_share_head(drafter.h, target.h))
+    drafter._target = target          # the target must outlive the drafter
+
+
+def ev_draft_tree(drafter, dcache, seq_slots, parents, root_tokens, root_feats, tokens_out, parents_out):
+    """seq_slots [B] int32 cuda, parents: host int32 numpy [T], root_tokens [B] int32 cuda, root_feats [B, H] f32 cuda,
+    tokens_out / parents_out [B, T] int32 cuda (filled)."""
+    import numpy as np
+    par = np.ascontiguousarray(parents, dtype=np.int32)
+    B, T = tokens_out.shape
+    a = ev_draft_args(B, T, seq_slots.data_ptr(), par.ctypes.data_as(C.c_void_p), root_tokens.data_ptr(), root_feats.data_ptr(),
+                      tokens_out.data_ptr(), parents_out.data_ptr())
+    _check(drafter.lib.ev_draft_tree(drafter.h, dcache.h, C.byref(a), _stream()))
+
+
+def ev_draft_extend(drafter, dcache, seq_slots, tokens, feats, n):
+    """tokens [B, T] int32, feats [B, T, H] f32, n [B] int32, seq_slots [B] int32: all cuda."""
+    B, T = tokens.shape
+    _check(drafter.lib.ev_draft_extend(drafter.h, dcache.h, B, T, seq_slots.data_ptr(), tokens.data_ptr(), feats.data_ptr(), n.data_ptr(), _stream()))
+
+
+def ev_gather_accepted(tokens, accept_len, accept_nodes, out_tokens, feat, carry, ext_tokens, ext_feats, ext_n, next_root):
+    B, T = tokens.shape
+    H = carry.shape[1]
+    _check(load_library().ev_gather_accepted(B, T, H, tokens.data_ptr(), accept_len.data_ptr(), accept_nodes.data_ptr(), out_tokens.data_ptr(),
+                                             feat.data_ptr(), carry.data_ptr(), ext_tokens.data_ptr(), ext_feats.data_ptr(), ext_n.data_ptr(),
+                                             next_root.data_ptr(), _stream()))

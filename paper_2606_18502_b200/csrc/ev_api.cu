@@ -14,6 +14,7 @@
 #include "ev_attention.cuh"
 #include "ev_attention_tc.cuh"
 #include "ev_common.cuh"
+#include "ev_drafter.cuh"
 #include "ev_elementwise.cuh"
 #include "ev_gemm.cuh"
 
@@ -132,7 +133,7 @@ struct AttnPlan { int n_splits, split_len; };
 constexpr int TRACE_CAP = 1024;
 struct GraphKey {
     int B, T, commit, force_all, n_splits, split_len, need_lm, pad;
-    const void* p[12];
+    const void* p[16];
 };
 struct GraphEntry { GraphKey key; cudaGraphExec_t exec; long launches; unsigned long stamp; };
 constexpr size_t MAX_GRAPHS = 16;
@@ -192,6 +193,21 @@ struct ev_model {
     cudaStream_t cap_stream = nullptr;
     std::vector<GraphEntry> graphs;
     unsigned long graph_clock = 0;
+    // draft side (ev_drafter.cuh): EAGLE front end and tree-expansion workspaces; all null / empty on a target model
+    QMat fc;                         // EV_W_DRAFT_FC [H][2H]
+    bool have_fc = false, shared_head = false;
+    ActBuf fq;                       // codes of [embed ; feature], K = 2H
+    float* logits_ws = nullptr;      // [M_cap][vocab] when top-k is asked for without a logits output
+    int32_t* d_topk = nullptr;       // [M_cap][TOPK_MAX]
+    float* d_fhat = nullptr;         // [M_cap][H] predicted features of the last drafter pass
+    float* d_feats = nullptr;        // [M_cap][H] predecessor features of the tree being drafted
+    int32_t* d_scratch = nullptr;    // required verify outputs of the drafter passes nobody reads
+    int32_t* d_topo = nullptr;       // [2][T] parents, child ranks of the static topology
+    int32_t* d_lvl_n = nullptr;      // [levels][max_batch] nodes in use per level
+    std::vector<int32_t> h_topo;     // host copy of the topology last uploaded
+    int32_t* d_tree_par = nullptr;   // [M_cap] that topology replicated per sequence (row stride T)
+    int32_t* d_chain_par = nullptr;  // [M_cap] chain parents (i - 1) at row stride chain_T
+    int chain_T = 0;
     std::vector<void*> allocs;
     std::vector<ev_cache*> caches;   // caches created on this model (their model pointer is cleared if the model dies first)
 };
@@ -603,6 +619,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     const float* ovr = in->dev_hidden_override;
     if (ovr) {
         EV_TRY(copy_f32(st, ovr, m->h, (long)M * H));
+    } else if (in->dev_features) {
+        // draft model (ev_drafter.cuh): layer-0 input = FC(Q8([embed(token) ; predecessor feature]))
+        QuantOut q;
+        q.codes = m->fq.codes; q.sx = m->fq.scale; q.static_scale = nullptr; q.site_amax = nullptr; q.clip_count = nullptr;
+        EV_TRY(launch_k(concat_quant_kernel, dim3(M), dim3(EW_THREADS), 0, st, in->dev_tokens, cfg.vocab, m->embed, in->dev_features, H, q));
+        LinOut fl;
+        EV_TRY(run_linear(m, st, m->fc, m->fq, M, EPI_RAW, &fl, nullptr, nullptr, PC_OTHER));
+        EV_TRY(launch_k(materialize_linear_kernel, dim3(M), dim3(256), 0, st, m->h, H, fl));
     } else {
         EV_TRY(launch_k(embed_gather_kernel, dim3(M), dim3(EW_THREADS), 0, st, in->dev_tokens, cfg.vocab, m->embed, H, m->h));
     }
@@ -742,7 +766,14 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
             ROW_DISPATCH_S(rp_h, pend.p ? pend.splits : 1, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers), pfp.take(false));
             pend = none;
         }
-        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, out->dev_logits, m->argmax_keys, PC_GEMM_LM, &pfp));
+        if (out->dev_final_hidden) EV_TRY(copy_f32(st, m->h, out->dev_final_hidden, (long)M * H));   // the final norm kernel wrote the residual back
+        float* lg = out->dev_logits ? out->dev_logits : (out->dev_topk ? m->logits_ws : nullptr);
+        EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, lg, m->argmax_keys, PC_GEMM_LM, &pfp));
+        if (out->dev_topk) {
+            TopkArgs ta;
+            ta.logits = lg; ta.V = cfg.vocab; ta.K = out->topk; ta.T = T; ta.nn_eff = m->nn_eff; ta.out = out->dev_topk;
+            EV_TRY(launch_k(topk_kernel, dim3(M), dim3(256), 0, st, ta));
+        }
     }
     m->n_traced = pfp.n_traced;
     AcceptArgs ac;
@@ -984,6 +1015,25 @@ int ev_model_set_weight(ev_model* m, int kind, int layer, const void* dev_bf16, 
             __nv_bfloat16** dst = kind == EV_W_NORM1 ? &m->layers[layer].g1 : kind == EV_W_NORM2 ? &m->layers[layer].g2 : &m->gf;
             if (!*dst) { EV_TRY(dev_alloc(m, dst, (size_t)H)); drop_graphs(m); }   // a graph captured before held a null gain pointer
             CUDA_TRY(cudaMemcpyAsync(*dst, dev_bf16, (size_t)H * 2, cudaMemcpyDeviceToDevice, st));
+            return EV_OK;
+        }
+        case EV_W_DRAFT_FC: {
+            if (!shape_is(H, 2 * H)) return bad_shape();
+            if (!m->fc.codes) {
+                EV_TRY(alloc_qmat(m, &m->fc, H, 2 * H));
+                EV_TRY(alloc_actbuf(m, &m->fq, 2 * H));
+                EV_TRY(dev_alloc(m, &m->d_topk, (size_t)m->M_cap * TOPK_MAX));
+                EV_TRY(dev_alloc(m, &m->d_fhat, (size_t)m->M_cap * H));
+                EV_TRY(dev_alloc(m, &m->d_feats, (size_t)m->M_cap * H));
+                EV_TRY(dev_alloc(m, &m->d_scratch, (size_t)2 * m->M_cap + 4 * c.max_batch));
+                EV_TRY(dev_alloc(m, &m->d_topo, (size_t)2 * EV_MAX_TREE_NODES));
+                EV_TRY(dev_alloc(m, &m->d_lvl_n, (size_t)(EV_MAX_TREE_NODES + 1) * c.max_batch));
+                EV_TRY(dev_alloc(m, &m->d_tree_par, (size_t)m->M_cap));
+                EV_TRY(dev_alloc(m, &m->d_chain_par, (size_t)m->M_cap));
+                drop_graphs(m);
+            }
+            EV_TRY(quant(m->fc, 0));
+            m->have_fc = true;
             return EV_OK;
         }
         default: return fail(EV_EINVAL, "unknown weight kind");
@@ -1248,6 +1298,13 @@ int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* o
         return fail(EV_EINVAL, "null required output array");
     const bool need_lm = !in->force_accept_all || m->recording;
     EV_TRY(check_ready(m, need_lm));
+    if (in->dev_features && !m->have_fc) return fail(EV_ESTATE, "dev_features given but EV_W_DRAFT_FC is not set (not a draft model)");
+    if (out->dev_topk) {
+        if (out->topk < 1 || out->topk > TOPK_MAX) return fail(EV_EINVAL, "topk must be 1..8");
+        if (!out->dev_logits && !m->logits_ws) {   // setup-time allocation (first use), not on the steady path
+            EV_TRY(dev_alloc(m, &m->logits_ws, (size_t)m->M_cap * m->cfg.vocab));
+        }
+    }
     cudaStream_t st = (cudaStream_t)stream;
     const AttnPlan plan = plan_attention(m, c, in);
     // Fast path: the whole step (~330 launches, PDL edges included) is captured once per distinct argument set
@@ -1263,9 +1320,9 @@ int ev_verify(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out* o
     memset(&key, 0, sizeof(key));
     key.B = in->n_seqs; key.T = in->n_nodes_max; key.commit = in->commit; key.force_all = in->force_accept_all;
     key.n_splits = plan.n_splits; key.split_len = plan.split_len; key.need_lm = need_lm;
-    const void* ptrs[12] = {c, in->dev_seq_slots, in->dev_tokens, in->dev_parents, in->dev_n_nodes, out->dev_accept_len,
+    const void* ptrs[16] = {c, in->dev_seq_slots, in->dev_tokens, in->dev_parents, in->dev_n_nodes, out->dev_accept_len,
                             out->dev_accept_nodes, out->dev_out_tokens, out->dev_new_ctx_len, out->dev_status, out->dev_argmax,
-                            out->dev_logits};
+                            out->dev_logits, in->dev_features, out->dev_final_hidden, out->dev_topk, (const void*)(size_t)out->topk};
     memcpy(key.p, ptrs, sizeof(ptrs));
     GraphEntry* hit = nullptr;
     for (auto& g : m->graphs)
@@ -1422,6 +1479,126 @@ int ev_model_calibrate(ev_model* m, const float* dev_hidden, int n_tok, float* d
     ev_cache_destroy(c);
     g_err = keep;
     return rc;
+}
+
+// ---- draft side ----------------------------------------------------------------------------------------
+int ev_model_share_head(ev_model* d, ev_model* t) {
+    if (!d || !t || d == t) return fail(EV_EINVAL, "bad argument");
+    if (d->cfg.hidden != t->cfg.hidden || d->cfg.vocab != t->cfg.vocab) return fail(EV_EINVAL, "drafter and target differ in hidden / vocab");
+    if (!t->have_embed || !t->have_lm) return fail(EV_ESTATE, "target embedding / LM head not set");
+    d->embed = t->embed; d->lm = t->lm; d->gf = t->gf;     // borrowed: the drafter's own (unused) buffers stay in its alloc list
+    d->have_embed = d->have_lm = d->shared_head = true;
+    drop_graphs(d);
+    return EV_OK;
+}
+
+static int draft_pass(ev_model* m, ev_cache* c, int B, int T, const int32_t* slots, const int32_t* tokens, const int32_t* parents,
+                      const int32_t* n_nodes, const float* feats, bool commit_all, int topk, cudaStream_t st) {
+    ev_verify_in in;
+    memset(&in, 0, sizeof(in));
+    in.n_seqs = B; in.n_nodes_max = T; in.dev_seq_slots = slots; in.dev_tokens = tokens; in.dev_parents = parents;
+    in.dev_n_nodes = n_nodes; in.commit = commit_all ? 1 : 0; in.force_accept_all = commit_all ? 1 : 0; in.dev_features = feats;
+    ev_verify_out o;
+    memset(&o, 0, sizeof(o));
+    o.tap_layer = -1;
+    const int Bm = m->cfg.max_batch;
+    o.dev_accept_len = m->d_scratch; o.dev_new_ctx_len = m->d_scratch + Bm; o.dev_status = m->d_scratch + 2 * Bm;
+    o.dev_accept_nodes = m->d_scratch + 4 * Bm; o.dev_out_tokens = o.dev_accept_nodes + m->M_cap;
+    if (!commit_all) { o.dev_final_hidden = m->d_fhat; o.dev_topk = m->d_topk; o.topk = topk; }
+    return ev_verify(m, c, &in, &o, (void*)st);
+}
+
+int ev_draft_tree(ev_model* m, ev_cache* c, const ev_draft_args* a, void* stream) {
+    if (!m || !c || !a || !a->dev_seq_slots || !a->host_parents || !a->dev_root_tokens || !a->dev_root_feats || !a->dev_tokens || !a->dev_parents)
+        return fail(EV_EINVAL, "null argument");
+    if (!m->have_fc) return fail(EV_ESTATE, "not a draft model (EV_W_DRAFT_FC not set)");
+    const int B = a->n_seqs, T = a->n_nodes, H = m->cfg.hidden;
+    if (B < 1 || B > m->cfg.max_batch || T < 1 || T > m->cfg.max_tree_nodes) return fail(EV_ECAPACITY, "batch or tree size exceeds the model's maxima");
+    cudaStream_t st = (cudaStream_t)stream;
+    // topology: depths must be non-decreasing in node order (levels are prefixes); child ranks; widest fan-out = top-k
+    std::vector<int> depth(T, 0), rank(T, 0), nchild(T, 0);
+    if (a->host_parents[0] != -1) return fail(EV_EINVAL, "parents[0] must be -1");
+    for (int i = 1; i < T; ++i) {
+        const int p = a->host_parents[i];
+        if (p < 0 || p >= i) return fail(EV_EINVAL, "parents[i] must be in [0, i)");
+        depth[i] = depth[p] + 1;
+        if (depth[i] < depth[i - 1]) return fail(EV_EINVAL, "nodes must be ordered by depth");
+        rank[i] = nchild[p]++;
+    }
+    int K = 1;
+    for (int i = 0; i < T; ++i) K = std::max(K, nchild[i]);
+    if (K > TOPK_MAX) return fail(EV_EINVAL, "a node has more than 8 children");
+    const int D = depth[T - 1];
+    std::vector<int32_t> topo(2 * T);
+    for (int i = 0; i < T; ++i) { topo[i] = a->host_parents[i]; topo[T + i] = rank[i]; }
+    if (m->h_topo != topo) {   // new topology: upload it (setup; the steady loop reuses it)
+        CUDA_TRY(cudaStreamSynchronize(st));
+        m->h_topo = topo;
+        CUDA_TRY(cudaMemcpy(m->d_topo, topo.data(), topo.size() * 4, cudaMemcpyHostToDevice));
+        std::vector<int32_t> lv((size_t)(D + 1) * m->cfg.max_batch), par((size_t)m->cfg.max_batch * T);
+        for (int d = 0; d <= D; ++d) {
+            int n = 0;
+            while (n < T && depth[n] <= d) ++n;
+            for (int b = 0; b < m->cfg.max_batch; ++b) lv[(size_t)d * m->cfg.max_batch + b] = n;
+        }
+        for (int b = 0; b < m->cfg.max_batch; ++b) memcpy(&par[(size_t)b * T], a->host_parents, (size_t)T * 4);
+        CUDA_TRY(cudaMemcpy(m->d_lvl_n, lv.data(), lv.size() * 4, cudaMemcpyHostToDevice));
+        CUDA_TRY(cudaMemcpy(m->d_tree_par, par.data(), par.size() * 4, cudaMemcpyHostToDevice));
+    }
+    // the per-sequence parents arrays ev_verify consumes, root tokens and root features into the tree's row 0 (all on the stream)
+    CUDA_TRY(cudaMemcpyAsync(a->dev_parents, m->d_tree_par, (size_t)B * T * 4, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpy2DAsync(a->dev_tokens, (size_t)T * 4, a->dev_root_tokens, 4, 4, B, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpy2DAsync(m->d_feats, (size_t)T * H * 4, a->dev_root_feats, (size_t)H * 4, (size_t)H * 4, B, cudaMemcpyDeviceToDevice, st));
+    for (int d = 0; d <= D; ++d) {
+        int n0 = 0;
+        while (n0 < T && depth[n0] <= d) ++n0;
+        if (d == D && n0 != T) return fail(EV_EINVAL, "topology depth mismatch");
+        EV_TRY(draft_pass(m, c, B, T, a->dev_seq_slots, a->dev_tokens, a->dev_parents, m->d_lvl_n + (size_t)d * m->cfg.max_batch, m->d_feats,
+                          false, K, st));
+        if (d == D) break;
+        int n1 = n0;
+        while (n1 < T && depth[n1] == d + 1) ++n1;
+        ExpandArgs ea;
+        ea.T = T; ea.H = H; ea.K = K; ea.n0 = n0; ea.parents = m->d_topo; ea.rank = m->d_topo + T; ea.topk = m->d_topk; ea.f_hat = m->d_fhat;
+        ea.tokens = a->dev_tokens; ea.feats = m->d_feats;
+        EV_TRY(launch_k(draft_expand_kernel, dim3(n1 - n0, B), dim3(256), 0, st, ea));
+    }
+    return EV_OK;
+}
+
+int ev_draft_extend(ev_model* m, ev_cache* c, int n_seqs, int n_nodes, const int32_t* dev_seq_slots, const int32_t* dev_tokens,
+                    const float* dev_feats, const int32_t* dev_n, void* stream) {
+    if (!m || !c || !dev_seq_slots || !dev_tokens || !dev_feats || !dev_n) return fail(EV_EINVAL, "null argument");
+    if (!m->have_fc) return fail(EV_ESTATE, "not a draft model (EV_W_DRAFT_FC not set)");
+    if (n_seqs < 1 || n_seqs > m->cfg.max_batch || n_nodes < 1 || n_nodes > m->cfg.max_tree_nodes) return fail(EV_ECAPACITY, "batch or chain too large");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (m->chain_T != n_nodes) {   // chain parents (row i: i - 1) at this row stride: uploaded once per stride (setup)
+        std::vector<int32_t> par((size_t)m->cfg.max_batch * n_nodes);
+        for (int b = 0; b < m->cfg.max_batch; ++b)
+            for (int i = 0; i < n_nodes; ++i) par[(size_t)b * n_nodes + i] = i - 1;
+        CUDA_TRY(cudaStreamSynchronize(st));
+        CUDA_TRY(cudaMemcpy(m->d_chain_par, par.data(), par.size() * 4, cudaMemcpyHostToDevice));
+        m->chain_T = n_nodes;
+    }
+    return draft_pass(m, c, n_seqs, n_nodes, dev_seq_slots, dev_tokens, m->d_chain_par, dev_n, dev_feats, true, 0, st);
+}
+
+int ev_gather_accepted(int n_seqs, int n_nodes, int hidden, const int32_t* dev_tokens, const int32_t* dev_accept_len,
+                       const int32_t* dev_accept_nodes, const int32_t* dev_out_tokens, const float* dev_feat, float* dev_carry,
+                       int32_t* dev_ext_tokens, float* dev_ext_feats, int32_t* dev_ext_n, int32_t* dev_next_root, void* stream) {
+    if (n_seqs < 1 || n_nodes < 1 || hidden < 1 || !dev_tokens || !dev_accept_len || !dev_accept_nodes || !dev_out_tokens || !dev_feat ||
+        !dev_carry || !dev_ext_tokens || !dev_ext_feats || !dev_ext_n || !dev_next_root)
+        return fail(EV_EINVAL, "bad argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    GatherArgs g;
+    g.T = n_nodes; g.H = hidden; g.tokens = dev_tokens; g.accept_len = dev_accept_len; g.accept_nodes = dev_accept_nodes;
+    g.out_tokens = dev_out_tokens; g.feat = dev_feat; g.carry = dev_carry; g.ext_tokens = dev_ext_tokens; g.ext_feats = dev_ext_feats;
+    g.ext_n = dev_ext_n; g.next_root = dev_next_root;
+    gather_accepted_kernel<<<dim3(n_nodes, n_seqs), 256, 0, st>>>(g);
+    LAUNCH_CHECK();
+    carry_update_kernel<<<n_seqs, 256, 0, st>>>(g);
+    LAUNCH_CHECK();
+    return EV_OK;
 }
 
 // ---- single operators --------------------------------------------------------------------------------

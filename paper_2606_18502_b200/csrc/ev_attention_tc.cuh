@@ -411,16 +411,24 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 mbar_wait(&tempty[ts], ((j / depth) & 1) ^ 1);     // the MMAs that read this slot's previous tile have finished
                 const uint8_t* src = raw + rs * C::RAW_BYTES;
                 uint8_t* dst = ring + ts * C::K_BYTES;
-#pragma unroll 4
-                for (int c = lane; c < TCA_BN * CPR; c += 32) {
-                    const int r = c / CPR, j8 = c % CPR;           // key row, chunk of 16 dims
-                    const uint4 in = *reinterpret_cast<const uint4*>(src + r * D + j8 * 16);
-                    uint4 lo, hi;
-                    e4m3x16_to_f16(in, lo, hi);
-                    const int h = j8 >> 2, jj = (j8 & 3) * 2;      // d half (64 dims), first of the two 16-byte chunks inside the 128-byte row
-                    uint8_t* rowp = dst + (r >> 3) * C::SBO + h * 1024 + (r & 7) * 128;
-                    *reinterpret_cast<uint4*>(rowp + ((jj ^ (r & 7)) << 4)) = lo;
-                    *reinterpret_cast<uint4*>(rowp + (((jj + 1) ^ (r & 7)) << 4)) = hi;
+                for (int c0 = 0; c0 < TCA_BN * CPR; c0 += 8 * 32) {   // 8 chunks per lane in flight: loads first, then convert + store
+                    uint4 in[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int c = c0 + u * 32 + lane;
+                        in[u] = *reinterpret_cast<const uint4*>(src + (c / CPR) * D + (c % CPR) * 16);
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const int c = c0 + u * 32 + lane;
+                        const int r = c / CPR, j8 = c % CPR;           // key row, chunk of 16 dims
+                        uint4 lo, hi;
+                        e4m3x16_to_f16(in[u], lo, hi);
+                        const int h = j8 >> 2, jj = (j8 & 3) * 2;      // d half (64 dims), first of the two 16-byte chunks inside the 128-byte row
+                        uint8_t* rowp = dst + (r >> 3) * C::SBO + h * 1024 + (r & 7) * 128;
+                        *reinterpret_cast<uint4*>(rowp + ((jj ^ (r & 7)) << 4)) = lo;
+                        *reinterpret_cast<uint4*>(rowp + (((jj + 1) ^ (r & 7)) << 4)) = hi;
+                    }
                 }
                 fence_proxy_async();      // generic-proxy stores -> visible to the tensor core's async-proxy reads
                 __syncwarp();
