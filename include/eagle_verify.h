@@ -277,6 +277,31 @@ int ev_gather_accepted(int n_seqs, int n_nodes, int hidden, const int32_t* dev_t
                        const int32_t* dev_accept_nodes, const int32_t* dev_out_tokens, const float* dev_feat, float* dev_carry,
                        int32_t* dev_ext_tokens, float* dev_ext_feats, int32_t* dev_ext_n, int32_t* dev_next_root, void* stream);
 
+/* ---- serving shell: continuous batching around verify ("continuous batching") -------------
+ * An engine owns a set of requests.  Every ev_engine_step is one iteration of iteration-level scheduling: waiting requests are
+ * admitted while batch rows and KV pages are free (their prompt is prefilled into the target cache and, with a drafter,
+ * into the drafter's cache with the target's features), then ONE speculative step runs for all active requests together
+ * (draft tree -> verify -> accept -> KV compaction -> drafter extend), emitted tokens are appended to each request's output
+ * and finished requests leave, freeing their pages - the next step's batch has a different composition.  Because every
+ * kernel of the path is batch-invariant, a request's tokens do not depend on which other requests share its steps.
+ * Without a drafter (drafter == NULL) the step is plain decoding (one node per sequence). */
+typedef struct ev_engine ev_engine;
+typedef struct {
+    int max_batch;                /* rows per step, <= both models' max_batch */
+    int n_nodes;                  /* T of the static draft topology (ignored without a drafter) */
+    const int32_t* host_parents;  /* [T] topology, nodes ordered by depth (copied) */
+} ev_engine_config;
+int ev_engine_create(ev_model* target, ev_cache* tcache, ev_model* drafter, ev_cache* dcache, const ev_engine_config*, ev_engine** out);
+/* Queues a request: host_prompt[n_prompt] (n_prompt >= 2, copied), generate max_new_tokens tokens.  Returns its id. */
+int ev_engine_submit(ev_engine*, const int32_t* host_prompt, int n_prompt, int max_new_tokens, int* request_id);
+/* One scheduling iteration on the stream; synchronises it (results come back to the host every step).  Outputs: requests active
+ * during the step, requests that finished in it, requests still waiting for rows or pages. */
+int ev_engine_step(ev_engine*, int* n_active, int* n_finished, int* n_waiting, void* stream);
+/* Copies up to cap generated tokens of a request to host_tokens_out; *n_out = tokens generated so far (capped at
+ * max_new_tokens), *finished = 1 once it has left the batch. */
+int ev_engine_poll(ev_engine*, int request_id, int32_t* host_tokens_out, int cap, int* n_out, int* finished);
+int ev_engine_destroy(ev_engine*);
+
 /* ---- single operators (per-kernel parity tests; same kernels the step uses) ------------------ */
 
 /* y[M][N] = (codes_x . W_kind^T) * s_x[m] * s_w[n] with the product GEMM kernel. */

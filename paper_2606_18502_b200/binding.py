@@ -46,6 +46,10 @@ class ev_verify_out(C.Structure):
                 ("dev_tap_st", C.c_void_p), ("dev_final_hidden", C.c_void_p), ("dev_topk", C.c_void_p), ("topk", C.c_int)]
 
 
+class ev_engine_config(C.Structure):
+    _fields_ = [("max_batch", C.c_int), ("n_nodes", C.c_int), ("host_parents", C.c_void_p)]
+
+
 class ev_draft_args(C.Structure):
     _fields_ = [("n_seqs", C.c_int), ("n_nodes", C.c_int), ("dev_seq_slots", C.c_void_p), ("host_parents", C.c_void_p),
                 ("dev_root_tokens", C.c_void_p), ("dev_root_feats", C.c_void_p), ("dev_tokens", C.c_void_p),
@@ -87,6 +91,11 @@ SIGNATURES = {
     "ev_draft_tree": (C.c_int, [_P, _P, C.POINTER(ev_draft_args), _P]),
     "ev_draft_extend": (C.c_int, [_P, _P, C.c_int, C.c_int, _P, _P, _P, _P, _P]),
     "ev_gather_accepted": (C.c_int, [C.c_int, C.c_int, C.c_int, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P, _P]),
+    "ev_engine_create": (C.c_int, [_P, _P, _P, _P, C.POINTER(ev_engine_config), C.POINTER(_P)]),
+    "ev_engine_submit": (C.c_int, [_P, _P, C.c_int, C.c_int, C.POINTER(C.c_int)]),
+    "ev_engine_step": (C.c_int, [_P, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_int), _P]),
+    "ev_engine_poll": (C.c_int, [_P, C.c_int, _P, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
+    "ev_engine_destroy": (C.c_int, [_P]),
     "ev_launch_count": (C.c_long, [C.c_int]),
     "ev_capture_count": (C.c_long, [C.c_int]),
     "ev_version": (C.c_int, []),
@@ -439,3 +448,47 @@ def ev_gather_accepted(tokens, accept_len, accept_nodes, out_tokens, feat, carry
     _check(load_library().ev_gather_accepted(B, T, H, tokens.data_ptr(), accept_len.data_ptr(), accept_nodes.data_ptr(), out_tokens.data_ptr(),
                                              feat.data_ptr(), carry.data_ptr(), ext_tokens.data_ptr(), ext_feats.data_ptr(), ext_n.data_ptr(),
                                              next_root.data_ptr(), _stream()))
+
+
+class Engine:
+    """ev_engine handle: continuous batching around verify (include/eagle_verify.h "serving shell")."""
+
+    def __init__(self, target, tcache, drafter=None, dcache=None, max_batch=1, parents=None):
+        import numpy as np
+        self.lib = load_library()
+        self._keep = (target, tcache, drafter, dcache)
+        par = np.ascontiguousarray(parents if parents is not None else [-1], dtype=np.int32)
+        cfg = ev_engine_config(max_batch, len(par), par.ctypes.data_as(C.c_void_p))
+        h = C.c_void_p()
+        _check(self.lib.ev_engine_create(target.h, tcache.h, drafter.h if drafter else None, dcache.h if dcache else None, C.byref(cfg), C.byref(h)))
+        self.h = h
+
+    def ev_engine_submit(self, prompt, max_new_tokens):
+        import numpy as np
+        p = np.ascontiguousarray(prompt, dtype=np.int32)
+        rid = C.c_int(-1)
+        _check(self.lib.ev_engine_submit(self.h, p.ctypes.data_as(C.c_void_p), len(p), max_new_tokens, C.byref(rid)))
+        return rid.value
+
+    def ev_engine_step(self):
+        a, f, w = C.c_int(0), C.c_int(0), C.c_int(0)
+        _check(self.lib.ev_engine_step(self.h, C.byref(a), C.byref(f), C.byref(w), _stream()))
+        return a.value, f.value, w.value
+
+    def ev_engine_poll(self, rid, cap=4096):
+        import numpy as np
+        out = np.zeros(cap, dtype=np.int32)
+        n, fin = C.c_int(0), C.c_int(0)
+        _check(self.lib.ev_engine_poll(self.h, rid, out.ctypes.data_as(C.c_void_p), cap, C.byref(n), C.byref(fin)))
+        return out[:min(n.value, cap)].copy(), bool(fin.value)
+
+    def ev_engine_destroy(self):
+        if self.h:
+            self.lib.ev_engine_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.ev_engine_destroy()
+        except Exception:
+            pass

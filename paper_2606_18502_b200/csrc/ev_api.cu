@@ -759,6 +759,10 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                           (l + 1 < cfg.n_layers) ? m->layers[l + 1].g1 : m->gf, H * 2));
         if (out->dev_hidden) { EV_TRY(materialize()); EV_TRY(copy_f32(st, m->h, out->dev_hidden + (size_t)(l + 1) * M * H, (long)M * H)); }
     }
+    if (out->dev_final_hidden) {   // the "feature" an EAGLE drafter consumes: the residual stream after the last layer
+        EV_TRY(materialize());
+        EV_TRY(copy_f32(st, m->h, out->dev_final_hidden, (long)M * H));
+    }
     if (need_lm) {
         if (lockstep) { pend = none; EV_TRY(copy_f32(st, ovr + (size_t)cfg.n_layers * M * H, m->h, (long)M * H)); }
         {
@@ -766,7 +770,6 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
             ROW_DISPATCH_S(rp_h, pend.p ? pend.splits : 1, rmsnorm_quant_kernel, dim3(M * rp_h.cl), dim3(NORM_THREADS), 0, st, m->h, H, pend, m->gf, cfg.rms_eps, quant_out(m, m->xq, 4 * cfg.n_layers), pfp.take(false));
             pend = none;
         }
-        if (out->dev_final_hidden) EV_TRY(copy_f32(st, m->h, out->dev_final_hidden, (long)M * H));   // the final norm kernel wrote the residual back
         float* lg = out->dev_logits ? out->dev_logits : (out->dev_topk ? m->logits_ws : nullptr);
         EV_TRY(run_linear(m, st, m->lm, m->xq, M, EPI_ARGMAX, nullptr, lg, m->argmax_keys, PC_GEMM_LM, &pfp));
         if (out->dev_topk) {
@@ -1727,3 +1730,5 @@ int ev_profile_trace(ev_model* m, unsigned long long* host_out, int max_entries,
 }
 
 }  // extern "C"
+
+#include "ev_engine.inc"
