@@ -735,7 +735,13 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         ma.pf = pfp.take(false);
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
-            ROW_DISPATCH(rp_q, attn_merge_quant_kernel, dim3(M * rp_q.cl), dim3(MERGE_THREADS), 0, st, ma);
+            const int Gq = cfg.n_q_heads / cfg.n_kv_heads;
+            if (rp_q.cl == 1 && D == 128 && cfg.n_kv_heads <= 8 && (Gq == 4 || Gq == 1)) {   // many rows: one warp per kv head
+                if (Gq == 4) EV_TRY(launch_k(attn_merge_rowkv_kernel<4>, dim3(M), dim3(32 * cfg.n_kv_heads), 0, st, ma));
+                else EV_TRY(launch_k(attn_merge_rowkv_kernel<1>, dim3(M), dim3(32 * cfg.n_kv_heads), 0, st, ma));
+            } else {
+                ROW_DISPATCH(rp_q, attn_merge_quant_kernel, dim3(M * rp_q.cl), dim3(MERGE_THREADS), 0, st, ma);
+            }
         }
         if (tap && out->dev_tap_aq) CUDA_TRY(cudaMemcpyAsync(out->dev_tap_aq, m->aq.codes, (size_t)M * m->q_dim, cudaMemcpyDeviceToDevice, st));
         if (tap && out->dev_tap_sa) EV_TRY(copy_f32(st, m->aq.scale, out->dev_tap_sa, M));
@@ -897,7 +903,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
     // default chunk length: short for models built for one or two sequences (every chunk is its own CTA: latency), long
     // for batched serving (fewer partial outputs per row); a function of the config only, hence fixed for the model's life
-    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : (cfg->max_batch <= 2 ? 256 : (cfg->max_ctx <= 10240 ? 1024 : 2048));
+    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : (cfg->max_batch <= 2 ? 256 : 2048);
     m->n_chunks_max = (cfg->max_ctx + m->attn_chunk - 1) / m->attn_chunk;
     A(dev_alloc(m, &m->o_part, (size_t)m->M_cap * m->n_chunks_max * m->q_dim));
     A(dev_alloc(m, &m->ml_part, (size_t)m->M_cap * m->n_chunks_max * cfg->n_q_heads * 2));

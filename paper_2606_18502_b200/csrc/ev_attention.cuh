@@ -11,7 +11,8 @@
 //   TAIL  = the last ATT_TAIL_R + 1 positions (youngest cached tokens, then the node's nearest ancestors in depth
 //           order, itself last), scored key by key in fp32 by the merge kernel;
 //   MERGE = out = (sum_j w_j O_j + sum_t e_t v_t) / (sum_j w_j l_j + sum_t e_t), chunks in index order, then the tail
-//           keys in position order, w_j = exp(m_j - M), e_t = exp(s_t - M), M = the overall maximum.
+//           keys in position order, w_j = exp(m_j - M), e_t = exp(s_t - M) (ex2.approx), M = the overall maximum; the division is a
+//           correctly rounded reciprocal and a multiply.
 // For trees no deeper than ATT_TAIL_R the bulk lies inside the committed context: which tree slots the ancestors sit
 // in, how many nodes and sequences share the launch and how many CTAs there are no longer enter the arithmetic.
 // Deeper trees (prefill chains) put the older ancestors into the bulk by slot (anc_bulk); chains stay invariant
@@ -470,7 +471,7 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
 #pragma unroll
             for (int u = 0; u < NB; ++u)
                 if (u < ns) {
-                    const float wt = (ml0[u].x == -INFINITY) ? 0.f : expf(ml0[u].x - mx);
+                    const float wt = (ml0[u].x == -INFINITY) ? 0.f : exp_fast(ml0[u].x - mx);
                     den = fmaf(wt, ml0[u].y, den);
                     num.x = fmaf(wt, t0[u].x, num.x); num.y = fmaf(wt, t0[u].y, num.y); num.z = fmaf(wt, t0[u].z, num.z); num.w = fmaf(wt, t0[u].w, num.w);
                 }
@@ -483,7 +484,7 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
                     if (s0 + u < ns) {
-                        const float wt = (ml[u].x == -INFINITY) ? 0.f : expf(ml[u].x - mx);
+                        const float wt = (ml[u].x == -INFINITY) ? 0.f : exp_fast(ml[u].x - mx);
                         den = fmaf(wt, ml[u].y, den);
                         num.x = fmaf(wt, t[u].x, num.x); num.y = fmaf(wt, t[u].y, num.y); num.z = fmaf(wt, t[u].z, num.z); num.w = fmaf(wt, t[u].w, num.w);
                     }
@@ -491,16 +492,180 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
 #pragma unroll
             for (int u = 0; u < ATT_TAIL_MAX; ++u)
                 if (u < nt) {
-                    const float et = expf(ts[u] - mx);
+                    const float et = exp_fast(ts[u] - mx);
                     const float4 v4 = a.pool8 ? kv_cvt4_e4m3(vr[u].x, a.v_scale) : kv_cvt4(vr[u], a.kv_f16);
                     den = __fadd_rn(den, et);
                     num.x = fmaf(et, v4.x, num.x); num.y = fmaf(et, v4.y, num.y); num.z = fmaf(et, v4.z, num.z); num.w = fmaf(et, v4.w, num.w);
                 }
-            v[k] = make_float4(div_rn(num.x, den), div_rn(num.y, den), div_rn(num.z, den), div_rn(num.w, den));
+            const float inv = __frcp_rn(den);   // one correctly rounded reciprocal, four rounded multiplies
+            v[k] = make_float4(mul_rn(num.x, inv), mul_rn(num.y, inv), mul_rn(num.z, inv), mul_rn(num.w, inv));
             if (a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + i) = v[k];
         }
     }
     quantize_regs<MERGE_NV4>(v, m, K, c0, c1, a.q, red, xch_f);
+    trace_exit(a.pf);
+}
+
+// ---- the same computation for many rows (D = 128, one CTA per row, no cluster): warp = one kv head, lane = 4 output dims.
+// The tail keys' K and V are loaded ONCE per kv head and shared by its G query heads (the generic kernel above loads them
+// per query head), every load of the warp's G heads is issued before the first use, and a thread ends up holding G float4s
+// of the row for the quantizer.  Same arithmetic, same order per (row, head): results are bit-identical to the generic
+// kernel (tests/test_gpu_verify_tiny.py runs D = 64 through the generic one, the 8B tests run both). ----
+template <int G>
+__global__ void __launch_bounds__(256, 2) attn_merge_rowkv_kernel(MergeArgs a) {
+    pdl_launch_dependents();
+    l2_prefetch_issue(a.pf);
+    pdl_wait();
+    trace_past_wait(a.pf);
+    constexpr int D = 128;
+    __shared__ float red[8];
+    __shared__ long long tbase[ATT_TAIL_MAX];
+    const int m = blockIdx.x;
+    const int b = m / a.T, node = m % a.T;
+    const int nn = a.nn_eff[b];
+    const int K = a.Hq * D, S = a.n_chunks;
+    const bool valid = node < nn;
+    const int L = a.Lsnap[b];
+    const int e = valid ? a.erow[m] : 0;
+    const int ns = valid ? (a.kend_row[m] + a.chunk - 1) / a.chunk : 0;
+    const int n_ctx = valid ? min(max(0, L - e), ATT_TAIL_MAX) : 0;
+    const unsigned long long anc_tail = valid ? (a.anc[m] & ~a.anc_bulk[m]) : 0ull;
+    const int nt = min(n_ctx + __popcll(anc_tail), ATT_TAIL_MAX);
+    const size_t kv_stride = (size_t)a.Hkv * a.page_size * D;
+    if ((int)threadIdx.x < nt) {
+        const int u = threadIdx.x;
+        int sl = e + u;
+        if (u >= n_ctx) {
+            unsigned long long at = anc_tail;
+            for (int i = n_ctx; i < u; ++i) at &= at - 1;
+            sl = L + __ffsll((long long)at) - 1;
+        }
+        const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+        tbase[u] = (long long)((size_t)pt[sl / a.page_size] * 2 * kv_stride + (size_t)(sl % a.page_size) * D);
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int kvh = warp;                 // blockDim = 32 * Hkv
+    const int d = lane * 4;
+    float4 v[G];
+    float amax = 0.f;
+    {
+        // every load of this warp, up front
+        uint2 kr[ATT_TAIL_MAX], vr[ATT_TAIL_MAX];
+        const size_t hoff = (size_t)kvh * a.page_size * D + d;
+#pragma unroll
+        for (int u = 0; u < ATT_TAIL_MAX; ++u) {
+            kr[u] = make_uint2(0u, 0u); vr[u] = make_uint2(0u, 0u);
+            if (valid && u < nt) {
+                if (a.pool8) {
+                    const uint8_t* kp = a.pool8 + tbase[u] + hoff;
+                    kr[u].x = *reinterpret_cast<const uint32_t*>(kp);
+                    vr[u].x = *reinterpret_cast<const uint32_t*>(kp + kv_stride);
+                } else {
+                    const __nv_bfloat16* kp = a.pool + tbase[u] + hoff;
+                    kr[u] = *reinterpret_cast<const uint2*>(kp);
+                    vr[u] = *reinterpret_cast<const uint2*>(kp + kv_stride);
+                }
+            }
+        }
+        constexpr int NB = 2;
+        float4 q4[G], t0[G][NB];
+        float2 ml0[G][NB];
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int h = kvh * G + g;
+            q4[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (valid) q4[g] = *reinterpret_cast<const float4*>(a.qkv + (size_t)m * a.q_ld + h * D + d);
+#pragma unroll
+            for (int u = 0; u < NB; ++u)
+                if (valid && u < ns) {
+                    t0[g][u] = __ldcg(reinterpret_cast<const float4*>(a.o_part + (((size_t)m * a.Hq + h) * S + u) * D + d));
+                    ml0[g][u] = __ldcg(reinterpret_cast<const float2*>(a.ml_part + (((size_t)m * a.Hq + h) * S + u) * 2));
+                }
+        }
+        float4 kf[ATT_TAIL_MAX];
+#pragma unroll
+        for (int u = 0; u < ATT_TAIL_MAX; ++u) kf[u] = a.pool8 ? kv_cvt4_e4m3(kr[u].x, a.k_scale) : kv_cvt4(kr[u], a.kv_f16);
+#pragma unroll
+        for (int g = 0; g < G; ++g) {
+            const int h = kvh * G + g;
+            const float* op = a.o_part + ((size_t)m * a.Hq + h) * S * D + d;
+            const float* mlp = a.ml_part + ((size_t)m * a.Hq + h) * S * 2;
+            float ts[ATT_TAIL_MAX];
+#pragma unroll
+            for (int u = 0; u < ATT_TAIL_MAX; ++u) {
+                float part = fmaf(q4[g].w, kf[u].w, fmaf(q4[g].z, kf[u].z, fmaf(q4[g].y, kf[u].y, __fmul_rn(q4[g].x, kf[u].x))));
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) part = __fadd_rn(part, __shfl_xor_sync(0xffffffffu, part, o));
+                ts[u] = mul_rn(part, a.scale);
+            }
+            v[g] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (valid) {
+                float mx = -INFINITY;
+#pragma unroll
+                for (int u = 0; u < NB; ++u)
+                    if (u < ns) mx = fmaxf(mx, ml0[g][u].x);
+                for (int j = NB; j < ns; ++j) mx = fmaxf(mx, __ldcg(mlp + 2 * j));
+#pragma unroll
+                for (int u = 0; u < ATT_TAIL_MAX; ++u)
+                    if (u < nt) mx = fmaxf(mx, ts[u]);
+                float den = 0.f;
+                float4 num = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int u = 0; u < NB; ++u)
+                    if (u < ns) {
+                        const float wt = (ml0[g][u].x == -INFINITY) ? 0.f : exp_fast(ml0[g][u].x - mx);
+                        den = fmaf(wt, ml0[g][u].y, den);
+                        num.x = fmaf(wt, t0[g][u].x, num.x); num.y = fmaf(wt, t0[g][u].y, num.y); num.z = fmaf(wt, t0[g][u].z, num.z); num.w = fmaf(wt, t0[g][u].w, num.w);
+                    }
+                for (int s0 = NB; s0 < ns; s0 += 4) {
+                    float4 t[4];
+                    float2 ml[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (s0 + u < ns) { t[u] = __ldcg(reinterpret_cast<const float4*>(op + (size_t)(s0 + u) * D)); ml[u] = __ldcg(reinterpret_cast<const float2*>(mlp + 2 * (s0 + u))); }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        if (s0 + u < ns) {
+                            const float wt = (ml[u].x == -INFINITY) ? 0.f : exp_fast(ml[u].x - mx);
+                            den = fmaf(wt, ml[u].y, den);
+                            num.x = fmaf(wt, t[u].x, num.x); num.y = fmaf(wt, t[u].y, num.y); num.z = fmaf(wt, t[u].z, num.z); num.w = fmaf(wt, t[u].w, num.w);
+                        }
+                }
+#pragma unroll
+                for (int u = 0; u < ATT_TAIL_MAX; ++u)
+                    if (u < nt) {
+                        const float et = exp_fast(ts[u] - mx);
+                        const float4 v4 = a.pool8 ? kv_cvt4_e4m3(vr[u].x, a.v_scale) : kv_cvt4(vr[u], a.kv_f16);
+                        den = __fadd_rn(den, et);
+                        num.x = fmaf(et, v4.x, num.x); num.y = fmaf(et, v4.y, num.y); num.z = fmaf(et, v4.z, num.z); num.w = fmaf(et, v4.w, num.w);
+                    }
+                const float inv = __frcp_rn(den);
+                v[g] = make_float4(mul_rn(num.x, inv), mul_rn(num.y, inv), mul_rn(num.z, inv), mul_rn(num.w, inv));
+                if (a.attn) *reinterpret_cast<float4*>(a.attn + (size_t)m * K + h * D + d) = v[g];
+            }
+            amax = fmaxf(amax, fmaxf(fmaxf(fabsf(v[g].x), fabsf(v[g].y)), fmaxf(fabsf(v[g].z), fabsf(v[g].w))));
+        }
+    }
+    // per-token quantization of the row (the tail of quantize_regs for this thread layout)
+    amax = block_max(amax, red);
+    const QuantOut& q = a.q;
+    float s;
+    if (q.static_scale) s = *q.static_scale;
+    else s = (amax == 0.f) ? 1.0f : div_rn(amax, 448.0f);
+    if (threadIdx.x == 0) {
+        q.sx[m] = s;
+        if (q.site_amax) atomicMax(reinterpret_cast<int*>(q.site_amax), __float_as_int(amax));
+    }
+    uint32_t* dst = reinterpret_cast<uint32_t*>(q.codes + (size_t)m * K);
+    const float thr = mul_rn(448.0f, s);
+    unsigned clipped = 0;
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+        dst[(kvh * G + g) * (D / 4) + lane] = e4m3x4(div_rn(v[g].x, s), div_rn(v[g].y, s), div_rn(v[g].z, s), div_rn(v[g].w, s));
+        if (q.clip_count) clipped += clip4(v[g].x, v[g].y, v[g].z, v[g].w, thr);
+    }
+    clip_add(q, clipped);
     trace_exit(a.pf);
 }
 

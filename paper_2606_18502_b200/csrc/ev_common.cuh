@@ -26,6 +26,14 @@ __device__ __forceinline__ uint32_t e4m3x4(float a, float b, float c, float d) {
 
 __device__ __forceinline__ float bf16_bits_to_float(uint16_t b) { return __uint_as_float(((uint32_t)b) << 16); }
 
+// e^x for the softmax weights of the attention merge: one FMUL + one MUFU.EX2 (2 ulp), the approximation the tensor-core
+// attention kernel uses for its own probabilities; deterministic (the same bits for the same input on every launch)
+__device__ __forceinline__ float exp_fast(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x * 1.4426950408889634f));
+    return y;
+}
+
 // ---- warp / block reductions ------------------------------------------------------------------
 __device__ __forceinline__ float warp_max(float v) {
 #pragma unroll
