@@ -444,6 +444,62 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
     return line
 
 
+def engine_leg(spec, args, torch, ev, log):
+    """Serving shell with the draft side (8(f)-3): B requests with the config's prompts run
+    through ev_engine - continuous batching around verify - as plain decoding (one node per sequence), with the EAGLE-style
+    drafter proposing a chain of k = 3, and with it proposing the config's tree (the chain-vs-tree trade-off is
+    drafting + verification overhead against accepted length; the drafter here has random weights, so its acceptance is ~0 and
+    the figures are the overhead side of that trade-off)."""
+    shape = spec.model
+    B = min(spec.batch, args.engine_batch)
+    ctx = wl.context_lengths(spec)[:B]
+    new_tokens = args.engine_steps * 8
+    max_ctx = int(ctx.max()) + new_tokens + 80
+    target = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=max_ctx, page_size=spec.page_size)
+    for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
+        target.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
+    import dataclasses
+    dshape = dataclasses.replace(shape, name=shape.name + "_drafter", n_layers=1)
+    drafter = ev.Model(dshape, max_batch=B, max_tree_nodes=64, max_ctx=max_ctx, page_size=spec.page_size)
+    for k in LAYER_KINDS:
+        drafter.ev_model_set_weight(k, 0, wl.weight_matrix_bf16(shape, spec.seed, k, shape.n_layers, device="cuda"))
+    drafter.ev_model_set_weight("d_fc", 0, wl.weight_matrix_bf16(shape, spec.seed, "d_fc", 0, device="cuda"))
+    ev.ev_model_share_head(drafter, target)
+    pages = sum((int(L) + new_tokens + 80) // spec.page_size + 2 for L in ctx)
+    out = {"batch": B, "context": [int(ctx.min()), int(ctx.max())], "steps": args.engine_steps,
+           "def": "ev_engine_step wall time after all requests are admitted (host sync per step); drafter = 1 decoder layer + FC of the "
+                  "target's shape, random weights (acceptance ~ 0: overhead side of the chain-vs-tree trade-off, PAPER.md:361-363)"}
+    prompts = [wl.context_ids(spec, b, int(ctx[b])) for b in range(B)]
+    for mode, parents in (("plain_decode", None), ("draft_chain_k3", wl.chain_parents(4)), ("draft_tree", tree_of(spec))):
+        tcache = ev.Cache(target, pages, B)
+        dcache = ev.Cache(drafter, pages, B) if parents is not None else None
+        eng = ev.Engine(target, tcache, drafter if parents is not None else None, dcache, max_batch=B, parents=parents)
+        rids = [eng.ev_engine_submit(p, new_tokens) for p in prompts]
+        t0 = time.time()
+        eng.ev_engine_step()                      # admits (prefills) every request and runs the first step
+        torch.cuda.synchronize()
+        t_admit = time.time() - t0
+        for _ in range(3):
+            eng.ev_engine_step()
+        torch.cuda.synchronize()
+        n0 = sum(len(eng.ev_engine_poll(r)[0]) for r in rids)
+        t0 = time.perf_counter()
+        for _ in range(args.engine_steps):
+            eng.ev_engine_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        n1 = sum(len(eng.ev_engine_poll(r)[0]) for r in rids)
+        T = 1 if parents is None else len(parents)
+        out[mode] = {"tree_nodes": T, "ms_per_step": round(1e3 * dt / args.engine_steps, 3),
+                     "emitted_tokens_per_s": round((n1 - n0) / dt, 1), "mean_emitted_per_step": round((n1 - n0) / (B * args.engine_steps), 3),
+                     "admission_s": round(t_admit, 2)}
+        log(f"engine {mode}: {out[mode]}")
+        eng.ev_engine_destroy()
+        del eng, tcache, dcache
+        torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -454,10 +510,18 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--loop", type=int, default=0, help="also run a sustained closed loop of this many committed steps")
     ap.add_argument("--kv", default="bf16", choices=["bf16", "fp8"], help="KV cache: bf16 (the configs' format) or fp8 = E4M3 (PAPER.md:98, SURVEY 8(f)-2)")
+    ap.add_argument("--layers", type=int, default=0, help="override the number of decoder layers (40 = the paper's ~10B block-expanded "
+                                                           "student shape, PAPER.md:76/102; SURVEY 8(f)-4)")
+    ap.add_argument("--engine", action="store_true", help="also run the serving shell + draft side leg (ev_engine: plain decode, chain, tree)")
+    ap.add_argument("--engine-steps", type=int, default=16)
+    ap.add_argument("--engine-batch", type=int, default=32)
     ap.add_argument("--also", default="auto", help="configs whose short line is added under 'also' (default: 2 = batch 32 "
                                                    "when the headline config 1 runs on one GPU; 'none' to skip)")
     args = ap.parse_args()
     spec = wl.CONFIGS[args.config]
+    if args.layers:
+        import dataclasses
+        spec = dataclasses.replace(spec, name=f"{spec.name}_{args.layers}layers", model=dataclasses.replace(spec.model, name=f"{spec.model.name}_{args.layers}l", n_layers=args.layers))
     if args.impl != "reference" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # N independent replicas, one process per GPU: start them the way the driver would
         import socket
@@ -513,6 +577,8 @@ def main():
                                                                    "planted_emitted_per_step", "emitted_tokens_per_s", "step_roofline", "roofline", "e2e", "clocks", "attention")}
         if line is not None:
             line["also"] = extra
+    if args.engine and rank == 0 and line is not None:
+        line["engine"] = engine_leg(spec, args, torch, ev, log)
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:
