@@ -595,7 +595,11 @@ AttnPlan plan_attention(ev_model* m, ev_cache* c, const ev_verify_in* in) {
             if (c->seq_used[i]) c->len_bound[i] = std::min(c->len_bound[i] + T, (int)c->seq_pages[i].size() * m->cfg.page_size);
     AttnPlan p;
     p.split_len = m->attn_chunk;
-    p.n_splits = std::min(m->n_chunks_max, std::max(1, (max_keys + p.split_len - 1) / p.split_len));
+    int need = std::max(1, (max_keys + p.split_len - 1) / p.split_len);
+    // short chunks (models built for one or two sequences): a growing sequence crosses a chunk boundary every few dozen steps and
+    // every new column count is a new CUDA graph - round the column count up to a power of two (the CTAs of empty columns leave at once)
+    if (p.split_len <= 512) need = pow2_ceil(need);
+    p.n_splits = std::min(m->n_chunks_max, need);
     return p;
 }
 
