@@ -22,9 +22,15 @@
  *     has passed the call.  The library owns handles, quantized weights, the page pool and its
  *     workspaces; they are released by the matching *_destroy.
  *   - Asynchrony: calls taking a stream only enqueue work; outputs are valid after the caller
- *     synchronises that stream.  ev_verify performs no host synchronisation and no allocation.
- *     Data-dependent failures (bad parent index, token id out of range, sequence over capacity)
- *     are reported per sequence in ev_verify_out.dev_status, not by return code.
+ *     synchronises that stream.  ev_verify in steady state performs no host synchronisation and no allocation:
+ *     it replays a CUDA graph.  The FIRST call with a new (batch, tree size, buffer set, attention chunk-column count)
+ *     captures and instantiates that graph (host work of a few ms; ev_capture_count counts them) and, when top-k is asked
+ *     for without a logits buffer, allocates a logits workspace once.  Data-dependent failures (bad parent index, token id out
+ *     of range, sequence over capacity or beyond the attention grid, two rows of one batch on the same sequence) are reported
+ *     per sequence in ev_verify_out.dev_status, not by return code.
+ *   - Batch invariance: every reduction's order is a function of the token's own data (DESIGN.md R-invariant): a row's
+ *     results do not depend on the other rows of the call, on the tree it arrives in (depth <= 8), or on the GPU.
+ *   - The shipped library reads no environment variable (bring-up switches exist only in -DEV_BRINGUP builds).
  *   - Layouts: all matrices row-major.  Weights [out_channels][in_channels] (K contiguous).
  *     Hidden states / logits [token][channel].  Batched tree arrays [B][T] with T = n_nodes_max.
  *   - A tree: node 0 is the root = the last emitted token, whose KV is not yet cached
