@@ -369,9 +369,17 @@ RowPlan row_plan(const ev_model* m, int M, int row_floats, int cl_par_max = CLUS
         else return fail(EV_EINVAL, "row too long for the row kernels");                                       \
     } while (0)
 
+// cudaFuncSetAttribute is per device: one flag per (kernel instantiation, device)
+inline bool& attr_flag(bool (&flags)[64]) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return flags[dev & 63];
+}
+
 template <int EPI, bool PAIR>
 int launch_gemm(cudaStream_t st, const CUtensorMap& tmX, const CUtensorMap& tmXh, const GemmArgs& a, int grid, int smem) {
-    static bool attr_set = false;
+    static bool flags[64] = {};
+    bool& attr_set = attr_flag(flags);
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(gemm_e4m3_kernel<EPI, PAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_set = true;
@@ -401,7 +409,8 @@ template <int MAXS>
 int launch_swiglu_s(ev_model* m, cudaStream_t st, bool smem_form, RowPlan rp, int M, const LinOut& gu, int F, float* tap, const QuantOut& q,
                     const L2Prefetch& pf) {
     if (smem_form) {
-        static bool attr_set = false;
+        static bool flags[64] = {};
+        bool& attr_set = attr_flag(flags);
         if (!attr_set) {
             CUDA_TRY(cudaFuncSetAttribute(swiglu_quant_smem_kernel<MAXS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
             attr_set = true;
@@ -560,7 +569,8 @@ int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
 
 template <int D, bool FP8>
 int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, dim3 grid) {
-    static bool attr_set = false;
+    static bool flags[64] = {};
+    bool& attr_set = attr_flag(flags);
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D, FP8>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D, FP8>::SMEM));
         attr_set = true;
@@ -571,7 +581,8 @@ int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, 
 template <int D>
 int launch_attn(cudaStream_t st, const AttnArgs& a, dim3 grid) {
     constexpr int smem = 2 * 2 * ATT_CH * D * 2 + ATT_WARPS * 3 * 16 * D * 2;
-    static bool attr_set = false;
+    static bool flags[64] = {};
+    bool& attr_set = attr_flag(flags);
     if (!attr_set) {
         CUDA_TRY(cudaFuncSetAttribute(tree_attn_partial_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         attr_set = true;

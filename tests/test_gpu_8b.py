@@ -1,6 +1,7 @@
-"""8B-shape parity at BASELINE.json's full sizes, in the launch configuration bench.py times, on sampled
-outputs the oracle computes one by one: the GPU runs the whole step (all 32 layers,
-whole batch); for sampled (sequence, layer) pairs the oracle recomputes that layer from the GPU's own layer
+"""8B-shape parity at BASELINE.json's full sizes on sampled outputs the oracle computes one by one (DESIGN.md
+section 5): the GPU runs the whole step (all 32 layers, whole batch) once EAGERLY with hidden / per-kernel taps (what the
+oracle is compared with) and once in the launch configuration bench.py times (no taps: the captured CUDA graph, the fused
+down-GEMM -> next-norm path), whose integer outputs must equal the eager run's; for sampled (sequence, layer) pairs the oracle recomputes that layer from the GPU's own layer
 input and the GPU's exported KV of that layer (verify = f(weights, KV, tree), DESIGN.md R-kv-input) and the
 outputs are compared at the north_star tolerances: hidden rel-L2 <= 1e-2 per layer, logits <= 2e-2 sigma,
 argmax equal where the oracle's top-2 gap >= 1e-3, acceptance walk / compaction indices bit-exact."""
@@ -131,6 +132,12 @@ def _run_config(spec, sample_layers, sample_seqs, batch=None, ctx_override=None)
         a = len(path) - 1
         assert acc[b] == a and nodes[b, :a + 1].tolist() == path and outs[b, :a + 1].tolist() == out
         assert newl[b] == int(ctx[b]) + a + 1
+    # the launch configuration bench.py times (CUDA graph replay, no taps) gives the same integers as the eager tapped run
+    for rep in range(2):       # first call captures, second replays
+        fast = run_verify(model, cache, slots, tokens, np.tile(parents, (B, 1)), commit=False, want_logits=False, want_hidden=False)
+        assert np.array_equal(fast.argmax.cpu().numpy(), am)
+        assert np.array_equal(fast.accept_len.cpu().numpy(), acc) and np.array_equal(fast.accept_nodes.cpu().numpy(), nodes)
+        assert np.array_equal(fast.out_tokens.cpu().numpy(), outs) and np.array_equal(fast.new_ctx_len.cpu().numpy(), newl)
     print("8B parity report (seq, layer|lm, rel-L2 | max|d|/sigma):", report)
     return report
 
