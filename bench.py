@@ -138,7 +138,7 @@ def plant(spec, parents, b, root, greedy_next, coins, base=None):
     return tk
 
 
-def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0, kv_fp8=False):
+def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0, kv_fp8=False, attn_chunk=0):
     shape = spec.model
     B, T = spec.batch, spec.n_nodes
     parents = tree_of(spec)
@@ -148,7 +148,7 @@ def build_gpu_workload(spec, steps_total, torch, ev, log, loop_steps=0, kv_fp8=F
     max_ctx = int(ctx.max()) + 64 + 8 + grow
     t0 = time.time()
     model = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=max_ctx, page_size=spec.page_size,
-                     act_scale_mode=spec.act_scale_mode, kv_dtype=1 if kv_fp8 else 0)
+                     act_scale_mode=spec.act_scale_mode, kv_dtype=1 if kv_fp8 else 0, attn_chunk=attn_chunk)
     for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
         model.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
     torch.cuda.synchronize()
@@ -256,7 +256,7 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
     """Builds the workload of one config, times `steps` verify steps (device events), the per-class pass, the end-to-end
     leg through ev_verify_host and - with --loop - the sustained closed loop.  Returns the JSON line as a dict."""
     kv_fp8 = args.kv == "fp8"
-    wk = build_gpu_workload(spec, warmup + steps, torch, ev, log, loop_steps=args.loop, kv_fp8=kv_fp8)
+    wk = build_gpu_workload(spec, warmup + steps, torch, ev, log, loop_steps=args.loop, kv_fp8=kv_fp8, attn_chunk=args.attn_chunk)
     model, cache, slots, ctx, parents, tokens = (wk[k] for k in ("model", "cache", "slots", "ctx", "parents", "tokens"))
     B, T = tokens.shape
     L0 = [int(x) for x in ctx]
@@ -429,7 +429,7 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
         "scaling": "weak", "vs_baseline": None, "dtype": f"e4m3 x e4m3 -> f32 ({'E4M3' if kv_fp8 else 'bf16'} KV, f32 residual)", "data": "synthetic",
         "config": {"workload": spec.name, "batch_per_gpu": B, "tree_nodes": T, "context": L0 if B <= 4 else [min(L0), max(L0)],
                    "cache_state": "cold: 7.5 GB of weights + KV exceed the 126 MB L2 every step", "replicas": world,
-                   "attn_chunk": "library default for this max_batch / max_ctx (ev_config.attn_chunk = 0)",
+                   "attn_chunk": args.attn_chunk or "library default for this max_batch (ev_config.attn_chunk = 0: 256 keys for <= 2 sequences, 2048 below 16, else 4096)",
                    "kv_cache": "E4M3, static per-tensor scales (PAPER.md:98; ev_config.kv_dtype = 1)" if kv_fp8 else "bf16 (BASELINE.json configs)"},
         "accepted_tokens_per_s": round(world * int(acc.sum()) / (ms_step * 1e-3), 1),
         "emitted_tokens_per_s": round(world * emitted / (ms_step * 1e-3), 1),
@@ -527,6 +527,7 @@ def main():
     ap.add_argument("--engine", action="store_true", help="also run the serving shell + draft side leg (ev_engine: plain decode, chain, tree)")
     ap.add_argument("--engine-steps", type=int, default=16)
     ap.add_argument("--engine-batch", type=int, default=32)
+    ap.add_argument("--attn-chunk", type=int, default=0, help="ev_config.attn_chunk (0 = the library's default for the model's max_batch)")
     ap.add_argument("--also", default="auto", help="configs whose short line is added under 'also' (default: 2 = batch 32 "
                                                    "when the headline config 1 runs on one GPU; 'none' to skip)")
     args = ap.parse_args()

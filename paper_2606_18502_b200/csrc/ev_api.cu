@@ -918,7 +918,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     A(dev_alloc(m, &m->attn, (size_t)m->M_pad * m->q_dim));
     // default chunk length: short for models built for one or two sequences (every chunk is its own CTA: latency), long
     // for batched serving (fewer partial outputs per row); a function of the config only, hence fixed for the model's life
-    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : (cfg->max_batch <= 2 ? 256 : 2048);
+    m->attn_chunk = cfg->attn_chunk > 0 ? cfg->attn_chunk : (cfg->max_batch <= 2 ? 256 : (cfg->max_batch < 16 ? 2048 : 4096));
     m->n_chunks_max = (cfg->max_ctx + m->attn_chunk - 1) / m->attn_chunk;
     A(dev_alloc(m, &m->o_part, (size_t)m->M_cap * m->n_chunks_max * m->q_dim));
     A(dev_alloc(m, &m->ml_part, (size_t)m->M_cap * m->n_chunks_max * cfg->n_q_heads * 2));
