@@ -251,12 +251,13 @@ def test_gpu_speculative_loop_is_lossless_teacher_forced(setup):
     """PAPER.md:92 on the GPU: a multi-step speculative loop (planted + random drafts).  Multi-step free-running
     comparison is not a fixed-tolerance statement (one E4M3 code flip moves a logit by up to ~0.05 sigma and the
     sequences then diverge for good: DESIGN.md section 5), so the oracle is teacher-forced with the GPU's history:
-    at every step it verifies the SAME tree on a cache holding the SAME tokens, and every token the GPU emits must be
-    the oracle's argmax at that node -- literally where the oracle's top-2 gap >= 1e-3 AND the two sides' logits agree
-    within the 2e-2 sigma tolerance; a mismatch is only admissible where the oracle's margin between the two tokens is
-    below twice that logit tolerance (both sides within tolerance of each other), and at most 2 of the 24 positions.
-    Then the GPU's own token-by-token greedy decode of the emitted sequence must reproduce it (tree-verify logits ==
-    decode logits on the GPU), same admissibility rule."""
+    at every step it verifies the SAME tree on a cache holding the SAME tokens.  In every step whose GPU logits agree with
+    the oracle's within the 2e-2 sigma tolerance, the north_star rule holds literally: every emitted token is the oracle's
+    argmax at its node unless the oracle's top-2 gap there is below 1e-3.  A step in which an E4M3 code flipped (logits off
+    by more than the tolerance; the noise floor of profiles/r2_parity_protocol.md shows such events at config[0] with a
+    GPU-prefilled cache) is counted - at most 2 of the steps - and only there the margin rule applies.
+    Then the paper's own guarantee, with NO allowance: the GPU's token-by-token greedy decode of the same context emits
+    exactly the speculative loop's tokens (R-invariant: tree-verify and decode reduce every token in the same order)."""
     from gpu_helpers import import_oracle_kv, run_verify
     spec, gm, om, ev = setup
     V = spec.model.vocab
@@ -288,12 +289,17 @@ def test_gpu_speculative_loop_is_lossless_teacher_forced(setup):
         out = buf.out_tokens.cpu().numpy()[0, :a + 1].tolist()
         assert path[0] == 0 and all(parents[path[k + 1]] == path[k] for k in range(a))
         assert out[:a] == [int(toks[c]) for c in path[1:]]
+        flipped = float(np.max(np.abs(buf.logits.cpu().numpy() - ref["logits"]))) > TOL_LOGIT_SIGMA * sigma
+        soft += int(flipped)
         for k, node in enumerate(path):     # the token emitted after `node` must be the target argmax there
             lg = ref["logits"][node]
             top = int(np.argmax(lg))
             if out[k] != top:
-                assert lg[top] - lg[out[k]] < 2 * TOL_LOGIT_SIGMA * sigma, (steps, k, lg[top] - lg[out[k]])
-                soft += 1
+                srt = np.sort(lg)
+                if not flipped:
+                    assert srt[-1] - srt[-2] < GAP, (steps, k, srt[-1] - srt[-2])          # literal north_star exemption
+                else:
+                    assert lg[top] - lg[out[k]] < 2 * TOL_LOGIT_SIGMA * sigma, (steps, k, lg[top] - lg[out[k]])
         vo.kv_compact(oc, 0, path)          # oracle cache follows the GPU's accepted path
         emitted += out
         root = out[-1]
@@ -305,16 +311,11 @@ def test_gpu_speculative_loop_is_lossless_teacher_forced(setup):
     slot2 = cache2.ev_cache_add_seq(160)
     import_oracle_kv(cache2, slot2, _oracle_ctx(om, ids), 0, L, 2)
     one = ev.VerifyBuffers(gm, 1, 1, want_logits=True, want_hidden=False)
-    tok, soft2 = 11, 0
+    tok = 11
     for i in range(n_tok):
         run_verify(gm, cache2, [slot2], np.array([[tok]], np.int32), np.array([[-1]], np.int32), commit=True, buf=one)
-        lg = one.logits.cpu().numpy()[0]
-        top = int(np.argmax(lg))
-        if top != emitted[i]:
-            assert lg[top] - lg[emitted[i]] < 2 * TOL_LOGIT_SIGMA * sigma, (i, lg[top] - lg[emitted[i]])
-            soft2 += 1
-        tok = emitted[i]
-    assert soft2 <= 2, soft2
+        tok = int(one.out_tokens.cpu().numpy()[0, 0])
+        assert tok == emitted[i], (i, tok, emitted[i])          # bit-exact: no tolerance, no exemption
 
 
 def test_kv_pool_container_round_trip(setup):
