@@ -304,6 +304,31 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
         step()
     prof = model.ev_profile_read()
     model.ev_profile_enable(False)
+    # duration of every kernel INSIDE the graph-replayed step (the library's step trace: %globaltimer when a kernel's first CTA
+    # passes griddepcontrol.wait and when its last CTA leaves); the CUDA-event class times above come from an eager pass
+    # whose launches are CPU-paced
+    ingraph = None
+    try:
+        model.ev_profile_enable(2)
+        step(); step()
+        torch.cuda.synchronize()
+        model.ev_profile_trace()
+        step()
+        torch.cuda.synchronize()
+        tr = np.asarray(model.ev_profile_trace(), dtype=np.float64)
+        names = ["rmsnorm_quant", "gemm_qkv", "rope_kvwrite", "tree_attention", "attn_merge_quant", "gemm_o", "rmsnorm_quant", "gemm_gateup",
+                 "swiglu_quant", "gemm_down"]
+        nl = spec.model.n_layers
+        if tr.shape[0] >= 10 * nl + 2:
+            ex = (tr[:, 2] - tr[:, 1]) / 1e3      # us: last exit - first past-wait
+            ingraph = {}
+            for i in range(10 * nl):
+                ingraph[names[i % 10]] = ingraph.get(names[i % 10], 0.0) + ex[i]
+            ingraph["gemm_lm_head"] = ex[10 * nl + 1]
+            ingraph["step_us"] = (tr[10 * nl + 1, 2] - tr[0, 0]) / 1e3
+    except Exception as e:  # pragma: no cover
+        log(f"step trace unavailable: {e}")
+    model.ev_profile_enable(0)
     work = algorithmic_work(spec, ctx, parents, kv_fp8)
     pk = peaks()
     gemm_ms = sum(v[0] for k, v in prof.items() if k.startswith("gemm_"))
@@ -334,6 +359,14 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
                     "peak": pk["hbm_gbs"], "peak_source": peak_src, "unit": "GB/s", "frac": round(kv_gbs / pk["hbm_gbs"], 4),
                     "bytes_per_launch": work["kv_bytes"] / (attn_n / steps), "gemm_frac_of_its_own_bound": roofline["frac"]}
         gemm_n, gemm_ms = attn_n, attn_ms
+    if ingraph is not None:
+        g_us = sum(v for k, v in ingraph.items() if k.startswith("gemm_"))
+        roofline["in_graph"] = {"us_per_step_by_class": {k: round(v, 1) for k, v in ingraph.items()},
+                                "gemm_gbs": round(work["weight_bytes"] / (g_us * 1e-6) / 1e9, 1),
+                                "gemm_frac_of_hbm": round(work["weight_bytes"] / (g_us * 1e-6) / 1e9 / pk["hbm_gbs"], 4),
+                                "gemm_tflops": round(lin_flops / (g_us * 1e-6) / 1e12, 1),
+                                "def": "per-kernel durations inside the CUDA-graph replay (step trace: first CTA past griddepcontrol.wait -> last CTA exit, "
+                                       "%globaltimer), summed per class over one step; the event-timed `achieved` above is from an eager, CPU-paced pass"}
     roofline.update({"launches_per_step": gemm_n // steps, "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic,
                      "time_share_by_class": share, "avg_launch_us_by_class": per_launch_us})
     t_roof = max((work["weight_bytes"] + work["kv_bytes"]) / (pk["hbm_gbs"] * 1e9), work["flops"] / fp8_peak[0])

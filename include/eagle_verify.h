@@ -324,8 +324,9 @@ int ev_op_quantize_rows(ev_model*, const float* dev_x, int M, int K, float stati
  * device, sums elapsed ms and launch counts per class into the host arrays and clears the record. */
 int ev_profile_enable(ev_model*, int on);
 int ev_profile_read(ev_model*, double* host_ms_by_class, long* host_count_by_class, int n_classes);
-/* Step trace (models created with EV_TRACE=1 in the environment): every kernel of the layer loop of the
- * last ev_verify (graph replays included) records, with %globaltimer, min over its CTAs of the time it
+/* ev_profile_enable(m, 1): per-class CUDA-event timing (the step then runs eagerly); (m, 2): step trace; (m, 0): both off.
+ * Step trace: every kernel of the layer loop of the last ev_verify (CUDA-graph replays included: this is how a kernel's
+ * duration INSIDE the replayed, programmatic-dependent-launch step is measured) records, with %globaltimer, min over its CTAs of the time it
  * entered, min and max of the time it passed griddepcontrol.wait, and max of the time it left.
  * host_out[i][8] = {t_enter, t_past_wait_first, t_exit, t_past_wait_last, 4 bring-up phase marks} in ns for launch i, in launch
  * order (per layer: norm, QKV, RoPE, attention, merge, O, norm, gate/up, SwiGLU, down; then norm, LM

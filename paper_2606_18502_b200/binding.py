@@ -240,7 +240,8 @@ class Model:
                        "rmsnorm_quant", "rope_kvwrite", "swiglu_quant", "other")
 
     def ev_profile_enable(self, on=True):
-        _check(self.lib.ev_profile_enable(self.h, 1 if on else 0))
+        """True / 1: per-class CUDA-event timing; 2: in-graph step trace (ev_profile_trace); False / 0: off"""
+        _check(self.lib.ev_profile_enable(self.h, int(on)))
 
     def ev_profile_read(self):
         """-> {class: (total_ms, launches)} since enable / the last read."""
@@ -252,7 +253,7 @@ class Model:
 
     def ev_profile_trace(self, max_entries=1024):
         """-> list of (t_enter, t_past_wait_first, t_exit, t_past_wait_last, 4 phase marks) in ns per traced launch of the
-        last verify step (needs EV_TRACE=1 in the environment when the model was created)."""
+        last verify step (after ev_profile_enable(2))."""
         buf = (C.c_ulonglong * (8 * max_entries))()
         n = C.c_int(0)
         _check(self.lib.ev_profile_trace(self.h, buf, max_entries, C.byref(n)))

@@ -158,7 +158,8 @@ struct ev_model {
     float* ml_part = nullptr;
     float* lin_out = nullptr;   // raw GEMM output [splits][M][N], consumed by the next element-wise kernel
     long lin_floats = 0;
-    unsigned long long* trace = nullptr;   // EV_TRACE=1: [TRACE_CAP][4] step trace, see ev_profile_trace
+    unsigned long long* trace = nullptr;   // ev_profile_enable(m, 2): [TRACE_CAP][TRACE_SLOTS] step trace, see ev_profile_trace
+    bool trace_on = false;
     int n_traced = 0;
     // tree state
     int32_t *attn_order = nullptr;
@@ -651,7 +652,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
     PfPlanner pfp;
     pfp.on = M <= m->l2pf_max_m && !m->profile;
     pfp.cap = (size_t)m->l2pf_cap; pfp.maxq = (size_t)m->l2pf_maxq;
-    pfp.trace = m->trace; pfp.trace_cap = TRACE_CAP;
+    pfp.trace = m->trace_on ? m->trace : nullptr; pfp.trace_cap = TRACE_CAP;
     pfp.mask = m->l2pf_mask; pfp.n_layer_launches = 10 * cfg.n_layers;
     if (pfp.on) {
         auto qbytes = [](const QMat& q) { return (size_t)q.n_tiles * q.total_kb * GEMM_WTILE; };
@@ -927,15 +928,6 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
         m->lin_floats = std::max<long>((long)m->M_pad * widest, 8L * std::min(m->M_pad, 256) * widest);
     }
     A(dev_alloc(m, &m->lin_out, (size_t)m->lin_floats));
-#ifdef EV_BRINGUP
-    const bool want_trace = getenv("EV_TRACE") && atoi(getenv("EV_TRACE")) != 0;
-#else
-    const bool want_trace = false;
-#endif
-    if (want_trace) {
-        A(dev_alloc(m, &m->trace, (size_t)TRACE_CAP * TRACE_SLOTS));
-        cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8);
-    }
     A(dev_alloc(m, &m->Lsnap, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->nn_eff, (size_t)cfg->max_batch));
     A(dev_alloc(m, &m->attn_order, (size_t)cfg->max_batch));
@@ -1717,8 +1709,17 @@ int ev_verify_host(ev_model* m, ev_cache* c, int n_seqs, int n_nodes, const int3
 // ---- per-kernel-class device timing (CUDA events on the launching stream) ----------------------------------
 int ev_profile_enable(ev_model* m, int on) {
     if (!m) return fail(EV_EINVAL, "null argument");
-    m->profile = on != 0;
+    m->profile = on == 1;
     m->prof_used = 0;
+    const bool want_trace = on == 2;
+    if (want_trace && !m->trace) {
+        EV_TRY(dev_alloc(m, &m->trace, (size_t)TRACE_CAP * TRACE_SLOTS));
+        CUDA_TRY(cudaMemset(m->trace, 0xFF, (size_t)TRACE_CAP * TRACE_SLOTS * 8));
+    }
+    if (want_trace != m->trace_on) {   // the trace slots are kernel arguments: captured steps are re-captured with / without them
+        m->trace_on = want_trace;
+        drop_graphs(m);
+    }
     return EV_OK;
 }
 int ev_profile_read(ev_model* m, double* host_ms_by_class, long* host_count_by_class, int n_classes) {
@@ -1739,7 +1740,7 @@ int ev_profile_read(ev_model* m, double* host_ms_by_class, long* host_count_by_c
 // bring-up: copies the per-CTA GEMM phase timestamps of the last launch (EV_GEMM_DBG & 16) to the host
 int ev_profile_trace(ev_model* m, unsigned long long* host_out, int max_entries, int* n_out) {
     if (!m || !host_out || !n_out) return fail(EV_EINVAL, "null argument");
-    if (!m->trace) return fail(EV_ESTATE, "step trace is off (create the model with EV_TRACE=1 in the environment)");
+    if (!m->trace || !m->trace_on) return fail(EV_ESTATE, "step trace is off (ev_profile_enable(model, 2) turns it on)");
     CUDA_TRY(cudaDeviceSynchronize());
     const int n = std::min(std::min(max_entries, m->n_traced), TRACE_CAP);
     CUDA_TRY(cudaMemcpy(host_out, m->trace, (size_t)n * TRACE_SLOTS * 8, cudaMemcpyDeviceToHost));
