@@ -175,7 +175,7 @@ def _rank0_chain(parents):
     return chain
 
 
-def _lossless(spec, B, ctx, n_steps=8, planted_p=0.7):
+def _lossless(spec, B, ctx, n_steps=8, planted_p=0.7, kv_fp8=False):
     import paper_2606_18502_b200 as ev
     from gpu_helpers import run_verify
     shape = spec.model
@@ -184,11 +184,11 @@ def _lossless(spec, B, ctx, n_steps=8, planted_p=0.7):
     depth = int(wl.tree_depths(parents).max())
     n_greedy = n_steps * (depth + 1) + depth + 1
     model = ev.Model(shape, max_batch=2 * B, max_tree_nodes=64, max_ctx=int(max(ctx)) + n_greedy + 80, page_size=spec.page_size,
-                     act_scale_mode=spec.act_scale_mode)
+                     act_scale_mode=spec.act_scale_mode, kv_dtype=1 if kv_fp8 else 0)
     for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
         model.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
-    if spec.act_scale_mode == 1:
-        model.ev_model_calibrate(torch.from_numpy(wl.calibration_hidden(spec)).cuda())
+    if spec.act_scale_mode == 1 or kv_fp8:
+        model.ev_model_calibrate(torch.from_numpy(wl.calibration_hidden(spec, None if spec.calib_tokens else 512)).cuda())
     cap = [int(L) + n_greedy + 72 for L in ctx]
     cache = ev.Cache(model, 2 * sum(c // spec.page_size + 2 for c in cap) + cap[0] // spec.page_size + 2, 2 * B + 1)
     s_slots = [cache.ev_cache_add_seq(c) for c in cap]     # speculative decoding
@@ -272,3 +272,74 @@ def test_config3_gpu_speculative_equals_gpu_greedy():
 
 def test_config4_gpu_speculative_equals_gpu_greedy():
     _lossless(wl.CONFIGS[4], 2, [16384, 16384])
+
+
+def test_config2_fp8_kv_cache_gpu_speculative_equals_gpu_greedy():
+    """SURVEY section 8(f)-2 at 8B shape: the same bit-exact self-consistency with the FP8 (E4M3) KV cache."""
+    import dataclasses
+    _lossless(dataclasses.replace(wl.CONFIGS[2], name="cfg2_fp8kv"), 3, [4096, 4096, 3000], kv_fp8=True)
+
+
+def test_drafter_forward_at_8b_shape_matches_oracle():
+    """SURVEY section 8(f)-3 at 8B shape: FC (K = 8192) + one decoder layer + shared LM head of the draft model against
+    oracle/drafter_oracle.py, lock-step from given predecessor features: predicted features rel-L2 <= 1e-2, logits <= 2e-2
+    sigma, top-k equal where the oracle's gaps are >= 1e-3."""
+    import dataclasses
+    import paper_2606_18502_b200 as ev
+    from oracle import drafter_oracle as do
+    from gpu_helpers import bf16_cuda_to_bits
+    shape = wl.LLAMA8B
+    seed = 9
+    dshape = dataclasses.replace(shape, name="llama8b_drafter", n_layers=1)
+    dg = ev.Model(dshape, 1, 64, 256)
+    tshape = dataclasses.replace(shape, name="llama8b_head_only", n_layers=1)     # a stand-in target: only its embedding, final norm and LM head are used
+    to = vo.OracleModel(tshape)
+    dm = do.DraftModel(to, shape)
+    for kind in ("embed", "lm_head"):
+        w = wl.weight_matrix_bf16(shape, seed, kind, 0, device="cuda")
+        dg.ev_model_set_weight(kind, 0, w)
+        to.set_weight(kind, 0, bf16_cuda_to_bits(w))
+    for k in LAYER_KINDS:
+        w = wl.weight_matrix_bf16(shape, seed, k, shape.n_layers, device="cuda")
+        dg.ev_model_set_weight(k, 0, w)
+        dm.set_weight(k, bf16_cuda_to_bits(w))
+    w = wl.weight_matrix_bf16(shape, seed, "d_fc", 0, device="cuda")
+    dg.ev_model_set_weight("d_fc", 0, w)
+    dm.set_weight("d_fc", bf16_cuda_to_bits(w))
+    del w
+    rng = np.random.default_rng(4)
+    H = shape.hidden
+    ctx_tok = rng.integers(0, shape.vocab, size=48).astype(np.int32)
+    ctx_feat = (rng.standard_normal((48, H)) * 2.0).astype(np.float32)
+    par = wl.tree_parents(12, (3, 2, 2))
+    toks = rng.integers(0, shape.vocab, size=12).astype(np.int32)
+    feats = (rng.standard_normal((12, H)) * 2.0).astype(np.float32)
+    odc = vo.OracleKV(dm.layer, 8, 16)
+    odc.add_seq(0, 100)
+    do.draft_extend(dm, odc, 0, ctx_tok, ctx_feat)
+    f_o, lg_o = do.draft_forward(dm, odc, 0, toks, feats, par)
+    dcache = ev.Cache(dg, 8, 1)
+    slot = dcache.ev_cache_add_seq(100)
+    i32 = lambda x: torch.as_tensor(np.asarray(x, dtype=np.int32)).cuda()  # noqa: E731
+    tb = torch.zeros((1, 64), dtype=torch.int32, device="cuda")
+    tb[0, :48] = i32(ctx_tok)
+    fb = torch.zeros((1, 64, H), dtype=torch.float32, device="cuda")
+    fb[0, :48] = torch.from_numpy(ctx_feat).cuda()
+    ev.ev_draft_extend(dg, dcache, i32([slot]), tb, fb, i32([48]))
+    buf = ev.VerifyBuffers(dg, 1, 12, want_logits=True, want_final_hidden=True, topk=4)
+    buf.set_inputs([slot], toks[None], par[None])
+    buf.features = torch.from_numpy(feats).cuda()
+    ev.ev_verify(dg, dcache, buf, commit=False)
+    torch.cuda.synchronize()
+    f_g = buf.final_hidden.cpu().numpy()
+    assert rel_l2(f_g, f_o) <= 1e-2, rel_l2(f_g, f_o)
+    # logits lock-step from the GPU's own predicted features (DESIGN.md section 5: one quantization site)
+    lg_ref = vo.lm_head(to, f_g)
+    lg = buf.logits.cpu().numpy()
+    assert np.max(np.abs(lg - lg_ref)) <= 2e-2 * lg_ref.std()
+    tk = buf.topk.cpu().numpy()
+    for i in range(12):
+        assert tk[i].tolist() == do.top_k_tokens(lg[i], 4).tolist(), i          # exactly the top-k of the GPU's own logits
+        srt = np.sort(lg_ref[i])[::-1]
+        if (srt[:4] - srt[1:5]).min() >= 1e-3:
+            assert tk[i].tolist() == do.top_k_tokens(lg_ref[i], 4).tolist(), i
