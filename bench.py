@@ -617,14 +617,21 @@ def main():
         args.loop = 0
         extra = {}
         for c in also:
-            l2 = measure(wl.CONFIGS[c], args, torch, ev, dist, rank, world, local_rank, log, 3, min(args.steps, 8), False, fp8_peak)
+            try:
+                l2 = measure(wl.CONFIGS[c], args, torch, ev, dist, rank, world, local_rank, log, 3, min(args.steps, 8), False, fp8_peak)
+            except Exception as e:   # the headline line must survive a failure of the ride-along config (it is reported, not hidden)
+                extra[wl.CONFIGS[c].name] = {"error": f"{type(e).__name__}: {e}"[:300]}
+                continue
             if l2 is not None:
                 extra[wl.CONFIGS[c].name] = {k: l2[k] for k in ("value", "unit", "ms_per_step", "steps", "config", "mean_emitted_per_step",
                                                                    "planted_emitted_per_step", "emitted_tokens_per_s", "step_roofline", "roofline", "e2e", "clocks", "attention")}
         if line is not None:
             line["also"] = extra
     if args.engine and rank == 0 and line is not None:
-        line["engine"] = engine_leg(spec, args, torch, ev, log)
+        try:
+            line["engine"] = engine_leg(spec, args, torch, ev, log)
+        except Exception as e:
+            line["engine"] = {"error": f"{type(e).__name__}: {e}"[:300]}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if dist is not None:
