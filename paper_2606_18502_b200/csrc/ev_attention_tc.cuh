@@ -51,7 +51,11 @@ struct TcaCfg {
     static constexpr int VS = FP8 ? 4 : TCA_VS;          // fp16 V tiles in flight
     static constexpr int RS = FP8 ? 4 : 0;               // raw E4M3 tiles in flight, per K and per V
     static constexpr int RAW_BYTES = TCA_BN * D;         // one raw tile: 64 keys x D bytes
-    static constexpr int THREADS = FP8 ? TCA_THREADS + 64 : TCA_THREADS;
+    // bf16 pool: Q.K^T and P.V have separate issuing warps (1 and 18).  FP8 pool: one issuer (warp 1) - a 21st warp would put six
+    // warps on one scheduler (80 registers per thread, 216 B of spills) and the converter warps set the pace there anyway.
+    static constexpr bool TWO_ISSUERS = !FP8;
+    static constexpr int PV_WARP = FP8 ? -1 : 18;
+    static constexpr int THREADS = FP8 ? TCA_THREADS + 64 : TCA_THREADS + 32;
     static constexpr int NH = D / 64;                    // 128-byte (64-element) halves of a head row
     static constexpr int Q_PART = NH * 128 * 128;        // bytes of one bf16 part of the 128 x D query tile
     static constexpr int Q_BYTES = 2 * Q_PART;
@@ -193,7 +197,8 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     uint64_t* p_full = s_full + C::NSP;                   // [3]
     uint64_t* o_full = p_full + C::NSP;                   // [2]
     uint64_t* o_empty = o_full + 2;                       // [2]
-    uint64_t* raw_full = o_empty + 2;                     // FP8: [2][RS] raw tile landed (K ring, then V ring)
+    uint64_t* sp_free = o_empty + 2;                      // [NSP] P.V has read P(j): the S/P region may take S(j + NSP)
+    uint64_t* raw_full = sp_free + C::NSP;                // FP8: [2][RS] raw tile landed (K ring, then V ring)
     uint64_t* raw_empty = raw_full + 8;                   // FP8: [2][RS] raw tile converted
     uint32_t* tmem_base_smem = reinterpret_cast<uint32_t*>(raw_empty + 8);
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
@@ -211,7 +216,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     if (threadIdx.x == 0) {
         for (int s = 0; s < TCA_KS; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
         for (int s = 0; s < TCA_VS; ++s) { mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
-        for (int i = 0; i < C::NSP; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); }
+        for (int i = 0; i < C::NSP; ++i) { mbar_init(&s_full[i], 1); mbar_init(&p_full[i], 8); mbar_init(&sp_free[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&o_full[i], 1); mbar_init(&o_empty[i], 8); }
         if (FP8) for (int i = 0; i < 8; ++i) { mbar_init(&raw_full[i], 1); mbar_init(&raw_empty[i], 1); }   // [K|V][slot], stride 4
         fence_barrier_init();
@@ -324,27 +329,30 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 tma_load_4d(ring + sl * C::K_BYTES + dst_off, &tmKV, &full[sl], 0, 0, 0, row_cur);
             }
         }
-    } else if (warp == 1) {
-        // ===== MMA issuer.  The WHOLE warp runs the loop (so addresses and descriptors are provably warp-uniform and
+    } else if (warp == 1 || warp == C::PV_WARP) {
+        // ===== MMA issuers.  The WHOLE warp runs the loop (so addresses and descriptors are provably warp-uniform and
         // live in uniform registers); one elected lane issues.  Under `if (lane == 0)` the compiler wrapped every
-        // tcgen05.mma in an ELECT / R2UR / BRA.U.ANY loop: ~100 cycles per instruction, 36 instructions per tile,
-        // which made this thread - not the tensor pipe, not the softmax - the bottleneck (profiles/r1_attention_v2.md).
+        // tcgen05.mma in an ELECT / R2UR / BRA.U.ANY loop: ~100 cycles per instruction (profiles/r1_attention_v2.md).
+        // A tcgen05.mma holds its issuing thread until the tensor pipe takes it: with ONE issuer the thread's time per tile
+        // was the pipe's 1,024 cycles + ~350 of barrier round trips and commits + its waits, during which the pipe drained
+        // (1,900 cycles per tile; profiles/r2_attention_issue.md).  With TWO_ISSUERS warp 1 issues Q.K^T and warp PV_WARP
+        // issues P.V, so one warp's waits run under the other's MMAs; the pipe then no longer orders S(j) behind
+        // P.V(j - NSP) by itself: sp_free says so. =====
         constexpr uint32_t idesc_qk = umma_idesc_f16(128, TCA_BN, 0);
         constexpr uint32_t idesc_pv = umma_idesc_f16(128, D, 1);
         const bool leader = elect_one();
-        constexpr bool do_mma = true;
         const uint32_t q_tmem = tmem_base + C::TQ;
         const uint32_t kv_addr = smem_u32(kv_s);
         auto issue_pv = [&](int i) {
             const int s = i % TCA_VS;
             mbar_wait(&v_full[s], (i / TCA_VS) & 1);
-            mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
             mbar_wait(&o_empty[i % C::NO], ((i / C::NO) & 1) ^ 1);   // the correction warps have read chunk i - NO
+            mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
             tc_fence_after();
             const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
             const uint32_t d_addr = tmem_base + C::TO + (i % C::NO) * D;
             const uint32_t p_addr = tmem_base + C::TP + (i % C::NSP) * C::SP;
-            if (leader && do_mma) {
+            if (leader) {
 #pragma unroll
                 for (int part = 1; part >= 0; --part) {
 #pragma unroll
@@ -352,8 +360,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                         umma_bf16_ts(d_addr, p_addr + part * 32 + t * 8, vdesc + (uint64_t)(t * (C::PAGE_BYTES >> 4)), idesc_pv,
                                      (part == 1 && t == 0) ? 0u : 1u);
                 }
-            }
-            if (leader) {
+                if (C::TWO_ISSUERS) umma_commit(&sp_free[i % C::NSP]);
                 umma_commit(&v_empty[s]);
                 umma_commit(&o_full[i % C::NO]);
             }
@@ -362,10 +369,11 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         auto issue_qk = [&](int j) {
             const int s = j % TCA_KS;
             mbar_wait(&k_full[s], (j / TCA_KS) & 1);
+            if (C::TWO_ISSUERS) mbar_wait(&sp_free[j % C::NSP], ((j / C::NSP) & 1) ^ 1);   // P.V(j - NSP) has read the region S(j) goes into
             tc_fence_after();
             const uint32_t k_addr = kv_addr + s * C::K_BYTES;
             const uint32_t s_addr = tmem_base + C::TS + (j % C::NSP) * C::SP;
-            if (leader && do_mma) {
+            if (leader) {
 #pragma unroll
                 for (int part = 1; part >= 0; --part) {
 #pragma unroll
@@ -377,20 +385,23 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                                          (part == 1 && h == 0 && ks == 0) ? 0u : 1u);
                     }
                 }
-            }
-            if (leader) {
                 umma_commit(&k_empty[s]);
                 umma_commit(&s_full[j % C::NSP]);
             }
             __syncwarp();
         };
-        // Q.K^T runs NSP - 1 tiles ahead of P.V: S(j + NSP - 1) goes into the region P(j-1) was read from by P.V(j-1),
-        // issued one iteration earlier (the tensor pipe executes in issue order)
-        constexpr int LA = C::NSP - 1;   // S/P regions - 1 tiles of look-ahead
-        for (int j = 0; j < min(LA, n_tiles); ++j) issue_qk(j);
-        for (int j = 0; j < n_tiles; ++j) {
-            if (j + LA < n_tiles) issue_qk(j + LA);
-            issue_pv(j);
+        if (C::TWO_ISSUERS) {
+            if (warp == 1) for (int j = 0; j < n_tiles; ++j) issue_qk(j);
+            else for (int i = 0; i < n_tiles; ++i) issue_pv(i);
+        } else {
+            // one issuer: Q.K^T runs NSP - 1 tiles ahead of P.V; S(j + NSP - 1) goes into the region P(j-1) was read from by
+            // P.V(j-1), issued one iteration earlier (the tensor pipe executes one thread's MMAs in issue order)
+            constexpr int LA = C::NSP - 1;
+            for (int j = 0; j < min(LA, n_tiles); ++j) issue_qk(j);
+            for (int j = 0; j < n_tiles; ++j) {
+                if (j + LA < n_tiles) issue_qk(j + LA);
+                issue_pv(j);
+            }
         }
     } else if (warp >= 18) {
         // ===== FP8 converters (warp 18: K tiles, warp 19: V tiles): raw [64 keys][D codes] -> fp16 tile in the layout the
@@ -449,7 +460,10 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         const uint32_t lane_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
         constexpr float LOG2E = 1.4426950408889634f;
         float m_run = -INFINITY, l_run = 0.f;   // l_run carries P's factor 2^15
+        // Scores stay RAW in the loop (S = 2^6 q . k): s = rn(S * qk_scale) is the method's rounded score and rounding is monotone,
+        // so the chunk's max is rn(max(S) * qk_scale), taken once when the chunk ends; the exponent (S - M) * k2 is one FFMA per key.
         const float qk_scale = FP8 ? mul_rn(a.scale * (1.f / TCA_QSCALE), ta.k_scale) : a.scale * (1.f / TCA_QSCALE);   // FP8: the K cache's static scale rides along
+        const float k2 = mul_rn(qk_scale, LOG2E);
 
         // (max, sum) of a finished chunk go to its partial slot (the two halves of a row meet in shared memory) and the
         // state restarts: t_left counts the tiles left in the current chunk
@@ -468,8 +482,6 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             tmem_ld32(lane_addr + C::TS + (j % C::NSP) * C::SP + wg * 32, sv);
             tmem_ld_wait();
             const int kb = k_begin + j * TCA_BN + wg * 32;
-#pragma unroll
-            for (int e = 0; e < 32; ++e) sv[e] = __float_as_uint(mul_rn(__uint_as_float(sv[e]), qk_scale));  // s = (q.k) / sqrt(d), rounded as the method states (2^6 of Q taken out exactly)
             if (kb + 32 > L - ATT_TAIL_R) {   // tile half reaches the end of some row's bulk (warp-uniform)
 #pragma unroll
                 for (int e = 0; e < 32; ++e)
@@ -487,10 +499,10 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             mx = fmaxf(mx, xmax[((j & 1) * 2 + (wg ^ 1)) * 128 + r]);
             const float mn = fmaxf(m_run, mx);
             const float mu = (mn == -INFINITY) ? 0.f : mn;
-            const float c = ex2_approx((m_run - mu) * LOG2E);  // 2^-inf = 0 on the first tile
+            const float c = ex2_approx((m_run - mu) * k2);  // 2^-inf = 0 on the first tile
             m_run = mn;
             if (wg == 0) xc[(j & 7) * 128 + r] = c;
-            const float nmk = fmaf(-mu, LOG2E, TCA_PSCALE_LOG2);   // p' = 2^15 p
+            const float nmk = fmaf(-mu, k2, TCA_PSCALE_LOG2);   // p' = 2^15 p
             float ls0 = 0.f, ls1 = 0.f;
             const uint32_t p_addr = lane_addr + C::TP + (j % C::NSP) * C::SP + wg * 16;
 #pragma unroll
@@ -498,8 +510,8 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 uint32_t ph[8], pl[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const float p0 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e]), LOG2E, nmk));
-                    const float p1 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e + 1]), LOG2E, nmk));
+                    const float p0 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e]), k2, nmk));
+                    const float p1 = ex2_approx(fmaf(__uint_as_float(sv[16 * h + 2 * e + 1]), k2, nmk));
                     ls0 += p0;
                     ls1 += p1;
                     split2_pack(p0, p1, ph[e], pl[e]);
@@ -515,7 +527,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             if (--t_left == 0 || j == n_tiles - 1) {   // chunk finished (CTA-uniform)
                 xsum[wg * 128 + r] = l_run * exp2f(-TCA_PSCALE_LOG2);   // exact
                 pair_bar_sync(1 + (warp & 3));
-                if (valid && wg == 0) *mlp = make_float2(m_run, xsum[r] + xsum[128 + r]);
+                if (valid && wg == 0) *mlp = make_float2(mul_rn(m_run, qk_scale), xsum[r] + xsum[128 + r]);
                 ++mlp;
                 m_run = -INFINITY; l_run = 0.f;
                 t_left = tpc;
