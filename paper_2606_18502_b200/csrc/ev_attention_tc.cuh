@@ -179,6 +179,17 @@ __device__ __forceinline__ void e4m3x16_to_f16(const uint4& in, uint4& lo, uint4
     cv(in.x, lo.x, lo.y); cv(in.y, lo.z, lo.w); cv(in.z, hi.x, hi.y); cv(in.w, hi.z, hi.w);
 }
 
+// Bring-up probe (-DEV_ATTN_PROBE, never in the product build): every role of CTA (0, 0, 0) adds up the cycles it spends in
+// each of its barrier waits and prints them for the first launches with >= 48 key tiles (profiles/r2_attention_issue.md).
+#ifdef EV_ATTN_PROBE
+__device__ int tca_probe_count = 0;
+#define TCA_WAIT(bar, ph, acc) do { const long long t0_ = clock64(); mbar_wait(bar, ph); acc += clock64() - t0_; } while (0)
+#define TCA_PROBE(...) __VA_ARGS__
+#define TCA_PROBE_ON (lane == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n_tiles >= 48 && tca_probe_count < 4)
+#else
+#define TCA_WAIT(bar, ph, acc) mbar_wait(bar, ph)
+#define TCA_PROBE(...)
+#endif
 template <int D, bool FP8>
 __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
     using C = TcaCfg<D, FP8>;
@@ -343,11 +354,12 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         const bool leader = elect_one();
         const uint32_t q_tmem = tmem_base + C::TQ;
         const uint32_t kv_addr = smem_u32(kv_s);
+        TCA_PROBE(long long pw[5] = {0, 0, 0, 0, 0}; const long long t_begin = clock64();)
         auto issue_pv = [&](int i) {
             const int s = i % TCA_VS;
-            mbar_wait(&v_full[s], (i / TCA_VS) & 1);
-            mbar_wait(&o_empty[i % C::NO], ((i / C::NO) & 1) ^ 1);   // the correction warps have read chunk i - NO
-            mbar_wait(&p_full[i % C::NSP], (i / C::NSP) & 1);
+            TCA_WAIT(&v_full[s], (i / TCA_VS) & 1, pw[2]);
+            TCA_WAIT(&o_empty[i % C::NO], ((i / C::NO) & 1) ^ 1, pw[3]);   // the correction warps have read chunk i - NO
+            TCA_WAIT(&p_full[i % C::NSP], (i / C::NSP) & 1, pw[4]);
             tc_fence_after();
             const uint64_t vdesc = umma_desc_mn128(kv_addr + (TCA_KS + s) * C::K_BYTES, 1024, C::SBO);
             const uint32_t d_addr = tmem_base + C::TO + (i % C::NO) * D;
@@ -368,8 +380,8 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         };
         auto issue_qk = [&](int j) {
             const int s = j % TCA_KS;
-            mbar_wait(&k_full[s], (j / TCA_KS) & 1);
-            if (C::TWO_ISSUERS) mbar_wait(&sp_free[j % C::NSP], ((j / C::NSP) & 1) ^ 1);   // P.V(j - NSP) has read the region S(j) goes into
+            TCA_WAIT(&k_full[s], (j / TCA_KS) & 1, pw[0]);
+            if (C::TWO_ISSUERS) TCA_WAIT(&sp_free[j % C::NSP], ((j / C::NSP) & 1) ^ 1, pw[1]);   // P.V(j - NSP) has read the region S(j) goes into
             tc_fence_after();
             const uint32_t k_addr = kv_addr + s * C::K_BYTES;
             const uint32_t s_addr = tmem_base + C::TS + (j % C::NSP) * C::SP;
@@ -403,6 +415,8 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 issue_pv(j);
             }
         }
+        TCA_PROBE(if (TCA_PROBE_ON) printf("mma warp %d: tiles %d total %lld | waits k_full %lld sp_free %lld v_full %lld o_empty %lld p_full %lld\n", warp, n_tiles,
+                                          clock64() - t_begin, pw[0], pw[1], pw[2], pw[3], pw[4]);)
     } else if (warp >= 18) {
         // ===== FP8 converters (warp 18: K tiles, warp 19: V tiles): raw [64 keys][D codes] -> fp16 tile in the layout the
         // 4-D TMA box of the bf16 path produces: [8-key group][d half][8 rows x 128 B], 16-byte chunks XOR-swizzled by row =====
@@ -469,8 +483,9 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         // state restarts: t_left counts the tiles left in the current chunk
         float2* mlp = reinterpret_cast<float2*>(a.ml_part) + ((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0;
         int t_left = tpc;
+        TCA_PROBE(long long pw[4] = {0, 0, 0, 0}; const long long t_begin = clock64();)
         for (int j = 0; j < n_tiles; ++j) {
-            mbar_wait(&s_full[j % C::NSP], (j / C::NSP) & 1);
+            TCA_WAIT(&s_full[j % C::NSP], (j / C::NSP) & 1, pw[0]);
             tc_fence_after();
             if (!warp_valid) {   // no live row in this warp (chain drafts: 16 of 128 rows): keep the barrier protocol only
                 tc_fence_before();
@@ -479,6 +494,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 continue;
             }
             uint32_t sv[32];
+            TCA_PROBE(const long long tA = clock64();)
             tmem_ld32(lane_addr + C::TS + (j % C::NSP) * C::SP + wg * 32, sv);
             tmem_ld_wait();
             const int kb = k_begin + j * TCA_BN + wg * 32;
@@ -495,7 +511,9 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             }
             float mx = fmaxf(mx0, mx1);
             xmax[((j & 1) * 2 + wg) * 128 + r] = mx;
+            TCA_PROBE(const long long tB = clock64(); pw[1] += tB - tA;)
             pair_bar_sync(1 + (warp & 3));
+            TCA_PROBE(const long long tC = clock64(); pw[2] += tC - tB;)
             mx = fmaxf(mx, xmax[((j & 1) * 2 + (wg ^ 1)) * 128 + r]);
             const float mn = fmaxf(m_run, mx);
             const float mu = (mn == -INFINITY) ? 0.f : mn;
@@ -524,6 +542,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(&p_full[j % C::NSP]);
+            TCA_PROBE(pw[3] += clock64() - tC;)
             if (--t_left == 0 || j == n_tiles - 1) {   // chunk finished (CTA-uniform)
                 xsum[wg * 128 + r] = l_run * exp2f(-TCA_PSCALE_LOG2);   // exact
                 pair_bar_sync(1 + (warp & 3));
@@ -533,6 +552,8 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 t_left = tpc;
             }
         }
+        TCA_PROBE(if ((warp == 2 || warp == 6) && TCA_PROBE_ON) printf("softmax warp %d: tiles %d total %lld | wait s_full %lld | ld + max %lld pair barrier %lld exp + split + st + arrive %lld\n",
+                                                                      warp, n_tiles, clock64() - t_begin, pw[0], pw[1], pw[2], pw[3]);)
     } else {
         // ===== correction: thread = (row, half of d).  O = O * c(i) + Oc(i), one rounded fp32 operation per tile;
         // c(i) was published by the softmax warps before they released P(i), which Oc(i) depends on. =====
@@ -549,8 +570,9 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         float* op = a.o_part + (((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0) * D + hh * C::DH;
         int t_left = tpc;
         const float oscale = FP8 ? mul_rn(exp2f(-TCA_PSCALE_LOG2), ta.v_scale) : exp2f(-TCA_PSCALE_LOG2);   // P's 2^15 out (exact); FP8: V's static scale in
+        TCA_PROBE(long long pw = 0; const long long t_begin = clock64();)
         for (int i = 0; i < n_tiles; ++i) {
-            mbar_wait(&o_full[i % C::NO], (i / C::NO) & 1);
+            TCA_WAIT(&o_full[i % C::NO], (i / C::NO) & 1, pw);
             tc_fence_after();
             if (!warp_valid) {   // no live row in this warp: release the chunk, nothing to add
                 tc_fence_before();
@@ -585,10 +607,12 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             }
             if (last) { op += D; t_left = tpc; }
         }
+        TCA_PROBE(if (warp == 10 && TCA_PROBE_ON) printf("correction warp 10: tiles %d total %lld | wait o_full %lld\n", n_tiles, clock64() - t_begin, pw);)
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<512>(tmem_base);
+    TCA_PROBE(if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n_tiles >= 48) atomicAdd(&tca_probe_count, 1);)
     trace_exit(ta.pf);
 }
 
