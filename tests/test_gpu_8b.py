@@ -343,3 +343,40 @@ def test_drafter_forward_at_8b_shape_matches_oracle():
         srt = np.sort(lg_ref[i])[::-1]
         if (srt[:4] - srt[1:5]).min() >= 1e-3:
             assert tk[i].tolist() == do.top_k_tokens(lg_ref[i], 4).tolist(), i
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("attn_chunk", [0, 256])
+def test_verify_is_repeatable_bit_for_bit_at_8b_shape(attn_chunk):
+    """No compute-sanitizer on this pool: a race in the warp-specialised kernels (the attention kernel's two MMA issuers and its
+    S/P hand-over, the GEMMs' pair epilogue) would show up as run-to-run differences.  The same verify step - two 8B-shaped
+    layers, ragged contexts spanning one to twelve key tiles per CTA, a 26-node tree - is run forty times without commit:
+    logits, final hidden states and accepted tokens must be identical bit for bit (attention chunking: the library default
+    and 256-key chunks = 4 tiles per CTA, many CTAs per sequence)."""
+    import dataclasses
+    import paper_2606_18502_b200 as ev
+    from gpu_helpers import run_verify
+    spec = wl.CONFIGS[2]
+    shape = dataclasses.replace(spec.model, name="llama8b_2layers", n_layers=2)
+    ctx = [37, 64, 700, 1543, 3001]
+    B, T = len(ctx), spec.n_nodes
+    parents = wl.tree_parents(T, spec.tree_caps)
+    model = ev.Model(shape, max_batch=B, max_tree_nodes=64, max_ctx=max(ctx) + 128, page_size=spec.page_size, attn_chunk=attn_chunk)
+    for kind, layer in [("embed", 0)] + [(k, l) for l in range(shape.n_layers) for k in LAYER_KINDS] + [("lm_head", 0)]:
+        model.ev_model_set_weight(kind, layer, wl.weight_matrix_bf16(shape, spec.seed, kind, layer, device="cuda"))
+    cache = ev.Cache(model, sum(c // spec.page_size + 8 for c in ctx), B)
+    slots = [cache.ev_cache_add_seq(c + 64) for c in ctx]
+    cache.ev_cache_prefill(slots, [wl.context_ids(spec, b, ctx[b]) for b in range(B)])
+    rng = np.random.default_rng(5)
+    tokens = rng.integers(0, shape.vocab, size=(B, T)).astype(np.int32)
+    ref = None
+    for it in range(40):
+        buf = run_verify(model, cache, slots, tokens, np.tile(parents, (B, 1)), commit=False, want_logits=True, want_hidden=True)
+        assert (buf.status.cpu().numpy() == 0).all()
+        cur = (buf.logits.view(torch.int32).clone(), buf.hidden.view(torch.int32).clone(), buf.out_tokens.clone(), buf.accept_len.clone())
+        if ref is None:
+            ref = cur
+            assert torch.isfinite(buf.logits).all()
+        else:
+            for a, b in zip(ref, cur):
+                assert torch.equal(a, b), it
