@@ -295,7 +295,13 @@ int alloc_qmat(ev_model* m, QMat* q, long N, long K) {
 // Every kernel of the step is launched with the programmatic-stream-serialization attribute (PDL): it may
 // become resident while its predecessor is still running, and executes griddepcontrol.wait before touching
 // anything the predecessor wrote.  Under stream capture these launches become programmatic graph edges.
+// ONE launch per step goes without it: the kernel right after tree_prep_kernel (serial_next_launch()).  It then starts only
+// when tree_prep_kernel has completed, and since a PDL kernel can become resident only after every CTA of its predecessor has
+// started, no later kernel of the step runs a single instruction before that either: the per-step metadata tree_prep_kernel
+// writes (Lsnap, nn_eff, order, erow, ...) may be read ahead of griddepcontrol.wait (tree_attn_tc_kernel does).
 bool g_use_pdl = true;
+thread_local bool g_serial_next = false;
+void serial_next_launch() { g_serial_next = true; }
 template <class... KArgs, class... Args>
 int launch_kc(int cluster, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t cfg;
@@ -306,7 +312,9 @@ int launch_kc(int cluster, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t
     cfg.stream = st;
     cudaLaunchAttribute at[2];
     int na = 0;
-    if (g_use_pdl) {
+    const bool serial = g_serial_next;
+    g_serial_next = false;
+    if (g_use_pdl && !serial) {
         at[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         at[na].val.programmaticStreamSerializationAllowed = 1;
         ++na;
@@ -639,11 +647,13 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         // draft model (ev_drafter.cuh): layer-0 input = FC(Q8([embed(token) ; predecessor feature]))
         QuantOut q;
         q.codes = m->fq.codes; q.sx = m->fq.scale; q.static_scale = nullptr; q.site_amax = nullptr; q.clip_count = nullptr;
+        serial_next_launch();
         EV_TRY(launch_k(concat_quant_kernel, dim3(M), dim3(EW_THREADS), 0, st, in->dev_tokens, cfg.vocab, m->embed, in->dev_features, H, q));
         LinOut fl;
         EV_TRY(run_linear(m, st, m->fc, m->fq, M, EPI_RAW, &fl, nullptr, nullptr, PC_OTHER));
         EV_TRY(launch_k(materialize_linear_kernel, dim3(M), dim3(256), 0, st, m->h, H, fl));
     } else {
+        serial_next_launch();
         EV_TRY(launch_k(embed_gather_kernel, dim3(M), dim3(EW_THREADS), 0, st, in->dev_tokens, cfg.vocab, m->embed, H, m->h));
     }
     if (out->dev_hidden) EV_TRY(copy_f32(st, m->h, out->dev_hidden, (long)M * H));

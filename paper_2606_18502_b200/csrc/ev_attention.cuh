@@ -372,27 +372,24 @@ template <int MERGE_NV4>
 __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(MergeArgs a) {
     pdl_launch_dependents();  // the O-projection GEMM may start prefetching its weights now
     l2_prefetch_issue(a.pf);
-    pdl_wait();
-    trace_past_wait(a.pf);
+    // The row's key plan (tree_prep_kernel's output, complete before any kernel of the step starts: ev_api.cu
+    // serial_next_launch) and the page lookups of its tail keys come BEFORE griddepcontrol.wait: three dependent L2 round
+    // trips that used to sit between the wait and the first K/V load.  __ldcg: no stale L1 line of the previous step.
     __shared__ float red[MERGE_THREADS / 32];
     __shared__ float xch_f[CLUSTER_MAX];
     __shared__ long long tbase[ATT_TAIL_MAX];   // element offset of the tail key's K row (kv head 0, dim 0) in this layer's pool
     const int m = blockIdx.x / cluster_nctarank();   // one token row per cluster
     const int b = m / a.T, node = m % a.T;
-    const int nn = a.nn_eff[b];
+    const int nn = __ldcg(a.nn_eff + b);
     const int K = a.Hq * a.D, S = a.n_chunks, D = a.D;
     const bool valid = node < nn;
-    const int L = a.Lsnap[b];
-    const int e = valid ? a.erow[m] : 0;
-    const int ns = valid ? (a.kend_row[m] + a.chunk - 1) / a.chunk : 0;
+    const int L = __ldcg(a.Lsnap + b);
+    const int e = valid ? __ldcg(a.erow + m) : 0;
+    const int ns = valid ? (__ldcg(a.kend_row + m) + a.chunk - 1) / a.chunk : 0;
     // tail keys, in position order: n_ctx cached slots e .. L-1, then the ancestors of the tail (lowest node index = lowest depth first)
     const int n_ctx = valid ? min(max(0, L - e), ATT_TAIL_MAX) : 0;
-    const unsigned long long anc_tail = valid ? (a.anc[m] & ~a.anc_bulk[m]) : 0ull;
-#ifdef EXP_NOTAIL
-    const int nt = 0;
-#else
+    const unsigned long long anc_tail = valid ? (__ldcg(a.anc + m) & ~__ldcg(a.anc_bulk + m)) : 0ull;
     const int nt = min(n_ctx + __popcll(anc_tail), ATT_TAIL_MAX);
-#endif
     const size_t kv_stride = (size_t)a.Hkv * a.page_size * D;   // K block -> V block of a page
     if ((int)threadIdx.x < nt) {
         const int u = threadIdx.x;
@@ -402,10 +399,12 @@ __global__ void __launch_bounds__(MERGE_THREADS, 2) attn_merge_quant_kernel(Merg
             for (int i = n_ctx; i < u; ++i) at &= at - 1;
             sl = L + __ffsll((long long)at) - 1;
         }
-        const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+        const int32_t* pt = a.page_table + (size_t)__ldcg(a.seq_slots + b) * a.max_pages;
         tbase[u] = (long long)((size_t)pt[sl / a.page_size] * 2 * kv_stride + (size_t)(sl % a.page_size) * D);
     }
     __syncthreads();
+    pdl_wait();
+    trace_past_wait(a.pf);
     const int G = a.Hq / a.Hkv;
     const int gl = D / 4;   // lanes per head group (32 or 16)
     float4 v[MERGE_NV4];
@@ -515,21 +514,20 @@ template <int G>
 __global__ void __launch_bounds__(256, 2) attn_merge_rowkv_kernel(MergeArgs a) {
     pdl_launch_dependents();
     l2_prefetch_issue(a.pf);
-    pdl_wait();
-    trace_past_wait(a.pf);
     constexpr int D = 128;
     __shared__ float red[8];
     __shared__ long long tbase[ATT_TAIL_MAX];
+    // key plan and page lookups before griddepcontrol.wait (see attn_merge_quant_kernel)
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
-    const int nn = a.nn_eff[b];
+    const int nn = __ldcg(a.nn_eff + b);
     const int K = a.Hq * D, S = a.n_chunks;
     const bool valid = node < nn;
-    const int L = a.Lsnap[b];
-    const int e = valid ? a.erow[m] : 0;
-    const int ns = valid ? (a.kend_row[m] + a.chunk - 1) / a.chunk : 0;
+    const int L = __ldcg(a.Lsnap + b);
+    const int e = valid ? __ldcg(a.erow + m) : 0;
+    const int ns = valid ? (__ldcg(a.kend_row + m) + a.chunk - 1) / a.chunk : 0;
     const int n_ctx = valid ? min(max(0, L - e), ATT_TAIL_MAX) : 0;
-    const unsigned long long anc_tail = valid ? (a.anc[m] & ~a.anc_bulk[m]) : 0ull;
+    const unsigned long long anc_tail = valid ? (__ldcg(a.anc + m) & ~__ldcg(a.anc_bulk + m)) : 0ull;
     const int nt = min(n_ctx + __popcll(anc_tail), ATT_TAIL_MAX);
     const size_t kv_stride = (size_t)a.Hkv * a.page_size * D;
     if ((int)threadIdx.x < nt) {
@@ -540,10 +538,12 @@ __global__ void __launch_bounds__(256, 2) attn_merge_rowkv_kernel(MergeArgs a) {
             for (int i = n_ctx; i < u; ++i) at &= at - 1;
             sl = L + __ffsll((long long)at) - 1;
         }
-        const int32_t* pt = a.page_table + (size_t)a.seq_slots[b] * a.max_pages;
+        const int32_t* pt = a.page_table + (size_t)__ldcg(a.seq_slots + b) * a.max_pages;
         tbase[u] = (long long)((size_t)pt[sl / a.page_size] * 2 * kv_stride + (size_t)(sl % a.page_size) * D);
     }
     __syncthreads();
+    pdl_wait();
+    trace_past_wait(a.pf);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int kvh = warp;                 // blockDim = 32 * Hkv
     const int d = lane * 4;

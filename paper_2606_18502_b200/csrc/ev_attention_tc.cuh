@@ -238,13 +238,19 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     __syncthreads();       // barriers and the TMEM base are visible to every warp (still before the wait)
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
-    pdl_wait();
-    trace_past_wait(ta.pf);
-    const int b = a.order ? a.order[blockIdx.z] : (int)blockIdx.z;
-    const int nn = a.nn_eff[b];
-    const int L = a.Lsnap[b];
-    const int seq_slot = a.seq_slots[b];
-    const int n_keys = a.kend_seq[b];                  // one past the last bulk key slot of the sequence (tree_prep_kernel)
+    // What tree_prep_kernel wrote at the head of the step is read BEFORE griddepcontrol.wait: the kernel launched right after
+    // tree_prep_kernel carries no programmatic-serialization attribute (ev_api.cu), so no later kernel of the step can be
+    // resident before tree_prep_kernel has completed; __ldcg: an L1 line left over from the previous step must not serve.
+    // The wait itself guards what the PRECEDING kernel (RoPE + K/V write) produced: Q, and the K/V of the tree's own slots.
+    const int b = a.order ? __ldcg(a.order + blockIdx.z) : (int)blockIdx.z;
+    const int nn = __ldcg(a.nn_eff + b);
+    const int L = __ldcg(a.Lsnap + b);
+    const int seq_slot = __ldcg(a.seq_slots + b);
+    const int n_keys = __ldcg(a.kend_seq + b);         // one past the last bulk key slot of the sequence (tree_prep_kernel)
+    if (warp != 0) {
+        pdl_wait();
+        trace_past_wait(ta.pf, 32);
+    }
     // This CTA walks a.cpg consecutive chunks; chunks sit at absolute key positions and each is reduced from a fresh
     // softmax state (batch-invariant, ev_attention.cuh), so how many chunks a CTA takes changes no result: the K/V
     // stream and the MMAs simply run on across chunk boundaries, the softmax / correction warps restart their state.
@@ -309,6 +315,9 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         // tile for K.  The lane that owns page 0 arms the tile's full barrier (arrive + expected bytes); a box of
         // another lane may complete first - the phase still cannot complete before that arrive.
         const int dst_off = pg * C::PAGE_BYTES;
+        // tiles that lie entirely in the committed context [0, L) were written by earlier steps: their loads start before
+        // griddepcontrol.wait, under the tail of the RoPE kernel (at batch 1 the first K/V tile used to arrive ~4 us after the wait)
+        const int n_old = min(n_tiles, max(0, L - k_begin) / TCA_BN);
         if (FP8) {
             // raw E4M3 page blocks: one linear 16-token x D-byte copy per (K|V, page) into the raw ring; lanes 0..3 stream K, 4..7 V
             if (lane < OPS) {
@@ -317,6 +326,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 uint8_t* ring = raw_s + kv * C::RS * C::RAW_BYTES;
                 int row_next = box_row(0);
                 for (int j = 0; j < n_tiles; ++j) {
+                    if (j == n_old) pdl_wait();
                     const int row_cur = row_next;
                     if (j + 1 < n_tiles) row_next = box_row(j + 1);
                     const int sl = j % C::RS;
@@ -332,6 +342,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             uint8_t* ring = kv_s + (kv ? TCA_KS * C::K_BYTES : 0);
             int row_next = box_row(0);
             for (int j = 0; j < n_tiles; ++j) {
+                if (j == n_old) pdl_wait();
                 const int row_cur = row_next;
                 if (j + 1 < n_tiles) row_next = box_row(j + 1);
                 const int sl = j % depth;

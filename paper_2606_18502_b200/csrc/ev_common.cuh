@@ -258,14 +258,14 @@ struct L2Prefetch {
     unsigned long long* trace;  // null, or this launch's TRACE_SLOTS step-trace slots (ev_profile_trace): min over CTAs of
                                 // t_enter, t_past_wait, ~t_exit, ~t_past_wait (globaltimer ns; memset 0xFF = empty)
 };
-__device__ __forceinline__ void trace_mark(const L2Prefetch& pf, int slot, bool complement) {
-    if (pf.trace && threadIdx.x == 0) {
+__device__ __forceinline__ void trace_mark(const L2Prefetch& pf, int slot, bool complement, unsigned tid = 0) {
+    if (pf.trace && threadIdx.x == tid) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         atomicMin(pf.trace + slot, complement ? ~t : t);
     }
 }
-__device__ __forceinline__ void trace_past_wait(const L2Prefetch& pf) { trace_mark(pf, 1, false); trace_mark(pf, 3, true); }
+__device__ __forceinline__ void trace_past_wait(const L2Prefetch& pf, unsigned tid = 0) { trace_mark(pf, 1, false, tid); trace_mark(pf, 3, true, tid); }
 __device__ __forceinline__ void trace_exit(const L2Prefetch& pf) { trace_mark(pf, 2, true); }
 // bring-up: phase k (0..3) reached by the LAST CTA (slots 4..7 hold ~t)
 __device__ __forceinline__ void trace_phase(const L2Prefetch& pf, int k) { trace_mark(pf, 4 + k, true); }

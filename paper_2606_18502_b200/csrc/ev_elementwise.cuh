@@ -501,24 +501,26 @@ template <int MAXS>
 __global__ void __launch_bounds__(ROPE_THREADS) rope_kvwrite_kernel(RopeArgs a) {
     pdl_launch_dependents();
     l2_prefetch_issue(a.pf);
-    pdl_wait();
-    trace_past_wait(a.pf);
+    // position, destination page (tree_prep_kernel's output and the page table: complete before any kernel of the step starts,
+    // ev_api.cu serial_next_launch) before griddepcontrol.wait; the wait guards the QKV GEMM's slabs and the activation scales
     const int m = blockIdx.x;
     const int b = m / a.T, node = m % a.T;
     const int D = a.D, D2 = D / 2;
-    const float sxm = __ldg(a.lin.sx + m);
     float* __restrict__ row = a.qkv_out + (size_t)m * a.ld;
-    const float2* cs = a.cs + (size_t)a.pos[m] * D2;
-    const bool write = node < a.nn_eff[b];
+    const float2* cs = a.cs + (size_t)__ldcg(a.pos + m) * D2;
+    const bool write = node < __ldcg(a.nn_eff + b);
     __nv_bfloat16* kdst = nullptr;
     __nv_bfloat16* vdst = nullptr;
     if (write) {
-        const int slot_tok = a.Lsnap[b] + node;
-        const int page = a.page_table[(size_t)a.seq_slots[b] * a.max_pages + slot_tok / a.page_size];
+        const int slot_tok = __ldcg(a.Lsnap + b) + node;
+        const int page = a.page_table[(size_t)__ldcg(a.seq_slots + b) * a.max_pages + slot_tok / a.page_size];
         const size_t base = (size_t)page * 2 * a.Hkv * a.page_size * D + (size_t)(slot_tok % a.page_size) * D;
         kdst = a.pool + base;
         vdst = a.pool + base + (size_t)a.Hkv * a.page_size * D;
     }
+    pdl_wait();
+    trace_past_wait(a.pf);
+    const float sxm = __ldg(a.lin.sx + m);
     const int n_rot4 = (a.Hq + a.Hkv) * D2 / 4;  // groups of 4 rotation pairs
     const int tid = blockIdx.y * blockDim.x + threadIdx.x, nthr = gridDim.y * blockDim.x;  // a row may be spread over gridDim.y CTAs
     for (int i = tid; i < n_rot4; i += nthr) {
