@@ -313,6 +313,21 @@ int ev_engine_destroy(ev_engine*);
 /* y[M][N] = (codes_x . W_kind^T) * s_x[m] * s_w[n] with the product GEMM kernel. */
 int ev_op_linear(ev_model*, int kind, int layer, const uint8_t* dev_codes_x, const float* dev_sx,
                  int M, float* dev_out, void* stream);
+/* ev_op_linear for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc).  Same GEMM kernel, same canonical K cuts, same result bit for bit; kinds Q (= fused QKV),
+ * O, GATE (= fused gate|up), DOWN.  The kernel's scratch - the fp32 K-piece slabs [pieces][M][N] its consumer sums - lives in a
+ * file-scope `static __device__` array of EV_STATIC_SCRATCH_BYTES (16 MiB, resident on every GPU that loads the library until
+ * the process exits) instead of the model's workspace; its device address is resolved with cudaGetSymbolAddress once per
+ * device at ev_model_create.  The call performs no cudaMalloc / cudaFree / allocating library call.
+ *   dev_codes_x [M][K] E4M3 codes, dev_sx [M] fp32 scales, dev_out [M][N] fp32: device pointers, caller-owned.
+ *   Limit: (M <= 256 ? 8 : 1) * M * N * 4 bytes <= EV_STATIC_SCRATCH_BYTES (the worst-case slab layout), else EV_ECAPACITY
+ *   (ev_last_error names both numbers) - e.g. M <= 60 for every layer GEMM of the 8B shape except gate|up (M <= 18).
+ *   The array is shared by every call from every model and thread and keeps the last call's contents; nothing has to start
+ *   at zero (each launch writes every slab element its consumer reads).  Two calls that overlap on the GPU (different
+ *   streams, or concurrent host threads) RACE on it: serialise them.  ev_verify and ev_op_linear never touch it. */
+#define EV_STATIC_SCRATCH_BYTES (16 << 20)
+int ev_op_linear_static(ev_model*, int kind, int layer, const uint8_t* dev_codes_x, const float* dev_sx,
+                        int M, float* dev_out, void* stream);
 /* per-token dynamic (or static, scale > 0) E4M3 quantization of fp32 rows */
 int ev_op_quantize_rows(ev_model*, const float* dev_x, int M, int K, float static_scale,
                         uint8_t* dev_codes, float* dev_sx, void* stream);

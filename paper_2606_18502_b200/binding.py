@@ -85,6 +85,7 @@ SIGNATURES = {
     "ev_profile_read": (C.c_int, [_P, _P, _P, C.c_int]),
     "ev_profile_trace": (C.c_int, [_P, _P, C.c_int, _P]),
     "ev_op_linear": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
+    "ev_op_linear_static": (C.c_int, [_P, C.c_int, C.c_int, _P, _P, C.c_int, _P, _P]),
     "ev_op_quantize_rows": (C.c_int, [_P, _P, C.c_int, C.c_int, C.c_float, _P, _P, _P]),
     "ev_last_error": (C.c_char_p, []),
     "ev_model_share_head": (C.c_int, [_P, _P]),
@@ -225,6 +226,11 @@ class Model:
         out = torch.empty((M, n_out), dtype=torch.float32, device="cuda")
         _check(self.lib.ev_op_linear(self.h, EV_W[kind], layer, _ptr(codes_x.contiguous()), _ptr(sx.contiguous()), M,
                                      _ptr(out), _stream()))
+        return out
+
+    def ev_op_linear_static(self, kind, layer, codes_x, sx, out):
+        """no-allocation variant: the caller passes the output tensor [M, N] too (include/eagle_verify.h)"""
+        _check(self.lib.ev_op_linear_static(self.h, EV_W[kind], layer, _ptr(codes_x), _ptr(sx), codes_x.shape[0], _ptr(out), _stream()))
         return out
 
     def ev_op_quantize_rows(self, x, static_scale=0.0):

@@ -853,6 +853,32 @@ int check_ready(ev_model* m, bool need_lm) {
 }  // namespace
 
 // ================================================================================================
+// ---- static scratch for callers that may not allocate (ev_op_linear_static, include/eagle_verify.h) ----------------
+// The K-piece slabs of gemm_e4m3_kernel (its scratch: raw fp32 accumulators [pieces][M][N] that the consumer sums) in a
+// file-scope device array instead of the model's cudaMalloc'ed workspace.  16 MiB of device memory on every GPU that loads
+// the library, held until the process exits.  In host code the NAME `ev_static_slabs` is a host-side stand-in, not a device
+// address (a kernel given it faults, or on a GPU that can reach host memory silently uses the wrong memory): host code
+// asks cudaGetSymbolAddress for the address, once per device with that device current, and passes THAT to the kernel.
+constexpr long EV_STATIC_SLAB_FLOATS = 4L << 20;   // 4 Mi floats = 16 MiB
+static __device__ __align__(256) float ev_static_slabs[EV_STATIC_SLAB_FLOATS];
+namespace {
+// device address of ev_static_slabs on the CURRENT device (resolved on first use per device; ev_model_create does it at set-up)
+int static_slabs_ptr(float** out) {
+    static float* ptrs[64] = {};
+    int dev = 0;
+    CUDA_TRY(cudaGetDevice(&dev));
+    float*& p = ptrs[dev & 63];
+    if (!p) {
+        void* q = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&q, ev_static_slabs);
+        if (e != cudaSuccess || !q) return fail(EV_ECUDA, std::string("cudaGetSymbolAddress(ev_static_slabs): ") + cudaGetErrorString(e));
+        p = static_cast<float*>(q);
+    }
+    *out = p;
+    return EV_OK;
+}
+}  // namespace
+
 extern "C" {
 
 const char* ev_last_error(void) { return g_err.c_str(); }
@@ -901,6 +927,7 @@ int ev_model_create(const ev_config* cfg, ev_model** out) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&m->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    { float* sp = nullptr; if (static_slabs_ptr(&sp) != EV_OK) { delete m; return EV_ECUDA; } }   // set-up of ev_op_linear_static's scratch address on this device
 #ifdef EV_BRINGUP   // bring-up builds only (-DEV_BRINGUP): the shipped library reads no environment variable
     if (getenv("EV_L2PF_MAX_M")) m->l2pf_max_m = atoi(getenv("EV_L2PF_MAX_M"));      // 0 = off
     if (getenv("EV_L2PF_MASK")) m->l2pf_mask = (unsigned)strtoul(getenv("EV_L2PF_MASK"), nullptr, 0);
@@ -1669,6 +1696,47 @@ int ev_op_linear(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, c
     }
     LinOut lin;
     EV_TRY(run_linear(m, st, *w, *x, M, EPI_RAW, &lin, nullptr, nullptr, PC_OTHER));
+    materialize_linear_kernel<<<M, 256, 0, st>>>(dev_out, (int)w->N, lin);
+    LAUNCH_CHECK();
+    return EV_OK;
+}
+
+// ev_op_linear for callers that may not allocate: the same GEMM kernel, same K cuts, same consumer - the kernel's scratch
+// (K-piece slabs) lives in the file-scope device array ev_static_slabs instead of the model's workspace.  No cudaMalloc /
+// cudaFree / allocating library call on this path (the address was resolved at set-up).
+int ev_op_linear_static(ev_model* m, int kind, int layer, const uint8_t* dev_codes_x, const float* dev_sx, int M, float* dev_out,
+                        void* stream) {
+    if (!m || !dev_codes_x || !dev_sx || !dev_out || M < 1) return fail(EV_EINVAL, "bad argument");
+    if (M > m->M_cap) return fail(EV_ECAPACITY, "M exceeds max_batch * max_tree_nodes");
+    cudaStream_t st = (cudaStream_t)stream;
+    QMat* w = nullptr;
+    ActBuf* x = nullptr;
+    if (layer < 0 || layer >= m->cfg.n_layers) return fail(EV_EINVAL, "layer out of range");
+    switch (kind) {
+        case EV_W_Q: w = &m->layers[layer].qkv; x = &m->xq; break;
+        case EV_W_O: w = &m->layers[layer].o; x = &m->aq; break;
+        case EV_W_GATE: w = &m->layers[layer].gu; x = &m->xq; break;
+        case EV_W_DOWN: w = &m->layers[layer].down; x = &m->tq; break;
+        default: return fail(EV_EINVAL, "ev_op_linear_static: kind must be Q (=fused QKV), O, GATE (=fused gate|up) or DOWN");
+    }
+    // worst case of the slab layout: 8 pieces per tile below 257 rows, one slab above (run_linear)
+    const long need = (M <= 256 ? 8L : 1L) * M * (long)w->N;
+    if (need > EV_STATIC_SLAB_FLOATS)
+        return fail(EV_ECAPACITY, "ev_op_linear_static: (M <= 256 ? 8 : 1) * M * N = " + std::to_string(need) + " floats exceeds the static scratch of " +
+                                      std::to_string(EV_STATIC_SLAB_FLOATS) + " floats (16 MiB); use ev_op_linear");
+    float* slabs = nullptr;
+    EV_TRY(static_slabs_ptr(&slabs));
+    CUDA_TRY(cudaMemcpyAsync(x->codes, dev_codes_x, (size_t)M * w->K, cudaMemcpyDeviceToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(x->scale, dev_sx, (size_t)M * 4, cudaMemcpyDeviceToDevice, st));
+    // the GEMM takes its slab pointer from the model: point it at the static array for this one launch.  Every slab element the
+    // consumer reads is written by this launch's GEMM (pieces cover their tiles completely), so nothing has to start at zero.
+    float* const saved_out = m->lin_out;
+    const long saved_floats = m->lin_floats;
+    m->lin_out = slabs; m->lin_floats = EV_STATIC_SLAB_FLOATS;
+    LinOut lin;
+    const int rc = run_linear(m, st, *w, *x, M, EPI_RAW, &lin, nullptr, nullptr, PC_OTHER);
+    m->lin_out = saved_out; m->lin_floats = saved_floats;
+    if (rc != EV_OK) return rc;
     materialize_linear_kernel<<<M, 256, 0, st>>>(dev_out, (int)w->N, lin);
     LAUNCH_CHECK();
     return EV_OK;
