@@ -308,6 +308,7 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
     # passes griddepcontrol.wait and when its last CTA leaves); the CUDA-event class times above come from an eager pass
     # whose launches are CPU-paced
     ingraph = None
+    layer_timeline = None
     try:
         model.ev_profile_enable(2)
         step(); step()
@@ -326,6 +327,30 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
                 ingraph[names[i % 10]] = ingraph.get(names[i % 10], 0.0) + ex[i]
             ingraph["gemm_lm_head"] = ex[10 * nl + 1]
             ingraph["step_us"] = (tr[10 * nl + 1, 2] - tr[0, 0]) / 1e3
+            # the ten kernels of a layer against their predecessor's last exit, averaged over the inner layers: when the first CTA
+            # enters (how early programmatic dependent launch makes it resident), when the first / the last CTA passes
+            # griddepcontrol.wait (a late last CTA = it could not be co-resident with the predecessor), when the last CTA leaves
+            lo, hi = (2, nl - 2) if nl > 6 else (1, nl)
+            tl = np.zeros((10, 4))
+            for l in range(lo, hi):
+                for k in range(10):
+                    r, prev = tr[10 * l + k], tr[10 * l + k - 1][2]
+                    tl[k] += [r[0] - prev, r[1] - prev, r[3] - prev, r[2] - prev]
+            tl /= max(hi - lo, 1) * 1e3
+            ph = np.zeros((10, 4))      # phase marks (only a bring-up build of the library records them: -DEV_GEMM_PROBE)
+            for l in range(lo, hi):
+                for k in range(10):
+                    ph[k] += tr[10 * l + k][4:8] - tr[10 * l + k - 1][2]
+            ph /= max(hi - lo, 1) * 1e3
+            layer_timeline = {"kernels": ["rmsnorm1_quant", "gemm_qkv", "rope_kvwrite", "tree_attention", "attn_merge_quant", "gemm_o",
+                                          "rmsnorm2_quant", "gemm_gateup", "swiglu_quant", "gemm_down"],
+                              "us_after_predecessor_exit": {key: [round(float(v), 2) if abs(v) < 1e6 else None for v in tl[:, col]]   # None: the kernel does not record that mark
+                                                            for col, key in enumerate(("first_cta_enters", "first_cta_past_wait", "last_cta_past_wait", "last_cta_exits"))},
+                              "layer_us": round(float(tl[:, 3].sum()), 2), "layers_averaged": [lo, hi]}
+            if (np.abs(ph) < 1e6).any():
+                layer_timeline["gemm_phase_marks_last_cta"] = {
+                    "def": "activations requested, first stage complete, first accumulator complete, epilogue holds it (us after the predecessor's last exit)",
+                    **{layer_timeline["kernels"][k]: [round(float(v), 2) for v in ph[k]] for k in range(10) if (np.abs(ph[k]) < 1e6).all()}}
     except Exception as e:  # pragma: no cover
         log(f"step trace unavailable: {e}")
     model.ev_profile_enable(0)
@@ -365,6 +390,7 @@ def measure(spec, args, torch, ev, dist, rank, world, local_rank, log, warmup, s
                                 "gemm_gbs": round(work["weight_bytes"] / (g_us * 1e-6) / 1e9, 1),
                                 "gemm_frac_of_hbm": round(work["weight_bytes"] / (g_us * 1e-6) / 1e9 / pk["hbm_gbs"], 4),
                                 "gemm_tflops": round(lin_flops / (g_us * 1e-6) / 1e12, 1),
+                                "layer_timeline": layer_timeline,
                                 "def": "per-kernel durations inside the CUDA-graph replay (step trace: first CTA past griddepcontrol.wait -> last CTA exit, "
                                        "%globaltimer), summed per class over one step; the event-timed `achieved` above is from an eager, CPU-paced pass"}
     roofline.update({"launches_per_step": gemm_n // steps, "avg_launch_us": round(1e3 * gemm_ms / gemm_n, 2), "traffic": traffic,

@@ -318,6 +318,9 @@ __global__ void __launch_bounds__((gemm_threads<EPI, PAIR>()), 1) gemm_e4m3_kern
                 tma_load_2d_hint(st + GEMM_WTILE, tm, bar, kb_abs * GEMM_BK, item.m0 + rank * rows, pol_x);
             };
             for (int i = 0; i < pre; ++i) ld_x(smem + i * stage_bytes, &full_bar[i], it0.kb0 + i, it0);
+#ifdef EV_GEMM_PROBE   // bring-up (-DEV_GEMM_PROBE): phase marks of the step trace (profiles/r2_step_timeline.md), last CTA each
+            trace_phase_any(a.pf, 0);   // activations of the prefilled stages requested
+#endif
             int s = pre;
             uint32_t ph = 0;
             if (s == a.stages) { s = 0; ph ^= 1; }
@@ -374,6 +377,10 @@ __global__ void __launch_bounds__((gemm_threads<EPI, PAIR>()), 1) gemm_e4m3_kern
                             mbar_wait(&full_bar[s], ph);
                             if (PAIR) mbar_wait(&peer_full_bar[s], ph);
                             tc_fence_after();
+#ifdef EV_GEMM_PROBE
+                            if (leader && n_acc == 0 && kb == kb0) trace_phase_any(a.pf, 1);          // first stage complete
+                            if (leader && n_acc == 0 && kb == kb_end - 1) trace_phase_any(a.pf, 2);   // last stage of the first accumulator complete
+#endif
                             const uint32_t wa = smem_base + (uint32_t)(s * stage_bytes);
                             const uint64_t adesc = umma_desc_k128(wa);
                             const uint64_t bdesc = umma_desc_k128(wa + GEMM_WTILE);
@@ -475,6 +482,9 @@ __global__ void __launch_bounds__((gemm_threads<EPI, PAIR>()), 1) gemm_e4m3_kern
             }
             mbar_wait(&tmem_full_bar[buf], (n_it >> 1) & 1);
             tc_fence_after();
+#ifdef EV_GEMM_PROBE
+            if (et == 0 && n_it == 0) trace_phase_any(a.pf, 3);   // the epilogue holds the first accumulator
+#endif
             const uint32_t t_addr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(buf * a.tok);
             float* outp = a.out + (size_t)it.split * a.M * a.ldo;
             for (int g = 0; g < n_groups; ++g) {
