@@ -65,7 +65,12 @@ struct TcaCfg {
     static constexpr int PAGE_BYTES = 2 * SBO;          // one 16-token (page, K|V, head) block
     static constexpr int BAR_BYTES = 512;
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
-    static constexpr int SMEM = 1024 + (KS + VS) * K_BYTES + 2 * RS * RAW_BYTES + BAR_BYTES + XCH_BYTES;   // Q lives in TMEM
+    // a chunk's partial output leaves through shared memory: a correction thread holds one ROW (TMEM lane), so its own stores hit
+    // 32 different lines per instruction (5,000 cycles per chunk at batch 1: profiles/r2_attention_issue.md section 5); staged
+    // OPW columns at a time in a [32 rows][OPW + 1] tile per warp, a store instruction writes whole rows
+    static constexpr int OPW = FP8 ? 16 : 32;
+    static constexpr int OST_BYTES = 8 * 32 * (OPW + 1) * 4;
+    static constexpr int SMEM = 1024 + (KS + VS) * K_BYTES + 2 * RS * RAW_BYTES + BAR_BYTES + XCH_BYTES + OST_BYTES;   // Q lives in TMEM
     // TMEM columns
     // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
     // pairs) written over it once both halves of the row have read S(j) (the pair barrier orders that).  (Three
@@ -185,10 +190,13 @@ __device__ __forceinline__ void e4m3x16_to_f16(const uint4& in, uint4& lo, uint4
 __device__ int tca_probe_count = 0;
 #define TCA_WAIT(bar, ph, acc) do { const long long t0_ = clock64(); mbar_wait(bar, ph); acc += clock64() - t0_; } while (0)
 #define TCA_PROBE(...) __VA_ARGS__
+__device__ int tca_tl_count = 0;
+#define TCA_TL(id) do { if (lane == 0) tca_tl[id] = clock64() - t_kernel0; } while (0)
 #define TCA_PROBE_ON (lane == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n_tiles >= 48 && tca_probe_count < 4)
 #else
 #define TCA_WAIT(bar, ph, acc) mbar_wait(bar, ph)
 #define TCA_PROBE(...)
+#define TCA_TL(id)
 #endif
 template <int D, bool FP8>
 __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
@@ -215,7 +223,9 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
     float* xsum = xmax + 2 * 2 * 128;                     // [2 wg][128]
     float* xc = xsum + 2 * 128;                           // [8 tiles][128] rescale factor of tile j at [j & 7]
+    float* ostage = xc + 8 * 128;                         // [8 correction warps][32 rows][OPW + 1] staging of a chunk's partial output
 
+    TCA_PROBE(const long long t_kernel0 = clock64(); __shared__ long long tca_tl[24];)
     const int split = blockIdx.x;
     const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -247,10 +257,12 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     const int L = __ldcg(a.Lsnap + b);
     const int seq_slot = __ldcg(a.seq_slots + b);
     const int n_keys = __ldcg(a.kend_seq + b);         // one past the last bulk key slot of the sequence (tree_prep_kernel)
+    if (warp == 2) TCA_TL(0);     // prologue done (barriers, TMEM, plan): at the wait
     if (warp != 0) {
         pdl_wait();
         trace_past_wait(ta.pf, 32);
     }
+    if (warp == 2) TCA_TL(1);     // past the wait
     // This CTA walks a.cpg consecutive chunks; chunks sit at absolute key positions and each is reduced from a fresh
     // softmax state (batch-invariant, ev_attention.cuh), so how many chunks a CTA takes changes no result: the K/V
     // stream and the MMAs simply run on across chunk boundaries, the softmax / correction warps restart their state.
@@ -290,8 +302,10 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         tc_fence_before();
     }
     if (warp != 0 && warp < 18) {
+        if (warp == 2) TCA_TL(2);     // this warp's part of Q is in TMEM
         asm volatile("bar.sync 5, %0;" ::"n"(TCA_THREADS - 32) : "memory");
         tc_fence_after();
+        if (warp == 2) TCA_TL(3);     // Q staged (all warps)
     }
 
     if (!active) {
@@ -498,6 +512,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         for (int j = 0; j < n_tiles; ++j) {
             TCA_WAIT(&s_full[j % C::NSP], (j / C::NSP) & 1, pw[0]);
             tc_fence_after();
+            if (warp == 2 && j < 4) TCA_TL(4 + j);    // S(j) ready
             if (!warp_valid) {   // no live row in this warp (chain drafts: 16 of 128 rows): keep the barrier protocol only
                 tc_fence_before();
                 __syncwarp();
@@ -563,6 +578,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 t_left = tpc;
             }
         }
+        if (warp == 2) TCA_TL(8);     // softmax done
         TCA_PROBE(if ((warp == 2 || warp == 6) && TCA_PROBE_ON) printf("softmax warp %d: tiles %d total %lld | wait s_full %lld | ld + max %lld pair barrier %lld exp + split + st + arrive %lld\n",
                                                                       warp, n_tiles, clock64() - t_begin, pw[0], pw[1], pw[2], pw[3]);)
     } else {
@@ -581,9 +597,11 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         float* op = a.o_part + (((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0) * D + hh * C::DH;
         int t_left = tpc;
         const float oscale = FP8 ? mul_rn(exp2f(-TCA_PSCALE_LOG2), ta.v_scale) : exp2f(-TCA_PSCALE_LOG2);   // P's 2^15 out (exact); FP8: V's static scale in
+        float* ost = ostage + (warp - 10) * 32 * (C::OPW + 1);
         TCA_PROBE(long long pw = 0; const long long t_begin = clock64();)
         for (int i = 0; i < n_tiles; ++i) {
             TCA_WAIT(&o_full[i % C::NO], (i / C::NO) & 1, pw);
+            if (warp == 10 && i == n_tiles - 1) TCA_TL(9);   // last P.V result ready
             tc_fence_after();
             if (!warp_valid) {   // no live row in this warp: release the chunk, nothing to add
                 tc_fence_before();
@@ -605,25 +623,45 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
                 }
 #pragma unroll
                 for (int e = 0; e < 16; ++e) o[cb * 16 + e] = fmaf(o[cb * 16 + e], c, __uint_as_float(ov[e]));
-                if (last) {   // the chunk's partial output goes out (P's factor 2^15 taken out exactly), fresh accumulator
-                    if (valid) {
-#pragma unroll
-                        for (int e = 0; e < 16; e += 4)
-                            *reinterpret_cast<float4*>(op + cb * 16 + e) = make_float4(o[cb * 16 + e] * oscale, o[cb * 16 + e + 1] * oscale,
-                                                                                       o[cb * 16 + e + 2] * oscale, o[cb * 16 + e + 3] * oscale);
-                    }
-#pragma unroll
-                    for (int e = 0; e < 16; ++e) o[cb * 16 + e] = 0.f;
-                }
             }
-            if (last) { op += D; t_left = tpc; }
+            if (last) {   // the chunk's partial output goes out (P's factor 2^15 taken out exactly), fresh accumulator
+                const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+                const unsigned long long opa = reinterpret_cast<unsigned long long>(op);
+                constexpr int RPI = 32 / C::OPW;     // rows per store instruction
+#pragma unroll
+                for (int ps = 0; ps < C::DH / C::OPW; ++ps) {
+#pragma unroll
+                    for (int e = 0; e < C::OPW; ++e) ost[lane * (C::OPW + 1) + e] = o[ps * C::OPW + e] * oscale;
+                    __syncwarp();
+#pragma unroll 4
+                    for (int it = 0; it < 32 / RPI; ++it) {
+                        const int rr = it * RPI + lane / C::OPW, cc = lane % C::OPW;
+                        const float v = ost[rr * (C::OPW + 1) + cc];
+                        const unsigned long long pa = __shfl_sync(0xffffffffu, opa, rr);
+                        if ((vmask >> rr) & 1u) reinterpret_cast<float*>(pa)[ps * C::OPW + cc] = v;
+                    }
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int e = 0; e < C::DH; ++e) o[e] = 0.f;
+                op += D; t_left = tpc;
+            }
         }
+        if (warp == 10) TCA_TL(10);   // partials written
         TCA_PROBE(if (warp == 10 && TCA_PROBE_ON) printf("correction warp 10: tiles %d total %lld | wait o_full %lld\n", n_tiles, clock64() - t_begin, pw);)
     }
     tc_fence_before();
     __syncthreads();
     if (warp == 1) tmem_dealloc<512>(tmem_base);
     TCA_PROBE(if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n_tiles >= 48) atomicAdd(&tca_probe_count, 1);)
+    TCA_PROBE(if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n_tiles > 0 && n_tiles <= 8) {
+        // short launches (batch 1): one CTA's timeline in cycles from kernel entry, printed for a few launches after warm-up
+        if (tca_tl_count >= 400 && tca_tl_count < 404)
+            printf("timeline (%d tiles): at wait %lld | past wait %lld | own Q part in TMEM %lld | Q staged %lld | S ready %lld %lld %lld %lld | softmax done %lld | "
+                   "last P.V ready %lld | partials written %lld | end %lld\n", n_tiles, tca_tl[0], tca_tl[1], tca_tl[2], tca_tl[3], tca_tl[4], tca_tl[5], tca_tl[6],
+                   tca_tl[7], tca_tl[8], tca_tl[9], tca_tl[10], clock64() - t_kernel0);
+        atomicAdd(&tca_tl_count, 1);
+    })
     trace_exit(ta.pf);
 }
 
