@@ -69,7 +69,9 @@ struct TcaCfg {
     // 32 different lines per instruction (5,000 cycles per chunk at batch 1: profiles/r2_attention_issue.md section 5); staged
     // OPW columns at a time in a [32 rows][OPW + 1] tile per warp, a store instruction writes whole rows
     static constexpr int OPW = FP8 ? 16 : 32;
-    static constexpr int OST_BYTES = 8 * 32 * (OPW + 1) * 4;
+    // the same region stages the Q tile on its way in (bf16 pool variant): 16 warps x [32 rows][D/8 + 1] words per fp16 part
+    static constexpr int QST_BYTES = FP8 ? 0 : 16 * 32 * (D / 8 + 1) * 4;
+    static constexpr int OST_BYTES = (8 * 32 * (OPW + 1) * 4 > QST_BYTES) ? 8 * 32 * (OPW + 1) * 4 : QST_BYTES;
     static constexpr int SMEM = 1024 + (KS + VS) * K_BYTES + 2 * RS * RAW_BYTES + BAR_BYTES + XCH_BYTES + OST_BYTES;   // Q lives in TMEM
     // TMEM columns
     // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
@@ -275,8 +277,58 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     // ---- Q tile -> TMEM (fp32 x 2^6 -> hi | lo fp16 pairs).  Softmax and correction threads stage it: a warp owns the
     // TMEM lanes of its 32 rows.  Warps 1..17 meet behind named barrier 5; warp 0 goes straight to its K/V
     // loads, which run under the staging (~1.5 us of a 15 us launch at batch 1). ----
-    if (active && warp >= 2 && warp < 18) {
-        // softmax AND correction warps: thread = (row, quarter of d); every load is issued before the first split
+    if (!FP8 && active && warp >= 2 && warp < 18) {
+        // softmax AND correction warps: warp = (32 rows, quarter of d).  The rows are read with the lanes ALONG d (whole 128-byte
+        // row quarters per access: a thread per row, the layout tcgen05.st wants, made every load instruction touch 32 lines and
+        // the 64-KiB tile took 6,000 cycles to arrive at batch 1; profiles/r2_attention_issue.md section 5), split into hi | lo
+        // fp16 pairs where they land, and turned through shared memory into the thread-per-row layout, one part at a time.
+        constexpr int FPR = D / 4;         // floats of a row this warp handles
+        constexpr int L4 = FPR / 4;        // lanes per row (one float4 each)
+        constexpr int RPI = 32 / L4;       // rows per load instruction
+        constexpr int NIT = 32 / RPI;      // load instructions (= D / 16)
+        constexpr int WPR = FPR / 2;       // words (fp16 pairs) per row and part
+        const int qd = (warp - 2) >> 2;   // 0..3
+        const int r = (warp & 3) * 32 + lane;
+        const int row = rg * 128 + r;
+        const int node = row / a.G, gi = row % a.G;
+        const bool valid = row < R && node < nn;
+        const int my_off = valid ? (int)((size_t)(b * a.T + node) * a.q_ld + (size_t)(kvh * a.G + gi) * D) : -1;   // this thread's own row
+        const uint32_t q_addr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + C::TQ + qd * (D / 8);
+        uint32_t* qst = reinterpret_cast<uint32_t*>(ostage) + (warp - 2) * 32 * (WPR + 1);
+        const int rsub = lane / L4, c4 = lane % L4;
+        float4 u[NIT];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int off = __shfl_sync(0xffffffffu, my_off, it * RPI + rsub);
+            u[it] = off >= 0 ? *reinterpret_cast<const float4*>(a.q + off + qd * FPR + c4 * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        uint32_t hw[2 * NIT], lw[2 * NIT];
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            split2_pack(u[it].x * TCA_QSCALE, u[it].y * TCA_QSCALE, hw[2 * it], lw[2 * it]);
+            split2_pack(u[it].z * TCA_QSCALE, u[it].w * TCA_QSCALE, hw[2 * it + 1], lw[2 * it + 1]);
+        }
+#pragma unroll
+        for (int part = 0; part < 2; ++part) {
+#pragma unroll
+            for (int it = 0; it < NIT; ++it) {
+                uint32_t* dst = qst + (it * RPI + rsub) * (WPR + 1) + 2 * c4;
+                dst[0] = part ? lw[2 * it] : hw[2 * it];
+                dst[1] = part ? lw[2 * it + 1] : hw[2 * it + 1];
+            }
+            __syncwarp();
+            uint32_t w[WPR];
+#pragma unroll
+            for (int j = 0; j < WPR; ++j) w[j] = qst[lane * (WPR + 1) + j];
+            if (WPR == 16) tmem_st16(q_addr + part * (D / 2), w);
+            else tmem_st8(q_addr + part * (D / 2), w);
+            __syncwarp();
+        }
+        tmem_st_wait();
+        tc_fence_before();
+    }
+    if (FP8 && active && warp >= 2 && warp < 18) {
+        // FP8 pool variant (no room for the staging tile beside the raw rings): thread = (row, quarter of d)
         const int qd = (warp - 2) >> 2;   // 0..3
         const int r = (warp & 3) * 32 + lane;
         const int row = rg * 128 + r;
