@@ -576,15 +576,15 @@ int copy_f32(cudaStream_t st, const float* src, float* dst, long n) {
     return EV_OK;
 }
 
-template <int D, bool FP8>
+template <int D, bool FP8, bool SMALL = false>
 int launch_attn_tc(cudaStream_t st, const CUtensorMap& tm, const TcAttnArgs& a, dim3 grid) {
     static bool flags[64] = {};
     bool& attr_set = attr_flag(flags);
     if (!attr_set) {
-        CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D, FP8>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D, FP8>::SMEM));
+        CUDA_TRY(cudaFuncSetAttribute(tree_attn_tc_kernel<D, FP8, SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, TcaCfg<D, FP8, SMALL>::SMEM));
         attr_set = true;
     }
-    return launch_k(tree_attn_tc_kernel<D, FP8>, grid, dim3(TcaCfg<D, FP8>::THREADS), TcaCfg<D, FP8>::SMEM, st, tm, a);
+    return launch_k(tree_attn_tc_kernel<D, FP8, SMALL>, grid, dim3(TcaCfg<D, FP8, SMALL>::THREADS), TcaCfg<D, FP8, SMALL>::SMEM, st, tm, a);
 }
 
 template <int D>
@@ -744,6 +744,7 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                 ta.k_scale = c->kv_fp8 ? m->kv_scales[2 * l] : 1.f; ta.v_scale = c->kv_fp8 ? m->kv_scales[2 * l + 1] : 1.f;
                 ta.pf = pfp.take(false);
                 if (c->kv_fp8) EV_TRY((launch_attn_tc<128, true>(st, c->tmKV, ta, agrid)));
+                else if (D == 128 && (long)aa.cpg * aa.chunk <= 8 * TCA_BN) EV_TRY((launch_attn_tc<128, false, true>(st, c->tmKV, ta, agrid)));   // short key ranges: small rings, more L1
                 else if (D == 128) EV_TRY((launch_attn_tc<128, false>(st, c->tmKV, ta, agrid))); else EV_TRY((launch_attn_tc<64, false>(st, c->tmKV, ta, agrid)));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));

@@ -45,10 +45,14 @@ constexpr int TCA_PAGE = 16;      // tokens per page this kernel is built for
 // raw 2-KiB page blocks arrive by linear bulk copies into raw rings, two extra warps (18: K, 19: V) turn each 64-key tile
 // into the fp16, 128-byte-swizzled tile the MMAs read (E4M3 -> fp16 is exact; the static per-tensor scales are applied in
 // fp32: K's in the score multiply, V's when the chunk's partial output is written), everything downstream is unchanged.
-template <int D, bool FP8 = false>
+// SMALL = launches whose CTAs walk at most 8 key tiles (batch 1: 256-key chunks): rings of 3 + 3 tiles instead of 6 + 5.
+// The arithmetic is the same; what changes is how much of the SM's 228 KiB is left as L1: the unified carve-out follows the
+// dynamic shared memory a kernel asks for, and with 223 KiB asked for, the 64-KiB Q tile and the partial outputs went through
+// ~5 KiB of L1 (a handful of lines in flight: 4,000 - 6,000 cycles each at batch 1; profiles/r2_attention_issue.md section 5).
+template <int D, bool FP8 = false, bool SMALL = false>
 struct TcaCfg {
-    static constexpr int KS = FP8 ? 4 : TCA_KS;          // fp16 K tiles in flight
-    static constexpr int VS = FP8 ? 4 : TCA_VS;          // fp16 V tiles in flight
+    static constexpr int KS = FP8 ? 4 : (SMALL ? 3 : TCA_KS);          // fp16 K tiles in flight
+    static constexpr int VS = FP8 ? 4 : (SMALL ? 3 : TCA_VS);          // fp16 V tiles in flight
     static constexpr int RS = FP8 ? 4 : 0;               // raw E4M3 tiles in flight, per K and per V
     static constexpr int RAW_BYTES = TCA_BN * D;         // one raw tile: 64 keys x D bytes
     // bf16 pool: Q.K^T and P.V have separate issuing warps (1 and 18).  FP8 pool: one issuer (warp 1) - a 21st warp would put six
@@ -67,11 +71,13 @@ struct TcaCfg {
     static constexpr int XCH_BYTES = (2 * 2 * 128 + 2 * 128 + 8 * 128) * 4;  // max exchange (double buffered) + sum exchange + rescale factors (8 tiles deep)
     // a chunk's partial output leaves through shared memory: a correction thread holds one ROW (TMEM lane), so its own stores hit
     // 32 different lines per instruction (5,000 cycles per chunk at batch 1: profiles/r2_attention_issue.md section 5); staged
-    // OPW columns at a time in a [32 rows][OPW + 1] tile per warp, a store instruction writes whole rows
+    // OPW columns at a time in a [32 rows][OSTR] tile per warp, a store instruction writes whole rows (128-bit accesses: few instructions,
+    // the chunk's end is a single warp's serial instruction stream)
     static constexpr int OPW = FP8 ? 16 : 32;
     // the same region stages the Q tile on its way in (bf16 pool variant): 16 warps x [32 rows][D/8 + 1] words per fp16 part
     static constexpr int QST_BYTES = FP8 ? 0 : 16 * 32 * (D / 8 + 1) * 4;
-    static constexpr int OST_BYTES = (8 * 32 * (OPW + 1) * 4 > QST_BYTES) ? 8 * 32 * (OPW + 1) * 4 : QST_BYTES;
+    static constexpr int OSTR = OPW + 4;     // floats between rows of the staging tile: 16-byte aligned rows, conflict-free 128-bit accesses
+    static constexpr int OST_BYTES = (8 * 32 * OSTR * 4 > QST_BYTES) ? 8 * 32 * OSTR * 4 : QST_BYTES;
     static constexpr int SMEM = 1024 + (KS + VS) * K_BYTES + 2 * RS * RAW_BYTES + BAR_BYTES + XCH_BYTES + OST_BYTES;   // Q lives in TMEM
     // TMEM columns
     // S[2] and P[2] share two 64-column regions: S(j) = 64 fp32 columns, P(j) = 2 parts x 32 columns (64 fp16
@@ -200,9 +206,9 @@ __device__ int tca_tl_count = 0;
 #define TCA_PROBE(...)
 #define TCA_TL(id)
 #endif
-template <int D, bool FP8>
-__global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
-    using C = TcaCfg<D, FP8>;
+template <int D, bool FP8, bool SMALL = false>
+__global__ void __launch_bounds__((TcaCfg<D, FP8, SMALL>::THREADS), 1) tree_attn_tc_kernel(const __grid_constant__ CUtensorMap tmKV, TcAttnArgs ta) {
+    using C = TcaCfg<D, FP8, SMALL>;
     constexpr int TCA_KS = C::KS, TCA_VS = C::VS;         // ring depths of this variant (shadow the bf16 defaults)
     const AttnArgs& a = ta.a;
     extern __shared__ uint8_t tca_smem_raw[];
@@ -225,7 +231,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
     float* xmax = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(bars) + C::BAR_BYTES);  // [2 buf][2 wg][128]
     float* xsum = xmax + 2 * 2 * 128;                     // [2 wg][128]
     float* xc = xsum + 2 * 128;                           // [8 tiles][128] rescale factor of tile j at [j & 7]
-    float* ostage = xc + 8 * 128;                         // [8 correction warps][32 rows][OPW + 1] staging of a chunk's partial output
+    float* ostage = xc + 8 * 128;                         // [8 correction warps][32 rows][OSTR] staging of a chunk's partial output (and of the Q tile)
 
     TCA_PROBE(const long long t_kernel0 = clock64(); __shared__ long long tca_tl[24];)
     const int split = blockIdx.x;
@@ -649,7 +655,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
         float* op = a.o_part + (((size_t)(b * a.T + (valid ? node : 0)) * a.Hq + kvh * a.G + (valid ? gi : 0)) * a.n_chunks + chunk0) * D + hh * C::DH;
         int t_left = tpc;
         const float oscale = FP8 ? mul_rn(exp2f(-TCA_PSCALE_LOG2), ta.v_scale) : exp2f(-TCA_PSCALE_LOG2);   // P's 2^15 out (exact); FP8: V's static scale in
-        float* ost = ostage + (warp - 10) * 32 * (C::OPW + 1);
+        float* ost = ostage + (warp - 10) * 32 * C::OSTR;
         TCA_PROBE(long long pw = 0; const long long t_begin = clock64();)
         for (int i = 0; i < n_tiles; ++i) {
             TCA_WAIT(&o_full[i % C::NO], (i / C::NO) & 1, pw);
@@ -679,18 +685,21 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8>::THREADS), 1) tree_attn_tc_ker
             if (last) {   // the chunk's partial output goes out (P's factor 2^15 taken out exactly), fresh accumulator
                 const unsigned vmask = __ballot_sync(0xffffffffu, valid);
                 const unsigned long long opa = reinterpret_cast<unsigned long long>(op);
-                constexpr int RPI = 32 / C::OPW;     // rows per store instruction
+                constexpr int L4 = C::OPW / 4;       // lanes per row (one float4 each)
+                constexpr int RPI = 32 / L4;         // rows per store instruction
 #pragma unroll
                 for (int ps = 0; ps < C::DH / C::OPW; ++ps) {
 #pragma unroll
-                    for (int e = 0; e < C::OPW; ++e) ost[lane * (C::OPW + 1) + e] = o[ps * C::OPW + e] * oscale;
+                    for (int e = 0; e < C::OPW; e += 4)
+                        *reinterpret_cast<float4*>(ost + lane * C::OSTR + e) = make_float4(o[ps * C::OPW + e] * oscale, o[ps * C::OPW + e + 1] * oscale,
+                                                                                          o[ps * C::OPW + e + 2] * oscale, o[ps * C::OPW + e + 3] * oscale);
                     __syncwarp();
-#pragma unroll 4
+#pragma unroll
                     for (int it = 0; it < 32 / RPI; ++it) {
-                        const int rr = it * RPI + lane / C::OPW, cc = lane % C::OPW;
-                        const float v = ost[rr * (C::OPW + 1) + cc];
+                        const int rr = it * RPI + lane / L4, c4 = lane % L4;
+                        const float4 v = *reinterpret_cast<const float4*>(ost + rr * C::OSTR + c4 * 4);
                         const unsigned long long pa = __shfl_sync(0xffffffffu, opa, rr);
-                        if ((vmask >> rr) & 1u) reinterpret_cast<float*>(pa)[ps * C::OPW + cc] = v;
+                        if ((vmask >> rr) & 1u) *reinterpret_cast<float4*>(reinterpret_cast<float*>(pa) + ps * C::OPW + c4 * 4) = v;
                     }
                     __syncwarp();
                 }
