@@ -242,6 +242,24 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8, SMALL>::THREADS), 1) tree_attn
     // ---- prologue that does not depend on the previous kernel (overlaps it under PDL): barriers, TMEM ----
     pdl_launch_dependents();
     l2_prefetch_issue(ta.pf);
+    // What tree_prep_kernel wrote at the head of the step is read BEFORE griddepcontrol.wait, and first of all: the kernel launched
+    // right after tree_prep_kernel carries no programmatic-serialization attribute (ev_api.cu), so no later kernel of the step can
+    // be resident before tree_prep_kernel has completed; __ldcg: an L1 line left over from the previous step must not serve.
+    // The wait itself guards what the PRECEDING kernel (RoPE + K/V write) produced: Q, and the K/V of the tree's own slots.
+    const int b = a.order ? __ldcg(a.order + blockIdx.z) : (int)blockIdx.z;
+    const int nn = __ldcg(a.nn_eff + b);
+    const int L = __ldcg(a.Lsnap + b);
+    const int seq_slot = __ldcg(a.seq_slots + b);
+    const int n_keys = __ldcg(a.kend_seq + b);         // one past the last bulk key slot of the sequence (tree_prep_kernel)
+    // The grid covers the chunk columns of the longest context the model may see (a power of two of them for short chunks, so that
+    // a growing context does not re-capture the graph): a CTA whose chunks lie beyond this sequence's keys leaves at once, before it
+    // takes barriers or tensor memory - with max_ctx well above the live context there are more such CTAs than SMs, and each used
+    // to hold an SM for its whole set-up (config[1] in a model sized for 2,900 tokens: 256 CTAs, 144 live, attention 426 us per
+    // step against 329 with a tight max_ctx).
+    if (nn == 0 || (long)blockIdx.x * a.cpg * a.chunk >= n_keys) {
+        trace_exit(ta.pf);
+        return;
+    }
     if (threadIdx.x == 0) {
         for (int s = 0; s < TCA_KS; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
         for (int s = 0; s < TCA_VS; ++s) { mbar_init(&v_full[s], 1); mbar_init(&v_empty[s], 1); }
@@ -256,15 +274,6 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8, SMALL>::THREADS), 1) tree_attn
     __syncthreads();       // barriers and the TMEM base are visible to every warp (still before the wait)
     tc_fence_after();
     const uint32_t tmem_base = *tmem_base_smem;
-    // What tree_prep_kernel wrote at the head of the step is read BEFORE griddepcontrol.wait: the kernel launched right after
-    // tree_prep_kernel carries no programmatic-serialization attribute (ev_api.cu), so no later kernel of the step can be
-    // resident before tree_prep_kernel has completed; __ldcg: an L1 line left over from the previous step must not serve.
-    // The wait itself guards what the PRECEDING kernel (RoPE + K/V write) produced: Q, and the K/V of the tree's own slots.
-    const int b = a.order ? __ldcg(a.order + blockIdx.z) : (int)blockIdx.z;
-    const int nn = __ldcg(a.nn_eff + b);
-    const int L = __ldcg(a.Lsnap + b);
-    const int seq_slot = __ldcg(a.seq_slots + b);
-    const int n_keys = __ldcg(a.kend_seq + b);         // one past the last bulk key slot of the sequence (tree_prep_kernel)
     if (warp == 2) TCA_TL(0);     // prologue done (barriers, TMEM, plan): at the wait
     if (warp != 0) {
         pdl_wait();
