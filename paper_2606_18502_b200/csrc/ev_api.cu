@@ -743,9 +743,10 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
                 ta.pool8 = reinterpret_cast<const uint8_t*>(c->pool);
                 ta.k_scale = c->kv_fp8 ? m->kv_scales[2 * l] : 1.f; ta.v_scale = c->kv_fp8 ? m->kv_scales[2 * l + 1] : 1.f;
                 ta.pf = pfp.take(false);
-                if (c->kv_fp8) EV_TRY((launch_attn_tc<128, true>(st, c->tmKV, ta, agrid)));
-                else if (D == 128 && (long)aa.cpg * aa.chunk <= 8 * TCA_BN) EV_TRY((launch_attn_tc<128, false, true>(st, c->tmKV, ta, agrid)));   // short key ranges: small rings, more L1
-                else if (D == 128) EV_TRY((launch_attn_tc<128, false>(st, c->tmKV, ta, agrid))); else EV_TRY((launch_attn_tc<64, false>(st, c->tmKV, ta, agrid)));
+                const dim3 tgrid(agrid.y, agrid.x, agrid.z);   // the tcgen05 kernel takes (kv head x row group, chunk column, sequence)
+                if (c->kv_fp8) EV_TRY((launch_attn_tc<128, true>(st, c->tmKV, ta, tgrid)));
+                else if (D == 128 && (long)aa.cpg * aa.chunk <= 8 * TCA_BN) EV_TRY((launch_attn_tc<128, false, true>(st, c->tmKV, ta, tgrid)));   // short key ranges: small rings, more L1
+                else if (D == 128) EV_TRY((launch_attn_tc<128, false>(st, c->tmKV, ta, tgrid))); else EV_TRY((launch_attn_tc<64, false>(st, c->tmKV, ta, tgrid)));
             } else {
                 if (D == 128) EV_TRY(launch_attn<128>(st, aa, agrid)); else EV_TRY(launch_attn<64>(st, aa, agrid));
             }

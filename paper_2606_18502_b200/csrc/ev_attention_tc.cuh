@@ -234,8 +234,10 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8, SMALL>::THREADS), 1) tree_attn
     float* ostage = xc + 8 * 128;                         // [8 correction warps][32 rows][OSTR] staging of a chunk's partial output (and of the Q tile)
 
     TCA_PROBE(const long long t_kernel0 = clock64(); __shared__ long long tca_tl[24];)
-    const int split = blockIdx.x;
-    const int kvh = blockIdx.y % a.Hkv, rg = blockIdx.y / a.Hkv;
+    // grid (kv head x row group, chunk column, sequence): CTAs start in x-fastest order, so the columns beyond the live context
+    // (they leave at once, below) come after every live CTA of the sequence instead of between them
+    const int split = blockIdx.y;
+    const int kvh = blockIdx.x % a.Hkv, rg = blockIdx.x / a.Hkv;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int R = a.T * a.G;
 
@@ -256,7 +258,7 @@ __global__ void __launch_bounds__((TcaCfg<D, FP8, SMALL>::THREADS), 1) tree_attn
     // takes barriers or tensor memory - with max_ctx well above the live context there are more such CTAs than SMs, and each used
     // to hold an SM for its whole set-up (config[1] in a model sized for 2,900 tokens: 256 CTAs, 144 live, attention 426 us per
     // step against 329 with a tight max_ctx).
-    if (nn == 0 || (long)blockIdx.x * a.cpg * a.chunk >= n_keys) {
+    if (nn == 0 || (long)split * a.cpg * a.chunk >= n_keys) {
         trace_exit(ta.pf);
         return;
     }
