@@ -297,7 +297,9 @@ constexpr int NORM_SEG_MAX = 32;   // 128-element segments of a row: hidden <= 4
 template <int NORM_NV4, int MAXS>
 // <4, 1> is the many-row form (one CTA per row, M > 256): six CTAs per SM (40 registers) put the 832 rows of config[2] in ONE wave (888 slots)
 // instead of 1.4 waves of four (norm class 858 -> 786 us per step)
-__global__ void __launch_bounds__(NORM_THREADS, (NORM_NV4 == 4 && MAXS == 1) ? 6 : 1) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
+// (every other form: four CTAs per SM = 64 registers, what the compiler chose without a bound; with an explicit 1 it took 72 - 101 and
+// the GEMM that follows could no longer be resident beside it: profiles/r2_step_timeline.md)
+__global__ void __launch_bounds__(NORM_THREADS, (NORM_NV4 == 4 && MAXS == 1) ? 6 : 4) rmsnorm_quant_kernel(float* __restrict__ h, int H, LinOut pend,
                                                                      const __nv_bfloat16* __restrict__ gain, float eps,
                                                                      QuantOut q, L2Prefetch pf) {
     pdl_launch_dependents();  // the next kernel (a GEMM) may start prefetching its weights now
