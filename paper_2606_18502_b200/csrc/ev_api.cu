@@ -509,8 +509,19 @@ int run_linear(ev_model* m, cudaStream_t st, const QMat& w, const ActBuf& x, int
     GemmArgs a;
     a.M = M; a.N = (int)w.N; a.total_kb = w.total_kb; a.n_tiles = w.n_tiles;   // n_tiles is even (alloc_qmat)
     a.m_tiles = (M + 255) / 256;
-    a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
     const bool pair = a.m_tiles >= 2;   // cta_group::2 kernel
+    if (pair && epi == EPI_RAW) {
+        // Token tiling of the many-row form is a scheduling choice (rows are independent, the K cuts do not move): an item is
+        // (pair of channel tiles, token tile) and the CTA pairs take whole items.  When the default (fewest, widest tiles) does not
+        // even fill ONE round of pairs, narrower tiles put more pairs to work at no cost in rounds: config[4] (480 rows) QKV 48 -> 72
+        // items on 74 pairs (735 -> 665 us per step), down 32 -> 64 items (1,378 -> 1,094).  Beyond one round it does not pay - the
+        // count rounds x tile width predicts -31 % for QKV at 832 rows (96 items of 208 -> 144 items of 144) and -17 % for gate|up at
+        // 480; measured +5 % and +73 %: narrower tiles re-read W and pay the per-item hand-overs more often.
+        const int pairs_avail = std::max(1, m->num_sms / 2), n_pairs_ = a.n_tiles / 2;
+        if (n_pairs_ * a.m_tiles < pairs_avail)
+            for (int mt = a.m_tiles + 1; mt <= 8 && n_pairs_ * mt <= pairs_avail; ++mt) a.m_tiles = mt;
+    }
+    a.tok = (int)round_up((M + a.m_tiles - 1) / a.m_tiles, 16);
     // balanced partition (ev_gemm.cuh, GemmArgs::bal): several token tiles -> items of up to 256 tokens cut from an even deal.
     // Used for the LM head (1002 n tiles: 27 items per CTA pair, 588 -> 548 us at M = 832).  The layer GEMMs have 1-6
     // items per pair; there the extra partial items (a 32-token item costs as much W traffic as a 208-token one)
