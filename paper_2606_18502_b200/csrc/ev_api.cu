@@ -687,7 +687,9 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
 
     const int n_splits = plan.n_splits, split_len = plan.split_len;
     const RowPlan rp_h = row_plan(m, M, H), rp_f = row_plan(m, M, F, CLUSTER_MAX), rp_q = row_plan(m, M, m->q_dim);
-    const bool swi_smem = M > 2 * m->num_sms && (size_t)F * 4 <= 160 * 1024;   // many rows: one CTA per row, row staged in smem
+    // many rows: one CTA per row, row staged in smem.  Measured cross-over with the register / cluster form: 480 rows 950 (smem) vs 778 us
+    // per step (clusters of 4), 832 rows 1,222 vs 1,379
+    const bool swi_smem = M > 4 * m->num_sms && (size_t)F * 4 <= 160 * 1024;
     const int rope_gy = (long)M * 4 <= 4L * m->num_sms ? 4 : 2;
     const int row_groups = (T * (cfg.n_q_heads / cfg.n_kv_heads) + 16 * ATT_WARPS - 1) / (16 * ATT_WARPS);
 
