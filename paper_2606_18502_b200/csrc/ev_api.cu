@@ -777,7 +777,8 @@ int run_forward(ev_model* m, ev_cache* c, const ev_verify_in* in, ev_verify_out*
         {
             ProfScope ps(m, st, PC_ATTN_MERGE);
             const int Gq = cfg.n_q_heads / cfg.n_kv_heads;
-            if (rp_q.cl == 1 && D == 128 && cfg.n_kv_heads <= 8 && (Gq == 4 || Gq == 1)) {   // many rows: one warp per kv head
+            // many rows: one warp per kv head (from 256 rows on: config[3], 256 rows, 789 us per step in clusters of 2 vs 720 this way)
+            if ((rp_q.cl == 1 || M >= 256) && D == 128 && cfg.n_kv_heads <= 8 && (Gq == 4 || Gq == 1)) {
                 if (Gq == 4) EV_TRY(launch_k(attn_merge_rowkv_kernel<4>, dim3(M), dim3(32 * cfg.n_kv_heads), 0, st, ma));
                 else EV_TRY(launch_k(attn_merge_rowkv_kernel<1>, dim3(M), dim3(32 * cfg.n_kv_heads), 0, st, ma));
             } else {
